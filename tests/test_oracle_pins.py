@@ -1,0 +1,340 @@
+"""Pins of the fp64 oracle (oracle/cp4d_ref.c) against what the paper and the mathematics fix.
+
+None of these calls the CUDA path.  Pin numbering P1..P8 follows SURVEY.md section 8(c) / DESIGN.md.
+"""
+import numpy as np
+import pytest
+
+from oracle import dense
+from paper_1809_09725_b200 import synth
+
+
+def tiny(oracle, n=8, nz=2, nd=8, n_angles=16, n_half_rot=2, m=2, lambda1=0.05, lambda2=1.5, seed=0):
+    phi = np.random.default_rng(seed).standard_normal((m, n_angles))
+    return oracle.Problem(n, nz, nd, n_angles, n_half_rot, m, phi, lambda1, lambda2)
+
+
+# ---------------------------------------------------------------- P1: static Joseph matrix (O1)
+@pytest.mark.parametrize("n,nd", [(8, 8), (9, 12), (16, 11), (32, 32)])
+def test_p1_ray_stepping_equals_closed_form(oracle, n, nd):
+    """Ray-stepping forward (C) == dense hat-function matrix typed in numpy, incl. 0, 45, 90, 135 deg."""
+    n_angles = 8
+    P = oracle.Problem(n, 1, nd, n_angles, 1, 1, np.ones((1, n_angles)))
+    f = np.random.default_rng(1).standard_normal(P.primal_shape)
+    g = P.forward(f)
+    for k in range(n_angles):
+        A = dense.joseph_matrix(n, nd, k * np.pi / n_angles)
+        np.testing.assert_allclose(g[0, k], A @ f.ravel(), atol=1e-12)
+        np.testing.assert_allclose(P.dense_A(k), A, atol=1e-13)
+        assert (A > 0).sum(axis=0).max() <= 2          # each (voxel, angle) touches at most 2 bins
+
+
+def test_p1_axis_angles_are_column_and_row_sums(oracle):
+    n = 16
+    P = oracle.Problem(n, 1, n, 2, 1, 1, np.ones((1, 2)))     # theta = 0, pi/2
+    f = np.random.default_rng(2).standard_normal((n, n))
+    g = P.forward(f.reshape(P.primal_shape))
+    np.testing.assert_allclose(g[0, 0], f.sum(axis=0), atol=1e-12)   # theta=0: integrate over y
+    np.testing.assert_allclose(g[0, 1], f.sum(axis=1), atol=1e-12)   # theta=pi/2: integrate over x
+
+
+# ---------------------------------------------------------------- P2: K1 / K1^T vs brute force
+def test_p2_dense_bruteforce_forward_and_adjoint(oracle):
+    P = tiny(oracle)
+    K = dense.dense_K1(P.n, P.nz, P.nd, P.n_angles, P.n_half_rot, P.m, P.phi)
+    rng = np.random.default_rng(3)
+    f, g = rng.standard_normal(P.primal_shape), rng.standard_normal(P.sino_shape)
+    np.testing.assert_allclose(P.forward(f).ravel(), K @ f.ravel(), atol=1e-12)
+    np.testing.assert_allclose(P.adjoint(g).ravel(), K.T @ g.ravel(), atol=1e-12)
+    np.testing.assert_allclose(P.forward(f, folded=True).ravel(), K @ f.ravel(), atol=1e-12)
+    np.testing.assert_allclose(P.adjoint(g, folded=True).ravel(), K.T @ g.ravel(), atol=1e-12)
+
+
+@pytest.mark.parametrize("cfg,kw", [(1, {}), (2, dict(n=48, nd=48, nz=3, n_angles=96)), (4, dict(n=24, nd=30, nz=2, n_angles=40))])
+def test_p2_adjoint_dot_product(oracle, cfg, kw):
+    c = synth.CONFIGS[cfg].scaled(**kw)
+    P = oracle.Problem.from_config(c)
+    f, g = synth.test_vectors(c)
+    Kf, Ktg = P.forward(f), P.adjoint(g)
+    lhs, rhs = np.vdot(Kf, g), np.vdot(f, Ktg)
+    assert abs(lhs - rhs) <= 1e-12 * np.linalg.norm(Kf) * np.linalg.norm(g)
+    Kf2, Ktg2 = P.forward(f, folded=True), P.adjoint(g, folded=True)
+    assert np.linalg.norm(Kf2 - Kf) <= 1e-13 * np.linalg.norm(Kf)
+    assert np.linalg.norm(Ktg2 - Ktg) <= 1e-13 * np.linalg.norm(Ktg)
+
+
+def test_sampled_entry_points_equal_full(oracle):
+    c = synth.CONFIGS[1].scaled(nz=2)
+    P = oracle.Problem.from_config(c)
+    f, g = synth.test_vectors(c)
+    rng = np.random.default_rng(5)
+    zkb = np.stack([rng.integers(0, c.nz, 64), rng.integers(0, c.n_angles, 64), rng.integers(0, c.nd, 64)], 1)
+    zyx = np.stack([rng.integers(0, c.nz, 64), rng.integers(0, c.n, 64), rng.integers(0, c.n, 64)], 1)
+    Kf, Ktg = P.forward(f), P.adjoint(g)
+    np.testing.assert_array_equal(P.forward_rays(f, zkb), Kf[zkb[:, 0], zkb[:, 1], zkb[:, 2]])
+    np.testing.assert_array_equal(P.adjoint_voxels(g, zyx), Ktg[zyx[:, 0], zyx[:, 1], zyx[:, 2]])
+
+
+def test_thread_count_does_not_change_bits(oracle):
+    c = synth.CONFIGS[1].scaled(nz=3)
+    P = oracle.Problem.from_config(c)
+    f, g = synth.test_vectors(c)
+    a1, b1, c1 = P.forward(f), P.adjoint(g), P.adjoint(g, folded=True)
+    oracle.set_threads(4)
+    try:
+        np.testing.assert_array_equal(P.forward(f), a1)
+        np.testing.assert_array_equal(P.adjoint(g), b1)
+        np.testing.assert_array_equal(P.adjoint(g, folded=True), c1)
+    finally:
+        oracle.set_threads(1)
+
+
+# ---------------------------------------------------------------- P3: closed-form Radon transforms
+def _radon_errors(oracle, n, kind):
+    n_angles = 12
+    P = oracle.Problem(n, 1, n, n_angles, 1, 1, np.ones((1, n_angles)))
+    x = np.arange(n) - (n - 1) / 2.0
+    X, Y = np.meshgrid(x, x, indexing="xy")
+    s = np.arange(n) - (n - 1) / 2.0
+    if kind == "gauss":
+        sig = n / 10.0
+        img = np.exp(-(X ** 2 + Y ** 2) / (2 * sig ** 2))
+        exact = sig * np.sqrt(2 * np.pi) * np.exp(-s ** 2 / (2 * sig ** 2))
+    else:
+        r = 0.3 * n
+        img = (X ** 2 + Y ** 2 <= r ** 2).astype(float)
+        exact = 2 * np.sqrt(np.maximum(0.0, r ** 2 - s ** 2))
+    g = P.forward(img.reshape(P.primal_shape))[0]
+    return np.linalg.norm(g - exact[None]) / np.linalg.norm(np.repeat(exact[None], n_angles, 0))
+
+
+def test_p3_gaussian_radon_second_order(oracle):
+    e = [_radon_errors(oracle, n, "gauss") for n in (32, 64, 128)]
+    assert e[1] < 2e-3
+    for a, b in zip(e, e[1:]):
+        assert 3.7 < a / b < 4.3          # exact 2nd-order convergence of the Joseph sum
+
+
+def test_p3_disk_radon(oracle):
+    e = [_radon_errors(oracle, n, "disk") for n in (32, 64, 128)]
+    assert e[1] < 2.5e-2 and e[0] > e[1] > e[2]
+
+
+# ---------------------------------------------------------------- P4: pi-periodicity fold (A8)
+def test_p4_pi_symmetry_of_static_matrix(oracle):
+    P = oracle.Problem(12, 1, 15, 40, 4, 1, np.ones((1, 40)))
+    n0 = 10
+    for k in range(n0):
+        for q in range(1, 4):
+            A0, Aq = P.dense_A(k), P.dense_A(k + q * n0)
+            np.testing.assert_allclose(Aq, A0[::-1] if q % 2 else A0, atol=1e-13)
+
+
+# ---------------------------------------------------------------- P5: proxes
+def test_p5_prox_f1_optimality(oracle):
+    """h' minimises <h',g> + |h'|^2/2 + |h-h'|^2/(2 sigma)  <=>  g + h' + (h'-h)/sigma = 0."""
+    P = tiny(oracle)
+    rng = np.random.default_rng(7)
+    h, kf, g = (rng.standard_normal(P.sino_shape) for _ in range(3))
+    sigma = 0.37
+    hp = P.prox_f1(h, kf, g, sigma)
+    arg = h + sigma * kf          # the prox argument of step 3
+    np.testing.assert_allclose(g + hp + (hp - arg) / sigma, 0, atol=1e-13)
+
+
+def test_p5_prox_f2_moreau_and_projection(oracle):
+    """prox_{sigma F*}(q) = q - sigma * prox_{F/sigma}(q/sigma), F = lambda1*|.|_2 pointwise (vector soft threshold)."""
+    P = tiny(oracle, lambda1=0.8)
+    rng = np.random.default_rng(8)
+    h2 = rng.standard_normal((4,) + P.primal_shape)
+    gr = rng.standard_normal((4,) + P.primal_shape)
+    sigma = 0.6
+    out, ncl = P.prox_f2(h2, gr, sigma)
+    q = h2 + sigma * gr
+    nq = np.sqrt((q ** 2).sum(0))
+    shrink = np.maximum(0.0, 1.0 - (P.lambda1 / sigma) / np.maximum(nq / sigma, 1e-300)) * (q / sigma)
+    np.testing.assert_allclose(out, q - sigma * shrink, atol=1e-13)
+    no = np.sqrt((out ** 2).sum(0))
+    assert no.max() <= P.lambda1 * (1 + 1e-14)
+    inside = nq <= P.lambda1
+    assert 0 < inside.sum() < inside.size and ncl == (~inside).sum()
+    np.testing.assert_array_equal(out[:, inside], q[:, inside])
+    # direction preserved
+    np.testing.assert_allclose(out * nq, q * no, atol=1e-13)
+
+
+# ---------------------------------------------------------------- P6: grad / div / norms
+def test_p6_grad_is_dense_forward_difference_and_div_is_minus_transpose(oracle):
+    P = tiny(oracle, n=5, nz=3, m=4, lambda2=2.0)
+    K2 = dense.dense_K2(P.n, P.nz, P.m, P.lambda2)
+    rng = np.random.default_rng(9)
+    f, p = rng.standard_normal(P.primal_shape), rng.standard_normal((4,) + P.primal_shape)
+    np.testing.assert_allclose(P.grad(f).ravel(), K2 @ f.ravel(), atol=1e-13)
+    np.testing.assert_allclose(P.div(p).ravel(), -(K2.T @ p.ravel()), atol=1e-13)
+    np.testing.assert_array_equal(P.grad(np.full(P.primal_shape, 3.25)), 0.0)
+    assert abs(np.vdot(P.grad(f), p) + np.vdot(f, P.div(p))) < 1e-12
+
+
+def test_p6_axis_of_length_one_contributes_nothing(oracle):
+    c = synth.CONFIGS[1]
+    P = oracle.Problem.from_config(c)
+    f = synth.test_vectors(c)[0]
+    assert np.all(P.grad(f)[2] == 0)
+
+
+@pytest.mark.parametrize("n,nz,m,lam2", [(5, 3, 6, 2.0), (8, 1, 4, 1.0)])
+def test_p6_norm_K2_closed_form(oracle, n, nz, m, lam2):
+    """||K2||^2 = sum_a w_a^2 (2 - 2 cos(pi (n_a-1)/n_a)): largest eigenvalue of path-graph Laplacians."""
+    P = tiny(oracle, n=n, nz=nz, m=m, lambda2=lam2)
+    lap = lambda k: 0.0 if k == 1 else 2 - 2 * np.cos(np.pi * (k - 1) / k)
+    closed = 2 * lap(n) + lap(nz) + lam2 ** 2 * lap(m)
+    sv = np.linalg.svd(dense.dense_K2(n, nz, m, lam2), compute_uv=False)[0]
+    assert abs(sv ** 2 - closed) < 1e-10
+    x0 = np.random.default_rng(10).standard_normal(P.primal_shape)
+    Ls = [P.power(x0, k, use_k1=False)[0] for k in (5, 50, 3000)]
+    assert Ls[0] <= Ls[1] <= Ls[2] <= np.sqrt(closed) * (1 + 1e-12)     # converges from below
+    assert abs(Ls[2] ** 2 - closed) < 1e-3 * closed
+    assert closed < 4 * (3 + lam2 ** 2)
+
+
+def test_p6_power_iteration_vs_dense_svd(oracle):
+    P = tiny(oracle)
+    K = np.vstack([dense.dense_K1(P.n, P.nz, P.nd, P.n_angles, P.n_half_rot, P.m, P.phi),
+                   dense.dense_K2(P.n, P.nz, P.m, P.lambda2)])
+    smax = np.linalg.svd(K, compute_uv=False)[0]
+    x0 = np.random.default_rng(11).standard_normal(P.primal_shape)
+    L60, L, = P.power(x0, 60)[0], P.power(x0, 4000)[0]      # random table: top singular values are close
+    assert L60 <= L <= smax * (1 + 1e-12) and abs(L - smax) <= 1e-6 * smax
+
+
+def test_p6_config1_norm_value(oracle):
+    """||K|| of config 1 (geometry + 4-term Fourier table, lambda2 = 1) against the dense SVD."""
+    c = synth.CONFIGS[1]
+    P = oracle.Problem.from_config(c)
+    K = np.vstack([dense.dense_K1(c.n, c.nz, c.nd, c.n_angles, c.n_half_rot, c.m, P.phi), dense.dense_K2(c.n, c.nz, c.m, 1.0)])
+    smax = np.linalg.svd(K, compute_uv=False)[0]
+    L, _ = P.power(synth.rng(1, 3).standard_normal(P.primal_shape), 30)
+    assert abs(L - smax) < 1e-6 * smax
+    golden = float(open(__file__.replace("test_oracle_pins.py", "golden/config1_norm.txt")).read().split()[0])
+    assert abs(L - golden) < 1e-9 * golden
+
+
+# ---------------------------------------------------------------- P7: the CP loop
+def _cp_setup(oracle, lambda1, seed=12, **kw):
+    P = tiny(oracle, lambda1=lambda1, **kw)
+    K1 = dense.dense_K1(P.n, P.nz, P.nd, P.n_angles, P.n_half_rot, P.m, P.phi)
+    K2 = dense.dense_K2(P.n, P.nz, P.m, P.lambda2)
+    g = np.random.default_rng(seed).standard_normal(P.sino_shape)
+    L = np.linalg.svd(np.vstack([K1, K2]), compute_uv=False)[0]
+    return P, K1, K2, g, 0.95 / L
+
+
+def test_p7_cp_step_matches_dense_algebra(oracle):
+    """Three iterations of Fig. 2 written with dense matrices (steps 3-6 verbatim) == the C loop."""
+    P, K1, K2, g, ts = _cp_setup(oracle, 0.3)
+    st = P.zero_state()
+    f = np.zeros(P.V); ft = f.copy(); h1 = np.zeros(P.S); h2 = np.zeros(4 * P.V)
+    for it in range(3):
+        P.cp(g, st, ts, ts, 1)
+        h1 = (h1 + ts * (K1 @ ft) - ts * g.ravel()) / (1 + ts)                       # step 3
+        q = (h2 + ts * (K2 @ ft)).reshape(4, -1)                                     # step 4
+        h2 = (q / np.maximum(1.0, np.sqrt((q ** 2).sum(0)) / P.lambda1)).ravel()
+        fn = f - ts * (K1.T @ h1) - ts * (K2.T @ h2)                                 # step 5 (div = -K2^T)
+        ft = fn + 1.0 * (fn - f)                                                     # step 6
+        f = fn
+        np.testing.assert_allclose(st["f"].ravel(), f, atol=1e-12)
+        np.testing.assert_allclose(st["ft"].ravel(), ft, atol=1e-12)
+        np.testing.assert_allclose(st["h1"].ravel(), h1, atol=1e-12)
+        np.testing.assert_allclose(st["h2"].ravel(), h2, atol=1e-12)
+
+
+def test_p7_lambda1_zero_is_least_squares(oracle):
+    P, K1, K2, g, ts = _cp_setup(oracle, 0.0)
+    st = P.zero_state()
+    P.cp(g, st, ts, ts, 1000)
+    f = st["f"].ravel()
+    assert np.all(st["h2"] == 0)
+    U, s, Vt = np.linalg.svd(K1)
+    null = Vt[(s > 1e-10 * s[0]).sum():]
+    assert np.linalg.norm(null @ f) <= 1e-12 * max(1.0, np.linalg.norm(f))           # f in range(K1^T)
+    res = np.linalg.norm(K1.T @ (K1 @ f - g.ravel())) / np.linalg.norm(K1.T @ g.ravel())
+    assert res < 1e-2
+    P.cp(g, st, ts, ts, 4000)
+    f = st["f"].ravel()
+    res2 = np.linalg.norm(K1.T @ (K1 @ f - g.ravel())) / np.linalg.norm(K1.T @ g.ravel())
+    assert res2 < 0.5 * res
+
+
+def test_p7_kkt_fejer_and_stationarity(oracle):
+    P, K1, K2, g, ts = _cp_setup(oracle, 0.3)
+    K = np.vstack([K1, K2])
+    # long run -> (f*, h*)
+    star = P.zero_state()
+    P.cp(g, star, ts, ts, 60000)
+    fs, hs = star["f"].ravel(), np.concatenate([star["h1"].ravel(), star["h2"].ravel()])
+    kkt0 = np.linalg.norm(K1.T @ g.ravel())
+    # (ii) KKT at the limit
+    assert np.linalg.norm(K.T @ hs) < 1e-6 * kkt0
+    np.testing.assert_allclose(star["h1"].ravel(), K1 @ fs - g.ravel(), atol=1e-6 * np.linalg.norm(g))
+    h2 = star["h2"].reshape(4, -1)
+    gf = (K2 @ fs).reshape(4, -1)
+    assert np.sqrt((h2 ** 2).sum(0)).max() <= P.lambda1 * (1 + 1e-12)
+    ng = np.sqrt((gf ** 2).sum(0))
+    act = ng > 1e-6 * ng.max()
+    assert act.any()
+    np.testing.assert_allclose((h2 * gf).sum(0)[act], P.lambda1 * ng[act], rtol=1e-4)
+    # (iv) a stationary point stays stationary
+    nxt = {k: v.copy() for k, v in star.items()}
+    P.cp(g, nxt, ts, ts, 1)
+    assert np.linalg.norm(nxt["f"] - star["f"]) < 1e-9 * np.linalg.norm(star["f"])
+    # (iii) Fejer monotonicity in the CP metric |f-f*|^2/tau - 2<K(f-f*),h-h*> + |h-h*|^2/sigma, and KKT residual decay
+    st = P.zero_state()
+    prev, kkt = np.inf, []
+    for n in range(200):
+        P.cp(g, st, ts, ts, 1)
+        df = st["f"].ravel() - fs
+        dh = np.concatenate([st["h1"].ravel(), st["h2"].ravel()]) - hs
+        d = df @ df / ts - 2 * (K @ df) @ dh + dh @ dh / ts
+        assert d <= prev * (1 + 1e-9) + 1e-12
+        prev = d
+        kkt.append(np.linalg.norm(K.T @ np.concatenate([st["h1"].ravel(), st["h2"].ravel()])))
+    assert kkt[-1] < 0.1 * kkt[0]
+
+
+# ---------------------------------------------------------------- P8: basis tables (inputs)
+@pytest.mark.parametrize("m,na", [(4, 128), (8, 720), (16, 1440)])
+def test_p8_fourier_table_orthogonality(m, na):
+    phi = synth.basis_table("fourier", m, na)
+    np.testing.assert_allclose(phi @ phi.T / na, np.diag([1.0] + [0.5] * (m - 1)), atol=1e-13)
+    t = np.arange(na) / na
+    if m == 4:   # the four functions config 1 lists
+        np.testing.assert_allclose(phi, [np.ones(na), np.cos(2 * np.pi * t), np.sin(2 * np.pi * t), np.cos(4 * np.pi * t)], atol=1e-15)
+
+
+def test_p8_bspline_partition_of_unity():
+    phi = synth.basis_table("bspline", 16, 3000)
+    np.testing.assert_allclose(phi.sum(0), 1.0, atol=1e-13)
+    assert phi.min() >= 0 and (phi > 0).sum(0).max() <= 4
+
+
+def test_synthetic_data_is_exact_radon_of_disks(oracle):
+    """Noise-free config-1 data (analytic disk integrals) vs the oracle projecting a rasterised static phantom:
+    pins the geometry conventions (bin centre, angle direction) shared by generator and oracle."""
+    c = synth.CONFIGS[1].scaled(n=128, nd=128, n_angles=32, n_half_rot=1)
+    p = synth.phantom_params(c)
+    p0 = dict(p); p0["vel"] = p["vel"] * 0
+    import paper_1809_09725_b200.synth as S
+    orig = S.phantom_params
+    S.phantom_params = lambda cc: p0
+    try:
+        g = S.sinogram(c, noise=False).numpy()
+    finally:
+        S.phantom_params = orig
+    x = np.arange(c.n) - (c.n - 1) / 2.0
+    X, Y = np.meshgrid(x, x, indexing="xy")
+    img = np.zeros((c.n, c.n))
+    for o in range(c.n_objects):
+        img += p0["rho"][o] * ((X - p0["c0"][o, 0]) ** 2 + (Y - p0["c0"][o, 1]) ** 2 <= p0["A0"][o] ** 2)
+    P = oracle.Problem(c.n, 1, c.nd, c.n_angles, 1, 1, np.ones((1, c.n_angles)))
+    gp = P.forward(img.reshape(P.primal_shape))
+    assert np.linalg.norm(gp - g) / np.linalg.norm(g) < 3e-2
