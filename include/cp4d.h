@@ -1,0 +1,138 @@
+/*
+ * cp4d.h -- C ABI of libcp4d.so: the Chambolle-Pock hot path of "Four-dimensional tomographic
+ * reconstruction by time domain decomposition" (arXiv 1809.09725; citations below are PAPER.md
+ * line numbers) as hand-written sm_100a CUDA kernels.  One GPU, fp32 arithmetic,
+ * no CPU fallback: every entry point that computes runs CUDA kernels or fails with an error code.
+ *
+ * Problem.  f(x,y,z,t) ~ sum_j f_j(x,y,z) phi_j(t), j < m (Eq. 8).  The primal variable
+ * is the coefficient stack f_j (reading C1).  Minimise (Eq. 6)
+ *      1/2 |K1 f - g|^2 + lambda1 | |K2 f| |_1 ,
+ *   K1 f [z,k,b] = sum_j Phi[j,k] * (R_{theta_k} f_j(.,.,z))[b]          (Eq. 9; L231)
+ *   K2 f         = grad_{lambda2} f = (d_x f, d_y f, d_z f, lambda2 d_t f)  (Eq. 5; L123)
+ * with the Chambolle-Pock iteration of Fig. 2 (L147-L168).  R is the static parallel-beam Radon
+ * transform discretised by the Joseph linear-interpolation ray sum (reading R3; the
+ * paper's own log-polar code is not specified, L281): equivalently the matrix
+ *      A_k[b; iy,ix] = Lambda((x_ix c_k + y_iy s_k - s_b)/a_k)/a_k,  Lambda(u) = max(0, 1-|u|),
+ *      a_k = max(|c_k|,|s_k|),  c_k = cos theta_k, s_k = sin theta_k.
+ *
+ * Geometry (R1/R2).  Unit voxel and bin spacing; voxel centres x_ix = ix-(n-1)/2,
+ * y_iy = iy-(n-1)/2; bin centres s_b = b-(nd-1)/2; theta_k = k*pi/n_theta0 with
+ * n_theta0 = n_angles/n_half_rot; t_k = k/n_angles (enters only through the caller's table Phi).
+ * Values outside the grid are zero; rays exist only for 0 <= b < nd.
+ *
+ * Layouts (dense, no padding, fp32, base pointers 16-byte aligned; V = nz*n*n*m, S = nz*n_angles*nd):
+ *   primal-shaped   f[z][iy][ix][j]        j fastest                      V floats
+ *   sinogram        g[z][k][b]             b fastest                      S floats
+ *   dual field      p[a][z][iy][ix][j]     a = 0..3 = (x, y, z, t)        4V floats, component-major
+ *   basis table     phi[j][k] = phi_j(t_k) host memory, copied at create  m*n_angles floats
+ *
+ * Pointers named *_dev are DEVICE pointers on `device`, *_host are HOST pointers.  The caller owns
+ * every buffer it passes (e.g. PyTorch tensors); the library never frees or resizes them and
+ * allocates no device memory: all state and scratch live in the caller's workspace.  Input and
+ * output buffers of one call must not overlap (CP4D_EINVAL) unless a parameter says "in/out".
+ * All kernels are enqueued on the stream given at create; calls are asynchronous unless they say
+ * "syncs".  Asynchronous faults surface at the next syncing call as CP4D_ECUDA.
+ *
+ * Every function returns 0 (CP4D_OK) or a negative error code; nothing throws, exits or prints.
+ */
+#ifndef CP4D_H
+#define CP4D_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define CP4D_OK            0
+#define CP4D_EINVAL       -1  /* null pointer, bad size, n_angles % n_half_rot, m % 4, m > 32, misaligned, aliasing */
+#define CP4D_EWORKSPACE   -2  /* workspace missing or smaller than cp4d_workspace_bytes() */
+#define CP4D_EUNSUPPORTED -3  /* no CUDA device / device is not compute capability 10.x */
+#define CP4D_ECUDA        -4  /* a CUDA runtime call or kernel failed; text in cp4d_last_error() */
+#define CP4D_ESTATE       -5  /* call order: cp4d_iterate before cp4d_set_data / cp4d_set_steps */
+
+typedef struct cp4d_ctx cp4d_ctx; /* opaque; owns host-side metadata only */
+
+typedef struct {
+    int32_t nx, ny;           /* grid side; the hot path requires nx == ny (= n)                          */
+    int32_t nz;               /* slices, >= 1                                                              */
+    int32_t nd;               /* detector bins, >= 2, unit spacing, centred                                */
+    int32_t n_angles;         /* N_theta, total projections                                                */
+    int32_t n_half_rot;       /* N_pi half-rotations; n_angles % n_half_rot == 0 (L200; C17)     */
+    int32_t m;                /* temporal basis functions (the paper's M); m % 4 == 0, 4 <= m <= 32        */
+    int32_t device;           /* CUDA device ordinal                                                       */
+    const float *phi_host;    /* HOST, m*n_angles, [j][k] = phi_j(t_k); copied at create (L176-L180)       */
+    float lambda1, lambda2;   /* Eq. (5)/(6): TV weight; temporal scale inside the 4-vector gradient       */
+    float theta_relax;        /* over-relaxation theta in [0,1] of Fig. 2 step 6 (C12: 1)        */
+    void *workspace_dev;      /* DEVICE, caller-allocated, >= cp4d_workspace_bytes(), 256-byte aligned     */
+    uint64_t workspace_bytes;
+    void *stream;             /* cudaStream_t (0 = legacy default stream)                                  */
+} cp4d_params;
+
+/* Bytes of device workspace a context for these sizes needs (state f, f~, K1^T h1, h2[4], h1, g,
+ * projector scratch, tables).  Host only; ignores workspace_dev/stream/phi_host. */
+int cp4d_workspace_bytes(const cp4d_params *p, uint64_t *bytes_out);
+
+/* Validate, compute the fp64 angle/tile tables on the host, copy them and phi into the workspace,
+ * carve the workspace.  Launches no kernel.  The context keeps workspace_dev and stream. */
+int cp4d_create(const cp4d_params *p, cp4d_ctx **ctx_out);
+int cp4d_destroy(cp4d_ctx *ctx);
+
+/* ---- stateless operators on caller-owned DEVICE buffers -------------------------------------- */
+/* g = K1 f  (Eq. 9; pi-folding L198-L202: ray sums over the n_theta0 base angles with all m
+ * coefficients accumulated per ray, then n_half_rot m-wide dot products with Phi).  f: V, g: S. */
+int cp4d_forward(cp4d_ctx *ctx, const float *f_dev, float *g_dev);
+/* f = K1^T g, overwrite (Eq. 10; fold L204-L212: gt_j = sum_q Phi[j,q n0+i] g[q n0+i, flip_q b],
+ * then one backprojection over [0,pi)).  Exact transpose of cp4d_forward up to fp32 rounding. */
+int cp4d_adjoint(cp4d_ctx *ctx, const float *g_dev, float *f_dev);
+/* p = K2 f: forward differences along x, y, z, t (t scaled by lambda2), 0 at the last index of
+ * each axis (R4).  f: V, p: 4V. */
+int cp4d_grad(cp4d_ctx *ctx, const float *f_dev, float *p_dev);
+/* f = div p = -K2^T p (L131-L133).  p: 4V, f: V. */
+int cp4d_div(cp4d_ctx *ctx, const float *p_dev, float *f_dev);
+
+/* ---- the three fused steps of Fig. 2 on caller-owned DEVICE buffers --------------------------- */
+/* step 3 (L154, L135): h1 <- (h1 + sigma (K1 ft - g)) / (1 + sigma).   h1 in/out (S), ft: V, g: S. */
+int cp4d_prox_f1(cp4d_ctx *ctx, float sigma, const float *ft_dev, const float *g_dev, float *h1_dev);
+/* step 4 (L158, L137; R5): q = h2 + sigma grad ft; h2 <- q / max(1, |q|_2 / lambda1)
+ * pointwise over the 4-vector at each (x,y,z,j); lambda1 == 0 gives h2 = 0.  h2 in/out (4V). */
+int cp4d_prox_f2(cp4d_ctx *ctx, float sigma, const float *ft_dev, float *h2_dev);
+/* steps 5-6 (L162-L166): f+ = f - tau K1^T h1 + tau div h2;  ft = f+ + theta (f+ - f);  f <- f+.
+ * f in/out (V), ft out (V), h1: S, h2: 4V. */
+int cp4d_primal_update(cp4d_ctx *ctx, float tau, const float *h1_dev, const float *h2_dev, float *f_dev,
+                       float *ft_dev);
+
+/* ---- reductions (fp32 in, fp64 accumulate).  Sync. ------------------------------------------- */
+int cp4d_dot(cp4d_ctx *ctx, const float *x_dev, const float *y_dev, uint64_t count, double *out_host);
+
+/* ---- power iteration for L = ||K||, K = (K1; K2) (L97, L147; R8) ------------------- */
+/* x0 = counter-based N(0,1) from `seed`; n_power_iters steps of y = K1^T K1 x + K2^T K2 x,
+ * L = sqrt(|y|/|x|).  Uses the CP state buffers as scratch (call before cp4d_reset).  Syncs. */
+int cp4d_norm(cp4d_ctx *ctx, int32_t n_power_iters, uint64_t seed, float *L_out_host);
+
+/* ---- Chambolle-Pock state machine; state (f, ft, h1, h2, g) lives in the workspace ----------- */
+int cp4d_set_data(cp4d_ctx *ctx, const float *g_dev);                 /* copy measured data g (S) */
+int cp4d_set_steps(cp4d_ctx *ctx, float tau, float sigma);            /* tau*sigma*L^2 < 1 is the caller's duty */
+int cp4d_reset(cp4d_ctx *ctx, const float *f0_dev /* nullable => zeros */); /* f = ft = f0, h1 = h2 = 0 */
+int cp4d_iterate(cp4d_ctx *ctx, int32_t n_iters);                     /* n_iters x steps 3-6, async */
+int cp4d_get_f(cp4d_ctx *ctx, float *f_dev_out);                      /* copy f (V) */
+/* device pointers of the state arrays inside the workspace (for inspection / teacher forcing);
+ * any of the out pointers may be null. */
+int cp4d_state_ptrs(cp4d_ctx *ctx, float **f, float **ft, float **h1, float **h2, float **g);
+
+/* ---- end-to-end call with HOST buffers (pinned or pageable) ---------------------------------- */
+/* H2D copy of g_host (S), reset to zeros, n_iters iterations with the current steps, D2H copy of f
+ * into f_host (V).  Syncs. */
+int cp4d_solve_host(cp4d_ctx *ctx, const float *g_host, int32_t n_iters, float *f_host);
+
+int cp4d_sync(cp4d_ctx *ctx);
+/* number of kernels (and memset nodes) this context has enqueued since create */
+int cp4d_launch_count(const cp4d_ctx *ctx, uint64_t *count_out);
+const char *cp4d_strerror(int code);
+const char *cp4d_last_error(const cp4d_ctx *ctx);
+const char *cp4d_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* CP4D_H */

@@ -1,0 +1,242 @@
+"""Thin ctypes binding of libcp4d.so (include/cp4d.h): argument marshalling only.
+
+Every step of the hot path runs in the CUDA kernels behind the C ABI; PyTorch is used for device memory
+(`torch.empty(..., device="cuda")`), `data_ptr()` and the current stream.  There is no CPU fallback:
+if the library is missing or the device is not sm_100, calls raise.
+"""
+from __future__ import annotations
+
+import ctypes as C
+from pathlib import Path
+
+import numpy as np
+
+_PKG = Path(__file__).resolve().parent
+LIB_PATH = _PKG / "libcp4d.so"
+_lib = None
+
+OK, EINVAL, EWORKSPACE, EUNSUPPORTED, ECUDA, ESTATE = 0, -1, -2, -3, -4, -5
+
+
+class Cp4dError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__(f"cp4d error {code}: {msg}")
+        self.code = code
+
+
+class Params(C.Structure):
+    _fields_ = [("nx", C.c_int32), ("ny", C.c_int32), ("nz", C.c_int32), ("nd", C.c_int32),
+                ("n_angles", C.c_int32), ("n_half_rot", C.c_int32), ("m", C.c_int32), ("device", C.c_int32),
+                ("phi_host", C.c_void_p), ("lambda1", C.c_float), ("lambda2", C.c_float),
+                ("theta_relax", C.c_float), ("workspace_dev", C.c_void_p), ("workspace_bytes", C.c_uint64),
+                ("stream", C.c_void_p)]
+
+
+def lib():
+    """Load libcp4d.so (built in-tree by paper_1809_09725_b200.build).  Raises if it is missing."""
+    global _lib
+    if _lib is None:
+        if not LIB_PATH.exists():
+            raise FileNotFoundError(f"{LIB_PATH} not built: run `python -c 'import __graft_entry__ as g; g.build()'` "
+                                    "(no CPU fallback exists)")
+        L = C.CDLL(str(LIB_PATH))
+        vp, f32, i32, u64 = C.c_void_p, C.c_float, C.c_int32, C.c_uint64
+        sig = {
+            "cp4d_workspace_bytes": [C.POINTER(Params), C.POINTER(u64)],
+            "cp4d_create": [C.POINTER(Params), C.POINTER(vp)],
+            "cp4d_destroy": [vp],
+            "cp4d_forward": [vp, vp, vp], "cp4d_adjoint": [vp, vp, vp], "cp4d_grad": [vp, vp, vp], "cp4d_div": [vp, vp, vp],
+            "cp4d_prox_f1": [vp, f32, vp, vp, vp], "cp4d_prox_f2": [vp, f32, vp, vp],
+            "cp4d_primal_update": [vp, f32, vp, vp, vp, vp],
+            "cp4d_dot": [vp, vp, vp, u64, C.POINTER(C.c_double)],
+            "cp4d_norm": [vp, i32, u64, C.POINTER(f32)],
+            "cp4d_set_data": [vp, vp], "cp4d_set_steps": [vp, f32, f32], "cp4d_reset": [vp, vp],
+            "cp4d_iterate": [vp, i32], "cp4d_get_f": [vp, vp],
+            "cp4d_state_ptrs": [vp] + [C.POINTER(vp)] * 5,
+            "cp4d_solve_host": [vp, vp, i32, vp], "cp4d_sync": [vp],
+            "cp4d_launch_count": [vp, C.POINTER(u64)],
+        }
+        for name, args in sig.items():
+            fn = getattr(L, name)
+            fn.argtypes, fn.restype = args, C.c_int
+        for name in ("cp4d_strerror", "cp4d_last_error", "cp4d_version"):
+            getattr(L, name).restype = C.c_char_p
+        L.cp4d_strerror.argtypes = [C.c_int]
+        L.cp4d_last_error.argtypes = [vp]
+        _lib = L
+    return _lib
+
+
+def make_params(n, nz, nd, n_angles, n_half_rot, m, phi=None, lambda1=1e-3, lambda2=1.0, theta=1.0, device=0,
+                workspace_ptr=0, workspace_bytes=0, stream=0, ny=None):
+    p = Params()
+    p.nx, p.ny, p.nz, p.nd = n, (n if ny is None else ny), nz, nd
+    p.n_angles, p.n_half_rot, p.m, p.device = n_angles, n_half_rot, m, device
+    p.phi_host = None if phi is None else phi.ctypes.data
+    p.lambda1, p.lambda2, p.theta_relax = lambda1, lambda2, theta
+    p.workspace_dev, p.workspace_bytes, p.stream = workspace_ptr or None, workspace_bytes, stream or None
+    return p
+
+
+def workspace_bytes(n, nz, nd, n_angles, n_half_rot, m) -> int:
+    out = C.c_uint64(0)
+    p = make_params(n, nz, nd, n_angles, n_half_rot, m)
+    r = lib().cp4d_workspace_bytes(C.byref(p), C.byref(out))
+    if r:
+        raise Cp4dError(r, lib().cp4d_strerror(r).decode())
+    return out.value
+
+
+class Context:
+    """One reconstruction problem on one GPU.  Tensors are torch CUDA float32, contiguous, layouts of cp4d.h."""
+
+    def __init__(self, n, nz, nd, n_angles, n_half_rot, m, phi, lambda1=1e-3, lambda2=1.0, theta=1.0, device=0):
+        import torch
+        self.torch = torch
+        self.n, self.nz, self.nd, self.n_angles, self.n_half_rot, self.m = n, nz, nd, n_angles, n_half_rot, m
+        self.primal_shape, self.sino_shape = (nz, n, n, m), (nz, n_angles, nd)
+        self.V, self.S = nz * n * n * m, nz * n_angles * nd
+        self.device = torch.device("cuda", device)
+        self._phi = np.ascontiguousarray(phi, dtype=np.float32).reshape(m, n_angles)
+        nbytes = workspace_bytes(n, nz, nd, n_angles, n_half_rot, m)
+        with torch.cuda.device(self.device):
+            self.workspace = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
+            base = (self.workspace.data_ptr() + 255) // 256 * 256
+            self.stream = torch.cuda.current_stream(self.device)
+            p = make_params(n, nz, nd, n_angles, n_half_rot, m, self._phi, lambda1, lambda2, theta, device,
+                            base, nbytes, self.stream.cuda_stream)
+            h = C.c_void_p()
+            r = lib().cp4d_create(C.byref(p), C.byref(h))
+        if r:
+            raise Cp4dError(r, lib().cp4d_strerror(r).decode())
+        self._h = h
+
+    @classmethod
+    def from_config(cls, c, phi=None, device=0, **kw):
+        from . import synth
+        if phi is None:
+            phi = synth.basis_table(c.basis, c.m, c.n_angles)
+        kw.setdefault("lambda1", c.lambda1)
+        kw.setdefault("lambda2", c.lambda2)
+        return cls(c.n, c.nz, c.nd, c.n_angles, c.n_half_rot, c.m, phi, device=device, **kw)
+
+    # -- helpers ---------------------------------------------------------------------------------
+    def _ck(self, r):
+        if r:
+            raise Cp4dError(r, f"{lib().cp4d_strerror(r).decode()}: {lib().cp4d_last_error(self._h).decode()}")
+
+    def _t(self, t, numel):
+        assert t.is_cuda and t.dtype == self.torch.float32 and t.is_contiguous() and t.numel() == numel, \
+            f"need contiguous cuda float32 tensor with {numel} elements, got {tuple(t.shape)} {t.dtype} {t.device}"
+        return t.data_ptr()
+
+    def empty_primal(self):
+        return self.torch.empty(self.primal_shape, dtype=self.torch.float32, device=self.device)
+
+    def empty_sino(self):
+        return self.torch.empty(self.sino_shape, dtype=self.torch.float32, device=self.device)
+
+    def empty_dual(self):
+        return self.torch.empty((4,) + self.primal_shape, dtype=self.torch.float32, device=self.device)
+
+    # -- operators (names of include/cp4d.h) -----------------------------------------------------
+    def forward(self, f, out=None):
+        out = self.empty_sino() if out is None else out
+        self._ck(lib().cp4d_forward(self._h, self._t(f, self.V), self._t(out, self.S)))
+        return out
+
+    def adjoint(self, g, out=None):
+        out = self.empty_primal() if out is None else out
+        self._ck(lib().cp4d_adjoint(self._h, self._t(g, self.S), self._t(out, self.V)))
+        return out
+
+    def grad(self, f, out=None):
+        out = self.empty_dual() if out is None else out
+        self._ck(lib().cp4d_grad(self._h, self._t(f, self.V), self._t(out, 4 * self.V)))
+        return out
+
+    def div(self, p, out=None):
+        out = self.empty_primal() if out is None else out
+        self._ck(lib().cp4d_div(self._h, self._t(p, 4 * self.V), self._t(out, self.V)))
+        return out
+
+    def prox_f1(self, sigma, ft, g, h1):
+        self._ck(lib().cp4d_prox_f1(self._h, sigma, self._t(ft, self.V), self._t(g, self.S), self._t(h1, self.S)))
+        return h1
+
+    def prox_f2(self, sigma, ft, h2):
+        self._ck(lib().cp4d_prox_f2(self._h, sigma, self._t(ft, self.V), self._t(h2, 4 * self.V)))
+        return h2
+
+    def primal_update(self, tau, h1, h2, f, ft):
+        self._ck(lib().cp4d_primal_update(self._h, tau, self._t(h1, self.S), self._t(h2, 4 * self.V),
+                                          self._t(f, self.V), self._t(ft, self.V)))
+        return f, ft
+
+    def dot(self, x, y):
+        out = C.c_double(0)
+        assert x.numel() == y.numel()
+        self._ck(lib().cp4d_dot(self._h, self._t(x, x.numel()), self._t(y, y.numel()), x.numel(), C.byref(out)))
+        return out.value
+
+    def norm(self, n_power_iters=30, seed=0):
+        out = C.c_float(0)
+        self._ck(lib().cp4d_norm(self._h, n_power_iters, seed, C.byref(out)))
+        return out.value
+
+    # -- CP state machine ------------------------------------------------------------------------
+    def set_data(self, g):
+        self._ck(lib().cp4d_set_data(self._h, self._t(g, self.S)))
+
+    def set_steps(self, tau, sigma):
+        self._ck(lib().cp4d_set_steps(self._h, tau, sigma))
+
+    def reset(self, f0=None):
+        self._ck(lib().cp4d_reset(self._h, None if f0 is None else self._t(f0, self.V)))
+
+    def iterate(self, n_iters):
+        self._ck(lib().cp4d_iterate(self._h, n_iters))
+
+    def get_f(self, out=None):
+        out = self.empty_primal() if out is None else out
+        self._ck(lib().cp4d_get_f(self._h, self._t(out, self.V)))
+        return out
+
+    def state(self):
+        """Views (no copy) of the state arrays inside the workspace: dict f, ft, h1, h2, g."""
+        ptrs = [C.c_void_p() for _ in range(5)]
+        self._ck(lib().cp4d_state_ptrs(self._h, *[C.byref(p) for p in ptrs]))
+        base = self.workspace.data_ptr()
+        shapes = [self.primal_shape, self.primal_shape, self.sino_shape, (4,) + self.primal_shape, self.sino_shape]
+        out = {}
+        for name, p, shp in zip(("f", "ft", "h1", "h2", "g"), ptrs, shapes):
+            off = p.value - base
+            nb = int(np.prod(shp)) * 4
+            out[name] = self.workspace[off:off + nb].view(self.torch.float32).view(shp)
+        return out
+
+    def solve_host(self, g_host, n_iters, f_host):
+        """g_host / f_host: CPU float32 torch tensors (pinned for full copy speed) or numpy arrays."""
+        gp = g_host.data_ptr() if hasattr(g_host, "data_ptr") else g_host.ctypes.data
+        fp = f_host.data_ptr() if hasattr(f_host, "data_ptr") else f_host.ctypes.data
+        self._ck(lib().cp4d_solve_host(self._h, gp, n_iters, fp))
+        return f_host
+
+    def sync(self):
+        self._ck(lib().cp4d_sync(self._h))
+
+    def launch_count(self) -> int:
+        out = C.c_uint64(0)
+        self._ck(lib().cp4d_launch_count(self._h, C.byref(out)))
+        return out.value
+
+    def close(self):
+        if getattr(self, "_h", None):
+            lib().cp4d_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass

@@ -1,0 +1,356 @@
+// C ABI of libcp4d.so (include/cp4d.h): validation, workspace carving, host-side fp64 tables, and the
+// stream-ordered orchestration of Fig. 2.  No kernel code here.
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "cp4d_internal.cuh"
+
+using namespace cp4d;
+
+namespace {
+
+constexpr uint64_t ALIGN = 256;
+inline uint64_t up(uint64_t x) { return (x + ALIGN - 1) / ALIGN * ALIGN; }
+
+int validate(const cp4d_params *p, Dims *d) {
+    if (!p) return CP4D_EINVAL;
+    if (p->nx != p->ny || p->nx < 2 || p->nz < 1 || p->nd < 2 || p->n_angles < 1 || p->n_half_rot < 1) return CP4D_EINVAL;
+    if (p->n_angles % p->n_half_rot) return CP4D_EINVAL;
+    if (p->m < 4 || p->m > MAX_M || p->m % 4) return CP4D_EINVAL;
+    if (!(p->lambda1 >= 0.f) || !(p->theta_relax >= 0.f && p->theta_relax <= 1.f) || !std::isfinite(p->lambda2)) return CP4D_EINVAL;
+    d->n = p->nx; d->nz = p->nz; d->nd = p->nd; d->na = p->n_angles; d->npi = p->n_half_rot;
+    d->n0 = d->na / d->npi; d->m = p->m; d->Q = p->m / 4;
+    d->tiles_1d = (d->n + TILE - 1) / TILE; d->tiles = d->tiles_1d * d->tiles_1d;
+    d->V = (int64_t)d->nz * d->n * d->n * d->m;
+    d->S = (int64_t)d->nz * d->na * d->nd;
+    d->slice4 = (int64_t)d->n * d->n * d->Q;
+    d->scratch4 = (int64_t)d->nz * d->n0 * d->Q * d->nd;
+    if (d->nz > 65535 || d->tiles > 2000000) return CP4D_EINVAL;
+    return CP4D_OK;
+}
+
+struct Carve {
+    uint64_t f, ft, bp, h2, h1, g, scratch, phi, ang, geo, red, total;
+};
+Carve carve(const Dims &d) {
+    Carve c;
+    uint64_t o = 0;
+    auto take = [&](uint64_t bytes) { uint64_t r = o; o += up(bytes); return r; };
+    c.f = take(d.V * 4); c.ft = take(d.V * 4); c.bp = take(d.V * 4); c.h2 = take(d.V * 16);
+    c.h1 = take(d.S * 4); c.g = take(d.S * 4); c.scratch = take(d.scratch4 * 16);
+    c.phi = take((uint64_t)d.m * d.na * 4); c.ang = take((uint64_t)d.n0 * sizeof(AngleTab));
+    c.geo = take((uint64_t)d.tiles * d.n0 * sizeof(TileGeo)); c.red = take(64);
+    c.total = o;
+    return c;
+}
+
+int fail(cp4d_ctx *c, int code, const char *what, cudaError_t e = cudaSuccess) {
+    if (c) {
+        c->err = what;
+        if (e != cudaSuccess) { c->err += ": "; c->err += cudaGetErrorString(e); }
+    }
+    return code;
+}
+#define CK(call, what)                                                  \
+    do {                                                                \
+        cudaError_t e__ = (call);                                       \
+        if (e__ != cudaSuccess) return fail(ctx, CP4D_ECUDA, what, e__); \
+    } while (0)
+
+bool overlap(const void *a, uint64_t na, const void *b, uint64_t nb) {
+    const uintptr_t x = (uintptr_t)a, y = (uintptr_t)b;
+    return x < y + nb && y < x + na;
+}
+bool bad_ptr(const void *p) { return !p || ((uintptr_t)p & 15); }
+
+int forward_into(cp4d_ctx *ctx, const float *f, int mode, float sigma, const float *g, float *out) {
+    CK(launch_forward_partial(ctx, f, ctx->scratch), "forward_partial");
+    CK(launch_synth(ctx, ctx->scratch, mode, sigma, g, out), "synth");
+    return CP4D_OK;
+}
+int adjoint_into(cp4d_ctx *ctx, const float *g, float *f) {
+    CK(launch_fold(ctx, g, ctx->scratch), "fold");
+    CK(launch_backproject(ctx, ctx->scratch, f), "backproject");
+    return CP4D_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char *cp4d_version(void) { return "cp4d 0.1 (sm_100a)"; }
+
+const char *cp4d_strerror(int code) {
+    switch (code) {
+    case CP4D_OK: return "ok";
+    case CP4D_EINVAL: return "invalid argument";
+    case CP4D_EWORKSPACE: return "workspace missing or too small";
+    case CP4D_EUNSUPPORTED: return "no sm_100 CUDA device";
+    case CP4D_ECUDA: return "CUDA error";
+    case CP4D_ESTATE: return "call order: set_data/set_steps before iterate";
+    default: return "unknown error";
+    }
+}
+
+const char *cp4d_last_error(const cp4d_ctx *ctx) { return ctx ? ctx->err.c_str() : "null context"; }
+
+int cp4d_workspace_bytes(const cp4d_params *p, uint64_t *out) {
+    Dims d;
+    if (!out) return CP4D_EINVAL;
+    int r = validate(p, &d);
+    if (r) return r;
+    *out = carve(d).total;
+    return CP4D_OK;
+}
+
+int cp4d_create(const cp4d_params *p, cp4d_ctx **out) {
+    if (!out) return CP4D_EINVAL;
+    *out = nullptr;
+    Dims d;
+    int r = validate(p, &d);
+    if (r) return r;
+    if (!p->phi_host) return CP4D_EINVAL;
+    const Carve cv = carve(d);
+    if (!p->workspace_dev || p->workspace_bytes < cv.total) return CP4D_EWORKSPACE;
+    if ((uintptr_t)p->workspace_dev & (ALIGN - 1)) return CP4D_EINVAL;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || p->device < 0 || p->device >= ndev) { cudaGetLastError(); return CP4D_EUNSUPPORTED; }
+    cudaDeviceProp prop;
+    if (cudaGetDeviceProperties(&prop, p->device) != cudaSuccess || prop.major != 10) { cudaGetLastError(); return CP4D_EUNSUPPORTED; }
+    if (cudaSetDevice(p->device) != cudaSuccess) return CP4D_ECUDA;
+
+    cp4d_ctx *ctx = new (std::nothrow) cp4d_ctx();
+    if (!ctx) return CP4D_EINVAL;
+    ctx->d = d; ctx->lambda1 = p->lambda1; ctx->lambda2 = p->lambda2; ctx->theta = p->theta_relax;
+    ctx->tau = ctx->sigma = 0.f; ctx->have_steps = ctx->have_data = false;
+    ctx->device = p->device; ctx->stream = (cudaStream_t)p->stream; ctx->launches = 0;
+    char *w = (char *)p->workspace_dev;
+    ctx->f = (float *)(w + cv.f); ctx->ft = (float *)(w + cv.ft); ctx->bp = (float *)(w + cv.bp);
+    ctx->h2 = (float *)(w + cv.h2); ctx->h1 = (float *)(w + cv.h1); ctx->g = (float *)(w + cv.g);
+    ctx->scratch = (float4 *)(w + cv.scratch); ctx->phi = (float *)(w + cv.phi);
+    ctx->ang = (AngleTab *)(w + cv.ang); ctx->geo = (TileGeo *)(w + cv.geo); ctx->red = (double *)(w + cv.red);
+
+    // host prologue: fp64 angle tables and per-(tile, angle) window geometry
+    std::vector<AngleTab> ang(d.n0);
+    std::vector<double> cs(2 * (size_t)d.n0);
+    const double PI = 3.14159265358979323846264338327950288;
+    for (int i = 0; i < d.n0; ++i) {
+        const double th = (double)i * PI / (double)d.n0, c = std::cos(th), s = std::sin(th);
+        cs[2 * i] = c; cs[2 * i + 1] = s;
+        ang[i].c = (float)c; ang[i].s = (float)s;
+        ang[i].inv_a = (float)(1.0 / std::fmax(std::fabs(c), std::fabs(s)));
+        ang[i].col_step = std::fabs(s) >= std::fabs(c) ? 1 : 0;
+    }
+    std::vector<TileGeo> geo((size_t)d.tiles * d.n0);
+    const double cen = 0.5 * (d.n - 1), cd = 0.5 * (d.nd - 1);
+    for (int t = 0; t < d.tiles; ++t) {
+        const double x0 = (double)(t % d.tiles_1d) * TILE - cen, y0 = (double)(t / d.tiles_1d) * TILE - cen;
+        for (int i = 0; i < d.n0; ++i) {
+            // the tables hold the fp32-rounded c, s the kernels multiply lx, ly with; the tile origin term is fp64
+            const double c = cs[2 * i], s = cs[2 * i + 1];
+            const double p0 = x0 * c + y0 * s + cd;
+            const double pmin = p0 + std::fmin(0.0, (TILE - 1) * c) + std::fmin(0.0, (TILE - 1) * s);
+            const double bs = std::floor(pmin) - 1.0;
+            geo[(size_t)t * d.n0 + i].bstart = (int32_t)bs;
+            geo[(size_t)t * d.n0 + i].delta = (float)(p0 - bs);
+        }
+    }
+    cudaError_t e;
+    if ((e = cudaMemcpyAsync(ctx->phi, p->phi_host, (size_t)d.m * d.na * 4, cudaMemcpyHostToDevice, ctx->stream)) != cudaSuccess ||
+        (e = cudaMemcpyAsync(ctx->ang, ang.data(), ang.size() * sizeof(AngleTab), cudaMemcpyHostToDevice, ctx->stream)) != cudaSuccess ||
+        (e = cudaMemcpyAsync(ctx->geo, geo.data(), geo.size() * sizeof(TileGeo), cudaMemcpyHostToDevice, ctx->stream)) != cudaSuccess ||
+        (e = cudaStreamSynchronize(ctx->stream)) != cudaSuccess) {
+        delete ctx;
+        return CP4D_ECUDA;
+    }
+    *out = ctx;
+    return CP4D_OK;
+}
+
+int cp4d_destroy(cp4d_ctx *ctx) {
+    delete ctx;
+    return CP4D_OK;
+}
+
+int cp4d_forward(cp4d_ctx *ctx, const float *f, float *g) {
+    if (!ctx) return CP4D_EINVAL;
+    if (bad_ptr(f) || bad_ptr(g) || overlap(f, ctx->d.V * 4, g, ctx->d.S * 4)) return fail(ctx, CP4D_EINVAL, "forward: bad pointers");
+    return forward_into(ctx, f, 0, 0.f, nullptr, g);
+}
+
+int cp4d_adjoint(cp4d_ctx *ctx, const float *g, float *f) {
+    if (!ctx) return CP4D_EINVAL;
+    if (bad_ptr(f) || bad_ptr(g) || overlap(f, ctx->d.V * 4, g, ctx->d.S * 4)) return fail(ctx, CP4D_EINVAL, "adjoint: bad pointers");
+    return adjoint_into(ctx, g, f);
+}
+
+int cp4d_grad(cp4d_ctx *ctx, const float *f, float *p) {
+    if (!ctx) return CP4D_EINVAL;
+    if (bad_ptr(f) || bad_ptr(p) || overlap(f, ctx->d.V * 4, p, ctx->d.V * 16)) return fail(ctx, CP4D_EINVAL, "grad: bad pointers");
+    CK(launch_grad(ctx, f, p), "grad");
+    return CP4D_OK;
+}
+
+int cp4d_div(cp4d_ctx *ctx, const float *p, float *f) {
+    if (!ctx) return CP4D_EINVAL;
+    if (bad_ptr(f) || bad_ptr(p) || overlap(f, ctx->d.V * 4, p, ctx->d.V * 16)) return fail(ctx, CP4D_EINVAL, "div: bad pointers");
+    CK(launch_div(ctx, p, f), "div");
+    return CP4D_OK;
+}
+
+int cp4d_prox_f1(cp4d_ctx *ctx, float sigma, const float *ft, const float *g, float *h1) {
+    if (!ctx) return CP4D_EINVAL;
+    const uint64_t Vb = ctx->d.V * 4, Sb = ctx->d.S * 4;
+    if (bad_ptr(ft) || bad_ptr(g) || bad_ptr(h1) || overlap(ft, Vb, h1, Sb) || overlap(g, Sb, h1, Sb) || !(sigma > 0.f))
+        return fail(ctx, CP4D_EINVAL, "prox_f1: bad arguments");
+    return forward_into(ctx, ft, 1, sigma, g, h1);
+}
+
+int cp4d_prox_f2(cp4d_ctx *ctx, float sigma, const float *ft, float *h2) {
+    if (!ctx) return CP4D_EINVAL;
+    if (bad_ptr(ft) || bad_ptr(h2) || overlap(ft, ctx->d.V * 4, h2, ctx->d.V * 16)) return fail(ctx, CP4D_EINVAL, "prox_f2: bad pointers");
+    CK(launch_prox_f2(ctx, sigma, ft, h2), "prox_f2");
+    return CP4D_OK;
+}
+
+int cp4d_primal_update(cp4d_ctx *ctx, float tau, const float *h1, const float *h2, float *f, float *ft) {
+    if (!ctx) return CP4D_EINVAL;
+    const uint64_t Vb = ctx->d.V * 4, Sb = ctx->d.S * 4;
+    if (bad_ptr(h1) || bad_ptr(h2) || bad_ptr(f) || bad_ptr(ft) || overlap(f, Vb, ft, Vb) || overlap(f, Vb, h2, 4 * Vb) ||
+        overlap(ft, Vb, h2, 4 * Vb) || overlap(h1, Sb, f, Vb) || overlap(h1, Sb, ft, Vb))
+        return fail(ctx, CP4D_EINVAL, "primal_update: bad pointers");
+    int r = adjoint_into(ctx, h1, ctx->bp);
+    if (r) return r;
+    CK(launch_update(ctx, tau, ctx->bp, h2, f, ft), "update");
+    return CP4D_OK;
+}
+
+int cp4d_dot(cp4d_ctx *ctx, const float *x, const float *y, uint64_t n, double *out) {
+    if (!ctx) return CP4D_EINVAL;
+    if (bad_ptr(x) || bad_ptr(y) || !out) return fail(ctx, CP4D_EINVAL, "dot: bad pointers");
+    CK(launch_sumsq_dot(ctx, x, y, n, ctx->red), "dot");
+    CK(cudaMemcpyAsync(out, ctx->red, sizeof(double), cudaMemcpyDeviceToHost, ctx->stream), "dot copy");
+    CK(cudaStreamSynchronize(ctx->stream), "dot sync");
+    return CP4D_OK;
+}
+
+int cp4d_norm(cp4d_ctx *ctx, int32_t n_iters, uint64_t seed, float *L_out) {
+    if (!ctx) return CP4D_EINVAL;
+    if (!L_out || n_iters < 1) return fail(ctx, CP4D_EINVAL, "norm: bad arguments");
+    const Dims &d = ctx->d;
+    float *x = ctx->ft, *y1 = ctx->bp, *y2 = ctx->f;
+    double v = 0.0, L = 0.0;
+    CK(launch_fill_normal(ctx, x, d.V, seed), "fill");
+    if (int r = cp4d_dot(ctx, x, x, d.V, &v)) return r;
+    CK(launch_scale_diff(ctx, x, x, nullptr, (float)(1.0 / std::sqrt(v)), d.V), "scale");
+    for (int it = 0; it < n_iters; ++it) {
+        if (int r = forward_into(ctx, x, 0, 0.f, nullptr, ctx->h1)) return r;   // K1 x
+        if (int r = adjoint_into(ctx, ctx->h1, y1)) return r;                   // K1^T K1 x
+        CK(launch_grad(ctx, x, ctx->h2), "grad");
+        CK(launch_div(ctx, ctx->h2, y2), "div");                                // -K2^T K2 x
+        CK(launch_scale_diff(ctx, y1, y1, y2, 1.0f, d.V), "diff");              // y = K^T K x
+        if (int r = cp4d_dot(ctx, y1, y1, d.V, &v)) return r;
+        const double ny = std::sqrt(v);
+        L = std::sqrt(ny);                                                      // |x| = 1
+        if (!(ny > 0.0)) break;
+        CK(launch_scale_diff(ctx, x, y1, nullptr, (float)(1.0 / ny), d.V), "normalise");
+    }
+    ctx->have_data = false;  // state buffers were used as scratch
+    *L_out = (float)L;
+    return CP4D_OK;
+}
+
+int cp4d_set_data(cp4d_ctx *ctx, const float *g) {
+    if (!ctx) return CP4D_EINVAL;
+    if (bad_ptr(g)) return fail(ctx, CP4D_EINVAL, "set_data: bad pointer");
+    CK(cudaMemcpyAsync(ctx->g, g, ctx->d.S * 4, cudaMemcpyDeviceToDevice, ctx->stream), "set_data");
+    ctx->have_data = true;
+    return CP4D_OK;
+}
+
+int cp4d_set_steps(cp4d_ctx *ctx, float tau, float sigma) {
+    if (!ctx) return CP4D_EINVAL;
+    if (!(tau > 0.f) || !(sigma > 0.f)) return fail(ctx, CP4D_EINVAL, "set_steps: tau, sigma must be > 0");
+    ctx->tau = tau; ctx->sigma = sigma; ctx->have_steps = true;
+    return CP4D_OK;
+}
+
+int cp4d_reset(cp4d_ctx *ctx, const float *f0) {
+    if (!ctx) return CP4D_EINVAL;
+    const Dims &d = ctx->d;
+    if (f0) {
+        if (bad_ptr(f0)) return fail(ctx, CP4D_EINVAL, "reset: bad pointer");
+        CK(cudaMemcpyAsync(ctx->f, f0, d.V * 4, cudaMemcpyDeviceToDevice, ctx->stream), "reset f");
+        CK(cudaMemcpyAsync(ctx->ft, f0, d.V * 4, cudaMemcpyDeviceToDevice, ctx->stream), "reset ft");
+    } else {
+        CK(cudaMemsetAsync(ctx->f, 0, d.V * 4, ctx->stream), "reset f");
+        CK(cudaMemsetAsync(ctx->ft, 0, d.V * 4, ctx->stream), "reset ft");
+    }
+    CK(cudaMemsetAsync(ctx->h1, 0, d.S * 4, ctx->stream), "reset h1");
+    CK(cudaMemsetAsync(ctx->h2, 0, d.V * 16, ctx->stream), "reset h2");
+    return CP4D_OK;
+}
+
+int cp4d_iterate(cp4d_ctx *ctx, int32_t n_iters) {
+    if (!ctx) return CP4D_EINVAL;
+    if (n_iters < 0) return fail(ctx, CP4D_EINVAL, "iterate: n_iters < 0");
+    if (!ctx->have_steps || !ctx->have_data) return fail(ctx, CP4D_ESTATE, "iterate: set_data and set_steps first");
+    for (int it = 0; it < n_iters; ++it) {
+        // step 3: h1 <- prox_{sigma F1*}(h1 + sigma K1 ft)
+        if (int r = forward_into(ctx, ctx->ft, 1, ctx->sigma, ctx->g, ctx->h1)) return r;
+        // step 4: h2 <- prox_{sigma F2*}(h2 + sigma K2 ft)
+        CK(launch_prox_f2(ctx, ctx->sigma, ctx->ft, ctx->h2), "prox_f2");
+        // steps 5-6: f <- f - tau K1^T h1 + tau div h2 ; ft <- f+ + theta (f+ - f)
+        if (int r = adjoint_into(ctx, ctx->h1, ctx->bp)) return r;
+        CK(launch_update(ctx, ctx->tau, ctx->bp, ctx->h2, ctx->f, ctx->ft), "update");
+    }
+    return CP4D_OK;
+}
+
+int cp4d_get_f(cp4d_ctx *ctx, float *out) {
+    if (!ctx) return CP4D_EINVAL;
+    if (bad_ptr(out)) return fail(ctx, CP4D_EINVAL, "get_f: bad pointer");
+    CK(cudaMemcpyAsync(out, ctx->f, ctx->d.V * 4, cudaMemcpyDeviceToDevice, ctx->stream), "get_f");
+    return CP4D_OK;
+}
+
+int cp4d_state_ptrs(cp4d_ctx *ctx, float **f, float **ft, float **h1, float **h2, float **g) {
+    if (!ctx) return CP4D_EINVAL;
+    if (f) *f = ctx->f;
+    if (ft) *ft = ctx->ft;
+    if (h1) *h1 = ctx->h1;
+    if (h2) *h2 = ctx->h2;
+    if (g) *g = ctx->g;
+    return CP4D_OK;
+}
+
+int cp4d_solve_host(cp4d_ctx *ctx, const float *g_host, int32_t n_iters, float *f_host) {
+    if (!ctx) return CP4D_EINVAL;
+    if (!g_host || !f_host || n_iters < 0) return fail(ctx, CP4D_EINVAL, "solve_host: bad arguments");
+    if (!ctx->have_steps) return fail(ctx, CP4D_ESTATE, "solve_host: set_steps first");
+    CK(cudaMemcpyAsync(ctx->g, g_host, ctx->d.S * 4, cudaMemcpyHostToDevice, ctx->stream), "solve_host h2d");
+    ctx->have_data = true;
+    if (int r = cp4d_reset(ctx, nullptr)) return r;
+    if (int r = cp4d_iterate(ctx, n_iters)) return r;
+    CK(cudaMemcpyAsync(f_host, ctx->f, ctx->d.V * 4, cudaMemcpyDeviceToHost, ctx->stream), "solve_host d2h");
+    CK(cudaStreamSynchronize(ctx->stream), "solve_host sync");
+    return CP4D_OK;
+}
+
+int cp4d_sync(cp4d_ctx *ctx) {
+    if (!ctx) return CP4D_EINVAL;
+    CK(cudaStreamSynchronize(ctx->stream), "sync");
+    CK(cudaGetLastError(), "sync");
+    return CP4D_OK;
+}
+
+int cp4d_launch_count(const cp4d_ctx *ctx, uint64_t *out) {
+    if (!ctx || !out) return CP4D_EINVAL;
+    *out = ctx->launches;
+    return CP4D_OK;
+}
+
+}  // extern "C"

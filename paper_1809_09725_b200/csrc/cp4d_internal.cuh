@@ -1,0 +1,74 @@
+// Internal declarations of libcp4d.so (sm_100a).  Not part of the C ABI (include/cp4d.h).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include <string>
+
+#include "cp4d.h"
+
+namespace cp4d {
+
+constexpr int TILE = 32;          // voxel tile side of both projector kernels
+constexpr int WIN = 48;           // bins a TILE x TILE tile can touch at one angle: floor(31*sqrt2)+4
+constexpr int MAX_M = 32;
+
+// per (tile, base angle) geometry, computed in fp64 on the host at create:
+// bin coordinate of tile-local voxel (lx, ly) relative to the window start is  delta + lx*c + ly*s.
+struct TileGeo {
+    int32_t bstart;  // first bin of the tile's window at this angle (may be < 0 or > nd-WIN)
+    float delta;     // p(tile origin) - bstart, in [1, WIN)
+};
+
+// per base angle, fp32 roundings of the fp64 host values
+struct AngleTab {
+    float c, s, inv_a;  // cos, sin, 1/max(|c|,|s|)
+    int32_t col_step;   // 1: |s| >= |c| (ray steps over columns ix), 0: steps over rows iy
+};
+
+struct Dims {
+    int n, nz, nd, na, npi, n0, m, Q;  // Q = m/4 float4 chunks per voxel
+    int tiles_1d, tiles;               // ceil(n/TILE), tiles_1d^2
+    int64_t V, S;                      // elements of a primal array / a sinogram
+    int64_t slice4;                    // float4 per slice: n*n*Q
+    int64_t scratch4;                  // float4 of projector scratch: nz*n0*Q*nd
+};
+
+}  // namespace cp4d
+
+struct cp4d_ctx {
+    cp4d::Dims d;
+    float lambda1, lambda2, theta;
+    float tau, sigma;
+    bool have_steps, have_data;
+    int device;
+    cudaStream_t stream;
+    // workspace carve-up (device pointers)
+    float *f, *ft, *bp, *h2, *h1, *g;
+    float4 *scratch;           // forward partial ray sums P / folded sinogram gt: [z][i][jc][b] float4
+    float *phi;                // [j][k]
+    cp4d::AngleTab *ang;       // [n0]
+    cp4d::TileGeo *geo;        // [tile][n0]
+    double *red;               // 8 doubles for reductions
+    uint64_t launches;
+    std::string err;
+};
+
+namespace cp4d {
+
+// launchers (each enqueues on ctx->stream and bumps ctx->launches); return cudaError_t
+cudaError_t launch_grad(cp4d_ctx *c, const float *f, float *p);
+cudaError_t launch_div(cp4d_ctx *c, const float *p, float *f);
+cudaError_t launch_prox_f2(cp4d_ctx *c, float sigma, const float *ft, float *h2);
+cudaError_t launch_update(cp4d_ctx *c, float tau, const float *bp, const float *h2, float *f, float *ft);
+cudaError_t launch_fold(cp4d_ctx *c, const float *g, float4 *gt);
+// synth: out = K1 f from partial sums P.  mode 0: g_out = v ; mode 1: h1 = (h1 + sigma (v - g))/(1+sigma)
+cudaError_t launch_synth(cp4d_ctx *c, const float4 *P, int mode, float sigma, const float *g, float *out);
+cudaError_t launch_forward_partial(cp4d_ctx *c, const float *f, float4 *P);
+cudaError_t launch_backproject(cp4d_ctx *c, const float4 *gt, float *f_out);
+cudaError_t launch_sumsq_dot(cp4d_ctx *c, const float *x, const float *y, uint64_t n, double *slot);
+cudaError_t launch_fill_normal(cp4d_ctx *c, float *x, uint64_t n, uint64_t seed);
+// x = (a - b) * scale   (b nullable)
+cudaError_t launch_scale_diff(cp4d_ctx *c, float *x, const float *a, const float *b, float scale, uint64_t n);
+
+}  // namespace cp4d

@@ -1,0 +1,328 @@
+// HBM-streaming kernels of the CP iteration (sm_100a): grad, div, the fused F2* prox (grad + projection,
+// Fig. 2 step 4), the fused primal update (div + steps 5-6), the pi-fold prologue of the adjoint, the
+// synthesis epilogue of the forward projector (optionally fused with the F1* prox, step 3), reductions.
+//
+// Layout f[z][iy][ix][j] (j fastest): one thread owns one float4 (4 consecutive coefficients j of one
+// voxel) and walks along z, so the z neighbour is carried in registers and every 4D element is read
+// from HBM once; x/y/t neighbours are served by L1/L2.  All global accesses are 16-byte, fully coalesced.
+#include "cp4d_internal.cuh"
+
+namespace cp4d {
+
+__device__ __forceinline__ float4 ld4(const float4 *p) { return __ldg(p); }
+__device__ __forceinline__ float4 sub4(float4 a, float4 b) { return make_float4(a.x - b.x, a.y - b.y, a.z - b.z, a.w - b.w); }
+
+struct StreamArgs {
+    int n, nz, Q, zper;
+    int64_t slice4, V4;
+    float lambda2;
+};
+
+// ---------------------------------------------------------------------------------------------------
+// grad (PROX=false):  p = K2 f.     prox (PROX=true): h2 <- proj_{|.|<=lambda1}(h2 + sigma K2 ft)
+// ---------------------------------------------------------------------------------------------------
+template <bool PROX>
+__global__ void __launch_bounds__(256) k_grad(const float *__restrict__ f, float *__restrict__ p, StreamArgs a,
+                                              float sigma, float inv_l1, int l1_zero) {
+    const int64_t e4 = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (e4 >= a.slice4) return;
+    const int c = (int)(e4 % a.Q);
+    const int64_t vox = e4 / a.Q;
+    const int x = (int)(vox % a.n), y = (int)(vox / a.n);
+    const int z0 = blockIdx.y * a.zper, z1 = min(a.nz, z0 + a.zper);
+    const float4 *F = reinterpret_cast<const float4 *>(f);
+    float4 *P = reinterpret_cast<float4 *>(p);
+    const bool hx = x + 1 < a.n, hy = y + 1 < a.n, ht = c + 1 < a.Q;
+    const int64_t sy = (int64_t)a.n * a.Q;
+    float4 cur = ld4(F + (int64_t)z0 * a.slice4 + e4);
+    for (int z = z0; z < z1; ++z) {
+        const int64_t idx = (int64_t)z * a.slice4 + e4;
+        const float4 fz = (z + 1 < a.nz) ? ld4(F + idx + a.slice4) : cur;
+        const float4 fx = hx ? ld4(F + idx + a.Q) : cur;
+        const float4 fy = hy ? ld4(F + idx + sy) : cur;
+        const float ft = ht ? __ldg(f + (idx + 1) * 4) : cur.w;
+        float4 gx = sub4(fx, cur), gy = sub4(fy, cur), gz = sub4(fz, cur);
+        float4 gt = make_float4(a.lambda2 * (cur.y - cur.x), a.lambda2 * (cur.z - cur.y), a.lambda2 * (cur.w - cur.z),
+                                a.lambda2 * (ft - cur.w));
+        if (PROX) {
+            float4 qx = P[idx], qy = P[idx + a.V4], qz = P[idx + 2 * a.V4], qt = P[idx + 3 * a.V4];
+#define CP4D_PROX1(C)                                                                             \
+    {                                                                                             \
+        float vx = fmaf(sigma, gx.C, qx.C), vy = fmaf(sigma, gy.C, qy.C), vz = fmaf(sigma, gz.C, qz.C), \
+              vt = fmaf(sigma, gt.C, qt.C);                                                       \
+        float nn = sqrtf(fmaf(vx, vx, fmaf(vy, vy, fmaf(vz, vz, vt * vt))));                      \
+        float r = l1_zero ? 0.0f : 1.0f / fmaxf(1.0f, nn * inv_l1);                               \
+        gx.C = vx * r; gy.C = vy * r; gz.C = vz * r; gt.C = vt * r;                               \
+    }
+            CP4D_PROX1(x) CP4D_PROX1(y) CP4D_PROX1(z) CP4D_PROX1(w)
+#undef CP4D_PROX1
+        }
+        P[idx] = gx;
+        P[idx + a.V4] = gy;
+        P[idx + 2 * a.V4] = gz;
+        P[idx + 3 * a.V4] = gt;
+        cur = fz;
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------
+// div (UPDATE=false): out = -K2^T p.
+// update (UPDATE=true): f+ = f - tau bp + tau div h2; ft = f+ + theta (f+ - f); f <- f+   (steps 5-6)
+// ---------------------------------------------------------------------------------------------------
+template <bool UPDATE>
+__global__ void __launch_bounds__(256) k_div(const float *__restrict__ p, float *__restrict__ out, StreamArgs a,
+                                             const float *__restrict__ bp, float *__restrict__ ft_out, float tau,
+                                             float theta) {
+    const int64_t e4 = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (e4 >= a.slice4) return;
+    const int c = (int)(e4 % a.Q);
+    const int64_t vox = e4 / a.Q;
+    const int x = (int)(vox % a.n), y = (int)(vox / a.n);
+    const int z0 = blockIdx.y * a.zper, z1 = min(a.nz, z0 + a.zper);
+    const float4 *PX = reinterpret_cast<const float4 *>(p);
+    const float4 *PY = PX + a.V4, *PZ = PX + 2 * a.V4, *PT = PX + 3 * a.V4;
+    const float *pt_s = p + 3 * a.V4 * 4;
+    const int64_t sy = (int64_t)a.n * a.Q;
+    const float4 zero = make_float4(0.f, 0.f, 0.f, 0.f);
+    float4 prevz = (z0 > 0) ? ld4(PZ + (int64_t)(z0 - 1) * a.slice4 + e4) : zero;
+    for (int z = z0; z < z1; ++z) {
+        const int64_t idx = (int64_t)z * a.slice4 + e4;
+        const float4 xc = (x < a.n - 1) ? ld4(PX + idx) : zero;
+        const float4 xm = (x > 0) ? ld4(PX + idx - a.Q) : zero;
+        const float4 yc = (y < a.n - 1) ? ld4(PY + idx) : zero;
+        const float4 ym = (y > 0) ? ld4(PY + idx - sy) : zero;
+        const float4 zc = (z < a.nz - 1) ? ld4(PZ + idx) : zero;
+        const float4 tc = ld4(PT + idx);
+        const float tm = (c > 0) ? __ldg(pt_s + idx * 4 - 1) : 0.0f;
+        const float tw = (c < a.Q - 1) ? tc.w : 0.0f;
+        float4 d;
+        d.x = (xc.x - xm.x) + (yc.x - ym.x) + (zc.x - prevz.x) + a.lambda2 * (tc.x - tm);
+        d.y = (xc.y - xm.y) + (yc.y - ym.y) + (zc.y - prevz.y) + a.lambda2 * (tc.y - tc.x);
+        d.z = (xc.z - xm.z) + (yc.z - ym.z) + (zc.z - prevz.z) + a.lambda2 * (tc.z - tc.y);
+        d.w = (xc.w - xm.w) + (yc.w - ym.w) + (zc.w - prevz.w) + a.lambda2 * (tw - tc.z);
+        if (UPDATE) {
+            float4 *F = reinterpret_cast<float4 *>(out);
+            const float4 fo = F[idx];
+            const float4 b = ld4(reinterpret_cast<const float4 *>(bp) + idx);
+            float4 fn, fr;
+            fn.x = fmaf(tau, d.x - b.x, fo.x); fn.y = fmaf(tau, d.y - b.y, fo.y);
+            fn.z = fmaf(tau, d.z - b.z, fo.z); fn.w = fmaf(tau, d.w - b.w, fo.w);
+            fr.x = fmaf(theta, fn.x - fo.x, fn.x); fr.y = fmaf(theta, fn.y - fo.y, fn.y);
+            fr.z = fmaf(theta, fn.z - fo.z, fn.z); fr.w = fmaf(theta, fn.w - fo.w, fn.w);
+            F[idx] = fn;
+            reinterpret_cast<float4 *>(ft_out)[idx] = fr;
+        } else {
+            reinterpret_cast<float4 *>(out)[idx] = d;
+        }
+        prevz = zc;
+    }
+}
+
+static StreamArgs make_args(const cp4d_ctx *c, dim3 &grid, dim3 &block) {
+    const Dims &d = c->d;
+    StreamArgs a;
+    a.n = d.n; a.nz = d.nz; a.Q = d.Q; a.slice4 = d.slice4; a.V4 = d.V / 4; a.lambda2 = c->lambda2;
+    block = dim3(256);
+    const int64_t bx = (d.slice4 + 255) / 256;
+    // enough CTAs to fill 148 SMs x 8 resident CTAs a few times over; otherwise split z
+    int zchunks = 1;
+    while (bx * zchunks < 148 * 16 && zchunks < d.nz) zchunks *= 2;
+    if (zchunks > d.nz) zchunks = d.nz;
+    a.zper = (d.nz + zchunks - 1) / zchunks;
+    grid = dim3((unsigned)bx, (unsigned)((d.nz + a.zper - 1) / a.zper));
+    return a;
+}
+
+cudaError_t launch_grad(cp4d_ctx *c, const float *f, float *p) {
+    dim3 g, b;
+    StreamArgs a = make_args(c, g, b);
+    k_grad<false><<<g, b, 0, c->stream>>>(f, p, a, 0.f, 0.f, 0);
+    c->launches++;
+    return cudaGetLastError();
+}
+cudaError_t launch_prox_f2(cp4d_ctx *c, float sigma, const float *ft, float *h2) {
+    dim3 g, b;
+    StreamArgs a = make_args(c, g, b);
+    const int l1z = !(c->lambda1 > 0.f);
+    k_grad<true><<<g, b, 0, c->stream>>>(ft, h2, a, sigma, l1z ? 0.f : 1.0f / c->lambda1, l1z);
+    c->launches++;
+    return cudaGetLastError();
+}
+cudaError_t launch_div(cp4d_ctx *c, const float *p, float *f) {
+    dim3 g, b;
+    StreamArgs a = make_args(c, g, b);
+    k_div<false><<<g, b, 0, c->stream>>>(p, f, a, nullptr, nullptr, 0.f, 0.f);
+    c->launches++;
+    return cudaGetLastError();
+}
+cudaError_t launch_update(cp4d_ctx *c, float tau, const float *bp, const float *h2, float *f, float *ft) {
+    dim3 g, b;
+    StreamArgs a = make_args(c, g, b);
+    k_div<true><<<g, b, 0, c->stream>>>(h2, f, a, bp, ft, tau, c->theta);
+    c->launches++;
+    return cudaGetLastError();
+}
+
+// ---------------------------------------------------------------------------------------------------
+// fold: gt[z][i][jc][b] (float4 over j) = sum_q Phi[j, q n0 + i] g[z][q n0 + i][flip_q b]
+// synth (PAPER.md:L198-L202 + Eq. 9): v[z][q n0+i][flip_q b] = sum_j Phi[j, q n0+i] P[z][i][.][b][j]
+// One CTA per (z, base angle i); the npi x m slice of Phi it needs sits in shared memory.
+// ---------------------------------------------------------------------------------------------------
+template <int Q>
+__global__ void __launch_bounds__(128) k_fold(const float *__restrict__ g, float4 *__restrict__ gt,
+                                              const float *__restrict__ phi, int nd, int na, int npi, int n0) {
+    extern __shared__ float phis[];  // [q][j]
+    const int z = blockIdx.x / n0, i = blockIdx.x % n0;
+    constexpr int m = 4 * Q;
+    for (int t = threadIdx.x; t < npi * m; t += blockDim.x) phis[t] = phi[(int64_t)(t % m) * na + (t / m) * n0 + i];
+    __syncthreads();
+    for (int b = threadIdx.x; b < nd; b += blockDim.x) {
+        float acc[m];
+#pragma unroll
+        for (int j = 0; j < m; ++j) acc[j] = 0.f;
+        for (int q = 0; q < npi; ++q) {
+            const int bb = (q & 1) ? nd - 1 - b : b;
+            const float gv = __ldg(g + ((int64_t)z * na + q * n0 + i) * nd + bb);
+#pragma unroll
+            for (int j = 0; j < m; ++j) acc[j] = fmaf(phis[q * m + j], gv, acc[j]);
+        }
+#pragma unroll
+        for (int jc = 0; jc < Q; ++jc)
+            gt[(((int64_t)z * n0 + i) * Q + jc) * nd + b] = make_float4(acc[4 * jc], acc[4 * jc + 1], acc[4 * jc + 2], acc[4 * jc + 3]);
+    }
+}
+
+template <int Q>
+__global__ void __launch_bounds__(128) k_synth(const float4 *__restrict__ P, int mode, float sigma,
+                                               const float *__restrict__ g, float *__restrict__ out,
+                                               const float *__restrict__ phi, int nd, int na, int npi, int n0) {
+    extern __shared__ float phis[];
+    const int z = blockIdx.x / n0, i = blockIdx.x % n0;
+    constexpr int m = 4 * Q;
+    for (int t = threadIdx.x; t < npi * m; t += blockDim.x) phis[t] = phi[(int64_t)(t % m) * na + (t / m) * n0 + i];
+    __syncthreads();
+    const float rs = 1.0f / (1.0f + sigma);
+    for (int b = threadIdx.x; b < nd; b += blockDim.x) {
+        float acc[m];
+#pragma unroll
+        for (int jc = 0; jc < Q; ++jc) {
+            const float4 v = P[(((int64_t)z * n0 + i) * Q + jc) * nd + b];
+            acc[4 * jc] = v.x; acc[4 * jc + 1] = v.y; acc[4 * jc + 2] = v.z; acc[4 * jc + 3] = v.w;
+        }
+        for (int q = 0; q < npi; ++q) {
+            const int bb = (q & 1) ? nd - 1 - b : b;
+            float v = 0.f;
+#pragma unroll
+            for (int j = 0; j < m; ++j) v = fmaf(phis[q * m + j], acc[j], v);
+            const int64_t idx = ((int64_t)z * na + q * n0 + i) * nd + bb;
+            if (mode == 0) out[idx] = v;
+            else out[idx] = (out[idx] + sigma * (v - __ldg(g + idx))) * rs;
+        }
+    }
+}
+
+#define CP4D_DISPATCH_Q(Qv, CALL)                          \
+    switch (Qv) {                                          \
+    case 1: { constexpr int QQ = 1; CALL; } break;         \
+    case 2: { constexpr int QQ = 2; CALL; } break;         \
+    case 3: { constexpr int QQ = 3; CALL; } break;         \
+    case 4: { constexpr int QQ = 4; CALL; } break;         \
+    case 5: { constexpr int QQ = 5; CALL; } break;         \
+    case 6: { constexpr int QQ = 6; CALL; } break;         \
+    case 7: { constexpr int QQ = 7; CALL; } break;         \
+    default: { constexpr int QQ = 8; CALL; } break;        \
+    }
+
+cudaError_t launch_fold(cp4d_ctx *c, const float *g, float4 *gt) {
+    const Dims &d = c->d;
+    const size_t sh = (size_t)d.npi * d.m * sizeof(float);
+    CP4D_DISPATCH_Q(d.Q, (k_fold<QQ><<<d.nz * d.n0, 128, sh, c->stream>>>(g, gt, c->phi, d.nd, d.na, d.npi, d.n0)));
+    c->launches++;
+    return cudaGetLastError();
+}
+cudaError_t launch_synth(cp4d_ctx *c, const float4 *P, int mode, float sigma, const float *g, float *out) {
+    const Dims &d = c->d;
+    const size_t sh = (size_t)d.npi * d.m * sizeof(float);
+    CP4D_DISPATCH_Q(d.Q, (k_synth<QQ><<<d.nz * d.n0, 128, sh, c->stream>>>(P, mode, sigma, g, out, c->phi, d.nd, d.na, d.npi, d.n0)));
+    c->launches++;
+    return cudaGetLastError();
+}
+
+// ---------------------------------------------------------------------------------------------------
+// reductions and vector helpers (power iteration, dot test)
+// ---------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) k_dot(const float *__restrict__ x, const float *__restrict__ y, uint64_t n,
+                                             double *slot) {
+    double acc = 0.0;
+    const uint64_t n4 = n / 4, stride = (uint64_t)gridDim.x * blockDim.x;
+    const float4 *X = reinterpret_cast<const float4 *>(x), *Y = reinterpret_cast<const float4 *>(y);
+    for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n4; i += stride) {
+        const float4 a = ld4(X + i), b = ld4(Y + i);
+        acc += (double)a.x * b.x + (double)a.y * b.y + (double)a.z * b.z + (double)a.w * b.w;
+    }
+    if (blockIdx.x == 0 && threadIdx.x < (n & 3)) acc += (double)x[n4 * 4 + threadIdx.x] * y[n4 * 4 + threadIdx.x];
+    for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+    __shared__ double part[8];
+    if ((threadIdx.x & 31) == 0) part[threadIdx.x >> 5] = acc;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double s = 0.0;
+        for (int w = 0; w < 8; ++w) s += part[w];
+        atomicAdd(slot, s);
+    }
+}
+
+cudaError_t launch_sumsq_dot(cp4d_ctx *c, const float *x, const float *y, uint64_t n, double *slot) {
+    cudaError_t e = cudaMemsetAsync(slot, 0, sizeof(double), c->stream);
+    if (e != cudaSuccess) return e;
+    uint64_t blocks = (n / 4 + 255) / 256;
+    if (blocks > 148 * 8) blocks = 148 * 8;
+    if (blocks < 1) blocks = 1;
+    k_dot<<<(unsigned)blocks, 256, 0, c->stream>>>(x, y, n, slot);
+    c->launches += 2;
+    return cudaGetLastError();
+}
+
+__device__ __forceinline__ uint64_t splitmix(uint64_t x) {
+    x += 0x9E3779B97F4A7C15ull;
+    x = (x ^ (x >> 30)) * 0xBF58476D1CE4E5B9ull;
+    x = (x ^ (x >> 27)) * 0x94D049BB133111EBull;
+    return x ^ (x >> 31);
+}
+__global__ void __launch_bounds__(256) k_fill_normal(float *x, uint64_t n, uint64_t seed) {
+    const uint64_t stride = (uint64_t)gridDim.x * blockDim.x;
+    for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
+        const uint64_t h = splitmix(seed * 0xD1342543DE82EF95ull + i);
+        const float u1 = ((uint32_t)(h >> 40) + 1.0f) * (1.0f / 16777217.0f);  // (0,1]
+        const float u2 = (uint32_t)(h & 0xFFFFFFu) * (1.0f / 16777216.0f);
+        x[i] = sqrtf(-2.0f * logf(u1)) * cospif(2.0f * u2);
+    }
+}
+cudaError_t launch_fill_normal(cp4d_ctx *c, float *x, uint64_t n, uint64_t seed) {
+    uint64_t blocks = (n + 255) / 256;
+    if (blocks > 148 * 8) blocks = 148 * 8;
+    k_fill_normal<<<(unsigned)blocks, 256, 0, c->stream>>>(x, n, seed);
+    c->launches++;
+    return cudaGetLastError();
+}
+
+__global__ void __launch_bounds__(256) k_scale_diff(float *x, const float *a, const float *b,
+                                                    float s, uint64_t n4) {
+    const uint64_t stride = (uint64_t)gridDim.x * blockDim.x;
+    float4 *X = reinterpret_cast<float4 *>(x);
+    const float4 *A = reinterpret_cast<const float4 *>(a), *B = reinterpret_cast<const float4 *>(b);
+    for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n4; i += stride) {
+        float4 v = A[i];
+        if (B) { const float4 w = B[i]; v = sub4(v, w); }
+        X[i] = make_float4(v.x * s, v.y * s, v.z * s, v.w * s);
+    }
+}
+cudaError_t launch_scale_diff(cp4d_ctx *c, float *x, const float *a, const float *b, float s, uint64_t n) {
+    uint64_t blocks = (n / 4 + 255) / 256;
+    if (blocks > 148 * 8) blocks = 148 * 8;
+    k_scale_diff<<<(unsigned)blocks, 256, 0, c->stream>>>(x, a, b, s, n / 4);  // V is a multiple of 4
+    c->launches++;
+    return cudaGetLastError();
+}
+
+}  // namespace cp4d

@@ -1,0 +1,75 @@
+"""C-ABI boundary checks that need no GPU: the library loads, exports every symbol include/cp4d.h declares,
+validates arguments on the host, and refuses to create a context without an sm_100 device (no CPU fallback)."""
+import ctypes as C
+import re
+from pathlib import Path
+
+import numpy as np
+import pytest
+
+ROOT = Path(__file__).resolve().parents[1]
+
+
+@pytest.fixture(scope="module")
+def L():
+    from paper_1809_09725_b200 import build, binding
+    build.build_lib()
+    return binding.lib()
+
+
+def declared_symbols():
+    hdr = (ROOT / "include" / "cp4d.h").read_text()
+    hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
+    return sorted(set(re.findall(r"\b(cp4d_[a-z0-9_]+)\s*\(", hdr)))
+
+
+def test_exports_every_declared_symbol(L):
+    syms = declared_symbols()
+    assert {"cp4d_create", "cp4d_forward", "cp4d_adjoint", "cp4d_grad", "cp4d_div", "cp4d_iterate", "cp4d_norm"} <= set(syms)
+    for s in syms:
+        assert hasattr(L, s), f"libcp4d.so does not export {s}"
+
+
+def test_workspace_bytes_counts_state(L):
+    from paper_1809_09725_b200 import binding, synth
+    for cfg in (1, 2, 3, 4, 5):
+        c = synth.CONFIGS[cfg]
+        nb = binding.workspace_bytes(c.n, c.nz, c.nd, c.n_angles, c.n_half_rot, c.m)
+        state = (7 * c.V + 2 * c.S) * 4                       # f, ft, K1^T h1, h2[4], h1, g
+        scratch = c.nz * c.n_theta0 * c.nd * c.m * 4
+        assert state + scratch <= nb <= state + scratch + (64 << 20)
+    c = synth.CONFIGS[5]
+    assert binding.workspace_bytes(c.n, c.nz, c.nd, c.n_angles, c.n_half_rot, c.m) < 170e9   # fits 180 GB HBM
+
+
+@pytest.mark.parametrize("bad", [dict(ny=31), dict(m=6), dict(m=36), dict(n_half_rot=3), dict(nd=1), dict(nz=0), dict(lambda1=-1.0)])
+def test_host_validation(L, bad):
+    from paper_1809_09725_b200 import binding
+    kw = dict(n=32, nz=1, nd=32, n_angles=128, n_half_rot=4, m=4)
+    kw.update(bad)
+    p = binding.make_params(**kw)
+    out = C.c_uint64(0)
+    assert L.cp4d_workspace_bytes(C.byref(p), C.byref(out)) == binding.EINVAL
+
+
+def test_create_needs_workspace_and_device(L):
+    from paper_1809_09725_b200 import binding
+    import torch
+    phi = np.ones((4, 128), dtype=np.float32)
+    p = binding.make_params(32, 1, 32, 128, 4, 4, phi)
+    h = C.c_void_p()
+    assert L.cp4d_create(C.byref(p), C.byref(h)) == binding.EWORKSPACE
+    if not torch.cuda.is_available():
+        p = binding.make_params(32, 1, 32, 128, 4, 4, phi, workspace_ptr=4096, workspace_bytes=1 << 30)
+        assert L.cp4d_create(C.byref(p), C.byref(h)) == binding.EUNSUPPORTED      # fails loudly: no CPU fallback
+        assert h.value is None
+    assert L.cp4d_forward(None, None, None) == binding.EINVAL
+    assert L.cp4d_strerror(binding.EUNSUPPORTED).decode().startswith("no sm_100")
+
+
+def test_product_does_not_import_oracle():
+    """The product path must not route through the oracle (it is test infrastructure)."""
+    for p in list((ROOT / "paper_1809_09725_b200").rglob("*.py")) + list((ROOT / "paper_1809_09725_b200" / "csrc").glob("*.cu*")):
+        txt = p.read_text()
+        assert not re.search(r"^\s*(from|import)\s+oracle|libcp4d_ref|cp4d_ref_|oracle[./]ref", txt, flags=re.M), \
+            f"{p} reaches into the oracle"

@@ -1,0 +1,180 @@
+"""Parity of the CUDA path (through the C ABI, via the ctypes binding) against the fp64 oracle, element by element
+on the same seeded inputs.  Tolerances are BASELINE.json north_star's: relative L2 error <= 1e-4 per operator (fp32)
+and <= 1e-3 on f after the CP iterations."""
+import numpy as np
+import pytest
+
+from paper_1809_09725_b200 import synth
+
+pytestmark = pytest.mark.gpu
+
+TOL_OP = 1e-4
+TOL_CP = 1e-3
+
+
+def rel(a, b):
+    a = np.asarray(a, dtype=np.float64)
+    return float(np.linalg.norm(a - b) / max(np.linalg.norm(b), 1e-300))
+
+
+@pytest.fixture(scope="module")
+def torch_cuda():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    from paper_1809_09725_b200 import build
+    build.build_lib()
+    return torch
+
+
+@pytest.fixture(scope="module")
+def fast_oracle(oracle):
+    oracle.set_threads(oracle.max_threads())
+    yield oracle
+    oracle.set_threads(1)
+
+
+def dev(torch, a):
+    return torch.as_tensor(np.ascontiguousarray(a, dtype=np.float32), device="cuda")
+
+
+# shapes: the two configs the oracle runs in full + ragged / odd cases spanning several tiles and a ragged tail
+CASES = {
+    "cfg1": synth.CONFIGS[1],
+    "cfg2": synth.CONFIGS[2],
+    "ragged": synth.CONFIGS[2].scaled(cfg=12, n=45, nd=50, nz=3, n_angles=35, n_half_rot=5, m=12, lambda2=0.7),
+    "wide_det": synth.CONFIGS[4].scaled(cfg=14, n=40, nd=75, nz=2, n_angles=36, n_half_rot=3, m=8),
+    "narrow_det_m32": synth.CONFIGS[2].scaled(cfg=15, n=70, nd=33, nz=1, n_angles=24, n_half_rot=2, m=32),
+    "one_angle_per_pi": synth.CONFIGS[1].scaled(cfg=16, n=33, nd=33, nz=2, n_angles=6, n_half_rot=6, m=4),
+}
+
+
+def make(case, fast_oracle):
+    from paper_1809_09725_b200 import binding
+    c = CASES[case]
+    phi = synth.basis_table(c.basis, c.m, c.n_angles)
+    P = fast_oracle.Problem.from_config(c, phi=phi)
+    ctx = binding.Context.from_config(c, phi=phi)
+    return c, P, ctx
+
+
+@pytest.mark.parametrize("case", list(CASES))
+def test_forward_adjoint(torch_cuda, fast_oracle, case):
+    c, P, ctx = make(case, fast_oracle)
+    f, g = synth.test_vectors(c)
+    f32, g32 = f.astype(np.float32), g.astype(np.float32)
+    Kf = ctx.forward(dev(torch_cuda, f32)).cpu().numpy()
+    Ktg = ctx.adjoint(dev(torch_cuda, g32)).cpu().numpy()
+    assert rel(Kf, P.forward(f32.astype(np.float64), folded=True)) <= TOL_OP
+    assert rel(Ktg, P.adjoint(g32.astype(np.float64), folded=True)) <= TOL_OP
+    # GPU-side adjoint identity in fp32 (fp64-accumulated dots)
+    lhs = ctx.dot(dev(torch_cuda, Kf), dev(torch_cuda, g32))
+    rhs = ctx.dot(dev(torch_cuda, f32), dev(torch_cuda, Ktg))
+    assert abs(lhs - rhs) <= 1e-5 * np.linalg.norm(Kf) * np.linalg.norm(g32)
+    ctx.close()
+
+
+@pytest.mark.parametrize("case", list(CASES))
+def test_grad_div(torch_cuda, fast_oracle, case):
+    c, P, ctx = make(case, fast_oracle)
+    f = synth.test_vectors(c)[0].astype(np.float32)
+    p = synth.rng(c.cfg, 5).standard_normal((4,) + P.primal_shape).astype(np.float32)
+    gp = ctx.grad(dev(torch_cuda, f)).cpu().numpy()
+    dp = ctx.div(dev(torch_cuda, p)).cpu().numpy()
+    ref_g, ref_d = P.grad(f.astype(np.float64)), P.div(p.astype(np.float64))
+    assert rel(gp, ref_g) <= 1e-6 and rel(dp, ref_d) <= 1e-6
+    assert np.array_equal(gp == 0, ref_g == 0) or rel(gp, ref_g) <= 1e-7      # boundary zeros in the same places
+    ctx.close()
+
+
+@pytest.mark.parametrize("case", ["cfg1", "ragged", "narrow_det_m32"])
+def test_fused_steps(torch_cuda, fast_oracle, case):
+    c, P, ctx = make(case, fast_oracle)
+    r = synth.rng(c.cfg, 6)
+    ft = r.standard_normal(P.primal_shape).astype(np.float32)
+    f = r.standard_normal(P.primal_shape).astype(np.float32)
+    g = r.standard_normal(P.sino_shape).astype(np.float32)
+    h1 = r.standard_normal(P.sino_shape).astype(np.float32)
+    h2 = r.standard_normal((4,) + P.primal_shape).astype(np.float32)
+    sigma, tau = 0.013, 0.021
+    d = lambda a: a.astype(np.float64)
+    # step 3
+    out = ctx.prox_f1(sigma, dev(torch_cuda, ft), dev(torch_cuda, g), dev(torch_cuda, h1)).cpu().numpy()
+    assert rel(out, P.prox_f1(d(h1), P.forward(d(ft), folded=True), d(g), sigma)) <= TOL_OP
+    # step 4, lambda1 chosen so both branches of max(1, .) occur
+    q = d(h2) + sigma * P.grad(d(ft))
+    lam = float(np.median(np.sqrt((q ** 2).sum(0))))
+    ctx2 = type(ctx).from_config(c.scaled(lambda1=lam))
+    ref, ncl = P.prox_f2(d(h2), P.grad(d(ft)), sigma, lambda1=float(np.float32(lam)))
+    assert 0.3 < ncl / (P.V) < 0.7
+    out = ctx2.prox_f2(sigma, dev(torch_cuda, ft), dev(torch_cuda, h2)).cpu().numpy()
+    assert rel(out, ref) <= 1e-6
+    assert np.sqrt((out.astype(np.float64) ** 2).sum(0)).max() <= lam * (1 + 1e-5)
+    # lambda1 = 0: h2 = 0
+    ctx0 = type(ctx).from_config(c.scaled(lambda1=0.0))
+    assert float(ctx0.prox_f2(sigma, dev(torch_cuda, ft), dev(torch_cuda, h2)).abs().max()) == 0.0
+    # steps 5-6
+    fo, fto = ctx.primal_update(tau, dev(torch_cuda, h1), dev(torch_cuda, h2), dev(torch_cuda, f), ctx.empty_primal())
+    fn = d(f) - tau * P.adjoint(d(h1), folded=True) + tau * P.div(d(h2))
+    assert rel(fo.cpu().numpy(), fn) <= TOL_OP
+    assert rel(fto.cpu().numpy(), fn + 1.0 * (fn - d(f))) <= TOL_OP
+    for x in (ctx, ctx2, ctx0):
+        x.close()
+
+
+def _data(c):
+    return synth.sinogram(c).numpy()
+
+
+@pytest.mark.parametrize("case,lam1", [("cfg1", 1e-3), ("cfg1", "mixed"), ("cfg2", 1e-3), ("cfg2", "mixed"), ("ragged", "mixed")])
+def test_cp_iterations(torch_cuda, fast_oracle, case, lam1):
+    """Full CP run (config iteration counts) from zero state with the oracle's tau = sigma = 0.95/L."""
+    c = CASES[case]
+    g = _data(c).astype(np.float32)
+    if lam1 == "mixed":      # lambda1 for which a good fraction of voxels is clamped AND a good fraction is not (C18)
+        lam1 = {"cfg1": 0.6, "cfg2": 0.25, "ragged": 0.15}[case]
+    c = c.scaled(lambda1=float(np.float32(lam1)))
+    from paper_1809_09725_b200 import binding
+    phi = synth.basis_table(c.basis, c.m, c.n_angles)
+    P = fast_oracle.Problem.from_config(c, phi=phi)
+    ctx = binding.Context.from_config(c, phi=phi)
+    L, _ = P.power(synth.rng(c.cfg, 3).standard_normal(P.primal_shape), 30, folded=True)
+    ts = float(np.float32(0.95 / L))
+    st = P.zero_state()
+    ncl = P.cp(g.astype(np.float64), st, ts, ts, c.iters, folded=True)
+    ctx.set_data(dev(torch_cuda, g))
+    ctx.set_steps(ts, ts)
+    ctx.reset()
+    ctx.iterate(c.iters)
+    ctx.sync()
+    s = ctx.state()
+    frac = ncl / P.V
+    print(f"{case} lambda1={lam1} clamped fraction at last iteration: {frac:.3f}")
+    if lam1 != 1e-3:
+        assert 0.05 < frac < 0.95
+    assert rel(s["f"].cpu().numpy(), st["f"]) <= TOL_CP
+    assert rel(s["h1"].cpu().numpy(), st["h1"]) <= TOL_CP
+    assert rel(ctx.get_f().cpu().numpy(), st["f"]) <= TOL_CP
+    ctx.close()
+
+
+@pytest.mark.parametrize("case", ["cfg1", "cfg2"])
+def test_power_iteration(torch_cuda, fast_oracle, case):
+    c, P, ctx = make(case, fast_oracle)
+    L_ref, _ = P.power(synth.rng(c.cfg, 3).standard_normal(P.primal_shape), 30, folded=True)
+    L = ctx.norm(30, seed=7)
+    assert abs(L - L_ref) <= 1e-4 * L_ref
+    ctx.close()
+
+
+def test_solve_host_equals_device_path(torch_cuda, fast_oracle):
+    c, P, ctx = make("cfg1", fast_oracle)
+    g = _data(c).astype(np.float32)
+    ctx.set_steps(0.015, 0.015)
+    ctx.set_data(dev(torch_cuda, g)); ctx.reset(); ctx.iterate(5)
+    a = ctx.get_f().cpu()
+    gh = torch_cuda.as_tensor(g).pin_memory()
+    fh = torch_cuda.empty(P.primal_shape, dtype=torch_cuda.float32).pin_memory()
+    ctx.solve_host(gh, 5, fh)
+    assert rel(fh.numpy(), a.numpy().astype(np.float64)) <= 1e-5       # atomics: summation order may differ
+    assert ctx.launch_count() > 0
+    ctx.close()
