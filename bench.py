@@ -1,0 +1,390 @@
+#!/usr/bin/env python
+"""bench.py -- one JSON line per run: CP iterations/s of the cp4d hot path on B200 (BASELINE.json metric).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config C] [--impl cp4d|reference]
+
+A "step" is ONE Chambolle-Pock iteration (Fig. 2: forward + F1* prox, grad + F2* prox,
+adjoint, div + primal update + over-relaxation) over the whole 4D problem of `--config` (BASELINE.json configs,
+numbered 1..5 as in SURVEY.md 8).  Inputs are seeded and synthetic (paper_1809_09725_b200/synth.py; DESIGN.md
+"Input recipe"); the iteration's cost does not depend on the values.
+
+  value    : iterations/s, state resident in HBM, K iterations enqueued by cp4d_iterate, CUDA events on the
+             context's stream, barrier + synchronize on both sides, max over ranks.
+  e2e      : the same metric through cp4d_solve_host(g_host, K, f_host): pinned HOST buffers, H2D of the
+             sinogram, reset, K iterations, D2H of f, all inside the timed region.
+  roofline : the dominant kernel of the step (largest share of device time in the timed region), timed live
+             by the library's per-kernel CUDA events (cp4d_profile_begin/end) during a second pass of K steps.
+  kernels  : the same for every kernel class, plus nominal voxel*angle*basis GUPS of forward and adjoint.
+  cpu_baseline : the fp64 oracle (oracle/cp4d_ref.c, as it stands) on this box's host cores, on a bounded
+             sample (a few full in-plane slices), extrapolated to the whole problem.
+
+N > 1: the path does not shard (north_star: one GPU); `--gpus N` runs N independent replicas, one per rank,
+no data-path collective ("replicas only").  `--impl reference` times the oracle only.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+from pathlib import Path
+
+import numpy as np
+
+ROOT = Path(__file__).resolve().parent
+if str(ROOT) not in sys.path:
+    sys.path.insert(0, str(ROOT))
+
+METRIC = "cp_iterations_per_s"
+UNIT = "it/s"
+N_SM, LANES = 148, 128
+
+
+def load_peaks():
+    """Roofline denominators: MEASURED_PEAKS.json (driver-written) else the profiling guide's fallback."""
+    p = ROOT / "MEASURED_PEAKS.json"
+    if p.exists():
+        d = json.loads(p.read_text())
+        return dict(hbm_gbs=float(d["hbm_gbs"]), sm_max_mhz=float(d.get("sm_max_mhz", 1965.0)), source="measured")
+    return dict(hbm_gbs=6650.0, sm_max_mhz=1965.0, source="fallback")
+
+
+def alu_peak_tflops(sm_mhz: float) -> float:
+    """Plain FP32 FMA pipe: 148 SMs x 128 lanes x 2 flop x clock."""
+    return N_SM * LANES * 2 * sm_mhz * 1e6 / 1e12
+
+
+# ------------------------------------------------------------------------------------------------------
+# algorithmic work per launch of each kernel class (bytes or flops per unit x units)
+# ------------------------------------------------------------------------------------------------------
+def algorithmic_work(c):
+    V, S = c.V, c.S
+    n0 = c.n_theta0
+    ray_fma = 2 * c.m * c.n * c.n * c.nz * n0            # 2 taps x m per voxel-step per base-angle ray
+    syn_fma = c.m * c.n_angles * c.nd * c.nz             # m-wide synthesis / analysis per sinogram sample
+    gt = c.nz * n0 * c.nd * c.m                          # folded sinogram / partial ray sums, elements
+    return {
+        # name: (bound, work per launch [flop or byte])
+        "forward": ("alu", 2.0 * ray_fma),
+        "backproject": ("alu", 2.0 * ray_fma),
+        "synth": ("hbm", 4.0 * (gt + 3 * S)),            # read P, read h1 + g, write h1 (prox fused)
+        "fold": ("hbm", 4.0 * (S + gt)),
+        "grad": ("hbm", 4.0 * 5 * V),
+        "div": ("hbm", 4.0 * 5 * V),
+        "prox_f2": ("hbm", 4.0 * 9 * V),                 # read ft + h2[4], write h2[4]
+        "update": ("hbm", 4.0 * 8 * V),                  # read h2[4] + f + K1^T h1, write f + ft
+    }
+
+
+class ClockSampler:
+    """nvidia-smi clocks + throttle reasons every 200 ms during the timed region (B200_PROFILING.md recipe)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, uuid: str | None):
+        self.rows, self.proc = [], None
+        cmd = ["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "200"]
+        if uuid:
+            cmd += ["-i", uuid]
+        try:
+            self.proc = subprocess.Popen(cmd, stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.th = threading.Thread(target=self._read, daemon=True)
+            self.th.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append((time.perf_counter(), [x.strip() for x in line.split(",")]))
+
+    def mark(self):
+        return time.perf_counter()
+
+    def stop(self, t0: float, t1: float) -> dict:
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.25)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        rows = [r for t, r in self.rows if t0 <= t <= t1 + 0.2] or [r for _, r in self.rows]
+        sm, mx, pw, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in rows:
+            try:
+                sm.append(float(r[0])); mx.append(float(r[1])); pw.append(float(r[2]))
+            except (ValueError, IndexError):
+                continue
+            for nm, v in zip(names, r[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+# ------------------------------------------------------------------------------------------------------
+# CPU baseline / reference arm: the fp64 oracle as it stands, on a bounded sample of the same workload
+# ------------------------------------------------------------------------------------------------------
+def oracle_sample_config(c, target_fma: float = 4e10):
+    """A sub-problem with the full in-plane size, angles and basis but only nz_s of the nz slices.
+    K1/K1^T and the proxes are independent per slice and the stencils cost the same per element, so one CP
+    iteration of the sub-problem x (nz/nz_s) is one CP iteration of the workload."""
+    per_slice = 4.0 * c.m * c.n * c.n * c.n_theta0          # forward + adjoint FMA of one slice, folded
+    nz_s = int(max(1, min(c.nz, round(target_fma / per_slice))))
+    return c.scaled(nz=nz_s), c.nz / nz_s
+
+
+def oracle_steps(c, steps: int, warmup: int, target_fma: float = 4e10):
+    """Times `steps` oracle CP iterations (all host cores, pi-folded operators -- bitwise equal to 1 thread)
+    on the sample; returns (it/s extrapolated to the workload, cores, sample text, seconds per sample step)."""
+    from oracle import ref
+    from paper_1809_09725_b200 import synth
+    ref.build()
+    cores = ref.max_threads()
+    ref.set_threads(cores)
+    cs, scale = oracle_sample_config(c, target_fma)
+    phi = synth.basis_table(cs.basis, cs.m, cs.n_angles)
+    P = ref.Problem.from_config(cs, phi=phi)
+    r = synth.rng(c.cfg, 1)
+    g = r.standard_normal(P.sino_shape)                      # cost does not depend on the values
+    st = P.zero_state()
+    st["ft"][:] = r.standard_normal(P.primal_shape)
+    ts = 0.01
+    for _ in range(warmup):
+        P.cp(g, st, ts, ts, 1, folded=True)
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        P.cp(g, st, ts, ts, 1, folded=True)
+    dt = (time.perf_counter() - t0) / max(steps, 1)
+    ref.set_threads(1)
+    sample = (f"{steps} oracle CP iteration(s) (fp64, pi-folded, OpenMP over outputs) on {cs.nz} of {c.nz} slices at full "
+              f"in-plane size {c.n}x{c.n}, {c.n_angles} angles, m={c.m}; x{scale:g} slices")
+    return 1.0 / (dt * scale), cores, sample, dt
+
+
+def run_reference(args, c, rank):
+    """--impl reference: the oracle on the host cores (rank 0 only), same metric/config as our arm."""
+    if rank != 0:
+        return
+    from paper_1809_09725_b200 import synth
+    val, cores, sample, dt = oracle_steps(c, args.steps, args.warmup, target_fma=1.5e10)
+    line = {
+        "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": 1e3 / val, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": synth.describe(c), "note": "fp64 CPU oracle (oracle/cp4d_ref.c), extrapolated from a slice sample"},
+        "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample,
+                         "sample_step_s": dt},
+        "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+# ------------------------------------------------------------------------------------------------------
+# our arm
+# ------------------------------------------------------------------------------------------------------
+def run_cp4d(args, c, rank, world):
+    import torch
+    import torch.distributed as dist
+    from paper_1809_09725_b200 import binding, build, synth
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device -- the cp4d hot path has no CPU fallback")
+    local = int(os.environ.get("LOCAL_RANK", rank))
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    if rank == 0:
+        build.build_lib()
+    if world > 1:
+        dist.barrier()
+    peaks = load_peaks()
+    K, W = args.steps, max(args.warmup, 0)
+
+    # ---- problem, data, step sizes (outside the timed region: SURVEY 8(d)) ----
+    phi = synth.basis_table(c.basis, c.m, c.n_angles)
+    ctx = binding.Context.from_config(c, phi=phi, device=local)
+    g = synth.sinogram(c, device=str(dev)).to(torch.float32).contiguous()
+    L = ctx.norm(args.power_iters, seed=3)
+    ts = 0.95 / L
+    ctx.set_steps(ts, ts)
+    ctx.set_data(g)
+    ctx.reset()
+    launches0 = ctx.launch_count()
+
+    def barrier():
+        torch.cuda.synchronize(dev)
+        if world > 1:
+            dist.barrier()
+            torch.cuda.synchronize(dev)
+
+    # ---- value: K iterations, state resident in HBM ----
+    ctx.iterate(W)
+    uuid = None
+    try:
+        uuid = "GPU-" + str(torch.cuda.get_device_properties(dev).uuid).replace("GPU-", "")
+    except Exception:
+        pass
+    sampler = ClockSampler(uuid)
+    barrier()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    l0 = ctx.launch_count()
+    t0 = sampler.mark()
+    e0.record(ctx.stream)
+    ctx.iterate(K)
+    e1.record(ctx.stream)
+    barrier()
+    t1 = sampler.mark()
+    launches = ctx.launch_count() - l0
+    ms = e0.elapsed_time(e1)
+
+    # ---- roofline: second pass of K steps with the library's per-kernel CUDA events on the same stream ----
+    ctx.profile_begin()
+    ctx.iterate(K)
+    prof = ctx.profile_end()
+    clocks = sampler.stop(t0, time.perf_counter())
+    if world > 1:
+        t = torch.tensor([ms], device=dev, dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+
+    # ---- standalone operators (grad/div are not launched by the fused iteration) ----
+    f_t, g_t = ctx.empty_primal().normal_(), ctx.empty_sino().normal_()
+    p_t = ctx.empty_dual()
+    ctx.profile_begin()
+    for _ in range(3):
+        ctx.grad(f_t, out=p_t)
+        ctx.div(p_t, out=f_t)
+    prof_gd = ctx.profile_end()
+    del p_t
+    ops = {}
+    for name, fn in (("forward_op", lambda: ctx.forward(f_t, out=g_t)), ("adjoint_op", lambda: ctx.adjoint(g_t, out=f_t))):
+        fn()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        tt = []
+        for _ in range(3):
+            a.record(ctx.stream); fn(); b.record(ctx.stream); b.synchronize()
+            tt.append(a.elapsed_time(b))
+        ops[name] = float(np.median(tt))
+    del f_t, g_t
+
+    # ---- e2e: cp4d_solve_host with pinned HOST buffers, copies inside the timed region ----
+    e2e = None
+    if not args.no_e2e:
+        g_host = g.cpu().pin_memory()
+        f_host = torch.empty(ctx.primal_shape, dtype=torch.float32).pin_memory()
+        ctx.solve_host(g_host, 1, f_host)                 # warm the copy paths
+        barrier()
+        w0 = time.perf_counter()
+        ctx.solve_host(g_host, K, f_host)                 # syncs before returning
+        w1 = time.perf_counter()
+        dt = w1 - w0
+        if world > 1:
+            t = torch.tensor([dt], device=dev, dtype=torch.float64)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            dt = float(t.item())
+        e2e = {"value": world * K / dt, "unit": UNIT, "h2d_bytes_per_step": c.S * 4 / K, "d2h_bytes_per_step": c.V * 4 / K,
+               "call": f"cp4d_solve_host(g_host, {K}, f_host): H2D {c.S * 4} B + reset + {K} iterations + D2H {c.V * 4} B, pinned host memory",
+               "seconds": dt}
+        del g_host, f_host
+    return ctx, dict(ms=ms, launches=launches, prof=prof, prof_gd=prof_gd, ops=ops, e2e=e2e, clocks=clocks, peaks=peaks,
+                     L=L, launches_total=ctx.launch_count() - launches0)
+
+
+def assemble(args, c, world, r):
+    from paper_1809_09725_b200 import synth
+    peaks, K = r["peaks"], args.steps
+    work = algorithmic_work(c)
+    alu_peak = alu_peak_tflops(peaks["sm_max_mhz"])
+    kernels, total_ms = {}, 0.0
+    merged = dict(r["prof"])
+    merged.update({k: v for k, v in r["prof_gd"].items() if k in ("grad", "div")})
+    for name, (ms_sum, n) in merged.items():
+        if name not in work or not n:
+            continue
+        bound, w = work[name]
+        avg = ms_sum / n
+        if bound == "alu":
+            ach, peak, unit = w / (avg * 1e-3) / 1e12, alu_peak, "TFLOP/s"
+        else:
+            ach, peak, unit = w / (avg * 1e-3) / 1e9, peaks["hbm_gbs"], "GB/s"
+        kernels[name] = {"bound": bound, "achieved": ach, "peak": peak, "unit": unit, "frac": ach / peak, "ms": avg,
+                         "launches": n, "in_step": name in r["prof"]}
+        if name in r["prof"]:
+            total_ms += ms_sum
+    for name, k in kernels.items():
+        k["share_of_step"] = (k["ms"] * k["launches"] / total_ms) if (k["in_step"] and total_ms) else None
+    dom = max((n for n in kernels if kernels[n]["in_step"]), key=lambda n: kernels[n]["ms"] * kernels[n]["launches"])
+    d = kernels[dom]
+    roofline = {"kernel": dom, "bound": d["bound"], "achieved": d["achieved"], "peak": d["peak"], "unit": d["unit"],
+                "frac": d["frac"], "traffic": None, "peak_source": peaks["source"], "avg_launch_ms": d["ms"],
+                "note": ("alu peak = 148 SM x 128 FP32 lanes x 2 flop x sm_max_mhz; achieved = algorithmic (pi-folded) flops"
+                         if d["bound"] == "alu" else "algorithmic bytes / CUDA-event time")}
+    tr = ROOT / "profiles" / "traffic.json"                  # dram bytes per launch from the committed ncu capture
+    if tr.exists():
+        try:
+            roofline["traffic"] = json.loads(tr.read_text()).get(synth.describe(c), {}).get(dom)
+        except Exception:
+            pass
+    gups = {n: c.nominal_updates / (r["ops"][n + "_op"] * 1e-3) / 1e9 for n in ("forward", "adjoint")}
+    ms_step = r["ms"] / K
+    line = {
+        "metric": METRIC, "value": world * K / (r["ms"] * 1e-3), "unit": UNIT, "n_gpus": world, "steps": K,
+        "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f32", "data": "synthetic",
+        "config": {"workload": synth.describe(c), "cfg": c.cfg, "n": c.n, "nz": c.nz, "nd": c.nd, "n_angles": c.n_angles,
+                   "n_half_rot": c.n_half_rot, "m": c.m, "basis": c.basis, "lambda1": c.lambda1, "lambda2": c.lambda2,
+                   "norm_K": r["L"], "parallelism": "replicas only" if world > 1 else "1 gpu",
+                   "l2": f"no flush: CP state {(7 * c.V + 2 * c.S) * 4 / 1e9:.2f} GB streams through every step (L2 = 126 MB)"},
+        "gups_nominal": {"forward": gups["forward"], "adjoint": gups["adjoint"], "unit": "1e9 voxel*angle*basis/s",
+                         "forward_ms": r["ops"]["forward_op"], "adjoint_ms": r["ops"]["adjoint_op"],
+                         "note": "nominal count N^2*Nz*N_theta*m per call; kernels use the pi-fold (N_theta0 base angles)"},
+        "roofline": roofline, "kernels": kernels, "clocks": r["clocks"], "e2e": r["e2e"],
+        "gpu_launches": r["launches"], "impl": "cp4d",
+    }
+    return line
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=3, help="BASELINE.json config 1..5 (SURVEY.md 8 numbering)")
+    ap.add_argument("--impl", default="cp4d", choices=["cp4d", "reference"])
+    ap.add_argument("--power-iters", type=int, default=10)
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    from paper_1809_09725_b200 import synth
+    c = synth.CONFIGS[args.config]
+    rank, world = int(os.environ.get("RANK", 0)), int(os.environ.get("WORLD_SIZE", 1))
+    if args.impl == "reference":
+        run_reference(args, c, rank)
+        return
+    if args.warmup < 3:
+        print(f"bench.py: warning: --warmup {args.warmup} < 3 (timing rules want >= 3)", file=sys.stderr)
+    ctx, r = run_cp4d(args, c, rank, world)
+    ctx.close()
+    if rank == 0:
+        line = assemble(args, c, world, r)
+        if not args.no_cpu_baseline and world == 1:
+            val, cores, sample, dt = oracle_steps(c, 1, 0)
+            line["cpu_baseline"] = {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample,
+                                    "sample_step_s": dt}
+        print(json.dumps(line), flush=True)
+    if world > 1:
+        import torch.distributed as dist
+        dist.barrier()
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -128,6 +128,29 @@ int cp4d_solve_host(cp4d_ctx *ctx, const float *g_host, int32_t n_iters, float *
 int cp4d_sync(cp4d_ctx *ctx);
 /* number of kernels (and memset nodes) this context has enqueued since create */
 int cp4d_launch_count(const cp4d_ctx *ctx, uint64_t *count_out);
+
+/* ---- per-kernel device timing (CUDA events on the context's stream) ------------- */
+/* Kernel classes of the hot path.  FORWARD includes the zero-fill of its partial-sum scratch. */
+#define CP4D_K_FORWARD     0  /* ray sums over the base angles, all m coefficients per ray (Eq. 9)       */
+#define CP4D_K_SYNTH       1  /* synthesis with Phi + unfold (+ F1* prox, step 3)                         */
+#define CP4D_K_FOLD        2  /* analysis with Phi + pi-fold of the sinogram (L204-L212)                  */
+#define CP4D_K_BACKPROJECT 3  /* backprojection over the base angles (Eq. 10)                             */
+#define CP4D_K_GRAD        4
+#define CP4D_K_DIV         5
+#define CP4D_K_PROX_F2     6  /* fused grad + projection (step 4)                                         */
+#define CP4D_K_UPDATE      7  /* fused div + primal update + over-relaxation (steps 5-6)                  */
+#define CP4D_K_REDUCE      8
+#define CP4D_K_MISC        9
+#define CP4D_K_COUNT      10
+typedef struct {
+    double   ms[CP4D_K_COUNT];        /* summed device time of the class since cp4d_profile_begin       */
+    uint64_t launches[CP4D_K_COUNT];  /* timed launches of the class                                      */
+} cp4d_profile;
+/* Start recording a CUDA event pair around every kernel this context enqueues (clears old records). */
+int cp4d_profile_begin(cp4d_ctx *ctx);
+/* Sync, stop recording, sum the event pairs per class into *out_host (HOST). */
+int cp4d_profile_end(cp4d_ctx *ctx, cp4d_profile *out_host);
+const char *cp4d_kernel_name(int kernel_class);
 const char *cp4d_strerror(int code);
 const char *cp4d_last_error(const cp4d_ctx *ctx);
 const char *cp4d_version(void);

@@ -32,6 +32,13 @@ class Params(C.Structure):
                 ("stream", C.c_void_p)]
 
 
+K_COUNT = 10
+
+
+class Profile(C.Structure):
+    _fields_ = [("ms", C.c_double * K_COUNT), ("launches", C.c_uint64 * K_COUNT)]
+
+
 def lib():
     """Load libcp4d.so (built in-tree by paper_1809_09725_b200.build).  Raises if it is missing."""
     global _lib
@@ -55,12 +62,14 @@ def lib():
             "cp4d_state_ptrs": [vp] + [C.POINTER(vp)] * 5,
             "cp4d_solve_host": [vp, vp, i32, vp], "cp4d_sync": [vp],
             "cp4d_launch_count": [vp, C.POINTER(u64)],
+            "cp4d_profile_begin": [vp], "cp4d_profile_end": [vp, C.POINTER(Profile)],
         }
         for name, args in sig.items():
             fn = getattr(L, name)
             fn.argtypes, fn.restype = args, C.c_int
-        for name in ("cp4d_strerror", "cp4d_last_error", "cp4d_version"):
+        for name in ("cp4d_strerror", "cp4d_last_error", "cp4d_version", "cp4d_kernel_name"):
             getattr(L, name).restype = C.c_char_p
+        L.cp4d_kernel_name.argtypes = [C.c_int]
         L.cp4d_strerror.argtypes = [C.c_int]
         L.cp4d_last_error.argtypes = [vp]
         _lib = L
@@ -229,6 +238,15 @@ class Context:
         out = C.c_uint64(0)
         self._ck(lib().cp4d_launch_count(self._h, C.byref(out)))
         return out.value
+
+    def profile_begin(self):
+        self._ck(lib().cp4d_profile_begin(self._h))
+
+    def profile_end(self) -> dict:
+        """{kernel class name: (summed device ms, timed launches)} since profile_begin; syncs."""
+        pr = Profile()
+        self._ck(lib().cp4d_profile_end(self._h, C.byref(pr)))
+        return {lib().cp4d_kernel_name(k).decode(): (pr.ms[k], int(pr.launches[k])) for k in range(K_COUNT) if pr.launches[k]}
 
     def close(self):
         if getattr(self, "_h", None):

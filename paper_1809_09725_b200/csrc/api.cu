@@ -126,7 +126,7 @@ int cp4d_create(const cp4d_params *p, cp4d_ctx **out) {
     if (!ctx) return CP4D_EINVAL;
     ctx->d = d; ctx->lambda1 = p->lambda1; ctx->lambda2 = p->lambda2; ctx->theta = p->theta_relax;
     ctx->tau = ctx->sigma = 0.f; ctx->have_steps = ctx->have_data = false;
-    ctx->device = p->device; ctx->stream = (cudaStream_t)p->stream; ctx->launches = 0;
+    ctx->device = p->device; ctx->stream = (cudaStream_t)p->stream; ctx->launches = 0; ctx->prof_on = false;
     char *w = (char *)p->workspace_dev;
     ctx->f = (float *)(w + cv.f); ctx->ft = (float *)(w + cv.ft); ctx->bp = (float *)(w + cv.bp);
     ctx->h2 = (float *)(w + cv.h2); ctx->h1 = (float *)(w + cv.h1); ctx->g = (float *)(w + cv.g);
@@ -171,6 +171,10 @@ int cp4d_create(const cp4d_params *p, cp4d_ctx **out) {
 }
 
 int cp4d_destroy(cp4d_ctx *ctx) {
+    if (ctx) {
+        for (auto &r : ctx->prof) { cudaEventDestroy(r.a); cudaEventDestroy(r.b); }
+        for (auto e : ctx->ev_pool) cudaEventDestroy(e);
+    }
     delete ctx;
     return CP4D_OK;
 }
@@ -345,6 +349,38 @@ int cp4d_sync(cp4d_ctx *ctx) {
     CK(cudaStreamSynchronize(ctx->stream), "sync");
     CK(cudaGetLastError(), "sync");
     return CP4D_OK;
+}
+
+int cp4d_profile_begin(cp4d_ctx *ctx) {
+    if (!ctx) return CP4D_EINVAL;
+    for (auto &r : ctx->prof) { ctx->ev_pool.push_back(r.a); ctx->ev_pool.push_back(r.b); }
+    ctx->prof.clear();
+    ctx->prof_on = true;
+    return CP4D_OK;
+}
+
+int cp4d_profile_end(cp4d_ctx *ctx, cp4d_profile *out) {
+    if (!ctx) return CP4D_EINVAL;
+    if (!out) return fail(ctx, CP4D_EINVAL, "profile_end: null output");
+    ctx->prof_on = false;
+    std::memset(out, 0, sizeof(*out));
+    CK(cudaStreamSynchronize(ctx->stream), "profile_end sync");
+    for (auto &r : ctx->prof) {
+        float ms = 0.f;
+        if (cudaEventElapsedTime(&ms, r.a, r.b) == cudaSuccess && r.cls >= 0 && r.cls < CP4D_K_COUNT) {
+            out->ms[r.cls] += ms;
+            out->launches[r.cls]++;
+        }
+        ctx->ev_pool.push_back(r.a); ctx->ev_pool.push_back(r.b);
+    }
+    cudaGetLastError();
+    ctx->prof.clear();
+    return CP4D_OK;
+}
+
+const char *cp4d_kernel_name(int k) {
+    static const char *names[CP4D_K_COUNT] = {"forward", "synth", "fold", "backproject", "grad", "div", "prox_f2", "update", "reduce", "misc"};
+    return (k >= 0 && k < CP4D_K_COUNT) ? names[k] : "?";
 }
 
 int cp4d_launch_count(const cp4d_ctx *ctx, uint64_t *out) {

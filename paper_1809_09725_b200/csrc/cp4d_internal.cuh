@@ -4,6 +4,7 @@
 #include <stdint.h>
 
 #include <string>
+#include <vector>
 
 #include "cp4d.h"
 
@@ -52,9 +53,37 @@ struct cp4d_ctx {
     double *red;               // 8 doubles for reductions
     uint64_t launches;
     std::string err;
+    // per-kernel event timing (cp4d_profile_begin/end)
+    bool prof_on;
+    struct ProfRec { int cls; cudaEvent_t a, b; };
+    std::vector<ProfRec> prof;       // records of the current profiling window
+    std::vector<cudaEvent_t> ev_pool;  // reusable events
 };
 
 namespace cp4d {
+
+// RAII event pair around the launches of one kernel class; no-op unless profiling is on
+struct ProfScope {
+    cp4d_ctx *c;
+    cudaEvent_t a, b;
+    int cls;
+    ProfScope(cp4d_ctx *ctx, int kernel_class) : c(ctx), a(nullptr), b(nullptr), cls(kernel_class) {
+        if (!c->prof_on) return;
+        a = take(); b = take();
+        if (a && b) cudaEventRecord(a, c->stream);
+    }
+    ~ProfScope() {
+        if (!a || !b) return;
+        cudaEventRecord(b, c->stream);
+        c->prof.push_back({cls, a, b});
+    }
+    cudaEvent_t take() {
+        if (!c->ev_pool.empty()) { cudaEvent_t e = c->ev_pool.back(); c->ev_pool.pop_back(); return e; }
+        cudaEvent_t e = nullptr;
+        if (cudaEventCreate(&e) != cudaSuccess) { cudaGetLastError(); return nullptr; }
+        return e;
+    }
+};
 
 // launchers (each enqueues on ctx->stream and bumps ctx->launches); return cudaError_t
 cudaError_t launch_grad(cp4d_ctx *c, const float *f, float *p);

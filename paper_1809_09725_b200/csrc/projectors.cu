@@ -233,6 +233,7 @@ static cudaError_t bp_launch(cp4d_ctx *c, const float4 *gt, float *f_out, const 
 }
 
 cudaError_t launch_forward_partial(cp4d_ctx *c, const float *f, float4 *P) {
+    ProfScope ps(c, CP4D_K_FORWARD);
     const Dims &d = c->d;
     ProjArgs a{d.n, d.nz, d.nd, d.n0, d.Q, c->ang, c->geo};
     cudaError_t e = cudaMemsetAsync(P, 0, (size_t)d.scratch4 * sizeof(float4), c->stream);
@@ -246,6 +247,7 @@ cudaError_t launch_forward_partial(cp4d_ctx *c, const float *f, float4 *P) {
 }
 
 cudaError_t launch_backproject(cp4d_ctx *c, const float4 *gt, float *f_out) {
+    ProfScope ps(c, CP4D_K_BACKPROJECT);
     const Dims &d = c->d;
     ProjArgs a{d.n, d.nz, d.nd, d.n0, d.Q, c->ang, c->geo};
     c->launches++;

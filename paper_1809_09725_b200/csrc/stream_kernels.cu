@@ -134,6 +134,7 @@ static StreamArgs make_args(const cp4d_ctx *c, dim3 &grid, dim3 &block) {
 }
 
 cudaError_t launch_grad(cp4d_ctx *c, const float *f, float *p) {
+    ProfScope ps(c, CP4D_K_GRAD);
     dim3 g, b;
     StreamArgs a = make_args(c, g, b);
     k_grad<false><<<g, b, 0, c->stream>>>(f, p, a, 0.f, 0.f, 0);
@@ -141,6 +142,7 @@ cudaError_t launch_grad(cp4d_ctx *c, const float *f, float *p) {
     return cudaGetLastError();
 }
 cudaError_t launch_prox_f2(cp4d_ctx *c, float sigma, const float *ft, float *h2) {
+    ProfScope ps(c, CP4D_K_PROX_F2);
     dim3 g, b;
     StreamArgs a = make_args(c, g, b);
     const int l1z = !(c->lambda1 > 0.f);
@@ -149,6 +151,7 @@ cudaError_t launch_prox_f2(cp4d_ctx *c, float sigma, const float *ft, float *h2)
     return cudaGetLastError();
 }
 cudaError_t launch_div(cp4d_ctx *c, const float *p, float *f) {
+    ProfScope ps(c, CP4D_K_DIV);
     dim3 g, b;
     StreamArgs a = make_args(c, g, b);
     k_div<false><<<g, b, 0, c->stream>>>(p, f, a, nullptr, nullptr, 0.f, 0.f);
@@ -156,6 +159,7 @@ cudaError_t launch_div(cp4d_ctx *c, const float *p, float *f) {
     return cudaGetLastError();
 }
 cudaError_t launch_update(cp4d_ctx *c, float tau, const float *bp, const float *h2, float *f, float *ft) {
+    ProfScope ps(c, CP4D_K_UPDATE);
     dim3 g, b;
     StreamArgs a = make_args(c, g, b);
     k_div<true><<<g, b, 0, c->stream>>>(h2, f, a, bp, ft, tau, c->theta);
@@ -234,6 +238,7 @@ __global__ void __launch_bounds__(128) k_synth(const float4 *__restrict__ P, int
     }
 
 cudaError_t launch_fold(cp4d_ctx *c, const float *g, float4 *gt) {
+    ProfScope ps(c, CP4D_K_FOLD);
     const Dims &d = c->d;
     const size_t sh = (size_t)d.npi * d.m * sizeof(float);
     CP4D_DISPATCH_Q(d.Q, (k_fold<QQ><<<d.nz * d.n0, 128, sh, c->stream>>>(g, gt, c->phi, d.nd, d.na, d.npi, d.n0)));
@@ -241,6 +246,7 @@ cudaError_t launch_fold(cp4d_ctx *c, const float *g, float4 *gt) {
     return cudaGetLastError();
 }
 cudaError_t launch_synth(cp4d_ctx *c, const float4 *P, int mode, float sigma, const float *g, float *out) {
+    ProfScope ps(c, CP4D_K_SYNTH);
     const Dims &d = c->d;
     const size_t sh = (size_t)d.npi * d.m * sizeof(float);
     CP4D_DISPATCH_Q(d.Q, (k_synth<QQ><<<d.nz * d.n0, 128, sh, c->stream>>>(P, mode, sigma, g, out, c->phi, d.nd, d.na, d.npi, d.n0)));
@@ -273,6 +279,7 @@ __global__ void __launch_bounds__(256) k_dot(const float *__restrict__ x, const 
 }
 
 cudaError_t launch_sumsq_dot(cp4d_ctx *c, const float *x, const float *y, uint64_t n, double *slot) {
+    ProfScope ps(c, CP4D_K_REDUCE);
     cudaError_t e = cudaMemsetAsync(slot, 0, sizeof(double), c->stream);
     if (e != cudaSuccess) return e;
     uint64_t blocks = (n / 4 + 255) / 256;
@@ -299,6 +306,7 @@ __global__ void __launch_bounds__(256) k_fill_normal(float *x, uint64_t n, uint6
     }
 }
 cudaError_t launch_fill_normal(cp4d_ctx *c, float *x, uint64_t n, uint64_t seed) {
+    ProfScope ps(c, CP4D_K_MISC);
     uint64_t blocks = (n + 255) / 256;
     if (blocks > 148 * 8) blocks = 148 * 8;
     k_fill_normal<<<(unsigned)blocks, 256, 0, c->stream>>>(x, n, seed);
@@ -318,6 +326,7 @@ __global__ void __launch_bounds__(256) k_scale_diff(float *x, const float *a, co
     }
 }
 cudaError_t launch_scale_diff(cp4d_ctx *c, float *x, const float *a, const float *b, float s, uint64_t n) {
+    ProfScope ps(c, CP4D_K_MISC);
     uint64_t blocks = (n / 4 + 255) / 256;
     if (blocks > 148 * 8) blocks = 148 * 8;
     k_scale_diff<<<(unsigned)blocks, 256, 0, c->stream>>>(x, a, b, s, n / 4);  // V is a multiple of 4

@@ -131,7 +131,7 @@ def test_cp_iterations(torch_cuda, fast_oracle, case, lam1):
     c = CASES[case]
     g = _data(c).astype(np.float32)
     if lam1 == "mixed":      # lambda1 for which a good fraction of voxels is clamped AND a good fraction is not (C18)
-        lam1 = {"cfg1": 0.6, "cfg2": 0.25, "ragged": 0.15}[case]
+        lam1 = {"cfg1": 0.02, "cfg2": 2e-4, "ragged": 0.003}[case]   # bisected with the oracle on the clamp fraction
     c = c.scaled(lambda1=float(np.float32(lam1)))
     from paper_1809_09725_b200 import binding
     phi = synth.basis_table(c.basis, c.m, c.n_angles)
