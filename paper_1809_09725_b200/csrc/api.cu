@@ -27,7 +27,14 @@ int validate(const cp4d_params *p, Dims *d) {
     d->V = (int64_t)d->nz * d->n * d->n * d->m;
     d->S = (int64_t)d->nz * d->na * d->nd;
     d->slice4 = (int64_t)d->n * d->n * d->Q;
-    d->scratch4 = (int64_t)d->nz * d->n0 * d->Q * d->nd;
+    // pads of the scratch rows: the window [bstart, bstart + WIN + 8) of a 32x32 tile (edge tiles reach past the grid) may
+    // leave the detector by at most sqrt2 * E - (nd-1)/2 + 2 bins, E = largest |coordinate| a tile covers
+    // (cp4d_create checks the exact values)
+    const double cen0 = 0.5 * (d->n - 1), ext = std::fmax(cen0, (double)d->tiles_1d * TILE - 1.0 - cen0);
+    const int over = (int)std::ceil(std::fmax(0.0, 1.41421356237309515 * ext - 0.5 * (d->nd - 1))) + 3;
+    d->gpl = over;
+    d->gp = d->nd + 2 * over + WIN + 8;
+    d->scratch4 = (int64_t)d->nz * d->n0 * d->Q * d->gp;
     if (d->nz > 65535 || d->tiles > 2000000) return CP4D_EINVAL;
     return CP4D_OK;
 }
@@ -143,6 +150,9 @@ int cp4d_create(const cp4d_params *p, cp4d_ctx **out) {
         ang[i].c = (float)c; ang[i].s = (float)s;
         ang[i].inv_a = (float)(1.0 / std::fmax(std::fabs(c), std::fabs(s)));
         ang[i].col_step = std::fabs(s) >= std::fabs(c) ? 1 : 0;
+        ang[i].pat = bp_pattern(ang[i].c, ang[i].s);
+        if (ang[i].pat < 0) { delete ctx; return CP4D_EINVAL; }
+        ang[i].pat_fl = bp_pattern_fl(ang[i].pat);
     }
     std::vector<TileGeo> geo((size_t)d.tiles * d.n0);
     const double cen = 0.5 * (d.n - 1), cd = 0.5 * (d.nd - 1);
@@ -155,6 +165,7 @@ int cp4d_create(const cp4d_params *p, cp4d_ctx **out) {
             const double pmin = p0 + std::fmin(0.0, (TILE - 1) * c) + std::fmin(0.0, (TILE - 1) * s);
             const double bs = std::floor(pmin) - 1.0;
             geo[(size_t)t * d.n0 + i].bstart = (int32_t)bs;
+            if ((int32_t)bs < -d.gpl || (int32_t)bs + WIN + 8 > d.gp - d.gpl) { delete ctx; return CP4D_EINVAL; }
             geo[(size_t)t * d.n0 + i].delta = (float)(p0 - bs);
         }
     }
@@ -162,6 +173,7 @@ int cp4d_create(const cp4d_params *p, cp4d_ctx **out) {
     if ((e = cudaMemcpyAsync(ctx->phi, p->phi_host, (size_t)d.m * d.na * 4, cudaMemcpyHostToDevice, ctx->stream)) != cudaSuccess ||
         (e = cudaMemcpyAsync(ctx->ang, ang.data(), ang.size() * sizeof(AngleTab), cudaMemcpyHostToDevice, ctx->stream)) != cudaSuccess ||
         (e = cudaMemcpyAsync(ctx->geo, geo.data(), geo.size() * sizeof(TileGeo), cudaMemcpyHostToDevice, ctx->stream)) != cudaSuccess ||
+        (e = cudaMemsetAsync(ctx->scratch, 0, (size_t)d.scratch4 * 16, ctx->stream)) != cudaSuccess ||
         (e = cudaStreamSynchronize(ctx->stream)) != cudaSuccess) {
         delete ctx;
         return CP4D_ECUDA;

@@ -1,0 +1,272 @@
+// Adjoint projector, stage 2 (Eq. 10; fold L204-L212): backprojection of the pi-folded sinogram
+// gt[z][i][jq][b] (float4 over 4 consecutive coefficients j) over the N_theta0 base angles.
+//
+// Operand delivery is what binds this kernel: shared memory hands out 32 lane-words/clk/SM, the FMA pipe
+// eats 128 lanes/clk/SM.  So every fetched bin is reused from registers: a thread owns a compact PATCH of 4 (x) x 2 (y)
+// voxels x MJ = 4*JQ coefficients.  At one angle the patch touches only NB <= 6 consecutive bins; they are loaded once
+// (NB*JQ LDS.128) and feed 16*MJ useful FMAs.
+//
+// Static register indexing.  With u = bin coordinate of a voxel, the patch's smallest coordinate is umin = K + phi
+// (K integer, 0 <= phi < 1, both per thread) and voxel v sits at umin + delta_v where delta_v = e*|c| + dy*s is the
+// same for every thread at this angle.  Choose an integer FL_v with 0 <= delta_v - FL_v <= 1 (the host picks one of 9
+// possible 8-tuples, the "pattern" of the angle); then t = phi + delta_v - FL_v is in [0,2) and the voxel touches only
+// bins K+FL_v+{0,1,2}, with Joseph hat weights max(0, 1/a - |t-k|/a^2) (one of the three is zero).  A warp-uniform
+// switch on the pattern selects straight-line code in which every register index is a compile-time constant.
+// For c < 0 the patch is traversed mirrored in x (e = 3-dx); the accumulators are swapped once when the sign changes.
+#include <cmath>
+
+#include "cp4d_internal.cuh"
+
+namespace cp4d {
+
+namespace {
+
+constexpr int BP_THREADS = 128;          // one thread per 4x2 patch of a 32x32 tile
+constexpr int BP_CHUNK = 8;              // angles staged per pipeline stage
+constexpr int WINP = WIN + 8;            // staged bins per (angle, jq): window + NB-1 spill, zero-filled outside the detector
+
+__host__ __device__ constexpr int bp_fl(int pat, int v) {
+    constexpr int T[BP_NPAT][8] = {
+        {0, 1, 2, 3, 0, 1, 2, 3}, {0, 0, 1, 2, 0, 1, 2, 3}, {0, 0, 1, 2, 0, 1, 2, 2}, {0, 0, 1, 1, 0, 1, 2, 2},
+        {0, 0, 1, 1, 0, 1, 1, 2}, {0, 0, 0, 1, 0, 1, 1, 2}, {0, 0, 0, 1, 0, 1, 1, 1}, {0, 0, 0, 0, 0, 1, 1, 1},
+        {0, 0, 0, 0, 1, 1, 1, 1}};
+    return T[pat][v];
+}
+__host__ __device__ constexpr int bp_nb(int pat) {
+    int mx = 0;
+    for (int v = 0; v < 8; ++v) mx = bp_fl(pat, v) > mx ? bp_fl(pat, v) : mx;
+    return mx + 3;
+}
+
+// acc += w * v on 4 coefficients as two packed fp32x2 FMAs (SASS FFMA2: same FMA rate, half the issue slots)
+__device__ __forceinline__ void fma4(float4 &a, const float2 ww, const float4 &v) {
+    const float2 lo = __ffma2_rn(ww, make_float2(v.x, v.y), make_float2(a.x, a.y));
+    const float2 hi = __ffma2_rn(ww, make_float2(v.z, v.w), make_float2(a.z, a.w));
+    a = make_float4(lo.x, lo.y, hi.x, hi.y);
+}
+// ---- TMA 1D bulk copy global -> shared, completion on an mbarrier (SASS UBLKCP) ----
+__device__ __forceinline__ unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t *bar, unsigned count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;\n" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, unsigned bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t *bar, unsigned parity) {
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_%=:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra DONE_%=;\n"
+        "bra WAIT_%=;\n"
+        "DONE_%=:\n"
+        "}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(void *dst_smem, const void *src_gmem, unsigned bytes, uint64_t *bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];\n" ::"r"(smem_u32(dst_smem)),
+                 "l"(src_gmem), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+}
+
+template <int PAT, int V, int JQ, int NB>
+__device__ __forceinline__ void bp_voxel(float4 (&acc)[8][JQ], const float4 (&B)[NB][JQ], float phi, float td,
+                                         float A1, float A2, float A3) {
+    constexpr int FL = bp_fl(PAT, V);
+    const float t = phi + td;                                                  // in [0,2)
+    const float x0 = fmaxf(0.f, fmaf(-A2, t, A1));
+    const float x1 = fmaxf(0.f, fmaf(-A2, fabsf(t - 1.0f), A1));
+    const float x2 = fmaxf(0.f, fmaf(A2, t, A3));                              // A3 = A1 - 2 A2
+    const float2 w0 = make_float2(x0, x0), w1 = make_float2(x1, x1), w2 = make_float2(x2, x2);
+#pragma unroll
+    for (int jc = 0; jc < JQ; ++jc) {
+        fma4(acc[V][jc], w0, B[FL][jc]);
+        fma4(acc[V][jc], w1, B[FL + 1][jc]);
+        fma4(acc[V][jc], w2, B[FL + 2][jc]);
+    }
+}
+
+template <int PAT, int JQ>
+__device__ __forceinline__ void bp_angle(float4 (&acc)[8][JQ], const float4 *wbase, float phi, const float4 tda,
+                                         const float4 tdb, float A1, float A2, float A3) {
+    constexpr int NB = bp_nb(PAT);
+    float4 B[NB][JQ];
+#pragma unroll
+    for (int k = 0; k < NB; ++k)
+#pragma unroll
+        for (int jc = 0; jc < JQ; ++jc) B[k][jc] = wbase[jc * WINP + k];
+    bp_voxel<PAT, 0, JQ, NB>(acc, B, phi, tda.x, A1, A2, A3);
+    bp_voxel<PAT, 1, JQ, NB>(acc, B, phi, tda.y, A1, A2, A3);
+    bp_voxel<PAT, 2, JQ, NB>(acc, B, phi, tda.z, A1, A2, A3);
+    bp_voxel<PAT, 3, JQ, NB>(acc, B, phi, tda.w, A1, A2, A3);
+    bp_voxel<PAT, 4, JQ, NB>(acc, B, phi, tdb.x, A1, A2, A3);
+    bp_voxel<PAT, 5, JQ, NB>(acc, B, phi, tdb.y, A1, A2, A3);
+    bp_voxel<PAT, 6, JQ, NB>(acc, B, phi, tdb.z, A1, A2, A3);
+    bp_voxel<PAT, 7, JQ, NB>(acc, B, phi, tdb.w, A1, A2, A3);
+}
+
+}  // namespace
+
+struct BpArgs {
+    int n, nz, nd, n0, Q, gp, gpl;
+    const AngleTab *ang;
+    const TileGeo *geo;
+};
+
+// per (CTA, staged angle) parameters in shared memory, read by every thread as warp-uniform (broadcast) loads
+struct BpAngle {
+    float4 g;    // delta (tile origin - window start), c, s, unused
+    float4 k;    // A1 = 1/a, A2 = 1/a^2, A3 = A1 - 2 A2, pattern (int bits)
+    float4 tda;  // delta_v - FL_v for voxels v = 0..3 (dy = 0, e = 0..3)
+    float4 tdb;  // v = 4..7 (dy = 1)
+};
+
+template <int JQ>
+__global__ void __launch_bounds__(BP_THREADS, 3) k_backproject(const float4 *__restrict__ gt, float *__restrict__ out, BpArgs a) {
+    __shared__ __align__(128) float4 win[2][BP_CHUNK][JQ][WINP];
+    __shared__ BpAngle sang[2][BP_CHUNK];
+    __shared__ __align__(8) uint64_t mbar[2];
+    const int tiles_1d = (a.n + TILE - 1) / TILE;
+    const int tix = blockIdx.x % tiles_1d, tiy = blockIdx.x / tiles_1d;
+    const int z = blockIdx.y, jg = blockIdx.z;
+    // lane -> patch: a quarter warp (the unit an LDS.128 is served in) covers 2 (x) x 4 (y) patches; their window starts
+    // differ by at most 4|c| + 6 s <= 7.2 < 8 slots of 16 B, so the 8 lanes never collide on a bank
+    const int l = threadIdx.x & 31, w = threadIdx.x >> 5;
+    const int pxi = (l & 1) | ((l >> 2) & 6), pyi = ((l >> 1) & 3) | (w << 2);
+    const float fx0 = (float)(4 * pxi), fy0 = (float)(2 * pyi);
+    const TileGeo *geo = a.geo + (int64_t)blockIdx.x * a.n0;
+    const int nch = (a.n0 + BP_CHUNK - 1) / BP_CHUNK;
+
+    auto stage = [&](int buf, int ch) {
+        const int i0 = ch * BP_CHUNK;
+        if (threadIdx.x < BP_CHUNK) {
+            const int i = min(i0 + (int)threadIdx.x, a.n0 - 1);
+            const AngleTab A = a.ang[i];
+            const float ca = fabsf(A.c), A2 = A.inv_a * A.inv_a;
+            float td[8];
+#pragma unroll
+            for (int v = 0; v < 8; ++v) td[v] = fmaf((float)(v & 3), ca, (float)(v >> 2) * A.s) - (float)((A.pat_fl >> (4 * v)) & 15);
+            BpAngle &S = sang[buf][threadIdx.x];
+            S.g = make_float4(geo[i].delta, A.c, A.s, 0.f);
+            S.k = make_float4(A.inv_a, A2, fmaf(-2.0f, A2, A.inv_a), __int_as_float(A.pat));
+            S.tda = make_float4(td[0], td[1], td[2], td[3]);
+            S.tdb = make_float4(td[4], td[5], td[6], td[7]);
+        }
+        // one TMA bulk copy per (angle, coefficient chunk) row of the window: WINP bins x 16 B, always inside the padded
+        // scratch row (cp4d_create checks), so no bounds logic; lanes 0..nrows-1 of warp 0 each issue one copy
+        if (threadIdx.x < 32) {
+            const int nrows = min(BP_CHUNK, a.n0 - i0) * JQ;
+            if (threadIdx.x == 0) mbar_expect_tx(&mbar[buf], (unsigned)(nrows * WINP * sizeof(float4)));
+            __syncwarp();
+            if ((int)threadIdx.x < nrows) {
+                const int aa = threadIdx.x / JQ, jc = threadIdx.x % JQ, i = i0 + aa;
+                const float4 *src = gt + (((int64_t)z * a.n0 + i) * a.Q + jg * JQ + jc) * a.gp + a.gpl + geo[i].bstart;
+                bulk_g2s(&win[buf][aa][jc][0], src, (unsigned)(WINP * sizeof(float4)), &mbar[buf]);
+            }
+        }
+    };
+
+    float4 acc[8][JQ];
+#pragma unroll
+    for (int v = 0; v < 8; ++v)
+#pragma unroll
+        for (int jc = 0; jc < JQ; ++jc) acc[v][jc] = make_float4(0.f, 0.f, 0.f, 0.f);
+    bool flipped = false;
+    auto flip = [&]() {
+#pragma unroll
+        for (int dy = 0; dy < 2; ++dy)
+#pragma unroll
+            for (int jc = 0; jc < JQ; ++jc) {
+                float4 t0 = acc[4 * dy + 0][jc]; acc[4 * dy + 0][jc] = acc[4 * dy + 3][jc]; acc[4 * dy + 3][jc] = t0;
+                float4 t1 = acc[4 * dy + 1][jc]; acc[4 * dy + 1][jc] = acc[4 * dy + 2][jc]; acc[4 * dy + 2][jc] = t1;
+            }
+        flipped = !flipped;
+    };
+
+    if (threadIdx.x == 0) {
+        mbar_init(&mbar[0], 1);
+        mbar_init(&mbar[1], 1);
+        asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
+    }
+    __syncthreads();
+    stage(0, 0);
+    __syncthreads();
+    for (int ch = 0; ch < nch; ++ch) {
+        const int buf = ch & 1;
+        // buffer buf^1 and sang[buf^1] were last read in iteration ch-1, which ended with __syncthreads
+        if (ch + 1 < nch) stage(buf ^ 1, ch + 1);
+        mbar_wait(&mbar[buf], (unsigned)((ch >> 1) & 1));
+        const int na = min(BP_CHUNK, a.n0 - ch * BP_CHUNK);
+        for (int aa = 0; aa < na; ++aa) {
+            const BpAngle &S = sang[buf][aa];
+            const float4 G = S.g, K = S.k;
+            const bool neg = G.y < 0.f;
+            if (neg != flipped) flip();
+            const float umin = fmaf(fx0 + (neg ? 3.0f : 0.0f), G.y, fmaf(fy0, G.z, G.x));
+            const float fk = floorf(umin);
+            const float phi = umin - fk;
+            const float4 *wbase = &win[buf][aa][0][(int)fk];
+            switch (__float_as_int(K.w)) {
+            case 0: bp_angle<0, JQ>(acc, wbase, phi, S.tda, S.tdb, K.x, K.y, K.z); break;
+            case 1: bp_angle<1, JQ>(acc, wbase, phi, S.tda, S.tdb, K.x, K.y, K.z); break;
+            case 2: bp_angle<2, JQ>(acc, wbase, phi, S.tda, S.tdb, K.x, K.y, K.z); break;
+            case 3: bp_angle<3, JQ>(acc, wbase, phi, S.tda, S.tdb, K.x, K.y, K.z); break;
+            case 4: bp_angle<4, JQ>(acc, wbase, phi, S.tda, S.tdb, K.x, K.y, K.z); break;
+            case 5: bp_angle<5, JQ>(acc, wbase, phi, S.tda, S.tdb, K.x, K.y, K.z); break;
+            case 6: bp_angle<6, JQ>(acc, wbase, phi, S.tda, S.tdb, K.x, K.y, K.z); break;
+            case 7: bp_angle<7, JQ>(acc, wbase, phi, S.tda, S.tdb, K.x, K.y, K.z); break;
+            default: bp_angle<8, JQ>(acc, wbase, phi, S.tda, S.tdb, K.x, K.y, K.z); break;
+            }
+        }
+        __syncthreads();
+    }
+    if (flipped) flip();
+    float4 *O = reinterpret_cast<float4 *>(out);
+#pragma unroll
+    for (int v = 0; v < 8; ++v) {
+        const int x = tix * TILE + 4 * pxi + (v & 3), y = tiy * TILE + 2 * pyi + (v >> 2);
+        if (x < a.n && y < a.n) {
+            float4 *dst = O + (((int64_t)z * a.n + y) * a.n + x) * a.Q + jg * JQ;
+#pragma unroll
+            for (int jc = 0; jc < JQ; ++jc) dst[jc] = acc[v][jc];
+        }
+    }
+}
+
+template <int JQ>
+static cudaError_t bp_launch(cp4d_ctx *c, const float4 *gt, float *f_out, const BpArgs &a) {
+    const Dims &d = c->d;
+    k_backproject<JQ><<<dim3(d.tiles, d.nz, d.Q / JQ), BP_THREADS, 0, c->stream>>>(gt, f_out, a);
+    return cudaGetLastError();
+}
+
+// host side of the pattern choice (cp4d_create): first pattern whose offsets all satisfy 0 <= delta_v - FL_v <= 1,
+// evaluated with the fp32-rounded |c|, s the kernel multiplies with
+int bp_pattern(float c, float s) {
+    const double ca = std::fabs((double)c), sd = (double)s;
+    for (int p = 0; p < BP_NPAT; ++p) {
+        bool ok = true;
+        for (int v = 0; v < 8 && ok; ++v) {
+            const double d = (v & 3) * ca + (v >> 2) * sd - bp_fl(p, v);
+            ok = d >= 0.0 && d <= 1.0;
+        }
+        if (ok) return p;
+    }
+    return -1;
+}
+
+uint32_t bp_pattern_fl(int pat) {
+    uint32_t r = 0;
+    for (int v = 0; v < 8; ++v) r |= (uint32_t)bp_fl(pat, v) << (4 * v);
+    return r;
+}
+
+cudaError_t launch_backproject(cp4d_ctx *c, const float4 *gt, float *f_out) {
+    ProfScope ps(c, CP4D_K_BACKPROJECT);
+    const Dims &d = c->d;
+    BpArgs a{d.n, d.nz, d.nd, d.n0, d.Q, d.gp, d.gpl, c->ang, c->geo};
+    c->launches++;
+    if (d.Q % 2 == 0) return bp_launch<2>(c, gt, f_out, a);
+    return bp_launch<1>(c, gt, f_out, a);
+}
+
+}  // namespace cp4d

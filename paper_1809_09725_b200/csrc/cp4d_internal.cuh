@@ -13,6 +13,7 @@ namespace cp4d {
 constexpr int TILE = 32;          // voxel tile side of both projector kernels
 constexpr int WIN = 48;           // bins a TILE x TILE tile can touch at one angle: floor(31*sqrt2)+4
 constexpr int MAX_M = 32;
+constexpr int BP_NPAT = 9;       // bin-offset patterns of a 4x2 voxel patch (backproject.cu)
 
 // per (tile, base angle) geometry, computed in fp64 on the host at create:
 // bin coordinate of tile-local voxel (lx, ly) relative to the window start is  delta + lx*c + ly*s.
@@ -25,6 +26,8 @@ struct TileGeo {
 struct AngleTab {
     float c, s, inv_a;  // cos, sin, 1/max(|c|,|s|)
     int32_t col_step;   // 1: |s| >= |c| (ray steps over columns ix), 0: steps over rows iy
+    int32_t pat;        // backprojection patch pattern, bp_pattern(c, s)
+    uint32_t pat_fl;    // its 8 bin offsets FL_v, 4 bits each
 };
 
 struct Dims {
@@ -32,7 +35,8 @@ struct Dims {
     int tiles_1d, tiles;               // ceil(n/TILE), tiles_1d^2
     int64_t V, S;                      // elements of a primal array / a sinogram
     int64_t slice4;                    // float4 per slice: n*n*Q
-    int64_t scratch4;                  // float4 of projector scratch: nz*n0*Q*nd
+    int gp, gpl;                       // row pitch / left pad (float4) of the projector scratch: a row holds bins -gpl .. gp-gpl-1
+    int64_t scratch4;                  // float4 of projector scratch: nz*n0*Q*gp
 };
 
 }  // namespace cp4d
@@ -46,7 +50,8 @@ struct cp4d_ctx {
     cudaStream_t stream;
     // workspace carve-up (device pointers)
     float *f, *ft, *bp, *h2, *h1, *g;
-    float4 *scratch;           // forward partial ray sums P / folded sinogram gt: [z][i][jc][b] float4
+    float4 *scratch;           // forward partial ray sums P / folded sinogram gt: [z][i][jc][gpl + b] float4, pitch gp;
+                               // the pads stay zero, so every tile window of the backprojector is readable memory
     float *phi;                // [j][k]
     cp4d::AngleTab *ang;       // [n0]
     cp4d::TileGeo *geo;        // [tile][n0]
@@ -95,6 +100,8 @@ cudaError_t launch_fold(cp4d_ctx *c, const float *g, float4 *gt);
 cudaError_t launch_synth(cp4d_ctx *c, const float4 *P, int mode, float sigma, const float *g, float *out);
 cudaError_t launch_forward_partial(cp4d_ctx *c, const float *f, float4 *P);
 cudaError_t launch_backproject(cp4d_ctx *c, const float4 *gt, float *f_out);
+int bp_pattern(float c, float s);  // host: pattern index in [0, BP_NPAT) or -1
+uint32_t bp_pattern_fl(int pat);   // host: the pattern's FL_v packed 4 bits each
 cudaError_t launch_sumsq_dot(cp4d_ctx *c, const float *x, const float *y, uint64_t n, double *slot);
 cudaError_t launch_fill_normal(cp4d_ctx *c, float *x, uint64_t n, uint64_t seed);
 // x = (a - b) * scale   (b nullable)

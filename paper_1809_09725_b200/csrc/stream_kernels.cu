@@ -174,7 +174,7 @@ cudaError_t launch_update(cp4d_ctx *c, float tau, const float *bp, const float *
 // ---------------------------------------------------------------------------------------------------
 template <int Q>
 __global__ void __launch_bounds__(128) k_fold(const float *__restrict__ g, float4 *__restrict__ gt,
-                                              const float *__restrict__ phi, int nd, int na, int npi, int n0) {
+                                              const float *__restrict__ phi, int nd, int na, int npi, int n0, int gp, int gpl) {
     extern __shared__ float phis[];  // [q][j]
     const int z = blockIdx.x / n0, i = blockIdx.x % n0;
     constexpr int m = 4 * Q;
@@ -192,14 +192,14 @@ __global__ void __launch_bounds__(128) k_fold(const float *__restrict__ g, float
         }
 #pragma unroll
         for (int jc = 0; jc < Q; ++jc)
-            gt[(((int64_t)z * n0 + i) * Q + jc) * nd + b] = make_float4(acc[4 * jc], acc[4 * jc + 1], acc[4 * jc + 2], acc[4 * jc + 3]);
+            gt[(((int64_t)z * n0 + i) * Q + jc) * gp + gpl + b] = make_float4(acc[4 * jc], acc[4 * jc + 1], acc[4 * jc + 2], acc[4 * jc + 3]);
     }
 }
 
 template <int Q>
 __global__ void __launch_bounds__(128) k_synth(const float4 *__restrict__ P, int mode, float sigma,
                                                const float *__restrict__ g, float *__restrict__ out,
-                                               const float *__restrict__ phi, int nd, int na, int npi, int n0) {
+                                               const float *__restrict__ phi, int nd, int na, int npi, int n0, int gp, int gpl) {
     extern __shared__ float phis[];
     const int z = blockIdx.x / n0, i = blockIdx.x % n0;
     constexpr int m = 4 * Q;
@@ -210,7 +210,7 @@ __global__ void __launch_bounds__(128) k_synth(const float4 *__restrict__ P, int
         float acc[m];
 #pragma unroll
         for (int jc = 0; jc < Q; ++jc) {
-            const float4 v = P[(((int64_t)z * n0 + i) * Q + jc) * nd + b];
+            const float4 v = P[(((int64_t)z * n0 + i) * Q + jc) * gp + gpl + b];
             acc[4 * jc] = v.x; acc[4 * jc + 1] = v.y; acc[4 * jc + 2] = v.z; acc[4 * jc + 3] = v.w;
         }
         for (int q = 0; q < npi; ++q) {
@@ -241,7 +241,7 @@ cudaError_t launch_fold(cp4d_ctx *c, const float *g, float4 *gt) {
     ProfScope ps(c, CP4D_K_FOLD);
     const Dims &d = c->d;
     const size_t sh = (size_t)d.npi * d.m * sizeof(float);
-    CP4D_DISPATCH_Q(d.Q, (k_fold<QQ><<<d.nz * d.n0, 128, sh, c->stream>>>(g, gt, c->phi, d.nd, d.na, d.npi, d.n0)));
+    CP4D_DISPATCH_Q(d.Q, (k_fold<QQ><<<d.nz * d.n0, 128, sh, c->stream>>>(g, gt, c->phi, d.nd, d.na, d.npi, d.n0, d.gp, d.gpl)));
     c->launches++;
     return cudaGetLastError();
 }
@@ -249,7 +249,7 @@ cudaError_t launch_synth(cp4d_ctx *c, const float4 *P, int mode, float sigma, co
     ProfScope ps(c, CP4D_K_SYNTH);
     const Dims &d = c->d;
     const size_t sh = (size_t)d.npi * d.m * sizeof(float);
-    CP4D_DISPATCH_Q(d.Q, (k_synth<QQ><<<d.nz * d.n0, 128, sh, c->stream>>>(P, mode, sigma, g, out, c->phi, d.nd, d.na, d.npi, d.n0)));
+    CP4D_DISPATCH_Q(d.Q, (k_synth<QQ><<<d.nz * d.n0, 128, sh, c->stream>>>(P, mode, sigma, g, out, c->phi, d.nd, d.na, d.npi, d.n0, d.gp, d.gpl)));
     c->launches++;
     return cudaGetLastError();
 }
