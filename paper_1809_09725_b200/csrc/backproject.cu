@@ -68,11 +68,12 @@ __device__ __forceinline__ void bulk_g2s(void *dst_smem, const void *src_gmem, u
                  "l"(src_gmem), "r"(bytes), "r"(smem_u32(bar)) : "memory");
 }
 
-template <int PAT, int V, int JQ, int NB>
-__device__ __forceinline__ void bp_voxel(float4 (&acc)[8][JQ], const float4 (&B)[NB][JQ], float phi, float td,
+template <int PAT, int V, bool NEG, int JQ, int NB>
+__device__ __forceinline__ void bp_voxel(float4 (&acc)[8][JQ], const float4 (&B)[NB][JQ], float phi, const float (&tdv)[8],
                                          float A1, float A2, float A3) {
-    constexpr int FL = bp_fl(PAT, V);
-    const float t = phi + td;                                                  // in [0,2)
+    // accumulator V is voxel (dx, dy) = (V & 3, V >> 2); for c < 0 its offset from the patch minimum is that of e = 3 - dx
+    constexpr int E = (NEG ? 3 - (V & 3) : (V & 3)) + (V & 4), FL = bp_fl(PAT, E);
+    const float t = phi + tdv[E];                                                 // in [0,2)
     const float x0 = fmaxf(0.f, fmaf(-A2, t, A1));
     const float x1 = fmaxf(0.f, fmaf(-A2, fabsf(t - 1.0f), A1));
     const float x2 = fmaxf(0.f, fmaf(A2, t, A3));                              // A3 = A1 - 2 A2
@@ -85,7 +86,7 @@ __device__ __forceinline__ void bp_voxel(float4 (&acc)[8][JQ], const float4 (&B)
     }
 }
 
-template <int PAT, int JQ>
+template <int PAT, bool NEG, int JQ>
 __device__ __forceinline__ void bp_angle(float4 (&acc)[8][JQ], const float4 *wbase, float phi, const float4 tda,
                                          const float4 tdb, float A1, float A2, float A3) {
     constexpr int NB = bp_nb(PAT);
@@ -94,14 +95,15 @@ __device__ __forceinline__ void bp_angle(float4 (&acc)[8][JQ], const float4 *wba
     for (int k = 0; k < NB; ++k)
 #pragma unroll
         for (int jc = 0; jc < JQ; ++jc) B[k][jc] = wbase[jc * WINP + k];
-    bp_voxel<PAT, 0, JQ, NB>(acc, B, phi, tda.x, A1, A2, A3);
-    bp_voxel<PAT, 1, JQ, NB>(acc, B, phi, tda.y, A1, A2, A3);
-    bp_voxel<PAT, 2, JQ, NB>(acc, B, phi, tda.z, A1, A2, A3);
-    bp_voxel<PAT, 3, JQ, NB>(acc, B, phi, tda.w, A1, A2, A3);
-    bp_voxel<PAT, 4, JQ, NB>(acc, B, phi, tdb.x, A1, A2, A3);
-    bp_voxel<PAT, 5, JQ, NB>(acc, B, phi, tdb.y, A1, A2, A3);
-    bp_voxel<PAT, 6, JQ, NB>(acc, B, phi, tdb.z, A1, A2, A3);
-    bp_voxel<PAT, 7, JQ, NB>(acc, B, phi, tdb.w, A1, A2, A3);
+    const float tdv[8] = {tda.x, tda.y, tda.z, tda.w, tdb.x, tdb.y, tdb.z, tdb.w};
+    bp_voxel<PAT, 0, NEG, JQ, NB>(acc, B, phi, tdv, A1, A2, A3);
+    bp_voxel<PAT, 1, NEG, JQ, NB>(acc, B, phi, tdv, A1, A2, A3);
+    bp_voxel<PAT, 2, NEG, JQ, NB>(acc, B, phi, tdv, A1, A2, A3);
+    bp_voxel<PAT, 3, NEG, JQ, NB>(acc, B, phi, tdv, A1, A2, A3);
+    bp_voxel<PAT, 4, NEG, JQ, NB>(acc, B, phi, tdv, A1, A2, A3);
+    bp_voxel<PAT, 5, NEG, JQ, NB>(acc, B, phi, tdv, A1, A2, A3);
+    bp_voxel<PAT, 6, NEG, JQ, NB>(acc, B, phi, tdv, A1, A2, A3);
+    bp_voxel<PAT, 7, NEG, JQ, NB>(acc, B, phi, tdv, A1, A2, A3);
 }
 
 }  // namespace
@@ -170,18 +172,6 @@ __global__ void __launch_bounds__(BP_THREADS, 3) k_backproject(const float4 *__r
     for (int v = 0; v < 8; ++v)
 #pragma unroll
         for (int jc = 0; jc < JQ; ++jc) acc[v][jc] = make_float4(0.f, 0.f, 0.f, 0.f);
-    bool flipped = false;
-    auto flip = [&]() {
-#pragma unroll
-        for (int dy = 0; dy < 2; ++dy)
-#pragma unroll
-            for (int jc = 0; jc < JQ; ++jc) {
-                float4 t0 = acc[4 * dy + 0][jc]; acc[4 * dy + 0][jc] = acc[4 * dy + 3][jc]; acc[4 * dy + 3][jc] = t0;
-                float4 t1 = acc[4 * dy + 1][jc]; acc[4 * dy + 1][jc] = acc[4 * dy + 2][jc]; acc[4 * dy + 2][jc] = t1;
-            }
-        flipped = !flipped;
-    };
-
     if (threadIdx.x == 0) {
         mbar_init(&mbar[0], 1);
         mbar_init(&mbar[1], 1);
@@ -200,26 +190,34 @@ __global__ void __launch_bounds__(BP_THREADS, 3) k_backproject(const float4 *__r
             const BpAngle &S = sang[buf][aa];
             const float4 G = S.g, K = S.k;
             const bool neg = G.y < 0.f;
-            if (neg != flipped) flip();
             const float umin = fmaf(fx0 + (neg ? 3.0f : 0.0f), G.y, fmaf(fy0, G.z, G.x));
             const float fk = floorf(umin);
             const float phi = umin - fk;
             const float4 *wbase = &win[buf][aa][0][(int)fk];
-            switch (__float_as_int(K.w)) {
-            case 0: bp_angle<0, JQ>(acc, wbase, phi, S.tda, S.tdb, K.x, K.y, K.z); break;
-            case 1: bp_angle<1, JQ>(acc, wbase, phi, S.tda, S.tdb, K.x, K.y, K.z); break;
-            case 2: bp_angle<2, JQ>(acc, wbase, phi, S.tda, S.tdb, K.x, K.y, K.z); break;
-            case 3: bp_angle<3, JQ>(acc, wbase, phi, S.tda, S.tdb, K.x, K.y, K.z); break;
-            case 4: bp_angle<4, JQ>(acc, wbase, phi, S.tda, S.tdb, K.x, K.y, K.z); break;
-            case 5: bp_angle<5, JQ>(acc, wbase, phi, S.tda, S.tdb, K.x, K.y, K.z); break;
-            case 6: bp_angle<6, JQ>(acc, wbase, phi, S.tda, S.tdb, K.x, K.y, K.z); break;
-            case 7: bp_angle<7, JQ>(acc, wbase, phi, S.tda, S.tdb, K.x, K.y, K.z); break;
-            default: bp_angle<8, JQ>(acc, wbase, phi, S.tda, S.tdb, K.x, K.y, K.z); break;
+            switch (__float_as_int(K.w) + (neg ? BP_NPAT : 0)) {
+            case 0: bp_angle<0, false, JQ>(acc, wbase, phi, S.tda, S.tdb, K.x, K.y, K.z); break;
+            case 1: bp_angle<1, false, JQ>(acc, wbase, phi, S.tda, S.tdb, K.x, K.y, K.z); break;
+            case 2: bp_angle<2, false, JQ>(acc, wbase, phi, S.tda, S.tdb, K.x, K.y, K.z); break;
+            case 3: bp_angle<3, false, JQ>(acc, wbase, phi, S.tda, S.tdb, K.x, K.y, K.z); break;
+            case 4: bp_angle<4, false, JQ>(acc, wbase, phi, S.tda, S.tdb, K.x, K.y, K.z); break;
+            case 5: bp_angle<5, false, JQ>(acc, wbase, phi, S.tda, S.tdb, K.x, K.y, K.z); break;
+            case 6: bp_angle<6, false, JQ>(acc, wbase, phi, S.tda, S.tdb, K.x, K.y, K.z); break;
+            case 7: bp_angle<7, false, JQ>(acc, wbase, phi, S.tda, S.tdb, K.x, K.y, K.z); break;
+            case 8: bp_angle<8, false, JQ>(acc, wbase, phi, S.tda, S.tdb, K.x, K.y, K.z); break;
+            case 9: bp_angle<0, true, JQ>(acc, wbase, phi, S.tda, S.tdb, K.x, K.y, K.z); break;
+            case 10: bp_angle<1, true, JQ>(acc, wbase, phi, S.tda, S.tdb, K.x, K.y, K.z); break;
+            case 11: bp_angle<2, true, JQ>(acc, wbase, phi, S.tda, S.tdb, K.x, K.y, K.z); break;
+            case 12: bp_angle<3, true, JQ>(acc, wbase, phi, S.tda, S.tdb, K.x, K.y, K.z); break;
+            case 13: bp_angle<4, true, JQ>(acc, wbase, phi, S.tda, S.tdb, K.x, K.y, K.z); break;
+            case 14: bp_angle<5, true, JQ>(acc, wbase, phi, S.tda, S.tdb, K.x, K.y, K.z); break;
+            case 15: bp_angle<6, true, JQ>(acc, wbase, phi, S.tda, S.tdb, K.x, K.y, K.z); break;
+            case 16: bp_angle<7, true, JQ>(acc, wbase, phi, S.tda, S.tdb, K.x, K.y, K.z); break;
+            case 17: bp_angle<8, true, JQ>(acc, wbase, phi, S.tda, S.tdb, K.x, K.y, K.z); break;
+            default: break;
             }
         }
         __syncthreads();
     }
-    if (flipped) flip();
     float4 *O = reinterpret_cast<float4 *>(out);
 #pragma unroll
     for (int v = 0; v < 8; ++v) {
