@@ -123,7 +123,7 @@ struct BpAngle {
 };
 
 template <int JQ>
-__global__ void __launch_bounds__(BP_THREADS, 3) k_backproject(const float4 *__restrict__ gt, float *__restrict__ out, BpArgs a) {
+__global__ void __launch_bounds__(BP_THREADS, 4) k_backproject(const float4 *__restrict__ gt, float *__restrict__ out, BpArgs a) {
     __shared__ __align__(128) float4 win[2][BP_CHUNK][JQ][WINP];
     __shared__ BpAngle sang[2][BP_CHUNK];
     __shared__ __align__(8) uint64_t mbar[2];
