@@ -327,10 +327,13 @@ def assemble(args, c, world, r):
                 "frac": d["frac"], "traffic": None, "peak_source": peaks["source"], "avg_launch_ms": d["ms"],
                 "note": ("alu peak = 148 SM x 128 FP32 lanes x 2 flop x sm_max_mhz; achieved = algorithmic (pi-folded) flops"
                          if d["bound"] == "alu" else "algorithmic bytes / CUDA-event time")}
-    tr = ROOT / "profiles" / "traffic.json"                  # dram bytes per launch from the committed ncu capture
+    tr = ROOT / "profiles" / "traffic.json"                  # dram bytes per launch from the committed ncu --set full capture
     if tr.exists():
         try:
-            roofline["traffic"] = json.loads(tr.read_text()).get(synth.describe(c), {}).get(dom)
+            per_kernel = json.loads(tr.read_text()).get(synth.describe(c), {})
+            roofline["traffic"] = per_kernel.get(dom)
+            for n, k in kernels.items():
+                k["traffic"] = per_kernel.get(n)
         except Exception:
             pass
     gups = {n: c.nominal_updates / (r["ops"][n + "_op"] * 1e-3) / 1e9 for n in ("forward", "adjoint")}
