@@ -79,6 +79,23 @@ def algorithmic_work(c):
     }
 
 
+def reduce_max(value: float, world: int, device="cpu") -> float:
+    """MAX over ranks of a per-rank time (the contract: multi-GPU numbers are the slowest rank's).  Uses the
+    initialised torch.distributed group (nccl on GPU boxes, gloo in the CPU tests); identity when world == 1."""
+    if world <= 1:
+        return float(value)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([float(value)], device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def replicas_value(world: int, steps: int, ms_max: float) -> float:
+    """Whole-job it/s of `world` independent replicas ("replicas only"): all ranks' steps / slowest rank's time."""
+    return world * steps / (ms_max * 1e-3)
+
+
 class ClockSampler:
     """nvidia-smi clocks + throttle reasons every 200 ms during the timed region (B200_PROFILING.md recipe)."""
     Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
@@ -250,10 +267,7 @@ def run_cp4d(args, c, rank, world):
     ctx.iterate(K)
     prof = ctx.profile_end()
     clocks = sampler.stop(t0, time.perf_counter())
-    if world > 1:
-        t = torch.tensor([ms], device=dev, dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
+    ms = reduce_max(ms, world, dev)
 
     # ---- standalone operators (grad/div are not launched by the fused iteration) ----
     f_t, g_t = ctx.empty_primal().normal_(), ctx.empty_sino().normal_()
@@ -286,10 +300,7 @@ def run_cp4d(args, c, rank, world):
         ctx.solve_host(g_host, K, f_host)                 # syncs before returning
         w1 = time.perf_counter()
         dt = w1 - w0
-        if world > 1:
-            t = torch.tensor([dt], device=dev, dtype=torch.float64)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            dt = float(t.item())
+        dt = reduce_max(dt, world, dev)
         e2e = {"value": world * K / dt, "unit": UNIT, "h2d_bytes_per_step": c.S * 4 / K, "d2h_bytes_per_step": c.V * 4 / K,
                "call": f"cp4d_solve_host(g_host, {K}, f_host): H2D {c.S * 4} B + reset + {K} iterations + D2H {c.V * 4} B, pinned host memory",
                "seconds": dt}
@@ -339,7 +350,7 @@ def assemble(args, c, world, r):
     gups = {n: c.nominal_updates / (r["ops"][n + "_op"] * 1e-3) / 1e9 for n in ("forward", "adjoint")}
     ms_step = r["ms"] / K
     line = {
-        "metric": METRIC, "value": world * K / (r["ms"] * 1e-3), "unit": UNIT, "n_gpus": world, "steps": K,
+        "metric": METRIC, "value": replicas_value(world, K, r["ms"]), "unit": UNIT, "n_gpus": world, "steps": K,
         "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f32", "data": "synthetic",
         "config": {"workload": synth.describe(c), "cfg": c.cfg, "n": c.n, "nz": c.nz, "nd": c.nd, "n_angles": c.n_angles,
