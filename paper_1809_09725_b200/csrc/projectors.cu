@@ -118,6 +118,93 @@ __global__ void __launch_bounds__(256) k_forward_partial(const float *__restrict
     }
 }
 
+
+// ---------------------------------------------------------------------------------------------------
+// forward, 16 coefficients per ray (m % 16 == 0): 8 lanes per ray, conflict-free shared-memory wavefronts
+// ---------------------------------------------------------------------------------------------------
+// The one-thread-per-ray kernel above is bound by shared-memory wavefronts, a third of which are bank conflicts (8 adjacent
+// rays span up to 10 rows, rows 8 apart share a bank group) or partially filled.  Here a ray is served by 8 lanes
+// = 2 step parities x 4 coefficient chunks: the tile is stored voxel-major ([row][col][16 coefficients], 64 B per voxel,
+// EVEN row pitch), lane (sp, jq) handles steps k = sp, sp+2, ... and chunk jq.  The 8 lanes of a quarter warp then read two
+// whole voxels, (r0, k) and (r1, k+1), whose 64 B blocks always differ in parity ((r1-r0)*pitch + 1 is odd): one full,
+// conflict-free 128 B wavefront per LDS.128.  Rays that step over rows use a second pass over a transposed copy of the tile,
+// so both passes run the same code.  The two step parities are summed with one shuffle before the vector RED into P.
+constexpr int FR_RAYS = WIN;                 // rays of a tile window
+constexpr int FR_THREADS = FR_RAYS * 8;      // 384
+constexpr int RSV = TILE + 2;                // voxels per tile row incl. the zero border; even
+static_assert(RSV % 2 == 0, "row pitch must be even for conflict-free step pairs");
+
+__global__ void __launch_bounds__(FR_THREADS, 3) k_forward_rays16(const float *__restrict__ f, float4 *__restrict__ P, ProjArgs a) {
+    extern __shared__ float4 tile[];  // [TILE+2][RSV][4], 1-voxel zero border
+    const int tiles_1d = (a.n + TILE - 1) / TILE;
+    const int tix = blockIdx.x % tiles_1d, tiy = blockIdx.x / tiles_1d;
+    const int z = blockIdx.y, jg = blockIdx.z;
+    const int x0 = tix * TILE, y0 = tiy * TILE;
+    const int u = threadIdx.x >> 3, sp = (threadIdx.x >> 2) & 1, jq = threadIdx.x & 3;
+    const float4 zero = make_float4(0.f, 0.f, 0.f, 0.f);
+    const float4 *F = reinterpret_cast<const float4 *>(f);
+    const TileGeo *geo = a.geo + (int64_t)blockIdx.x * a.n0;
+
+    for (int pass = 0; pass < 2; ++pass) {   // pass 0: rays stepping over columns; pass 1: over rows, on the transposed tile
+        __syncthreads();
+        for (int t = threadIdx.x; t < (TILE + 2) * RSV * 4; t += FR_THREADS) tile[t] = zero;
+        __syncthreads();
+        for (int t = threadIdx.x; t < TILE * TILE * 4; t += FR_THREADS) {
+            const int jc = t & 3, lx = (t >> 2) & (TILE - 1), ly = t >> 7;
+            const int gx = x0 + lx, gy = y0 + ly;
+            if (gx < a.n && gy < a.n) {
+                const int row = pass ? lx : ly, col = pass ? ly : lx;
+                tile[((row + 1) * RSV + col + 1) * 4 + jc] = __ldg(F + (((int64_t)z * a.n + gy) * a.n + gx) * a.Q + jg * 4 + jc);
+            }
+        }
+        __syncthreads();
+        for (int i = 0; i < a.n0; ++i) {
+            const AngleTab A = a.ang[i];
+            if ((A.col_step != 0) != (pass == 0)) continue;
+            const TileGeo G = geo[i];
+            // pass 0: the ray crosses column k at row (du - k c)/s; pass 1: it crosses row k at column (du - k s)/c
+            const float cc = pass ? A.s : A.c, ss = pass ? A.c : A.s;
+            const float inv = 1.0f / ss, step = -cc * inv, base = ((float)u - G.delta) * inv;
+            float4 acc = zero;
+            bool touched = false;
+#pragma unroll 4
+            for (int k = sp; k < TILE; k += 2) {
+                const float ys = fmaf((float)k, step, base);
+                const float fl = floorf(ys);
+                const int r = (int)fl;
+                if ((unsigned)(r + 1) <= (unsigned)TILE) {
+                    const float w1 = ys - fl, w0 = 1.0f - w1;
+                    const float4 *p0 = tile + ((r + 1) * RSV + k + 1) * 4 + jq;
+                    const float4 t0 = p0[0], t1 = p0[RSV * 4];
+                    fma4(acc, w0, t0);
+                    fma4(acc, w1, t1);
+                    touched = true;
+                }
+            }
+            // sum the two step parities (lanes l and l^4 serve the same ray and chunk)
+            acc.x += __shfl_xor_sync(0xffffffffu, acc.x, 4);
+            acc.y += __shfl_xor_sync(0xffffffffu, acc.y, 4);
+            acc.z += __shfl_xor_sync(0xffffffffu, acc.z, 4);
+            acc.w += __shfl_xor_sync(0xffffffffu, acc.w, 4);
+            touched = __shfl_xor_sync(0xffffffffu, (int)touched, 4) || touched;
+            const int b = G.bstart + u;
+            if (sp == 0 && touched && b >= 0 && b < a.nd) {
+                float4 *dst = P + (((int64_t)z * a.n0 + i) * a.Q + jg * 4 + jq) * a.gp + a.gpl + b;
+                atomicAdd(dst, make_float4(acc.x * A.inv_a, acc.y * A.inv_a, acc.z * A.inv_a, acc.w * A.inv_a));
+            }
+        }
+    }
+}
+
+static cudaError_t fwd_launch_rays16(cp4d_ctx *c, const float *f, float4 *P, const ProjArgs &a) {
+    const Dims &d = c->d;
+    const size_t sh = (size_t)(TILE + 2) * RSV * 4 * sizeof(float4);
+    cudaError_t e = cudaFuncSetAttribute(k_forward_rays16, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sh);
+    if (e != cudaSuccess) return e;
+    k_forward_rays16<<<dim3(d.tiles, d.nz, d.Q / 4), FR_THREADS, sh, c->stream>>>(f, P, a);
+    return cudaGetLastError();
+}
+
 static int pick_jq(int Q) { return (Q % 4 == 0) ? 4 : (Q % 2 == 0) ? 2 : 1; }
 
 template <int JQ>
@@ -138,7 +225,7 @@ cudaError_t launch_forward_partial(cp4d_ctx *c, const float *f, float4 *P) {
     if (e != cudaSuccess) return e;
     c->launches += 2;
     switch (pick_jq(d.Q)) {
-    case 4: return fwd_launch<4>(c, f, P, a);
+    case 4: return fwd_launch_rays16(c, f, P, a);
     case 2: return fwd_launch<2>(c, f, P, a);
     default: return fwd_launch<1>(c, f, P, a);
     }
