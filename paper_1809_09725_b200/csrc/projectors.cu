@@ -165,20 +165,39 @@ __global__ void __launch_bounds__(FR_THREADS, 3) k_forward_rays16(const float *_
             // pass 0: the ray crosses column k at row (du - k c)/s; pass 1: it crosses row k at column (du - k s)/c
             const float cc = pass ? A.s : A.c, ss = pass ? A.c : A.s;
             const float inv = 1.0f / ss, step = -cc * inv, base = ((float)u - G.delta) * inv;
+            // steps k with -1 <= base + k step < TILE (one extra on each side; the body is exact on its own)
+            int klo = 0, khi = TILE - 1;
+            if (fabsf(step) > 1e-6f) {
+                const float is = 1.0f / step, ta = (-1.0f - base) * is, tb = ((float)TILE - base) * is;
+                klo = max(0, (int)floorf(fminf(ta, tb)));
+                khi = min(TILE - 1, (int)ceilf(fmaxf(ta, tb)));
+            } else if (!(base >= -1.0f && base < (float)TILE)) {
+                klo = TILE; khi = -1;
+            }
+            const bool touched = klo <= khi;
+            const int klo_w = __reduce_min_sync(0xffffffffu, touched ? klo : TILE);
+            const int khi_w = __reduce_max_sync(0xffffffffu, touched ? khi : -1);
             float4 acc = zero;
-            bool touched = false;
-#pragma unroll 4
-            for (int k = sp; k < TILE; k += 2) {
-                const float ys = fmaf((float)k, step, base);
-                const float fl = floorf(ys);
-                const int r = (int)fl;
-                if ((unsigned)(r + 1) <= (unsigned)TILE) {
-                    const float w1 = ys - fl, w0 = 1.0f - w1;
-                    const float4 *p0 = tile + ((r + 1) * RSV + k + 1) * 4 + jq;
-                    const float4 t0 = p0[0], t1 = p0[RSV * 4];
-                    fma4(acc, w0, t0);
-                    fma4(acc, w1, t1);
-                    touched = true;
+            // floor without the conversion pipe: rf = rn(ys - 1/2) by the 1.5 * 2^23 trick; any integer r with ys - r in [0,1]
+            // gives the same Joseph sample (w1 = 1 on row r equals w1 = 0 on row r+1)
+            const float MAGIC = 12582912.0f;
+            const float bh = base - 0.5f;
+            const float4 *plane = tile + jq + 4;          // + 4: column k lives at tile column k+1
+            for (int kc = klo_w & ~7; kc <= khi_w; kc += 8) {
+                const float t0 = fmaf((float)(kc + sp), step, bh);
+                const float4 *pc = plane + (kc + sp) * 4;
+#pragma unroll
+                for (int j = 0; j < 4; ++j) {
+                    const float t = fmaf((float)(2 * j), step, t0);         // ys - 1/2 at step k = kc + sp + 2j
+                    const float tm = t + MAGIC;
+                    const float d = t - (tm - MAGIC);                       // in [-1/2, 1/2]
+                    const int row = __float_as_int(tm) - (0x4B400000 - 1);  // floor + 1 = tile row of the first tap
+                    const bool ok = (unsigned)row <= (unsigned)TILE;
+                    const float w1 = ok ? d + 0.5f : 0.0f, w0 = ok ? 0.5f - d : 0.0f;
+                    const float4 *p0 = pc + (ok ? row : 0) * (RSV * 4) + j * 8;
+                    const float4 v0 = p0[0], v1 = p0[RSV * 4];
+                    fma4(acc, w0, v0);
+                    fma4(acc, w1, v1);
                 }
             }
             // sum the two step parities (lanes l and l^4 serve the same ray and chunk)
@@ -186,7 +205,6 @@ __global__ void __launch_bounds__(FR_THREADS, 3) k_forward_rays16(const float *_
             acc.y += __shfl_xor_sync(0xffffffffu, acc.y, 4);
             acc.z += __shfl_xor_sync(0xffffffffu, acc.z, 4);
             acc.w += __shfl_xor_sync(0xffffffffu, acc.w, 4);
-            touched = __shfl_xor_sync(0xffffffffu, (int)touched, 4) || touched;
             const int b = G.bstart + u;
             if (sp == 0 && touched && b >= 0 && b < a.nd) {
                 float4 *dst = P + (((int64_t)z * a.n0 + i) * a.Q + jg * 4 + jq) * a.gp + a.gpl + b;
