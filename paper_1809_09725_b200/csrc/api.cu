@@ -150,6 +150,11 @@ int cp4d_create(const cp4d_params *p, cp4d_ctx **out) {
         ang[i].c = (float)c; ang[i].s = (float)s;
         ang[i].inv_a = (float)(1.0 / std::fmax(std::fabs(c), std::fabs(s)));
         ang[i].col_step = std::fabs(s) >= std::fabs(c) ? 1 : 0;
+        {
+            const double cc = ang[i].col_step ? c : s, ss = ang[i].col_step ? s : c, st = -cc / ss;
+            ang[i].fw_inv = (float)(1.0 / ss); ang[i].fw_step = (float)st;
+            ang[i].fw_istep = std::fabs(st) < 1e-6 ? 0.0f : (float)(1.0 / st);
+        }
         ang[i].pat = bp_pattern(ang[i].c, ang[i].s);
         if (ang[i].pat < 0) { delete ctx; return CP4D_EINVAL; }
         ang[i].pat_fl = bp_pattern_fl(ang[i].pat);

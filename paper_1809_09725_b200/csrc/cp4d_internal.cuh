@@ -28,6 +28,9 @@ struct AngleTab {
     int32_t col_step;   // 1: |s| >= |c| (ray steps over columns ix), 0: steps over rows iy
     int32_t pat;        // backprojection patch pattern, bp_pattern(c, s)
     uint32_t pat_fl;    // its 8 bin offsets FL_v, 4 bits each
+    // forward projector, dominant-axis stepping: the ray with window coordinate du crosses step k at (du - k cc)/ss,
+    // (cc, ss) = (c, s) when col_step else (s, c)
+    float fw_inv, fw_step, fw_istep;  // 1/ss, -cc/ss, 1/fw_step (0 when |fw_step| < 1e-6), rounded from fp64
 };
 
 struct Dims {

@@ -135,7 +135,7 @@ constexpr int RSV = TILE + 2;                // voxels per tile row incl. the ze
 static_assert(RSV % 2 == 0, "row pitch must be even for conflict-free step pairs");
 
 __global__ void __launch_bounds__(FR_THREADS, 3) k_forward_rays16(const float *__restrict__ f, float4 *__restrict__ P, ProjArgs a) {
-    extern __shared__ float4 tile[];  // [TILE+2][RSV][4], 1-voxel zero border
+    extern __shared__ float4 tile[];  // [TILE+3][RSV][4]: 1-voxel zero border, plus a second zero row at the bottom
     const int tiles_1d = (a.n + TILE - 1) / TILE;
     const int tix = blockIdx.x % tiles_1d, tiy = blockIdx.x / tiles_1d;
     const int z = blockIdx.y, jg = blockIdx.z;
@@ -147,7 +147,7 @@ __global__ void __launch_bounds__(FR_THREADS, 3) k_forward_rays16(const float *_
 
     for (int pass = 0; pass < 2; ++pass) {   // pass 0: rays stepping over columns; pass 1: over rows, on the transposed tile
         __syncthreads();
-        for (int t = threadIdx.x; t < (TILE + 2) * RSV * 4; t += FR_THREADS) tile[t] = zero;
+        for (int t = threadIdx.x; t < (TILE + 3) * RSV * 4; t += FR_THREADS) tile[t] = zero;
         __syncthreads();
         for (int t = threadIdx.x; t < TILE * TILE * 4; t += FR_THREADS) {
             const int jc = t & 3, lx = (t >> 2) & (TILE - 1), ly = t >> 7;
@@ -163,38 +163,33 @@ __global__ void __launch_bounds__(FR_THREADS, 3) k_forward_rays16(const float *_
             if ((A.col_step != 0) != (pass == 0)) continue;
             const TileGeo G = geo[i];
             // pass 0: the ray crosses column k at row (du - k c)/s; pass 1: it crosses row k at column (du - k s)/c
-            const float cc = pass ? A.s : A.c, ss = pass ? A.c : A.s;
-            const float inv = 1.0f / ss, step = -cc * inv, base = ((float)u - G.delta) * inv;
-            // steps k with -1 <= base + k step < TILE (one extra on each side; the body is exact on its own)
+            const float step = A.fw_step, base = ((float)u - G.delta) * A.fw_inv;
+            // this ray's steps k with -1 <= base + k step < TILE (one extra on each side; the body is exact on its own)
             int klo = 0, khi = TILE - 1;
-            if (fabsf(step) > 1e-6f) {
-                const float is = 1.0f / step, ta = (-1.0f - base) * is, tb = ((float)TILE - base) * is;
+            if (A.fw_istep != 0.0f) {
+                const float ta = (-1.0f - base) * A.fw_istep, tb = ((float)TILE - base) * A.fw_istep;
                 klo = max(0, (int)floorf(fminf(ta, tb)));
                 khi = min(TILE - 1, (int)ceilf(fmaxf(ta, tb)));
             } else if (!(base >= -1.0f && base < (float)TILE)) {
                 klo = TILE; khi = -1;
             }
             const bool touched = klo <= khi;
-            const int klo_w = __reduce_min_sync(0xffffffffu, touched ? klo : TILE);
-            const int khi_w = __reduce_max_sync(0xffffffffu, touched ? khi : -1);
             float4 acc = zero;
-            // floor without the conversion pipe: rf = rn(ys - 1/2) by the 1.5 * 2^23 trick; any integer r with ys - r in [0,1]
-            // gives the same Joseph sample (w1 = 1 on row r equals w1 = 0 on row r+1)
+            // floor without the conversion pipe: tm = ys + 1.5 * 2^23 rounded DOWN holds floor(ys) in its low mantissa bits
             const float MAGIC = 12582912.0f;
-            const float bh = base - 0.5f;
             const float4 *plane = tile + jq + 4;          // + 4: column k lives at tile column k+1
-            for (int kc = klo_w & ~7; kc <= khi_w; kc += 8) {
-                const float t0 = fmaf((float)(kc + sp), step, bh);
+            // per-ray chunk range: lanes of other rays in the warp are masked off, so no wavefront is spent outside the chord
+            for (int kc = klo & ~7; kc <= khi; kc += 8) {
+                const float y0s = fmaf((float)(kc + sp), step, base);
                 const float4 *pc = plane + (kc + sp) * 4;
 #pragma unroll
                 for (int j = 0; j < 4; ++j) {
-                    const float t = fmaf((float)(2 * j), step, t0);         // ys - 1/2 at step k = kc + sp + 2j
-                    const float tm = t + MAGIC;
-                    const float d = t - (tm - MAGIC);                       // in [-1/2, 1/2]
-                    const int row = __float_as_int(tm) - (0x4B400000 - 1);  // floor + 1 = tile row of the first tap
-                    const bool ok = (unsigned)row <= (unsigned)TILE;
-                    const float w1 = ok ? d + 0.5f : 0.0f, w0 = ok ? 0.5f - d : 0.0f;
-                    const float4 *p0 = pc + (ok ? row : 0) * (RSV * 4) + j * 8;
+                    const float ys = fmaf((float)(2 * j), step, y0s);       // crossing at step k = kc + sp + 2j
+                    const float tm = __fadd_rd(ys, MAGIC);
+                    const float w1 = ys - (tm - MAGIC), w0 = 1.0f - w1;     // w1 in [0,1)
+                    // tile row of the first tap = floor(ys) + 1; anything outside [0, TILE] reads the two zero rows TILE+1, TILE+2
+                    const unsigned row = min((unsigned)(__float_as_int(tm) - (0x4B400000 - 1)), (unsigned)(TILE + 1));
+                    const float4 *p0 = pc + row * (RSV * 4) + j * 8;
                     const float4 v0 = p0[0], v1 = p0[RSV * 4];
                     fma4(acc, w0, v0);
                     fma4(acc, w1, v1);
@@ -216,7 +211,7 @@ __global__ void __launch_bounds__(FR_THREADS, 3) k_forward_rays16(const float *_
 
 static cudaError_t fwd_launch_rays16(cp4d_ctx *c, const float *f, float4 *P, const ProjArgs &a) {
     const Dims &d = c->d;
-    const size_t sh = (size_t)(TILE + 2) * RSV * 4 * sizeof(float4);
+    const size_t sh = (size_t)(TILE + 3) * RSV * 4 * sizeof(float4);
     cudaError_t e = cudaFuncSetAttribute(k_forward_rays16, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sh);
     if (e != cudaSuccess) return e;
     k_forward_rays16<<<dim3(d.tiles, d.nz, d.Q / 4), FR_THREADS, sh, c->stream>>>(f, P, a);
