@@ -145,17 +145,15 @@ __global__ void __launch_bounds__(FR_THREADS, 3) k_forward_rays16(const float *_
     const float4 *F = reinterpret_cast<const float4 *>(f);
     const TileGeo *geo = a.geo + (int64_t)blockIdx.x * a.n0;
 
+    for (int t = threadIdx.x; t < (TILE + 3) * RSV * 4; t += FR_THREADS) tile[t] = zero;   // borders stay zero in both passes
     for (int pass = 0; pass < 2; ++pass) {   // pass 0: rays stepping over columns; pass 1: over rows, on the transposed tile
-        __syncthreads();
-        for (int t = threadIdx.x; t < (TILE + 3) * RSV * 4; t += FR_THREADS) tile[t] = zero;
         __syncthreads();
         for (int t = threadIdx.x; t < TILE * TILE * 4; t += FR_THREADS) {
             const int jc = t & 3, lx = (t >> 2) & (TILE - 1), ly = t >> 7;
             const int gx = x0 + lx, gy = y0 + ly;
-            if (gx < a.n && gy < a.n) {
-                const int row = pass ? lx : ly, col = pass ? ly : lx;
-                tile[((row + 1) * RSV + col + 1) * 4 + jc] = __ldg(F + (((int64_t)z * a.n + gy) * a.n + gx) * a.Q + jg * 4 + jc);
-            }
+            const int row = pass ? lx : ly, col = pass ? ly : lx;
+            tile[((row + 1) * RSV + col + 1) * 4 + jc] =
+                (gx < a.n && gy < a.n) ? __ldg(F + (((int64_t)z * a.n + gy) * a.n + gx) * a.Q + jg * 4 + jc) : zero;
         }
         __syncthreads();
         for (int i = 0; i < a.n0; ++i) {
