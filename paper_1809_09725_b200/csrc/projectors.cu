@@ -1,16 +1,14 @@
-// Time-decomposed parallel-beam projector pair on sm_100a (Eq. 9/10, L184/L196, with the pi-fold of
-// L198-L212).  Both kernels work on TILE x TILE voxel tiles of one slice and keep all coefficients j of a
-// ray / voxel in registers, so the m coefficients are read once per tap and the synthesised frame
-// sum_j Phi[j,k] f_j is never materialised:
+// Forward half of the time-decomposed parallel-beam projector pair on sm_100a (Eq. 9, with the pi-fold
+// of L198-L202).  A CTA stages one TILE x TILE voxel tile of one slice (all coefficients of a group) in shared memory
+// once, then walks ALL base angles; every ray of the tile's window gathers its Joseph taps along the dominant axis with
+// all coefficients of the group accumulated in registers, so the m coefficients are read once per tap and the synthesised
+// frame sum_j Phi[j,k] f_j is never materialised.  The per-tile partial ray sums go to P[z][i][jq][b] with one vector RED
+// per ray and coefficient chunk; the synthesis with Phi (and the F1* prox) is the k_synth epilogue in stream_kernels.cu.
 //
-//   k_forward_partial : the CTA stages its f tile (all j of a chunk group) in shared memory once, then walks ALL
-//                       base angles; a thread owns one ray (bin) of the tile's window at that angle and gathers the
-//                       Joseph taps along the dominant axis (2 LDS.128 + 8 FFMA per step and coefficient chunk);
-//                       the per-tile partial ray sums go to P[z][i][jc][b] with one vector RED per ray and chunk.
-//                       The synthesis with Phi (and the F1* prox) is the k_synth epilogue in stream_kernels.cu.
-//   k_backproject     : voxel-driven gather from the folded sinogram gt[z][i][jc][b]; the <= WIN bins a tile can touch
-//                       at an angle are staged in shared memory with cp.async (zero-fill outside the detector),
-//                       double-buffered over chunks of ANG_CHUNK angles; a thread owns 4 voxels x all j of the group.
+//   k_forward_rays16  : m % 16 == 0 (configs 3-5).  8 lanes per ray, voxel-major tile, conflict-free full wavefronts.
+//   k_forward_partial : any m % 4 == 0.  One thread per ray, coefficient-plane-major tile.
+//
+// The backprojector lives in backproject.cu.
 //
 // Coordinates: the host computes, in fp64, for every (tile, base angle) the window start `bstart` and the offset
 // `delta` such that the bin coordinate of tile-local voxel (lx,ly) is  u = delta + lx*c + ly*s  with 1 <= u < WIN-1;
@@ -19,7 +17,6 @@
 
 namespace cp4d {
 
-constexpr int ANG_CHUNK = 8;
 constexpr int RS = TILE + 3;             // row stride of the forward tile in float4 (odd: rows rotate bank groups)
 constexpr int PLANE = (TILE + 2) * RS;   // float4 per coefficient chunk plane
 
