@@ -73,16 +73,21 @@ __device__ __forceinline__ void bp_voxel(float4 (&acc)[8][JQ], const float4 (&B)
                                          float A1, float A2, float A3) {
     // accumulator V is voxel (dx, dy) = (V & 3, V >> 2); for c < 0 its offset from the patch minimum is that of e = 3 - dx
     constexpr int E = (NEG ? 3 - (V & 3) : (V & 3)) + (V & 4), FL = bp_fl(PAT, E);
-    const float t = phi + tdv[E];                                                 // in [0,2)
+    // E == 0 is the patch minimum itself: delta = 0, t = phi < 1, so its third candidate bin always has weight 0
+    const float t = E == 0 ? phi : phi + tdv[E];                                  // in [0,2)
     const float x0 = fmaxf(0.f, fmaf(-A2, t, A1));
     const float x1 = fmaxf(0.f, fmaf(-A2, fabsf(t - 1.0f), A1));
-    const float x2 = fmaxf(0.f, fmaf(A2, t, A3));                              // A3 = A1 - 2 A2
-    const float2 w0 = make_float2(x0, x0), w1 = make_float2(x1, x1), w2 = make_float2(x2, x2);
+    const float2 w0 = make_float2(x0, x0), w1 = make_float2(x1, x1);
 #pragma unroll
     for (int jc = 0; jc < JQ; ++jc) {
         fma4(acc[V][jc], w0, B[FL][jc]);
         fma4(acc[V][jc], w1, B[FL + 1][jc]);
-        fma4(acc[V][jc], w2, B[FL + 2][jc]);
+    }
+    if (E != 0) {
+        const float x2 = fmaxf(0.f, fmaf(A2, t, A3));                          // A3 = A1 - 2 A2
+        const float2 w2 = make_float2(x2, x2);
+#pragma unroll
+        for (int jc = 0; jc < JQ; ++jc) fma4(acc[V][jc], w2, B[FL + 2][jc]);
     }
 }
 
