@@ -369,8 +369,8 @@ def assemble(args, c, world, r):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=10)
-    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--steps", type=int, default=50)
+    ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--config", type=int, default=3, help="BASELINE.json config 1..5 (SURVEY.md 8 numbering)")
     ap.add_argument("--impl", default="cp4d", choices=["cp4d", "reference"])
     ap.add_argument("--power-iters", type=int, default=10)
