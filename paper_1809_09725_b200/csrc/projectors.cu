@@ -129,6 +129,7 @@ __global__ void __launch_bounds__(256) k_forward_partial(const float *__restrict
 constexpr int FR_RAYS = WIN;                 // rays of a tile window
 constexpr int FR_THREADS = FR_RAYS * 8;      // 384
 constexpr int RSV = TILE + 2;                // voxels per tile row incl. the zero border; even
+constexpr int FR_UNROLL = 4;                 // steps per lane and chunk: a chunk is 2 * FR_UNROLL columns of the chord
 static_assert(RSV % 2 == 0, "row pitch must be even for conflict-free step pairs");
 
 __global__ void __launch_bounds__(FR_THREADS, 3) k_forward_rays16(const float *__restrict__ f, float4 *__restrict__ P, ProjArgs a) {
@@ -174,17 +175,17 @@ __global__ void __launch_bounds__(FR_THREADS, 3) k_forward_rays16(const float *_
             const float MAGIC = 12582912.0f;
             const float4 *plane = tile + jq + 4;          // + 4: column k lives at tile column k+1
             // per-ray chunk range: lanes of other rays in the warp are masked off, so no wavefront is spent outside the chord
-            for (int kc = klo & ~7; kc <= khi; kc += 8) {
+            for (int kc = klo & ~(2 * FR_UNROLL - 1); kc <= khi; kc += 2 * FR_UNROLL) {
                 const float y0s = fmaf((float)(kc + sp), step, base);
                 const float4 *pc = plane + (kc + sp) * 4;
 #pragma unroll
-                for (int j = 0; j < 4; ++j) {
+                for (int j = 0; j < FR_UNROLL; ++j) {
                     const float ys = fmaf((float)(2 * j), step, y0s);       // crossing at step k = kc + sp + 2j
                     const float tm = __fadd_rd(ys, MAGIC);
                     const float w1 = ys - (tm - MAGIC), w0 = 1.0f - w1;     // w1 in [0,1)
                     // tile row of the first tap = floor(ys) + 1; anything outside [0, TILE] reads the two zero rows TILE+1, TILE+2
                     const unsigned row = min((unsigned)(__float_as_int(tm) - (0x4B400000 - 1)), (unsigned)(TILE + 1));
-                    const float4 *p0 = pc + row * (RSV * 4) + j * 8;
+                    const float4 *p0 = reinterpret_cast<const float4 *>(reinterpret_cast<const char *>(pc) + row * (RSV * 64)) + j * 8;
                     const float4 v0 = p0[0], v1 = p0[RSV * 4];
                     fma4(acc, w0, v0);
                     fma4(acc, w1, v1);
