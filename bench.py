@@ -390,7 +390,7 @@ def main():
     if rank == 0:
         line = assemble(args, c, world, r)
         if not args.no_cpu_baseline and world == 1:
-            val, cores, sample, dt = oracle_steps(c, 1, 0)
+            val, cores, sample, dt = oracle_steps(c, 1, 0, target_fma=1.2e11)   # about 10 s of oracle work on 16 cores
             line["cpu_baseline"] = {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample,
                                     "sample_step_s": dt}
         print(json.dumps(line), flush=True)
