@@ -178,3 +178,45 @@ def test_solve_host_equals_device_path(torch_cuda, fast_oracle):
     assert rel(fh.numpy(), a.numpy().astype(np.float64)) <= 1e-5       # atomics: summation order may differ
     assert ctx.launch_count() > 0
     ctx.close()
+
+
+def test_relaxation_and_warm_start(torch_cuda, fast_oracle):
+    """theta = 0.5 (L97: theta in [0,1]) and a non-zero initial guess through cp4d_reset(f0) (L147 'some initial guess')."""
+    from paper_1809_09725_b200 import binding
+    c = CASES["wide_det"].scaled(lambda1=0.01)
+    phi = synth.basis_table(c.basis, c.m, c.n_angles)
+    P = fast_oracle.Problem.from_config(c, phi=phi)
+    ctx = binding.Context.from_config(c, phi=phi, theta=0.5)
+    r = synth.rng(c.cfg, 9)
+    g = r.standard_normal(P.sino_shape).astype(np.float32)
+    f0 = r.standard_normal(P.primal_shape).astype(np.float32)
+    st = P.zero_state()
+    st["f"][:] = f0
+    st["ft"][:] = f0
+    P.cp(g.astype(np.float64), st, 0.004, 0.006, 7, theta=0.5, folded=True)
+    ctx.set_data(dev(torch_cuda, g)); ctx.set_steps(0.004, 0.006); ctx.reset(dev(torch_cuda, f0))
+    ctx.iterate(0)                                   # no-op
+    assert rel(ctx.get_f().cpu().numpy(), f0) == 0.0
+    ctx.iterate(3); ctx.iterate(4)                   # 3 + 4 = 7: the state machine carries over
+    ctx.sync()
+    s = ctx.state()
+    for name in ("f", "ft", "h1", "h2"):
+        assert rel(s[name].cpu().numpy(), st[name]) <= TOL_CP, name
+    ctx.close()
+
+
+def test_call_order_and_aliasing_errors(torch_cuda):
+    from paper_1809_09725_b200 import binding
+    c = CASES["cfg1"]
+    ctx = binding.Context.from_config(c)
+    with pytest.raises(binding.Cp4dError) as e:
+        ctx.iterate(1)                               # no data, no steps
+    assert e.value.code == binding.ESTATE
+    f = ctx.empty_primal().zero_()
+    with pytest.raises(binding.Cp4dError) as e:      # in/out aliasing is rejected
+        ctx._ck(binding.lib().cp4d_grad(ctx._h, f.data_ptr(), f.data_ptr()))
+    assert e.value.code == binding.EINVAL
+    with pytest.raises(binding.Cp4dError) as e:
+        ctx.set_steps(0.0, 1.0)
+    assert e.value.code == binding.EINVAL
+    ctx.close()
