@@ -22,7 +22,7 @@ namespace cp4d {
 namespace {
 
 constexpr int BP_THREADS = 128;          // one thread per 4x2 patch of a 32x32 tile
-constexpr int BP_CHUNK = 8;              // angles staged per pipeline stage
+constexpr int BP_CHUNK = 12;             // angles staged per pipeline stage
 constexpr int WINP = WIN + 8;            // staged bins per (angle, jq): window + NB-1 spill, zero-filled outside the detector
 
 __host__ __device__ constexpr int bp_fl(int pat, int v) {
