@@ -120,6 +120,14 @@ int cp4d_get_f(cp4d_ctx *ctx, float *f_dev_out);                      /* copy f 
  * any of the out pointers may be null. */
 int cp4d_state_ptrs(cp4d_ctx *ctx, float **f, float **ft, float **h1, float **h2, float **g);
 
+/* ---- convergence monitor (off the timed path).  Syncs. ---------------------------------------- */
+/* primal    = 1/2 |K1 f - g|^2 + lambda1 * sum over (x,y,z,j) of |K2 f|_2          (Eq. 6)
+ * cond_dual = -1/2 |h1|^2 - <h1, g>   (dual value of Eq. 7 with the constraint K^T h = 0 of G = 0 ignored; not a lower
+ *             bound while K^T h != 0, C19)
+ * kkt_resid = |K1^T h1 - div h2|_2    (dual residual; -> 0 at a saddle point)
+ * Out pointers are HOST and may be null.  Uses the K1^T h1 buffer and the projector scratch; state is untouched. */
+int cp4d_objective(cp4d_ctx *ctx, double *primal, double *cond_dual, double *kkt_resid);
+
 /* ---- end-to-end call with HOST buffers (pinned or pageable) ---------------------------------- */
 /* H2D copy of g_host (S), reset to zeros, n_iters iterations with the current steps, D2H copy of f
  * into f_host (V).  Syncs. */

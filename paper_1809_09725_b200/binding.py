@@ -61,6 +61,7 @@ def lib():
             "cp4d_iterate": [vp, i32], "cp4d_get_f": [vp, vp],
             "cp4d_state_ptrs": [vp] + [C.POINTER(vp)] * 5,
             "cp4d_solve_host": [vp, vp, i32, vp], "cp4d_sync": [vp],
+            "cp4d_objective": [vp] + [C.POINTER(C.c_double)] * 3,
             "cp4d_launch_count": [vp, C.POINTER(u64)],
             "cp4d_profile_begin": [vp], "cp4d_profile_end": [vp, C.POINTER(Profile)],
         }
@@ -230,6 +231,12 @@ class Context:
         fp = f_host.data_ptr() if hasattr(f_host, "data_ptr") else f_host.ctypes.data
         self._ck(lib().cp4d_solve_host(self._h, gp, n_iters, fp))
         return f_host
+
+    def objective(self):
+        """(primal value, conditional dual value, dual residual |K1^T h1 - div h2|) of the current state; syncs."""
+        out = [C.c_double(0) for _ in range(3)]
+        self._ck(lib().cp4d_objective(self._h, *[C.byref(o) for o in out]))
+        return tuple(o.value for o in out)
 
     def sync(self):
         self._ck(lib().cp4d_sync(self._h))

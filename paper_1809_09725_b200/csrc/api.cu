@@ -40,14 +40,14 @@ int validate(const cp4d_params *p, Dims *d) {
 }
 
 struct Carve {
-    uint64_t f, ft, bp, h2, h1, g, scratch, phi, ang, geo, red, total;
+    uint64_t f, ft, bp, h2, h1, g, tmp_s, scratch, phi, ang, geo, red, total;
 };
 Carve carve(const Dims &d) {
     Carve c;
     uint64_t o = 0;
     auto take = [&](uint64_t bytes) { uint64_t r = o; o += up(bytes); return r; };
     c.f = take(d.V * 4); c.ft = take(d.V * 4); c.bp = take(d.V * 4); c.h2 = take(d.V * 16);
-    c.h1 = take(d.S * 4); c.g = take(d.S * 4); c.scratch = take(d.scratch4 * 16);
+    c.h1 = take(d.S * 4); c.g = take(d.S * 4); c.tmp_s = take(d.S * 4); c.scratch = take(d.scratch4 * 16);
     c.phi = take((uint64_t)d.m * d.na * 4); c.ang = take((uint64_t)d.n0 * sizeof(AngleTab));
     c.geo = take((uint64_t)d.tiles * d.n0 * sizeof(TileGeo)); c.red = take(64);
     c.total = o;
@@ -137,6 +137,7 @@ int cp4d_create(const cp4d_params *p, cp4d_ctx **out) {
     char *w = (char *)p->workspace_dev;
     ctx->f = (float *)(w + cv.f); ctx->ft = (float *)(w + cv.ft); ctx->bp = (float *)(w + cv.bp);
     ctx->h2 = (float *)(w + cv.h2); ctx->h1 = (float *)(w + cv.h1); ctx->g = (float *)(w + cv.g);
+    ctx->tmp_s = (float *)(w + cv.tmp_s);
     ctx->scratch = (float4 *)(w + cv.scratch); ctx->phi = (float *)(w + cv.phi);
     ctx->ang = (AngleTab *)(w + cv.ang); ctx->geo = (TileGeo *)(w + cv.geo); ctx->red = (double *)(w + cv.red);
 
@@ -358,6 +359,37 @@ int cp4d_solve_host(cp4d_ctx *ctx, const float *g_host, int32_t n_iters, float *
     if (int r = cp4d_iterate(ctx, n_iters)) return r;
     CK(cudaMemcpyAsync(f_host, ctx->f, ctx->d.V * 4, cudaMemcpyDeviceToHost, ctx->stream), "solve_host d2h");
     CK(cudaStreamSynchronize(ctx->stream), "solve_host sync");
+    return CP4D_OK;
+}
+
+int cp4d_objective(cp4d_ctx *ctx, double *primal, double *cond_dual, double *kkt_resid) {
+    if (!ctx) return CP4D_EINVAL;
+    if (!ctx->have_data) return fail(ctx, CP4D_ESTATE, "objective: set_data first");
+    const Dims &d = ctx->d;
+    double v[5] = {0, 0, 0, 0, 0};
+    // primal: 1/2 |K1 f - g|^2 + lambda1 sum |K2 f|_2   (Eq. 6)
+    if (int r = forward_into(ctx, ctx->f, 0, 0.f, nullptr, ctx->tmp_s)) return r;
+    // |K1 f - g|^2 = |K1 f|^2 - 2 <K1 f, g> + |g|^2 with fp64-accumulated dots (products of fp32 numbers are exact in fp64)
+    {
+        double kk = 0, kg = 0, gg = 0;
+        if (int r = cp4d_dot(ctx, ctx->tmp_s, ctx->tmp_s, (uint64_t)d.S, &kk)) return r;
+        if (int r = cp4d_dot(ctx, ctx->tmp_s, ctx->g, (uint64_t)d.S, &kg)) return r;
+        if (int r = cp4d_dot(ctx, ctx->g, ctx->g, (uint64_t)d.S, &gg)) return r;
+        v[0] = kk - 2.0 * kg + gg;
+    }
+    CK(launch_tv_sum(ctx, ctx->f, ctx->red + 1), "tv");
+    // dual value with the constraint K^T h = 0 ignored (G = 0): -1/2 |h1|^2 - <h1, g>; |h2| <= lambda1 holds by construction
+    if (int r = cp4d_dot(ctx, ctx->h1, ctx->h1, (uint64_t)d.S, &v[2])) return r;
+    if (int r = cp4d_dot(ctx, ctx->h1, ctx->g, (uint64_t)d.S, &v[3])) return r;
+    // dual residual |K1^T h1 - div h2|_2 (tends to 0 at a saddle point)
+    if (int r = adjoint_into(ctx, ctx->h1, ctx->bp)) return r;
+    CK(launch_kkt_sum(ctx, ctx->bp, ctx->h2, ctx->red + 2), "kkt");
+    double r2[2];
+    CK(cudaMemcpyAsync(r2, ctx->red + 1, 2 * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream), "objective copy");
+    CK(cudaStreamSynchronize(ctx->stream), "objective sync");
+    if (primal) *primal = 0.5 * v[0] + (double)ctx->lambda1 * r2[0];
+    if (cond_dual) *cond_dual = -0.5 * v[2] - v[3];
+    if (kkt_resid) *kkt_resid = std::sqrt(r2[1]);
     return CP4D_OK;
 }
 

@@ -52,7 +52,7 @@ struct cp4d_ctx {
     int device;
     cudaStream_t stream;
     // workspace carve-up (device pointers)
-    float *f, *ft, *bp, *h2, *h1, *g;
+    float *f, *ft, *bp, *h2, *h1, *g, *tmp_s;
     float4 *scratch;           // forward partial ray sums P / folded sinogram gt: [z][i][jc][gpl + b] float4, pitch gp;
                                // the pads stay zero, so every tile window of the backprojector is readable memory
     float *phi;                // [j][k]
@@ -105,6 +105,8 @@ cudaError_t launch_forward_partial(cp4d_ctx *c, const float *f, float4 *P);
 cudaError_t launch_backproject(cp4d_ctx *c, const float4 *gt, float *f_out);
 int bp_pattern(float c, float s);  // host: pattern index in [0, BP_NPAT) or -1
 uint32_t bp_pattern_fl(int pat);   // host: the pattern's FL_v packed 4 bits each
+cudaError_t launch_tv_sum(cp4d_ctx *c, const float *f, double *slot);                       // sum |K2 f|_2
+cudaError_t launch_kkt_sum(cp4d_ctx *c, const float *bp, const float *h2, double *slot);    // sum (bp - div h2)^2
 cudaError_t launch_sumsq_dot(cp4d_ctx *c, const float *x, const float *y, uint64_t n, double *slot);
 cudaError_t launch_fill_normal(cp4d_ctx *c, float *x, uint64_t n, uint64_t seed);
 // x = (a - b) * scale   (b nullable)

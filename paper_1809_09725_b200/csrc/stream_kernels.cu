@@ -12,6 +12,20 @@ namespace cp4d {
 __device__ __forceinline__ float4 ld4(const float4 *p) { return __ldg(p); }
 __device__ __forceinline__ float4 sub4(float4 a, float4 b) { return make_float4(a.x - b.x, a.y - b.y, a.z - b.z, a.w - b.w); }
 
+// sum of v over the CTA, added to *slot (fp64)
+__device__ __forceinline__ void block_add(double v, double *slot) {
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    __shared__ double part[32];
+    const int w = threadIdx.x >> 5, nw = (blockDim.x + 31) >> 5;
+    if ((threadIdx.x & 31) == 0) part[w] = v;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double t = 0.0;
+        for (int i = 0; i < nw; ++i) t += part[i];
+        atomicAdd(slot, t);
+    }
+}
+
 struct StreamArgs {
     int n, nz, Q, zper;
     int64_t slice4, V4;
@@ -19,13 +33,17 @@ struct StreamArgs {
 };
 
 // ---------------------------------------------------------------------------------------------------
-// grad (PROX=false):  p = K2 f.     prox (PROX=true): h2 <- proj_{|.|<=lambda1}(h2 + sigma K2 ft)
+// MODE 0 grad:  p = K2 f.     MODE 1 prox: h2 <- proj_{|.|<=lambda1}(h2 + sigma K2 ft)
+// MODE 2 tv:    *red += sum over (voxel, j) of |K2 f|_2   (the penalty of Eq. 6 without lambda1; nothing is stored)
 // ---------------------------------------------------------------------------------------------------
-template <bool PROX>
+template <int MODE>
 __global__ void __launch_bounds__(256) k_grad(const float *__restrict__ f, float *__restrict__ p, StreamArgs a,
-                                              float sigma, float inv_l1, int l1_zero) {
-    const int64_t e4 = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (e4 >= a.slice4) return;
+                                              float sigma, float inv_l1, int l1_zero, double *red) {
+    const int64_t e4r = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const bool live = e4r < a.slice4;
+    if (MODE != 2 && !live) return;
+    const int64_t e4 = live ? e4r : 0;   // MODE 2: idle threads still join the block reduction
+    double tv = 0.0;
     const int c = (int)(e4 % a.Q);
     const int64_t vox = e4 / a.Q;
     const int x = (int)(vox % a.n), y = (int)(vox / a.n);
@@ -44,7 +62,7 @@ __global__ void __launch_bounds__(256) k_grad(const float *__restrict__ f, float
         float4 gx = sub4(fx, cur), gy = sub4(fy, cur), gz = sub4(fz, cur);
         float4 gt = make_float4(a.lambda2 * (cur.y - cur.x), a.lambda2 * (cur.z - cur.y), a.lambda2 * (cur.w - cur.z),
                                 a.lambda2 * (ft - cur.w));
-        if (PROX) {
+        if (MODE == 1) {
             float4 qx = P[idx], qy = P[idx + a.V4], qz = P[idx + 2 * a.V4], qt = P[idx + 3 * a.V4];
 #define CP4D_PROX1(C)                                                                             \
     {                                                                                             \
@@ -57,24 +75,37 @@ __global__ void __launch_bounds__(256) k_grad(const float *__restrict__ f, float
             CP4D_PROX1(x) CP4D_PROX1(y) CP4D_PROX1(z) CP4D_PROX1(w)
 #undef CP4D_PROX1
         }
-        P[idx] = gx;
-        P[idx + a.V4] = gy;
-        P[idx + 2 * a.V4] = gz;
-        P[idx + 3 * a.V4] = gt;
+        if (MODE == 2) {
+            if (live)
+                tv += (double)sqrtf(gx.x * gx.x + gy.x * gy.x + gz.x * gz.x + gt.x * gt.x) +
+                      (double)sqrtf(gx.y * gx.y + gy.y * gy.y + gz.y * gz.y + gt.y * gt.y) +
+                      (double)sqrtf(gx.z * gx.z + gy.z * gy.z + gz.z * gz.z + gt.z * gt.z) +
+                      (double)sqrtf(gx.w * gx.w + gy.w * gy.w + gz.w * gz.w + gt.w * gt.w);
+        } else {
+            P[idx] = gx;
+            P[idx + a.V4] = gy;
+            P[idx + 2 * a.V4] = gz;
+            P[idx + 3 * a.V4] = gt;
+        }
         cur = fz;
     }
+    if (MODE == 2) block_add(tv, red);
 }
 
 // ---------------------------------------------------------------------------------------------------
-// div (UPDATE=false): out = -K2^T p.
-// update (UPDATE=true): f+ = f - tau bp + tau div h2; ft = f+ + theta (f+ - f); f <- f+   (steps 5-6)
+// div (MODE 0): out = -K2^T p.
+// update (MODE 1): f+ = f - tau bp + tau div h2; ft = f+ + theta (f+ - f); f <- f+   (steps 5-6)
+// kkt (MODE 2): *red += sum (bp - div p)^2, nothing stored (bp = K1^T h1: the dual residual |K^T h|^2)
 // ---------------------------------------------------------------------------------------------------
-template <bool UPDATE>
+template <int MODE>
 __global__ void __launch_bounds__(256) k_div(const float *__restrict__ p, float *__restrict__ out, StreamArgs a,
                                              const float *__restrict__ bp, float *__restrict__ ft_out, float tau,
-                                             float theta) {
-    const int64_t e4 = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (e4 >= a.slice4) return;
+                                             float theta, double *red) {
+    const int64_t e4r = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const bool live = e4r < a.slice4;
+    if (MODE != 2 && !live) return;
+    const int64_t e4 = live ? e4r : 0;
+    double kk = 0.0;
     const int c = (int)(e4 % a.Q);
     const int64_t vox = e4 / a.Q;
     const int x = (int)(vox % a.n), y = (int)(vox / a.n);
@@ -100,7 +131,11 @@ __global__ void __launch_bounds__(256) k_div(const float *__restrict__ p, float 
         d.y = (xc.y - xm.y) + (yc.y - ym.y) + (zc.y - prevz.y) + a.lambda2 * (tc.y - tc.x);
         d.z = (xc.z - xm.z) + (yc.z - ym.z) + (zc.z - prevz.z) + a.lambda2 * (tc.z - tc.y);
         d.w = (xc.w - xm.w) + (yc.w - ym.w) + (zc.w - prevz.w) + a.lambda2 * (tw - tc.z);
-        if (UPDATE) {
+        if (MODE == 2) {
+            const float4 b = ld4(reinterpret_cast<const float4 *>(bp) + idx);
+            const float ex = b.x - d.x, ey = b.y - d.y, ez = b.z - d.z, ew = b.w - d.w;
+            if (live) kk += (double)ex * ex + (double)ey * ey + (double)ez * ez + (double)ew * ew;
+        } else if (MODE == 1) {
             float4 *F = reinterpret_cast<float4 *>(out);
             const float4 fo = F[idx];
             const float4 b = ld4(reinterpret_cast<const float4 *>(bp) + idx);
@@ -116,6 +151,7 @@ __global__ void __launch_bounds__(256) k_div(const float *__restrict__ p, float 
         }
         prevz = zc;
     }
+    if (MODE == 2) block_add(kk, red);
 }
 
 static StreamArgs make_args(const cp4d_ctx *c, dim3 &grid, dim3 &block) {
@@ -137,7 +173,7 @@ cudaError_t launch_grad(cp4d_ctx *c, const float *f, float *p) {
     ProfScope ps(c, CP4D_K_GRAD);
     dim3 g, b;
     StreamArgs a = make_args(c, g, b);
-    k_grad<false><<<g, b, 0, c->stream>>>(f, p, a, 0.f, 0.f, 0);
+    k_grad<0><<<g, b, 0, c->stream>>>(f, p, a, 0.f, 0.f, 0, nullptr);
     c->launches++;
     return cudaGetLastError();
 }
@@ -146,7 +182,7 @@ cudaError_t launch_prox_f2(cp4d_ctx *c, float sigma, const float *ft, float *h2)
     dim3 g, b;
     StreamArgs a = make_args(c, g, b);
     const int l1z = !(c->lambda1 > 0.f);
-    k_grad<true><<<g, b, 0, c->stream>>>(ft, h2, a, sigma, l1z ? 0.f : 1.0f / c->lambda1, l1z);
+    k_grad<1><<<g, b, 0, c->stream>>>(ft, h2, a, sigma, l1z ? 0.f : 1.0f / c->lambda1, l1z, nullptr);
     c->launches++;
     return cudaGetLastError();
 }
@@ -154,7 +190,7 @@ cudaError_t launch_div(cp4d_ctx *c, const float *p, float *f) {
     ProfScope ps(c, CP4D_K_DIV);
     dim3 g, b;
     StreamArgs a = make_args(c, g, b);
-    k_div<false><<<g, b, 0, c->stream>>>(p, f, a, nullptr, nullptr, 0.f, 0.f);
+    k_div<0><<<g, b, 0, c->stream>>>(p, f, a, nullptr, nullptr, 0.f, 0.f, nullptr);
     c->launches++;
     return cudaGetLastError();
 }
@@ -162,8 +198,30 @@ cudaError_t launch_update(cp4d_ctx *c, float tau, const float *bp, const float *
     ProfScope ps(c, CP4D_K_UPDATE);
     dim3 g, b;
     StreamArgs a = make_args(c, g, b);
-    k_div<true><<<g, b, 0, c->stream>>>(h2, f, a, bp, ft, tau, c->theta);
+    k_div<1><<<g, b, 0, c->stream>>>(h2, f, a, bp, ft, tau, c->theta, nullptr);
     c->launches++;
+    return cudaGetLastError();
+}
+
+// reductions for cp4d_objective: *slot is zeroed first, then accumulated by the kernel
+cudaError_t launch_tv_sum(cp4d_ctx *c, const float *f, double *slot) {
+    ProfScope ps(c, CP4D_K_REDUCE);
+    dim3 g, b;
+    StreamArgs a = make_args(c, g, b);
+    cudaError_t e = cudaMemsetAsync(slot, 0, sizeof(double), c->stream);
+    if (e != cudaSuccess) return e;
+    k_grad<2><<<g, b, 0, c->stream>>>(f, nullptr, a, 0.f, 0.f, 0, slot);
+    c->launches += 2;
+    return cudaGetLastError();
+}
+cudaError_t launch_kkt_sum(cp4d_ctx *c, const float *bp, const float *h2, double *slot) {
+    ProfScope ps(c, CP4D_K_REDUCE);
+    dim3 g, b;
+    StreamArgs a = make_args(c, g, b);
+    cudaError_t e = cudaMemsetAsync(slot, 0, sizeof(double), c->stream);
+    if (e != cudaSuccess) return e;
+    k_div<2><<<g, b, 0, c->stream>>>(h2, nullptr, a, bp, nullptr, 0.f, 0.f, slot);
+    c->launches += 2;
     return cudaGetLastError();
 }
 

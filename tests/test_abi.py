@@ -35,7 +35,7 @@ def test_workspace_bytes_counts_state(L):
     for cfg in (1, 2, 3, 4, 5):
         c = synth.CONFIGS[cfg]
         nb = binding.workspace_bytes(c.n, c.nz, c.nd, c.n_angles, c.n_half_rot, c.m)
-        state = (7 * c.V + 2 * c.S) * 4                       # f, ft, K1^T h1, h2[4], h1, g
+        state = (7 * c.V + 3 * c.S) * 4                       # f, ft, K1^T h1, h2[4], h1, g, sinogram temporary
         # projector scratch rows are padded so that every tile window is readable memory (include/cp4d.h):
         # at most (sqrt2 (n-1) - (nd-1))/2 + 3 bins each side plus one window of 56 bins
         pad = 2 * (int(np.ceil(max(0.0, 0.5 * (np.sqrt(2.0) * (c.n - 1) - (c.nd - 1))))) + 3) + 56

@@ -220,3 +220,28 @@ def test_call_order_and_aliasing_errors(torch_cuda):
         ctx.set_steps(0.0, 1.0)
     assert e.value.code == binding.EINVAL
     ctx.close()
+
+
+@pytest.mark.parametrize("case", ["cfg1", "ragged"])
+def test_objective_monitor(torch_cuda, fast_oracle, case):
+    """cp4d_objective against the same quantities assembled from oracle operators (Eq. 6; C19)."""
+    from paper_1809_09725_b200 import binding
+    c = CASES[case].scaled(lambda1=0.02)
+    phi = synth.basis_table(c.basis, c.m, c.n_angles)
+    P = fast_oracle.Problem.from_config(c, phi=phi)
+    ctx = binding.Context.from_config(c, phi=phi)
+    g = _data(c).astype(np.float32)
+    ctx.set_data(dev(torch_cuda, g)); ctx.set_steps(0.01, 0.01); ctx.reset(); ctx.iterate(6); ctx.sync()
+    s = {k: v.cpu().numpy().astype(np.float64) for k, v in ctx.state().items()}
+    primal, dual, kkt = ctx.objective()
+    gr = P.grad(s["f"])
+    ref_primal = 0.5 * np.sum((P.forward(s["f"], folded=True) - g) ** 2) + float(np.float32(0.02)) * np.sqrt((gr ** 2).sum(0)).sum()
+    ref_dual = -0.5 * np.sum(s["h1"] ** 2) - np.sum(s["h1"] * g)
+    ref_kkt = np.linalg.norm(P.adjoint(s["h1"], folded=True) - P.div(s["h2"]))
+    assert abs(primal - ref_primal) <= 1e-4 * abs(ref_primal)
+    assert abs(dual - ref_dual) <= 1e-5 * max(abs(ref_dual), 1e-30)
+    assert abs(kkt - ref_kkt) <= 1e-4 * ref_kkt
+    # the monitor leaves the state alone
+    s2 = {k: v.cpu().numpy().astype(np.float64) for k, v in ctx.state().items()}
+    assert all(np.array_equal(s[k], s2[k]) for k in s)
+    ctx.close()
