@@ -45,6 +45,8 @@ CASES = {
     "wide_det": synth.CONFIGS[4].scaled(cfg=14, n=40, nd=75, nz=2, n_angles=36, n_half_rot=3, m=8),
     "narrow_det_m32": synth.CONFIGS[2].scaled(cfg=15, n=70, nd=33, nz=1, n_angles=24, n_half_rot=2, m=32),
     "one_angle_per_pi": synth.CONFIGS[1].scaled(cfg=16, n=33, nd=33, nz=2, n_angles=6, n_half_rot=6, m=4),
+    # m = 16: the 8-lanes-per-ray forward kernel and two coefficient groups in the backprojector, on ragged tiles
+    "ragged_m16": synth.CONFIGS[3].scaled(cfg=17, n=75, nd=90, nz=3, n_angles=78, n_half_rot=3, m=16, iters=12, n_objects=5),
 }
 
 
@@ -86,7 +88,7 @@ def test_grad_div(torch_cuda, fast_oracle, case):
     ctx.close()
 
 
-@pytest.mark.parametrize("case", ["cfg1", "ragged", "narrow_det_m32"])
+@pytest.mark.parametrize("case", ["cfg1", "ragged", "narrow_det_m32", "ragged_m16"])
 def test_fused_steps(torch_cuda, fast_oracle, case):
     c, P, ctx = make(case, fast_oracle)
     r = synth.rng(c.cfg, 6)
@@ -125,7 +127,7 @@ def _data(c):
     return synth.sinogram(c).numpy()
 
 
-@pytest.mark.parametrize("case,lam1", [("cfg1", 1e-3), ("cfg1", "mixed"), ("cfg2", 1e-3), ("cfg2", "mixed"), ("ragged", "mixed")])
+@pytest.mark.parametrize("case,lam1", [("cfg1", 1e-3), ("cfg1", "mixed"), ("cfg2", 1e-3), ("cfg2", "mixed"), ("ragged", "mixed"), ("ragged_m16", 1e-3)])
 def test_cp_iterations(torch_cuda, fast_oracle, case, lam1):
     """Full CP run (config iteration counts) from zero state with the oracle's tau = sigma = 0.95/L."""
     c = CASES[case]
@@ -160,6 +162,9 @@ def test_cp_iterations(torch_cuda, fast_oracle, case, lam1):
 @pytest.mark.parametrize("case", ["cfg1", "cfg2"])
 def test_power_iteration(torch_cuda, fast_oracle, case):
     c, P, ctx = make(case, fast_oracle)
+    # the two sides start from different random vectors (each its own generator), so both must have converged; 30 steps do
+    # on configs 1-2 (R8).  (On small m = 16 problems the top of the spectrum is clustered and two starts still
+    # differ by 2e-4 after 300 steps while the operators agree to 1e-7 on the iterates -- not a parity case.)
     L_ref, _ = P.power(synth.rng(c.cfg, 3).standard_normal(P.primal_shape), 30, folded=True)
     L = ctx.norm(30, seed=7)
     assert abs(L - L_ref) <= 1e-4 * L_ref
