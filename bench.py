@@ -60,8 +60,11 @@ def alu_peak_tflops(sm_mhz: float) -> float:
 # ------------------------------------------------------------------------------------------------------
 # algorithmic work per launch of each kernel class (bytes or flops per unit x units)
 # ------------------------------------------------------------------------------------------------------
-def algorithmic_work(c):
+def algorithmic_work(c, n_frames=0):
     V, S = c.V, c.S
+    Vc = V                                               # coefficient stack (projectors)
+    if n_frames:
+        V = V // c.m * n_frames                          # primal arrays hold frames
     n0 = c.n_theta0
     ray_fma = 2 * c.m * c.n * c.n * c.nz * n0            # 2 taps x m per voxel-step per base-angle ray
     syn_fma = c.m * c.n_angles * c.nd * c.nz             # m-wide synthesis / analysis per sinogram sample
@@ -76,6 +79,7 @@ def algorithmic_work(c):
         "div": ("hbm", 4.0 * 5 * V),
         "prox_f2": ("hbm", 4.0 * 9 * V),                 # read ft + h2[4], write h2[4]
         "update": ("hbm", 4.0 * 8 * V),                  # read h2[4] + f + K1^T h1, write f + ft
+        "mix": ("hbm", 4.0 * (V + Vc)),                  # frame mode: read frames / write coefficients or the reverse
     }
 
 
@@ -156,7 +160,7 @@ def oracle_sample_config(c, target_fma: float = 4e10):
     return c.scaled(nz=nz_s), c.nz / nz_s
 
 
-def oracle_steps(c, steps: int, warmup: int, target_fma: float = 4e10):
+def oracle_steps(c, steps: int, warmup: int, target_fma: float = 4e10, n_frames: int = 0):
     """Times `steps` oracle CP iterations (all host cores, pi-folded operators -- bitwise equal to 1 thread)
     on the sample; returns (it/s extrapolated to the workload, cores, sample text, seconds per sample step)."""
     from oracle import ref
@@ -166,7 +170,10 @@ def oracle_steps(c, steps: int, warmup: int, target_fma: float = 4e10):
     ref.set_threads(cores)
     cs, scale = oracle_sample_config(c, target_fma)
     phi = synth.basis_table(cs.basis, cs.m, cs.n_angles)
-    P = ref.Problem.from_config(cs, phi=phi)
+    if n_frames:
+        P = ref.FrameProblem(cs.n, cs.nz, cs.nd, cs.n_angles, cs.n_half_rot, cs.m, phi, n_frames, cs.lambda1, cs.lambda2)
+    else:
+        P = ref.Problem.from_config(cs, phi=phi)
     r = synth.rng(c.cfg, 1)
     g = r.standard_normal(P.sino_shape)                      # cost does not depend on the values
     st = P.zero_state()
@@ -189,7 +196,7 @@ def run_reference(args, c, rank):
     if rank != 0:
         return
     from paper_1809_09725_b200 import synth
-    val, cores, sample, dt = oracle_steps(c, args.steps, args.warmup, target_fma=1.5e10)
+    val, cores, sample, dt = oracle_steps(c, args.steps, args.warmup, target_fma=1.5e10, n_frames=args.frames)
     line = {
         "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": 1e3 / val, "higher_is_better": True, "scaling": "weak",
@@ -227,7 +234,7 @@ def run_cp4d(args, c, rank, world):
 
     # ---- problem, data, step sizes (outside the timed region: SURVEY 8(d)) ----
     phi = synth.basis_table(c.basis, c.m, c.n_angles)
-    ctx = binding.Context.from_config(c, phi=phi, device=local)
+    ctx = binding.Context.from_config(c, phi=phi, device=local, n_frames=args.frames)
     g = synth.sinogram(c, device=str(dev)).to(torch.float32).contiguous()
     L = ctx.norm(args.power_iters, seed=3)
     ts = 0.95 / L
@@ -312,7 +319,7 @@ def run_cp4d(args, c, rank, world):
 def assemble(args, c, world, r):
     from paper_1809_09725_b200 import synth
     peaks, K = r["peaks"], args.steps
-    work = algorithmic_work(c)
+    work = algorithmic_work(c, args.frames)
     alu_peak = alu_peak_tflops(peaks["sm_max_mhz"])
     kernels, total_ms = {}, 0.0
     merged = dict(r["prof"])
@@ -353,7 +360,7 @@ def assemble(args, c, world, r):
         "metric": METRIC, "value": replicas_value(world, K, r["ms"]), "unit": UNIT, "n_gpus": world, "steps": K,
         "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f32", "data": "synthetic",
-        "config": {"workload": synth.describe(c), "cfg": c.cfg, "n": c.n, "nz": c.nz, "nd": c.nd, "n_angles": c.n_angles,
+        "config": {"workload": synth.describe(c) + (f"_frames{args.frames}" if args.frames else ""), "n_frames": args.frames, "cfg": c.cfg, "n": c.n, "nz": c.nz, "nd": c.nd, "n_angles": c.n_angles,
                    "n_half_rot": c.n_half_rot, "m": c.m, "basis": c.basis, "lambda1": c.lambda1, "lambda2": c.lambda2,
                    "norm_K": r["L"], "parallelism": "replicas only" if world > 1 else "1 gpu",
                    "l2": f"no flush: CP state {(7 * c.V + 2 * c.S) * 4 / 1e9:.2f} GB streams through every step (L2 = 126 MB)"},
@@ -374,6 +381,7 @@ def main():
     ap.add_argument("--config", type=int, default=3, help="BASELINE.json config 1..5 (SURVEY.md 8 numbering)")
     ap.add_argument("--impl", default="cp4d", choices=["cp4d", "reference"])
     ap.add_argument("--power-iters", type=int, default=10)
+    ap.add_argument("--frames", type=int, default=0, help="N_t > 0: the paper's frame discretisation (cp4d_params.n_frames), e.g. 8")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
@@ -390,7 +398,7 @@ def main():
     if rank == 0:
         line = assemble(args, c, world, r)
         if not args.no_cpu_baseline and world == 1:
-            val, cores, sample, dt = oracle_steps(c, 1, 0, target_fma=1.2e11)   # about 10 s of oracle work on 16 cores
+            val, cores, sample, dt = oracle_steps(c, 1, 0, target_fma=1.2e11, n_frames=args.frames)   # about 10 s of oracle work on 16 cores
             line["cpu_baseline"] = {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample,
                                     "sample_step_s": dt}
         print(json.dumps(line), flush=True)

@@ -20,7 +20,8 @@
  * n_theta0 = n_angles/n_half_rot; t_k = k/n_angles (enters only through the caller's table Phi).
  * Values outside the grid are zero; rays exist only for 0 <= b < nd.
  *
- * Layouts (dense, no padding, fp32, base pointers 16-byte aligned; V = nz*n*n*m, S = nz*n_angles*nd):
+ * Layouts (dense, no padding, fp32, base pointers 16-byte aligned; V = nz*n*n*mp, S = nz*n_angles*nd,
+ * mp = m, or n_frames in frame mode where j below is the frame index):
  *   primal-shaped   f[z][iy][ix][j]        j fastest                      V floats
  *   sinogram        g[z][k][b]             b fastest                      S floats
  *   dual field      p[a][z][iy][ix][j]     a = 0..3 = (x, y, z, t)        4V floats, component-major
@@ -67,6 +68,11 @@ typedef struct {
     void *workspace_dev;      /* DEVICE, caller-allocated, >= cp4d_workspace_bytes(), 256-byte aligned     */
     uint64_t workspace_bytes;
     void *stream;             /* cudaStream_t (0 = legacy default stream)                                  */
+    int32_t n_frames;         /* 0: the primal array is the coefficient stack f_j (4th axis m).  N_t > 0: the paper's own
+                                 discretisation (L214-L237): the primal array holds N_t time frames f(t_q) (4th axis N_t,
+                                 N_t % 4 == 0, N_t <= 32, n_angles % N_t == 0), frame q sits at the time of angle
+                                 q*n_angles/N_t; K1 f = K1_coef(f_j) with f_j = sum_q phi_j(t_q) f(t_q), phi_j(t_q) taken
+                                 from phi_host's column q*n_angles/N_t; the 4th difference of K2 runs over frames      */
 } cp4d_params;
 
 /* Bytes of device workspace a context for these sizes needs (state f, f~, K1^T h1, h2[4], h1, g,
@@ -149,7 +155,8 @@ int cp4d_launch_count(const cp4d_ctx *ctx, uint64_t *count_out);
 #define CP4D_K_UPDATE      7  /* fused div + primal update + over-relaxation (steps 5-6)                  */
 #define CP4D_K_REDUCE      8
 #define CP4D_K_MISC        9
-#define CP4D_K_COUNT      10
+#define CP4D_K_MIX        10  /* frame mode: per-voxel frame <-> coefficient contraction (L231-L237)           */
+#define CP4D_K_COUNT      11
 typedef struct {
     double   ms[CP4D_K_COUNT];        /* summed device time of the class since cp4d_profile_begin       */
     uint64_t launches[CP4D_K_COUNT];  /* timed launches of the class                                      */

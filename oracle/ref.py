@@ -183,3 +183,60 @@ class Problem:
         L = lib().cp4d_ref_power(self._ref(), _p(x), C.c_int(int(n_steps)), C.c_int(int(use_k1)),
                                  C.c_int(int(use_k2)), C.c_int(int(folded)))
         return float(L), x
+
+
+class FrameProblem:
+    """The paper's own temporal discretisation, TEST INFRASTRUCTURE like everything in oracle/.
+
+    The primal variable is N_t time frames f(t_q) (4th axis of length N_t); frame q sits at the time of angle
+    q*N_theta/N_t (Eq. 11).  The coefficients entering Eq. (9) are
+        f_j = sum_q f(t_q) phi_j(t_q)                                              (L231-L237)
+    i.e. f_coef = f_frames @ Psi^T with Psi[j,q] = phi_j(t_q) = Phi[j, q*N_theta/N_t], so
+        K1' = K1 o analysis,   K1'^T = analysis^T o K1^T,
+    and K2 differences the frames (L225-L227; the scale alpha/Delta_theta is absorbed in lambda2, R4).
+    Written as plain numpy compositions of the operators of `Problem` (a matmul serves as the analysis step); the CP loop
+    below is Fig. 2 (L147-L168) line by line.
+    """
+
+    def __init__(self, n, nz, nd, n_angles, n_half_rot, m, phi, n_frames, lambda1=1e-3, lambda2=1.0):
+        assert n_angles % n_frames == 0
+        self.coef = Problem(n, nz, nd, n_angles, n_half_rot, m, phi, lambda1, lambda2)
+        self.psi = np.ascontiguousarray(np.asarray(phi, dtype=np.float64).reshape(m, n_angles)[:, ::n_angles // n_frames])
+        # grad / div / proxes only see the array shape: a Problem whose 4th axis has n_frames entries
+        self.frames = Problem(n, nz, nd, n_angles, n_half_rot, n_frames, np.zeros((n_frames, n_angles)), lambda1, lambda2)
+        self.n_frames, self.lambda1, self.lambda2 = n_frames, lambda1, lambda2
+        self.primal_shape, self.sino_shape = self.frames.primal_shape, self.coef.sino_shape
+
+    def analysis(self, u):
+        return np.ascontiguousarray(np.asarray(u, dtype=np.float64) @ self.psi.T)
+
+    def analysis_t(self, f):
+        return np.ascontiguousarray(np.asarray(f, dtype=np.float64) @ self.psi)
+
+    def forward(self, u, folded=False):
+        return self.coef.forward(self.analysis(u), folded=folded)
+
+    def adjoint(self, g, folded=False):
+        return self.analysis_t(self.coef.adjoint(g, folded=folded))
+
+    def grad(self, u):
+        return self.frames.grad(u)
+
+    def div(self, p):
+        return self.frames.div(p)
+
+    def zero_state(self):
+        return dict(f=np.zeros(self.primal_shape), ft=np.zeros(self.primal_shape),
+                    h1=np.zeros(self.sino_shape), h2=np.zeros((4,) + self.primal_shape))
+
+    def cp(self, g, state, tau, sigma, n_iters, theta=1.0, folded=False):
+        """Fig. 2, steps 3-6, on the frames; returns the number of clamped 4-vectors of the last step 4."""
+        g = np.asarray(g, dtype=np.float64)
+        ncl = 0
+        for _ in range(n_iters):
+            state["h1"] = self.frames.prox_f1(state["h1"], self.forward(state["ft"], folded), g, sigma)          # step 3
+            state["h2"], ncl = self.frames.prox_f2(state["h2"], self.grad(state["ft"]), sigma, self.lambda1)     # step 4
+            f_new = state["f"] - tau * self.adjoint(state["h1"], folded) + tau * self.div(state["h2"])           # step 5
+            state["ft"] = f_new + theta * (f_new - state["f"])                                                   # step 6
+            state["f"] = f_new
+        return ncl

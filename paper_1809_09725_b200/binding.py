@@ -29,10 +29,10 @@ class Params(C.Structure):
                 ("n_angles", C.c_int32), ("n_half_rot", C.c_int32), ("m", C.c_int32), ("device", C.c_int32),
                 ("phi_host", C.c_void_p), ("lambda1", C.c_float), ("lambda2", C.c_float),
                 ("theta_relax", C.c_float), ("workspace_dev", C.c_void_p), ("workspace_bytes", C.c_uint64),
-                ("stream", C.c_void_p)]
+                ("stream", C.c_void_p), ("n_frames", C.c_int32)]
 
 
-K_COUNT = 10
+K_COUNT = 11
 
 
 class Profile(C.Structure):
@@ -78,19 +78,20 @@ def lib():
 
 
 def make_params(n, nz, nd, n_angles, n_half_rot, m, phi=None, lambda1=1e-3, lambda2=1.0, theta=1.0, device=0,
-                workspace_ptr=0, workspace_bytes=0, stream=0, ny=None):
+                workspace_ptr=0, workspace_bytes=0, stream=0, ny=None, n_frames=0):
     p = Params()
     p.nx, p.ny, p.nz, p.nd = n, (n if ny is None else ny), nz, nd
     p.n_angles, p.n_half_rot, p.m, p.device = n_angles, n_half_rot, m, device
     p.phi_host = None if phi is None else phi.ctypes.data
     p.lambda1, p.lambda2, p.theta_relax = lambda1, lambda2, theta
     p.workspace_dev, p.workspace_bytes, p.stream = workspace_ptr or None, workspace_bytes, stream or None
+    p.n_frames = n_frames
     return p
 
 
-def workspace_bytes(n, nz, nd, n_angles, n_half_rot, m) -> int:
+def workspace_bytes(n, nz, nd, n_angles, n_half_rot, m, n_frames=0) -> int:
     out = C.c_uint64(0)
-    p = make_params(n, nz, nd, n_angles, n_half_rot, m)
+    p = make_params(n, nz, nd, n_angles, n_half_rot, m, n_frames=n_frames)
     r = lib().cp4d_workspace_bytes(C.byref(p), C.byref(out))
     if r:
         raise Cp4dError(r, lib().cp4d_strerror(r).decode())
@@ -100,21 +101,23 @@ def workspace_bytes(n, nz, nd, n_angles, n_half_rot, m) -> int:
 class Context:
     """One reconstruction problem on one GPU.  Tensors are torch CUDA float32, contiguous, layouts of cp4d.h."""
 
-    def __init__(self, n, nz, nd, n_angles, n_half_rot, m, phi, lambda1=1e-3, lambda2=1.0, theta=1.0, device=0):
+    def __init__(self, n, nz, nd, n_angles, n_half_rot, m, phi, lambda1=1e-3, lambda2=1.0, theta=1.0, device=0, n_frames=0):
         import torch
         self.torch = torch
         self.n, self.nz, self.nd, self.n_angles, self.n_half_rot, self.m = n, nz, nd, n_angles, n_half_rot, m
-        self.primal_shape, self.sino_shape = (nz, n, n, m), (nz, n_angles, nd)
-        self.V, self.S = nz * n * n * m, nz * n_angles * nd
+        self.n_frames = n_frames
+        mp = n_frames or m                                   # length of the primal 4th axis (frames or coefficients)
+        self.primal_shape, self.sino_shape = (nz, n, n, mp), (nz, n_angles, nd)
+        self.V, self.S = nz * n * n * mp, nz * n_angles * nd
         self.device = torch.device("cuda", device)
         self._phi = np.ascontiguousarray(phi, dtype=np.float32).reshape(m, n_angles)
-        nbytes = workspace_bytes(n, nz, nd, n_angles, n_half_rot, m)
+        nbytes = workspace_bytes(n, nz, nd, n_angles, n_half_rot, m, n_frames)
         with torch.cuda.device(self.device):
             self.workspace = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
             base = (self.workspace.data_ptr() + 255) // 256 * 256
             self.stream = torch.cuda.current_stream(self.device)
             p = make_params(n, nz, nd, n_angles, n_half_rot, m, self._phi, lambda1, lambda2, theta, device,
-                            base, nbytes, self.stream.cuda_stream)
+                            base, nbytes, self.stream.cuda_stream, n_frames=n_frames)
             h = C.c_void_p()
             r = lib().cp4d_create(C.byref(p), C.byref(h))
         if r:
@@ -122,13 +125,13 @@ class Context:
         self._h = h
 
     @classmethod
-    def from_config(cls, c, phi=None, device=0, **kw):
+    def from_config(cls, c, phi=None, device=0, n_frames=0, **kw):
         from . import synth
         if phi is None:
             phi = synth.basis_table(c.basis, c.m, c.n_angles)
         kw.setdefault("lambda1", c.lambda1)
         kw.setdefault("lambda2", c.lambda2)
-        return cls(c.n, c.nz, c.nd, c.n_angles, c.n_half_rot, c.m, phi, device=device, **kw)
+        return cls(c.n, c.nz, c.nd, c.n_angles, c.n_half_rot, c.m, phi, device=device, n_frames=n_frames, **kw)
 
     # -- helpers ---------------------------------------------------------------------------------
     def _ck(self, r):

@@ -23,10 +23,14 @@ int validate(const cp4d_params *p, Dims *d) {
     if (!(p->lambda1 >= 0.f) || !(p->theta_relax >= 0.f && p->theta_relax <= 1.f) || !std::isfinite(p->lambda2)) return CP4D_EINVAL;
     d->n = p->nx; d->nz = p->nz; d->nd = p->nd; d->na = p->n_angles; d->npi = p->n_half_rot;
     d->n0 = d->na / d->npi; d->m = p->m; d->Q = p->m / 4;
+    // frame mode (L214-L237): n_frames frames every n_angles/n_frames angles; the primal 4th axis is the frame index
+    if (p->n_frames < 0 || (p->n_frames > 0 && (p->n_frames % 4 || p->n_frames > MAX_M || p->n_angles % p->n_frames))) return CP4D_EINVAL;
+    d->nf = p->n_frames; d->mp = d->nf ? d->nf : d->m; d->Qp = d->mp / 4;
     d->tiles_1d = (d->n + TILE - 1) / TILE; d->tiles = d->tiles_1d * d->tiles_1d;
-    d->V = (int64_t)d->nz * d->n * d->n * d->m;
+    d->V = (int64_t)d->nz * d->n * d->n * d->mp;
+    d->Vc = (int64_t)d->nz * d->n * d->n * d->m;
     d->S = (int64_t)d->nz * d->na * d->nd;
-    d->slice4 = (int64_t)d->n * d->n * d->Q;
+    d->slice4 = (int64_t)d->n * d->n * d->Qp;
     // pads of the scratch rows: the window [bstart, bstart + WIN + 8) of a 32x32 tile (edge tiles reach past the grid) may
     // leave the detector by at most sqrt2 * E - (nd-1)/2 + 2 bins, E = largest |coordinate| a tile covers
     // (cp4d_create checks the exact values)
@@ -40,7 +44,7 @@ int validate(const cp4d_params *p, Dims *d) {
 }
 
 struct Carve {
-    uint64_t f, ft, bp, h2, h1, g, tmp_s, scratch, phi, ang, geo, red, total;
+    uint64_t f, ft, bp, h2, h1, g, tmp_s, scratch, phi, ang, geo, red, cf, cb, psi, total;
 };
 Carve carve(const Dims &d) {
     Carve c;
@@ -50,6 +54,8 @@ Carve carve(const Dims &d) {
     c.h1 = take(d.S * 4); c.g = take(d.S * 4); c.tmp_s = take(d.S * 4); c.scratch = take(d.scratch4 * 16);
     c.phi = take((uint64_t)d.m * d.na * 4); c.ang = take((uint64_t)d.n0 * sizeof(AngleTab));
     c.geo = take((uint64_t)d.tiles * d.n0 * sizeof(TileGeo)); c.red = take(64);
+    c.cf = c.cb = c.psi = 0;
+    if (d.nf) { c.cf = take(d.Vc * 4); c.cb = take(d.Vc * 4); c.psi = take((uint64_t)d.m * d.nf * 4); }
     c.total = o;
     return c;
 }
@@ -73,14 +79,20 @@ bool overlap(const void *a, uint64_t na, const void *b, uint64_t nb) {
 }
 bool bad_ptr(const void *p) { return !p || ((uintptr_t)p & 15); }
 
+// f is primal-shaped: the coefficient stack, or (frame mode) the frames, analysed into ctx->cf first
 int forward_into(cp4d_ctx *ctx, const float *f, int mode, float sigma, const float *g, float *out) {
+    if (ctx->d.nf) {
+        CK(launch_mix(ctx, f, ctx->cf, ctx->d.m, ctx->d.nf, ctx->d.nf, 1), "analysis");    // T(j,q) = psi[j*nf + q]
+        f = ctx->cf;
+    }
     CK(launch_forward_partial(ctx, f, ctx->scratch), "forward_partial");
     CK(launch_synth(ctx, ctx->scratch, mode, sigma, g, out), "synth");
     return CP4D_OK;
 }
 int adjoint_into(cp4d_ctx *ctx, const float *g, float *f) {
     CK(launch_fold(ctx, g, ctx->scratch), "fold");
-    CK(launch_backproject(ctx, ctx->scratch, f), "backproject");
+    CK(launch_backproject(ctx, ctx->scratch, ctx->d.nf ? ctx->cb : f), "backproject");
+    if (ctx->d.nf) CK(launch_mix(ctx, ctx->cb, f, ctx->d.nf, ctx->d.m, 1, ctx->d.nf), "analysis^T");  // T(q,j) = psi[j*nf + q]
     return CP4D_OK;
 }
 
@@ -138,6 +150,8 @@ int cp4d_create(const cp4d_params *p, cp4d_ctx **out) {
     ctx->f = (float *)(w + cv.f); ctx->ft = (float *)(w + cv.ft); ctx->bp = (float *)(w + cv.bp);
     ctx->h2 = (float *)(w + cv.h2); ctx->h1 = (float *)(w + cv.h1); ctx->g = (float *)(w + cv.g);
     ctx->tmp_s = (float *)(w + cv.tmp_s);
+    ctx->cf = d.nf ? (float *)(w + cv.cf) : nullptr; ctx->cb = d.nf ? (float *)(w + cv.cb) : nullptr;
+    ctx->psi = d.nf ? (float *)(w + cv.psi) : nullptr;
     ctx->scratch = (float4 *)(w + cv.scratch); ctx->phi = (float *)(w + cv.phi);
     ctx->ang = (AngleTab *)(w + cv.ang); ctx->geo = (TileGeo *)(w + cv.geo); ctx->red = (double *)(w + cv.red);
 
@@ -175,8 +189,13 @@ int cp4d_create(const cp4d_params *p, cp4d_ctx **out) {
             geo[(size_t)t * d.n0 + i].delta = (float)(p0 - bs);
         }
     }
+    // frame mode: Psi[j][q] = phi_j(t_q), t_q the time of angle q * n_angles / n_frames (L231-L237: f_j = sum_q f(t_q) phi_j(t_q))
+    std::vector<float> psi((size_t)d.m * (d.nf ? d.nf : 1));
+    for (int j = 0; j < d.m && d.nf; ++j)
+        for (int q = 0; q < d.nf; ++q) psi[(size_t)j * d.nf + q] = p->phi_host[(size_t)j * d.na + (size_t)q * (d.na / d.nf)];
     cudaError_t e;
-    if ((e = cudaMemcpyAsync(ctx->phi, p->phi_host, (size_t)d.m * d.na * 4, cudaMemcpyHostToDevice, ctx->stream)) != cudaSuccess ||
+    if ((d.nf && (e = cudaMemcpyAsync(ctx->psi, psi.data(), psi.size() * 4, cudaMemcpyHostToDevice, ctx->stream)) != cudaSuccess) ||
+        (e = cudaMemcpyAsync(ctx->phi, p->phi_host, (size_t)d.m * d.na * 4, cudaMemcpyHostToDevice, ctx->stream)) != cudaSuccess ||
         (e = cudaMemcpyAsync(ctx->ang, ang.data(), ang.size() * sizeof(AngleTab), cudaMemcpyHostToDevice, ctx->stream)) != cudaSuccess ||
         (e = cudaMemcpyAsync(ctx->geo, geo.data(), geo.size() * sizeof(TileGeo), cudaMemcpyHostToDevice, ctx->stream)) != cudaSuccess ||
         (e = cudaMemsetAsync(ctx->scratch, 0, (size_t)d.scratch4 * 16, ctx->stream)) != cudaSuccess ||
@@ -428,7 +447,7 @@ int cp4d_profile_end(cp4d_ctx *ctx, cp4d_profile *out) {
 }
 
 const char *cp4d_kernel_name(int k) {
-    static const char *names[CP4D_K_COUNT] = {"forward", "synth", "fold", "backproject", "grad", "div", "prox_f2", "update", "reduce", "misc"};
+    static const char *names[CP4D_K_COUNT] = {"forward", "synth", "fold", "backproject", "grad", "div", "prox_f2", "update", "reduce", "misc", "mix"};
     return (k >= 0 && k < CP4D_K_COUNT) ? names[k] : "?";
 }
 

@@ -34,10 +34,13 @@ struct AngleTab {
 };
 
 struct Dims {
-    int n, nz, nd, na, npi, n0, m, Q;  // Q = m/4 float4 chunks per voxel
+    int n, nz, nd, na, npi, n0, m, Q;  // Q = m/4 float4 chunks per voxel of a coefficient stack
+    int nf, mp, Qp;                    // frame mode: nf frames (0 = coefficient mode); mp = nf ? nf : m is the
+                                       // length of the primal 4th axis, Qp = mp/4
+    int64_t Vc;                        // elements of a coefficient stack nz*n*n*m (== V in coefficient mode)
     int tiles_1d, tiles;               // ceil(n/TILE), tiles_1d^2
-    int64_t V, S;                      // elements of a primal array / a sinogram
-    int64_t slice4;                    // float4 per slice: n*n*Q
+    int64_t V, S;                      // elements of a primal array nz*n*n*mp / a sinogram
+    int64_t slice4;                    // float4 per primal slice: n*n*Qp
     int gp, gpl;                       // row pitch / left pad (float4) of the projector scratch: a row holds bins -gpl .. gp-gpl-1
     int64_t scratch4;                  // float4 of projector scratch: nz*n0*Q*gp
 };
@@ -53,6 +56,7 @@ struct cp4d_ctx {
     cudaStream_t stream;
     // workspace carve-up (device pointers)
     float *f, *ft, *bp, *h2, *h1, *g, *tmp_s;
+    float *cf, *cb, *psi;      // frame mode: coefficient stacks (analysis output, backprojection output), Psi[j][q] = phi_j(t_q)
     float4 *scratch;           // forward partial ray sums P / folded sinogram gt: [z][i][jc][gpl + b] float4, pitch gp;
                                // the pads stay zero, so every tile window of the backprojector is readable memory
     float *phi;                // [j][k]
@@ -105,6 +109,8 @@ cudaError_t launch_forward_partial(cp4d_ctx *c, const float *f, float4 *P);
 cudaError_t launch_backproject(cp4d_ctx *c, const float4 *gt, float *f_out);
 int bp_pattern(float c, float s);  // host: pattern index in [0, BP_NPAT) or -1
 uint32_t bp_pattern_fl(int pat);   // host: the pattern's FL_v packed 4 bits each
+// out[v][a] = sum_b T(a,b) in[v][b] per voxel v, T(a,b) = psi[a*sa + b*sb]  (frame <-> coefficient contraction, L231-L237)
+cudaError_t launch_mix(cp4d_ctx *c, const float *in, float *out, int na_out, int nb_in, int sa, int sb);
 cudaError_t launch_tv_sum(cp4d_ctx *c, const float *f, double *slot);                       // sum |K2 f|_2
 cudaError_t launch_kkt_sum(cp4d_ctx *c, const float *bp, const float *h2, double *slot);    // sum (bp - div h2)^2
 cudaError_t launch_sumsq_dot(cp4d_ctx *c, const float *x, const float *y, uint64_t n, double *slot);

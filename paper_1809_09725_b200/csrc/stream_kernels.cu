@@ -157,7 +157,7 @@ __global__ void __launch_bounds__(256) k_div(const float *__restrict__ p, float 
 static StreamArgs make_args(const cp4d_ctx *c, dim3 &grid, dim3 &block) {
     const Dims &d = c->d;
     StreamArgs a;
-    a.n = d.n; a.nz = d.nz; a.Q = d.Q; a.slice4 = d.slice4; a.V4 = d.V / 4; a.lambda2 = c->lambda2;
+    a.n = d.n; a.nz = d.nz; a.Q = d.Qp; a.slice4 = d.slice4; a.V4 = d.V / 4; a.lambda2 = c->lambda2;
     block = dim3(256);
     const int64_t bx = (d.slice4 + 255) / 256;
     // enough CTAs to fill 148 SMs x 8 resident CTAs a few times over; otherwise split z
@@ -199,6 +199,49 @@ cudaError_t launch_update(cp4d_ctx *c, float tau, const float *bp, const float *
     dim3 g, b;
     StreamArgs a = make_args(c, g, b);
     k_div<1><<<g, b, 0, c->stream>>>(h2, f, a, bp, ft, tau, c->theta, nullptr);
+    c->launches++;
+    return cudaGetLastError();
+}
+
+// ---------------------------------------------------------------------------------------------------
+// frame <-> coefficient contraction per voxel:  out[v][a] = sum_b T(a,b) in[v][b]
+//   analysis     f_j = sum_q phi_j(t_q) f(t_q):  a = j, b = q;   its transpose (after K1^T):  a = q, b = j
+// One thread per (voxel, 4 outputs); T sits in shared memory as Tt[b][a]; HBM-bound (reads NB, writes NA floats per voxel).
+// ---------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) k_mix(const float4 *__restrict__ in, float4 *__restrict__ out, const float *__restrict__ psi,
+                                             int64_t nvox, int QA, int QB, int sa, int sb) {
+    extern __shared__ float Tt[];  // [NB][NA]
+    const int NA = 4 * QA, NB = 4 * QB;
+    for (int t = threadIdx.x; t < NA * NB; t += blockDim.x) {
+        const int b = t / NA, a = t % NA;
+        Tt[t] = psi[a * sa + b * sb];
+    }
+    __syncthreads();
+    const int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (e >= nvox * QA) return;
+    const int64_t v = e / QA;
+    const int ca = (int)(e % QA);
+    float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
+    const float4 *row = in + v * QB;
+    for (int bc = 0; bc < QB; ++bc) {
+        const float4 x = ld4(row + bc);
+        const float4 *T4 = reinterpret_cast<const float4 *>(Tt + (4 * bc) * NA + 4 * ca);
+        const float4 t0 = T4[0], t1 = T4[NA / 4], t2 = T4[2 * (NA / 4)], t3 = T4[3 * (NA / 4)];
+        acc.x = fmaf(t0.x, x.x, fmaf(t1.x, x.y, fmaf(t2.x, x.z, fmaf(t3.x, x.w, acc.x))));
+        acc.y = fmaf(t0.y, x.x, fmaf(t1.y, x.y, fmaf(t2.y, x.z, fmaf(t3.y, x.w, acc.y))));
+        acc.z = fmaf(t0.z, x.x, fmaf(t1.z, x.y, fmaf(t2.z, x.z, fmaf(t3.z, x.w, acc.z))));
+        acc.w = fmaf(t0.w, x.x, fmaf(t1.w, x.y, fmaf(t2.w, x.z, fmaf(t3.w, x.w, acc.w))));
+    }
+    out[e] = acc;
+}
+
+cudaError_t launch_mix(cp4d_ctx *c, const float *in, float *out, int na_out, int nb_in, int sa, int sb) {
+    ProfScope ps(c, CP4D_K_MIX);
+    const Dims &d = c->d;
+    const int64_t nvox = (int64_t)d.nz * d.n * d.n;
+    const int64_t total = nvox * (na_out / 4);
+    k_mix<<<(unsigned)((total + 255) / 256), 256, (size_t)na_out * nb_in * sizeof(float), c->stream>>>(
+        reinterpret_cast<const float4 *>(in), reinterpret_cast<float4 *>(out), c->psi, nvox, na_out / 4, nb_in / 4, sa, sb);
     c->launches++;
     return cudaGetLastError();
 }

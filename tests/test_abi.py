@@ -45,7 +45,8 @@ def test_workspace_bytes_counts_state(L):
     assert binding.workspace_bytes(c.n, c.nz, c.nd, c.n_angles, c.n_half_rot, c.m) < 170e9   # fits 180 GB HBM
 
 
-@pytest.mark.parametrize("bad", [dict(ny=31), dict(m=6), dict(m=36), dict(n_half_rot=3), dict(nd=1), dict(nz=0), dict(lambda1=-1.0)])
+@pytest.mark.parametrize("bad", [dict(ny=31), dict(m=6), dict(m=36), dict(n_half_rot=3), dict(nd=1), dict(nz=0), dict(lambda1=-1.0),
+                                 dict(n_frames=6), dict(n_frames=-4), dict(n_frames=12), dict(n_frames=36)])
 def test_host_validation(L, bad):
     from paper_1809_09725_b200 import binding
     kw = dict(n=32, nz=1, nd=32, n_angles=128, n_half_rot=4, m=4)
@@ -53,6 +54,16 @@ def test_host_validation(L, bad):
     p = binding.make_params(**kw)
     out = C.c_uint64(0)
     assert L.cp4d_workspace_bytes(C.byref(p), C.byref(out)) == binding.EINVAL
+
+
+def test_frame_mode_workspace(L):
+    """Frame mode (n_frames > 0): primal arrays have n_frames planes, plus two coefficient stacks and the Psi table."""
+    from paper_1809_09725_b200 import binding
+    n, nz, nd, na, npi, m, nt = 64, 4, 64, 96, 2, 16, 8
+    a = binding.workspace_bytes(n, nz, nd, na, npi, m)
+    b = binding.workspace_bytes(n, nz, nd, na, npi, m, n_frames=nt)
+    vox = nz * n * n
+    assert b - a == pytest.approx((7 * (nt - m) + 2 * m) * vox * 4, abs=1 << 16)
 
 
 def test_create_needs_workspace_and_device(L):

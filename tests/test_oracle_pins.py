@@ -338,3 +338,58 @@ def test_synthetic_data_is_exact_radon_of_disks(oracle):
     P = oracle.Problem(c.n, 1, c.nd, c.n_angles, 1, 1, np.ones((1, c.n_angles)))
     gp = P.forward(img.reshape(P.primal_shape))
     assert np.linalg.norm(gp - g) / np.linalg.norm(g) < 3e-2
+
+
+# ---------------------------------------------------------------- P9: the paper's frame discretisation (L214-L237)
+def _frame_problem(oracle, n_frames, basis="fourier", m=4, n=8, nz=2, nd=8, n_angles=16, n_half_rot=2, lambda1=0.05, lambda2=1.5):
+    phi = synth.basis_table(basis, m, n_angles)
+    return oracle.FrameProblem(n, nz, nd, n_angles, n_half_rot, m, phi, n_frames, lambda1=lambda1, lambda2=lambda2), phi
+
+
+def test_p9_frame_operator_is_dense_K1_times_analysis(oracle):
+    """K1' = K1 (I (x) Psi) with Psi[j,q] = phi_j(t_q) typed here from the definition t_q = (q N_theta/N_t)/N_theta (Eq. 11)."""
+    F, phi = _frame_problem(oracle, 8)
+    P = F.coef
+    t_q = (np.arange(8) * (P.n_angles // 8)) / P.n_angles
+    psi = np.stack([np.ones(8), np.cos(2 * np.pi * t_q), np.sin(2 * np.pi * t_q), np.cos(4 * np.pi * t_q)])   # config-1 basis list
+    K = dense.dense_K1(P.n, P.nz, P.nd, P.n_angles, P.n_half_rot, P.m, P.phi) @ np.kron(np.eye(P.nz * P.n * P.n), psi)
+    rng = np.random.default_rng(5)
+    u, g = rng.standard_normal(F.primal_shape), rng.standard_normal(F.sino_shape)
+    np.testing.assert_allclose(F.forward(u).ravel(), K @ u.ravel(), atol=1e-12)
+    np.testing.assert_allclose(F.adjoint(g).ravel(), K.T @ g.ravel(), atol=1e-12)
+    assert abs(np.vdot(F.forward(u, folded=True), g) - np.vdot(u, F.adjoint(g, folded=True))) <= 1e-12 * np.linalg.norm(u) * np.linalg.norm(g) * 50
+
+
+def test_p9_cardinal_basis_with_Nt_equal_M_is_the_coefficient_model(oracle):
+    """With the box basis and N_t = M, phi_j(t_q) = delta_jq: frames are coefficients (C1) and the two CP loops coincide."""
+    F, phi = _frame_problem(oracle, 4, basis="box")
+    np.testing.assert_array_equal(F.psi, np.eye(4))
+    P = F.coef
+    g = np.random.default_rng(6).standard_normal(P.sino_shape)
+    sa, sb = P.zero_state(), F.zero_state()
+    P.cp(g, sa, 0.01, 0.02, 6)
+    F.cp(g, sb, 0.01, 0.02, 6)
+    for k in ("f", "ft", "h1", "h2"):
+        np.testing.assert_allclose(sb[k], sa[k], rtol=0, atol=1e-13)
+
+
+def test_p9_frame_cp_step_matches_dense_algebra(oracle):
+    F, phi = _frame_problem(oracle, 8)
+    P = F.coef
+    K1 = dense.dense_K1(P.n, P.nz, P.nd, P.n_angles, P.n_half_rot, P.m, P.phi) @ np.kron(np.eye(P.nz * P.n * P.n), F.psi)
+    K2 = dense.dense_K2(P.n, P.nz, 8, 1.5)
+    rng = np.random.default_rng(7)
+    st = dict(f=rng.standard_normal(F.primal_shape), ft=rng.standard_normal(F.primal_shape),
+              h1=rng.standard_normal(F.sino_shape), h2=0.05 * rng.standard_normal((4,) + F.primal_shape))
+    g = rng.standard_normal(F.sino_shape)
+    tau, sigma, lam1 = 0.02, 0.03, 0.05
+    h1 = (st["h1"].ravel() + sigma * (K1 @ st["ft"].ravel() - g.ravel())) / (1 + sigma)
+    q = (st["h2"].ravel() + sigma * (K2 @ st["ft"].ravel())).reshape(4, -1)
+    h2 = q / np.maximum(1.0, np.sqrt((q ** 2).sum(0)) / lam1)
+    f = st["f"].ravel() - tau * (K1.T @ h1) - tau * (K2.T @ h2.ravel())
+    ft = 2 * f - st["f"].ravel()
+    F.cp(g, st, tau, sigma, 1)
+    np.testing.assert_allclose(st["h1"].ravel(), h1, atol=1e-12)
+    np.testing.assert_allclose(st["h2"].reshape(4, -1), h2, atol=1e-12)
+    np.testing.assert_allclose(st["f"].ravel(), f, atol=1e-12)
+    np.testing.assert_allclose(st["ft"].ravel(), ft, atol=1e-12)
