@@ -5,6 +5,8 @@
 // Layout f[z][iy][ix][j] (j fastest): one thread owns one float4 (4 consecutive coefficients j of one
 // voxel) and walks along z, so the z neighbour is carried in registers and every 4D element is read
 // from HBM once; x/y/t neighbours are served by L1/L2.  All global accesses are 16-byte, fully coalesced.
+#include <algorithm>
+
 #include "cp4d_internal.cuh"
 
 namespace cp4d {
@@ -217,22 +219,23 @@ __global__ void __launch_bounds__(256) k_mix(const float4 *__restrict__ in, floa
         Tt[t] = psi[a * sa + b * sb];
     }
     __syncthreads();
-    const int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (e >= nvox * QA) return;
-    const int64_t v = e / QA;
-    const int ca = (int)(e % QA);
-    float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
-    const float4 *row = in + v * QB;
-    for (int bc = 0; bc < QB; ++bc) {
-        const float4 x = ld4(row + bc);
-        const float4 *T4 = reinterpret_cast<const float4 *>(Tt + (4 * bc) * NA + 4 * ca);
-        const float4 t0 = T4[0], t1 = T4[NA / 4], t2 = T4[2 * (NA / 4)], t3 = T4[3 * (NA / 4)];
-        acc.x = fmaf(t0.x, x.x, fmaf(t1.x, x.y, fmaf(t2.x, x.z, fmaf(t3.x, x.w, acc.x))));
-        acc.y = fmaf(t0.y, x.x, fmaf(t1.y, x.y, fmaf(t2.y, x.z, fmaf(t3.y, x.w, acc.y))));
-        acc.z = fmaf(t0.z, x.x, fmaf(t1.z, x.y, fmaf(t2.z, x.z, fmaf(t3.z, x.w, acc.z))));
-        acc.w = fmaf(t0.w, x.x, fmaf(t1.w, x.y, fmaf(t2.w, x.z, fmaf(t3.w, x.w, acc.w))));
+    const int64_t total = nvox * QA, stride = (int64_t)gridDim.x * blockDim.x;
+    for (int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < total; e += stride) {
+        const int64_t v = e / QA;
+        const int ca = (int)(e % QA);
+        float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
+        const float4 *row = in + v * QB;
+        for (int bc = 0; bc < QB; ++bc) {
+            const float4 x = ld4(row + bc);
+            const float4 *T4 = reinterpret_cast<const float4 *>(Tt + (4 * bc) * NA + 4 * ca);
+            const float4 t0 = T4[0], t1 = T4[NA / 4], t2 = T4[2 * (NA / 4)], t3 = T4[3 * (NA / 4)];
+            acc.x = fmaf(t0.x, x.x, fmaf(t1.x, x.y, fmaf(t2.x, x.z, fmaf(t3.x, x.w, acc.x))));
+            acc.y = fmaf(t0.y, x.x, fmaf(t1.y, x.y, fmaf(t2.y, x.z, fmaf(t3.y, x.w, acc.y))));
+            acc.z = fmaf(t0.z, x.x, fmaf(t1.z, x.y, fmaf(t2.z, x.z, fmaf(t3.z, x.w, acc.z))));
+            acc.w = fmaf(t0.w, x.x, fmaf(t1.w, x.y, fmaf(t2.w, x.z, fmaf(t3.w, x.w, acc.w))));
+        }
+        out[e] = acc;
     }
-    out[e] = acc;
 }
 
 cudaError_t launch_mix(cp4d_ctx *c, const float *in, float *out, int na_out, int nb_in, int sa, int sb) {
@@ -240,7 +243,8 @@ cudaError_t launch_mix(cp4d_ctx *c, const float *in, float *out, int na_out, int
     const Dims &d = c->d;
     const int64_t nvox = (int64_t)d.nz * d.n * d.n;
     const int64_t total = nvox * (na_out / 4);
-    k_mix<<<(unsigned)((total + 255) / 256), 256, (size_t)na_out * nb_in * sizeof(float), c->stream>>>(
+    const int64_t blocks = std::min<int64_t>((total + 255) / 256, 148 * 16);   // grid-stride: Psi is staged once per CTA
+    k_mix<<<(unsigned)blocks, 256, (size_t)na_out * nb_in * sizeof(float), c->stream>>>(
         reinterpret_cast<const float4 *>(in), reinterpret_cast<float4 *>(out), c->psi, nvox, na_out / 4, nb_in / 4, sa, sb);
     c->launches++;
     return cudaGetLastError();
