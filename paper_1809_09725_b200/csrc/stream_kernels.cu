@@ -289,11 +289,20 @@ __global__ void __launch_bounds__(128) k_fold(const float *__restrict__ g, float
         float acc[m];
 #pragma unroll
         for (int j = 0; j < m; ++j) acc[j] = 0.f;
-        for (int q = 0; q < npi; ++q) {
-            const int bb = (q & 1) ? nd - 1 - b : b;
-            const float gv = __ldg(g + ((int64_t)z * na + q * n0 + i) * nd + bb);
+        for (int q0 = 0; q0 < npi; q0 += 4) {     // 4 half-rotations per batch: their loads are in flight together
+            float gv[4];
 #pragma unroll
-            for (int j = 0; j < m; ++j) acc[j] = fmaf(phis[q * m + j], gv, acc[j]);
+            for (int u = 0; u < 4; ++u) {
+                const int q = min(q0 + u, npi - 1), bb = (q & 1) ? nd - 1 - b : b;
+                gv[u] = __ldg(g + ((int64_t)z * na + q * n0 + i) * nd + bb);
+            }
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                if (q0 + u < npi) {
+#pragma unroll
+                    for (int j = 0; j < m; ++j) acc[j] = fmaf(phis[(q0 + u) * m + j], gv[u], acc[j]);
+                }
+            }
         }
 #pragma unroll
         for (int jc = 0; jc < Q; ++jc)
@@ -318,14 +327,24 @@ __global__ void __launch_bounds__(128) k_synth(const float4 *__restrict__ P, int
             const float4 v = P[(((int64_t)z * n0 + i) * Q + jc) * gp + gpl + b];
             acc[4 * jc] = v.x; acc[4 * jc + 1] = v.y; acc[4 * jc + 2] = v.z; acc[4 * jc + 3] = v.w;
         }
-        for (int q = 0; q < npi; ++q) {
-            const int bb = (q & 1) ? nd - 1 - b : b;
-            float v = 0.f;
+        for (int q0 = 0; q0 < npi; q0 += 4) {     // 4 half-rotations per batch: their loads are in flight together
+            float ho[4], gg[4];
+            int64_t idx[4];
 #pragma unroll
-            for (int j = 0; j < m; ++j) v = fmaf(phis[q * m + j], acc[j], v);
-            const int64_t idx = ((int64_t)z * na + q * n0 + i) * nd + bb;
-            if (mode == 0) out[idx] = v;
-            else out[idx] = (out[idx] + sigma * (v - __ldg(g + idx))) * rs;
+            for (int u = 0; u < 4; ++u) {
+                const int q = min(q0 + u, npi - 1), bb = (q & 1) ? nd - 1 - b : b;
+                idx[u] = ((int64_t)z * na + q * n0 + i) * nd + bb;
+                if (mode != 0) { ho[u] = out[idx[u]]; gg[u] = __ldg(g + idx[u]); }
+            }
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                if (q0 + u < npi) {
+                    float v = 0.f;
+#pragma unroll
+                    for (int j = 0; j < m; ++j) v = fmaf(phis[(q0 + u) * m + j], acc[j], v);
+                    out[idx[u]] = (mode == 0) ? v : (ho[u] + sigma * (v - gg[u])) * rs;
+                }
+            }
         }
     }
 }
