@@ -200,6 +200,8 @@ int cp4d_create(const cp4d_params *p, cp4d_ctx **out) {
         (e = cudaMemcpyAsync(ctx->geo, geo.data(), geo.size() * sizeof(TileGeo), cudaMemcpyHostToDevice, ctx->stream)) != cudaSuccess ||
         (e = cudaMemsetAsync(ctx->scratch, 0, (size_t)d.scratch4 * 16, ctx->stream)) != cudaSuccess ||
         (e = cudaStreamSynchronize(ctx->stream)) != cudaSuccess) {
+        ctx->err = cudaGetErrorString(e);   // (the context dies with the error: the caller only sees CP4D_ECUDA)
+        cudaGetLastError();
         delete ctx;
         return CP4D_ECUDA;
     }
