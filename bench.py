@@ -62,13 +62,16 @@ def alu_peak_tflops(sm_mhz: float) -> float:
 # ------------------------------------------------------------------------------------------------------
 def algorithmic_work(c, n_frames=0):
     V, S = c.V, c.S
-    Vc = V                                               # coefficient stack (projectors)
+    n0 = c.n_theta0
+    mproj = c.m                                          # images the projector pair carries per voxel
+    Vc = V                                               # coefficient stack (K1 o A path)
     if n_frames:
         V = V // c.m * n_frames                          # primal arrays hold frames
-    n0 = c.n_theta0
-    ray_fma = 2 * c.m * c.n * c.n * c.nz * n0            # 2 taps x m per voxel-step per base-angle ray
-    syn_fma = c.m * c.n_angles * c.nd * c.nz             # m-wide synthesis / analysis per sinogram sample
-    gt = c.nz * n0 * c.nd * c.m                          # folded sinogram / partial ray sums, elements
+        if n_frames <= c.m:                              # collapsed frame mode: the projectors carry the N_t frames
+            mproj, Vc = n_frames, 0
+    ray_fma = 2 * mproj * c.n * c.n * c.nz * n0          # 2 taps x images per voxel-step per base-angle ray
+    syn_fma = mproj * c.n_angles * c.nd * c.nz           # synthesis / analysis per sinogram sample
+    gt = c.nz * n0 * c.nd * mproj                        # folded sinogram / partial ray sums, elements
     return {
         # name: (bound, work per launch [flop or byte])
         "forward": ("alu", 2.0 * ray_fma),

@@ -26,6 +26,11 @@ int validate(const cp4d_params *p, Dims *d) {
     // frame mode (L214-L237): n_frames frames every n_angles/n_frames angles; the primal 4th axis is the frame index
     if (p->n_frames < 0 || (p->n_frames > 0 && (p->n_frames % 4 || p->n_frames > MAX_M || p->n_angles % p->n_frames))) return CP4D_EINVAL;
     d->nf = p->n_frames; d->mp = d->nf ? d->nf : d->m; d->Qp = d->mp / 4;
+    d->mb = p->m;
+    // Collapsed frame mode (N_t <= M): K1 o A = sum_q W[k,q] R f(t_q) with W[k,q] = sum_j phi_j(t_k) phi_j(t_q), so the projector
+    // pair can carry the N_t frames themselves with the N_t x N_theta table W^T in place of Phi: no analysis pass, N_t/M of the
+    // projector work.  From here on it is a coefficient-mode problem with m = N_t (cp4d_create builds the table).
+    if (d->nf && d->nf <= d->m) { d->m = d->nf; d->Q = d->nf / 4; d->nf = 0; }
     d->tiles_1d = (d->n + TILE - 1) / TILE; d->tiles = d->tiles_1d * d->tiles_1d;
     d->V = (int64_t)d->nz * d->n * d->n * d->mp;
     d->Vc = (int64_t)d->nz * d->n * d->n * d->m;
@@ -55,7 +60,7 @@ Carve carve(const Dims &d) {
     c.phi = take((uint64_t)d.m * d.na * 4); c.ang = take((uint64_t)d.n0 * sizeof(AngleTab));
     c.geo = take((uint64_t)d.tiles * d.n0 * sizeof(TileGeo)); c.red = take(64);
     c.cf = c.cb = c.psi = 0;
-    if (d.nf) { c.cf = take(d.Vc * 4); c.cb = take(d.Vc * 4); c.psi = take((uint64_t)d.m * d.nf * 4); }
+    if (d.nf) { c.cf = take(d.Vc * 4); c.cb = take(d.Vc * 4); c.psi = take((uint64_t)d.mb * d.nf * 4); }
     c.total = o;
     return c;
 }
@@ -82,7 +87,7 @@ bool bad_ptr(const void *p) { return !p || ((uintptr_t)p & 15); }
 // f is primal-shaped: the coefficient stack, or (frame mode) the frames, analysed into ctx->cf first
 int forward_into(cp4d_ctx *ctx, const float *f, int mode, float sigma, const float *g, float *out) {
     if (ctx->d.nf) {
-        CK(launch_mix(ctx, f, ctx->cf, ctx->d.m, ctx->d.nf, ctx->d.nf, 1), "analysis");    // T(j,q) = psi[j*nf + q]
+        CK(launch_mix(ctx, f, ctx->cf, ctx->d.m, ctx->d.nf, ctx->d.nf, 1), "analysis");     // (here m == mb)    // T(j,q) = psi[j*nf + q]
         f = ctx->cf;
     }
     CK(launch_forward_partial(ctx, f, ctx->scratch), "forward_partial");
@@ -190,12 +195,23 @@ int cp4d_create(const cp4d_params *p, cp4d_ctx **out) {
         }
     }
     // frame mode: Psi[j][q] = phi_j(t_q), t_q the time of angle q * n_angles / n_frames (L231-L237: f_j = sum_q f(t_q) phi_j(t_q))
-    std::vector<float> psi((size_t)d.m * (d.nf ? d.nf : 1));
-    for (int j = 0; j < d.m && d.nf; ++j)
-        for (int q = 0; q < d.nf; ++q) psi[(size_t)j * d.nf + q] = p->phi_host[(size_t)j * d.na + (size_t)q * (d.na / d.nf)];
+    const int ntf = p->n_frames, fstride = ntf ? d.na / ntf : 0;
+    std::vector<float> psi((size_t)d.mb * (d.nf ? d.nf : 1));
+    for (int j = 0; j < d.mb && d.nf; ++j)
+        for (int q = 0; q < d.nf; ++q) psi[(size_t)j * d.nf + q] = p->phi_host[(size_t)j * d.na + (size_t)q * fstride];
+    // the table the projector pair uses: Phi itself, or in collapsed frame mode W^T[q][k] = sum_j phi_j(t_q) phi_j(t_k) (fp64 sums)
+    std::vector<float> phi_eff((size_t)d.m * d.na);
+    const bool collapsed = ntf > 0 && d.nf == 0;
+    for (int r = 0; r < d.m; ++r)
+        for (int k = 0; k < d.na; ++k) {
+            if (!collapsed) { phi_eff[(size_t)r * d.na + k] = p->phi_host[(size_t)r * d.na + k]; continue; }
+            double acc = 0.0;
+            for (int j = 0; j < d.mb; ++j) acc += (double)p->phi_host[(size_t)j * d.na + (size_t)r * fstride] * (double)p->phi_host[(size_t)j * d.na + k];
+            phi_eff[(size_t)r * d.na + k] = (float)acc;
+        }
     cudaError_t e;
     if ((d.nf && (e = cudaMemcpyAsync(ctx->psi, psi.data(), psi.size() * 4, cudaMemcpyHostToDevice, ctx->stream)) != cudaSuccess) ||
-        (e = cudaMemcpyAsync(ctx->phi, p->phi_host, (size_t)d.m * d.na * 4, cudaMemcpyHostToDevice, ctx->stream)) != cudaSuccess ||
+        (e = cudaMemcpyAsync(ctx->phi, phi_eff.data(), (size_t)d.m * d.na * 4, cudaMemcpyHostToDevice, ctx->stream)) != cudaSuccess ||
         (e = cudaMemcpyAsync(ctx->ang, ang.data(), ang.size() * sizeof(AngleTab), cudaMemcpyHostToDevice, ctx->stream)) != cudaSuccess ||
         (e = cudaMemcpyAsync(ctx->geo, geo.data(), geo.size() * sizeof(TileGeo), cudaMemcpyHostToDevice, ctx->stream)) != cudaSuccess ||
         (e = cudaMemsetAsync(ctx->scratch, 0, (size_t)d.scratch4 * 16, ctx->stream)) != cudaSuccess ||

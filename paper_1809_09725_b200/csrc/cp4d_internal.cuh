@@ -38,6 +38,8 @@ struct Dims {
     int nf, mp, Qp;                    // frame mode: nf frames (0 = coefficient mode); mp = nf ? nf : m is the
                                        // length of the primal 4th axis, Qp = mp/4
     int64_t Vc;                        // elements of a coefficient stack nz*n*n*m (== V in coefficient mode)
+    int mb;                            // rows of the caller's basis table phi_host (the paper's M); m above is what the
+                                       // projector pair carries per voxel: M, or N_t in collapsed frame mode
     int tiles_1d, tiles;               // ceil(n/TILE), tiles_1d^2
     int64_t V, S;                      // elements of a primal array nz*n*n*mp / a sinogram
     int64_t slice4;                    // float4 per primal slice: n*n*Qp

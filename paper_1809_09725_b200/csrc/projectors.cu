@@ -5,8 +5,9 @@
 // frame sum_j Phi[j,k] f_j is never materialised.  The per-tile partial ray sums go to P[z][i][jq][b] with one vector RED
 // per ray and coefficient chunk; the synthesis with Phi (and the F1* prox) is the k_synth epilogue in stream_kernels.cu.
 //
-//   k_forward_rays16  : m % 16 == 0 (configs 3-5).  8 lanes per ray, voxel-major tile, conflict-free full wavefronts.
-//   k_forward_partial : any m % 4 == 0.  One thread per ray, coefficient-plane-major tile.
+//   k_forward_rays<4|2> : m % 16 == 0 (configs 3-5) / m % 8 == 0.  8 lanes per ray, voxel-major tile, conflict-free full
+//                         wavefronts.
+//   k_forward_partial<1>: m % 8 != 0.  One thread per ray, coefficient-plane-major tile.
 //
 // The backprojector lives in backproject.cu.
 //
@@ -117,7 +118,7 @@ __global__ void __launch_bounds__(256) k_forward_partial(const float *__restrict
 
 
 // ---------------------------------------------------------------------------------------------------
-// forward, 16 coefficients per ray (m % 16 == 0): 8 lanes per ray, conflict-free shared-memory wavefronts
+// forward, 16 or 8 coefficients per ray (m % 8 == 0): 8 lanes per ray, conflict-free shared-memory wavefronts
 // ---------------------------------------------------------------------------------------------------
 // The one-thread-per-ray kernel above is bound by shared-memory wavefronts, a third of which are bank conflicts (8 adjacent
 // rays span up to 10 rows, rows 8 apart share a bank group) or partially filled.  Here a ray is served by 8 lanes
@@ -127,31 +128,46 @@ __global__ void __launch_bounds__(256) k_forward_partial(const float *__restrict
 // conflict-free 128 B wavefront per LDS.128.  Rays that step over rows use a second pass over a transposed copy of the tile,
 // so both passes run the same code.  The two step parities are summed with one shuffle before the vector RED into P.
 constexpr int FR_RAYS = WIN;                 // rays of a tile window
-constexpr int FR_THREADS = FR_RAYS * 8;      // 384
-constexpr int RSV = TILE + 2;                // voxels per tile row incl. the zero border; even
-constexpr int FR_UNROLL = 4;                 // steps per lane and chunk: a chunk is 2 * FR_UNROLL columns of the chord
-static_assert(RSV % 2 == 0, "row pitch must be even for conflict-free step pairs");
+constexpr int FR_THREADS = FR_RAYS * 8;      // 384: 8 lanes per ray
+constexpr int FR_UNROLL = 4;                 // steps per lane and chunk
 
-__global__ void __launch_bounds__(FR_THREADS, 3) k_forward_rays16(const float *__restrict__ f, float4 *__restrict__ P, ProjArgs a) {
-    extern __shared__ float4 tile[];  // [TILE+3][RSV][4]: 1-voxel zero border, plus a second zero row at the bottom
+// JQ = coefficient chunks (float4) per voxel: 4 (16 coefficients, 64 B voxels, 2 step phases) or 2 (8 coefficients, 32 B
+// voxels, 4 step phases).  Lane = (phase sp, chunk jq); the 8 lanes of a quarter warp read the voxels (r_s, k+s), s < NPH,
+// whose blocks of 16*JQ bytes sit at (row*RSV + col) mod NPH = (k + s + 1) mod NPH when RSV % NPH == 0: NPH distinct
+// residues, i.e. one full conflict-free 128 B wavefront per LDS.128.
+template <int JQ>
+struct FwRays {
+    static constexpr int NPH = 8 / JQ;                          // step phases = lanes per (ray, chunk)
+    static constexpr int RSV = JQ == 4 ? TILE + 2 : TILE + 4;   // voxels per tile row incl. the zero border; multiple of NPH
+    static constexpr int UNROLL = FR_UNROLL;                    // steps per lane and chunk (2 and 8 were slower for JQ = 2)
+    static constexpr int CHUNK = NPH * UNROLL;                  // columns of the chord per loop trip
+    static constexpr size_t SMEM = (size_t)(TILE + 3) * RSV * JQ * sizeof(float4);
+    static_assert(RSV % NPH == 0, "row pitch must be a multiple of the number of step phases");
+};
+
+template <int JQ>
+__global__ void __launch_bounds__(FR_THREADS, 3) k_forward_rays(const float *__restrict__ f, float4 *__restrict__ P, ProjArgs a) {
+    using C = FwRays<JQ>;
+    constexpr int NPH = C::NPH, RSV = C::RSV, CHUNK = C::CHUNK, UNROLL = C::UNROLL;
+    extern __shared__ float4 tile[];  // [TILE+3][RSV][JQ]: 1-voxel zero border, plus a second zero row at the bottom
     const int tiles_1d = (a.n + TILE - 1) / TILE;
     const int tix = blockIdx.x % tiles_1d, tiy = blockIdx.x / tiles_1d;
     const int z = blockIdx.y, jg = blockIdx.z;
     const int x0 = tix * TILE, y0 = tiy * TILE;
-    const int u = threadIdx.x >> 3, sp = (threadIdx.x >> 2) & 1, jq = threadIdx.x & 3;
+    const int u = threadIdx.x >> 3, sp = (threadIdx.x & 7) / JQ, jq = threadIdx.x & (JQ - 1);
     const float4 zero = make_float4(0.f, 0.f, 0.f, 0.f);
     const float4 *F = reinterpret_cast<const float4 *>(f);
     const TileGeo *geo = a.geo + (int64_t)blockIdx.x * a.n0;
 
-    for (int t = threadIdx.x; t < (TILE + 3) * RSV * 4; t += FR_THREADS) tile[t] = zero;   // borders stay zero in both passes
+    for (int t = threadIdx.x; t < (TILE + 3) * RSV * JQ; t += FR_THREADS) tile[t] = zero;   // borders stay zero in both passes
     for (int pass = 0; pass < 2; ++pass) {   // pass 0: rays stepping over columns; pass 1: over rows, on the transposed tile
         __syncthreads();
-        for (int t = threadIdx.x; t < TILE * TILE * 4; t += FR_THREADS) {
-            const int jc = t & 3, lx = (t >> 2) & (TILE - 1), ly = t >> 7;
+        for (int t = threadIdx.x; t < TILE * TILE * JQ; t += FR_THREADS) {
+            const int jc = t & (JQ - 1), lx = (t / JQ) & (TILE - 1), ly = t / (JQ * TILE);
             const int gx = x0 + lx, gy = y0 + ly;
             const int row = pass ? lx : ly, col = pass ? ly : lx;
-            tile[((row + 1) * RSV + col + 1) * 4 + jc] =
-                (gx < a.n && gy < a.n) ? __ldg(F + (((int64_t)z * a.n + gy) * a.n + gx) * a.Q + jg * 4 + jc) : zero;
+            tile[((row + 1) * RSV + col + 1) * JQ + jc] =
+                (gx < a.n && gy < a.n) ? __ldg(F + (((int64_t)z * a.n + gy) * a.n + gx) * a.Q + jg * JQ + jc) : zero;
         }
         __syncthreads();
         for (int i = 0; i < a.n0; ++i) {
@@ -173,44 +189,48 @@ __global__ void __launch_bounds__(FR_THREADS, 3) k_forward_rays16(const float *_
             float4 acc = zero;
             // floor without the conversion pipe: tm = ys + 1.5 * 2^23 rounded DOWN holds floor(ys) in its low mantissa bits
             const float MAGIC = 12582912.0f;
-            const float4 *plane = tile + jq + 4;          // + 4: column k lives at tile column k+1
+            const float4 *plane = tile + jq + JQ;         // + JQ: column k lives at tile column k+1
             // per-ray chunk range: lanes of other rays in the warp are masked off, so no wavefront is spent outside the chord
-            for (int kc = klo & ~(2 * FR_UNROLL - 1); kc <= khi; kc += 2 * FR_UNROLL) {
+            for (int kc = klo & ~(CHUNK - 1); kc <= khi; kc += CHUNK) {
                 const float y0s = fmaf((float)(kc + sp), step, base);
-                const float4 *pc = plane + (kc + sp) * 4;
+                const float4 *pc = plane + (kc + sp) * JQ;
 #pragma unroll
-                for (int j = 0; j < FR_UNROLL; ++j) {
-                    const float ys = fmaf((float)(2 * j), step, y0s);       // crossing at step k = kc + sp + 2j
+                for (int j = 0; j < UNROLL; ++j) {
+                    const float ys = fmaf((float)(NPH * j), step, y0s);     // crossing at step k = kc + sp + NPH j
                     const float tm = __fadd_rd(ys, MAGIC);
                     const float w1 = ys - (tm - MAGIC), w0 = 1.0f - w1;     // w1 in [0,1)
                     // tile row of the first tap = floor(ys) + 1; anything outside [0, TILE] reads the two zero rows TILE+1, TILE+2
                     const unsigned row = min((unsigned)(__float_as_int(tm) - (0x4B400000 - 1)), (unsigned)(TILE + 1));
-                    const float4 *p0 = reinterpret_cast<const float4 *>(reinterpret_cast<const char *>(pc) + row * (RSV * 64)) + j * 8;
-                    const float4 v0 = p0[0], v1 = p0[RSV * 4];
+                    const float4 *p0 = reinterpret_cast<const float4 *>(reinterpret_cast<const char *>(pc) + row * (RSV * JQ * 16)) + j * (NPH * JQ);
+                    const float4 v0 = p0[0], v1 = p0[RSV * JQ];
                     fma4(acc, w0, v0);
                     fma4(acc, w1, v1);
                 }
             }
-            // sum the two step parities (lanes l and l^4 serve the same ray and chunk)
-            acc.x += __shfl_xor_sync(0xffffffffu, acc.x, 4);
-            acc.y += __shfl_xor_sync(0xffffffffu, acc.y, 4);
-            acc.z += __shfl_xor_sync(0xffffffffu, acc.z, 4);
-            acc.w += __shfl_xor_sync(0xffffffffu, acc.w, 4);
+            // sum the step phases (lanes differing in the phase bits serve the same ray and chunk)
+#pragma unroll
+            for (int o = JQ; o < 8; o <<= 1) {
+                acc.x += __shfl_xor_sync(0xffffffffu, acc.x, o);
+                acc.y += __shfl_xor_sync(0xffffffffu, acc.y, o);
+                acc.z += __shfl_xor_sync(0xffffffffu, acc.z, o);
+                acc.w += __shfl_xor_sync(0xffffffffu, acc.w, o);
+            }
             const int b = G.bstart + u;
             if (sp == 0 && touched && b >= 0 && b < a.nd) {
-                float4 *dst = P + (((int64_t)z * a.n0 + i) * a.Q + jg * 4 + jq) * a.gp + a.gpl + b;
+                float4 *dst = P + (((int64_t)z * a.n0 + i) * a.Q + jg * JQ + jq) * a.gp + a.gpl + b;
                 atomicAdd(dst, make_float4(acc.x * A.inv_a, acc.y * A.inv_a, acc.z * A.inv_a, acc.w * A.inv_a));
             }
         }
     }
 }
 
-static cudaError_t fwd_launch_rays16(cp4d_ctx *c, const float *f, float4 *P, const ProjArgs &a) {
+template <int JQ>
+static cudaError_t fwd_launch_rays(cp4d_ctx *c, const float *f, float4 *P, const ProjArgs &a) {
     const Dims &d = c->d;
-    const size_t sh = (size_t)(TILE + 3) * RSV * 4 * sizeof(float4);
-    cudaError_t e = cudaFuncSetAttribute(k_forward_rays16, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sh);
+    const size_t sh = FwRays<JQ>::SMEM;
+    cudaError_t e = cudaFuncSetAttribute(k_forward_rays<JQ>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sh);
     if (e != cudaSuccess) return e;
-    k_forward_rays16<<<dim3(d.tiles, d.nz, d.Q / 4), FR_THREADS, sh, c->stream>>>(f, P, a);
+    k_forward_rays<JQ><<<dim3(d.tiles, d.nz, d.Q / JQ), FR_THREADS, sh, c->stream>>>(f, P, a);
     return cudaGetLastError();
 }
 
@@ -234,8 +254,8 @@ cudaError_t launch_forward_partial(cp4d_ctx *c, const float *f, float4 *P) {
     if (e != cudaSuccess) return e;
     c->launches += 2;
     switch (pick_jq(d.Q)) {
-    case 4: return fwd_launch_rays16(c, f, P, a);
-    case 2: return fwd_launch<2>(c, f, P, a);
+    case 4: return fwd_launch_rays<4>(c, f, P, a);
+    case 2: return fwd_launch_rays<2>(c, f, P, a);
     default: return fwd_launch<1>(c, f, P, a);
     }
 }

@@ -57,13 +57,15 @@ def test_host_validation(L, bad):
 
 
 def test_frame_mode_workspace(L):
-    """Frame mode (n_frames > 0): primal arrays have n_frames planes, plus two coefficient stacks and the Psi table."""
+    """Frame mode (n_frames > 0).  N_t <= M collapses to a coefficient-mode problem with N_t planes (the projector pair carries
+    the frames); N_t > M keeps M-plane coefficient stacks beside the N_t-plane state plus the Psi table."""
     from paper_1809_09725_b200 import binding
-    n, nz, nd, na, npi, m, nt = 64, 4, 64, 96, 2, 16, 8
-    a = binding.workspace_bytes(n, nz, nd, na, npi, m)
-    b = binding.workspace_bytes(n, nz, nd, na, npi, m, n_frames=nt)
+    n, nz, nd, na, npi = 64, 4, 64, 96, 2
+    assert binding.workspace_bytes(n, nz, nd, na, npi, 16, n_frames=8) == binding.workspace_bytes(n, nz, nd, na, npi, 8)
+    a = binding.workspace_bytes(n, nz, nd, na, npi, 4)
+    b = binding.workspace_bytes(n, nz, nd, na, npi, 4, n_frames=8)
     vox = nz * n * n
-    assert b - a == pytest.approx((7 * (nt - m) + 2 * m) * vox * 4, abs=1 << 16)
+    assert b - a == pytest.approx((7 * (8 - 4) + 2 * 4) * vox * 4, abs=1 << 16)
 
 
 def test_create_needs_workspace_and_device(L):
