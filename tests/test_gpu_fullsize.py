@@ -169,3 +169,38 @@ def test_teacher_forced_cp_step(torch_cuda, fast_oracle, cfg):
             assert rel(ft_got, f_ref + 1.0 * (f_ref - f_old)) <= TOL_OP
     assert 0.2 < n_clamped / n_total < 0.8, (n_clamped, n_total)     # both branches of max(1, |q|/lambda1) exercised
     ctx.close()
+
+
+@pytest.mark.parametrize("cfg,nt", [(3, 8), (4, 8)])
+def test_sampled_frame_mode(torch_cuda, fast_oracle, cfg, nt):
+    """Frame mode at full size: N_t = 8 frames, M = 16 basis functions -- the collapsed route
+    (projectors carry the frames) against the oracle's K1 o A at sampled rays / voxels."""
+    torch = torch_cuda
+    from paper_1809_09725_b200 import binding
+    c = synth.CONFIGS[cfg]
+    phi = synth.basis_table(c.basis, c.m, c.n_angles)
+    psi = phi[:, ::c.n_angles // nt]                                   # Psi[j,q] = phi_j(t_q), Eq. 11
+    ctx = binding.Context.from_config(c, phi=phi, n_frames=nt)
+    assert ctx.primal_shape == (c.nz, c.n, c.n, nt)
+    gen = torch.Generator(device="cuda").manual_seed(3000 + cfg)
+    zs = _slices(c)
+    P3 = _sub_problem(fast_oracle, c, phi, len(zs))
+    r = synth.rng(cfg, 9)
+    u = torch.randn(ctx.primal_shape, generator=gen, device="cuda", dtype=torch.float32)
+    Ku = ctx.forward(u)
+    zi = r.integers(0, len(zs), NS)
+    kk, bb = r.integers(0, c.n_angles, NS), r.integers(0, c.nd, NS)
+    f3 = np.stack([u[z].cpu().numpy() for z in zs]).astype(np.float64) @ psi.T          # analysis, L231-L237
+    ref = P3.forward_rays(f3, np.stack([zi, kk, bb], 1).astype(np.int32))
+    zsel = torch.as_tensor(np.asarray(zs)[zi], device="cuda")
+    got = Ku[zsel, torch.as_tensor(kk, device="cuda"), torch.as_tensor(bb, device="cuda")].cpu().numpy()
+    assert rel(got, ref) <= TOL_OP
+    del f3
+    g = torch.randn(ctx.sino_shape, generator=gen, device="cuda", dtype=torch.float32)
+    Ktg = ctx.adjoint(g, out=u)
+    yy, xx = r.integers(0, c.n, NS), r.integers(0, c.n, NS)
+    g3 = np.stack([g[z].cpu().numpy() for z in zs]).astype(np.float64)
+    ref = P3.adjoint_voxels(g3, np.stack([zi, yy, xx], 1).astype(np.int32)) @ psi       # A^T after K1^T
+    got = Ktg[zsel, torch.as_tensor(yy, device="cuda"), torch.as_tensor(xx, device="cuda")].cpu().numpy()
+    assert rel(got, ref) <= TOL_OP
+    ctx.close()
