@@ -49,7 +49,7 @@ int validate(const cp4d_params *p, Dims *d) {
 }
 
 struct Carve {
-    uint64_t f, ft, bp, h2, h1, g, tmp_s, scratch, phi, ang, geo, red, cf, cb, psi, total;
+    uint64_t f, ft, bp, h2, h1, g, tmp_s, scratch, phi, ang, geo, red, cf, cb, psi, fwang, fworder, total;
 };
 Carve carve(const Dims &d) {
     Carve c;
@@ -59,6 +59,7 @@ Carve carve(const Dims &d) {
     c.h1 = take(d.S * 4); c.g = take(d.S * 4); c.tmp_s = take(d.S * 4); c.scratch = take(d.scratch4 * 16);
     c.phi = take((uint64_t)d.m * d.na * 4); c.ang = take((uint64_t)d.n0 * sizeof(AngleTab));
     c.geo = take((uint64_t)d.tiles * d.n0 * sizeof(TileGeo)); c.red = take(64);
+    c.fwang = take((uint64_t)d.n0 * sizeof(FwAngle)); c.fworder = take((uint64_t)d.n0 * 4);
     c.cf = c.cb = c.psi = 0;
     if (d.nf) { c.cf = take(d.Vc * 4); c.cb = take(d.Vc * 4); c.psi = take((uint64_t)d.mb * d.nf * 4); }
     c.total = o;
@@ -155,6 +156,7 @@ int cp4d_create(const cp4d_params *p, cp4d_ctx **out) {
     ctx->f = (float *)(w + cv.f); ctx->ft = (float *)(w + cv.ft); ctx->bp = (float *)(w + cv.bp);
     ctx->h2 = (float *)(w + cv.h2); ctx->h1 = (float *)(w + cv.h1); ctx->g = (float *)(w + cv.g);
     ctx->tmp_s = (float *)(w + cv.tmp_s);
+    ctx->fwang = (FwAngle *)(w + cv.fwang); ctx->fworder = (int32_t *)(w + cv.fworder);
     ctx->cf = d.nf ? (float *)(w + cv.cf) : nullptr; ctx->cb = d.nf ? (float *)(w + cv.cb) : nullptr;
     ctx->psi = d.nf ? (float *)(w + cv.psi) : nullptr;
     ctx->scratch = (float4 *)(w + cv.scratch); ctx->phi = (float *)(w + cv.phi);
@@ -179,6 +181,14 @@ int cp4d_create(const cp4d_params *p, cp4d_ctx **out) {
         if (ang[i].pat < 0) { delete ctx; return CP4D_EINVAL; }
         ang[i].pat_fl = bp_pattern_fl(ang[i].pat);
     }
+    std::vector<FwAngle> fwang(d.n0);
+    std::vector<int32_t> fworder;
+    for (int pass = 0; pass < 2; ++pass) {
+        for (int i = 0; i < d.n0; ++i)
+            if ((ang[i].col_step != 0) == (pass == 0)) fworder.push_back(i);
+        if (pass == 0) ctx->n_colstep = (int)fworder.size();
+    }
+    for (int i = 0; i < d.n0; ++i) fwang[i] = FwAngle{ang[i].fw_inv, ang[i].fw_step, ang[i].fw_istep, ang[i].inv_a};
     std::vector<TileGeo> geo((size_t)d.tiles * d.n0);
     const double cen = 0.5 * (d.n - 1), cd = 0.5 * (d.nd - 1);
     for (int t = 0; t < d.tiles; ++t) {
@@ -213,6 +223,8 @@ int cp4d_create(const cp4d_params *p, cp4d_ctx **out) {
     if ((d.nf && (e = cudaMemcpyAsync(ctx->psi, psi.data(), psi.size() * 4, cudaMemcpyHostToDevice, ctx->stream)) != cudaSuccess) ||
         (e = cudaMemcpyAsync(ctx->phi, phi_eff.data(), (size_t)d.m * d.na * 4, cudaMemcpyHostToDevice, ctx->stream)) != cudaSuccess ||
         (e = cudaMemcpyAsync(ctx->ang, ang.data(), ang.size() * sizeof(AngleTab), cudaMemcpyHostToDevice, ctx->stream)) != cudaSuccess ||
+        (e = cudaMemcpyAsync(ctx->fwang, fwang.data(), fwang.size() * sizeof(FwAngle), cudaMemcpyHostToDevice, ctx->stream)) != cudaSuccess ||
+        (e = cudaMemcpyAsync(ctx->fworder, fworder.data(), fworder.size() * 4, cudaMemcpyHostToDevice, ctx->stream)) != cudaSuccess ||
         (e = cudaMemcpyAsync(ctx->geo, geo.data(), geo.size() * sizeof(TileGeo), cudaMemcpyHostToDevice, ctx->stream)) != cudaSuccess ||
         (e = cudaMemsetAsync(ctx->scratch, 0, (size_t)d.scratch4 * 16, ctx->stream)) != cudaSuccess ||
         (e = cudaStreamSynchronize(ctx->stream)) != cudaSuccess) {

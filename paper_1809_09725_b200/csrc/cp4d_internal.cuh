@@ -33,6 +33,11 @@ struct AngleTab {
     float fw_inv, fw_step, fw_istep;  // 1/ss, -cc/ss, 1/fw_step (0 when |fw_step| < 1e-6), rounded from fp64
 };
 
+// forward projector parameters of one base angle, one 16-byte load (see AngleTab::fw_*)
+struct FwAngle {
+    float inv, step, istep, inv_a;
+};
+
 struct Dims {
     int n, nz, nd, na, npi, n0, m, Q;  // Q = m/4 float4 chunks per voxel of a coefficient stack
     int nf, mp, Qp;                    // frame mode: nf frames (0 = coefficient mode); mp = nf ? nf : m is the
@@ -63,6 +68,9 @@ struct cp4d_ctx {
                                // the pads stay zero, so every tile window of the backprojector is readable memory
     float *phi;                // [j][k]
     cp4d::AngleTab *ang;       // [n0]
+    cp4d::FwAngle *fwang;      // [n0]
+    int32_t *fworder;          // [n0]: base angles whose rays step over columns first, then the others
+    int n_colstep;             // how many of the former
     cp4d::TileGeo *geo;        // [tile][n0]
     double *red;               // 8 doubles for reductions
     uint64_t launches;

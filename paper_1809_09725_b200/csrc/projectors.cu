@@ -29,6 +29,9 @@ struct ProjArgs {
     int n, nz, nd, n0, Q, gp, gpl;
     const AngleTab *ang;
     const TileGeo *geo;
+    const FwAngle *fwang;      // k_forward_rays: packed per-angle parameters and the angle order by stepping axis
+    const int32_t *fworder;
+    int n_colstep;
 };
 
 // ---------------------------------------------------------------------------------------------------
@@ -170,16 +173,17 @@ __global__ void __launch_bounds__(FR_THREADS, 3) k_forward_rays(const float *__r
                 (gx < a.n && gy < a.n) ? __ldg(F + (((int64_t)z * a.n + gy) * a.n + gx) * a.Q + jg * JQ + jc) : zero;
         }
         __syncthreads();
-        for (int i = 0; i < a.n0; ++i) {
-            const AngleTab A = a.ang[i];
-            if ((A.col_step != 0) != (pass == 0)) continue;
+        const int ii0 = pass ? a.n_colstep : 0, ii1 = pass ? a.n0 : a.n_colstep;
+        for (int ii = ii0; ii < ii1; ++ii) {
+            const int i = a.fworder[ii];
+            const FwAngle A = a.fwang[i];
             const TileGeo G = geo[i];
             // pass 0: the ray crosses column k at row (du - k c)/s; pass 1: it crosses row k at column (du - k s)/c
-            const float step = A.fw_step, base = ((float)u - G.delta) * A.fw_inv;
+            const float step = A.step, base = ((float)u - G.delta) * A.inv;
             // this ray's steps k with -1 <= base + k step < TILE (one extra on each side; the body is exact on its own)
             int klo = 0, khi = TILE - 1;
-            if (A.fw_istep != 0.0f) {
-                const float ta = (-1.0f - base) * A.fw_istep, tb = ((float)TILE - base) * A.fw_istep;
+            if (A.istep != 0.0f) {
+                const float ta = (-1.0f - base) * A.istep, tb = ((float)TILE - base) * A.istep;
                 klo = max(0, (int)floorf(fminf(ta, tb)));
                 khi = min(TILE - 1, (int)ceilf(fmaxf(ta, tb)));
             } else if (!(base >= -1.0f && base < (float)TILE)) {
@@ -249,7 +253,7 @@ static cudaError_t fwd_launch(cp4d_ctx *c, const float *f, float4 *P, const Proj
 cudaError_t launch_forward_partial(cp4d_ctx *c, const float *f, float4 *P) {
     ProfScope ps(c, CP4D_K_FORWARD);
     const Dims &d = c->d;
-    ProjArgs a{d.n, d.nz, d.nd, d.n0, d.Q, d.gp, d.gpl, c->ang, c->geo};
+    ProjArgs a{d.n, d.nz, d.nd, d.n0, d.Q, d.gp, d.gpl, c->ang, c->geo, c->fwang, c->fworder, c->n_colstep};
     cudaError_t e = cudaMemsetAsync(P, 0, (size_t)d.scratch4 * sizeof(float4), c->stream);
     if (e != cudaSuccess) return e;
     c->launches += 2;
