@@ -383,7 +383,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--config", type=int, default=3, help="BASELINE.json config 1..5 (SURVEY.md 8 numbering)")
     ap.add_argument("--impl", default="cp4d", choices=["cp4d", "reference"])
-    ap.add_argument("--power-iters", type=int, default=10)
+    ap.add_argument("--power-iters", type=int, default=30, help="power-iteration steps for ||K|| (DESIGN.md R8: 30)")
     ap.add_argument("--frames", type=int, default=0, help="N_t > 0: the paper's frame discretisation (cp4d_params.n_frames), e.g. 8")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
