@@ -75,8 +75,9 @@ typedef struct {
                                  from phi_host's column q*n_angles/N_t; the 4th difference of K2 runs over frames      */
 } cp4d_params;
 
-/* Bytes of device workspace a context for these sizes needs (state f, f~, K1^T h1, h2[4], h1, g,
- * projector scratch, tables).  Host only; ignores workspace_dev/stream/phi_host. */
+/* Bytes of device workspace a context for these sizes needs (state f, f~, K1^T h1, h2[4], h1, g, one sinogram-sized
+ * temporary, zero-padded projector scratch, tables; in frame mode with N_t > m two coefficient stacks as well).
+ * Host only; ignores workspace_dev/stream/phi_host.  Errors: CP4D_EINVAL (see cp4d_params). */
 int cp4d_workspace_bytes(const cp4d_params *p, uint64_t *bytes_out);
 
 /* Validate, compute the fp64 angle/tile tables on the host, copy them and phi into the workspace,
@@ -85,6 +86,9 @@ int cp4d_create(const cp4d_params *p, cp4d_ctx **ctx_out);
 int cp4d_destroy(cp4d_ctx *ctx);
 
 /* ---- stateless operators on caller-owned DEVICE buffers -------------------------------------- */
+/* Every function below returns CP4D_EINVAL for a null context, a null or misaligned (16 B) pointer or overlapping in/out
+ * buffers, and CP4D_ECUDA (text in cp4d_last_error) if a launch fails.  "V" is the primal size: in frame mode f holds
+ * the n_frames frames and K1 includes the analysis f_j = sum_q phi_j(t_q) f(t_q). */
 /* g = K1 f  (Eq. 9; pi-folding L198-L202: ray sums over the n_theta0 base angles with all m
  * coefficients accumulated per ray, then n_half_rot m-wide dot products with Phi).  f: V, g: S. */
 int cp4d_forward(cp4d_ctx *ctx, const float *f_dev, float *g_dev);
