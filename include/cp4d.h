@@ -138,6 +138,15 @@ int cp4d_state_ptrs(cp4d_ctx *ctx, float **f, float **ft, float **h1, float **h2
  * Out pointers are HOST and may be null.  Uses the K1^T h1 buffer and the projector scratch; state is untouched. */
 int cp4d_objective(cp4d_ctx *ctx, double *primal, double *cond_dual, double *kkt_resid);
 
+/* ---- static filtered backprojection per half-rotation (L243, L257-L259: the paper's comparison method and initial guess) */
+/* out[z][iy][ix][q], q < Q4 = 4*ceil(n_half_rot/4) (planes q >= n_half_rot are zero):
+ *     out_q = (pi / n_theta0) * sum_{i < n_theta0} R*_{theta_i} ( h_SL * g[q n_theta0 + i] ),
+ * h_SL[n] = -2 / (pi^2 (4 n^2 - 1)) the Shepp-Logan filter at unit bin spacing, R* the same (Joseph) backprojector as
+ * cp4d_adjoint with odd half-rotations bin-flipped.  In frame mode with n_frames == n_half_rot == Q4, out is a valid f0 for
+ * cp4d_reset.  g: S, out: nz*n*n*Q4 floats, DEVICE.  Needs Q4 <= m (else CP4D_EUNSUPPORTED).  Uses the sinogram temporary and
+ * the projector scratch. */
+int cp4d_fbp(cp4d_ctx *ctx, const float *g_dev, float *out_dev);
+
 /* ---- end-to-end call with HOST buffers (pinned or pageable) ---------------------------------- */
 /* H2D copy of g_host (S), reset to zeros, n_iters iterations with the current steps, D2H copy of f
  * into f_host (V).  Syncs. */

@@ -240,3 +240,30 @@ class FrameProblem:
             state["ft"] = f_new + theta * (f_new - state["f"])                                                   # step 6
             state["f"] = f_new
         return ncl
+
+
+def shepp_logan_kernel(nd):
+    """h[n] = -2 / (pi^2 (4 n^2 - 1)), n = -(nd-1) .. nd-1: the Shepp-Logan filter sampled at unit bin spacing."""
+    n = np.arange(-(nd - 1), nd, dtype=np.float64)
+    return -2.0 / (np.pi ** 2 * (4.0 * n * n - 1.0))
+
+
+def fbp_half_rotations(n, nz, nd, n_angles, n_half_rot, g):
+    """Static filtered backprojection of every half-rotation, TEST INFRASTRUCTURE.
+
+    out[z,iy,ix,q] = (pi/n0) sum_{i<n0} R*_{theta_i}(h_SL * g[z, q n0 + i, .]); R* is the Joseph backprojector of `Problem`
+    (R3), reached through the box basis phi_q = 1 on half-rotation q, for which K1^T stacks the N_pi static
+    backprojections.  Plain definition: direct convolution per row, then the pinned adjoint.
+    """
+    n0 = n_angles // n_half_rot
+    g = np.asarray(g, dtype=np.float64)
+    h = shepp_logan_kernel(nd)
+    gf = np.empty_like(g)
+    for z in range(nz):
+        for k in range(n_angles):
+            gf[z, k] = np.convolve(g[z, k], h)[nd - 1:2 * nd - 1]        # sum_b' h[b - b'] g[b']
+    box = np.zeros((n_half_rot, n_angles))
+    for q in range(n_half_rot):
+        box[q, q * n0:(q + 1) * n0] = 1.0
+    P = Problem(n, nz, nd, n_angles, n_half_rot, n_half_rot, box)
+    return (np.pi / n0) * P.adjoint(gf)

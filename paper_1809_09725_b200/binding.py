@@ -61,7 +61,7 @@ def lib():
             "cp4d_iterate": [vp, i32], "cp4d_get_f": [vp, vp],
             "cp4d_state_ptrs": [vp] + [C.POINTER(vp)] * 5,
             "cp4d_solve_host": [vp, vp, i32, vp], "cp4d_sync": [vp],
-            "cp4d_objective": [vp] + [C.POINTER(C.c_double)] * 3,
+            "cp4d_objective": [vp] + [C.POINTER(C.c_double)] * 3, "cp4d_fbp": [vp, vp, vp],
             "cp4d_launch_count": [vp, C.POINTER(u64)],
             "cp4d_profile_begin": [vp], "cp4d_profile_end": [vp, C.POINTER(Profile)],
         }
@@ -234,6 +234,14 @@ class Context:
         fp = f_host.data_ptr() if hasattr(f_host, "data_ptr") else f_host.ctypes.data
         self._ck(lib().cp4d_solve_host(self._h, gp, n_iters, fp))
         return f_host
+
+    def fbp(self, g, out=None):
+        """Static Shepp-Logan FBP of every half-rotation: (nz, n, n, 4*ceil(n_half_rot/4))."""
+        q4 = (self.n_half_rot + 3) // 4 * 4
+        if out is None:
+            out = self.torch.empty((self.nz, self.n, self.n, q4), dtype=self.torch.float32, device=self.device)
+        self._ck(lib().cp4d_fbp(self._h, self._t(g, self.S), self._t(out, self.nz * self.n * self.n * q4)))
+        return out
 
     def objective(self):
         """(primal value, conditional dual value, dual residual |K1^T h1 - div h2|) of the current state; syncs."""

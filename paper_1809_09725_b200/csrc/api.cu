@@ -442,6 +442,23 @@ int cp4d_objective(cp4d_ctx *ctx, double *primal, double *cond_dual, double *kkt
     return CP4D_OK;
 }
 
+int cp4d_fbp(cp4d_ctx *ctx, const float *g, float *out) {
+    if (!ctx) return CP4D_EINVAL;
+    const Dims &d = ctx->d;
+    const int Qf = (d.npi + 3) / 4;
+    const uint64_t out_bytes = (uint64_t)d.nz * d.n * d.n * Qf * 16;
+    if (bad_ptr(g) || bad_ptr(out) || overlap(g, d.S * 4, out, out_bytes)) return fail(ctx, CP4D_EINVAL, "fbp: bad pointers");
+    if (Qf > d.Q) return fail(ctx, CP4D_EUNSUPPORTED, "fbp: needs ceil(n_half_rot/4)*4 <= m (the projector scratch is sized for m)");
+    CK(launch_filter_sl(ctx, g, ctx->tmp_s), "filter");
+    // the scratch rows keep their zero pads: only bins [0, nd) of the first Qf chunk planes... every plane stride is gp, and
+    // with Qf != Q the row addressing differs from the fold's, so clear the scratch once and restore the invariant afterwards
+    CK(cudaMemsetAsync(ctx->scratch, 0, (size_t)d.scratch4 * 16, ctx->stream), "fbp clear");
+    CK(launch_fold_halfrot(ctx, ctx->tmp_s, ctx->scratch, Qf, (float)(3.14159265358979323846 / d.n0)), "fold_halfrot");
+    CK(launch_backproject(ctx, ctx->scratch, out, Qf), "fbp backproject");
+    CK(cudaMemsetAsync(ctx->scratch, 0, (size_t)d.scratch4 * 16, ctx->stream), "fbp clear");
+    return CP4D_OK;
+}
+
 int cp4d_sync(cp4d_ctx *ctx) {
     if (!ctx) return CP4D_EINVAL;
     CK(cudaStreamSynchronize(ctx->stream), "sync");

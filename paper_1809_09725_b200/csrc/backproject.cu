@@ -238,7 +238,7 @@ __global__ void __launch_bounds__(BP_THREADS, 4) k_backproject(const float4 *__r
 template <int JQ>
 static cudaError_t bp_launch(cp4d_ctx *c, const float4 *gt, float *f_out, const BpArgs &a) {
     const Dims &d = c->d;
-    k_backproject<JQ><<<dim3(d.tiles, d.nz, d.Q / JQ), BP_THREADS, 0, c->stream>>>(gt, f_out, a);
+    k_backproject<JQ><<<dim3(d.tiles, d.nz, a.Q / JQ), BP_THREADS, 0, c->stream>>>(gt, f_out, a);
     return cudaGetLastError();
 }
 
@@ -263,12 +263,14 @@ uint32_t bp_pattern_fl(int pat) {
     return r;
 }
 
-cudaError_t launch_backproject(cp4d_ctx *c, const float4 *gt, float *f_out) {
+// Q_override > 0: backproject Q_override float4 chunks per bin / voxel instead of the context's Q (cp4d_fbp)
+cudaError_t launch_backproject(cp4d_ctx *c, const float4 *gt, float *f_out, int Q_override) {
     ProfScope ps(c, CP4D_K_BACKPROJECT);
     const Dims &d = c->d;
-    BpArgs a{d.n, d.nz, d.nd, d.n0, d.Q, d.gp, d.gpl, c->ang, c->geo};
+    const int Q = Q_override > 0 ? Q_override : d.Q;
+    BpArgs a{d.n, d.nz, d.nd, d.n0, Q, d.gp, d.gpl, c->ang, c->geo};
     c->launches++;
-    if (d.Q % 2 == 0) return bp_launch<2>(c, gt, f_out, a);
+    if (Q % 2 == 0) return bp_launch<2>(c, gt, f_out, a);
     return bp_launch<1>(c, gt, f_out, a);
 }
 

@@ -116,7 +116,10 @@ cudaError_t launch_fold(cp4d_ctx *c, const float *g, float4 *gt);
 // synth: out = K1 f from partial sums P.  mode 0: g_out = v ; mode 1: h1 = (h1 + sigma (v - g))/(1+sigma)
 cudaError_t launch_synth(cp4d_ctx *c, const float4 *P, int mode, float sigma, const float *g, float *out);
 cudaError_t launch_forward_partial(cp4d_ctx *c, const float *f, float4 *P);
-cudaError_t launch_backproject(cp4d_ctx *c, const float4 *gt, float *f_out);
+cudaError_t launch_backproject(cp4d_ctx *c, const float4 *gt, float *f_out, int Q_override = 0);
+// cp4d_fbp: Shepp-Logan filter along the bins; per-half-rotation rows gathered into the projector scratch (box basis)
+cudaError_t launch_filter_sl(cp4d_ctx *c, const float *g, float *gf);
+cudaError_t launch_fold_halfrot(cp4d_ctx *c, const float *gf, float4 *gt, int Qf, float scale);
 int bp_pattern(float c, float s);  // host: pattern index in [0, BP_NPAT) or -1
 uint32_t bp_pattern_fl(int pat);   // host: the pattern's FL_v packed 4 bits each
 // out[v][a] = sum_b T(a,b) in[v][b] per voxel v, T(a,b) = psi[a*sa + b*sb]  (frame <-> coefficient contraction, L231-L237)

@@ -250,6 +250,57 @@ cudaError_t launch_mix(cp4d_ctx *c, const float *in, float *out, int na_out, int
     return cudaGetLastError();
 }
 
+// ---------------------------------------------------------------------------------------------------
+// static FBP per half-rotation
+// ---------------------------------------------------------------------------------------------------
+// Shepp-Logan filter, unit bin spacing, direct convolution:  gf[b] = sum_b' h[b-b'] g[b'],  h[n] = -2 / (pi^2 (4 n^2 - 1)).
+// One CTA per sinogram row (z, k); the row sits in shared memory.
+__global__ void __launch_bounds__(256) k_filter_sl(const float *__restrict__ g, float *__restrict__ gf, int nd) {
+    extern __shared__ float row[];
+    const float *src = g + (int64_t)blockIdx.x * nd;
+    for (int b = threadIdx.x; b < nd; b += blockDim.x) row[b] = __ldg(src + b);
+    __syncthreads();
+    const float k0 = -0.20264236728467555f;   // -2 / pi^2
+    for (int b = threadIdx.x; b < nd; b += blockDim.x) {
+        float acc = 0.f;
+        for (int bp = 0; bp < nd; ++bp) {
+            const float n = (float)(b - bp);
+            acc = fmaf(__fdividef(k0, fmaf(4.0f * n, n, -1.0f)), row[bp], acc);
+        }
+        gf[(int64_t)blockIdx.x * nd + b] = acc;
+    }
+}
+cudaError_t launch_filter_sl(cp4d_ctx *c, const float *g, float *gf) {
+    ProfScope ps(c, CP4D_K_MISC);
+    const Dims &d = c->d;
+    k_filter_sl<<<(unsigned)(d.nz * d.na), 256, (size_t)d.nd * sizeof(float), c->stream>>>(g, gf, d.nd);
+    c->launches++;
+    return cudaGetLastError();
+}
+// gt[z][i][qc][gpl + b] = scale * (gf[z][q n0 + i][flip_q b])_{q = 4 qc .. 4 qc + 3}: the fold with the box basis
+// phi_q = 1 on half-rotation q, whose backprojection is the static reconstruction of every half-rotation at once
+__global__ void __launch_bounds__(128) k_fold_halfrot(const float *__restrict__ gf, float4 *__restrict__ gt, int nd, int na, int npi,
+                                                     int n0, int gp, int gpl, int Qf, float scale) {
+    const int z = blockIdx.x / n0, i = blockIdx.x % n0;
+    for (int t = threadIdx.x; t < Qf * nd; t += blockDim.x) {
+        const int qc = t / nd, b = t % nd;
+        float v[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            const int q = 4 * qc + u;
+            v[u] = q < npi ? scale * __ldg(gf + ((int64_t)z * na + q * n0 + i) * nd + ((q & 1) ? nd - 1 - b : b)) : 0.f;
+        }
+        gt[(((int64_t)z * n0 + i) * Qf + qc) * gp + gpl + b] = make_float4(v[0], v[1], v[2], v[3]);
+    }
+}
+cudaError_t launch_fold_halfrot(cp4d_ctx *c, const float *gf, float4 *gt, int Qf, float scale) {
+    ProfScope ps(c, CP4D_K_FOLD);
+    const Dims &d = c->d;
+    k_fold_halfrot<<<d.nz * d.n0, 128, 0, c->stream>>>(gf, gt, d.nd, d.na, d.npi, d.n0, d.gp, d.gpl, Qf, scale);
+    c->launches++;
+    return cudaGetLastError();
+}
+
 // reductions for cp4d_objective: *slot is zeroed first, then accumulated by the kernel
 cudaError_t launch_tv_sum(cp4d_ctx *c, const float *f, double *slot) {
     ProfScope ps(c, CP4D_K_REDUCE);

@@ -250,3 +250,37 @@ def test_objective_monitor(torch_cuda, fast_oracle, case):
     s2 = {k: v.cpu().numpy().astype(np.float64) for k, v in ctx.state().items()}
     assert all(np.array_equal(s[k], s2[k]) for k in s)
     ctx.close()
+
+
+@pytest.mark.parametrize("case", ["ragged", "ragged_m16", "cfg2"])
+def test_fbp_half_rotations(torch_cuda, fast_oracle, case):
+    """cp4d_fbp against the oracle's plain definition; then as the initial guess of a frame-mode run."""
+    c, P, ctx = make(case, fast_oracle)
+    g = synth.rng(c.cfg, 11).standard_normal(P.sino_shape).astype(np.float32)
+    ref = fast_oracle.fbp_half_rotations(c.n, c.nz, c.nd, c.n_angles, c.n_half_rot, g.astype(np.float64))
+    out = ctx.fbp(dev(torch_cuda, g)).cpu().numpy()
+    q4 = (c.n_half_rot + 3) // 4 * 4
+    assert out.shape == (c.nz, c.n, c.n, q4)
+    assert rel(out[..., :c.n_half_rot], ref) <= TOL_OP
+    assert not out[..., c.n_half_rot:].any()
+    # the call leaves the projector scratch usable: the adjoint still matches
+    Ktg = ctx.adjoint(dev(torch_cuda, g)).cpu().numpy()
+    assert rel(Ktg, P.adjoint(g.astype(np.float64), folded=True)) <= TOL_OP
+    ctx.close()
+
+
+def test_fbp_as_initial_guess_in_frame_mode(torch_cuda, fast_oracle):
+    from paper_1809_09725_b200 import binding
+    c = synth.CONFIGS[1].scaled(cfg=25, n=40, nd=44, nz=2, n_angles=64, n_half_rot=4, m=4, lambda1=7e-4)
+    phi = synth.basis_table(c.basis, c.m, c.n_angles)
+    F = fast_oracle.FrameProblem(c.n, c.nz, c.nd, c.n_angles, c.n_half_rot, c.m, phi, 4, lambda1=c.lambda1, lambda2=c.lambda2)
+    ctx = binding.Context.from_config(c, phi=phi, n_frames=4)          # N_t = N_pi: one frame per half-rotation
+    g = synth.rng(c.cfg, 1).standard_normal(F.sino_shape).astype(np.float32)
+    f0 = fast_oracle.fbp_half_rotations(c.n, c.nz, c.nd, c.n_angles, c.n_half_rot, g.astype(np.float64))
+    st = F.zero_state()
+    st["f"][:] = f0; st["ft"][:] = f0
+    F.cp(g.astype(np.float64), st, 0.004, 0.004, 6, folded=True)
+    f0_gpu = ctx.fbp(dev(torch_cuda, g))
+    ctx.set_data(dev(torch_cuda, g)); ctx.set_steps(0.004, 0.004); ctx.reset(f0_gpu); ctx.iterate(6); ctx.sync()
+    assert rel(ctx.get_f().cpu().numpy(), st["f"]) <= TOL_CP
+    ctx.close()

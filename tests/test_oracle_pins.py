@@ -393,3 +393,35 @@ def test_p9_frame_cp_step_matches_dense_algebra(oracle):
     np.testing.assert_allclose(st["h2"].reshape(4, -1), h2, atol=1e-12)
     np.testing.assert_allclose(st["f"].ravel(), f, atol=1e-12)
     np.testing.assert_allclose(st["ft"].ravel(), ft, atol=1e-12)
+
+
+# ---------------------------------------------------------------- P10: static FBP per half-rotation (L243, L257-L259)
+def test_p10_shepp_logan_kernel_properties(oracle):
+    h = oracle.shepp_logan_kernel(4097)
+    assert h[4096] == pytest.approx(2.0 / np.pi ** 2)                   # h[0]
+    assert np.all(np.delete(h, 4096) < 0)                                # negative side lobes
+    assert abs(h.sum()) < 1e-4                                           # sum over Z of -2/(pi^2 (4n^2-1)) = 0: no DC gain
+    # its transfer function is the band-limited ramp |sin(w/2)| / pi  (= |xi| for xi = w / 2 pi -> 0)
+    n = np.arange(-4096, 4097)
+    for w in (0.05, 0.5, 1.0, 2.0, 3.0):
+        assert np.sum(h * np.cos(w * n)) == pytest.approx(abs(np.sin(w / 2.0)) / np.pi, rel=1e-3, abs=1e-5)
+
+
+def test_p10_fbp_reconstructs_a_disk(oracle):
+    """Exact Radon data of a centred disk (closed form 2 sqrt(r^2 - s^2)), two half-rotations: every half-rotation's FBP is the
+    disk: ~1 inside, ~0 outside (Joseph backprojector + unit-spacing filter: a few per cent)."""
+    n = nd = 64
+    na, npi, r = 180, 2, 18.0
+    s = np.arange(nd) - (nd - 1) / 2.0
+    row = 2.0 * np.sqrt(np.maximum(0.0, r * r - s * s))
+    g = np.broadcast_to(row, (1, na, nd)).copy()
+    rec = oracle.fbp_half_rotations(n, 1, nd, na, npi, g)
+    assert rec.shape == (1, n, n, npi)
+    x = np.arange(n) - (n - 1) / 2.0
+    rho = np.hypot(*np.meshgrid(x, x))
+    for q in range(npi):
+        img = rec[0, :, :, q]
+        assert abs(img[rho < r - 3].mean() - 1.0) < 0.02
+        assert np.abs(img[rho < r - 3] - 1.0).max() < 0.08
+        assert np.abs(img[(rho > r + 3) & (rho < 30)]).max() < 0.08
+    np.testing.assert_allclose(rec[..., 0], rec[..., 1], atol=1e-9)     # symmetric data: the bin flip changes nothing
