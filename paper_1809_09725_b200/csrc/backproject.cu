@@ -9,7 +9,7 @@
 // Static register indexing.  With u = bin coordinate of a voxel, the patch's smallest coordinate is umin = K + phi
 // (K integer, 0 <= phi < 1, both per thread) and voxel v sits at umin + delta_v where delta_v = e*|c| + dy*s is the
 // same for every thread at this angle.  Choose an integer FL_v with 0 <= delta_v - FL_v <= 1 (the host picks one of 9
-// possible 8-tuples, the "pattern" of the angle); then t = phi + delta_v - FL_v is in [0,2) and the voxel touches only
+// 7 covering 8-tuples, the "pattern" of the angle); then t = phi + delta_v - FL_v is in [0,2) and the voxel touches only
 // bins K+FL_v+{0,1,2}, with Joseph hat weights max(0, 1/a - |t-k|/a^2) (one of the three is zero).  A warp-uniform
 // switch on the pattern selects straight-line code in which every register index is a compile-time constant.
 // For c < 0 the patch is traversed mirrored in x (e = 3-dx); the accumulators are swapped once when the sign changes.
@@ -26,10 +26,11 @@ constexpr int BP_CHUNK = 12;             // angles staged per pipeline stage
 constexpr int WINP = WIN + 8;            // staged bins per (angle, jq): window + NB-1 spill, zero-filled outside the detector
 
 __host__ __device__ constexpr int bp_fl(int pat, int v) {
+    // 9 tuples floor(delta_v) occur over [0, pi); with the relaxed condition 0 <= delta_v - FL_v <= 1 these 7 cover every angle
+    // (the tuples of theta = 0 and theta = pi/2 exactly are absorbed by their neighbours with an offset of exactly 1)
     constexpr int T[BP_NPAT][8] = {
-        {0, 1, 2, 3, 0, 1, 2, 3}, {0, 0, 1, 2, 0, 1, 2, 3}, {0, 0, 1, 2, 0, 1, 2, 2}, {0, 0, 1, 1, 0, 1, 2, 2},
-        {0, 0, 1, 1, 0, 1, 1, 2}, {0, 0, 0, 1, 0, 1, 1, 2}, {0, 0, 0, 1, 0, 1, 1, 1}, {0, 0, 0, 0, 0, 1, 1, 1},
-        {0, 0, 0, 0, 1, 1, 1, 1}};
+        {0, 0, 1, 2, 0, 1, 2, 3}, {0, 0, 0, 0, 0, 1, 1, 1}, {0, 0, 1, 2, 0, 1, 2, 2}, {0, 0, 0, 1, 0, 1, 1, 2},
+        {0, 0, 1, 1, 0, 1, 1, 2}, {0, 0, 1, 1, 0, 1, 2, 2}, {0, 0, 0, 1, 0, 1, 1, 1}};
     return T[pat][v];
 }
 __host__ __device__ constexpr int bp_nb(int pat) {
@@ -207,17 +208,13 @@ __global__ void __launch_bounds__(BP_THREADS, 4) k_backproject(const float4 *__r
             case 4: bp_angle<4, false, JQ>(acc, wbase, phi, S.tda, S.tdb, K.x, K.y, K.z); break;
             case 5: bp_angle<5, false, JQ>(acc, wbase, phi, S.tda, S.tdb, K.x, K.y, K.z); break;
             case 6: bp_angle<6, false, JQ>(acc, wbase, phi, S.tda, S.tdb, K.x, K.y, K.z); break;
-            case 7: bp_angle<7, false, JQ>(acc, wbase, phi, S.tda, S.tdb, K.x, K.y, K.z); break;
-            case 8: bp_angle<8, false, JQ>(acc, wbase, phi, S.tda, S.tdb, K.x, K.y, K.z); break;
-            case 9: bp_angle<0, true, JQ>(acc, wbase, phi, S.tda, S.tdb, K.x, K.y, K.z); break;
-            case 10: bp_angle<1, true, JQ>(acc, wbase, phi, S.tda, S.tdb, K.x, K.y, K.z); break;
-            case 11: bp_angle<2, true, JQ>(acc, wbase, phi, S.tda, S.tdb, K.x, K.y, K.z); break;
-            case 12: bp_angle<3, true, JQ>(acc, wbase, phi, S.tda, S.tdb, K.x, K.y, K.z); break;
-            case 13: bp_angle<4, true, JQ>(acc, wbase, phi, S.tda, S.tdb, K.x, K.y, K.z); break;
-            case 14: bp_angle<5, true, JQ>(acc, wbase, phi, S.tda, S.tdb, K.x, K.y, K.z); break;
-            case 15: bp_angle<6, true, JQ>(acc, wbase, phi, S.tda, S.tdb, K.x, K.y, K.z); break;
-            case 16: bp_angle<7, true, JQ>(acc, wbase, phi, S.tda, S.tdb, K.x, K.y, K.z); break;
-            case 17: bp_angle<8, true, JQ>(acc, wbase, phi, S.tda, S.tdb, K.x, K.y, K.z); break;
+            case 7: bp_angle<0, true, JQ>(acc, wbase, phi, S.tda, S.tdb, K.x, K.y, K.z); break;
+            case 8: bp_angle<1, true, JQ>(acc, wbase, phi, S.tda, S.tdb, K.x, K.y, K.z); break;
+            case 9: bp_angle<2, true, JQ>(acc, wbase, phi, S.tda, S.tdb, K.x, K.y, K.z); break;
+            case 10: bp_angle<3, true, JQ>(acc, wbase, phi, S.tda, S.tdb, K.x, K.y, K.z); break;
+            case 11: bp_angle<4, true, JQ>(acc, wbase, phi, S.tda, S.tdb, K.x, K.y, K.z); break;
+            case 12: bp_angle<5, true, JQ>(acc, wbase, phi, S.tda, S.tdb, K.x, K.y, K.z); break;
+            case 13: bp_angle<6, true, JQ>(acc, wbase, phi, S.tda, S.tdb, K.x, K.y, K.z); break;
             default: break;
             }
         }

@@ -13,7 +13,7 @@ namespace cp4d {
 constexpr int TILE = 32;          // voxel tile side of both projector kernels
 constexpr int WIN = 48;           // bins a TILE x TILE tile can touch at one angle: floor(31*sqrt2)+4
 constexpr int MAX_M = 32;
-constexpr int BP_NPAT = 9;       // bin-offset patterns of a 4x2 voxel patch (backproject.cu)
+constexpr int BP_NPAT = 7;       // bin-offset patterns of a 4x2 voxel patch (backproject.cu)
 
 // per (tile, base angle) geometry, computed in fp64 on the host at create:
 // bin coordinate of tile-local voxel (lx, ly) relative to the window start is  delta + lx*c + ly*s.
