@@ -181,6 +181,10 @@ int cp4d_create(const cp4d_params *p, cp4d_ctx **out) {
         if (ang[i].pat < 0) { delete ctx; return CP4D_EINVAL; }
         ang[i].pat_fl = bp_pattern_fl(ang[i].pat);
     }
+    ctx->n_cpos = 0;
+    while (ctx->n_cpos < d.n0 && ang[ctx->n_cpos].c >= 0.f) ++ctx->n_cpos;
+    for (int i = ctx->n_cpos; i < d.n0; ++i)
+        if (ang[i].c >= 0.f) { delete ctx; return CP4D_EINVAL; }   // cos is monotone on [0, pi): cannot happen
     std::vector<FwAngle> fwang(d.n0);
     std::vector<int32_t> fworder;
     for (int pass = 0; pass < 2; ++pass) {

@@ -12,7 +12,8 @@
 // 7 covering 8-tuples, the "pattern" of the angle); then t = phi + delta_v - FL_v is in [0,2) and the voxel touches only
 // bins K+FL_v+{0,1,2}, with Joseph hat weights max(0, 1/a - |t-k|/a^2) (one of the three is zero).  A warp-uniform
 // switch on the pattern selects straight-line code in which every register index is a compile-time constant.
-// For c < 0 the patch is traversed mirrored in x (e = 3-dx); the accumulators are swapped once when the sign changes.
+// For c < 0 the patch is traversed mirrored in x (e = 3-dx): the staged chunks never mix the signs of c, and the accumulators
+// are mirrored once, between the last chunk with c >= 0 and the first with c < 0.
 #include <cmath>
 
 #include "cp4d_internal.cuh"
@@ -69,11 +70,12 @@ __device__ __forceinline__ void bulk_g2s(void *dst_smem, const void *src_gmem, u
                  "l"(src_gmem), "r"(bytes), "r"(smem_u32(bar)) : "memory");
 }
 
-template <int PAT, int V, bool NEG, int JQ, int NB>
+template <int PAT, int V, int JQ, int NB>
 __device__ __forceinline__ void bp_voxel(float4 (&acc)[8][JQ], const float4 (&B)[NB][JQ], float phi, const float (&tdv)[8],
                                          float A1, float A2, float A3) {
-    // accumulator V is voxel (dx, dy) = (V & 3, V >> 2); for c < 0 its offset from the patch minimum is that of e = 3 - dx
-    constexpr int E = (NEG ? 3 - (V & 3) : (V & 3)) + (V & 4), FL = bp_fl(PAT, E);
+    // accumulator V holds the voxel at offset (e, dy) = (V & 3, V >> 2) from the patch minimum: dx = e for c >= 0, dx = 3 - e
+    // for c < 0 (the kernel mirrors the accumulators once when the sign of c changes)
+    constexpr int E = V, FL = bp_fl(PAT, E);
     // E == 0 is the patch minimum itself: delta = 0, t = phi < 1, so its third candidate bin always has weight 0
     const float t = E == 0 ? phi : phi + tdv[E];                                  // in [0,2)
     const float x0 = fmaxf(0.f, fmaf(-A2, t, A1));
@@ -92,7 +94,7 @@ __device__ __forceinline__ void bp_voxel(float4 (&acc)[8][JQ], const float4 (&B)
     }
 }
 
-template <int PAT, bool NEG, int JQ>
+template <int PAT, int JQ>
 __device__ __forceinline__ void bp_angle(float4 (&acc)[8][JQ], const float4 *wbase, float phi, const float4 tda,
                                          const float4 tdb, float A1, float A2, float A3) {
     constexpr int NB = bp_nb(PAT);
@@ -102,20 +104,20 @@ __device__ __forceinline__ void bp_angle(float4 (&acc)[8][JQ], const float4 *wba
 #pragma unroll
         for (int jc = 0; jc < JQ; ++jc) B[k][jc] = wbase[jc * WINP + k];
     const float tdv[8] = {tda.x, tda.y, tda.z, tda.w, tdb.x, tdb.y, tdb.z, tdb.w};
-    bp_voxel<PAT, 0, NEG, JQ, NB>(acc, B, phi, tdv, A1, A2, A3);
-    bp_voxel<PAT, 1, NEG, JQ, NB>(acc, B, phi, tdv, A1, A2, A3);
-    bp_voxel<PAT, 2, NEG, JQ, NB>(acc, B, phi, tdv, A1, A2, A3);
-    bp_voxel<PAT, 3, NEG, JQ, NB>(acc, B, phi, tdv, A1, A2, A3);
-    bp_voxel<PAT, 4, NEG, JQ, NB>(acc, B, phi, tdv, A1, A2, A3);
-    bp_voxel<PAT, 5, NEG, JQ, NB>(acc, B, phi, tdv, A1, A2, A3);
-    bp_voxel<PAT, 6, NEG, JQ, NB>(acc, B, phi, tdv, A1, A2, A3);
-    bp_voxel<PAT, 7, NEG, JQ, NB>(acc, B, phi, tdv, A1, A2, A3);
+    bp_voxel<PAT, 0, JQ, NB>(acc, B, phi, tdv, A1, A2, A3);
+    bp_voxel<PAT, 1, JQ, NB>(acc, B, phi, tdv, A1, A2, A3);
+    bp_voxel<PAT, 2, JQ, NB>(acc, B, phi, tdv, A1, A2, A3);
+    bp_voxel<PAT, 3, JQ, NB>(acc, B, phi, tdv, A1, A2, A3);
+    bp_voxel<PAT, 4, JQ, NB>(acc, B, phi, tdv, A1, A2, A3);
+    bp_voxel<PAT, 5, JQ, NB>(acc, B, phi, tdv, A1, A2, A3);
+    bp_voxel<PAT, 6, JQ, NB>(acc, B, phi, tdv, A1, A2, A3);
+    bp_voxel<PAT, 7, JQ, NB>(acc, B, phi, tdv, A1, A2, A3);
 }
 
 }  // namespace
 
 struct BpArgs {
-    int n, nz, nd, n0, Q, gp, gpl;
+    int n, nz, nd, n0, Q, gp, gpl, n_pos;   // n_pos: the first n_pos base angles have c >= 0, the others c < 0
     const AngleTab *ang;
     const TileGeo *geo;
 };
@@ -142,10 +144,13 @@ __global__ void __launch_bounds__(BP_THREADS, 4) k_backproject(const float4 *__r
     const int pxi = (l & 1) | ((l >> 2) & 6), pyi = ((l >> 1) & 3) | (w << 2);
     const float fx0 = (float)(4 * pxi), fy0 = (float)(2 * pyi);
     const TileGeo *geo = a.geo + (int64_t)blockIdx.x * a.n0;
-    const int nch = (a.n0 + BP_CHUNK - 1) / BP_CHUNK;
+    // chunks never mix the signs of c: chunks of the angles with c >= 0 first, then of those with c < 0
+    const int nchA = (a.n_pos + BP_CHUNK - 1) / BP_CHUNK, nch = nchA + (a.n0 - a.n_pos + BP_CHUNK - 1) / BP_CHUNK;
+    auto chunk_begin = [&](int ch) { return ch < nchA ? ch * BP_CHUNK : a.n_pos + (ch - nchA) * BP_CHUNK; };
+    auto chunk_count = [&](int ch) { return min(BP_CHUNK, (ch < nchA ? a.n_pos : a.n0) - chunk_begin(ch)); };
 
     auto stage = [&](int buf, int ch) {
-        const int i0 = ch * BP_CHUNK;
+        const int i0 = chunk_begin(ch), cnt = chunk_count(ch);
         if (threadIdx.x < BP_CHUNK) {
             const int i = min(i0 + (int)threadIdx.x, a.n0 - 1);
             const AngleTab A = a.ang[i];
@@ -162,7 +167,7 @@ __global__ void __launch_bounds__(BP_THREADS, 4) k_backproject(const float4 *__r
         // one TMA bulk copy per (angle, coefficient chunk) row of the window: WINP bins x 16 B, always inside the padded
         // scratch row (cp4d_create checks), so no bounds logic; lanes 0..nrows-1 of warp 0 each issue one copy
         if (threadIdx.x < 32) {
-            const int nrows = min(BP_CHUNK, a.n0 - i0) * JQ;
+            const int nrows = cnt * JQ;
             if (threadIdx.x == 0) mbar_expect_tx(&mbar[buf], (unsigned)(nrows * WINP * sizeof(float4)));
             __syncwarp();
             if ((int)threadIdx.x < nrows) {
@@ -191,31 +196,34 @@ __global__ void __launch_bounds__(BP_THREADS, 4) k_backproject(const float4 *__r
         // buffer buf^1 and sang[buf^1] were last read in iteration ch-1, which ended with __syncthreads
         if (ch + 1 < nch) stage(buf ^ 1, ch + 1);
         mbar_wait(&mbar[buf], (unsigned)((ch >> 1) & 1));
-        const int na = min(BP_CHUNK, a.n0 - ch * BP_CHUNK);
+        const int na = chunk_count(ch);
+        // from the first chunk with c < 0 on, the patch is traversed mirrored in x (offset e = 3 - dx): swap the accumulators
+        // once (warp-uniform, outside the angle loop) so that the same straight-line bodies serve both signs
+        const bool neg = ch >= nchA;
+        if (ch == nchA) {
+#pragma unroll
+            for (int dy = 0; dy < 2; ++dy)
+#pragma unroll
+                for (int jc = 0; jc < JQ; ++jc) {
+                    const float4 t0 = acc[4 * dy + 0][jc]; acc[4 * dy + 0][jc] = acc[4 * dy + 3][jc]; acc[4 * dy + 3][jc] = t0;
+                    const float4 t1 = acc[4 * dy + 1][jc]; acc[4 * dy + 1][jc] = acc[4 * dy + 2][jc]; acc[4 * dy + 2][jc] = t1;
+                }
+        }
         for (int aa = 0; aa < na; ++aa) {
             const BpAngle &S = sang[buf][aa];
             const float4 G = S.g, K = S.k;
-            const bool neg = G.y < 0.f;
             const float umin = fmaf(fx0 + (neg ? 3.0f : 0.0f), G.y, fmaf(fy0, G.z, G.x));
             const float fk = floorf(umin);
             const float phi = umin - fk;
             const float4 *wbase = &win[buf][aa][0][(int)fk];
-            switch (__float_as_int(K.w) + (neg ? BP_NPAT : 0)) {
-            case 0: bp_angle<0, false, JQ>(acc, wbase, phi, S.tda, S.tdb, K.x, K.y, K.z); break;
-            case 1: bp_angle<1, false, JQ>(acc, wbase, phi, S.tda, S.tdb, K.x, K.y, K.z); break;
-            case 2: bp_angle<2, false, JQ>(acc, wbase, phi, S.tda, S.tdb, K.x, K.y, K.z); break;
-            case 3: bp_angle<3, false, JQ>(acc, wbase, phi, S.tda, S.tdb, K.x, K.y, K.z); break;
-            case 4: bp_angle<4, false, JQ>(acc, wbase, phi, S.tda, S.tdb, K.x, K.y, K.z); break;
-            case 5: bp_angle<5, false, JQ>(acc, wbase, phi, S.tda, S.tdb, K.x, K.y, K.z); break;
-            case 6: bp_angle<6, false, JQ>(acc, wbase, phi, S.tda, S.tdb, K.x, K.y, K.z); break;
-            case 7: bp_angle<0, true, JQ>(acc, wbase, phi, S.tda, S.tdb, K.x, K.y, K.z); break;
-            case 8: bp_angle<1, true, JQ>(acc, wbase, phi, S.tda, S.tdb, K.x, K.y, K.z); break;
-            case 9: bp_angle<2, true, JQ>(acc, wbase, phi, S.tda, S.tdb, K.x, K.y, K.z); break;
-            case 10: bp_angle<3, true, JQ>(acc, wbase, phi, S.tda, S.tdb, K.x, K.y, K.z); break;
-            case 11: bp_angle<4, true, JQ>(acc, wbase, phi, S.tda, S.tdb, K.x, K.y, K.z); break;
-            case 12: bp_angle<5, true, JQ>(acc, wbase, phi, S.tda, S.tdb, K.x, K.y, K.z); break;
-            case 13: bp_angle<6, true, JQ>(acc, wbase, phi, S.tda, S.tdb, K.x, K.y, K.z); break;
-            default: break;
+            switch (__float_as_int(K.w)) {
+            case 0: bp_angle<0, JQ>(acc, wbase, phi, S.tda, S.tdb, K.x, K.y, K.z); break;
+            case 1: bp_angle<1, JQ>(acc, wbase, phi, S.tda, S.tdb, K.x, K.y, K.z); break;
+            case 2: bp_angle<2, JQ>(acc, wbase, phi, S.tda, S.tdb, K.x, K.y, K.z); break;
+            case 3: bp_angle<3, JQ>(acc, wbase, phi, S.tda, S.tdb, K.x, K.y, K.z); break;
+            case 4: bp_angle<4, JQ>(acc, wbase, phi, S.tda, S.tdb, K.x, K.y, K.z); break;
+            case 5: bp_angle<5, JQ>(acc, wbase, phi, S.tda, S.tdb, K.x, K.y, K.z); break;
+            default: bp_angle<6, JQ>(acc, wbase, phi, S.tda, S.tdb, K.x, K.y, K.z); break;
             }
         }
         __syncthreads();
@@ -223,7 +231,7 @@ __global__ void __launch_bounds__(BP_THREADS, 4) k_backproject(const float4 *__r
     float4 *O = reinterpret_cast<float4 *>(out);
 #pragma unroll
     for (int v = 0; v < 8; ++v) {
-        const int x = tix * TILE + 4 * pxi + (v & 3), y = tiy * TILE + 2 * pyi + (v >> 2);
+        const int x = tix * TILE + 4 * pxi + (nch > nchA ? 3 - (v & 3) : (v & 3)), y = tiy * TILE + 2 * pyi + (v >> 2);
         if (x < a.n && y < a.n) {
             float4 *dst = O + (((int64_t)z * a.n + y) * a.n + x) * a.Q + jg * JQ;
 #pragma unroll
@@ -265,7 +273,7 @@ cudaError_t launch_backproject(cp4d_ctx *c, const float4 *gt, float *f_out, int 
     ProfScope ps(c, CP4D_K_BACKPROJECT);
     const Dims &d = c->d;
     const int Q = Q_override > 0 ? Q_override : d.Q;
-    BpArgs a{d.n, d.nz, d.nd, d.n0, Q, d.gp, d.gpl, c->ang, c->geo};
+    BpArgs a{d.n, d.nz, d.nd, d.n0, Q, d.gp, d.gpl, c->n_cpos, c->ang, c->geo};
     c->launches++;
     if (Q % 2 == 0) return bp_launch<2>(c, gt, f_out, a);
     return bp_launch<1>(c, gt, f_out, a);

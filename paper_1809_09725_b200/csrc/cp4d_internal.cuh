@@ -71,6 +71,7 @@ struct cp4d_ctx {
     cp4d::FwAngle *fwang;      // [n0]
     int32_t *fworder;          // [n0]: base angles whose rays step over columns first, then the others
     int n_colstep;             // how many of the former
+    int n_cpos;                // the first n_cpos base angles have cos >= 0 (backprojector: chunks never mix the signs)
     cp4d::TileGeo *geo;        // [tile][n0]
     double *red;               // 8 doubles for reductions
     uint64_t launches;
