@@ -12,6 +12,8 @@
 // Coordinates: the host computes, in fp64, for every (tile, base angle) the window start `bstart` and the offset
 // `delta` such that the bin coordinate of tile-local voxel (lx,ly) is  u = delta + lx*c + ly*s  with 1 <= u < WIN-1;
 // all fp32 arithmetic in the kernels is on these small tile-local numbers.
+#include <algorithm>
+
 #include "cp4d_internal.cuh"
 
 namespace cp4d {
@@ -27,6 +29,7 @@ struct ProjArgs {
     const FwAngle *fwang;      // k_forward_rays: packed per-angle parameters and the angle order by stepping axis
     const int32_t *fworder;
     int n_colstep;
+    int tiles, agroups;        // blockIdx.x = tile + tiles * angle group (small problems split the base angles over CTAs)
 };
 
 // ---------------------------------------------------------------------------------------------------
@@ -65,17 +68,22 @@ __global__ void __launch_bounds__(FR_THREADS, 3) k_forward_rays(const float *__r
     constexpr int ZZ = C::ZZ;
     extern __shared__ float4 tile[];  // [TILE+3][RSV][4]: 1-voxel zero border, plus a second zero row at the bottom
     const int tiles_1d = (a.n + TILE - 1) / TILE;
-    const int tix = blockIdx.x % tiles_1d, tiy = blockIdx.x / tiles_1d;
+    const int tile_id = blockIdx.x % a.tiles, ag = blockIdx.x / a.tiles;
+    const int tix = tile_id % tiles_1d, tiy = tile_id / tiles_1d;
     const int z0 = blockIdx.y * ZZ, jg = blockIdx.z;
     const int x0 = tix * TILE, y0 = tiy * TILE;
     const int u = threadIdx.x >> 3, sp = (threadIdx.x >> 2) & 1, c4 = threadIdx.x & 3;   // chunk c4 = (slice zz, coefficient chunk jc)
     const int zz = c4 / JQ, jc = c4 % JQ, z = z0 + zz;
     const float4 zero = make_float4(0.f, 0.f, 0.f, 0.f);
     const float4 *F = reinterpret_cast<const float4 *>(f);
-    const TileGeo *geo = a.geo + (int64_t)blockIdx.x * a.n0;
+    const TileGeo *geo = a.geo + (int64_t)tile_id * a.n0;
 
     for (int t = threadIdx.x; t < (TILE + 3) * RSV * 4; t += FR_THREADS) tile[t] = zero;   // borders stay zero in both passes
     for (int pass = 0; pass < 2; ++pass) {   // pass 0: rays stepping over columns; pass 1: over rows, on the transposed tile
+        // this pass's slice of the angle list, split evenly over the angle groups
+        const int l0 = pass ? a.n_colstep : 0, l1 = pass ? a.n0 : a.n_colstep;
+        const int ii0 = l0 + (int)((int64_t)(l1 - l0) * ag / a.agroups), ii1 = l0 + (int)((int64_t)(l1 - l0) * (ag + 1) / a.agroups);
+        if (ii0 == ii1) continue;            // (CTA-uniform) no angle of this class for this CTA
         __syncthreads();
         for (int t = threadIdx.x; t < TILE * TILE * 4; t += FR_THREADS) {
             const int c = t & 3, lx = (t >> 2) & (TILE - 1), ly = t >> 7;
@@ -85,7 +93,6 @@ __global__ void __launch_bounds__(FR_THREADS, 3) k_forward_rays(const float *__r
                 ? __ldg(F + (((int64_t)gz * a.n + gy) * a.n + gx) * a.Q + jg * JQ + c % JQ) : zero;
         }
         __syncthreads();
-        const int ii0 = pass ? a.n_colstep : 0, ii1 = pass ? a.n0 : a.n_colstep;
         for (int ii = ii0; ii < ii1; ++ii) {
             const int i = a.fworder[ii];
             const FwAngle A = a.fwang[i];
@@ -143,7 +150,12 @@ static cudaError_t fwd_launch_rays(cp4d_ctx *c, const float *f, float4 *P, const
     const size_t sh = FwRays<JQ>::SMEM;
     cudaError_t e = cudaFuncSetAttribute(k_forward_rays<JQ>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sh);
     if (e != cudaSuccess) return e;
-    k_forward_rays<JQ><<<dim3(d.tiles, (d.nz + FwRays<JQ>::ZZ - 1) / FwRays<JQ>::ZZ, d.Q / JQ), FR_THREADS, sh, c->stream>>>(f, P, a);
+    // small problems: split the base angles over up to 8 CTAs per tile so that the grid fills the 148 SMs x 3 CTAs twice
+    const int nzz = (d.nz + FwRays<JQ>::ZZ - 1) / FwRays<JQ>::ZZ;
+    const int64_t ctas = (int64_t)d.tiles * nzz * (d.Q / JQ);
+    ProjArgs b = a;
+    b.agroups = (int)std::max<int64_t>(1, std::min<int64_t>(std::min(8, d.n0), (2 * 148 * 3 + ctas - 1) / ctas));
+    k_forward_rays<JQ><<<dim3(d.tiles * b.agroups, nzz, d.Q / JQ), FR_THREADS, sh, c->stream>>>(f, P, b);
     return cudaGetLastError();
 }
 
@@ -152,7 +164,7 @@ static int pick_jq(int Q) { return (Q % 4 == 0) ? 4 : (Q % 2 == 0) ? 2 : 1; }
 cudaError_t launch_forward_partial(cp4d_ctx *c, const float *f, float4 *P) {
     ProfScope ps(c, CP4D_K_FORWARD);
     const Dims &d = c->d;
-    ProjArgs a{d.n, d.nz, d.nd, d.n0, d.Q, d.gp, d.gpl, c->ang, c->geo, c->fwang, c->fworder, c->n_colstep};
+    ProjArgs a{d.n, d.nz, d.nd, d.n0, d.Q, d.gp, d.gpl, c->ang, c->geo, c->fwang, c->fworder, c->n_colstep, d.tiles, 1};
     cudaError_t e = cudaMemsetAsync(P, 0, (size_t)d.scratch4 * sizeof(float4), c->stream);
     if (e != cudaSuccess) return e;
     c->launches += 2;
