@@ -43,6 +43,7 @@ int validate(const cp4d_params *p, Dims *d) {
     const int over = (int)std::ceil(std::fmax(0.0, 1.41421356237309515 * ext - 0.5 * (d->nd - 1))) + 3;
     d->gpl = over;
     d->gp = d->nd + 2 * over + WIN + 8;
+    if (d->gp % 8 == 0) d->gp += 1;   // a pitch of whole 128-byte lines measured 1 % slower in the forward projector's REDs
     d->scratch4 = (int64_t)d->nz * d->n0 * d->Q * d->gp;
     if (d->nz > 65535 || d->tiles > 2000000) return CP4D_EINVAL;
     return CP4D_OK;
