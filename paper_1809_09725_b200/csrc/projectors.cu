@@ -130,15 +130,15 @@ __global__ void __launch_bounds__(FR_THREADS, 3) k_forward_rays(const float *__r
                     fma4(acc, w1, v1);
                 }
             }
-            // sum the step phases (lanes differing in the phase bits serve the same ray and chunk)
-            acc.x += __shfl_xor_sync(0xffffffffu, acc.x, 4);
-            acc.y += __shfl_xor_sync(0xffffffffu, acc.y, 4);
-            acc.z += __shfl_xor_sync(0xffffffffu, acc.z, 4);
-            acc.w += __shfl_xor_sync(0xffffffffu, acc.w, 4);
+            // sum the two step parities (lanes l and l^4 serve the same ray and chunk) with 2 shuffles instead of 4: the sp = 0
+            // lane ends up with the (x, y) totals, the sp = 1 lane with (z, w), and each adds its half to P with one 8-byte RED
+            const float s0 = sp ? acc.x : acc.z, s1 = sp ? acc.y : acc.w;          // what the partner needs
+            const float r0 = __shfl_xor_sync(0xffffffffu, s0, 4), r1 = __shfl_xor_sync(0xffffffffu, s1, 4);
+            const float2 tot = sp ? make_float2(acc.z + r0, acc.w + r1) : make_float2(acc.x + r0, acc.y + r1);
             const int b = G.bstart + u;
-            if (sp == 0 && touched && b >= 0 && b < a.nd && z < a.nz) {
-                float4 *dst = P + (((int64_t)z * a.n0 + i) * a.Q + jg * JQ + jc) * a.gp + a.gpl + b;
-                atomicAdd(dst, make_float4(acc.x * A.inv_a, acc.y * A.inv_a, acc.z * A.inv_a, acc.w * A.inv_a));
+            if (touched && b >= 0 && b < a.nd && z < a.nz) {
+                float2 *dst = reinterpret_cast<float2 *>(P + (((int64_t)z * a.n0 + i) * a.Q + jg * JQ + jc) * a.gp + a.gpl + b) + sp;
+                atomicAdd(dst, make_float2(tot.x * A.inv_a, tot.y * A.inv_a));
             }
         }
     }
