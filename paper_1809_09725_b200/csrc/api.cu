@@ -153,6 +153,7 @@ int cp4d_create(const cp4d_params *p, cp4d_ctx **out) {
     ctx->d = d; ctx->lambda1 = p->lambda1; ctx->lambda2 = p->lambda2; ctx->theta = p->theta_relax;
     ctx->tau = ctx->sigma = 0.f; ctx->have_steps = ctx->have_data = false;
     ctx->device = p->device; ctx->stream = (cudaStream_t)p->stream; ctx->launches = 0; ctx->prof_on = false;
+    ctx->fwtab_host = nullptr;
     char *w = (char *)p->workspace_dev;
     ctx->f = (float *)(w + cv.f); ctx->ft = (float *)(w + cv.ft); ctx->bp = (float *)(w + cv.bp);
     ctx->h2 = (float *)(w + cv.h2); ctx->h1 = (float *)(w + cv.h1); ctx->g = (float *)(w + cv.g);
@@ -194,6 +195,7 @@ int cp4d_create(const cp4d_params *p, cp4d_ctx **out) {
         if (pass == 0) ctx->n_colstep = (int)fworder.size();
     }
     for (int i = 0; i < d.n0; ++i) fwang[i] = FwAngle{ang[i].fw_inv, ang[i].fw_step, ang[i].fw_istep, ang[i].inv_a};
+    ctx->fwtab_host = fwtable_new(fwang.data(), fworder.data(), d.n0);
     std::vector<TileGeo> geo((size_t)d.tiles * d.n0);
     const double cen = 0.5 * (d.n - 1), cd = 0.5 * (d.nd - 1);
     for (int t = 0; t < d.tiles; ++t) {
@@ -205,7 +207,7 @@ int cp4d_create(const cp4d_params *p, cp4d_ctx **out) {
             const double pmin = p0 + std::fmin(0.0, (TILE - 1) * c) + std::fmin(0.0, (TILE - 1) * s);
             const double bs = std::floor(pmin) - 1.0;
             geo[(size_t)t * d.n0 + i].bstart = (int32_t)bs;
-            if ((int32_t)bs < -d.gpl || (int32_t)bs + WIN + 8 > d.gp - d.gpl) { delete ctx; return CP4D_EINVAL; }
+            if ((int32_t)bs < -d.gpl || (int32_t)bs + WIN + 8 > d.gp - d.gpl) { cp4d_destroy(ctx); return CP4D_EINVAL; }
             geo[(size_t)t * d.n0 + i].delta = (float)(p0 - bs);
         }
     }
@@ -235,7 +237,7 @@ int cp4d_create(const cp4d_params *p, cp4d_ctx **out) {
         (e = cudaStreamSynchronize(ctx->stream)) != cudaSuccess) {
         ctx->err = cudaGetErrorString(e);   // (the context dies with the error: the caller only sees CP4D_ECUDA)
         cudaGetLastError();
-        delete ctx;
+        cp4d_destroy(ctx);
         return CP4D_ECUDA;
     }
     *out = ctx;
@@ -246,6 +248,7 @@ int cp4d_destroy(cp4d_ctx *ctx) {
     if (ctx) {
         for (auto &r : ctx->prof) { cudaEventDestroy(r.a); cudaEventDestroy(r.b); }
         for (auto e : ctx->ev_pool) cudaEventDestroy(e);
+        fwtable_free(ctx->fwtab_host);
     }
     delete ctx;
     return CP4D_OK;

@@ -38,6 +38,8 @@ struct FwAngle {
     float inv, step, istep, inv_a;
 };
 
+struct FwTable;   // projectors.cu: the forward kernel's per-angle parameters as a kernel parameter (constant bank)
+
 struct Dims {
     int n, nz, nd, na, npi, n0, m, Q;  // Q = m/4 float4 chunks per voxel of a coefficient stack
     int nf, mp, Qp;                    // frame mode: nf frames (0 = coefficient mode); mp = nf ? nf : m is the
@@ -71,6 +73,7 @@ struct cp4d_ctx {
     cp4d::FwAngle *fwang;      // [n0]
     int32_t *fworder;          // [n0]: base angles whose rays step over columns first, then the others
     int n_colstep;             // how many of the former
+    cp4d::FwTable *fwtab_host; // host copy of fwang / fworder for the kernel-parameter path (n0 <= 512), else null
     int n_cpos;                // the first n_cpos base angles have cos >= 0 (backprojector: chunks never mix the signs)
     cp4d::TileGeo *geo;        // [tile][n0]
     double *red;               // 8 doubles for reductions
@@ -116,6 +119,9 @@ cudaError_t launch_update(cp4d_ctx *c, float tau, const float *bp, const float *
 cudaError_t launch_fold(cp4d_ctx *c, const float *g, float4 *gt);
 // synth: out = K1 f from partial sums P.  mode 0: g_out = v ; mode 1: h1 = (h1 + sigma (v - g))/(1+sigma)
 cudaError_t launch_synth(cp4d_ctx *c, const float4 *P, int mode, float sigma, const float *g, float *out);
+// host helpers of projectors.cu for cp4d_create / cp4d_destroy
+FwTable *fwtable_new(const FwAngle *ang, const int32_t *order, int n0);   // null when n0 is too large
+void fwtable_free(FwTable *t);
 cudaError_t launch_forward_partial(cp4d_ctx *c, const float *f, float4 *P);
 cudaError_t launch_backproject(cp4d_ctx *c, const float4 *gt, float *f_out, int Q_override = 0);
 // cp4d_fbp: Shepp-Logan filter along the bins; per-half-rotation rows gathered into the projector scratch (box basis)

@@ -61,8 +61,18 @@ struct FwRays {
     static_assert(RSV % NPH == 0, "row pitch must be a multiple of the number of step phases");
 };
 
-template <int JQ>
-__global__ void __launch_bounds__(FR_THREADS, 3) k_forward_rays(const float *__restrict__ f, float4 *__restrict__ P, ProjArgs a) {
+// per-angle parameters in kernel-parameter (constant bank) space: indexed loads from it go through the constant cache, not
+// through the LSU data pipe that binds this kernel.  Used when n_theta0 <= FW_TAB; otherwise the same data is read from
+// global memory.
+constexpr int FW_TAB = 512;
+struct FwTable {
+    FwAngle a[FW_TAB];
+    int32_t order[FW_TAB];
+};
+
+template <int JQ, bool CONST_TAB>
+__global__ void __launch_bounds__(FR_THREADS, 3) k_forward_rays(const float *__restrict__ f, float4 *__restrict__ P, ProjArgs a,
+                                                                const __grid_constant__ FwTable tab) {
     using C = FwRays<JQ>;
     constexpr int NPH = C::NPH, RSV = C::RSV, CHUNK = C::CHUNK, UNROLL = C::UNROLL;
     constexpr int ZZ = C::ZZ;
@@ -94,8 +104,8 @@ __global__ void __launch_bounds__(FR_THREADS, 3) k_forward_rays(const float *__r
         }
         __syncthreads();
         for (int ii = ii0; ii < ii1; ++ii) {
-            const int i = a.fworder[ii];
-            const FwAngle A = a.fwang[i];
+            const int i = CONST_TAB ? tab.order[ii] : a.fworder[ii];
+            const FwAngle A = CONST_TAB ? tab.a[i] : a.fwang[i];
             const TileGeo G = geo[i];
             // pass 0: the ray crosses column k at row (du - k c)/s; pass 1: it crosses row k at column (du - k s)/c
             const float step = A.step, base = ((float)u - G.delta) * A.inv;
@@ -148,18 +158,32 @@ template <int JQ>
 static cudaError_t fwd_launch_rays(cp4d_ctx *c, const float *f, float4 *P, const ProjArgs &a) {
     const Dims &d = c->d;
     const size_t sh = FwRays<JQ>::SMEM;
-    cudaError_t e = cudaFuncSetAttribute(k_forward_rays<JQ>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sh);
-    if (e != cudaSuccess) return e;
     // small problems: split the base angles over up to 8 CTAs per tile so that the grid fills the 148 SMs x 3 CTAs twice
     const int nzz = (d.nz + FwRays<JQ>::ZZ - 1) / FwRays<JQ>::ZZ;
     const int64_t ctas = (int64_t)d.tiles * nzz * (d.Q / JQ);
     ProjArgs b = a;
     b.agroups = (int)std::max<int64_t>(1, std::min<int64_t>(std::min(8, d.n0), (2 * 148 * 3 + ctas - 1) / ctas));
-    k_forward_rays<JQ><<<dim3(d.tiles * b.agroups, nzz, d.Q / JQ), FR_THREADS, sh, c->stream>>>(f, P, b);
+    const dim3 grid(d.tiles * b.agroups, nzz, d.Q / JQ);
+    cudaError_t e;
+    if (d.n0 <= FW_TAB) {
+        if ((e = cudaFuncSetAttribute(k_forward_rays<JQ, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sh)) != cudaSuccess) return e;
+        k_forward_rays<JQ, true><<<grid, FR_THREADS, sh, c->stream>>>(f, P, b, *c->fwtab_host);
+    } else {
+        if ((e = cudaFuncSetAttribute(k_forward_rays<JQ, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sh)) != cudaSuccess) return e;
+        k_forward_rays<JQ, false><<<grid, FR_THREADS, sh, c->stream>>>(f, P, b, FwTable{});
+    }
     return cudaGetLastError();
 }
 
 static int pick_jq(int Q) { return (Q % 4 == 0) ? 4 : (Q % 2 == 0) ? 2 : 1; }
+
+FwTable *fwtable_new(const FwAngle *ang, const int32_t *order, int n0) {
+    if (n0 > FW_TAB) return nullptr;
+    FwTable *t = new FwTable();
+    for (int i = 0; i < n0; ++i) { t->a[i] = ang[i]; t->order[i] = order[i]; }
+    return t;
+}
+void fwtable_free(FwTable *t) { delete t; }
 
 cudaError_t launch_forward_partial(cp4d_ctx *c, const float *f, float4 *P) {
     ProfScope ps(c, CP4D_K_FORWARD);
