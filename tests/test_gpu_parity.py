@@ -47,6 +47,10 @@ CASES = {
     "one_angle_per_pi": synth.CONFIGS[1].scaled(cfg=16, n=33, nd=33, nz=2, n_angles=6, n_half_rot=6, m=4),
     # m = 16: the 8-lanes-per-ray forward kernel and two coefficient groups in the backprojector, on ragged tiles
     "ragged_m16": synth.CONFIGS[3].scaled(cfg=17, n=75, nd=90, nz=3, n_angles=78, n_half_rot=3, m=16, iters=12, n_objects=5),
+    # more than 512 base angles: the forward kernel reads its per-angle tables from global memory instead of the kernel parameter
+    "many_angles": synth.CONFIGS[1].scaled(cfg=18, n=36, nd=41, nz=2, n_angles=530, n_half_rot=1, m=4),
+    # a volume smaller than one tile and a detector wider than the scratch window
+    "tiny": synth.CONFIGS[1].scaled(cfg=19, n=5, nd=9, nz=1, n_angles=14, n_half_rot=2, m=4),
 }
 
 
