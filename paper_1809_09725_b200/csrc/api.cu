@@ -154,6 +154,7 @@ int cp4d_create(const cp4d_params *p, cp4d_ctx **out) {
     ctx->tau = ctx->sigma = 0.f; ctx->have_steps = ctx->have_data = false;
     ctx->device = p->device; ctx->stream = (cudaStream_t)p->stream; ctx->launches = 0; ctx->prof_on = false;
     ctx->fwtab_host = nullptr;
+    ctx->iter_graph = nullptr; ctx->iter_graph_launches = 0; ctx->iter_graph_off = false;
     char *w = (char *)p->workspace_dev;
     ctx->f = (float *)(w + cv.f); ctx->ft = (float *)(w + cv.ft); ctx->bp = (float *)(w + cv.bp);
     ctx->h2 = (float *)(w + cv.h2); ctx->h1 = (float *)(w + cv.h1); ctx->g = (float *)(w + cv.g);
@@ -249,6 +250,7 @@ int cp4d_destroy(cp4d_ctx *ctx) {
         for (auto &r : ctx->prof) { cudaEventDestroy(r.a); cudaEventDestroy(r.b); }
         for (auto e : ctx->ev_pool) cudaEventDestroy(e);
         fwtable_free(ctx->fwtab_host);
+        if (ctx->iter_graph) cudaGraphExecDestroy(ctx->iter_graph);
     }
     delete ctx;
     return CP4D_OK;
@@ -353,6 +355,10 @@ int cp4d_set_data(cp4d_ctx *ctx, const float *g) {
 int cp4d_set_steps(cp4d_ctx *ctx, float tau, float sigma) {
     if (!ctx) return CP4D_EINVAL;
     if (!(tau > 0.f) || !(sigma > 0.f)) return fail(ctx, CP4D_EINVAL, "set_steps: tau, sigma must be > 0");
+    if (ctx->iter_graph && (tau != ctx->tau || sigma != ctx->sigma)) {   // the step sizes are baked into the captured launches
+        cudaGraphExecDestroy(ctx->iter_graph);
+        ctx->iter_graph = nullptr;
+    }
     ctx->tau = tau; ctx->sigma = sigma; ctx->have_steps = true;
     return CP4D_OK;
 }
@@ -373,18 +379,57 @@ int cp4d_reset(cp4d_ctx *ctx, const float *f0) {
     return CP4D_OK;
 }
 
+// one pass of Fig. 2, enqueued on the context's stream
+static int iterate_once(cp4d_ctx *ctx) {
+    // step 3: h1 <- prox_{sigma F1*}(h1 + sigma K1 ft)
+    if (int r = forward_into(ctx, ctx->ft, 1, ctx->sigma, ctx->g, ctx->h1)) return r;
+    // step 4: h2 <- prox_{sigma F2*}(h2 + sigma K2 ft)
+    CK(launch_prox_f2(ctx, ctx->sigma, ctx->ft, ctx->h2), "prox_f2");
+    // steps 5-6: f <- f - tau K1^T h1 + tau div h2 ; ft <- f+ + theta (f+ - f)
+    if (int r = adjoint_into(ctx, ctx->h1, ctx->bp)) return r;
+    CK(launch_update(ctx, ctx->tau, ctx->bp, ctx->h2, ctx->f, ctx->ft), "update");
+    return CP4D_OK;
+}
+
+// capture one iteration into ctx->iter_graph; false (and eager launches from then on) if the stream cannot be captured
+static bool capture_iteration(cp4d_ctx *ctx) {
+    if (ctx->iter_graph_off || ctx->stream == nullptr || ctx->stream == cudaStreamLegacy) return false;
+    const uint64_t l0 = ctx->launches;
+    if (cudaStreamBeginCapture(ctx->stream, cudaStreamCaptureModeThreadLocal) != cudaSuccess) {
+        cudaGetLastError();
+        ctx->iter_graph_off = true;
+        return false;
+    }
+    const int r = iterate_once(ctx);
+    cudaGraph_t g = nullptr;
+    const cudaError_t e = cudaStreamEndCapture(ctx->stream, &g);
+    ctx->iter_graph_launches = ctx->launches - l0;
+    ctx->launches = l0;
+    bool ok = r == CP4D_OK && e == cudaSuccess && g != nullptr;
+    if (ok) ok = cudaGraphInstantiate(&ctx->iter_graph, g, 0) == cudaSuccess;
+    if (g) cudaGraphDestroy(g);
+    if (!ok) {
+        cudaGetLastError();
+        ctx->iter_graph = nullptr;
+        ctx->iter_graph_off = true;
+        ctx->err.clear();
+    }
+    return ok;
+}
+
 int cp4d_iterate(cp4d_ctx *ctx, int32_t n_iters) {
     if (!ctx) return CP4D_EINVAL;
     if (n_iters < 0) return fail(ctx, CP4D_EINVAL, "iterate: n_iters < 0");
     if (!ctx->have_steps || !ctx->have_data) return fail(ctx, CP4D_ESTATE, "iterate: set_data and set_steps first");
+    // the per-kernel timing of cp4d_profile_begin records events between the launches, so it takes the eager path
+    const bool graph = !ctx->prof_on && n_iters >= 2 && (ctx->iter_graph || capture_iteration(ctx));
     for (int it = 0; it < n_iters; ++it) {
-        // step 3: h1 <- prox_{sigma F1*}(h1 + sigma K1 ft)
-        if (int r = forward_into(ctx, ctx->ft, 1, ctx->sigma, ctx->g, ctx->h1)) return r;
-        // step 4: h2 <- prox_{sigma F2*}(h2 + sigma K2 ft)
-        CK(launch_prox_f2(ctx, ctx->sigma, ctx->ft, ctx->h2), "prox_f2");
-        // steps 5-6: f <- f - tau K1^T h1 + tau div h2 ; ft <- f+ + theta (f+ - f)
-        if (int r = adjoint_into(ctx, ctx->h1, ctx->bp)) return r;
-        CK(launch_update(ctx, ctx->tau, ctx->bp, ctx->h2, ctx->f, ctx->ft), "update");
+        if (graph) {
+            CK(cudaGraphLaunch(ctx->iter_graph, ctx->stream), "iterate (graph)");
+            ctx->launches += ctx->iter_graph_launches;
+        } else if (int r = iterate_once(ctx)) {
+            return r;
+        }
     }
     return CP4D_OK;
 }

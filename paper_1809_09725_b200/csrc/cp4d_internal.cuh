@@ -73,6 +73,11 @@ struct cp4d_ctx {
     cp4d::FwAngle *fwang;      // [n0]
     int32_t *fworder;          // [n0]: base angles whose rays step over columns first, then the others
     int n_colstep;             // how many of the former
+    // one CP iteration captured as a CUDA graph (cp4d_iterate replays it; rebuilt when tau / sigma change).  Not available on
+    // the legacy default stream, which cannot be captured: the launches are then issued one by one.
+    cudaGraphExec_t iter_graph;
+    uint64_t iter_graph_launches;
+    bool iter_graph_off;
     cp4d::FwTable *fwtab_host; // host copy of fwang / fworder for the kernel-parameter path (n0 <= 512), else null
     int n_cpos;                // the first n_cpos base angles have cos >= 0 (backprojector: chunks never mix the signs)
     cp4d::TileGeo *geo;        // [tile][n0]
