@@ -226,6 +226,9 @@ def run_cp4d(args, c, rank, world):
     local = int(os.environ.get("LOCAL_RANK", rank))
     torch.cuda.set_device(local)
     dev = torch.device("cuda", local)
+    # everything runs on one non-default stream: cp4d_iterate replays a CUDA graph of one iteration there (the legacy
+    # default stream cannot be captured); the CUDA events below are recorded on this same stream
+    torch.cuda.set_stream(torch.cuda.Stream(dev))
     if world > 1:
         dist.init_process_group("nccl", device_id=dev)
     if rank == 0:
@@ -271,6 +274,7 @@ def run_cp4d(args, c, rank, world):
     t1 = sampler.mark()
     launches = ctx.launch_count() - l0
     ms = e0.elapsed_time(e1)
+    graph_replays = ctx.graph_replays()
 
     # ---- roofline: second pass of K steps with the library's per-kernel CUDA events on the same stream ----
     ctx.profile_begin()
@@ -316,7 +320,7 @@ def run_cp4d(args, c, rank, world):
                "seconds": dt}
         del g_host, f_host
     return ctx, dict(ms=ms, launches=launches, prof=prof, prof_gd=prof_gd, ops=ops, e2e=e2e, clocks=clocks, peaks=peaks,
-                     L=L, launches_total=ctx.launch_count() - launches0)
+                     L=L, launches_total=ctx.launch_count() - launches0, graph_replays=graph_replays)
 
 
 def assemble(args, c, world, r):
@@ -371,7 +375,7 @@ def assemble(args, c, world, r):
                          "forward_ms": r["ops"]["forward_op"], "adjoint_ms": r["ops"]["adjoint_op"],
                          "note": "nominal count N^2*Nz*N_theta*m per call; kernels use the pi-fold (N_theta0 base angles)"},
         "roofline": roofline, "kernels": kernels, "clocks": r["clocks"], "e2e": r["e2e"],
-        "gpu_launches": r["launches"], "impl": "cp4d",
+        "gpu_launches": r["launches"], "cuda_graph_replays": r["graph_replays"], "impl": "cp4d",
     }
     return line
 

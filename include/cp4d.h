@@ -155,6 +155,12 @@ int cp4d_solve_host(cp4d_ctx *ctx, const float *g_host, int32_t n_iters, float *
 int cp4d_sync(cp4d_ctx *ctx);
 /* number of kernels (and memset nodes) this context has enqueued since create */
 int cp4d_launch_count(const cp4d_ctx *ctx, uint64_t *count_out);
+/* cp4d_iterate(n >= 2) on a capturable stream (any stream but the legacy default stream 0) captures one iteration of
+ * Fig. 2 into a CUDA graph on first use and replays it n times; the graph is rebuilt when cp4d_set_steps changes tau or
+ * sigma, and it is bypassed while cp4d_profile_begin is active (the per-kernel events sit between the launches) and on
+ * stream 0, where the launches are issued one by one.  count_out: graph replays since create (each one is counted in
+ * cp4d_launch_count with the number of kernels and memset nodes of one iteration). */
+int cp4d_graph_replays(const cp4d_ctx *ctx, uint64_t *count_out);
 
 /* ---- per-kernel device timing (CUDA events on the context's stream) ------------- */
 /* Kernel classes of the hot path.  FORWARD includes the zero-fill of its partial-sum scratch. */

@@ -63,6 +63,7 @@ def lib():
             "cp4d_solve_host": [vp, vp, i32, vp], "cp4d_sync": [vp],
             "cp4d_objective": [vp] + [C.POINTER(C.c_double)] * 3, "cp4d_fbp": [vp, vp, vp],
             "cp4d_launch_count": [vp, C.POINTER(u64)],
+            "cp4d_graph_replays": [vp, C.POINTER(u64)],
             "cp4d_profile_begin": [vp], "cp4d_profile_end": [vp, C.POINTER(Profile)],
         }
         for name, args in sig.items():
@@ -255,6 +256,12 @@ class Context:
     def launch_count(self) -> int:
         out = C.c_uint64(0)
         self._ck(lib().cp4d_launch_count(self._h, C.byref(out)))
+        return out.value
+
+    def graph_replays(self) -> int:
+        """CUDA-graph replays of one CP iteration issued by iterate() so far (0 on the legacy default stream)."""
+        out = C.c_uint64(0)
+        self._ck(lib().cp4d_graph_replays(self._h, C.byref(out)))
         return out.value
 
     def profile_begin(self):

@@ -154,7 +154,7 @@ int cp4d_create(const cp4d_params *p, cp4d_ctx **out) {
     ctx->tau = ctx->sigma = 0.f; ctx->have_steps = ctx->have_data = false;
     ctx->device = p->device; ctx->stream = (cudaStream_t)p->stream; ctx->launches = 0; ctx->prof_on = false;
     ctx->fwtab_host = nullptr;
-    ctx->iter_graph = nullptr; ctx->iter_graph_launches = 0; ctx->iter_graph_off = false;
+    ctx->iter_graph = nullptr; ctx->iter_graph_launches = 0; ctx->graph_replays = 0; ctx->iter_graph_off = false;
     char *w = (char *)p->workspace_dev;
     ctx->f = (float *)(w + cv.f); ctx->ft = (float *)(w + cv.ft); ctx->bp = (float *)(w + cv.bp);
     ctx->h2 = (float *)(w + cv.h2); ctx->h1 = (float *)(w + cv.h1); ctx->g = (float *)(w + cv.g);
@@ -427,6 +427,7 @@ int cp4d_iterate(cp4d_ctx *ctx, int32_t n_iters) {
         if (graph) {
             CK(cudaGraphLaunch(ctx->iter_graph, ctx->stream), "iterate (graph)");
             ctx->launches += ctx->iter_graph_launches;
+            ctx->graph_replays++;
         } else if (int r = iterate_once(ctx)) {
             return r;
         }
@@ -549,6 +550,12 @@ int cp4d_profile_end(cp4d_ctx *ctx, cp4d_profile *out) {
 const char *cp4d_kernel_name(int k) {
     static const char *names[CP4D_K_COUNT] = {"forward", "synth", "fold", "backproject", "grad", "div", "prox_f2", "update", "reduce", "misc", "mix"};
     return (k >= 0 && k < CP4D_K_COUNT) ? names[k] : "?";
+}
+
+int cp4d_graph_replays(const cp4d_ctx *ctx, uint64_t *out) {
+    if (!ctx || !out) return CP4D_EINVAL;
+    *out = ctx->graph_replays;
+    return CP4D_OK;
 }
 
 int cp4d_launch_count(const cp4d_ctx *ctx, uint64_t *out) {

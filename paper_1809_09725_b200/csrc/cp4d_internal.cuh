@@ -76,7 +76,7 @@ struct cp4d_ctx {
     // one CP iteration captured as a CUDA graph (cp4d_iterate replays it; rebuilt when tau / sigma change).  Not available on
     // the legacy default stream, which cannot be captured: the launches are then issued one by one.
     cudaGraphExec_t iter_graph;
-    uint64_t iter_graph_launches;
+    uint64_t iter_graph_launches, graph_replays;
     bool iter_graph_off;
     cp4d::FwTable *fwtab_host; // host copy of fwang / fworder for the kernel-parameter path (n0 <= 512), else null
     int n_cpos;                // the first n_cpos base angles have cos >= 0 (backprojector: chunks never mix the signs)

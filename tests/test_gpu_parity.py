@@ -189,6 +189,37 @@ def test_solve_host_equals_device_path(torch_cuda, fast_oracle):
     ctx.close()
 
 
+@pytest.mark.parametrize("case", ["ragged", "ragged_m16"])
+def test_iterate_graph_replay(torch_cuda, case):
+    """On a capturable (non-default) stream cp4d_iterate captures one iteration into a CUDA graph and replays it; on the legacy
+    default stream it launches kernel by kernel.  Same iterates, same launch count; new step sizes rebuild the graph."""
+    from paper_1809_09725_b200 import binding
+    torch = torch_cuda
+    c = CASES[case].scaled(lambda1=0.003)
+    g = _data(c).astype(np.float32)
+
+    def run(ctx):
+        ctx.set_data(dev(torch, g)); ctx.set_steps(0.011, 0.012); ctx.reset()
+        ctx.iterate(4); ctx.iterate(3)                 # second call reuses the graph
+        ctx.set_steps(0.009, 0.012); ctx.iterate(2)    # new tau: graph rebuilt
+        ctx.iterate(1)                                 # single iterations are launched directly
+        ctx.sync()
+        s = ctx.state()
+        return {k: s[k].cpu().numpy().astype(np.float64) for k in ("f", "ft", "h1", "h2")}, (ctx.launch_count(), ctx.graph_replays())
+
+    eager = binding.Context.from_config(c)             # current stream = legacy default stream: not capturable
+    a, na = run(eager)
+    side = torch.cuda.Stream()
+    with torch.cuda.stream(side):
+        graph = binding.Context.from_config(c)
+        b, nb = run(graph)
+        graph.close()
+    eager.close()
+    assert na == (nb[0], 0) and nb[1] == 4 + 3 + 2
+    for k in a:
+        assert rel(b[k], a[k]) <= 1e-5, k               # atomics: summation order may differ
+
+
 def test_relaxation_and_warm_start(torch_cuda, fast_oracle):
     """theta = 0.5 (L97: theta in [0,1]) and a non-zero initial guess through cp4d_reset(f0) (L147 'some initial guess')."""
     from paper_1809_09725_b200 import binding
