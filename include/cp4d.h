@@ -73,6 +73,13 @@ typedef struct {
                                  N_t % 4 == 0, N_t <= 32, n_angles % N_t == 0), frame q sits at the time of angle
                                  q*n_angles/N_t; K1 f = K1_coef(f_j) with f_j = sum_q phi_j(t_q) f(t_q), phi_j(t_q) taken
                                  from phi_host's column q*n_angles/N_t; the 4th difference of K2 runs over frames      */
+    int32_t z_open;           /* 0: the context holds the whole volume.  Otherwise it is a z-SLAB of a taller volume (PAPER.md
+                                 L283: "split computations by slices ... we transfer to GPU two extra slices located before and
+                                 after the current set of slices", kept read-only): bit 0 = the face below slice 0 is interior,
+                                 bit 1 = the face above slice nz-1 is interior.  K1 / K1^T act per slice and need nothing; the
+                                 z-differences of K2 / K2^T take the neighbour's slice through the halo arguments of the
+                                 *_slab calls below.  cp4d_grad, cp4d_div, cp4d_prox_f2, cp4d_primal_update, cp4d_iterate,
+                                 cp4d_norm, cp4d_objective and cp4d_solve_host return CP4D_ESTATE on a slab context.          */
 } cp4d_params;
 
 /* Bytes of device workspace a context for these sizes needs (state f, f~, K1^T h1, h2[4], h1, g, one sinogram-sized
@@ -146,6 +153,23 @@ int cp4d_objective(cp4d_ctx *ctx, double *primal, double *cond_dual, double *kkt
  * cp4d_reset.  g: S, out: nz*n*n*Q4 floats, DEVICE.  Needs Q4 <= m (else CP4D_EUNSUPPORTED).  Uses the sinogram temporary and
  * the projector scratch. */
 int cp4d_fbp(cp4d_ctx *ctx, const float *g_dev, float *out_dev);
+
+/* ---- z-slab contexts (cp4d_params.z_open != 0) ---------------- */
+/* Halo arguments are DEVICE pointers to ONE slice [iy][ix][j] (n*n*mp floats, 16-byte aligned) owned by the caller (a
+ * neighbour context's state on this device, or a receive buffer); read-only, never retained.  A halo must be given exactly
+ * for the faces z_open marks interior, else CP4D_EINVAL.  The calls also work on a whole-volume context (both halos null).
+ *   f_above : the neighbour's slice of f (or ft) at z = nz        (forward z-difference of the last slice)
+ *   pz_below: the neighbour's slice of the z-component of p (h2) at z = -1   (backward z-difference of slice 0)      */
+/* change which faces are interior (a pool of contexts that slabs of a taller volume pass through one after the other) */
+int cp4d_set_z_open(cp4d_ctx *ctx, int32_t z_open);
+int cp4d_grad_slab(cp4d_ctx *ctx, const float *f_dev, const float *f_above, float *p_dev);
+int cp4d_div_slab(cp4d_ctx *ctx, const float *p_dev, const float *pz_below, float *f_dev);
+/* Fig. 2 steps 3-4 on the context's state: h1 <- prox_{sigma F1*}(h1 + sigma K1 ft), h2 <- prox_{sigma F2*}(h2 + sigma K2 ft).
+ * ft_above: the upper neighbour's FIRST slice of ft, as it was BEFORE that neighbour's cp4d_step_primal of this iteration. */
+int cp4d_step_dual(cp4d_ctx *ctx, const float *ft_above);
+/* Fig. 2 steps 5-6: f <- f - tau K1^T h1 + tau div h2, ft <- f+ + theta (f+ - f).
+ * h2z_below: the lower neighbour's LAST slice of the z-component of h2, AFTER that neighbour's cp4d_step_dual of this iteration. */
+int cp4d_step_primal(cp4d_ctx *ctx, const float *h2z_below);
 
 /* ---- end-to-end call with HOST buffers (pinned or pageable) ---------------------------------- */
 /* H2D copy of g_host (S), reset to zeros, n_iters iterations with the current steps, D2H copy of f

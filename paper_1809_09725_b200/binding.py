@@ -29,7 +29,7 @@ class Params(C.Structure):
                 ("n_angles", C.c_int32), ("n_half_rot", C.c_int32), ("m", C.c_int32), ("device", C.c_int32),
                 ("phi_host", C.c_void_p), ("lambda1", C.c_float), ("lambda2", C.c_float),
                 ("theta_relax", C.c_float), ("workspace_dev", C.c_void_p), ("workspace_bytes", C.c_uint64),
-                ("stream", C.c_void_p), ("n_frames", C.c_int32)]
+                ("stream", C.c_void_p), ("n_frames", C.c_int32), ("z_open", C.c_int32)]
 
 
 K_COUNT = 11
@@ -62,6 +62,8 @@ def lib():
             "cp4d_state_ptrs": [vp] + [C.POINTER(vp)] * 5,
             "cp4d_solve_host": [vp, vp, i32, vp], "cp4d_sync": [vp],
             "cp4d_objective": [vp] + [C.POINTER(C.c_double)] * 3, "cp4d_fbp": [vp, vp, vp],
+            "cp4d_grad_slab": [vp, vp, vp, vp], "cp4d_div_slab": [vp, vp, vp, vp],
+            "cp4d_step_dual": [vp, vp], "cp4d_step_primal": [vp, vp], "cp4d_set_z_open": [vp, i32],
             "cp4d_launch_count": [vp, C.POINTER(u64)],
             "cp4d_graph_replays": [vp, C.POINTER(u64)],
             "cp4d_profile_begin": [vp], "cp4d_profile_end": [vp, C.POINTER(Profile)],
@@ -79,14 +81,14 @@ def lib():
 
 
 def make_params(n, nz, nd, n_angles, n_half_rot, m, phi=None, lambda1=1e-3, lambda2=1.0, theta=1.0, device=0,
-                workspace_ptr=0, workspace_bytes=0, stream=0, ny=None, n_frames=0):
+                workspace_ptr=0, workspace_bytes=0, stream=0, ny=None, n_frames=0, z_open=0):
     p = Params()
     p.nx, p.ny, p.nz, p.nd = n, (n if ny is None else ny), nz, nd
     p.n_angles, p.n_half_rot, p.m, p.device = n_angles, n_half_rot, m, device
     p.phi_host = None if phi is None else phi.ctypes.data
     p.lambda1, p.lambda2, p.theta_relax = lambda1, lambda2, theta
     p.workspace_dev, p.workspace_bytes, p.stream = workspace_ptr or None, workspace_bytes, stream or None
-    p.n_frames = n_frames
+    p.n_frames, p.z_open = n_frames, z_open
     return p
 
 
@@ -102,11 +104,12 @@ def workspace_bytes(n, nz, nd, n_angles, n_half_rot, m, n_frames=0) -> int:
 class Context:
     """One reconstruction problem on one GPU.  Tensors are torch CUDA float32, contiguous, layouts of cp4d.h."""
 
-    def __init__(self, n, nz, nd, n_angles, n_half_rot, m, phi, lambda1=1e-3, lambda2=1.0, theta=1.0, device=0, n_frames=0):
+    def __init__(self, n, nz, nd, n_angles, n_half_rot, m, phi, lambda1=1e-3, lambda2=1.0, theta=1.0, device=0, n_frames=0,
+                 z_open=0):
         import torch
         self.torch = torch
         self.n, self.nz, self.nd, self.n_angles, self.n_half_rot, self.m = n, nz, nd, n_angles, n_half_rot, m
-        self.n_frames = n_frames
+        self.n_frames, self.z_open = n_frames, z_open
         mp = n_frames or m                                   # length of the primal 4th axis (frames or coefficients)
         self.primal_shape, self.sino_shape = (nz, n, n, mp), (nz, n_angles, nd)
         self.V, self.S = nz * n * n * mp, nz * n_angles * nd
@@ -118,7 +121,7 @@ class Context:
             base = (self.workspace.data_ptr() + 255) // 256 * 256
             self.stream = torch.cuda.current_stream(self.device)
             p = make_params(n, nz, nd, n_angles, n_half_rot, m, self._phi, lambda1, lambda2, theta, device,
-                            base, nbytes, self.stream.cuda_stream, n_frames=n_frames)
+                            base, nbytes, self.stream.cuda_stream, n_frames=n_frames, z_open=z_open)
             h = C.c_void_p()
             r = lib().cp4d_create(C.byref(p), C.byref(h))
         if r:
@@ -173,6 +176,32 @@ class Context:
         out = self.empty_primal() if out is None else out
         self._ck(lib().cp4d_div(self._h, self._t(p, 4 * self.V), self._t(out, self.V)))
         return out
+
+    # -- z-slab contexts (z_open != 0): the neighbour's slice enters as a one-slice tensor or a raw device pointer ----
+    def _halo(self, h):
+        if h is None or isinstance(h, int):
+            return h or None
+        return self._t(h, self.V // self.nz)
+
+    def set_z_open(self, z_open):
+        self._ck(lib().cp4d_set_z_open(self._h, z_open))
+        self.z_open = z_open
+
+    def grad_slab(self, f, f_above=None, out=None):
+        out = self.empty_dual() if out is None else out
+        self._ck(lib().cp4d_grad_slab(self._h, self._t(f, self.V), self._halo(f_above), self._t(out, 4 * self.V)))
+        return out
+
+    def div_slab(self, p, pz_below=None, out=None):
+        out = self.empty_primal() if out is None else out
+        self._ck(lib().cp4d_div_slab(self._h, self._t(p, 4 * self.V), self._halo(pz_below), self._t(out, self.V)))
+        return out
+
+    def step_dual(self, ft_above=None):
+        self._ck(lib().cp4d_step_dual(self._h, self._halo(ft_above)))
+
+    def step_primal(self, h2z_below=None):
+        self._ck(lib().cp4d_step_primal(self._h, self._halo(h2z_below)))
 
     def prox_f1(self, sigma, ft, g, h1):
         self._ck(lib().cp4d_prox_f1(self._h, sigma, self._t(ft, self.V), self._t(g, self.S), self._t(h1, self.S)))

@@ -25,6 +25,7 @@ int validate(const cp4d_params *p, Dims *d) {
     d->n0 = d->na / d->npi; d->m = p->m; d->Q = p->m / 4;
     // frame mode (L214-L237): n_frames frames every n_angles/n_frames angles; the primal 4th axis is the frame index
     if (p->n_frames < 0 || (p->n_frames > 0 && (p->n_frames % 4 || p->n_frames > MAX_M || p->n_angles % p->n_frames))) return CP4D_EINVAL;
+    if (p->z_open < 0 || p->z_open > 3) return CP4D_EINVAL;
     d->nf = p->n_frames; d->mp = d->nf ? d->nf : d->m; d->Qp = d->mp / 4;
     d->mb = p->m;
     // Collapsed frame mode (N_t <= M): K1 o A = sum_q W[k,q] R f(t_q) with W[k,q] = sum_j phi_j(t_k) phi_j(t_q), so the projector
@@ -150,7 +151,7 @@ int cp4d_create(const cp4d_params *p, cp4d_ctx **out) {
 
     cp4d_ctx *ctx = new (std::nothrow) cp4d_ctx();
     if (!ctx) return CP4D_EINVAL;
-    ctx->d = d; ctx->lambda1 = p->lambda1; ctx->lambda2 = p->lambda2; ctx->theta = p->theta_relax;
+    ctx->d = d; ctx->lambda1 = p->lambda1; ctx->lambda2 = p->lambda2; ctx->theta = p->theta_relax; ctx->z_open = p->z_open;
     ctx->tau = ctx->sigma = 0.f; ctx->have_steps = ctx->have_data = false;
     ctx->device = p->device; ctx->stream = (cudaStream_t)p->stream; ctx->launches = 0; ctx->prof_on = false;
     ctx->fwtab_host = nullptr;
@@ -270,6 +271,7 @@ int cp4d_adjoint(cp4d_ctx *ctx, const float *g, float *f) {
 
 int cp4d_grad(cp4d_ctx *ctx, const float *f, float *p) {
     if (!ctx) return CP4D_EINVAL;
+    if (ctx->z_open) return fail(ctx, CP4D_ESTATE, "grad: z-slab context, use the *_slab / cp4d_step_* calls");
     if (bad_ptr(f) || bad_ptr(p) || overlap(f, ctx->d.V * 4, p, ctx->d.V * 16)) return fail(ctx, CP4D_EINVAL, "grad: bad pointers");
     CK(launch_grad(ctx, f, p), "grad");
     return CP4D_OK;
@@ -277,6 +279,7 @@ int cp4d_grad(cp4d_ctx *ctx, const float *f, float *p) {
 
 int cp4d_div(cp4d_ctx *ctx, const float *p, float *f) {
     if (!ctx) return CP4D_EINVAL;
+    if (ctx->z_open) return fail(ctx, CP4D_ESTATE, "div: z-slab context, use the *_slab / cp4d_step_* calls");
     if (bad_ptr(f) || bad_ptr(p) || overlap(f, ctx->d.V * 4, p, ctx->d.V * 16)) return fail(ctx, CP4D_EINVAL, "div: bad pointers");
     CK(launch_div(ctx, p, f), "div");
     return CP4D_OK;
@@ -292,6 +295,7 @@ int cp4d_prox_f1(cp4d_ctx *ctx, float sigma, const float *ft, const float *g, fl
 
 int cp4d_prox_f2(cp4d_ctx *ctx, float sigma, const float *ft, float *h2) {
     if (!ctx) return CP4D_EINVAL;
+    if (ctx->z_open) return fail(ctx, CP4D_ESTATE, "prox_f2: z-slab context, use the *_slab / cp4d_step_* calls");
     if (bad_ptr(ft) || bad_ptr(h2) || overlap(ft, ctx->d.V * 4, h2, ctx->d.V * 16)) return fail(ctx, CP4D_EINVAL, "prox_f2: bad pointers");
     CK(launch_prox_f2(ctx, sigma, ft, h2), "prox_f2");
     return CP4D_OK;
@@ -299,6 +303,7 @@ int cp4d_prox_f2(cp4d_ctx *ctx, float sigma, const float *ft, float *h2) {
 
 int cp4d_primal_update(cp4d_ctx *ctx, float tau, const float *h1, const float *h2, float *f, float *ft) {
     if (!ctx) return CP4D_EINVAL;
+    if (ctx->z_open) return fail(ctx, CP4D_ESTATE, "primal_update: z-slab context, use the *_slab / cp4d_step_* calls");
     const uint64_t Vb = ctx->d.V * 4, Sb = ctx->d.S * 4;
     if (bad_ptr(h1) || bad_ptr(h2) || bad_ptr(f) || bad_ptr(ft) || overlap(f, Vb, ft, Vb) || overlap(f, Vb, h2, 4 * Vb) ||
         overlap(ft, Vb, h2, 4 * Vb) || overlap(h1, Sb, f, Vb) || overlap(h1, Sb, ft, Vb))
@@ -320,6 +325,7 @@ int cp4d_dot(cp4d_ctx *ctx, const float *x, const float *y, uint64_t n, double *
 
 int cp4d_norm(cp4d_ctx *ctx, int32_t n_iters, uint64_t seed, float *L_out) {
     if (!ctx) return CP4D_EINVAL;
+    if (ctx->z_open) return fail(ctx, CP4D_ESTATE, "norm: z-slab context, use the *_slab / cp4d_step_* calls");
     if (!L_out || n_iters < 1) return fail(ctx, CP4D_EINVAL, "norm: bad arguments");
     const Dims &d = ctx->d;
     float *x = ctx->ft, *y1 = ctx->bp, *y2 = ctx->f;
@@ -419,6 +425,7 @@ static bool capture_iteration(cp4d_ctx *ctx) {
 
 int cp4d_iterate(cp4d_ctx *ctx, int32_t n_iters) {
     if (!ctx) return CP4D_EINVAL;
+    if (ctx->z_open) return fail(ctx, CP4D_ESTATE, "iterate: z-slab context, use the *_slab / cp4d_step_* calls");
     if (n_iters < 0) return fail(ctx, CP4D_EINVAL, "iterate: n_iters < 0");
     if (!ctx->have_steps || !ctx->have_data) return fail(ctx, CP4D_ESTATE, "iterate: set_data and set_steps first");
     // the per-kernel timing of cp4d_profile_begin records events between the launches, so it takes the eager path
@@ -432,6 +439,55 @@ int cp4d_iterate(cp4d_ctx *ctx, int32_t n_iters) {
             return r;
         }
     }
+    return CP4D_OK;
+}
+
+// ---- z-slab contexts ----
+static int check_halos(cp4d_ctx *ctx, const void *above, const void *below, bool need_above, bool need_below, const char *what) {
+    if ((need_above && ((ctx->z_open & 2) != 0) != (above != nullptr)) || (need_below && ((ctx->z_open & 1) != 0) != (below != nullptr)) ||
+        (above && bad_ptr(above)) || (below && bad_ptr(below)))
+        return fail(ctx, CP4D_EINVAL, what);
+    return CP4D_OK;
+}
+
+int cp4d_set_z_open(cp4d_ctx *ctx, int32_t z_open) {
+    if (!ctx) return CP4D_EINVAL;
+    if (z_open < 0 || z_open > 3) return fail(ctx, CP4D_EINVAL, "set_z_open: flags are 0..3");
+    ctx->z_open = z_open;
+    return CP4D_OK;
+}
+
+int cp4d_grad_slab(cp4d_ctx *ctx, const float *f, const float *f_above, float *p) {
+    if (!ctx) return CP4D_EINVAL;
+    if (bad_ptr(f) || bad_ptr(p) || overlap(f, ctx->d.V * 4, p, ctx->d.V * 16)) return fail(ctx, CP4D_EINVAL, "grad_slab: bad pointers");
+    if (int r = check_halos(ctx, f_above, nullptr, true, false, "grad_slab: a halo slice is needed exactly on an interior face")) return r;
+    CK(launch_grad(ctx, f, p, f_above), "grad");
+    return CP4D_OK;
+}
+
+int cp4d_div_slab(cp4d_ctx *ctx, const float *p, const float *pz_below, float *f) {
+    if (!ctx) return CP4D_EINVAL;
+    if (bad_ptr(f) || bad_ptr(p) || overlap(f, ctx->d.V * 4, p, ctx->d.V * 16)) return fail(ctx, CP4D_EINVAL, "div_slab: bad pointers");
+    if (int r = check_halos(ctx, nullptr, pz_below, false, true, "div_slab: a halo slice is needed exactly on an interior face")) return r;
+    CK(launch_div(ctx, p, f, pz_below), "div");
+    return CP4D_OK;
+}
+
+int cp4d_step_dual(cp4d_ctx *ctx, const float *ft_above) {
+    if (!ctx) return CP4D_EINVAL;
+    if (!ctx->have_steps || !ctx->have_data) return fail(ctx, CP4D_ESTATE, "step_dual: set_data and set_steps first");
+    if (int r = check_halos(ctx, ft_above, nullptr, true, false, "step_dual: a halo slice is needed exactly on an interior face")) return r;
+    if (int r = forward_into(ctx, ctx->ft, 1, ctx->sigma, ctx->g, ctx->h1)) return r;
+    CK(launch_prox_f2(ctx, ctx->sigma, ctx->ft, ctx->h2, ft_above), "prox_f2");
+    return CP4D_OK;
+}
+
+int cp4d_step_primal(cp4d_ctx *ctx, const float *h2z_below) {
+    if (!ctx) return CP4D_EINVAL;
+    if (!ctx->have_steps || !ctx->have_data) return fail(ctx, CP4D_ESTATE, "step_primal: set_data and set_steps first");
+    if (int r = check_halos(ctx, nullptr, h2z_below, false, true, "step_primal: a halo slice is needed exactly on an interior face")) return r;
+    if (int r = adjoint_into(ctx, ctx->h1, ctx->bp)) return r;
+    CK(launch_update(ctx, ctx->tau, ctx->bp, ctx->h2, ctx->f, ctx->ft, h2z_below), "update");
     return CP4D_OK;
 }
 
@@ -454,6 +510,7 @@ int cp4d_state_ptrs(cp4d_ctx *ctx, float **f, float **ft, float **h1, float **h2
 
 int cp4d_solve_host(cp4d_ctx *ctx, const float *g_host, int32_t n_iters, float *f_host) {
     if (!ctx) return CP4D_EINVAL;
+    if (ctx->z_open) return fail(ctx, CP4D_ESTATE, "solve_host: z-slab context, use the *_slab / cp4d_step_* calls");
     if (!g_host || !f_host || n_iters < 0) return fail(ctx, CP4D_EINVAL, "solve_host: bad arguments");
     if (!ctx->have_steps) return fail(ctx, CP4D_ESTATE, "solve_host: set_steps first");
     CK(cudaMemcpyAsync(ctx->g, g_host, ctx->d.S * 4, cudaMemcpyHostToDevice, ctx->stream), "solve_host h2d");
@@ -467,6 +524,7 @@ int cp4d_solve_host(cp4d_ctx *ctx, const float *g_host, int32_t n_iters, float *
 
 int cp4d_objective(cp4d_ctx *ctx, double *primal, double *cond_dual, double *kkt_resid) {
     if (!ctx) return CP4D_EINVAL;
+    if (ctx->z_open) return fail(ctx, CP4D_ESTATE, "objective: z-slab context, use the *_slab / cp4d_step_* calls");
     if (!ctx->have_data) return fail(ctx, CP4D_ESTATE, "objective: set_data first");
     const Dims &d = ctx->d;
     double v[5] = {0, 0, 0, 0, 0};

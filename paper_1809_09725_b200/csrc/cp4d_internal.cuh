@@ -59,6 +59,7 @@ struct Dims {
 struct cp4d_ctx {
     cp4d::Dims d;
     float lambda1, lambda2, theta;
+    int z_open;                  // cp4d_params.z_open: bit 0 lower face interior, bit 1 upper face interior (z-slab of a taller volume)
     float tau, sigma;
     bool have_steps, have_data;
     int device;
@@ -117,10 +118,11 @@ struct ProfScope {
 };
 
 // launchers (each enqueues on ctx->stream and bumps ctx->launches); return cudaError_t
-cudaError_t launch_grad(cp4d_ctx *c, const float *f, float *p);
-cudaError_t launch_div(cp4d_ctx *c, const float *p, float *f);
-cudaError_t launch_prox_f2(cp4d_ctx *c, float sigma, const float *ft, float *h2);
-cudaError_t launch_update(cp4d_ctx *c, float tau, const float *bp, const float *h2, float *f, float *ft);
+// halo: the neighbour slab's slice (grad / prox: f at z = nz; div / update: p_z at z = -1), null on a closed face
+cudaError_t launch_grad(cp4d_ctx *c, const float *f, float *p, const float *halo = nullptr);
+cudaError_t launch_div(cp4d_ctx *c, const float *p, float *f, const float *halo = nullptr);
+cudaError_t launch_prox_f2(cp4d_ctx *c, float sigma, const float *ft, float *h2, const float *halo = nullptr);
+cudaError_t launch_update(cp4d_ctx *c, float tau, const float *bp, const float *h2, float *f, float *ft, const float *halo = nullptr);
 cudaError_t launch_fold(cp4d_ctx *c, const float *g, float4 *gt);
 // synth: out = K1 f from partial sums P.  mode 0: g_out = v ; mode 1: h1 = (h1 + sigma (v - g))/(1+sigma)
 cudaError_t launch_synth(cp4d_ctx *c, const float4 *P, int mode, float sigma, const float *g, float *out);

@@ -32,6 +32,11 @@ struct StreamArgs {
     int n, nz, Q, zper;
     int64_t slice4, V4;
     float lambda2;
+    // z-slab contexts (cp4d_params.z_open): one read-only halo slice from the neighbour.
+    //   k_grad: the slice of f above the slab (z = nz), so the z-difference of the last slice is not the boundary's 0;
+    //   k_div:  the slice of p_z below the slab (z = -1); with hi_open the last slice's p_z is interior, not the boundary's 0
+    const float4 *halo;
+    int hi_open;
 };
 
 // ---------------------------------------------------------------------------------------------------
@@ -57,7 +62,7 @@ __global__ void __launch_bounds__(256) k_grad(const float *__restrict__ f, float
     float4 cur = ld4(F + (int64_t)z0 * a.slice4 + e4);
     for (int z = z0; z < z1; ++z) {
         const int64_t idx = (int64_t)z * a.slice4 + e4;
-        const float4 fz = (z + 1 < a.nz) ? ld4(F + idx + a.slice4) : cur;
+        const float4 fz = (z + 1 < a.nz) ? ld4(F + idx + a.slice4) : (a.halo ? ld4(a.halo + e4) : cur);
         const float4 fx = hx ? ld4(F + idx + a.Q) : cur;
         const float4 fy = hy ? ld4(F + idx + sy) : cur;
         const float ft = ht ? __ldg(f + (idx + 1) * 4) : cur.w;
@@ -117,14 +122,14 @@ __global__ void __launch_bounds__(256) k_div(const float *__restrict__ p, float 
     const float *pt_s = p + 3 * a.V4 * 4;
     const int64_t sy = (int64_t)a.n * a.Q;
     const float4 zero = make_float4(0.f, 0.f, 0.f, 0.f);
-    float4 prevz = (z0 > 0) ? ld4(PZ + (int64_t)(z0 - 1) * a.slice4 + e4) : zero;
+    float4 prevz = (z0 > 0) ? ld4(PZ + (int64_t)(z0 - 1) * a.slice4 + e4) : (a.halo ? ld4(a.halo + e4) : zero);
     for (int z = z0; z < z1; ++z) {
         const int64_t idx = (int64_t)z * a.slice4 + e4;
         const float4 xc = (x < a.n - 1) ? ld4(PX + idx) : zero;
         const float4 xm = (x > 0) ? ld4(PX + idx - a.Q) : zero;
         const float4 yc = (y < a.n - 1) ? ld4(PY + idx) : zero;
         const float4 ym = (y > 0) ? ld4(PY + idx - sy) : zero;
-        const float4 zc = (z < a.nz - 1) ? ld4(PZ + idx) : zero;
+        const float4 zc = (z < a.nz - 1 || a.hi_open) ? ld4(PZ + idx) : zero;
         const float4 tc = ld4(PT + idx);
         const float tm = (c > 0) ? __ldg(pt_s + idx * 4 - 1) : 0.0f;
         const float tw = (c < a.Q - 1) ? tc.w : 0.0f;
@@ -156,10 +161,11 @@ __global__ void __launch_bounds__(256) k_div(const float *__restrict__ p, float 
     if (MODE == 2) block_add(kk, red);
 }
 
-static StreamArgs make_args(const cp4d_ctx *c, dim3 &grid, dim3 &block) {
+static StreamArgs make_args(const cp4d_ctx *c, dim3 &grid, dim3 &block, const float *halo = nullptr) {
     const Dims &d = c->d;
     StreamArgs a;
     a.n = d.n; a.nz = d.nz; a.Q = d.Qp; a.slice4 = d.slice4; a.V4 = d.V / 4; a.lambda2 = c->lambda2;
+    a.halo = reinterpret_cast<const float4 *>(halo); a.hi_open = (c->z_open & 2) ? 1 : 0;
     block = dim3(256);
     const int64_t bx = (d.slice4 + 255) / 256;
     // enough CTAs to fill 148 SMs x 8 resident CTAs a few times over; otherwise split z
@@ -171,35 +177,35 @@ static StreamArgs make_args(const cp4d_ctx *c, dim3 &grid, dim3 &block) {
     return a;
 }
 
-cudaError_t launch_grad(cp4d_ctx *c, const float *f, float *p) {
+cudaError_t launch_grad(cp4d_ctx *c, const float *f, float *p, const float *halo) {
     ProfScope ps(c, CP4D_K_GRAD);
     dim3 g, b;
-    StreamArgs a = make_args(c, g, b);
+    StreamArgs a = make_args(c, g, b, halo);
     k_grad<0><<<g, b, 0, c->stream>>>(f, p, a, 0.f, 0.f, 0, nullptr);
     c->launches++;
     return cudaGetLastError();
 }
-cudaError_t launch_prox_f2(cp4d_ctx *c, float sigma, const float *ft, float *h2) {
+cudaError_t launch_prox_f2(cp4d_ctx *c, float sigma, const float *ft, float *h2, const float *halo) {
     ProfScope ps(c, CP4D_K_PROX_F2);
     dim3 g, b;
-    StreamArgs a = make_args(c, g, b);
+    StreamArgs a = make_args(c, g, b, halo);
     const int l1z = !(c->lambda1 > 0.f);
     k_grad<1><<<g, b, 0, c->stream>>>(ft, h2, a, sigma, l1z ? 0.f : 1.0f / c->lambda1, l1z, nullptr);
     c->launches++;
     return cudaGetLastError();
 }
-cudaError_t launch_div(cp4d_ctx *c, const float *p, float *f) {
+cudaError_t launch_div(cp4d_ctx *c, const float *p, float *f, const float *halo) {
     ProfScope ps(c, CP4D_K_DIV);
     dim3 g, b;
-    StreamArgs a = make_args(c, g, b);
+    StreamArgs a = make_args(c, g, b, halo);
     k_div<0><<<g, b, 0, c->stream>>>(p, f, a, nullptr, nullptr, 0.f, 0.f, nullptr);
     c->launches++;
     return cudaGetLastError();
 }
-cudaError_t launch_update(cp4d_ctx *c, float tau, const float *bp, const float *h2, float *f, float *ft) {
+cudaError_t launch_update(cp4d_ctx *c, float tau, const float *bp, const float *h2, float *f, float *ft, const float *halo) {
     ProfScope ps(c, CP4D_K_UPDATE);
     dim3 g, b;
-    StreamArgs a = make_args(c, g, b);
+    StreamArgs a = make_args(c, g, b, halo);
     k_div<1><<<g, b, 0, c->stream>>>(h2, f, a, bp, ft, tau, c->theta, nullptr);
     c->launches++;
     return cudaGetLastError();
