@@ -323,6 +323,33 @@ def run_cp4d(args, c, rank, world):
                      L=L, launches_total=ctx.launch_count() - launches0, graph_replays=graph_replays)
 
 
+def run_streamed(args, c, L):
+    """Out-of-core variant: the CP state stays in pinned host memory and passes through the
+    GPU slab by slab every iteration, copies on their own streams.  Wall-clock over K iterations after one warm-up sweep."""
+    import torch
+    from paper_1809_09725_b200 import slabs, synth
+    phi = synth.basis_table(c.basis, c.m, c.n_angles)
+    T = slabs.StreamedSolver(c.n, c.nz, c.nd, c.n_angles, c.n_half_rot, c.m, phi, slab_nz=args.streamed, n_frames=args.frames,
+                             lambda1=c.lambda1, lambda2=c.lambda2)
+    T.set_data(synth.sinogram(c).to(torch.float32))
+    T.set_steps(0.95 / L, 0.95 / L)
+    T.reset()
+    T.iterate(max(1, min(args.warmup, 2)))
+    torch.cuda.synchronize()
+    K = max(2, args.steps // 5)
+    b0, d0 = T.bytes_h2d, T.bytes_d2h
+    t0 = time.perf_counter()
+    T.iterate(K)
+    torch.cuda.synchronize()
+    dt = time.perf_counter() - t0
+    h2d, d2h = (T.bytes_h2d - b0) / K, (T.bytes_d2h - d0) / K
+    out = {"value": K / dt, "unit": UNIT, "steps": K, "slab_nz": args.streamed, "slabs": T.n_slabs, "device_contexts": T.depth,
+           "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "h2d_gbs": h2d * K / dt / 1e9, "d2h_gbs": d2h * K / dt / 1e9,
+           "note": "state (f, ft, h2, h1, g) in pinned host memory; every iteration streams it through the GPU once"}
+    T.close()
+    return out
+
+
 def assemble(args, c, world, r):
     from paper_1809_09725_b200 import synth
     peaks, K = r["peaks"], args.steps
@@ -389,6 +416,8 @@ def main():
     ap.add_argument("--impl", default="cp4d", choices=["cp4d", "reference"])
     ap.add_argument("--power-iters", type=int, default=30, help="power-iteration steps for ||K|| (DESIGN.md R8: 30)")
     ap.add_argument("--frames", type=int, default=0, help="N_t > 0: the paper's frame discretisation (cp4d_params.n_frames), e.g. 8")
+    ap.add_argument("--streamed", type=int, default=0, metavar="SLAB_NZ",
+                    help="also time the out-of-core path (slabs.StreamedSolver: state in pinned host memory, slabs of SLAB_NZ slices)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
@@ -402,8 +431,11 @@ def main():
         print(f"bench.py: warning: --warmup {args.warmup} < 3 (timing rules want >= 3)", file=sys.stderr)
     ctx, r = run_cp4d(args, c, rank, world)
     ctx.close()
+    streamed = run_streamed(args, c, r["L"]) if (args.streamed and world == 1) else None
     if rank == 0:
         line = assemble(args, c, world, r)
+        if streamed:
+            line["streamed"] = streamed
         if not args.no_cpu_baseline and world == 1:
             val, cores, sample, dt = oracle_steps(c, 1, 0, target_fma=1.2e11, n_frames=args.frames)   # about 10 s of oracle work on 16 cores
             line["cpu_baseline"] = {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample,
