@@ -379,6 +379,17 @@ def assemble(args, c, world, r):
                 "frac": d["frac"], "traffic": None, "peak_source": peaks["source"], "avg_launch_ms": d["ms"],
                 "note": ("alu peak = 148 SM x 128 FP32 lanes x 2 flop x sm_max_mhz; achieved = algorithmic (pi-folded) flops"
                          if d["bound"] == "alu" else "algorithmic bytes / CUDA-event time")}
+    # the projectors fetch one fp32 operand from shared memory per FMA at best: their second, tighter roof is the
+    # shared-memory bandwidth, 128 B/clk/SM (measured: profiles/r1_microbench_fma_lds.md).  Algorithmic bytes = 4 B per FMA for the
+    # forward gather; the backprojector reuses fetched bins from registers, so this roof only binds the forward kernel.
+    if "forward" in kernels:
+        k = kernels["forward"]
+        smem_peak = N_SM * 128 * peaks["sm_max_mhz"] * 1e6 / 1e9                       # GB/s
+        smem_ach = (work["forward"][1] / 2.0) * 4.0 / (k["ms"] * 1e-3) / 1e9           # flop / 2 = FMAs; 4 B each
+        k["smem_roof"] = {"bound": "smem", "achieved": smem_ach, "peak": smem_peak, "unit": "GB/s", "frac": smem_ach / smem_peak,
+                          "note": "one 4-byte operand per FMA through shared memory: 148 SM x 128 B/clk x sm_max_mhz"}
+        if dom == "forward":
+            roofline["smem_roof"] = k["smem_roof"]
     tr = ROOT / "profiles" / "traffic.json"                  # dram bytes per launch from the committed ncu --set full capture
     if tr.exists():
         try:
