@@ -330,13 +330,13 @@ def run_streamed(args, c, L):
     from paper_1809_09725_b200 import slabs, synth
     phi = synth.basis_table(c.basis, c.m, c.n_angles)
     T = slabs.StreamedSolver(c.n, c.nz, c.nd, c.n_angles, c.n_half_rot, c.m, phi, slab_nz=args.streamed, n_frames=args.frames,
-                             lambda1=c.lambda1, lambda2=c.lambda2)
+                             block=args.stream_block, lambda1=c.lambda1, lambda2=c.lambda2)
     T.set_data(synth.sinogram(c).to(torch.float32))
     T.set_steps(0.95 / L, 0.95 / L)
     T.reset()
-    T.iterate(max(1, min(args.warmup, 2)))
+    T.iterate(max(1, min(args.warmup, 2)) * args.stream_block)
     torch.cuda.synchronize()
-    K = max(2, args.steps // 5)
+    K = max(2, args.steps // 5) * args.stream_block
     b0, d0 = T.bytes_h2d, T.bytes_d2h
     t0 = time.perf_counter()
     T.iterate(K)
@@ -344,6 +344,7 @@ def run_streamed(args, c, L):
     dt = time.perf_counter() - t0
     h2d, d2h = (T.bytes_h2d - b0) / K, (T.bytes_d2h - d0) / K
     out = {"value": K / dt, "unit": UNIT, "steps": K, "slab_nz": args.streamed, "slabs": T.n_slabs, "device_contexts": T.depth,
+           "block": args.stream_block, "window_nz": T.win_nz if args.stream_block > 1 else args.streamed,
            "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "h2d_gbs": h2d * K / dt / 1e9, "d2h_gbs": d2h * K / dt / 1e9,
            "note": "state (f, ft, h2, h1, g) in pinned host memory; every iteration streams it through the GPU once"}
     T.close()
@@ -429,6 +430,8 @@ def main():
     ap.add_argument("--frames", type=int, default=0, help="N_t > 0: the paper's frame discretisation (cp4d_params.n_frames), e.g. 8")
     ap.add_argument("--streamed", type=int, default=0, metavar="SLAB_NZ",
                     help="also time the out-of-core path (slabs.StreamedSolver: state in pinned host memory, slabs of SLAB_NZ slices)")
+    ap.add_argument("--stream-block", type=int, default=1, metavar="K",
+                    help="with --streamed: temporal blocking, K iterations per residency of a window of SLAB_NZ + 2K slices")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()

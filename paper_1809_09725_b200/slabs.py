@@ -145,12 +145,18 @@ class StreamedSolver:
     Device: `depth` slab contexts (default 2) used round-robin; copies in on `s_in`, kernels on each context's stream,
     copies out on `s_out`, ordered by events, so the upload of slab s+1 and the download of slab s-1 overlap the kernels of
     slab s.  All slabs but the last have the same height, so at most two distinct context shapes are needed per pool slot.
+
+    block = k > 1 (temporal blocking): a window of slab_nz + 2k slices is uploaded, iterated k times as a closed volume and
+    only its core of slab_nz slices is written back (to a second host copy, since the neighbours still need iterate n): k times
+    less PCIe traffic per iteration for (slab_nz + 2k) / slab_nz more kernel work.  See `windows`.
     """
 
-    def __init__(self, n, nz, nd, n_angles, n_half_rot, m, phi, slab_nz, device=0, depth=2, n_frames=0, **kw):
+    def __init__(self, n, nz, nd, n_angles, n_half_rot, m, phi, slab_nz, device=0, depth=2, n_frames=0, block=1, **kw):
         import torch
         self.torch = torch
         self.dev = torch.device("cuda", device)
+        self.block, self.slab_nz = max(1, int(block)), slab_nz
+        self.win_nz = min(nz, slab_nz + 2 * self.block)      # temporal blocking: slices per device window
         self.n, self.nz, self.nd, self.na = n, nz, nd, n_angles
         self.mp = n_frames or m
         n_slabs = (nz + slab_nz - 1) // slab_nz
@@ -164,10 +170,13 @@ class StreamedSolver:
         self.f, self.ft = pin(nz, n, n, self.mp), pin(nz, n, n, self.mp)
         self.h2 = pin(4, nz, n, n, self.mp)
         self.h1, self.g = pin(nz, n_angles, nd), pin(nz, n_angles, nd)
+        # temporal blocking reads iterate n and writes iterate n + block: a second host copy of the state
+        self._nxt = dict(f=pin(nz, n, n, self.mp), ft=pin(nz, n, n, self.mp), h2=pin(4, nz, n, n, self.mp),
+                         h1=pin(nz, n_angles, nd)) if self.block > 1 else None
         dev_buf = lambda *shape: torch.empty(shape, dtype=torch.float32, device=self.dev)
         self.halo_ft = [dev_buf(n, n, self.mp) for _ in range(self.depth)]
         self.halo_h2z = [dev_buf(n, n, self.mp) for _ in range(2)]
-        self.g_stage = [dev_buf(slab_nz, n_angles, nd) for _ in range(self.depth)]
+        self.g_stage = [dev_buf(self.win_nz if self.block > 1 else slab_nz, n_angles, nd) for _ in range(self.depth)]
         self.tau = self.sigma = None
         self.bytes_h2d = self.bytes_d2h = 0
 
@@ -208,10 +217,75 @@ class StreamedSolver:
             self.f.copy_(self.torch.as_tensor(f0, dtype=self.torch.float32))
             self.ft.copy_(self.f)
 
+    def windows(self):
+        """Temporal blocking: per slab the device window (w0, w1) of win_nz slices and its core (z0, z1).  After k <= block
+        iterations of the CLOSED window the wrong boundary condition at an interior window end has spoiled k slices next to it
+        (one per iteration: the dual step needs ft[z+1], the primal step h2_z[z-1]); the core keeps at least `block` slices of
+        distance from every interior end, a window end at the volume's own boundary is exact."""
+        out = []
+        for z0, z1 in self.ranges:
+            w0 = max(0, min(z0 - self.block, self.nz - self.win_nz))
+            out.append((w0, w0 + self.win_nz, z0, z1))
+        return out
+
+    def _iterate_blocked(self, k):
+        """k <= block iterations for the whole volume: every slab's window goes up from the current host copy, runs
+        cp4d_iterate(k) (a CUDA-graph replay) as an ordinary closed volume, and its core comes down into the other host copy."""
+        torch = self.torch
+        Event = torch.cuda.Event
+        cur = dict(f=self.f, ft=self.ft, h2=self.h2, h1=self.h1)
+        nxt = self._nxt
+        slot_free = [None] * self.depth
+        for i, (w0, w1, z0, z1) in enumerate(self.windows()):
+            slot = i % self.depth
+            key = (slot, w1 - w0)
+            if key not in self._ctx:
+                self._ctx[key] = self._mk(w1 - w0, self.s_cmp[slot])
+                self._ctx[key].set_steps(self.tau, self.sigma)
+            c = self._ctx[key]
+            st, cs = c.state(), self.s_cmp[slot]
+            with torch.cuda.stream(self.s_in):
+                if slot_free[slot] is not None:
+                    self.s_in.wait_event(slot_free[slot])
+                st["f"].copy_(cur["f"][w0:w1], non_blocking=True)
+                st["ft"].copy_(cur["ft"][w0:w1], non_blocking=True)
+                for a in range(4):
+                    st["h2"][a].copy_(cur["h2"][a, w0:w1], non_blocking=True)
+                st["h1"].copy_(cur["h1"][w0:w1], non_blocking=True)
+                self.g_stage[slot][:w1 - w0].copy_(self.g[w0:w1], non_blocking=True)
+                up = Event(); up.record(self.s_in)
+            self.bytes_h2d += (w1 - w0) * (6 * self.n * self.n * self.mp + 2 * self.na * self.nd) * 4
+            with torch.cuda.stream(cs):
+                cs.wait_event(up)
+                c.set_data(self.g_stage[slot][:w1 - w0])
+                c.iterate(k)
+                done = Event(); done.record(cs)
+            a0, a1 = z0 - w0, z1 - w0
+            with torch.cuda.stream(self.s_out):
+                self.s_out.wait_event(done)
+                nxt["f"][z0:z1].copy_(st["f"][a0:a1], non_blocking=True)
+                nxt["ft"][z0:z1].copy_(st["ft"][a0:a1], non_blocking=True)
+                for a in range(4):
+                    nxt["h2"][a, z0:z1].copy_(st["h2"][a, a0:a1], non_blocking=True)
+                nxt["h1"][z0:z1].copy_(st["h1"][a0:a1], non_blocking=True)
+                fr = Event(); fr.record(self.s_out)
+                slot_free[slot] = fr
+            self.bytes_d2h += (z1 - z0) * (6 * self.n * self.n * self.mp + self.na * self.nd) * 4
+        self.s_out.synchronize()
+        self._nxt = cur
+        self.f, self.ft, self.h2, self.h1 = nxt["f"], nxt["ft"], nxt["h2"], nxt["h1"]
+
     def iterate(self, n_iters):
         torch = self.torch
         if self.tau is None:
             raise binding.Cp4dError(binding.ESTATE, "set_steps first")
+        if self.block > 1:
+            left = n_iters
+            while left > 0:
+                k = min(self.block, left)
+                self._iterate_blocked(k)
+                left -= k
+            return
         Event = torch.cuda.Event
         slot_free = [None] * self.depth                  # event: the slot's previous download has finished
         for _ in range(n_iters):

@@ -104,6 +104,30 @@ def test_streamed_solver_matches_in_core(torch_cuda, slab_nz, depth):
     T.close(); whole.close()
 
 
+@pytest.mark.parametrize("slab_nz,block,iters", [(2, 2, 9), (3, 4, 8), (1, 3, 7)])
+def test_streamed_solver_temporal_blocking(torch_cuda, slab_nz, block, iters):
+    """block = k: windows of slab_nz + 2k slices iterated k times as closed volumes, cores written to the second host copy."""
+    from paper_1809_09725_b200 import binding, slabs
+    torch = torch_cuda
+    c = CASE
+    phi = synth.basis_table(c.basis, c.m, c.n_angles)
+    g = synth.sinogram(c).numpy().astype(np.float32)
+    whole = binding.Context.from_config(c, phi=phi)
+    whole.set_data(dev(torch, g)); whole.set_steps(0.012, 0.011); whole.reset(); whole.iterate(iters); whole.sync()
+    sw = whole.state()
+    T = slabs.StreamedSolver(c.n, c.nz, c.nd, c.n_angles, c.n_half_rot, c.m, phi, slab_nz=slab_nz, depth=2, block=block,
+                             lambda1=c.lambda1, lambda2=c.lambda2)
+    T.set_data(g); T.set_steps(0.012, 0.011); T.reset(); T.iterate(iters)       # iters is not a multiple of block: a short last sweep
+    T.get_f()
+    for k, v in (("f", T.f), ("ft", T.ft), ("h2", T.h2), ("h1", T.h1)):
+        assert rel(v.numpy(), sw[k].cpu().numpy()) <= 1e-5, k
+    sweeps = -(-iters // block)
+    n_sl = (c.nz + slab_nz - 1) // slab_nz
+    assert T.bytes_h2d == sweeps * n_sl * T.win_nz * (6 * c.n * c.n * c.m + 2 * c.n_angles * c.nd) * 4
+    assert sum(x.graph_replays() for x in T._ctx.values()) > 0                   # the windows run cp4d_iterate's graph path
+    T.close(); whole.close()
+
+
 def test_slab_context_call_rules(torch_cuda):
     from paper_1809_09725_b200 import binding
     torch = torch_cuda

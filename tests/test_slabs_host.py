@@ -131,3 +131,38 @@ def test_halo_protocol_gloo_world2_matches_whole_volume_oracle(oracle):
     assert np.abs(h2 - st["h2"]).max() <= 1e-12 * np.abs(st["h2"]).max()
     # and the z-coupling is really exercised: without the halos the slabs give a different answer
     assert np.abs(st["h2"][2, res[0][2] - 1]).max() > 0
+
+
+def test_temporal_blocking_windows_keep_the_core_exact(oracle):
+    """The claim slabs.StreamedSolver.windows rests on: k iterations of a CLOSED window of slices spoil exactly k slices next to
+    each interior window end, so a core at distance >= k is the whole-volume iterate.  Checked with the oracle: every slab's window
+    iterated on its own equals the whole-volume run on its core, and the slice just outside the safe distance does not."""
+    from paper_1809_09725_b200 import slabs, synth
+    c = synth.CONFIGS[1].scaled(cfg=32, n=10, nd=12, nz=11, n_angles=8, n_half_rot=2, m=4, lambda1=0.02, lambda2=0.8)
+    phi = synth.basis_table(c.basis, c.m, c.n_angles)
+    g = synth.rng(c.cfg, 2).standard_normal((c.nz, c.n_angles, c.nd))
+    k = 3
+    P = oracle.Problem.from_config(c, phi=phi)
+    whole = P.zero_state()
+    P.cp(g, whole, 0.03, 0.04, 2, folded=True)          # a non-trivial starting iterate n
+    start = {a: v.copy() for a, v in whole.items()}
+    assert 0 < P.cp(g, whole, 0.03, 0.04, k, folded=True) < P.V
+
+    class Geo:                                          # the window arithmetic of StreamedSolver without a device
+        block, nz, slab_nz = k, c.nz, 2
+    Geo.win_nz = min(c.nz, Geo.slab_nz + 2 * k)
+    Geo.ranges = [(i * 2, min(c.nz, i * 2 + 2)) for i in range((c.nz + 1) // 2)]
+    wins = slabs.StreamedSolver.windows(Geo)
+    assert [w[2:] for w in wins] == Geo.ranges and all(w1 - w0 == Geo.win_nz for w0, w1, _, _ in wins)
+    spoiled = 0
+    for w0, w1, z0, z1 in wins:
+        assert (w0 == 0 or z0 - w0 >= k) and (w1 == c.nz or w1 - z1 >= k)
+        Pw = oracle.Problem.from_config(c.scaled(nz=w1 - w0), phi=phi)
+        st = {a: np.array(v[:, w0:w1] if a == "h2" else v[w0:w1], order="C") for a, v in start.items()}   # copies: cp works in place
+        Pw.cp(g[w0:w1], st, 0.03, 0.04, k, folded=True)
+        for a in ("f", "ft", "h1"):
+            assert np.array_equal(st[a][z0 - w0:z1 - w0], whole[a][z0:z1]), a
+        assert np.array_equal(st["h2"][:, z0 - w0:z1 - w0], whole["h2"][:, z0:z1])
+        if w0 > 0:                                      # one slice closer than k to the interior end is already wrong
+            spoiled += not np.array_equal(st["f"][k - 1], whole["f"][w0 + k - 1])
+    assert spoiled > 0
