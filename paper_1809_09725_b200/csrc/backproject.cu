@@ -8,12 +8,13 @@
 //
 // Static register indexing.  With u = bin coordinate of a voxel, the patch's smallest coordinate is umin = K + phi
 // (K integer, 0 <= phi < 1, both per thread) and voxel v sits at umin + delta_v where delta_v = e*|c| + dy*s is the
-// same for every thread at this angle.  Choose an integer FL_v with 0 <= delta_v - FL_v <= 1 (the host picks one of 9
+// same for every thread at this angle.  Choose an integer FL_v with 0 <= delta_v - FL_v <= 1 (the host picks one of
 // 7 covering 8-tuples, the "pattern" of the angle); then t = phi + delta_v - FL_v is in [0,2) and the voxel touches only
 // bins K+FL_v+{0,1,2}, with Joseph hat weights max(0, 1/a - |t-k|/a^2) (one of the three is zero).  A warp-uniform
 // switch on the pattern selects straight-line code in which every register index is a compile-time constant.
 // For c < 0 the patch is traversed mirrored in x (e = 3-dx): the staged chunks never mix the signs of c, and the accumulators
 // are mirrored once, between the last chunk with c >= 0 and the first with c < 0.
+#include <algorithm>
 #include <cmath>
 
 #include "cp4d_internal.cuh"
@@ -118,6 +119,8 @@ __device__ __forceinline__ void bp_angle(float4 (&acc)[8][JQ], const float4 *wba
 
 struct BpArgs {
     int n, nz, nd, n0, Q, gp, gpl, n_pos;   // n_pos: the first n_pos base angles have c >= 0, the others c < 0
+    int tiles, agroups;                     // blockIdx.x = tile + tiles * angle group (small grids split the base angles over CTAs,
+                                            // which then ADD their partial sums to a zeroed output)
     const AngleTab *ang;
     const TileGeo *geo;
 };
@@ -136,18 +139,22 @@ __global__ void __launch_bounds__(BP_THREADS, 4) k_backproject(const float4 *__r
     __shared__ BpAngle sang[2][BP_CHUNK];
     __shared__ __align__(8) uint64_t mbar[2];
     const int tiles_1d = (a.n + TILE - 1) / TILE;
-    const int tix = blockIdx.x % tiles_1d, tiy = blockIdx.x / tiles_1d;
+    const int tile_id = blockIdx.x % a.tiles, ag = blockIdx.x / a.tiles;
+    const int tix = tile_id % tiles_1d, tiy = tile_id / tiles_1d;
     const int z = blockIdx.y, jg = blockIdx.z;
     // lane -> patch: a quarter warp (the unit an LDS.128 is served in) covers 2 (x) x 4 (y) patches; their window starts
     // differ by at most 4|c| + 6 s <= 7.2 < 8 slots of 16 B, so the 8 lanes never collide on a bank
     const int l = threadIdx.x & 31, w = threadIdx.x >> 5;
     const int pxi = (l & 1) | ((l >> 2) & 6), pyi = ((l >> 1) & 3) | (w << 2);
     const float fx0 = (float)(4 * pxi), fy0 = (float)(2 * pyi);
-    const TileGeo *geo = a.geo + (int64_t)blockIdx.x * a.n0;
+    const TileGeo *geo = a.geo + (int64_t)tile_id * a.n0;
     // chunks never mix the signs of c: chunks of the angles with c >= 0 first, then of those with c < 0
-    const int nchA = (a.n_pos + BP_CHUNK - 1) / BP_CHUNK, nch = nchA + (a.n0 - a.n_pos + BP_CHUNK - 1) / BP_CHUNK;
-    auto chunk_begin = [&](int ch) { return ch < nchA ? ch * BP_CHUNK : a.n_pos + (ch - nchA) * BP_CHUNK; };
-    auto chunk_count = [&](int ch) { return min(BP_CHUNK, (ch < nchA ? a.n_pos : a.n0) - chunk_begin(ch)); };
+    // this CTA's share [g0, g1) of the base angles, as its part [p0, p1) of those with c >= 0 and [q0, q1) of those with c < 0
+    const int g0 = (int)((int64_t)a.n0 * ag / a.agroups), g1 = (int)((int64_t)a.n0 * (ag + 1) / a.agroups);
+    const int p0 = min(g0, a.n_pos), p1 = min(g1, a.n_pos), q0 = max(g0, a.n_pos), q1 = max(g1, a.n_pos);
+    const int nchA = (p1 - p0 + BP_CHUNK - 1) / BP_CHUNK, nch = nchA + (q1 - q0 + BP_CHUNK - 1) / BP_CHUNK;
+    auto chunk_begin = [&](int ch) { return ch < nchA ? p0 + ch * BP_CHUNK : q0 + (ch - nchA) * BP_CHUNK; };
+    auto chunk_count = [&](int ch) { return min(BP_CHUNK, (ch < nchA ? p1 : q1) - chunk_begin(ch)); };
 
     auto stage = [&](int buf, int ch) {
         const int i0 = chunk_begin(ch), cnt = chunk_count(ch);
@@ -189,7 +196,7 @@ __global__ void __launch_bounds__(BP_THREADS, 4) k_backproject(const float4 *__r
         asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
     }
     __syncthreads();
-    stage(0, 0);
+    if (nch > 0) stage(0, 0);
     __syncthreads();
     for (int ch = 0; ch < nch; ++ch) {
         const int buf = ch & 1;
@@ -234,8 +241,13 @@ __global__ void __launch_bounds__(BP_THREADS, 4) k_backproject(const float4 *__r
         const int x = tix * TILE + 4 * pxi + (nch > nchA ? 3 - (v & 3) : (v & 3)), y = tiy * TILE + 2 * pyi + (v >> 2);
         if (x < a.n && y < a.n) {
             float4 *dst = O + (((int64_t)z * a.n + y) * a.n + x) * a.Q + jg * JQ;
+            if (a.agroups == 1) {
 #pragma unroll
-            for (int jc = 0; jc < JQ; ++jc) dst[jc] = acc[v][jc];
+                for (int jc = 0; jc < JQ; ++jc) dst[jc] = acc[v][jc];
+            } else {
+#pragma unroll
+                for (int jc = 0; jc < JQ; ++jc) atomicAdd(dst + jc, acc[v][jc]);
+            }
         }
     }
 }
@@ -243,7 +255,22 @@ __global__ void __launch_bounds__(BP_THREADS, 4) k_backproject(const float4 *__r
 template <int JQ>
 static cudaError_t bp_launch(cp4d_ctx *c, const float4 *gt, float *f_out, const BpArgs &a) {
     const Dims &d = c->d;
-    k_backproject<JQ><<<dim3(d.tiles, d.nz, a.Q / JQ), BP_THREADS, 0, c->stream>>>(gt, f_out, a);
+    // small grids: whole waves of 148 SMs x 4 resident CTAs, least (waves x angles per CTA); the partial sums of the angle groups
+    // are added into a zeroed output
+    const int64_t ctas = (int64_t)d.tiles * d.nz * (a.Q / JQ);
+    BpArgs b = a;
+    double best = 1e300;
+    for (int ag = 1; ag <= std::min(8, d.n0); ++ag) {
+        const int64_t waves = (ctas * ag + 148 * 4 - 1) / (148 * 4);
+        const double cost = (double)waves * ((d.n0 + ag - 1) / ag + (ag > 1 ? 6 : 0));
+        if (cost < best) { best = cost; b.agroups = ag; }
+    }
+    if (b.agroups > 1) {
+        cudaError_t e = cudaMemsetAsync(f_out, 0, (size_t)d.nz * d.n * d.n * a.Q * sizeof(float4), c->stream);
+        if (e != cudaSuccess) return e;
+        c->launches++;
+    }
+    k_backproject<JQ><<<dim3(d.tiles * b.agroups, d.nz, a.Q / JQ), BP_THREADS, 0, c->stream>>>(gt, f_out, b);
     return cudaGetLastError();
 }
 
@@ -273,7 +300,7 @@ cudaError_t launch_backproject(cp4d_ctx *c, const float4 *gt, float *f_out, int 
     ProfScope ps(c, CP4D_K_BACKPROJECT);
     const Dims &d = c->d;
     const int Q = Q_override > 0 ? Q_override : d.Q;
-    BpArgs a{d.n, d.nz, d.nd, d.n0, Q, d.gp, d.gpl, c->n_cpos, c->ang, c->geo};
+    BpArgs a{d.n, d.nz, d.nd, d.n0, Q, d.gp, d.gpl, c->n_cpos, d.tiles, 1, c->ang, c->geo};
     c->launches++;
     if (Q % 2 == 0) return bp_launch<2>(c, gt, f_out, a);
     return bp_launch<1>(c, gt, f_out, a);

@@ -24,7 +24,6 @@ __device__ __forceinline__ void fma4(float4 &a, float w, const float4 &v) {
 
 struct ProjArgs {
     int n, nz, nd, n0, Q, gp, gpl;
-    const AngleTab *ang;
     const TileGeo *geo;
     const FwAngle *fwang;      // k_forward_rays: packed per-angle parameters and the angle order by stepping axis
     const int32_t *fworder;
@@ -158,11 +157,19 @@ template <int JQ>
 static cudaError_t fwd_launch_rays(cp4d_ctx *c, const float *f, float4 *P, const ProjArgs &a) {
     const Dims &d = c->d;
     const size_t sh = FwRays<JQ>::SMEM;
-    // small problems: split the base angles over up to 8 CTAs per tile so that the grid fills the 148 SMs x 3 CTAs twice
+    // small problems: split the base angles over up to 8 CTAs per tile
     const int nzz = (d.nz + FwRays<JQ>::ZZ - 1) / FwRays<JQ>::ZZ;
     const int64_t ctas = (int64_t)d.tiles * nzz * (d.Q / JQ);
     ProjArgs b = a;
-    b.agroups = (int)std::max<int64_t>(1, std::min<int64_t>(std::min(8, d.n0), (2 * 148 * 3 + ctas - 1) / ctas));
+    // whole waves of 148 SMs x 3 resident CTAs: pick the split with the least (waves x work per CTA), the work of a CTA being its
+    // share of the base angles plus the staging of its tile and its REDs (about 16 angles' worth, measured)
+    b.agroups = 1;
+    double best = 1e300;
+    for (int ag = 1; ag <= std::min(8, d.n0); ++ag) {
+        const int64_t waves = (ctas * ag + 148 * 3 - 1) / (148 * 3);
+        const double cost = (double)waves * ((d.n0 + ag - 1) / ag + 16);
+        if (cost < best) { best = cost; b.agroups = ag; }
+    }
     const dim3 grid(d.tiles * b.agroups, nzz, d.Q / JQ);
     cudaError_t e;
     if (d.n0 <= FW_TAB) {
@@ -188,7 +195,7 @@ void fwtable_free(FwTable *t) { delete t; }
 cudaError_t launch_forward_partial(cp4d_ctx *c, const float *f, float4 *P) {
     ProfScope ps(c, CP4D_K_FORWARD);
     const Dims &d = c->d;
-    ProjArgs a{d.n, d.nz, d.nd, d.n0, d.Q, d.gp, d.gpl, c->ang, c->geo, c->fwang, c->fworder, c->n_colstep, d.tiles, 1};
+    ProjArgs a{d.n, d.nz, d.nd, d.n0, d.Q, d.gp, d.gpl, c->geo, c->fwang, c->fworder, c->n_colstep, d.tiles, 1};
     cudaError_t e = cudaMemsetAsync(P, 0, (size_t)d.scratch4 * sizeof(float4), c->stream);
     if (e != cudaSuccess) return e;
     c->launches += 2;
