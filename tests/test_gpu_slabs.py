@@ -128,6 +128,29 @@ def test_streamed_solver_temporal_blocking(torch_cuda, slab_nz, block, iters):
     T.close(); whole.close()
 
 
+@pytest.mark.parametrize("n_frames", [4, 12])
+def test_slabs_in_frame_mode(torch_cuda, n_frames):
+    """Frame mode (N_t <= M collapsed into the projector table, N_t > M through k_mix) cut into 3 slabs, all-resident and streamed."""
+    from paper_1809_09725_b200 import binding, slabs
+    torch = torch_cuda
+    c = CASE
+    phi = synth.basis_table(c.basis, c.m, c.n_angles)
+    g = synth.sinogram(c).numpy().astype(np.float32)
+    whole = binding.Context.from_config(c, phi=phi, n_frames=n_frames)
+    S = slabs.SlabSolver.from_config(c, phi=phi, n_slabs=3, n_frames=n_frames)
+    T = slabs.StreamedSolver(c.n, c.nz, c.nd, c.n_angles, c.n_half_rot, c.m, phi, slab_nz=3, n_frames=n_frames, block=2,
+                             lambda1=c.lambda1, lambda2=c.lambda2)
+    for x in (whole, S):
+        x.set_data(dev(torch, g)); x.set_steps(0.01, 0.01); x.reset(); x.iterate(6); x.sync()
+    T.set_data(g); T.set_steps(0.01, 0.01); T.reset(); T.iterate(6); T.get_f()
+    sw = whole.state()
+    assert sw["f"].shape[-1] == n_frames and float(sw["h2"].abs().max()) > 0
+    for k in ("f", "ft", "h1", "h2"):
+        assert rel(S.gather(k).cpu().numpy(), sw[k].cpu().numpy()) <= 1e-5, k
+        assert rel(getattr(T, k).numpy(), sw[k].cpu().numpy()) <= 1e-5, k
+    whole.close(); S.close(); T.close()
+
+
 def test_slab_context_call_rules(torch_cuda):
     from paper_1809_09725_b200 import binding
     torch = torch_cuda
