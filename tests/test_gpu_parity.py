@@ -287,6 +287,33 @@ def test_objective_monitor(torch_cuda, fast_oracle, case):
     ctx.close()
 
 
+def test_long_run_converges(torch_cuda):
+    """2000 iterations at config 2 with tau = sigma = 0.95/L (tau sigma L^2 < 1, L97): every iterate finite, the primal value
+    and the dual residual |K1^T h1 - div h2| fall, the duality gap estimate closes, and |h2| <= lambda1 holds throughout."""
+    from paper_1809_09725_b200 import binding
+    torch = torch_cuda
+    c = CASES["cfg2"].scaled(lambda1=2e-4)
+    side = torch.cuda.Stream()
+    with torch.cuda.stream(side):                       # the CUDA-graph path
+        ctx = binding.Context.from_config(c)
+        g = synth.sinogram(c, device="cuda").to(torch.float32).contiguous()
+        ts = 0.95 / ctx.norm(30, seed=2)
+        ctx.set_data(g); ctx.set_steps(ts, ts); ctx.reset()
+        hist = []
+        for n in (10, 90, 400, 1500):
+            ctx.iterate(n)
+            hist.append(ctx.objective())
+            st = ctx.state()
+            assert all(bool(torch.isfinite(st[k]).all()) for k in ("f", "ft", "h1", "h2"))
+            assert float(torch.sqrt((st["h2"].double() ** 2).sum(0)).max()) <= 2e-4 * (1 + 1e-5)
+        assert ctx.graph_replays() == 2000
+        ctx.close()
+    primal, dual, kkt = zip(*hist)
+    assert primal[0] > primal[1] > primal[2] > primal[3] > 0
+    assert kkt[0] > kkt[1] > kkt[2] > kkt[3]
+    assert primal[3] - dual[3] < 0.2 * (primal[0] - dual[0])       # conditional gap (the dual constraint K^T h = 0 holds only in the limit)
+
+
 @pytest.mark.parametrize("case", ["ragged", "ragged_m16", "cfg2"])
 def test_fbp_half_rotations(torch_cuda, fast_oracle, case):
     """cp4d_fbp against the oracle's plain definition; then as the initial guess of a frame-mode run."""
