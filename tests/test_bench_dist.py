@@ -47,3 +47,34 @@ def test_single_rank_is_identity():
     import bench
     assert bench.reduce_max(3.5, 1) == 3.5
     assert bench.replicas_value(1, 10, 100.0) == pytest.approx(100.0)
+
+
+def test_json_line_contract_offline():
+    """bench.assemble on a canned run record: the keys and invariants of the bench contract (no GPU needed)."""
+    sys.path.insert(0, str(ROOT))
+    import bench
+    from paper_1809_09725_b200 import synth
+
+    class A:
+        steps, warmup, frames = 50, 5, 0
+    c = synth.CONFIGS[3]
+    prof = {k: (ms * 50, 50) for k, ms in dict(forward=6.7, backproject=3.8, prox_f2=0.76, update=0.61, synth=0.09, fold=0.07).items()}
+    r = dict(ms=600.0, launches=350, prof=prof, prof_gd={"grad": (1.38, 3), "div": (1.2, 3)}, ops={"forward_op": 6.7, "adjoint_op": 3.85},
+             e2e={"value": 81.0, "unit": bench.UNIT, "h2d_bytes_per_step": 1.0, "d2h_bytes_per_step": 2.0},
+             clocks={"sm_mhz": 1965.0, "sm_max_mhz": 1965.0, "reasons": []}, peaks=bench.load_peaks(), L=1.0, launches_total=1,
+             graph_replays=55)
+    line = bench.assemble(A, c, 1, r)
+    for k in ("metric", "value", "unit", "n_gpus", "steps", "warmup", "ms_per_step", "higher_is_better", "scaling", "vs_baseline",
+              "dtype", "data", "config", "roofline", "e2e", "clocks", "gpu_launches"):
+        assert k in line, k
+    assert line["value"] == pytest.approx(50 / 0.6) and line["ms_per_step"] == pytest.approx(12.0)
+    assert line["dtype"] == "f32" and line["data"] == "synthetic" and line["vs_baseline"] is None and line["scaling"] == "weak"
+    assert "workload" in line["config"] and "model" not in line["config"]
+    rf = line["roofline"]
+    assert rf["kernel"] == "forward" and rf["bound"] == "alu" and rf["unit"] == "TFLOP/s"
+    assert rf["frac"] == pytest.approx(rf["achieved"] / rf["peak"]) and 0 < rf["frac"] < 1
+    # algorithmic flops of the forward kernel: 2 flop x 2 taps x m x N^2 Nz N_theta0 (DESIGN.md 7)
+    assert rf["achieved"] * 1e12 * 6.7e-3 == pytest.approx(2 * 2 * c.m * c.n ** 2 * c.nz * c.n_theta0, rel=1e-9)
+    assert rf["smem_roof"]["frac"] == pytest.approx(4 * rf["frac"] * (148 * 128 * 2 * r["peaks"]["sm_max_mhz"] * 1e6 / 1e12) / rf["peak"], rel=1e-6)
+    hbm = line["kernels"]["prox_f2"]
+    assert hbm["bound"] == "hbm" and hbm["achieved"] == pytest.approx(9 * c.V * 4 / 0.76e-3 / 1e9)
