@@ -47,7 +47,7 @@ def build_lib(force: bool = False, verbose: bool = False) -> Path:
     if verbose:
         print("\n".join(log))
     tmp = LIB.with_suffix(f".tmp{os.getpid()}.so")
-    subprocess.check_call([nvcc, "-shared", "-o", str(tmp), *objs, "-cudart", "static"])
+    subprocess.check_call([nvcc, "-shared", "-Wno-deprecated-gpu-targets", "-o", str(tmp), *objs, "-cudart", "static"])
     os.replace(tmp, LIB)
     return LIB
 
