@@ -155,6 +155,8 @@ int cp4d_create(const cp4d_params *p, cp4d_ctx **out) {
     ctx->tau = ctx->sigma = 0.f; ctx->have_steps = ctx->have_data = false;
     ctx->device = p->device; ctx->stream = (cudaStream_t)p->stream; ctx->launches = 0; ctx->prof_on = false;
     ctx->fwtab_host = nullptr;
+    ctx->zs = 0; ctx->nzs = d.nz; ctx->side = nullptr; ctx->ev_join = nullptr;
+    for (auto &e : ctx->ev_slab) e = nullptr;
     ctx->iter_graph = nullptr; ctx->iter_graph_launches = 0; ctx->graph_replays = 0; ctx->iter_graph_off = false;
     char *w = (char *)p->workspace_dev;
     ctx->f = (float *)(w + cv.f); ctx->ft = (float *)(w + cv.ft); ctx->bp = (float *)(w + cv.bp);

@@ -119,7 +119,8 @@ __device__ __forceinline__ void bp_angle(float4 (&acc)[8][JQ], const float4 *wba
 
 struct BpArgs {
     int n, nz, nd, n0, Q, gp, gpl, n_pos;   // n_pos: the first n_pos base angles have c >= 0, the others c < 0
-    int tiles, agroups;                     // blockIdx.x = tile + tiles * angle group (small grids split the base angles over CTAs,
+    int n_work;                             // work items = tiles * agroups * nz * (Q / JQ)
+    int tiles, agroups;                     // item = tile + tiles * angle group (small grids split the base angles over CTAs,
                                             // which then ADD their partial sums to a zeroed output)
     const AngleTab *ang;
     const TileGeo *geo;
@@ -139,9 +140,20 @@ __global__ void __launch_bounds__(BP_THREADS, 4) k_backproject(const float4 *__r
     __shared__ BpAngle sang[2][BP_CHUNK];
     __shared__ __align__(8) uint64_t mbar[2];
     const int tiles_1d = (a.n + TILE - 1) / TILE;
-    const int tile_id = blockIdx.x % a.tiles, ag = blockIdx.x / a.tiles;
+    // work item w = (tile, angle group, slice, coefficient group).  The ordinary launch has one CTA per item; the launch that runs
+    // beside the forward projector is a persistent grid of 2 CTAs per SM striding over the items
+    const int per_z = a.tiles * a.agroups;
+    unsigned cc = 0;                         // chunks staged so far by this CTA: buffer = cc & 1, mbarrier parity = (cc >> 1) & 1
+    if (threadIdx.x == 0) {
+        mbar_init(&mbar[0], 1);
+        mbar_init(&mbar[1], 1);
+        asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
+    }
+    __syncthreads();
+    for (int wi = blockIdx.x; wi < a.n_work; wi += gridDim.x) {
+    const int tile_id = (wi % per_z) % a.tiles, ag = (wi % per_z) / a.tiles;
     const int tix = tile_id % tiles_1d, tiy = tile_id / tiles_1d;
-    const int z = blockIdx.y, jg = blockIdx.z;
+    const int z = (wi / per_z) % a.nz, jg = wi / (per_z * a.nz);
     // lane -> patch: a quarter warp (the unit an LDS.128 is served in) covers 2 (x) x 4 (y) patches; their window starts
     // differ by at most 4|c| + 6 s <= 7.2 < 8 slots of 16 B, so the 8 lanes never collide on a bank
     const int l = threadIdx.x & 31, w = threadIdx.x >> 5;
@@ -190,19 +202,13 @@ __global__ void __launch_bounds__(BP_THREADS, 4) k_backproject(const float4 *__r
     for (int v = 0; v < 8; ++v)
 #pragma unroll
         for (int jc = 0; jc < JQ; ++jc) acc[v][jc] = make_float4(0.f, 0.f, 0.f, 0.f);
-    if (threadIdx.x == 0) {
-        mbar_init(&mbar[0], 1);
-        mbar_init(&mbar[1], 1);
-        asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
-    }
+    if (nch > 0) stage((int)(cc & 1), 0);
     __syncthreads();
-    if (nch > 0) stage(0, 0);
-    __syncthreads();
-    for (int ch = 0; ch < nch; ++ch) {
-        const int buf = ch & 1;
-        // buffer buf^1 and sang[buf^1] were last read in iteration ch-1, which ended with __syncthreads
+    for (int ch = 0; ch < nch; ++ch, ++cc) {
+        const int buf = (int)(cc & 1);
+        // buffer buf^1 and sang[buf^1] were last read in the previous chunk iteration, which ended with __syncthreads
         if (ch + 1 < nch) stage(buf ^ 1, ch + 1);
-        mbar_wait(&mbar[buf], (unsigned)((ch >> 1) & 1));
+        mbar_wait(&mbar[buf], (cc >> 1) & 1);
         const int na = chunk_count(ch);
         // from the first chunk with c < 0 on, the patch is traversed mirrored in x (offset e = 3 - dx): swap the accumulators
         // once (warp-uniform, outside the angle loop) so that the same straight-line bodies serve both signs
@@ -250,14 +256,15 @@ __global__ void __launch_bounds__(BP_THREADS, 4) k_backproject(const float4 *__r
             }
         }
     }
+    }   // work items
 }
 
 template <int JQ>
-static cudaError_t bp_launch(cp4d_ctx *c, const float4 *gt, float *f_out, const BpArgs &a) {
+static cudaError_t bp_launch(cp4d_ctx *c, const float4 *gt, float *f_out, const BpArgs &a, bool persistent) {
     const Dims &d = c->d;
     // small grids: whole waves of 148 SMs x 4 resident CTAs, least (waves x angles per CTA); the partial sums of the angle groups
     // are added into a zeroed output
-    const int64_t ctas = (int64_t)d.tiles * d.nz * (a.Q / JQ);
+    const int64_t ctas = (int64_t)d.tiles * a.nz * (a.Q / JQ);
     BpArgs b = a;
     double best = 1e300;
     for (int ag = 1; ag <= std::min(8, d.n0); ++ag) {
@@ -266,11 +273,14 @@ static cudaError_t bp_launch(cp4d_ctx *c, const float4 *gt, float *f_out, const 
         if (cost < best) { best = cost; b.agroups = ag; }
     }
     if (b.agroups > 1) {
-        cudaError_t e = cudaMemsetAsync(f_out, 0, (size_t)d.nz * d.n * d.n * a.Q * sizeof(float4), c->stream);
+        const cudaError_t e = cudaMemsetAsync(f_out, 0, (size_t)a.nz * d.n * d.n * a.Q * sizeof(float4), c->stream);
         if (e != cudaSuccess) return e;
         c->launches++;
     }
-    k_backproject<JQ><<<dim3(d.tiles * b.agroups, d.nz, a.Q / JQ), BP_THREADS, 0, c->stream>>>(gt, f_out, b);
+    b.n_work = (int)(ctas * b.agroups);
+    // persistent: 2 CTAs per SM stay resident and leave the rest of every SM to the forward projector launched after it
+    const int grid = persistent ? std::min(b.n_work, 2 * 148) : b.n_work;
+    k_backproject<JQ><<<grid, BP_THREADS, 0, c->stream>>>(gt, f_out, b);
     return cudaGetLastError();
 }
 
@@ -296,14 +306,16 @@ uint32_t bp_pattern_fl(int pat) {
 }
 
 // Q_override > 0: backproject Q_override float4 chunks per bin / voxel instead of the context's Q (cp4d_fbp)
-cudaError_t launch_backproject(cp4d_ctx *c, const float4 *gt, float *f_out, int Q_override) {
+cudaError_t launch_backproject(cp4d_ctx *c, const float4 *gt, float *f_out, int Q_override, bool persistent) {
     ProfScope ps(c, CP4D_K_BACKPROJECT);
     const Dims &d = c->d;
     const int Q = Q_override > 0 ? Q_override : d.Q;
-    BpArgs a{d.n, d.nz, d.nd, d.n0, Q, d.gp, d.gpl, c->n_cpos, d.tiles, 1, c->ang, c->geo};
+    gt += (size_t)c->zs * d.n0 * Q * d.gp;                 // the context's z-window
+    f_out += (size_t)c->zs * d.n * d.n * Q * 4;
+    BpArgs a{d.n, c->nzs, d.nd, d.n0, Q, d.gp, d.gpl, c->n_cpos, 0, d.tiles, 1, c->ang, c->geo};
     c->launches++;
-    if (Q % 2 == 0) return bp_launch<2>(c, gt, f_out, a);
-    return bp_launch<1>(c, gt, f_out, a);
+    if (Q % 2 == 0) return bp_launch<2>(c, gt, f_out, a, persistent);
+    return bp_launch<1>(c, gt, f_out, a, persistent);
 }
 
 }  // namespace cp4d

@@ -158,7 +158,7 @@ static cudaError_t fwd_launch_rays(cp4d_ctx *c, const float *f, float4 *P, const
     const Dims &d = c->d;
     const size_t sh = FwRays<JQ>::SMEM;
     // small problems: split the base angles over up to 8 CTAs per tile
-    const int nzz = (d.nz + FwRays<JQ>::ZZ - 1) / FwRays<JQ>::ZZ;
+    const int nzz = (a.nz + FwRays<JQ>::ZZ - 1) / FwRays<JQ>::ZZ;
     const int64_t ctas = (int64_t)d.tiles * nzz * (d.Q / JQ);
     ProjArgs b = a;
     // whole waves of 148 SMs x 3 resident CTAs: pick the split with the least (waves x work per CTA), the work of a CTA being its
@@ -195,8 +195,11 @@ void fwtable_free(FwTable *t) { delete t; }
 cudaError_t launch_forward_partial(cp4d_ctx *c, const float *f, float4 *P) {
     ProfScope ps(c, CP4D_K_FORWARD);
     const Dims &d = c->d;
-    ProjArgs a{d.n, d.nz, d.nd, d.n0, d.Q, d.gp, d.gpl, c->geo, c->fwang, c->fworder, c->n_colstep, d.tiles, 1};
-    cudaError_t e = cudaMemsetAsync(P, 0, (size_t)d.scratch4 * sizeof(float4), c->stream);
+    // the context's z-window: slices are independent, so a window is the same launch on offset pointers
+    f += (size_t)c->zs * d.n * d.n * d.Q * 4;
+    P += (size_t)c->zs * d.n0 * d.Q * d.gp;
+    ProjArgs a{d.n, c->nzs, d.nd, d.n0, d.Q, d.gp, d.gpl, c->geo, c->fwang, c->fworder, c->n_colstep, d.tiles, 1};
+    cudaError_t e = cudaMemsetAsync(P, 0, (size_t)c->nzs * d.n0 * d.Q * d.gp * sizeof(float4), c->stream);
     if (e != cudaSuccess) return e;
     c->launches += 2;
     switch (pick_jq(d.Q)) {
