@@ -229,18 +229,20 @@ def _cp_setup(oracle, lambda1, seed=12, **kw):
     return P, K1, K2, g, 0.95 / L
 
 
-def test_p7_cp_step_matches_dense_algebra(oracle):
-    """Three iterations of Fig. 2 written with dense matrices (steps 3-6 verbatim) == the C loop."""
+@pytest.mark.parametrize("theta", [1.0, 0.5, 0.0])
+def test_p7_cp_step_matches_dense_algebra(oracle, theta):
+    """Three iterations of Fig. 2 written with dense matrices (steps 3-6 verbatim) == the C loop, for the over-relaxation
+    theta = 1 (R7) and for theta = 0.5, 0 (theta in [0,1])."""
     P, K1, K2, g, ts = _cp_setup(oracle, 0.3)
     st = P.zero_state()
     f = np.zeros(P.V); ft = f.copy(); h1 = np.zeros(P.S); h2 = np.zeros(4 * P.V)
     for it in range(3):
-        P.cp(g, st, ts, ts, 1)
+        P.cp(g, st, ts, ts, 1, theta=theta)
         h1 = (h1 + ts * (K1 @ ft) - ts * g.ravel()) / (1 + ts)                       # step 3
         q = (h2 + ts * (K2 @ ft)).reshape(4, -1)                                     # step 4
         h2 = (q / np.maximum(1.0, np.sqrt((q ** 2).sum(0)) / P.lambda1)).ravel()
         fn = f - ts * (K1.T @ h1) - ts * (K2.T @ h2)                                 # step 5 (div = -K2^T)
-        ft = fn + 1.0 * (fn - f)                                                     # step 6
+        ft = fn + theta * (fn - f)                                                   # step 6
         f = fn
         np.testing.assert_allclose(st["f"].ravel(), f, atol=1e-12)
         np.testing.assert_allclose(st["ft"].ravel(), ft, atol=1e-12)
@@ -425,3 +427,38 @@ def test_p10_fbp_reconstructs_a_disk(oracle):
         assert np.abs(img[rho < r - 3] - 1.0).max() < 0.08
         assert np.abs(img[(rho > r + 3) & (rho < 30)]).max() < 0.08
     np.testing.assert_allclose(rec[..., 0], rec[..., 1], atol=1e-9)     # symmetric data: the bin flip changes nothing
+
+
+def test_p10_fbp_follows_a_disk_that_moves_between_half_rotations(oracle):
+    """An OFF-CENTRE disk that jumps to another place at every half-rotation ("time frames 3, 4 ... by using
+    projections from the intervals [3 pi, 4 pi) and [4 pi, 5 pi)").  Data: exact chord lengths at the TRUE angle theta_k = k pi/n0
+    (>= pi from the second half-rotation on, so the detector coordinate is mirrored there, L202).  Plane q of the FBP must show
+    the disk where it was during half-rotation q and nothing where it was during the others: a half-rotation assigned to the
+    wrong plane, or an odd one backprojected without the flip, lands the disk at the wrong place (the positions are chosen so
+    that no two of them, nor their mirror images, overlap)."""
+    n = nd = 64
+    n0, npi, r = 120, 3, 6.0
+    na = n0 * npi
+    centres = [(12.0, 5.0), (-9.0, 11.0), (4.0, -14.0)]
+    s = np.arange(nd) - (nd - 1) / 2.0
+    g = np.zeros((1, na, nd))
+    for k in range(na):
+        th = k * np.pi / n0
+        cx, cy = centres[k // n0]
+        g[0, k] = 2.0 * np.sqrt(np.maximum(0.0, r * r - (s - cx * np.cos(th) - cy * np.sin(th)) ** 2))
+    rec = oracle.fbp_half_rotations(n, 1, nd, na, npi, g)
+    x = np.arange(n) - (n - 1) / 2.0
+    X, Y = np.meshgrid(x, x, indexing="xy")
+    for q in range(npi):
+        img = rec[0, :, :, q]
+        for p, (cx, cy) in enumerate(centres):
+            inside = np.hypot(X - cx, Y - cy) < r - 2.5
+            mirrored = np.hypot(X + cx, Y + cy) < r - 2.5        # where a missing flip would put it
+            if p == q:
+                assert abs(img[inside].mean() - 1.0) < 0.05, (q, p, img[inside].mean())
+                assert abs(img[mirrored].mean()) < 0.1
+            else:
+                assert abs(img[inside].mean()) < 0.1, (q, p, img[inside].mean())
+        # centre of mass of the clearly positive part sits at the disk of this half-rotation
+        w = np.where(img > 0.5, img, 0.0)
+        assert abs((w * X).sum() / w.sum() - centres[q][0]) < 0.5 and abs((w * Y).sum() / w.sum() - centres[q][1]) < 0.5
