@@ -18,14 +18,22 @@ numbered 1..5 as in SURVEY.md 8).  Inputs are seeded and synthetic (paper_1809_0
   cpu_baseline : the fp64 oracle (oracle/cp4d_ref.c, as it stands) on this box's host cores, on a bounded
              sample (a few full in-plane slices), extrapolated to the whole problem.
 
+The default workload is config 5 (2048^2 x 32, 3600 angles, m = 16: the largest single-GPU configuration of BASELINE.json,
+65 GB of workspace); `--config 3` is the quick one.
+
 N > 1: the path does not shard (north_star: one GPU); `--gpus N` runs N independent replicas, one per rank,
-no data-path collective ("replicas only").  `--impl reference` times the oracle only.
+no data-path collective ("replicas only"): the value is REPLICA throughput.  Started without a
+launcher (`python bench.py --gpus N`, no WORLD_SIZE in the environment) it re-executes itself under
+`python -m torch.distributed.run --nproc-per-node N`; if the box has fewer than N GPUs, or WORLD_SIZE disagrees with N,
+it exits non-zero instead of printing a line for fewer GPUs.  `--impl reference` times the oracle only.
 """
 from __future__ import annotations
 
 import argparse
+import hashlib
 import json
 import os
+import socket
 import subprocess
 import sys
 import threading
@@ -50,6 +58,17 @@ def load_peaks():
         d = json.loads(p.read_text())
         return dict(hbm_gbs=float(d["hbm_gbs"]), sm_max_mhz=float(d.get("sm_max_mhz", 1965.0)), source="measured")
     return dict(hbm_gbs=6650.0, sm_max_mhz=1965.0, source="fallback")
+
+
+def csrc_sha1() -> str:
+    """SHA-1 over the kernel sources: profiles/traffic.json stores the one its ncu capture was taken with, and its DRAM bytes
+    are only reported for the kernels that are actually running (a stale capture gives "traffic": null)."""
+    h = hashlib.sha1()
+    d = ROOT / "paper_1809_09725_b200" / "csrc"
+    for f in sorted(list(d.glob("*.cu")) + list(d.glob("*.cuh"))):
+        h.update(f.name.encode())
+        h.update(f.read_bytes())
+    return h.hexdigest()
 
 
 def alu_peak_tflops(sm_mhz: float) -> float:
@@ -194,17 +213,28 @@ def oracle_steps(c, steps: int, warmup: int, target_fma: float = 4e10, n_frames:
     return 1.0 / (dt * scale), cores, sample, dt
 
 
+def workload_config(c, n_frames=0):
+    """The `config` object both arms print (same keys, so the driver can tell they ran the same workload)."""
+    from paper_1809_09725_b200 import synth
+    return {"workload": synth.describe(c) + (f"_frames{n_frames}" if n_frames else ""), "n_frames": n_frames, "cfg": c.cfg,
+            "n": c.n, "nz": c.nz, "nd": c.nd, "n_angles": c.n_angles, "n_half_rot": c.n_half_rot, "m": c.m, "basis": c.basis,
+            "lambda1": c.lambda1, "lambda2": c.lambda2}
+
+
 def run_reference(args, c, rank):
     """--impl reference: the oracle on the host cores (rank 0 only), same metric/config as our arm."""
     if rank != 0:
         return
     from paper_1809_09725_b200 import synth
-    val, cores, sample, dt = oracle_steps(c, args.steps, args.warmup, target_fma=1.5e10, n_frames=args.frames)
+    # every step is one oracle CP iteration on a bounded slice sample (one slice at configs 4-5); W untimed + K timed steps
+    val, cores, sample, dt = oracle_steps(c, args.steps, min(args.warmup, 1), target_fma=1.5e10, n_frames=args.frames)
     line = {
         "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
-        "warmup": args.warmup, "ms_per_step": 1e3 / val, "higher_is_better": True, "scaling": "weak",
+        "warmup": args.warmup, "ms_per_step": dt * 1e3, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": synth.describe(c), "note": "fp64 CPU oracle (oracle/cp4d_ref.c), extrapolated from a slice sample"},
+        "config": workload_config(c, args.frames),
+        "note": ("fp64 CPU oracle (oracle/cp4d_ref.c): ms_per_step is the measured time of one step on the slice sample; value is "
+                 "the whole-workload it/s, i.e. 1 / (ms_per_step x slices / sample slices)"),
         "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample,
                          "sample_step_s": dt},
         "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
@@ -236,7 +266,7 @@ def run_cp4d(args, c, rank, world):
     if world > 1:
         dist.barrier()
     peaks = load_peaks()
-    K, W = args.steps, max(args.warmup, 0)
+    K, W = args.steps, max(args.warmup, 2)     # >= 2: the CUDA graph of one iteration is captured and instantiated in the warm-up
 
     # ---- problem, data, step sizes (outside the timed region: SURVEY 8(d)) ----
     phi = synth.basis_table(c.basis, c.m, c.n_angles)
@@ -391,13 +421,21 @@ def assemble(args, c, world, r):
                           "note": "one 4-byte operand per FMA through shared memory: 148 SM x 128 B/clk x sm_max_mhz"}
         if dom == "forward":
             roofline["smem_roof"] = k["smem_roof"]
-    tr = ROOT / "profiles" / "traffic.json"                  # dram bytes per launch from the committed ncu --set full capture
+    # dram bytes per launch from the committed `ncu --set full` capture -- only if it was taken with the kernel sources that
+    # are running now (profiles/traffic.json records their SHA-1); otherwise null, never a stale number
+    tr = ROOT / "profiles" / "traffic.json"
+    roofline["traffic_source"] = None
     if tr.exists():
         try:
-            per_kernel = json.loads(tr.read_text()).get(synth.describe(c), {})
-            roofline["traffic"] = per_kernel.get(dom)
-            for n, k in kernels.items():
-                k["traffic"] = per_kernel.get(n)
+            tj = json.loads(tr.read_text())
+            if tj.get("csrc_sha1") == csrc_sha1():
+                per_kernel = tj.get(synth.describe(c), {})
+                roofline["traffic"] = per_kernel.get(dom)
+                roofline["traffic_source"] = f"profiles/traffic.json (ncu --set full, csrc sha1 {tj['csrc_sha1'][:12]})"
+                for n, k in kernels.items():
+                    k["traffic"] = per_kernel.get(n)
+            else:
+                roofline["traffic_source"] = "profiles/traffic.json is from other kernel sources: not reported"
         except Exception:
             pass
     gups = {n: c.nominal_updates / (r["ops"][n + "_op"] * 1e-3) / 1e9 for n in ("forward", "adjoint")}
@@ -406,10 +444,10 @@ def assemble(args, c, world, r):
         "metric": METRIC, "value": replicas_value(world, K, r["ms"]), "unit": UNIT, "n_gpus": world, "steps": K,
         "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f32", "data": "synthetic",
-        "config": {"workload": synth.describe(c) + (f"_frames{args.frames}" if args.frames else ""), "n_frames": args.frames, "cfg": c.cfg, "n": c.n, "nz": c.nz, "nd": c.nd, "n_angles": c.n_angles,
-                   "n_half_rot": c.n_half_rot, "m": c.m, "basis": c.basis, "lambda1": c.lambda1, "lambda2": c.lambda2,
-                   "norm_K": r["L"], "parallelism": "replicas only" if world > 1 else "1 gpu",
-                   "l2": f"no flush: CP state {(7 * c.V + 2 * c.S) * 4 / 1e9:.2f} GB streams through every step (L2 = 126 MB)"},
+        "config": workload_config(c, args.frames),
+        "run": {"norm_K": r["L"], "parallelism": "replicas only (independent problems, no collective)" if world > 1 else "1 gpu",
+                "warmup_run": max(args.warmup, 2),
+                "l2": f"no flush: CP state {(7 * c.V + 2 * c.S) * 4 / 1e9:.2f} GB streams through every step (L2 = 126 MB)"},
         "gups_nominal": {"forward": gups["forward"], "adjoint": gups["adjoint"], "unit": "1e9 voxel*angle*basis/s",
                          "forward_ms": r["ops"]["forward_op"], "adjoint_ms": r["ops"]["adjoint_op"],
                          "note": "nominal count N^2*Nz*N_theta*m per call; kernels use the pi-fold (N_theta0 base angles)"},
@@ -419,12 +457,29 @@ def assemble(args, c, world, r):
     return line
 
 
+def spawn_ranks(n: int) -> int:
+    """`python bench.py --gpus N` without a launcher: re-execute under torch.distributed.run, one rank per GPU (the command the
+    driver itself uses for N > 1).  Returns the launcher's exit code; refuses (non-zero) when the box has fewer GPUs."""
+    import torch
+    have = torch.cuda.device_count()
+    if have < n:
+        print(f"bench.py: --gpus {n} but only {have} CUDA device(s) visible: not printing a line for fewer GPUs", file=sys.stderr)
+        return 2
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={n}", "--master-addr", "127.0.0.1",
+           "--master-port", str(port), str(Path(__file__).resolve()), *sys.argv[1:]]
+    return subprocess.call(cmd)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=50)
+    ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=5)
-    ap.add_argument("--config", type=int, default=3, help="BASELINE.json config 1..5 (SURVEY.md 8 numbering)")
+    ap.add_argument("--config", type=int, default=5,
+                    help="BASELINE.json config 1..5 (SURVEY.md 8 numbering); default 5 = the largest single-GPU config, 3 = quick")
     ap.add_argument("--impl", default="cp4d", choices=["cp4d", "reference"])
     ap.add_argument("--power-iters", type=int, default=30, help="power-iteration steps for ||K|| (DESIGN.md R8: 30)")
     ap.add_argument("--frames", type=int, default=0, help="N_t > 0: the paper's frame discretisation (cp4d_params.n_frames), e.g. 8")
@@ -437,10 +492,19 @@ def main():
     args = ap.parse_args()
     from paper_1809_09725_b200 import synth
     c = synth.CONFIGS[args.config]
+    if args.gpus < 1:
+        raise SystemExit("bench.py: --gpus must be >= 1")
     rank, world = int(os.environ.get("RANK", 0)), int(os.environ.get("WORLD_SIZE", 1))
-    if args.impl == "reference":
+    if args.impl == "reference":                       # the oracle on the host cores: rank 0 alone works, whatever N is
         run_reference(args, c, rank)
         return
+    if "WORLD_SIZE" not in os.environ and args.gpus > 1:
+        sys.exit(spawn_ranks(args.gpus))               # no launcher: start N ranks ourselves, one replica per GPU
+    if world != args.gpus:
+        raise SystemExit(f"bench.py: --gpus {args.gpus} but WORLD_SIZE={world}: refusing to print a line for another GPU count")
+    import torch
+    if torch.cuda.device_count() < int(os.environ.get("LOCAL_WORLD_SIZE", world)):
+        raise SystemExit(f"bench.py: {world} ranks but only {torch.cuda.device_count()} CUDA device(s) visible")
     if args.warmup < 3:
         print(f"bench.py: warning: --warmup {args.warmup} < 3 (timing rules want >= 3)", file=sys.stderr)
     ctx, r = run_cp4d(args, c, rank, world)

@@ -32,7 +32,8 @@
  * allocates no device memory: all state and scratch live in the caller's workspace.  Input and
  * output buffers of one call must not overlap (CP4D_EINVAL) unless a parameter says "in/out".
  * All kernels are enqueued on the stream given at create; calls are asynchronous unless they say
- * "syncs".  Asynchronous faults surface at the next syncing call as CP4D_ECUDA.
+ * "syncs".  Every call makes the context's device current for its duration and restores the caller's current device
+ * before it returns (cp4d_create included), so contexts of several devices can be driven from one thread.  Asynchronous faults surface at the next syncing call as CP4D_ECUDA.
  *
  * Every function returns 0 (CP4D_OK) or a negative error code; nothing throws, exits or prints.
  */
@@ -51,6 +52,9 @@ extern "C" {
 #define CP4D_EUNSUPPORTED -3  /* no CUDA device / device is not compute capability 10.x */
 #define CP4D_ECUDA        -4  /* a CUDA runtime call or kernel failed; text in cp4d_last_error() */
 #define CP4D_ESTATE       -5  /* call order: cp4d_iterate before cp4d_set_data / cp4d_set_steps */
+#define CP4D_ENOMEM       -6  /* a host allocation failed (cp4d_create) */
+#define CP4D_EINTERNAL    -7  /* an invariant of the host prologue failed (cp4d_create: no backprojection pattern covers an
+                                 angle, or a tile window leaves the padded scratch row); a bug, never an input error */
 
 typedef struct cp4d_ctx cp4d_ctx; /* opaque; owns host-side metadata only */
 
@@ -59,7 +63,8 @@ typedef struct {
     int32_t nz;               /* slices, >= 1                                                              */
     int32_t nd;               /* detector bins, >= 2, unit spacing, centred                                */
     int32_t n_angles;         /* N_theta, total projections                                                */
-    int32_t n_half_rot;       /* N_pi half-rotations; n_angles % n_half_rot == 0 (L200; C17)     */
+    int32_t n_half_rot;       /* N_pi half-rotations; n_angles % n_half_rot == 0 (L200; C17);
+                                 n_half_rot * m <= 12288 (the slice of Phi of one base angle sits in shared memory)  */
     int32_t m;                /* temporal basis functions (the paper's M); m % 4 == 0, 4 <= m <= 32        */
     int32_t device;           /* CUDA device ordinal                                                       */
     const float *phi_host;    /* HOST, m*n_angles, [j][k] = phi_j(t_k); copied at create (L176-L180)       */
@@ -126,6 +131,10 @@ int cp4d_dot(cp4d_ctx *ctx, const float *x_dev, const float *y_dev, uint64_t cou
 /* x0 = counter-based N(0,1) from `seed`; n_power_iters steps of y = K1^T K1 x + K2^T K2 x,
  * L = sqrt(|y|/|x|).  Uses the CP state buffers as scratch (call before cp4d_reset).  Syncs. */
 int cp4d_norm(cp4d_ctx *ctx, int32_t n_power_iters, uint64_t seed, float *L_out_host);
+/* The same iteration from the caller's start vector x0 (DEVICE, V floats, any non-zero finite vector; it is copied and
+ * normalised), so that a reference implementation handed the same x0 can be compared step for step.  CP4D_EINVAL if x0 is
+ * null, misaligned, zero or not finite.  Syncs. */
+int cp4d_norm_start(cp4d_ctx *ctx, int32_t n_power_iters, const float *x0_dev, float *L_out_host);
 
 /* ---- Chambolle-Pock state machine; state (f, ft, h1, h2, g) lives in the workspace ----------- */
 int cp4d_set_data(cp4d_ctx *ctx, const float *g_dev);                 /* copy measured data g (S) */
@@ -185,6 +194,10 @@ int cp4d_launch_count(const cp4d_ctx *ctx, uint64_t *count_out);
  * stream 0, where the launches are issued one by one.  count_out: graph replays since create (each one is counted in
  * cp4d_launch_count with the number of kernels and memset nodes of one iteration). */
 int cp4d_graph_replays(const cp4d_ctx *ctx, uint64_t *count_out);
+/* "" while cp4d_iterate replays the graph (or has not tried yet); otherwise the reason it launches one by one (legacy
+ * stream, or the CUDA error text of the failed capture / instantiation).  The eager path computes the same iterates, so a
+ * failed capture is not an error of cp4d_iterate -- but it is never silent. */
+const char *cp4d_graph_note(const cp4d_ctx *ctx);
 
 /* ---- per-kernel device timing (CUDA events on the context's stream) ------------- */
 /* Kernel classes of the hot path.  FORWARD includes the zero-fill of its partial-sum scratch. */

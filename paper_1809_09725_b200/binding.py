@@ -15,7 +15,7 @@ _PKG = Path(__file__).resolve().parent
 LIB_PATH = _PKG / "libcp4d.so"
 _lib = None
 
-OK, EINVAL, EWORKSPACE, EUNSUPPORTED, ECUDA, ESTATE = 0, -1, -2, -3, -4, -5
+OK, EINVAL, EWORKSPACE, EUNSUPPORTED, ECUDA, ESTATE, ENOMEM, EINTERNAL = 0, -1, -2, -3, -4, -5, -6, -7
 
 
 class Cp4dError(RuntimeError):
@@ -57,6 +57,7 @@ def lib():
             "cp4d_primal_update": [vp, f32, vp, vp, vp, vp],
             "cp4d_dot": [vp, vp, vp, u64, C.POINTER(C.c_double)],
             "cp4d_norm": [vp, i32, u64, C.POINTER(f32)],
+            "cp4d_norm_start": [vp, i32, vp, C.POINTER(f32)],
             "cp4d_set_data": [vp, vp], "cp4d_set_steps": [vp, f32, f32], "cp4d_reset": [vp, vp],
             "cp4d_iterate": [vp, i32], "cp4d_get_f": [vp, vp],
             "cp4d_state_ptrs": [vp] + [C.POINTER(vp)] * 5,
@@ -71,11 +72,12 @@ def lib():
         for name, args in sig.items():
             fn = getattr(L, name)
             fn.argtypes, fn.restype = args, C.c_int
-        for name in ("cp4d_strerror", "cp4d_last_error", "cp4d_version", "cp4d_kernel_name"):
+        for name in ("cp4d_strerror", "cp4d_last_error", "cp4d_version", "cp4d_kernel_name", "cp4d_graph_note"):
             getattr(L, name).restype = C.c_char_p
         L.cp4d_kernel_name.argtypes = [C.c_int]
         L.cp4d_strerror.argtypes = [C.c_int]
         L.cp4d_last_error.argtypes = [vp]
+        L.cp4d_graph_note.argtypes = [vp]
         _lib = L
     return _lib
 
@@ -227,6 +229,12 @@ class Context:
         self._ck(lib().cp4d_norm(self._h, n_power_iters, seed, C.byref(out)))
         return out.value
 
+    def norm_start(self, x0, n_power_iters=30):
+        """Power iteration from the caller's start vector x0 (primal-shaped cuda tensor; copied, not modified)."""
+        out = C.c_float(0)
+        self._ck(lib().cp4d_norm_start(self._h, n_power_iters, self._t(x0, self.V), C.byref(out)))
+        return out.value
+
     # -- CP state machine ------------------------------------------------------------------------
     def set_data(self, g):
         self._ck(lib().cp4d_set_data(self._h, self._t(g, self.S)))
@@ -292,6 +300,10 @@ class Context:
         out = C.c_uint64(0)
         self._ck(lib().cp4d_graph_replays(self._h, C.byref(out)))
         return out.value
+
+    def graph_note(self) -> str:
+        """Why iterate() is not replaying a CUDA graph ("" if it is, or has not tried yet)."""
+        return lib().cp4d_graph_note(self._h).decode()
 
     def profile_begin(self):
         self._ck(lib().cp4d_profile_begin(self._h))

@@ -26,6 +26,8 @@ int validate(const cp4d_params *p, Dims *d) {
     // frame mode (L214-L237): n_frames frames every n_angles/n_frames angles; the primal 4th axis is the frame index
     if (p->n_frames < 0 || (p->n_frames > 0 && (p->n_frames % 4 || p->n_frames > MAX_M || p->n_angles % p->n_frames))) return CP4D_EINVAL;
     if (p->z_open < 0 || p->z_open > 3) return CP4D_EINVAL;
+    // k_fold / k_synth keep the n_half_rot x m slice of Phi of their base angle in (default-limit) dynamic shared memory
+    if ((int64_t)p->n_half_rot * p->m * 4 > 48 * 1024) return CP4D_EINVAL;
     d->nf = p->n_frames; d->mp = d->nf ? d->nf : d->m; d->Qp = d->mp / 4;
     d->mb = p->m;
     // Collapsed frame mode (N_t <= M): K1 o A = sum_q W[k,q] R f(t_q) with W[k,q] = sum_j phi_j(t_k) phi_j(t_q), so the projector
@@ -81,6 +83,22 @@ int fail(cp4d_ctx *c, int code, const char *what, cudaError_t e = cudaSuccess) {
         if (e__ != cudaSuccess) return fail(ctx, CP4D_ECUDA, what, e__); \
     } while (0)
 
+// Every entry point runs with the context's device current and puts the caller's device back on exit: a context made for
+// device 1 works whatever device the calling thread has selected (streams, events and launches are per device).
+struct DevGuard {
+    int prev = -1;
+    explicit DevGuard(int dev) {
+        int cur = -1;
+        if (cudaGetDevice(&cur) != cudaSuccess) { cudaGetLastError(); cur = -1; }
+        if (cur != dev && cudaSetDevice(dev) == cudaSuccess) prev = cur;
+    }
+    ~DevGuard() {
+        if (prev >= 0) cudaSetDevice(prev);
+    }
+    DevGuard(const DevGuard &) = delete;
+    DevGuard &operator=(const DevGuard &) = delete;
+};
+
 bool overlap(const void *a, uint64_t na, const void *b, uint64_t nb) {
     const uintptr_t x = (uintptr_t)a, y = (uintptr_t)b;
     return x < y + nb && y < x + na;
@@ -118,6 +136,8 @@ const char *cp4d_strerror(int code) {
     case CP4D_EUNSUPPORTED: return "no sm_100 CUDA device";
     case CP4D_ECUDA: return "CUDA error";
     case CP4D_ESTATE: return "call order: set_data/set_steps before iterate";
+    case CP4D_ENOMEM: return "host allocation failed";
+    case CP4D_EINTERNAL: return "internal invariant violated (backprojection pattern or scratch window)";
     default: return "unknown error";
     }
 }
@@ -147,16 +167,19 @@ int cp4d_create(const cp4d_params *p, cp4d_ctx **out) {
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || p->device < 0 || p->device >= ndev) { cudaGetLastError(); return CP4D_EUNSUPPORTED; }
     cudaDeviceProp prop;
     if (cudaGetDeviceProperties(&prop, p->device) != cudaSuccess || prop.major != 10) { cudaGetLastError(); return CP4D_EUNSUPPORTED; }
-    if (cudaSetDevice(p->device) != cudaSuccess) return CP4D_ECUDA;
+    DevGuard dev_guard(p->device);     // the caller's current device is restored on return
+    {
+        int cur = -1;
+        if (cudaGetDevice(&cur) != cudaSuccess || cur != p->device) { cudaGetLastError(); return CP4D_ECUDA; }
+    }
+    if (forward_init() != cudaSuccess) { cudaGetLastError(); return CP4D_ECUDA; }
 
     cp4d_ctx *ctx = new (std::nothrow) cp4d_ctx();
-    if (!ctx) return CP4D_EINVAL;
+    if (!ctx) return CP4D_ENOMEM;
     ctx->d = d; ctx->lambda1 = p->lambda1; ctx->lambda2 = p->lambda2; ctx->theta = p->theta_relax; ctx->z_open = p->z_open;
     ctx->tau = ctx->sigma = 0.f; ctx->have_steps = ctx->have_data = false;
     ctx->device = p->device; ctx->stream = (cudaStream_t)p->stream; ctx->launches = 0; ctx->prof_on = false;
     ctx->fwtab_host = nullptr;
-    ctx->zs = 0; ctx->nzs = d.nz; ctx->side = nullptr; ctx->ev_join = nullptr;
-    for (auto &e : ctx->ev_slab) e = nullptr;
     ctx->iter_graph = nullptr; ctx->iter_graph_launches = 0; ctx->graph_replays = 0; ctx->iter_graph_off = false;
     char *w = (char *)p->workspace_dev;
     ctx->f = (float *)(w + cv.f); ctx->ft = (float *)(w + cv.ft); ctx->bp = (float *)(w + cv.bp);
@@ -184,13 +207,13 @@ int cp4d_create(const cp4d_params *p, cp4d_ctx **out) {
             ang[i].fw_istep = std::fabs(st) < 1e-6 ? 0.0f : (float)(1.0 / st);
         }
         ang[i].pat = bp_pattern(ang[i].c, ang[i].s);
-        if (ang[i].pat < 0) { delete ctx; return CP4D_EINVAL; }
+        if (ang[i].pat < 0) { delete ctx; return CP4D_EINTERNAL; }   // the 7 patterns cover [0, pi): cannot happen
         ang[i].pat_fl = bp_pattern_fl(ang[i].pat);
     }
     ctx->n_cpos = 0;
     while (ctx->n_cpos < d.n0 && ang[ctx->n_cpos].c >= 0.f) ++ctx->n_cpos;
     for (int i = ctx->n_cpos; i < d.n0; ++i)
-        if (ang[i].c >= 0.f) { delete ctx; return CP4D_EINVAL; }   // cos is monotone on [0, pi): cannot happen
+        if (ang[i].c >= 0.f) { delete ctx; return CP4D_EINTERNAL; }   // cos is monotone on [0, pi): cannot happen
     std::vector<FwAngle> fwang(d.n0);
     std::vector<int32_t> fworder;
     for (int pass = 0; pass < 2; ++pass) {
@@ -211,7 +234,8 @@ int cp4d_create(const cp4d_params *p, cp4d_ctx **out) {
             const double pmin = p0 + std::fmin(0.0, (TILE - 1) * c) + std::fmin(0.0, (TILE - 1) * s);
             const double bs = std::floor(pmin) - 1.0;
             geo[(size_t)t * d.n0 + i].bstart = (int32_t)bs;
-            if ((int32_t)bs < -d.gpl || (int32_t)bs + WIN + 8 > d.gp - d.gpl) { cp4d_destroy(ctx); return CP4D_EINVAL; }
+            // validate() sized the pads of the scratch rows for this: cannot happen
+            if ((int32_t)bs < -d.gpl || (int32_t)bs + WIN + 8 > d.gp - d.gpl) { cp4d_destroy(ctx); return CP4D_EINTERNAL; }
             geo[(size_t)t * d.n0 + i].delta = (float)(p0 - bs);
         }
     }
@@ -250,6 +274,7 @@ int cp4d_create(const cp4d_params *p, cp4d_ctx **out) {
 
 int cp4d_destroy(cp4d_ctx *ctx) {
     if (ctx) {
+        DevGuard dev_guard(ctx->device);
         for (auto &r : ctx->prof) { cudaEventDestroy(r.a); cudaEventDestroy(r.b); }
         for (auto e : ctx->ev_pool) cudaEventDestroy(e);
         fwtable_free(ctx->fwtab_host);
@@ -261,18 +286,21 @@ int cp4d_destroy(cp4d_ctx *ctx) {
 
 int cp4d_forward(cp4d_ctx *ctx, const float *f, float *g) {
     if (!ctx) return CP4D_EINVAL;
+    DevGuard dev_guard(ctx->device);
     if (bad_ptr(f) || bad_ptr(g) || overlap(f, ctx->d.V * 4, g, ctx->d.S * 4)) return fail(ctx, CP4D_EINVAL, "forward: bad pointers");
     return forward_into(ctx, f, 0, 0.f, nullptr, g);
 }
 
 int cp4d_adjoint(cp4d_ctx *ctx, const float *g, float *f) {
     if (!ctx) return CP4D_EINVAL;
+    DevGuard dev_guard(ctx->device);
     if (bad_ptr(f) || bad_ptr(g) || overlap(f, ctx->d.V * 4, g, ctx->d.S * 4)) return fail(ctx, CP4D_EINVAL, "adjoint: bad pointers");
     return adjoint_into(ctx, g, f);
 }
 
 int cp4d_grad(cp4d_ctx *ctx, const float *f, float *p) {
     if (!ctx) return CP4D_EINVAL;
+    DevGuard dev_guard(ctx->device);
     if (ctx->z_open) return fail(ctx, CP4D_ESTATE, "grad: z-slab context, use the *_slab / cp4d_step_* calls");
     if (bad_ptr(f) || bad_ptr(p) || overlap(f, ctx->d.V * 4, p, ctx->d.V * 16)) return fail(ctx, CP4D_EINVAL, "grad: bad pointers");
     CK(launch_grad(ctx, f, p), "grad");
@@ -281,6 +309,7 @@ int cp4d_grad(cp4d_ctx *ctx, const float *f, float *p) {
 
 int cp4d_div(cp4d_ctx *ctx, const float *p, float *f) {
     if (!ctx) return CP4D_EINVAL;
+    DevGuard dev_guard(ctx->device);
     if (ctx->z_open) return fail(ctx, CP4D_ESTATE, "div: z-slab context, use the *_slab / cp4d_step_* calls");
     if (bad_ptr(f) || bad_ptr(p) || overlap(f, ctx->d.V * 4, p, ctx->d.V * 16)) return fail(ctx, CP4D_EINVAL, "div: bad pointers");
     CK(launch_div(ctx, p, f), "div");
@@ -289,6 +318,7 @@ int cp4d_div(cp4d_ctx *ctx, const float *p, float *f) {
 
 int cp4d_prox_f1(cp4d_ctx *ctx, float sigma, const float *ft, const float *g, float *h1) {
     if (!ctx) return CP4D_EINVAL;
+    DevGuard dev_guard(ctx->device);
     const uint64_t Vb = ctx->d.V * 4, Sb = ctx->d.S * 4;
     if (bad_ptr(ft) || bad_ptr(g) || bad_ptr(h1) || overlap(ft, Vb, h1, Sb) || overlap(g, Sb, h1, Sb) || !(sigma > 0.f))
         return fail(ctx, CP4D_EINVAL, "prox_f1: bad arguments");
@@ -297,6 +327,7 @@ int cp4d_prox_f1(cp4d_ctx *ctx, float sigma, const float *ft, const float *g, fl
 
 int cp4d_prox_f2(cp4d_ctx *ctx, float sigma, const float *ft, float *h2) {
     if (!ctx) return CP4D_EINVAL;
+    DevGuard dev_guard(ctx->device);
     if (ctx->z_open) return fail(ctx, CP4D_ESTATE, "prox_f2: z-slab context, use the *_slab / cp4d_step_* calls");
     if (bad_ptr(ft) || bad_ptr(h2) || overlap(ft, ctx->d.V * 4, h2, ctx->d.V * 16)) return fail(ctx, CP4D_EINVAL, "prox_f2: bad pointers");
     CK(launch_prox_f2(ctx, sigma, ft, h2), "prox_f2");
@@ -305,6 +336,7 @@ int cp4d_prox_f2(cp4d_ctx *ctx, float sigma, const float *ft, float *h2) {
 
 int cp4d_primal_update(cp4d_ctx *ctx, float tau, const float *h1, const float *h2, float *f, float *ft) {
     if (!ctx) return CP4D_EINVAL;
+    DevGuard dev_guard(ctx->device);
     if (ctx->z_open) return fail(ctx, CP4D_ESTATE, "primal_update: z-slab context, use the *_slab / cp4d_step_* calls");
     const uint64_t Vb = ctx->d.V * 4, Sb = ctx->d.S * 4;
     if (bad_ptr(h1) || bad_ptr(h2) || bad_ptr(f) || bad_ptr(ft) || overlap(f, Vb, ft, Vb) || overlap(f, Vb, h2, 4 * Vb) ||
@@ -318,6 +350,7 @@ int cp4d_primal_update(cp4d_ctx *ctx, float tau, const float *h1, const float *h
 
 int cp4d_dot(cp4d_ctx *ctx, const float *x, const float *y, uint64_t n, double *out) {
     if (!ctx) return CP4D_EINVAL;
+    DevGuard dev_guard(ctx->device);
     if (bad_ptr(x) || bad_ptr(y) || !out) return fail(ctx, CP4D_EINVAL, "dot: bad pointers");
     CK(launch_sumsq_dot(ctx, x, y, n, ctx->red), "dot");
     CK(cudaMemcpyAsync(out, ctx->red, sizeof(double), cudaMemcpyDeviceToHost, ctx->stream), "dot copy");
@@ -325,15 +358,14 @@ int cp4d_dot(cp4d_ctx *ctx, const float *x, const float *y, uint64_t n, double *
     return CP4D_OK;
 }
 
-int cp4d_norm(cp4d_ctx *ctx, int32_t n_iters, uint64_t seed, float *L_out) {
-    if (!ctx) return CP4D_EINVAL;
-    if (ctx->z_open) return fail(ctx, CP4D_ESTATE, "norm: z-slab context, use the *_slab / cp4d_step_* calls");
-    if (!L_out || n_iters < 1) return fail(ctx, CP4D_EINVAL, "norm: bad arguments");
+// power iteration from the start vector in ctx->ft
+static int norm_from_ft(cp4d_ctx *ctx, int32_t n_iters, float *L_out) {
     const Dims &d = ctx->d;
     float *x = ctx->ft, *y1 = ctx->bp, *y2 = ctx->f;
     double v = 0.0, L = 0.0;
-    CK(launch_fill_normal(ctx, x, d.V, seed), "fill");
+    ctx->have_data = false;  // state buffers are used as scratch
     if (int r = cp4d_dot(ctx, x, x, d.V, &v)) return r;
+    if (!(v > 0.0) || !std::isfinite(v)) return fail(ctx, CP4D_EINVAL, "norm: the start vector is zero or not finite");
     CK(launch_scale_diff(ctx, x, x, nullptr, (float)(1.0 / std::sqrt(v)), d.V), "scale");
     for (int it = 0; it < n_iters; ++it) {
         if (int r = forward_into(ctx, x, 0, 0.f, nullptr, ctx->h1)) return r;   // K1 x
@@ -347,13 +379,31 @@ int cp4d_norm(cp4d_ctx *ctx, int32_t n_iters, uint64_t seed, float *L_out) {
         if (!(ny > 0.0)) break;
         CK(launch_scale_diff(ctx, x, y1, nullptr, (float)(1.0 / ny), d.V), "normalise");
     }
-    ctx->have_data = false;  // state buffers were used as scratch
     *L_out = (float)L;
     return CP4D_OK;
 }
 
+int cp4d_norm(cp4d_ctx *ctx, int32_t n_iters, uint64_t seed, float *L_out) {
+    if (!ctx) return CP4D_EINVAL;
+    DevGuard dev_guard(ctx->device);
+    if (ctx->z_open) return fail(ctx, CP4D_ESTATE, "norm: z-slab context, use the *_slab / cp4d_step_* calls");
+    if (!L_out || n_iters < 1) return fail(ctx, CP4D_EINVAL, "norm: bad arguments");
+    CK(launch_fill_normal(ctx, ctx->ft, ctx->d.V, seed), "fill");
+    return norm_from_ft(ctx, n_iters, L_out);
+}
+
+int cp4d_norm_start(cp4d_ctx *ctx, int32_t n_iters, const float *x0, float *L_out) {
+    if (!ctx) return CP4D_EINVAL;
+    DevGuard dev_guard(ctx->device);
+    if (ctx->z_open) return fail(ctx, CP4D_ESTATE, "norm_start: z-slab context, use the *_slab / cp4d_step_* calls");
+    if (!L_out || n_iters < 1 || bad_ptr(x0)) return fail(ctx, CP4D_EINVAL, "norm_start: bad arguments");
+    CK(cudaMemcpyAsync(ctx->ft, x0, ctx->d.V * 4, cudaMemcpyDeviceToDevice, ctx->stream), "norm_start copy");
+    return norm_from_ft(ctx, n_iters, L_out);
+}
+
 int cp4d_set_data(cp4d_ctx *ctx, const float *g) {
     if (!ctx) return CP4D_EINVAL;
+    DevGuard dev_guard(ctx->device);
     if (bad_ptr(g)) return fail(ctx, CP4D_EINVAL, "set_data: bad pointer");
     CK(cudaMemcpyAsync(ctx->g, g, ctx->d.S * 4, cudaMemcpyDeviceToDevice, ctx->stream), "set_data");
     ctx->have_data = true;
@@ -362,6 +412,7 @@ int cp4d_set_data(cp4d_ctx *ctx, const float *g) {
 
 int cp4d_set_steps(cp4d_ctx *ctx, float tau, float sigma) {
     if (!ctx) return CP4D_EINVAL;
+    DevGuard dev_guard(ctx->device);
     if (!(tau > 0.f) || !(sigma > 0.f)) return fail(ctx, CP4D_EINVAL, "set_steps: tau, sigma must be > 0");
     if (ctx->iter_graph && (tau != ctx->tau || sigma != ctx->sigma)) {   // the step sizes are baked into the captured launches
         cudaGraphExecDestroy(ctx->iter_graph);
@@ -373,6 +424,7 @@ int cp4d_set_steps(cp4d_ctx *ctx, float tau, float sigma) {
 
 int cp4d_reset(cp4d_ctx *ctx, const float *f0) {
     if (!ctx) return CP4D_EINVAL;
+    DevGuard dev_guard(ctx->device);
     const Dims &d = ctx->d;
     if (f0) {
         if (bad_ptr(f0)) return fail(ctx, CP4D_EINVAL, "reset: bad pointer");
@@ -401,10 +453,17 @@ static int iterate_once(cp4d_ctx *ctx) {
 
 // capture one iteration into ctx->iter_graph; false (and eager launches from then on) if the stream cannot be captured
 static bool capture_iteration(cp4d_ctx *ctx) {
-    if (ctx->iter_graph_off || ctx->stream == nullptr || ctx->stream == cudaStreamLegacy) return false;
+    if (ctx->iter_graph_off) return false;
+    if (ctx->stream == nullptr || ctx->stream == cudaStreamLegacy) {
+        ctx->note = "the legacy default stream cannot be captured: launches are issued one by one";
+        ctx->iter_graph_off = true;
+        return false;
+    }
     const uint64_t l0 = ctx->launches;
-    if (cudaStreamBeginCapture(ctx->stream, cudaStreamCaptureModeThreadLocal) != cudaSuccess) {
+    cudaError_t ce = cudaStreamBeginCapture(ctx->stream, cudaStreamCaptureModeThreadLocal);
+    if (ce != cudaSuccess) {
         cudaGetLastError();
+        ctx->note = std::string("cudaStreamBeginCapture failed (") + cudaGetErrorString(ce) + "): launches are issued one by one";
         ctx->iter_graph_off = true;
         return false;
     }
@@ -414,10 +473,15 @@ static bool capture_iteration(cp4d_ctx *ctx) {
     ctx->iter_graph_launches = ctx->launches - l0;
     ctx->launches = l0;
     bool ok = r == CP4D_OK && e == cudaSuccess && g != nullptr;
-    if (ok) ok = cudaGraphInstantiate(&ctx->iter_graph, g, 0) == cudaSuccess;
+    cudaError_t ie = cudaSuccess;
+    if (ok) ok = (ie = cudaGraphInstantiate(&ctx->iter_graph, g, 0)) == cudaSuccess;
     if (g) cudaGraphDestroy(g);
     if (!ok) {
         cudaGetLastError();
+        // not an error of cp4d_iterate (the eager path computes the same iterates), but never silent: cp4d_graph_note tells why
+        ctx->note = "graph capture of one iteration failed (" +
+                    (r != CP4D_OK ? "a launch failed during capture: " + ctx->err
+                                  : std::string(cudaGetErrorString(e != cudaSuccess ? e : ie))) + "): launches are issued one by one";
         ctx->iter_graph = nullptr;
         ctx->iter_graph_off = true;
         ctx->err.clear();
@@ -427,6 +491,7 @@ static bool capture_iteration(cp4d_ctx *ctx) {
 
 int cp4d_iterate(cp4d_ctx *ctx, int32_t n_iters) {
     if (!ctx) return CP4D_EINVAL;
+    DevGuard dev_guard(ctx->device);
     if (ctx->z_open) return fail(ctx, CP4D_ESTATE, "iterate: z-slab context, use the *_slab / cp4d_step_* calls");
     if (n_iters < 0) return fail(ctx, CP4D_EINVAL, "iterate: n_iters < 0");
     if (!ctx->have_steps || !ctx->have_data) return fail(ctx, CP4D_ESTATE, "iterate: set_data and set_steps first");
@@ -454,6 +519,7 @@ static int check_halos(cp4d_ctx *ctx, const void *above, const void *below, bool
 
 int cp4d_set_z_open(cp4d_ctx *ctx, int32_t z_open) {
     if (!ctx) return CP4D_EINVAL;
+    DevGuard dev_guard(ctx->device);
     if (z_open < 0 || z_open > 3) return fail(ctx, CP4D_EINVAL, "set_z_open: flags are 0..3");
     ctx->z_open = z_open;
     return CP4D_OK;
@@ -461,6 +527,7 @@ int cp4d_set_z_open(cp4d_ctx *ctx, int32_t z_open) {
 
 int cp4d_grad_slab(cp4d_ctx *ctx, const float *f, const float *f_above, float *p) {
     if (!ctx) return CP4D_EINVAL;
+    DevGuard dev_guard(ctx->device);
     if (bad_ptr(f) || bad_ptr(p) || overlap(f, ctx->d.V * 4, p, ctx->d.V * 16)) return fail(ctx, CP4D_EINVAL, "grad_slab: bad pointers");
     if (int r = check_halos(ctx, f_above, nullptr, true, false, "grad_slab: a halo slice is needed exactly on an interior face")) return r;
     CK(launch_grad(ctx, f, p, f_above), "grad");
@@ -469,6 +536,7 @@ int cp4d_grad_slab(cp4d_ctx *ctx, const float *f, const float *f_above, float *p
 
 int cp4d_div_slab(cp4d_ctx *ctx, const float *p, const float *pz_below, float *f) {
     if (!ctx) return CP4D_EINVAL;
+    DevGuard dev_guard(ctx->device);
     if (bad_ptr(f) || bad_ptr(p) || overlap(f, ctx->d.V * 4, p, ctx->d.V * 16)) return fail(ctx, CP4D_EINVAL, "div_slab: bad pointers");
     if (int r = check_halos(ctx, nullptr, pz_below, false, true, "div_slab: a halo slice is needed exactly on an interior face")) return r;
     CK(launch_div(ctx, p, f, pz_below), "div");
@@ -477,6 +545,7 @@ int cp4d_div_slab(cp4d_ctx *ctx, const float *p, const float *pz_below, float *f
 
 int cp4d_step_dual(cp4d_ctx *ctx, const float *ft_above) {
     if (!ctx) return CP4D_EINVAL;
+    DevGuard dev_guard(ctx->device);
     if (!ctx->have_steps || !ctx->have_data) return fail(ctx, CP4D_ESTATE, "step_dual: set_data and set_steps first");
     if (int r = check_halos(ctx, ft_above, nullptr, true, false, "step_dual: a halo slice is needed exactly on an interior face")) return r;
     if (int r = forward_into(ctx, ctx->ft, 1, ctx->sigma, ctx->g, ctx->h1)) return r;
@@ -486,6 +555,7 @@ int cp4d_step_dual(cp4d_ctx *ctx, const float *ft_above) {
 
 int cp4d_step_primal(cp4d_ctx *ctx, const float *h2z_below) {
     if (!ctx) return CP4D_EINVAL;
+    DevGuard dev_guard(ctx->device);
     if (!ctx->have_steps || !ctx->have_data) return fail(ctx, CP4D_ESTATE, "step_primal: set_data and set_steps first");
     if (int r = check_halos(ctx, nullptr, h2z_below, false, true, "step_primal: a halo slice is needed exactly on an interior face")) return r;
     if (int r = adjoint_into(ctx, ctx->h1, ctx->bp)) return r;
@@ -495,6 +565,7 @@ int cp4d_step_primal(cp4d_ctx *ctx, const float *h2z_below) {
 
 int cp4d_get_f(cp4d_ctx *ctx, float *out) {
     if (!ctx) return CP4D_EINVAL;
+    DevGuard dev_guard(ctx->device);
     if (bad_ptr(out)) return fail(ctx, CP4D_EINVAL, "get_f: bad pointer");
     CK(cudaMemcpyAsync(out, ctx->f, ctx->d.V * 4, cudaMemcpyDeviceToDevice, ctx->stream), "get_f");
     return CP4D_OK;
@@ -502,6 +573,7 @@ int cp4d_get_f(cp4d_ctx *ctx, float *out) {
 
 int cp4d_state_ptrs(cp4d_ctx *ctx, float **f, float **ft, float **h1, float **h2, float **g) {
     if (!ctx) return CP4D_EINVAL;
+    DevGuard dev_guard(ctx->device);
     if (f) *f = ctx->f;
     if (ft) *ft = ctx->ft;
     if (h1) *h1 = ctx->h1;
@@ -512,6 +584,7 @@ int cp4d_state_ptrs(cp4d_ctx *ctx, float **f, float **ft, float **h1, float **h2
 
 int cp4d_solve_host(cp4d_ctx *ctx, const float *g_host, int32_t n_iters, float *f_host) {
     if (!ctx) return CP4D_EINVAL;
+    DevGuard dev_guard(ctx->device);
     if (ctx->z_open) return fail(ctx, CP4D_ESTATE, "solve_host: z-slab context, use the *_slab / cp4d_step_* calls");
     if (!g_host || !f_host || n_iters < 0) return fail(ctx, CP4D_EINVAL, "solve_host: bad arguments");
     if (!ctx->have_steps) return fail(ctx, CP4D_ESTATE, "solve_host: set_steps first");
@@ -526,6 +599,7 @@ int cp4d_solve_host(cp4d_ctx *ctx, const float *g_host, int32_t n_iters, float *
 
 int cp4d_objective(cp4d_ctx *ctx, double *primal, double *cond_dual, double *kkt_resid) {
     if (!ctx) return CP4D_EINVAL;
+    DevGuard dev_guard(ctx->device);
     if (ctx->z_open) return fail(ctx, CP4D_ESTATE, "objective: z-slab context, use the *_slab / cp4d_step_* calls");
     if (!ctx->have_data) return fail(ctx, CP4D_ESTATE, "objective: set_data first");
     const Dims &d = ctx->d;
@@ -558,11 +632,13 @@ int cp4d_objective(cp4d_ctx *ctx, double *primal, double *cond_dual, double *kkt
 
 int cp4d_fbp(cp4d_ctx *ctx, const float *g, float *out) {
     if (!ctx) return CP4D_EINVAL;
+    DevGuard dev_guard(ctx->device);
     const Dims &d = ctx->d;
     const int Qf = (d.npi + 3) / 4;
     const uint64_t out_bytes = (uint64_t)d.nz * d.n * d.n * Qf * 16;
     if (bad_ptr(g) || bad_ptr(out) || overlap(g, d.S * 4, out, out_bytes)) return fail(ctx, CP4D_EINVAL, "fbp: bad pointers");
     if (Qf > d.Q) return fail(ctx, CP4D_EUNSUPPORTED, "fbp: needs ceil(n_half_rot/4)*4 <= m (the projector scratch is sized for m)");
+    if ((int64_t)d.nd * 4 > 48 * 1024) return fail(ctx, CP4D_EUNSUPPORTED, "fbp: the filter keeps one sinogram row in shared memory, nd <= 12288");
     CK(launch_filter_sl(ctx, g, ctx->tmp_s), "filter");
     // the scratch rows keep their zero pads: only bins [0, nd) of the first Qf chunk planes... every plane stride is gp, and
     // with Qf != Q the row addressing differs from the fold's, so clear the scratch once and restore the invariant afterwards
@@ -575,6 +651,7 @@ int cp4d_fbp(cp4d_ctx *ctx, const float *g, float *out) {
 
 int cp4d_sync(cp4d_ctx *ctx) {
     if (!ctx) return CP4D_EINVAL;
+    DevGuard dev_guard(ctx->device);
     CK(cudaStreamSynchronize(ctx->stream), "sync");
     CK(cudaGetLastError(), "sync");
     return CP4D_OK;
@@ -582,6 +659,7 @@ int cp4d_sync(cp4d_ctx *ctx) {
 
 int cp4d_profile_begin(cp4d_ctx *ctx) {
     if (!ctx) return CP4D_EINVAL;
+    DevGuard dev_guard(ctx->device);
     for (auto &r : ctx->prof) { ctx->ev_pool.push_back(r.a); ctx->ev_pool.push_back(r.b); }
     ctx->prof.clear();
     ctx->prof_on = true;
@@ -590,6 +668,7 @@ int cp4d_profile_begin(cp4d_ctx *ctx) {
 
 int cp4d_profile_end(cp4d_ctx *ctx, cp4d_profile *out) {
     if (!ctx) return CP4D_EINVAL;
+    DevGuard dev_guard(ctx->device);
     if (!out) return fail(ctx, CP4D_EINVAL, "profile_end: null output");
     ctx->prof_on = false;
     std::memset(out, 0, sizeof(*out));
@@ -617,6 +696,8 @@ int cp4d_graph_replays(const cp4d_ctx *ctx, uint64_t *out) {
     *out = ctx->graph_replays;
     return CP4D_OK;
 }
+
+const char *cp4d_graph_note(const cp4d_ctx *ctx) { return ctx ? ctx->note.c_str() : "null context"; }
 
 int cp4d_launch_count(const cp4d_ctx *ctx, uint64_t *out) {
     if (!ctx || !out) return CP4D_EINVAL;

@@ -140,8 +140,7 @@ __global__ void __launch_bounds__(BP_THREADS, 4) k_backproject(const float4 *__r
     __shared__ BpAngle sang[2][BP_CHUNK];
     __shared__ __align__(8) uint64_t mbar[2];
     const int tiles_1d = (a.n + TILE - 1) / TILE;
-    // work item w = (tile, angle group, slice, coefficient group).  The ordinary launch has one CTA per item; the launch that runs
-    // beside the forward projector is a persistent grid of 2 CTAs per SM striding over the items
+    // work item w = (tile, angle group, slice, coefficient group), one CTA per item (the loop lets a smaller grid stride over them)
     const int per_z = a.tiles * a.agroups;
     unsigned cc = 0;                         // chunks staged so far by this CTA: buffer = cc & 1, mbarrier parity = (cc >> 1) & 1
     if (threadIdx.x == 0) {
@@ -260,7 +259,7 @@ __global__ void __launch_bounds__(BP_THREADS, 4) k_backproject(const float4 *__r
 }
 
 template <int JQ>
-static cudaError_t bp_launch(cp4d_ctx *c, const float4 *gt, float *f_out, const BpArgs &a, bool persistent) {
+static cudaError_t bp_launch(cp4d_ctx *c, const float4 *gt, float *f_out, const BpArgs &a) {
     const Dims &d = c->d;
     // small grids: whole waves of 148 SMs x 4 resident CTAs, least (waves x angles per CTA); the partial sums of the angle groups
     // are added into a zeroed output
@@ -278,9 +277,7 @@ static cudaError_t bp_launch(cp4d_ctx *c, const float4 *gt, float *f_out, const 
         c->launches++;
     }
     b.n_work = (int)(ctas * b.agroups);
-    // persistent: 2 CTAs per SM stay resident and leave the rest of every SM to the forward projector launched after it
-    const int grid = persistent ? std::min(b.n_work, 2 * 148) : b.n_work;
-    k_backproject<JQ><<<grid, BP_THREADS, 0, c->stream>>>(gt, f_out, b);
+    k_backproject<JQ><<<b.n_work, BP_THREADS, 0, c->stream>>>(gt, f_out, b);
     return cudaGetLastError();
 }
 
@@ -306,16 +303,14 @@ uint32_t bp_pattern_fl(int pat) {
 }
 
 // Q_override > 0: backproject Q_override float4 chunks per bin / voxel instead of the context's Q (cp4d_fbp)
-cudaError_t launch_backproject(cp4d_ctx *c, const float4 *gt, float *f_out, int Q_override, bool persistent) {
+cudaError_t launch_backproject(cp4d_ctx *c, const float4 *gt, float *f_out, int Q_override) {
     ProfScope ps(c, CP4D_K_BACKPROJECT);
     const Dims &d = c->d;
     const int Q = Q_override > 0 ? Q_override : d.Q;
-    gt += (size_t)c->zs * d.n0 * Q * d.gp;                 // the context's z-window
-    f_out += (size_t)c->zs * d.n * d.n * Q * 4;
-    BpArgs a{d.n, c->nzs, d.nd, d.n0, Q, d.gp, d.gpl, c->n_cpos, 0, d.tiles, 1, c->ang, c->geo};
+    BpArgs a{d.n, d.nz, d.nd, d.n0, Q, d.gp, d.gpl, c->n_cpos, 0, d.tiles, 1, c->ang, c->geo};
     c->launches++;
-    if (Q % 2 == 0) return bp_launch<2>(c, gt, f_out, a, persistent);
-    return bp_launch<1>(c, gt, f_out, a, persistent);
+    if (Q % 2 == 0) return bp_launch<2>(c, gt, f_out, a);
+    return bp_launch<1>(c, gt, f_out, a);
 }
 
 }  // namespace cp4d

@@ -75,12 +75,7 @@ struct cp4d_ctx {
     int32_t *fworder;          // [n0]: base angles whose rays step over columns first, then the others
     int n_colstep;             // how many of the former
     // one CP iteration captured as a CUDA graph (cp4d_iterate replays it; rebuilt when tau / sigma change).  Not available on
-    // the legacy default stream, which cannot be captured: the launches are then issued one by one.
-    // z-window of the projector launches (forward_partial, synth, fold, backproject): slices [zs, zs + nzs); the whole volume
-    // except inside the pipelined iteration ("forward and backprojection side by side")
-    int zs, nzs;
-    cudaStream_t side;           // high-priority helper stream of the pipelined iteration, and its fork / join events
-    cudaEvent_t ev_slab[8], ev_join;
+    // the legacy default stream, which cannot be captured: the launches are then issued one by one, and `note` says why.
     cudaGraphExec_t iter_graph;
     uint64_t iter_graph_launches, graph_replays;
     bool iter_graph_off;
@@ -89,7 +84,8 @@ struct cp4d_ctx {
     cp4d::TileGeo *geo;        // [tile][n0]
     double *red;               // 8 doubles for reductions
     uint64_t launches;
-    std::string err;
+    std::string err;             // text of the last error (cp4d_last_error)
+    std::string note;            // why cp4d_iterate is not replaying a CUDA graph, if it is not (cp4d_graph_note)
     // per-kernel event timing (cp4d_profile_begin/end)
     bool prof_on;
     struct ProfRec { int cls; cudaEvent_t a, b; };
@@ -135,7 +131,8 @@ cudaError_t launch_synth(cp4d_ctx *c, const float4 *P, int mode, float sigma, co
 FwTable *fwtable_new(const FwAngle *ang, const int32_t *order, int n0);   // null when n0 is too large
 void fwtable_free(FwTable *t);
 cudaError_t launch_forward_partial(cp4d_ctx *c, const float *f, float4 *P);
-cudaError_t launch_backproject(cp4d_ctx *c, const float4 *gt, float *f_out, int Q_override = 0, bool persistent = false);
+cudaError_t forward_init();        // once per process and device: opt in to the forward kernels' dynamic shared memory
+cudaError_t launch_backproject(cp4d_ctx *c, const float4 *gt, float *f_out, int Q_override = 0);
 // cp4d_fbp: Shepp-Logan filter along the bins; per-half-rotation rows gathered into the projector scratch (box basis)
 cudaError_t launch_filter_sl(cp4d_ctx *c, const float *g, float *gf);
 cudaError_t launch_fold_halfrot(cp4d_ctx *c, const float *gf, float4 *gt, int Qf, float scale);

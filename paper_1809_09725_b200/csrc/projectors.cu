@@ -171,15 +171,24 @@ static cudaError_t fwd_launch_rays(cp4d_ctx *c, const float *f, float4 *P, const
         if (cost < best) { best = cost; b.agroups = ag; }
     }
     const dim3 grid(d.tiles * b.agroups, nzz, d.Q / JQ);
-    cudaError_t e;
-    if (d.n0 <= FW_TAB) {
-        if ((e = cudaFuncSetAttribute(k_forward_rays<JQ, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sh)) != cudaSuccess) return e;
+    if (d.n0 <= FW_TAB)
         k_forward_rays<JQ, true><<<grid, FR_THREADS, sh, c->stream>>>(f, P, b, *c->fwtab_host);
-    } else {
-        if ((e = cudaFuncSetAttribute(k_forward_rays<JQ, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sh)) != cudaSuccess) return e;
+    else
         k_forward_rays<JQ, false><<<grid, FR_THREADS, sh, c->stream>>>(f, P, b, FwTable{});
-    }
     return cudaGetLastError();
+}
+
+template <int JQ>
+static cudaError_t fwd_init_one() {
+    cudaError_t e = cudaFuncSetAttribute(k_forward_rays<JQ, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FwRays<JQ>::SMEM);
+    if (e != cudaSuccess) return e;
+    return cudaFuncSetAttribute(k_forward_rays<JQ, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FwRays<JQ>::SMEM);
+}
+// cp4d_create calls this once per context (the attribute is per device and sticks)
+cudaError_t forward_init() {
+    cudaError_t e;
+    if ((e = fwd_init_one<4>()) != cudaSuccess || (e = fwd_init_one<2>()) != cudaSuccess) return e;
+    return fwd_init_one<1>();
 }
 
 static int pick_jq(int Q) { return (Q % 4 == 0) ? 4 : (Q % 2 == 0) ? 2 : 1; }
@@ -195,11 +204,8 @@ void fwtable_free(FwTable *t) { delete t; }
 cudaError_t launch_forward_partial(cp4d_ctx *c, const float *f, float4 *P) {
     ProfScope ps(c, CP4D_K_FORWARD);
     const Dims &d = c->d;
-    // the context's z-window: slices are independent, so a window is the same launch on offset pointers
-    f += (size_t)c->zs * d.n * d.n * d.Q * 4;
-    P += (size_t)c->zs * d.n0 * d.Q * d.gp;
-    ProjArgs a{d.n, c->nzs, d.nd, d.n0, d.Q, d.gp, d.gpl, c->geo, c->fwang, c->fworder, c->n_colstep, d.tiles, 1};
-    cudaError_t e = cudaMemsetAsync(P, 0, (size_t)c->nzs * d.n0 * d.Q * d.gp * sizeof(float4), c->stream);
+    ProjArgs a{d.n, d.nz, d.nd, d.n0, d.Q, d.gp, d.gpl, c->geo, c->fwang, c->fworder, c->n_colstep, d.tiles, 1};
+    cudaError_t e = cudaMemsetAsync(P, 0, (size_t)d.nz * d.n0 * d.Q * d.gp * sizeof(float4), c->stream);
     if (e != cudaSuccess) return e;
     c->launches += 2;
     switch (pick_jq(d.Q)) {

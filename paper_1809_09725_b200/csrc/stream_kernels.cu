@@ -422,9 +422,7 @@ cudaError_t launch_fold(cp4d_ctx *c, const float *g, float4 *gt) {
     ProfScope ps(c, CP4D_K_FOLD);
     const Dims &d = c->d;
     const size_t sh = (size_t)d.npi * d.m * sizeof(float);
-    g += (size_t)c->zs * d.na * d.nd;                       // the context's z-window
-    gt += (size_t)c->zs * d.n0 * d.Q * d.gp;
-    CP4D_DISPATCH_Q(d.Q, (k_fold<QQ><<<c->nzs * d.n0, 128, sh, c->stream>>>(g, gt, c->phi, d.nd, d.na, d.npi, d.n0, d.gp, d.gpl)));
+    CP4D_DISPATCH_Q(d.Q, (k_fold<QQ><<<d.nz * d.n0, 128, sh, c->stream>>>(g, gt, c->phi, d.nd, d.na, d.npi, d.n0, d.gp, d.gpl)));
     c->launches++;
     return cudaGetLastError();
 }
@@ -432,11 +430,7 @@ cudaError_t launch_synth(cp4d_ctx *c, const float4 *P, int mode, float sigma, co
     ProfScope ps(c, CP4D_K_SYNTH);
     const Dims &d = c->d;
     const size_t sh = (size_t)d.npi * d.m * sizeof(float);
-    const size_t so = (size_t)c->zs * d.na * d.nd;         // the context's z-window
-    P += (size_t)c->zs * d.n0 * d.Q * d.gp;
-    if (g) g += so;
-    out += so;
-    CP4D_DISPATCH_Q(d.Q, (k_synth<QQ><<<c->nzs * d.n0, 128, sh, c->stream>>>(P, mode, sigma, g, out, c->phi, d.nd, d.na, d.npi, d.n0, d.gp, d.gpl)));
+    CP4D_DISPATCH_Q(d.Q, (k_synth<QQ><<<d.nz * d.n0, 128, sh, c->stream>>>(P, mode, sigma, g, out, c->phi, d.nd, d.na, d.npi, d.n0, d.gp, d.gpl)));
     c->launches++;
     return cudaGetLastError();
 }

@@ -71,10 +71,12 @@ class SlabSolver:
         return self._st[i - 1]["h2"][2, -1] if i > 0 else None
 
     def split(self, t):
-        """Per-slab contiguous pieces of a tensor whose first axis is z (axis 1 for dual tensors [4][z]...)."""
-        if t.shape[0] == self.nz:
-            return [t[z0:z1].contiguous() for z0, z1 in self.ranges]
-        return [t[:, z0:z1].contiguous() for z0, z1 in self.ranges]
+        """Per-slab contiguous pieces of a tensor whose first axis is z: primal [z][y][x][j] and sinogram [z][k][b] tensors; dual
+        tensors [4][z][y][x][j] (5 axes) are cut along axis 1.  Chosen by the number of axes, never by comparing sizes (nz = 4
+        would be ambiguous)."""
+        if t.dim() == 5:
+            return [t[:, z0:z1].contiguous() for z0, z1 in self.ranges]
+        return [t[z0:z1].contiguous() for z0, z1 in self.ranges]
 
     def set_data(self, g):
         for c, gs in zip(self.ctx, self.split(g)):

@@ -57,6 +57,17 @@ def test_host_validation(L, bad):
     assert L.cp4d_workspace_bytes(C.byref(p), C.byref(out)) == binding.EINVAL
 
 
+def test_phi_slice_must_fit_shared_memory(L):
+    """k_fold / k_synth stage the n_half_rot x m slice of Phi in 48 KB of shared memory: larger products are refused at
+    validation instead of failing at the first launch."""
+    from paper_1809_09725_b200 import binding
+    out = C.c_uint64(0)
+    ok = binding.make_params(n=32, nz=1, nd=32, n_angles=384 * 2, n_half_rot=384, m=32)
+    assert L.cp4d_workspace_bytes(C.byref(ok), C.byref(out)) == binding.OK
+    bad = binding.make_params(n=32, nz=1, nd=32, n_angles=385 * 2, n_half_rot=385, m=32)
+    assert L.cp4d_workspace_bytes(C.byref(bad), C.byref(out)) == binding.EINVAL
+
+
 def test_frame_mode_workspace(L):
     """Frame mode (n_frames > 0).  N_t <= M collapses to a coefficient-mode problem with N_t planes (the projector pair carries
     the frames); N_t > M keeps M-plane coefficient stacks beside the N_t-plane state plus the Psi table."""

@@ -78,3 +78,35 @@ def test_json_line_contract_offline():
     assert rf["smem_roof"]["frac"] == pytest.approx(4 * rf["frac"] * (148 * 128 * 2 * r["peaks"]["sm_max_mhz"] * 1e6 / 1e12) / rf["peak"], rel=1e-6)
     hbm = line["kernels"]["prox_f2"]
     assert hbm["bound"] == "hbm" and hbm["achieved"] == pytest.approx(9 * c.V * 4 / 0.76e-3 / 1e9)
+
+
+def _run_bench(argv, env_extra=None):
+    import subprocess
+    env = {k: v for k, v in os.environ.items() if k not in ("WORLD_SIZE", "RANK", "LOCAL_RANK")}
+    env.update(env_extra or {})
+    return subprocess.run([sys.executable, str(ROOT / "bench.py"), *argv], env=env, capture_output=True, text=True, timeout=300)
+
+
+def test_gpus_n_without_enough_devices_exits_nonzero():
+    """`python bench.py --gpus N` starts N ranks itself; with fewer than N CUDA devices it must refuse, not print an N = 1 line."""
+    import torch
+    if torch.cuda.device_count() >= 2:
+        pytest.skip("box has >= 2 GPUs")
+    r = _run_bench(["--gpus", "2", "--steps", "1"])
+    assert r.returncode != 0 and r.stdout.strip() == "" and "--gpus 2" in r.stderr
+
+
+def test_gpus_n_disagreeing_with_world_size_exits_nonzero():
+    r = _run_bench(["--gpus", "2", "--steps", "1"], {"WORLD_SIZE": "4", "RANK": "0"})
+    assert r.returncode != 0 and r.stdout.strip() == "" and "WORLD_SIZE=4" in r.stderr
+
+
+def test_traffic_is_tied_to_the_kernel_sources():
+    """profiles/traffic.json carries the SHA-1 of csrc/ it was captured with; bench.py reports its numbers only on a match."""
+    import json
+    sys.path.insert(0, str(ROOT))
+    import bench
+    sha = bench.csrc_sha1()
+    assert len(sha) == 40 and sha == bench.csrc_sha1()
+    tj = json.loads((ROOT / "profiles" / "traffic.json").read_text())
+    assert "csrc_sha1" in tj

@@ -175,6 +175,44 @@ def test_power_iteration(torch_cuda, fast_oracle, case):
     ctx.close()
 
 
+@pytest.mark.parametrize("case", ["cfg1", "cfg2", "ragged_m16", "ragged"])
+def test_power_iteration_same_start(torch_cuda, fast_oracle, case):
+    """cp4d_norm_start takes the oracle's start vector: the two power iterations are compared step for step (12 steps, no
+    convergence needed -- the m = 16 case above that two different starts cannot settle is a parity case this way)."""
+    c, P, ctx = make(case, fast_oracle)
+    x0 = synth.rng(c.cfg, 3).standard_normal(P.primal_shape).astype(np.float32)
+    for steps in (1, 12):
+        L_ref, _ = P.power(x0.astype(np.float64), steps, folded=True)
+        L = ctx.norm_start(dev(torch_cuda, x0), steps)
+        assert abs(L - L_ref) <= 1e-5 * L_ref, (steps, L, L_ref)
+    from paper_1809_09725_b200 import binding
+    with pytest.raises(binding.Cp4dError):
+        ctx.norm_start(torch_cuda.zeros(P.primal_shape, device="cuda"), 3)       # a zero start vector is refused
+    ctx.close()
+
+
+def test_graph_note_and_device_restored(torch_cuda, fast_oracle):
+    """cp4d_iterate on the legacy default stream cannot replay a graph: it must say so (cp4d_graph_note), not fall back silently;
+    and no call leaves another device current than the caller's."""
+    torch = torch_cuda
+    from paper_1809_09725_b200 import binding
+    c = CASES["cfg1"]
+    phi = synth.basis_table(c.basis, c.m, c.n_angles)
+    g = dev(torch, _data(c))
+    cur = torch.cuda.current_device()
+    with torch.cuda.stream(torch.cuda.default_stream()):
+        ctx = binding.Context.from_config(c, phi=phi)
+        ctx.set_data(g); ctx.set_steps(0.01, 0.01); ctx.reset(); ctx.iterate(3); ctx.sync()
+        assert ctx.graph_replays() == 0 and "legacy default stream" in ctx.graph_note()
+        ctx.close()
+    with torch.cuda.stream(torch.cuda.Stream()):
+        ctx = binding.Context.from_config(c, phi=phi)
+        ctx.set_data(g); ctx.set_steps(0.01, 0.01); ctx.reset(); ctx.iterate(3); ctx.sync()
+        assert ctx.graph_replays() == 3 and ctx.graph_note() == ""
+        ctx.close()
+    assert torch.cuda.current_device() == cur
+
+
 def test_solve_host_equals_device_path(torch_cuda, fast_oracle):
     c, P, ctx = make("cfg1", fast_oracle)
     g = _data(c).astype(np.float32)
