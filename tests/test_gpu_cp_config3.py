@@ -48,7 +48,8 @@ def problem(torch_cuda, fast_oracle):
     c = synth.CONFIGS[3]
     phi = synth.basis_table(c.basis, c.m, c.n_angles)
     P = fast_oracle.Problem.from_config(c, phi=phi)
-    ctx = binding.Context.from_config(c, phi=phi)
+    with torch_cuda.cuda.stream(torch_cuda.cuda.Stream()):      # a capturable stream: cp4d_iterate replays its CUDA graph, as in bench.py
+        ctx = binding.Context.from_config(c, phi=phi)
     g32 = synth.sinogram(c).numpy().astype(np.float32)          # both sides get the fp32-rounded data
     yield c, P, ctx, g32
     ctx.close()
@@ -67,7 +68,8 @@ def test_power_iteration_same_start(torch_cuda, problem):
     t0 = time.perf_counter()
     L_ref, _ = P.power(x0.astype(np.float64), N_POWER, folded=True)
     t_or = time.perf_counter() - t0
-    L = ctx.norm_start(_dev(torch_cuda, x0), N_POWER)
+    xd = _dev(torch_cuda, x0)
+    L = ctx.norm_start(xd, N_POWER)
     print(f"config 3 power iteration, {N_POWER} steps from the same start: oracle {L_ref:.6f} ({t_or:.0f} s), gpu {L:.6f}")
     assert abs(L - L_ref) <= 1e-4 * L_ref
     # the step sizes bench.py uses rest on 30 steps from the library's own start vector: the estimates grow with the step count
@@ -85,7 +87,8 @@ def test_cp_20_iterations_config_lambda(torch_cuda, problem):
     n_it = 20
     L = ctx.norm(30, seed=3)
     ts = float(np.float32(0.95 / L))
-    ctx.set_data(_dev(torch, g32)); ctx.set_steps(ts, ts); ctx.reset(); ctx.iterate(n_it); ctx.sync()
+    gd = _dev(torch, g32)                                          # kept alive until the sync: the context runs on its own stream
+    ctx.set_data(gd); ctx.set_steps(ts, ts); ctx.reset(); ctx.iterate(n_it); ctx.sync()
     assert ctx.graph_replays() > 0, ctx.graph_note()
     st = P.zero_state()
     t0 = time.perf_counter()
@@ -117,7 +120,8 @@ def test_cp_mixed_branches(torch_cuda, problem):
     P.lambda1 = c.lambda1
     frac = ncl / P.V
     ctx2 = type(ctx).from_config(c, phi=synth.basis_table(c.basis, c.m, c.n_angles), lambda1=lam)
-    ctx2.set_data(_dev(torch, g32)); ctx2.set_steps(ts, ts); ctx2.reset(); ctx2.iterate(4); ctx2.sync()
+    gd = _dev(torch, g32)
+    ctx2.set_data(gd); ctx2.set_steps(ts, ts); ctx2.reset(); ctx2.iterate(4); ctx2.sync()
     s = ctx2.state()
     errs = {k: rel(s[k].cpu().numpy(), st[k]) for k in ("f", "ft", "h1", "h2")}
     print(f"config 3, 4 CP iterations, lambda1 = {lam:.4g}: clamp fraction at the last step {frac:.3f}, rel-L2 {errs}")
