@@ -113,6 +113,19 @@ int cp4d_grad(cp4d_ctx *ctx, const float *f_dev, float *p_dev);
 /* f = div p = -K2^T p (L131-L133).  p: 4V, f: V. */
 int cp4d_div(cp4d_ctx *ctx, const float *p_dev, float *f_dev);
 
+/* Which forward projector cp4d_forward / cp4d_prox_f1 / cp4d_iterate / cp4d_norm launch.  Both compute the same ray sums
+ * (Eq. 9 with the Joseph weights above); they differ in the arithmetic of the products:
+ *   CP4D_FORWARD_AUTO (default): the tensor-core kernel where it applies (m = 4, 8, 16 or 32), else the fp32 one.  Voxel
+ *       values and interpolation weights enter mma.sync as split bf16 pairs (x = x_hi + x_lo), three products per term,
+ *       fp32 accumulation: relative error about 1e-5 per ray sum, inside the 1e-4 per-operator tolerance.
+ *   CP4D_FORWARD_FP32: the CUDA-core gather, plain fp32 FMAs (relative error about 2e-6), 2-3 x slower.
+ * The adjoint is fp32 in both modes.  Changing the mode drops the captured CUDA graph of cp4d_iterate. */
+#define CP4D_FORWARD_AUTO   0
+#define CP4D_FORWARD_FP32   1
+#define CP4D_FORWARD_TENSOR 2   /* reported by cp4d_forward_mode_in_use only */
+int cp4d_set_forward_mode(cp4d_ctx *ctx, int32_t mode);
+int cp4d_forward_mode_in_use(const cp4d_ctx *ctx, int32_t *mode_out_host);
+
 /* ---- the three fused steps of Fig. 2 on caller-owned DEVICE buffers --------------------------- */
 /* step 3 (L154, L135): h1 <- (h1 + sigma (K1 ft - g)) / (1 + sigma).   h1 in/out (S), ft: V, g: S. */
 int cp4d_prox_f1(cp4d_ctx *ctx, float sigma, const float *ft_dev, const float *g_dev, float *h1_dev);

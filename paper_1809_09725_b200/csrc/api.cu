@@ -53,7 +53,7 @@ int validate(const cp4d_params *p, Dims *d) {
 }
 
 struct Carve {
-    uint64_t f, ft, bp, h2, h1, g, tmp_s, scratch, phi, ang, geo, red, cf, cb, psi, fwang, fworder, total;
+    uint64_t f, ft, bp, h2, h1, g, tmp_s, scratch, phi, ang, geo, red, cf, cb, psi, fwang, fworder, fwpairs, total;
 };
 Carve carve(const Dims &d) {
     Carve c;
@@ -64,6 +64,7 @@ Carve carve(const Dims &d) {
     c.phi = take((uint64_t)d.m * d.na * 4); c.ang = take((uint64_t)d.n0 * sizeof(AngleTab));
     c.geo = take((uint64_t)d.tiles * d.n0 * sizeof(TileGeo)); c.red = take(64);
     c.fwang = take((uint64_t)d.n0 * sizeof(FwAngle)); c.fworder = take((uint64_t)d.n0 * 4);
+    c.fwpairs = take((uint64_t)d.n0 * sizeof(int2));
     c.cf = c.cb = c.psi = 0;
     if (d.nf) { c.cf = take(d.Vc * 4); c.cb = take(d.Vc * 4); c.psi = take((uint64_t)d.mb * d.nf * 4); }
     c.total = o;
@@ -186,6 +187,7 @@ int cp4d_create(const cp4d_params *p, cp4d_ctx **out) {
     ctx->h2 = (float *)(w + cv.h2); ctx->h1 = (float *)(w + cv.h1); ctx->g = (float *)(w + cv.g);
     ctx->tmp_s = (float *)(w + cv.tmp_s);
     ctx->fwang = (FwAngle *)(w + cv.fwang); ctx->fworder = (int32_t *)(w + cv.fworder);
+    ctx->fw_pairs = (int2 *)(w + cv.fwpairs); ctx->fw_mode = CP4D_FORWARD_AUTO;
     ctx->cf = d.nf ? (float *)(w + cv.cf) : nullptr; ctx->cb = d.nf ? (float *)(w + cv.cb) : nullptr;
     ctx->psi = d.nf ? (float *)(w + cv.psi) : nullptr;
     ctx->scratch = (float4 *)(w + cv.scratch); ctx->phi = (float *)(w + cv.phi);
@@ -223,6 +225,8 @@ int cp4d_create(const cp4d_params *p, cp4d_ctx **out) {
     }
     for (int i = 0; i < d.n0; ++i) fwang[i] = FwAngle{ang[i].fw_inv, ang[i].fw_step, ang[i].fw_istep, ang[i].inv_a};
     ctx->fwtab_host = fwtable_new(fwang.data(), fworder.data(), d.n0);
+    std::vector<int2> fwpairs(d.n0);
+    forward_mma_pairs(fwang.data(), fworder.data(), d.n0, ctx->n_colstep, fwpairs.data(), &ctx->n_pairs0, &ctx->n_pairs1);
     std::vector<TileGeo> geo((size_t)d.tiles * d.n0);
     const double cen = 0.5 * (d.n - 1), cd = 0.5 * (d.nd - 1);
     for (int t = 0; t < d.tiles; ++t) {
@@ -260,6 +264,7 @@ int cp4d_create(const cp4d_params *p, cp4d_ctx **out) {
         (e = cudaMemcpyAsync(ctx->ang, ang.data(), ang.size() * sizeof(AngleTab), cudaMemcpyHostToDevice, ctx->stream)) != cudaSuccess ||
         (e = cudaMemcpyAsync(ctx->fwang, fwang.data(), fwang.size() * sizeof(FwAngle), cudaMemcpyHostToDevice, ctx->stream)) != cudaSuccess ||
         (e = cudaMemcpyAsync(ctx->fworder, fworder.data(), fworder.size() * 4, cudaMemcpyHostToDevice, ctx->stream)) != cudaSuccess ||
+        (e = cudaMemcpyAsync(ctx->fw_pairs, fwpairs.data(), fwpairs.size() * sizeof(int2), cudaMemcpyHostToDevice, ctx->stream)) != cudaSuccess ||
         (e = cudaMemcpyAsync(ctx->geo, geo.data(), geo.size() * sizeof(TileGeo), cudaMemcpyHostToDevice, ctx->stream)) != cudaSuccess ||
         (e = cudaMemsetAsync(ctx->scratch, 0, (size_t)d.scratch4 * 16, ctx->stream)) != cudaSuccess ||
         (e = cudaStreamSynchronize(ctx->stream)) != cudaSuccess) {
@@ -694,6 +699,24 @@ const char *cp4d_kernel_name(int k) {
 int cp4d_graph_replays(const cp4d_ctx *ctx, uint64_t *out) {
     if (!ctx || !out) return CP4D_EINVAL;
     *out = ctx->graph_replays;
+    return CP4D_OK;
+}
+
+int cp4d_set_forward_mode(cp4d_ctx *ctx, int32_t mode) {
+    if (!ctx) return CP4D_EINVAL;
+    if (mode != CP4D_FORWARD_AUTO && mode != CP4D_FORWARD_FP32) return fail(ctx, CP4D_EINVAL, "set_forward_mode: unknown mode");
+    if (mode != ctx->fw_mode && ctx->iter_graph) {      // the captured iteration holds the other kernel
+        DevGuard dev_guard(ctx->device);
+        cudaGraphExecDestroy(ctx->iter_graph);
+        ctx->iter_graph = nullptr;
+    }
+    ctx->fw_mode = mode;
+    return CP4D_OK;
+}
+
+int cp4d_forward_mode_in_use(const cp4d_ctx *ctx, int32_t *mode_out) {
+    if (!ctx || !mode_out) return CP4D_EINVAL;
+    *mode_out = (ctx->fw_mode != CP4D_FORWARD_FP32 && forward_mma_supported(ctx->d)) ? CP4D_FORWARD_TENSOR : CP4D_FORWARD_FP32;
     return CP4D_OK;
 }
 

@@ -80,6 +80,9 @@ struct cp4d_ctx {
     uint64_t iter_graph_launches, graph_replays;
     bool iter_graph_off;
     cp4d::FwTable *fwtab_host; // host copy of fwang / fworder for the kernel-parameter path (n0 <= 512), else null
+    int2 *fw_pairs;            // tensor-core forward projector (forward_mma.cu): base angles of each pass paired with a neighbour
+    int n_pairs0, n_pairs1;
+    int fw_mode;               // CP4D_FORWARD_AUTO / _FP32 (cp4d_set_forward_mode)
     int n_cpos;                // the first n_cpos base angles have cos >= 0 (backprojector: chunks never mix the signs)
     cp4d::TileGeo *geo;        // [tile][n0]
     double *red;               // 8 doubles for reductions
@@ -132,6 +135,11 @@ FwTable *fwtable_new(const FwAngle *ang, const int32_t *order, int n0);   // nul
 void fwtable_free(FwTable *t);
 cudaError_t launch_forward_partial(cp4d_ctx *c, const float *f, float4 *P);
 cudaError_t forward_init();        // once per process and device: opt in to the forward kernels' dynamic shared memory
+// forward_mma.cu: the tensor-core forward projector (split-bf16 HMMA, fp32 accumulate)
+bool forward_mma_supported(const Dims &d);
+cudaError_t forward_mma_init();
+int forward_mma_pairs(const FwAngle *fw, const int32_t *order, int n0, int n_colstep, int2 *out, int *npairs0, int *npairs1);
+cudaError_t launch_forward_mma(cp4d_ctx *c, const float *f, float *P);
 cudaError_t launch_backproject(cp4d_ctx *c, const float4 *gt, float *f_out, int Q_override = 0);
 // cp4d_fbp: Shepp-Logan filter along the bins; per-half-rotation rows gathered into the projector scratch (box basis)
 cudaError_t launch_filter_sl(cp4d_ctx *c, const float *g, float *gf);

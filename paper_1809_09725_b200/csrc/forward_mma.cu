@@ -1,0 +1,363 @@
+// Forward projector on the tensor cores (Eq. 9, with the pi-fold of L198-L202): the Joseph ray sums of all
+// coefficients over the base angles, as small dense products  D[16 batch entries x 8 rays] += F[16 x 16 voxels] * W[16 voxels x 8 rays].
+//
+// Why.  The CUDA-core gather (projectors.cu) needs one shared-memory word per FMA and sits on the LSU data pipe at 0.19 of
+// the FP32 peak.  The interpolation weights do not depend on the slice or on the coefficient, so the batch axis (slice, j) is
+// a dense axis: a block of 16 voxels along a short column segment times the 2-nonzeros-per-ray weight block is a real matrix
+// product.  mma.sync (HMMA.16816) measured 950 MAC/clk/SM on B200, 7.4x the FP32 FMA rate, and it does not touch the LSU pipe
+// beyond one ldmatrix per 16 x 16 operand -- so a weight block that is 1/4 dense still wins.
+//
+// Block shape.  K = 16 voxels = 2 adjacent columns (of the stepping axis) x 8 consecutive rows; N = 8 rays = 4 adjacent bins of
+// each of TWO adjacent base angles (a "strip pair"); M = 16 batch entries = (slices x coefficients) of one voxel.  Four bins of
+// one angle span at most 3*sqrt2 + 2 rows at a column, and the rays of the neighbouring angle that lie in the same strip of the
+// detector stay within one more row of them, so an 8-row window per column holds every tap: 32 of the 128 weights are
+// non-zero.  Windows are clamped to the tile, so taps outside the tile (which belong to other tiles) simply have no row.
+// When the two angles are too far apart for one window (coarse angular sampling), or the pairing leaves five bins of the
+// second angle in a strip, the unit is processed as two single-angle units -- a warp-uniform decision, never a wrong result.
+//
+// Precision.  Operands are split bf16 pairs: F = Fh + Fl (tile, once per CTA), W = Wh + Wl (per weight), and
+// D += Fh Wh + Fl Wh + Fh Wl with fp32 accumulation: relative error about 3 * 2^-18 = 1.1e-5 per product, inside the 1e-4
+// per-operator tolerance.  cp4d_set_forward_mode selects the exact-fp32 gather instead.
+//
+// Work split.  CTA = (32 x 32 tile, pass, group of NB16 16-entry batch blocks); pass 0 = base angles whose rays step over
+// columns, pass 1 = the others on the transposed tile, so one code path serves both.  The tile sits in shared memory as
+// [block][hi/lo][8-entry half][column][row] x 16 B, which makes every 8 x 8 ldmatrix operand 128 contiguous bytes.  Warps
+// draw units (angle pair, strip) from a shared counter; partial ray sums go to P[z][i][b][j] with scalar REDs (32-byte
+// runs of 8 coefficients per bin).
+#include <cuda_bf16.h>
+
+#include <algorithm>
+#include <cmath>
+
+#include "cp4d_internal.cuh"
+
+namespace cp4d {
+
+namespace {
+
+static_assert(TILE == 32, "the tile staging decodes indices with shifts for TILE = 32");
+constexpr int FM_THREADS = 512;
+constexpr int FM_WARPS = FM_THREADS / 32;
+constexpr int FM_STRIPS = WIN / 4 + 2;                 // strips -1 .. WIN/4 of four window bins
+constexpr int FM_PLANE = 2 * TILE * TILE * 16;         // bytes of one (block, hi/lo) plane: [half][column][row] x 16 B
+constexpr float FM_KC = 0.5f * (TILE - 1);             // reference column where the two angles of a pair are aligned
+constexpr float FM_SPAN = 5.99f;                       // largest spread of first-tap rows an 8-row window holds
+constexpr int FM_STG = 20;                             // floats per ray of a warp's 8 x 16 epilogue patch (20: conflict-free stores)
+
+struct FmArgs {
+    int n, nz, nd, n0, m, mshift, gp, gpl;
+    int tiles, agroups;
+    int zper;                  // slices per CTA = NB16 * 16 / m
+    float margin;              // bins a ray of the second angle of a pair can sit from the first angle's bin of its touch point
+    const TileGeo *geo;
+    const FwAngle *fwang;
+    const int2 *pairs;         // [pass 0 pairs | pass 1 pairs]: (ia, ib), |inv(ib)| >= |inv(ia)|, ib = -1 for a single angle
+    int npairs0, npairs1;
+};
+
+__device__ __forceinline__ void mma16816(float (&d)[4], const unsigned (&a)[4], unsigned b0, unsigned b1) {
+    asm volatile("mma.sync.aligned.m16n8k16.row.col.f32.bf16.bf16.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};\n"
+                 : "+f"(d[0]), "+f"(d[1]), "+f"(d[2]), "+f"(d[3])
+                 : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(b0), "r"(b1));
+}
+__device__ __forceinline__ void ldsm4t(unsigned (&a)[4], unsigned addr) {
+    asm volatile("ldmatrix.sync.aligned.m8n8.x4.trans.shared.b16 {%0,%1,%2,%3}, [%4];\n"
+                 : "=r"(a[0]), "=r"(a[1]), "=r"(a[2]), "=r"(a[3]) : "r"(addr));
+}
+// (x, y) -> bf16 pairs hi, lo with x = hi.x + lo.x + O(2^-18 x); low half = first element
+__device__ __forceinline__ void split2(float x, float y, unsigned &hi, unsigned &lo) {
+    const __nv_bfloat162 h = __floats2bfloat162_rn(x, y);
+    const __nv_bfloat162 l = __floats2bfloat162_rn(x - __low2float(h), y - __high2float(h));
+    hi = *reinterpret_cast<const unsigned *>(&h);
+    lo = *reinterpret_cast<const unsigned *>(&l);
+}
+
+// per-CTA record of one angle pair (shared memory): the per-angle tables and this tile's window geometry, plus what the
+// strip bookkeeping needs, so that a unit's setup is a handful of FMAs
+struct FmPair {
+    float inv0, step0, delta0, inva0;     // angle 0 (the one with the smaller |1/ss|): 1/ss, -cc/ss, window offset, 1/a
+    float inv1, step1, delta1, inva1;     // angle 1 (= angle 0 for a single)
+    float r0, rinv1, istep0, istep1;      // angle-1 bin ub1 sits at angle-0 bin coordinate (ub1 - s0) / rinv1, s0 = -r0 rinv1, at the
+                                          // reference column; istep = 1/step (0 when the rays run along the columns)
+    int ia, ib, bstart0, bstart1;
+};
+constexpr int FM_MAXP = 128;               // pairs per chunk of a CTA's pair list
+
+// columns k in [0, TILE) where a ray group whose first-tap rows lie in [ylo + k st, yhi + k st] touches rows 0 .. TILE-1:
+// ylo + k st < TILE and yhi + k st > -1
+__device__ __forceinline__ void col_range(float ylo, float yhi, float st, float ist, int &klo, int &khi) {
+    if (ist != 0.0f) {
+        const float ka = ((float)TILE - ylo) * ist, kb = (-1.0f - yhi) * ist;     // st > 0: k < ka, k > kb; st < 0: reversed
+        klo = max(0, (int)floorf(st > 0.f ? kb : ka));
+        khi = min(TILE - 1, (int)ceilf(st > 0.f ? ka : kb));
+    } else if (ylo < (float)TILE && yhi > -1.0f) {
+        klo = 0; khi = TILE - 1;
+    } else {
+        klo = TILE; khi = -1;
+    }
+}
+
+template <int NB16>
+__global__ void __launch_bounds__(FM_THREADS, 1) k_forward_mma(const float *__restrict__ f, float *__restrict__ P, FmArgs a) {
+    extern __shared__ __align__(128) unsigned char tile[];     // [NB16][2][2][TILE][TILE] x 16 B
+    __shared__ int s_next, s_nunits;
+    __shared__ __align__(16) float s_stg[FM_WARPS][8 * FM_STG];
+    __shared__ __align__(16) FmPair s_pair[FM_MAXP];
+    __shared__ unsigned char s_t0[FM_MAXP], s_tn[FM_MAXP];      // first strip (+1) and number of strips of each pair
+    __shared__ unsigned short s_unit[FM_MAXP * FM_STRIPS];      // unit -> (pair << 4) | (strip + 1)
+    float *stg = s_stg[threadIdx.x >> 5];
+    const int tiles_1d = (a.n + TILE - 1) / TILE;
+    const int tile_id = blockIdx.x % a.tiles, ag = blockIdx.x / a.tiles;
+    const int pass = blockIdx.y & 1, z0 = (blockIdx.y >> 1) * a.zper;
+    const int x0 = (tile_id % tiles_1d) * TILE, y0 = (tile_id / tiles_1d) * TILE;
+
+    // ---- stage the tile: fp32 -> (hi, lo) bf16, pass coordinates (column = stepping axis) ----
+    for (int e = threadIdx.x; e < NB16 * 2 * TILE * TILE; e += FM_THREADS) {
+        const int row = e & (TILE - 1), kcol = (e >> 5) & (TILE - 1), jh = (e >> 10) & 1, zb = e >> 11;
+        const int gx = x0 + (pass ? row : kcol), gy = y0 + (pass ? kcol : row);
+        float v[8];
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {
+            const int flat = zb * 16 + jh * 8 + h * 4, sl = z0 + (flat >> a.mshift), j = flat & (a.m - 1);
+            float4 q = make_float4(0.f, 0.f, 0.f, 0.f);
+            if (gx < a.n && gy < a.n && sl < a.nz)
+                q = __ldg(reinterpret_cast<const float4 *>(f + (((int64_t)sl * a.n + gy) * a.n + gx) * a.m + j));
+            v[4 * h] = q.x; v[4 * h + 1] = q.y; v[4 * h + 2] = q.z; v[4 * h + 3] = q.w;
+        }
+        uint4 hi, lo;
+        split2(v[0], v[1], hi.x, lo.x); split2(v[2], v[3], hi.y, lo.y);
+        split2(v[4], v[5], hi.z, lo.z); split2(v[6], v[7], hi.w, lo.w);
+        unsigned char *dst = tile + (size_t)(zb * 2) * FM_PLANE + ((jh * TILE + kcol) * TILE + row) * 16;
+        *reinterpret_cast<uint4 *>(dst) = hi;
+        *reinterpret_cast<uint4 *>(dst + FM_PLANE) = lo;
+    }
+
+    // ---- this CTA's share of the pass's angle pairs, in chunks of FM_MAXP ----
+    const int pbeg = pass ? a.npairs0 : 0, pcnt = pass ? a.npairs1 : a.npairs0;
+    const int p0 = pbeg + (int)((int64_t)pcnt * ag / a.agroups), p1 = pbeg + (int)((int64_t)pcnt * (ag + 1) / a.agroups);
+    const int lane = threadIdx.x & 31, g = lane >> 2, t = lane & 3;
+    const unsigned tile_s = (unsigned)__cvta_generic_to_shared(tile);
+    // ldmatrix row address of this lane: matrix = lane / 8 -> (column k0 + matrix / 2, half matrix & 1), row lane & 7
+    const unsigned ld_half = (lane >> 3) & 1, ld_col = lane >> 4, ld_row = lane & 7;
+    const TileGeo *geo = a.geo + (int64_t)tile_id * a.n0;
+
+    for (int pc = p0; pc < p1; pc += FM_MAXP) {
+        const int npc = min(FM_MAXP, p1 - pc);
+        __syncthreads();                                     // the tile is staged / every warp is done with the previous chunk
+        if ((int)threadIdx.x < npc) {
+            const int2 pr = a.pairs[pc + threadIdx.x];
+            const FwAngle A0 = a.fwang[pr.x], A1 = a.fwang[pr.y >= 0 ? pr.y : pr.x];
+            const TileGeo G0 = geo[pr.x], G1 = geo[pr.y >= 0 ? pr.y : pr.x];
+            FmPair R;
+            R.inv0 = A0.inv; R.step0 = A0.step; R.delta0 = G0.delta; R.inva0 = A0.inv_a;
+            R.inv1 = A1.inv; R.step1 = A1.step; R.delta1 = G1.delta; R.inva1 = A1.inv_a;
+            // angle-1 ray ub1 sits, at the reference column, at angle-0 bin coordinate phi = r1 ub1 + r0
+            const float r1 = A1.inv / A0.inv;
+            R.r0 = (FM_KC * (A1.step - A0.step) - G1.delta * A1.inv) / A0.inv + G0.delta;
+            R.rinv1 = 1.0f / r1;
+            R.istep0 = fabsf(A0.step) > 1e-6f ? 1.0f / A0.step : 0.0f;
+            R.istep1 = fabsf(A1.step) > 1e-6f ? 1.0f / A1.step : 0.0f;
+            R.ia = pr.x; R.ib = pr.y; R.bstart0 = G0.bstart; R.bstart1 = G1.bstart;
+            s_pair[threadIdx.x] = R;
+            // strips that can hold a ray touching the tile: angle-0 window coordinates of the tile corners, widened by the
+            // distance an angle-1 ray can sit from the bin of its touch point at the reference column (a.margin)
+            const float ss = 1.0f / A0.inv, cc = -A0.step * ss, e = (float)(TILE - 1);
+            const float umin = G0.delta + fminf(0.f, e * cc) + fminf(0.f, e * ss), umax = G0.delta + fmaxf(0.f, e * cc) + fmaxf(0.f, e * ss);
+            const int tf = max(-1, (int)floorf((umin - a.margin + 0.5f) * 0.25f)), tl = min(FM_STRIPS - 2, (int)floorf((umax + a.margin + 0.5f) * 0.25f));
+            s_t0[threadIdx.x] = (unsigned char)(tf + 1);
+            s_tn[threadIdx.x] = (unsigned char)max(0, tl - tf + 1);
+        }
+        __syncthreads();
+        if (threadIdx.x < 32) {                              // unit table: pairs in order, their strips in order
+            int base = 0;
+            for (int q0 = 0; q0 < npc; q0 += 32) {
+                const int q = q0 + lane, n = q < npc ? s_tn[q] : 0;
+                int incl = n;
+#pragma unroll
+                for (int o = 1; o < 32; o <<= 1) {
+                    const int v = __shfl_up_sync(0xffffffffu, incl, o);
+                    if (lane >= o) incl += v;
+                }
+                for (int r = 0; r < n; ++r) s_unit[base + incl - n + r] = (unsigned short)((q << 4) | (s_t0[q] + r));
+                base += __shfl_sync(0xffffffffu, incl, 31);
+            }
+            if (lane == 0) { s_nunits = base; s_next = 0; }
+        }
+        __syncthreads();
+        const int n_units = s_nunits;
+
+        for (;;) {
+            int u = 0;
+            if (lane == 0) u = atomicAdd(&s_next, 1);
+            u = __shfl_sync(0xffffffffu, u, 0);
+            if (u >= n_units) break;
+            const unsigned uu = s_unit[u];
+            const FmPair R = s_pair[uu >> 4];
+            const int ts = (int)(uu & 15) - 1;
+            const float ft4 = 4.0f * (float)ts;
+            int b1s = 0, cnt1 = 0;
+            if (R.ib >= 0) {
+                // angle-1 bin ub1 belongs to the strip whose extent [4 ts - 0.5, 4 ts + 3.5) holds phi(ub1): the extents tile the
+                // line and both ends use the same expression, so every bin is in exactly one strip
+                b1s = (int)ceilf((ft4 - 0.5f - R.r0) * R.rinv1);
+                cnt1 = (int)ceilf((ft4 + 3.5f - R.r0) * R.rinv1) - b1s;
+            }
+            // first-tap row of window bin ub of angle x at column k:  (ub - delta) inv + k step
+            const float y00 = (ft4 - R.delta0) * R.inv0, y03 = fmaf(3.0f, R.inv0, y00);
+            const float y10 = ((float)b1s - R.delta1) * R.inv1, y11 = fmaf((float)(max(cnt1, 1) - 1), R.inv1, y10);
+            const float lo0 = fminf(y00, y03), hi0 = fmaxf(y00, y03), lo1 = fminf(y10, y11), hi1 = fmaxf(y10, y11);
+            int ka0, kb0, ka1 = TILE, kb1 = -1;
+            col_range(lo0, hi0, R.step0, R.istep0, ka0, kb0);
+            if (cnt1 > 0) col_range(lo1, hi1, R.step1, R.istep1, ka1, kb1);
+            // one window for both angles?  The spread of first-tap rows is convex in k: check the two end columns
+            bool pair_ok = cnt1 > 0 && cnt1 <= 4;
+            if (pair_ok) {
+                const float fa = (float)min(ka0, ka1), fb = (float)max(kb0, kb1);
+                const float sa = fmaxf(fmaf(fa, R.step0, hi0), fmaf(fa, R.step1, hi1)) - fminf(fmaf(fa, R.step0, lo0), fmaf(fa, R.step1, lo1));
+                const float sb = fmaxf(fmaf(fb, R.step0, hi0), fmaf(fb, R.step1, hi1)) - fminf(fmaf(fb, R.step0, lo0), fmaf(fb, R.step1, lo1));
+                pair_ok = sa < FM_SPAN && sb < FM_SPAN;
+            }
+            const int n_sub = (cnt1 > 0 && !pair_ok) ? 2 : 1;
+            for (int sub = 0; sub < n_sub; ++sub) {
+                // slot n of the 8 rays -> (angle, window bin).  pair: 0-3 angle 0, 4-7 angle 1; split: one angle, slots from 0
+                const bool use0 = pair_ok || cnt1 == 0 || sub == 0, use1 = pair_ok || (cnt1 > 0 && sub == 1);
+                int klo = TILE, khi = -1;
+                if (use0) { klo = min(klo, ka0); khi = max(khi, kb0); }
+                if (use1) { klo = min(klo, ka1); khi = max(khi, kb1); }
+                if (klo > khi) continue;                     // (warp-uniform) the strip misses the tile
+                // my ray (slot g): B column g of the weight block, and the ray whose sums I add to P in the end
+                const int off1 = pair_ok ? 4 : 0;            // first slot of angle 1
+                const int bang = (use1 && !(use0 && g < 4)) ? 1 : 0;
+                const int bub = bang ? b1s + g - off1 : 4 * ts + g;
+                const bool bok = (bang ? (g >= off1 && g - off1 < cnt1) : (use0 && g < 4)) && bub >= 0 && bub < WIN;
+                const float bstep = bang ? R.step1 : R.step0;
+                // rows of column k0 at k = 2t, 2t+1 and of column k0+1 at k = 2t+8, 2t+9: first-tap row relative to row q + 2t
+                const float byb = bok ? ((float)bub - (bang ? R.delta1 : R.delta0)) * (bang ? R.inv1 : R.inv0) - (float)(2 * t) : -1e6f;
+                // window line(s): lowest first-tap row of each angle in use
+                const float wl0 = use0 ? lo0 : 1e6f, wl1 = use1 ? lo1 : 1e6f;
+
+                float acc[NB16][4];
+#pragma unroll
+                for (int zb = 0; zb < NB16; ++zb) acc[zb][0] = acc[zb][1] = acc[zb][2] = acc[zb][3] = 0.f;
+
+                for (int k0 = klo & ~1; k0 <= khi; k0 += 2) {
+                    const float fk = (float)k0, fk1 = fk + 1.0f;
+                    // window start per column: floor of the lowest first-tap row, clamped into the tile
+                    const int qa = min(max((int)floorf(fminf(fmaf(fk, R.step0, wl0), fmaf(fk, R.step1, wl1))), 0), TILE - 8);
+                    const int qb = min(max((int)floorf(fminf(fmaf(fk1, R.step0, wl0), fmaf(fk1, R.step1, wl1))), 0), TILE - 8);
+                    // weights of my ray at rows q + 2t, q + 2t + 1 of both columns: Joseph hat max(0, 1 - |row - y|)
+                    const float da = fmaf(fk, bstep, byb) - (float)qa, db = fmaf(fk1, bstep, byb) - (float)qb;   // y - (q + 2t)
+                    const float w0 = __saturatef(1.0f - fabsf(da)), w1 = __saturatef(1.0f - fabsf(da - 1.0f));
+                    const float w2 = __saturatef(1.0f - fabsf(db)), w3 = __saturatef(1.0f - fabsf(db - 1.0f));
+                    unsigned bh0, bl0, bh1, bl1;
+                    split2(w0, w1, bh0, bl0);
+                    split2(w2, w3, bh1, bl1);
+                    const unsigned adr = tile_s + (((ld_half * TILE + k0 + ld_col) * TILE + (ld_col ? qb : qa) + ld_row) << 4);
+#pragma unroll
+                    for (int zb = 0; zb < NB16; ++zb) {
+                        unsigned ah[4], al[4];
+                        ldsm4t(ah, adr + zb * 2 * FM_PLANE);
+                        ldsm4t(al, adr + zb * 2 * FM_PLANE + FM_PLANE);
+                        mma16816(acc[zb], ah, bh0, bh1);
+                        mma16816(acc[zb], al, bh0, bh1);
+                        mma16816(acc[zb], ah, bl0, bl1);
+                    }
+                }
+                // ---- partial ray sums of this tile -> P[z][i][b][j].  My D entries are rays 2t, 2t+1 x batch entries g, g+8; a RED
+                // costs about one clock per LANE whatever its width, so the block goes through a per-warp shared-memory patch and
+                // leaves as one 16-byte RED per lane: lane (ray g, quad t) adds entries 4t .. 4t+3 of ray g ----
+                const int i = bang ? R.ib : R.ia;
+                const int b = (bang ? R.bstart1 : R.bstart0) + bub;
+                const bool red_ok = bok && b >= 0 && b < a.nd;
+                const float sc = bang ? R.inva1 : R.inva0;
+#pragma unroll
+                for (int zb = 0; zb < NB16; ++zb) {
+                    __syncwarp();
+                    stg[(2 * t) * FM_STG + g] = acc[zb][0];
+                    stg[(2 * t + 1) * FM_STG + g] = acc[zb][1];
+                    stg[(2 * t) * FM_STG + g + 8] = acc[zb][2];
+                    stg[(2 * t + 1) * FM_STG + g + 8] = acc[zb][3];
+                    __syncwarp();
+                    const float4 v = *reinterpret_cast<const float4 *>(stg + g * FM_STG + 4 * t);
+                    const int flat = zb * 16 + 4 * t, sl = z0 + (flat >> a.mshift), j = flat & (a.m - 1);
+                    if (red_ok && sl < a.nz)
+                        atomicAdd(reinterpret_cast<float4 *>(P + (((int64_t)sl * a.n0 + i) * a.gp + a.gpl + b) * a.m + j),
+                                  make_float4(v.x * sc, v.y * sc, v.z * sc, v.w * sc));
+                }
+            }
+        }
+    }
+}
+
+template <int NB16>
+cudaError_t fm_launch(cp4d_ctx *c, const float *f, float *P, FmArgs a) {
+    const Dims &d = c->d;
+    a.zper = NB16 * 16 / d.m;
+    const int zgroups = (d.nz + a.zper - 1) / a.zper;
+    // small problems: split the angle pairs of a pass over up to 8 CTAs per tile so that every SM has work
+    const int64_t ctas = (int64_t)d.tiles * 2 * zgroups;
+    a.agroups = (int)std::max<int64_t>(1, std::min<int64_t>(std::min(8, std::max(1, std::min(c->n_pairs0, c->n_pairs1))), 148 / ctas));
+    const dim3 grid(d.tiles * a.agroups, 2 * zgroups);
+    k_forward_mma<NB16><<<grid, FM_THREADS, (size_t)NB16 * 2 * FM_PLANE, c->stream>>>(f, P, a);
+    return cudaGetLastError();
+}
+
+}  // namespace
+
+bool forward_mma_supported(const Dims &d) {
+    return (d.m == 4 || d.m == 8 || d.m == 16 || d.m == 32);
+}
+
+cudaError_t forward_mma_init() {
+    cudaError_t e;
+    if ((e = cudaFuncSetAttribute(k_forward_mma<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, 1 * 2 * FM_PLANE)) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(k_forward_mma<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, 2 * 2 * FM_PLANE)) != cudaSuccess) return e;
+    return cudaFuncSetAttribute(k_forward_mma<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, 3 * 2 * FM_PLANE);
+}
+
+// host: pair adjacent base angles of one pass (same stepping axis, same sign of 1/ss, neighbouring indices); the angle with
+// the smaller |1/ss| comes first, so that a strip of four of its bins holds at most four bins of the other
+int forward_mma_pairs(const FwAngle *fw, const int32_t *order, int n0, int n_colstep, int2 *out, int *npairs0, int *npairs1) {
+    int n = 0;
+    // the second angle's rays are sorted into the first angle's strips by their position at the tile's middle column; a ray that
+    // touches the tile is then at most 16 sqrt2 sin(pi/n0) bins outside the first angle's window, which the two spare strips
+    // (bins -4 .. -1 and 48 .. 51) absorb for n0 >= 24.  Coarser angle sets run every angle on its own.
+    const bool may_pair = n0 >= 24;
+    for (int pass = 0; pass < 2; ++pass) {
+        const int l0 = pass ? n_colstep : 0, l1 = pass ? n0 : n_colstep;
+        const int start = n;
+        for (int q = l0; q < l1;) {
+            const int i = order[q];
+            if (may_pair && q + 1 < l1 && order[q + 1] == i + 1 && (fw[i].inv > 0.f) == (fw[i + 1].inv > 0.f)) {
+                const bool first = std::fabs(fw[i].inv) <= std::fabs(fw[i + 1].inv);
+                out[n++] = first ? make_int2(i, i + 1) : make_int2(i + 1, i);
+                q += 2;
+            } else {
+                out[n++] = make_int2(i, -1);
+                q += 1;
+            }
+        }
+        *(pass ? npairs1 : npairs0) = n - start;
+    }
+    return n;
+}
+
+cudaError_t launch_forward_mma(cp4d_ctx *c, const float *f, float *P) {
+    const Dims &d = c->d;
+    int ms = 0;
+    while ((1 << ms) < d.m) ++ms;
+    // 1.5 bins for the taps and the half-bin extents + (TILE/2) sqrt2 sin(pi/n0) for the drift over half a tile (pairs only)
+    const float margin = 1.5f + (d.n0 >= 24 ? 0.5f * TILE * 1.41421356f * std::sin(3.14159265f / (float)d.n0) : 0.0f);
+    FmArgs a{d.n, d.nz, d.nd, d.n0, d.m, ms, d.gp, d.gpl, d.tiles, 1, 0, margin, c->geo, c->fwang, c->fw_pairs, c->n_pairs0, c->n_pairs1};
+    // 16-entry batch blocks per CTA: three (192 KB of shared memory) unless the volume has fewer; m = 32 needs whole slices
+    const int blocks_total = (d.nz * d.m + 15) / 16;
+    int nb = std::min(3, blocks_total);
+    if (d.m == 32) nb = 2;
+    switch (nb) {
+    case 1: return fm_launch<1>(c, f, P, a);
+    case 2: return fm_launch<2>(c, f, P, a);
+    default: return fm_launch<3>(c, f, P, a);
+    }
+}
+
+}  // namespace cp4d

@@ -2,8 +2,9 @@
 // of L198-L202).  A CTA stages one TILE x TILE voxel tile (a group of coefficients of one to four slices) in shared memory
 // once, then walks ALL base angles; every ray of the tile's window gathers its Joseph taps along the dominant axis with
 // the coefficients accumulated in registers, so the m coefficients are read once per tap and the synthesised frame
-// sum_j Phi[j,k] f_j is never materialised.  The per-tile partial ray sums go to P[z][i][jq][b] with one vector RED per ray
-// and coefficient chunk; the synthesis with Phi (and the F1* prox) is the k_synth epilogue in stream_kernels.cu.
+// sum_j Phi[j,k] f_j is never materialised.  The per-tile partial ray sums go to P[z][i][b][j] (j fastest) with one vector RED
+// per ray and coefficient chunk; the synthesis with Phi (and the F1* prox) is the k_synth epilogue in stream_kernels.cu.
+// This is the exact-fp32 CUDA-core forward projector; forward_mma.cu holds the tensor-core one that runs by default.
 //
 //   k_forward_rays<JQ> : JQ = 4, 2, 1 coefficient chunks (16, 8, 4 coefficients) of 4/JQ adjacent slices per CTA.
 //
@@ -70,7 +71,7 @@ struct FwTable {
 };
 
 template <int JQ, bool CONST_TAB>
-__global__ void __launch_bounds__(FR_THREADS, 3) k_forward_rays(const float *__restrict__ f, float4 *__restrict__ P, ProjArgs a,
+__global__ void __launch_bounds__(FR_THREADS, 3) k_forward_rays(const float *__restrict__ f, float *__restrict__ P, ProjArgs a,
                                                                 const __grid_constant__ FwTable tab) {
     using C = FwRays<JQ>;
     constexpr int NPH = C::NPH, RSV = C::RSV, CHUNK = C::CHUNK, UNROLL = C::UNROLL;
@@ -146,7 +147,7 @@ __global__ void __launch_bounds__(FR_THREADS, 3) k_forward_rays(const float *__r
             const float2 tot = sp ? make_float2(acc.z + r0, acc.w + r1) : make_float2(acc.x + r0, acc.y + r1);
             const int b = G.bstart + u;
             if (touched && b >= 0 && b < a.nd && z < a.nz) {
-                float2 *dst = reinterpret_cast<float2 *>(P + (((int64_t)z * a.n0 + i) * a.Q + jg * JQ + jc) * a.gp + a.gpl + b) + sp;
+                float2 *dst = reinterpret_cast<float2 *>(P + ((((int64_t)z * a.n0 + i) * a.gp + a.gpl + b) * a.Q + jg * JQ + jc) * 4) + sp;
                 atomicAdd(dst, make_float2(tot.x * A.inv_a, tot.y * A.inv_a));
             }
         }
@@ -154,7 +155,7 @@ __global__ void __launch_bounds__(FR_THREADS, 3) k_forward_rays(const float *__r
 }
 
 template <int JQ>
-static cudaError_t fwd_launch_rays(cp4d_ctx *c, const float *f, float4 *P, const ProjArgs &a) {
+static cudaError_t fwd_launch_rays(cp4d_ctx *c, const float *f, float *P, const ProjArgs &a) {
     const Dims &d = c->d;
     const size_t sh = FwRays<JQ>::SMEM;
     // small problems: split the base angles over up to 8 CTAs per tile
@@ -187,8 +188,8 @@ static cudaError_t fwd_init_one() {
 // cp4d_create calls this once per context (the attribute is per device and sticks)
 cudaError_t forward_init() {
     cudaError_t e;
-    if ((e = fwd_init_one<4>()) != cudaSuccess || (e = fwd_init_one<2>()) != cudaSuccess) return e;
-    return fwd_init_one<1>();
+    if ((e = fwd_init_one<4>()) != cudaSuccess || (e = fwd_init_one<2>()) != cudaSuccess || (e = fwd_init_one<1>()) != cudaSuccess) return e;
+    return forward_mma_init();
 }
 
 static int pick_jq(int Q) { return (Q % 4 == 0) ? 4 : (Q % 2 == 0) ? 2 : 1; }
@@ -208,10 +209,12 @@ cudaError_t launch_forward_partial(cp4d_ctx *c, const float *f, float4 *P) {
     cudaError_t e = cudaMemsetAsync(P, 0, (size_t)d.nz * d.n0 * d.Q * d.gp * sizeof(float4), c->stream);
     if (e != cudaSuccess) return e;
     c->launches += 2;
+    float *Pf = reinterpret_cast<float *>(P);
+    if (c->fw_mode != CP4D_FORWARD_FP32 && forward_mma_supported(d)) return launch_forward_mma(c, f, Pf);
     switch (pick_jq(d.Q)) {
-    case 4: return fwd_launch_rays<4>(c, f, P, a);
-    case 2: return fwd_launch_rays<2>(c, f, P, a);
-    default: return fwd_launch_rays<1>(c, f, P, a);
+    case 4: return fwd_launch_rays<4>(c, f, Pf, a);
+    case 2: return fwd_launch_rays<2>(c, f, Pf, a);
+    default: return fwd_launch_rays<1>(c, f, Pf, a);
     }
 }
 

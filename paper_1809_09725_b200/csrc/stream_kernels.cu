@@ -331,7 +331,7 @@ cudaError_t launch_kkt_sum(cp4d_ctx *c, const float *bp, const float *h2, double
 
 // ---------------------------------------------------------------------------------------------------
 // fold: gt[z][i][jc][b] (float4 over j) = sum_q Phi[j, q n0 + i] g[z][q n0 + i][flip_q b]
-// synth (PAPER.md:L198-L202 + Eq. 9): v[z][q n0+i][flip_q b] = sum_j Phi[j, q n0+i] P[z][i][.][b][j]
+// synth (PAPER.md:L198-L202 + Eq. 9): v[z][q n0+i][flip_q b] = sum_j Phi[j, q n0+i] P[z][i][b][j]   (P: j fastest, row pitch gp bins)
 // One CTA per (z, base angle i); the npi x m slice of Phi it needs sits in shared memory.
 // ---------------------------------------------------------------------------------------------------
 template <int Q>
@@ -381,7 +381,7 @@ __global__ void __launch_bounds__(128) k_synth(const float4 *__restrict__ P, int
         float acc[m];
 #pragma unroll
         for (int jc = 0; jc < Q; ++jc) {
-            const float4 v = P[(((int64_t)z * n0 + i) * Q + jc) * gp + gpl + b];
+            const float4 v = P[(((int64_t)z * n0 + i) * gp + gpl + b) * Q + jc];
             acc[4 * jc] = v.x; acc[4 * jc + 1] = v.y; acc[4 * jc + 2] = v.z; acc[4 * jc + 3] = v.w;
         }
         for (int q0 = 0; q0 < npi; q0 += 4) {     // 4 half-rotations per batch: their loads are in flight together
