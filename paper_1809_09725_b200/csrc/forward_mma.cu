@@ -81,7 +81,7 @@ struct FmPair {
                                           // reference column; istep = 1/step (0 when the rays run along the columns)
     int ia, ib, bstart0, bstart1;
 };
-constexpr int FM_MAXP = 128;               // pairs per chunk of a CTA's pair list
+constexpr int FM_MAXP = 64;                // pairs per chunk of a CTA's pair list
 
 // columns k in [0, TILE) where a ray group whose first-tap rows lie in [ylo + k st, yhi + k st] touches rows 0 .. TILE-1:
 // ylo + k st < TILE and yhi + k st > -1
@@ -97,39 +97,62 @@ __device__ __forceinline__ void col_range(float ylo, float yhi, float st, float 
     }
 }
 
+// one work item of a CTA: (angle pair, strip, which of the two angles) with its trimmed column range, built once per CTA by
+// all threads in parallel so that a warp's per-item setup is a decode and a few FMAs
+struct FmItem {
+    unsigned short pair_strip;     // (pair << 4) | (strip + 1)
+    unsigned char klo, khi;        // columns of the tile the strip's rays touch
+    signed char b1s;               // first window bin of the second angle's group in this strip
+    unsigned char cnt1;            // bins of that group
+    unsigned char mode;            // 0: both angles in one window (slots 0-3 / 4-7), 1: first angle only, 2: second angle only
+    unsigned char pad;
+};
+static_assert(sizeof(FmItem) == 8, "FmItem is one 8-byte shared-memory word");
+
 template <int NB16>
 __global__ void __launch_bounds__(FM_THREADS, 1) k_forward_mma(const float *__restrict__ f, float *__restrict__ P, FmArgs a) {
     extern __shared__ __align__(128) unsigned char tile[];     // [NB16][2][2][TILE][TILE] x 16 B
-    __shared__ int s_next, s_nunits;
+    __shared__ int s_next, s_nitems, s_ncand;
     __shared__ __align__(16) float s_stg[FM_WARPS][8 * FM_STG];
     __shared__ __align__(16) FmPair s_pair[FM_MAXP];
     __shared__ unsigned char s_t0[FM_MAXP], s_tn[FM_MAXP];      // first strip (+1) and number of strips of each pair
-    __shared__ unsigned short s_unit[FM_MAXP * FM_STRIPS];      // unit -> (pair << 4) | (strip + 1)
+    __shared__ unsigned short s_cand[FM_MAXP * FM_STRIPS];      // candidate -> (pair << 4) | (strip + 1)
+    __shared__ __align__(8) FmItem s_item[2 * FM_MAXP * FM_STRIPS];
     float *stg = s_stg[threadIdx.x >> 5];
     const int tiles_1d = (a.n + TILE - 1) / TILE;
     const int tile_id = blockIdx.x % a.tiles, ag = blockIdx.x / a.tiles;
     const int pass = blockIdx.y & 1, z0 = (blockIdx.y >> 1) * a.zper;
     const int x0 = (tile_id % tiles_1d) * TILE, y0 = (tile_id / tiles_1d) * TILE;
 
-    // ---- stage the tile: fp32 -> (hi, lo) bf16, pass coordinates (column = stepping axis) ----
-    for (int e = threadIdx.x; e < NB16 * 2 * TILE * TILE; e += FM_THREADS) {
-        const int row = e & (TILE - 1), kcol = (e >> 5) & (TILE - 1), jh = (e >> 10) & 1, zb = e >> 11;
-        const int gx = x0 + (pass ? row : kcol), gy = y0 + (pass ? kcol : row);
-        float v[8];
+    // ---- stage the tile: fp32 -> (hi, lo) bf16, pass coordinates (column = stepping axis); 4 entries (8 loads) in flight ----
+    constexpr int N_ENT = NB16 * 2 * TILE * TILE;
+    static_assert(N_ENT % (4 * FM_THREADS) == 0, "staging loop is unrolled by 4");
+    for (int e0 = threadIdx.x; e0 < N_ENT; e0 += 4 * FM_THREADS) {
+        float4 q[4][2];
 #pragma unroll
-        for (int h = 0; h < 2; ++h) {
-            const int flat = zb * 16 + jh * 8 + h * 4, sl = z0 + (flat >> a.mshift), j = flat & (a.m - 1);
-            float4 q = make_float4(0.f, 0.f, 0.f, 0.f);
-            if (gx < a.n && gy < a.n && sl < a.nz)
-                q = __ldg(reinterpret_cast<const float4 *>(f + (((int64_t)sl * a.n + gy) * a.n + gx) * a.m + j));
-            v[4 * h] = q.x; v[4 * h + 1] = q.y; v[4 * h + 2] = q.z; v[4 * h + 3] = q.w;
+        for (int r = 0; r < 4; ++r) {
+            const int e = e0 + r * FM_THREADS;
+            const int row = e & (TILE - 1), kcol = (e >> 5) & (TILE - 1), jh = (e >> 10) & 1, zb = e >> 11;
+            const int gx = x0 + (pass ? row : kcol), gy = y0 + (pass ? kcol : row);
+#pragma unroll
+            for (int h = 0; h < 2; ++h) {
+                const int flat = zb * 16 + jh * 8 + h * 4, sl = z0 + (flat >> a.mshift), j = flat & (a.m - 1);
+                q[r][h] = make_float4(0.f, 0.f, 0.f, 0.f);
+                if (gx < a.n && gy < a.n && sl < a.nz)
+                    q[r][h] = __ldg(reinterpret_cast<const float4 *>(f + (((int64_t)sl * a.n + gy) * a.n + gx) * a.m + j));
+            }
         }
-        uint4 hi, lo;
-        split2(v[0], v[1], hi.x, lo.x); split2(v[2], v[3], hi.y, lo.y);
-        split2(v[4], v[5], hi.z, lo.z); split2(v[6], v[7], hi.w, lo.w);
-        unsigned char *dst = tile + (size_t)(zb * 2) * FM_PLANE + ((jh * TILE + kcol) * TILE + row) * 16;
-        *reinterpret_cast<uint4 *>(dst) = hi;
-        *reinterpret_cast<uint4 *>(dst + FM_PLANE) = lo;
+#pragma unroll
+        for (int r = 0; r < 4; ++r) {
+            const int e = e0 + r * FM_THREADS;
+            const int row = e & (TILE - 1), kcol = (e >> 5) & (TILE - 1), jh = (e >> 10) & 1, zb = e >> 11;
+            uint4 hi, lo;
+            split2(q[r][0].x, q[r][0].y, hi.x, lo.x); split2(q[r][0].z, q[r][0].w, hi.y, lo.y);
+            split2(q[r][1].x, q[r][1].y, hi.z, lo.z); split2(q[r][1].z, q[r][1].w, hi.w, lo.w);
+            unsigned char *dst = tile + (size_t)(zb * 2) * FM_PLANE + ((jh * TILE + kcol) * TILE + row) * 16;
+            *reinterpret_cast<uint4 *>(dst) = hi;
+            *reinterpret_cast<uint4 *>(dst + FM_PLANE) = lo;
+        }
     }
 
     // ---- this CTA's share of the pass's angle pairs, in chunks of FM_MAXP ----
@@ -168,7 +191,7 @@ __global__ void __launch_bounds__(FM_THREADS, 1) k_forward_mma(const float *__re
             s_tn[threadIdx.x] = (unsigned char)max(0, tl - tf + 1);
         }
         __syncthreads();
-        if (threadIdx.x < 32) {                              // unit table: pairs in order, their strips in order
+        if (threadIdx.x < 32) {                              // candidate table: pairs in order, their strips in order
             int base = 0;
             for (int q0 = 0; q0 < npc; q0 += 32) {
                 const int q = q0 + lane, n = q < npc ? s_tn[q] : 0;
@@ -178,20 +201,16 @@ __global__ void __launch_bounds__(FM_THREADS, 1) k_forward_mma(const float *__re
                     const int v = __shfl_up_sync(0xffffffffu, incl, o);
                     if (lane >= o) incl += v;
                 }
-                for (int r = 0; r < n; ++r) s_unit[base + incl - n + r] = (unsigned short)((q << 4) | (s_t0[q] + r));
+                for (int r = 0; r < n; ++r) s_cand[base + incl - n + r] = (unsigned short)((q << 4) | (s_t0[q] + r));
                 base += __shfl_sync(0xffffffffu, incl, 31);
             }
-            if (lane == 0) { s_nunits = base; s_next = 0; }
+            if (lane == 0) { s_ncand = base; s_nitems = 0; s_next = 0; }
         }
         __syncthreads();
-        const int n_units = s_nunits;
-
-        for (;;) {
-            int u = 0;
-            if (lane == 0) u = atomicAdd(&s_next, 1);
-            u = __shfl_sync(0xffffffffu, u, 0);
-            if (u >= n_units) break;
-            const unsigned uu = s_unit[u];
+        // ---- work items: every candidate (pair, strip) is examined by one thread: the second angle's group of bins, the columns
+        // the rays touch, and whether one 8-row window per column holds both angles (else one item per angle) ----
+        for (int cnd = threadIdx.x; cnd < s_ncand; cnd += FM_THREADS) {
+            const unsigned uu = s_cand[cnd];
             const FmPair R = s_pair[uu >> 4];
             const int ts = (int)(uu & 15) - 1;
             const float ft4 = 4.0f * (float)ts;
@@ -208,82 +227,99 @@ __global__ void __launch_bounds__(FM_THREADS, 1) k_forward_mma(const float *__re
             const float lo0 = fminf(y00, y03), hi0 = fmaxf(y00, y03), lo1 = fminf(y10, y11), hi1 = fmaxf(y10, y11);
             int ka0, kb0, ka1 = TILE, kb1 = -1;
             col_range(lo0, hi0, R.step0, R.istep0, ka0, kb0);
-            if (cnt1 > 0) col_range(lo1, hi1, R.step1, R.istep1, ka1, kb1);
+            if (4 * ts + 3 < 0 || 4 * ts >= WIN) { ka0 = TILE; kb0 = -1; }          // no bin of the first angle's window in this strip
+            if (cnt1 > 0 && b1s + cnt1 > 0 && b1s < WIN) col_range(lo1, hi1, R.step1, R.istep1, ka1, kb1);
             // one window for both angles?  The spread of first-tap rows is convex in k: check the two end columns
-            bool pair_ok = cnt1 > 0 && cnt1 <= 4;
+            bool pair_ok = cnt1 > 0 && cnt1 <= 4 && ka0 <= kb0 && ka1 <= kb1;
             if (pair_ok) {
                 const float fa = (float)min(ka0, ka1), fb = (float)max(kb0, kb1);
                 const float sa = fmaxf(fmaf(fa, R.step0, hi0), fmaf(fa, R.step1, hi1)) - fminf(fmaf(fa, R.step0, lo0), fmaf(fa, R.step1, lo1));
                 const float sb = fmaxf(fmaf(fb, R.step0, hi0), fmaf(fb, R.step1, hi1)) - fminf(fmaf(fb, R.step0, lo0), fmaf(fb, R.step1, lo1));
                 pair_ok = sa < FM_SPAN && sb < FM_SPAN;
             }
-            const int n_sub = (cnt1 > 0 && !pair_ok) ? 2 : 1;
-            for (int sub = 0; sub < n_sub; ++sub) {
-                // slot n of the 8 rays -> (angle, window bin).  pair: 0-3 angle 0, 4-7 angle 1; split: one angle, slots from 0
-                const bool use0 = pair_ok || cnt1 == 0 || sub == 0, use1 = pair_ok || (cnt1 > 0 && sub == 1);
-                int klo = TILE, khi = -1;
-                if (use0) { klo = min(klo, ka0); khi = max(khi, kb0); }
-                if (use1) { klo = min(klo, ka1); khi = max(khi, kb1); }
-                if (klo > khi) continue;                     // (warp-uniform) the strip misses the tile
-                // my ray (slot g): B column g of the weight block, and the ray whose sums I add to P in the end
-                const int off1 = pair_ok ? 4 : 0;            // first slot of angle 1
-                const int bang = (use1 && !(use0 && g < 4)) ? 1 : 0;
-                const int bub = bang ? b1s + g - off1 : 4 * ts + g;
-                const bool bok = (bang ? (g >= off1 && g - off1 < cnt1) : (use0 && g < 4)) && bub >= 0 && bub < WIN;
-                const float bstep = bang ? R.step1 : R.step0;
-                // rows of column k0 at k = 2t, 2t+1 and of column k0+1 at k = 2t+8, 2t+9: first-tap row relative to row q + 2t
-                const float byb = bok ? ((float)bub - (bang ? R.delta1 : R.delta0)) * (bang ? R.inv1 : R.inv0) - (float)(2 * t) : -1e6f;
-                // window line(s): lowest first-tap row of each angle in use
-                const float wl0 = use0 ? lo0 : 1e6f, wl1 = use1 ? lo1 : 1e6f;
+            FmItem it;
+            it.pair_strip = (unsigned short)uu; it.b1s = (signed char)max(-100, min(100, b1s)); it.cnt1 = (unsigned char)min(cnt1, 8); it.pad = 0;
+            if (pair_ok) {
+                it.mode = 0; it.klo = (unsigned char)min(ka0, ka1); it.khi = (unsigned char)max(kb0, kb1);
+                s_item[atomicAdd(&s_nitems, 1)] = it;
+            } else {
+                if (ka0 <= kb0) { it.mode = 1; it.klo = (unsigned char)ka0; it.khi = (unsigned char)kb0; s_item[atomicAdd(&s_nitems, 1)] = it; }
+                if (ka1 <= kb1) { it.mode = 2; it.klo = (unsigned char)ka1; it.khi = (unsigned char)kb1; s_item[atomicAdd(&s_nitems, 1)] = it; }
+            }
+        }
+        __syncthreads();
+        const int n_items = s_nitems;
 
-                float acc[NB16][4];
-#pragma unroll
-                for (int zb = 0; zb < NB16; ++zb) acc[zb][0] = acc[zb][1] = acc[zb][2] = acc[zb][3] = 0.f;
+        for (;;) {
+            int u = 0;
+            if (lane == 0) u = atomicAdd(&s_next, 1);
+            u = __shfl_sync(0xffffffffu, u, 0);
+            if (u >= n_items) break;
+            const FmItem it = s_item[u];
+            const FmPair R = s_pair[it.pair_strip >> 4];
+            const int ts = (int)(it.pair_strip & 15) - 1, klo = it.klo, khi = it.khi, b1s = it.b1s, cnt1 = it.cnt1;
+            // slot n of the 8 rays -> (angle, window bin).  mode 0: 0-3 first angle, 4-7 second; else one angle, slots from 0
+            const bool use0 = it.mode != 2, use1 = it.mode != 1;
+            const int off1 = it.mode == 0 ? 4 : 0;               // first slot of the second angle
+            // lowest first-tap row of each angle in use at column 0: the window lines
+            const float y00 = (4.0f * (float)ts - R.delta0) * R.inv0, y10 = ((float)b1s - R.delta1) * R.inv1;
+            const float wl0 = use0 ? fminf(y00, fmaf(3.0f, R.inv0, y00)) : 1e6f;
+            const float wl1 = use1 ? fminf(y10, fmaf((float)(max(cnt1, 1) - 1), R.inv1, y10)) : 1e6f;
+            // my ray (slot g): B column g of the weight block, and the ray whose sums I add to P in the end
+            const int bang = (use1 && !(use0 && g < 4)) ? 1 : 0;
+            const int bub = bang ? b1s + g - off1 : 4 * ts + g;
+            const bool bok = (bang ? (g >= off1 && g - off1 < cnt1) : (use0 && g < 4)) && bub >= 0 && bub < WIN;
+            const float bstep = bang ? R.step1 : R.step0;
+            // rows of column k0 at k = 2t, 2t+1 and of column k0+1 at k = 2t+8, 2t+9: first-tap row relative to row q + 2t
+            const float byb = bok ? ((float)bub - (bang ? R.delta1 : R.delta0)) * (bang ? R.inv1 : R.inv0) - (float)(2 * t) : -1e6f;
 
-                for (int k0 = klo & ~1; k0 <= khi; k0 += 2) {
-                    const float fk = (float)k0, fk1 = fk + 1.0f;
-                    // window start per column: floor of the lowest first-tap row, clamped into the tile
-                    const int qa = min(max((int)floorf(fminf(fmaf(fk, R.step0, wl0), fmaf(fk, R.step1, wl1))), 0), TILE - 8);
-                    const int qb = min(max((int)floorf(fminf(fmaf(fk1, R.step0, wl0), fmaf(fk1, R.step1, wl1))), 0), TILE - 8);
-                    // weights of my ray at rows q + 2t, q + 2t + 1 of both columns: Joseph hat max(0, 1 - |row - y|)
-                    const float da = fmaf(fk, bstep, byb) - (float)qa, db = fmaf(fk1, bstep, byb) - (float)qb;   // y - (q + 2t)
-                    const float w0 = __saturatef(1.0f - fabsf(da)), w1 = __saturatef(1.0f - fabsf(da - 1.0f));
-                    const float w2 = __saturatef(1.0f - fabsf(db)), w3 = __saturatef(1.0f - fabsf(db - 1.0f));
-                    unsigned bh0, bl0, bh1, bl1;
-                    split2(w0, w1, bh0, bl0);
-                    split2(w2, w3, bh1, bl1);
-                    const unsigned adr = tile_s + (((ld_half * TILE + k0 + ld_col) * TILE + (ld_col ? qb : qa) + ld_row) << 4);
+            float acc[NB16][4];
 #pragma unroll
-                    for (int zb = 0; zb < NB16; ++zb) {
-                        unsigned ah[4], al[4];
-                        ldsm4t(ah, adr + zb * 2 * FM_PLANE);
-                        ldsm4t(al, adr + zb * 2 * FM_PLANE + FM_PLANE);
-                        mma16816(acc[zb], ah, bh0, bh1);
-                        mma16816(acc[zb], al, bh0, bh1);
-                        mma16816(acc[zb], ah, bl0, bl1);
-                    }
-                }
-                // ---- partial ray sums of this tile -> P[z][i][b][j].  My D entries are rays 2t, 2t+1 x batch entries g, g+8; a RED
-                // costs about one clock per LANE whatever its width, so the block goes through a per-warp shared-memory patch and
-                // leaves as one 16-byte RED per lane: lane (ray g, quad t) adds entries 4t .. 4t+3 of ray g ----
-                const int i = bang ? R.ib : R.ia;
-                const int b = (bang ? R.bstart1 : R.bstart0) + bub;
-                const bool red_ok = bok && b >= 0 && b < a.nd;
-                const float sc = bang ? R.inva1 : R.inva0;
+            for (int zb = 0; zb < NB16; ++zb) acc[zb][0] = acc[zb][1] = acc[zb][2] = acc[zb][3] = 0.f;
+
+            for (int k0 = klo & ~1; k0 <= khi; k0 += 2) {
+                const float fk = (float)k0, fk1 = fk + 1.0f;
+                // window start per column: floor of the lowest first-tap row, clamped into the tile
+                const int qa = min(max((int)floorf(fminf(fmaf(fk, R.step0, wl0), fmaf(fk, R.step1, wl1))), 0), TILE - 8);
+                const int qb = min(max((int)floorf(fminf(fmaf(fk1, R.step0, wl0), fmaf(fk1, R.step1, wl1))), 0), TILE - 8);
+                // weights of my ray at rows q + 2t, q + 2t + 1 of both columns: Joseph hat max(0, 1 - |row - y|)
+                const float da = fmaf(fk, bstep, byb) - (float)qa, db = fmaf(fk1, bstep, byb) - (float)qb;   // y - (q + 2t)
+                const float w0 = __saturatef(1.0f - fabsf(da)), w1 = __saturatef(1.0f - fabsf(da - 1.0f));
+                const float w2 = __saturatef(1.0f - fabsf(db)), w3 = __saturatef(1.0f - fabsf(db - 1.0f));
+                unsigned bh0, bl0, bh1, bl1;
+                split2(w0, w1, bh0, bl0);
+                split2(w2, w3, bh1, bl1);
+                const unsigned adr = tile_s + (((ld_half * TILE + k0 + ld_col) * TILE + (ld_col ? qb : qa) + ld_row) << 4);
 #pragma unroll
                 for (int zb = 0; zb < NB16; ++zb) {
-                    __syncwarp();
-                    stg[(2 * t) * FM_STG + g] = acc[zb][0];
-                    stg[(2 * t + 1) * FM_STG + g] = acc[zb][1];
-                    stg[(2 * t) * FM_STG + g + 8] = acc[zb][2];
-                    stg[(2 * t + 1) * FM_STG + g + 8] = acc[zb][3];
-                    __syncwarp();
-                    const float4 v = *reinterpret_cast<const float4 *>(stg + g * FM_STG + 4 * t);
-                    const int flat = zb * 16 + 4 * t, sl = z0 + (flat >> a.mshift), j = flat & (a.m - 1);
-                    if (red_ok && sl < a.nz)
-                        atomicAdd(reinterpret_cast<float4 *>(P + (((int64_t)sl * a.n0 + i) * a.gp + a.gpl + b) * a.m + j),
-                                  make_float4(v.x * sc, v.y * sc, v.z * sc, v.w * sc));
+                    unsigned ah[4], al[4];
+                    ldsm4t(ah, adr + zb * 2 * FM_PLANE);
+                    ldsm4t(al, adr + zb * 2 * FM_PLANE + FM_PLANE);
+                    mma16816(acc[zb], ah, bh0, bh1);
+                    mma16816(acc[zb], al, bh0, bh1);
+                    mma16816(acc[zb], ah, bl0, bl1);
                 }
+            }
+            // ---- partial ray sums of this tile -> P[z][i][b][j].  My D entries are rays 2t, 2t+1 x batch entries g, g+8; a RED
+            // costs about one clock per LANE whatever its width, so the block goes through a per-warp shared-memory patch and
+            // leaves as one 16-byte RED per lane: lane (ray g, quad t) adds entries 4t .. 4t+3 of ray g ----
+            const int i = bang ? R.ib : R.ia;
+            const int b = (bang ? R.bstart1 : R.bstart0) + bub;
+            const bool red_ok = bok && b >= 0 && b < a.nd;
+            const float sc = bang ? R.inva1 : R.inva0;
+#pragma unroll
+            for (int zb = 0; zb < NB16; ++zb) {
+                __syncwarp();
+                stg[(2 * t) * FM_STG + g] = acc[zb][0];
+                stg[(2 * t + 1) * FM_STG + g] = acc[zb][1];
+                stg[(2 * t) * FM_STG + g + 8] = acc[zb][2];
+                stg[(2 * t + 1) * FM_STG + g + 8] = acc[zb][3];
+                __syncwarp();
+                const float4 v = *reinterpret_cast<const float4 *>(stg + g * FM_STG + 4 * t);
+                const int flat = zb * 16 + 4 * t, sl = z0 + (flat >> a.mshift), j = flat & (a.m - 1);
+                if (red_ok && sl < a.nz)
+                    atomicAdd(reinterpret_cast<float4 *>(P + (((int64_t)sl * a.n0 + i) * a.gp + a.gpl + b) * a.m + j),
+                              make_float4(v.x * sc, v.y * sc, v.z * sc, v.w * sc));
             }
         }
     }
