@@ -53,7 +53,7 @@ int validate(const cp4d_params *p, Dims *d) {
 }
 
 struct Carve {
-    uint64_t f, ft, bp, h2, h1, g, tmp_s, scratch, phi, ang, geo, red, cf, cb, psi, fwang, fworder, fwpairs, total;
+    uint64_t f, ft, bp, h2, h1, g, tmp_s, scratch, psum, phi, ang, geo, red, cf, cb, psi, fwang, fworder, fwpairs, total;
 };
 Carve carve(const Dims &d) {
     Carve c;
@@ -61,6 +61,7 @@ Carve carve(const Dims &d) {
     auto take = [&](uint64_t bytes) { uint64_t r = o; o += up(bytes); return r; };
     c.f = take(d.V * 4); c.ft = take(d.V * 4); c.bp = take(d.V * 4); c.h2 = take(d.V * 16);
     c.h1 = take(d.S * 4); c.g = take(d.S * 4); c.tmp_s = take(d.S * 4); c.scratch = take(d.scratch4 * 16);
+    c.psum = take((uint64_t)d.nz * d.n0 * d.nd * d.m * 4);
     c.phi = take((uint64_t)d.m * d.na * 4); c.ang = take((uint64_t)d.n0 * sizeof(AngleTab));
     c.geo = take((uint64_t)d.tiles * d.n0 * sizeof(TileGeo)); c.red = take(64);
     c.fwang = take((uint64_t)d.n0 * sizeof(FwAngle)); c.fworder = take((uint64_t)d.n0 * 4);
@@ -112,8 +113,8 @@ int forward_into(cp4d_ctx *ctx, const float *f, int mode, float sigma, const flo
         CK(launch_mix(ctx, f, ctx->cf, ctx->d.m, ctx->d.nf, ctx->d.nf, 1), "analysis");     // (here m == mb)    // T(j,q) = psi[j*nf + q]
         f = ctx->cf;
     }
-    CK(launch_forward_partial(ctx, f, ctx->scratch), "forward_partial");
-    CK(launch_synth(ctx, ctx->scratch, mode, sigma, g, out), "synth");
+    CK(launch_forward_partial(ctx, f, ctx->psum), "forward_partial");
+    CK(launch_synth(ctx, ctx->psum, mode, sigma, g, out), "synth");
     return CP4D_OK;
 }
 int adjoint_into(cp4d_ctx *ctx, const float *g, float *f) {
@@ -190,7 +191,7 @@ int cp4d_create(const cp4d_params *p, cp4d_ctx **out) {
     ctx->fw_pairs = (int2 *)(w + cv.fwpairs); ctx->fw_mode = CP4D_FORWARD_AUTO;
     ctx->cf = d.nf ? (float *)(w + cv.cf) : nullptr; ctx->cb = d.nf ? (float *)(w + cv.cb) : nullptr;
     ctx->psi = d.nf ? (float *)(w + cv.psi) : nullptr;
-    ctx->scratch = (float4 *)(w + cv.scratch); ctx->phi = (float *)(w + cv.phi);
+    ctx->scratch = (float4 *)(w + cv.scratch); ctx->psum = (float4 *)(w + cv.psum); ctx->phi = (float *)(w + cv.phi);
     ctx->ang = (AngleTab *)(w + cv.ang); ctx->geo = (TileGeo *)(w + cv.geo); ctx->red = (double *)(w + cv.red);
 
     // host prologue: fp64 angle tables and per-(tile, angle) window geometry

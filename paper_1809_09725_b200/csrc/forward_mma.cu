@@ -384,7 +384,7 @@ cudaError_t launch_forward_mma(cp4d_ctx *c, const float *f, float *P) {
     while ((1 << ms) < d.m) ++ms;
     // 1.5 bins for the taps and the half-bin extents + (TILE/2) sqrt2 sin(pi/n0) for the drift over half a tile (pairs only)
     const float margin = 1.5f + (d.n0 >= 24 ? 0.5f * TILE * 1.41421356f * std::sin(3.14159265f / (float)d.n0) : 0.0f);
-    FmArgs a{d.n, d.nz, d.nd, d.n0, d.m, ms, d.gp, d.gpl, d.tiles, 1, 0, margin, c->geo, c->fwang, c->fw_pairs, c->n_pairs0, c->n_pairs1};
+    FmArgs a{d.n, d.nz, d.nd, d.n0, d.m, ms, d.nd, 0, d.tiles, 1, 0, margin, c->geo, c->fwang, c->fw_pairs, c->n_pairs0, c->n_pairs1};
     // 16-entry batch blocks per CTA: three (192 KB of shared memory) unless the volume has fewer; m = 32 needs whole slices
     const int blocks_total = (d.nz * d.m + 15) / 16;
     int nb = std::min(3, blocks_total);

@@ -205,8 +205,8 @@ void fwtable_free(FwTable *t) { delete t; }
 cudaError_t launch_forward_partial(cp4d_ctx *c, const float *f, float4 *P) {
     ProfScope ps(c, CP4D_K_FORWARD);
     const Dims &d = c->d;
-    ProjArgs a{d.n, d.nz, d.nd, d.n0, d.Q, d.gp, d.gpl, c->geo, c->fwang, c->fworder, c->n_colstep, d.tiles, 1};
-    cudaError_t e = cudaMemsetAsync(P, 0, (size_t)d.nz * d.n0 * d.Q * d.gp * sizeof(float4), c->stream);
+    ProjArgs a{d.n, d.nz, d.nd, d.n0, d.Q, d.nd, 0, c->geo, c->fwang, c->fworder, c->n_colstep, d.tiles, 1};
+    cudaError_t e = cudaMemsetAsync(P, 0, (size_t)d.nz * d.n0 * d.nd * d.Q * sizeof(float4), c->stream);
     if (e != cudaSuccess) return e;
     c->launches += 2;
     float *Pf = reinterpret_cast<float *>(P);

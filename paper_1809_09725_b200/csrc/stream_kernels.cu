@@ -430,7 +430,7 @@ cudaError_t launch_synth(cp4d_ctx *c, const float4 *P, int mode, float sigma, co
     ProfScope ps(c, CP4D_K_SYNTH);
     const Dims &d = c->d;
     const size_t sh = (size_t)d.npi * d.m * sizeof(float);
-    CP4D_DISPATCH_Q(d.Q, (k_synth<QQ><<<d.nz * d.n0, 128, sh, c->stream>>>(P, mode, sigma, g, out, c->phi, d.nd, d.na, d.npi, d.n0, d.gp, d.gpl)));
+    CP4D_DISPATCH_Q(d.Q, (k_synth<QQ><<<d.nz * d.n0, 128, sh, c->stream>>>(P, mode, sigma, g, out, c->phi, d.nd, d.na, d.npi, d.n0, d.nd, 0)));
     c->launches++;
     return cudaGetLastError();
 }

@@ -40,7 +40,8 @@ def test_workspace_bytes_counts_state(L):
         # at most (sqrt2 (n-1) - (nd-1))/2 + 3 bins each side plus one window of 56 bins
         pad = 2 * (int(np.ceil(max(0.0, 0.5 * (np.sqrt(2.0) * (c.n - 1) - (c.nd - 1))))) + 3) + 56
         pitch = c.nd + pad + (1 if (c.nd + pad) % 8 == 0 else 0)
-        scratch = c.nz * c.n_theta0 * pitch * c.m * 4
+        scratch = c.nz * c.n_theta0 * pitch * c.m * 4          # folded sinogram of the adjoint (zero-padded rows)
+        scratch += c.nz * c.n_theta0 * c.nd * c.m * 4          # partial ray sums of the forward projector (no padding)
         assert state + scratch <= nb <= state + scratch + (64 << 20)
     c = synth.CONFIGS[5]
     assert binding.workspace_bytes(c.n, c.nz, c.nd, c.n_angles, c.n_half_rot, c.m) < 170e9   # fits 180 GB HBM
