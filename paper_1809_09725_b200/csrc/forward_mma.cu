@@ -81,15 +81,18 @@ struct FmPair {
                                           // reference column; istep = 1/step (0 when the rays run along the columns)
     int ia, ib, bstart0, bstart1;
 };
-constexpr int FM_MAXP = 64;                // pairs per chunk of a CTA's pair list
+constexpr int FM_MAXP = 64;
+constexpr int FM_MAXITEMS = 2 * FM_MAXP * FM_STRIPS;   // every (pair, strip) may fall apart into two items
+constexpr int FM_LONG = 14;                           // columns from which an item counts as long               // pairs per chunk of a CTA's pair list
 
 // columns k in [0, TILE) where a ray group whose first-tap rows lie in [ylo + k st, yhi + k st] touches rows 0 .. TILE-1:
 // ylo + k st < TILE and yhi + k st > -1
 __device__ __forceinline__ void col_range(float ylo, float yhi, float st, float ist, int &klo, int &khi) {
     if (ist != 0.0f) {
         const float ka = ((float)TILE - ylo) * ist, kb = (-1.0f - yhi) * ist;     // st > 0: k < ka, k > kb; st < 0: reversed
-        klo = max(0, (int)floorf(st > 0.f ? kb : ka));
-        khi = min(TILE - 1, (int)ceilf(st > 0.f ? ka : kb));
+        // integer k strictly inside (lo, hi); the 1e-3 keeps a column whose bound is an integer up to rounding
+        klo = max(0, (int)floorf((st > 0.f ? kb : ka) + (1.0f - 1e-3f)));
+        khi = min(TILE - 1, (int)ceilf((st > 0.f ? ka : kb) - (1.0f - 1e-3f)));
     } else if (ylo < (float)TILE && yhi > -1.0f) {
         klo = 0; khi = TILE - 1;
     } else {
@@ -112,12 +115,12 @@ static_assert(sizeof(FmItem) == 8, "FmItem is one 8-byte shared-memory word");
 template <int NB16>
 __global__ void __launch_bounds__(FM_THREADS, 1) k_forward_mma(const float *__restrict__ f, float *__restrict__ P, FmArgs a) {
     extern __shared__ __align__(128) unsigned char tile[];     // [NB16][2][2][TILE][TILE] x 16 B
-    __shared__ int s_next, s_nitems, s_ncand;
+    __shared__ int s_next, s_nlong, s_nshort, s_ncand;
     __shared__ __align__(16) float s_stg[FM_WARPS][8 * FM_STG];
     __shared__ __align__(16) FmPair s_pair[FM_MAXP];
     __shared__ unsigned char s_t0[FM_MAXP], s_tn[FM_MAXP];      // first strip (+1) and number of strips of each pair
     __shared__ unsigned short s_cand[FM_MAXP * FM_STRIPS];      // candidate -> (pair << 4) | (strip + 1)
-    __shared__ __align__(8) FmItem s_item[2 * FM_MAXP * FM_STRIPS];
+    __shared__ __align__(8) FmItem s_item[FM_MAXITEMS];
     float *stg = s_stg[threadIdx.x >> 5];
     const int tiles_1d = (a.n + TILE - 1) / TILE;
     const int tile_id = blockIdx.x % a.tiles, ag = blockIdx.x / a.tiles;
@@ -204,7 +207,7 @@ __global__ void __launch_bounds__(FM_THREADS, 1) k_forward_mma(const float *__re
                 for (int r = 0; r < n; ++r) s_cand[base + incl - n + r] = (unsigned short)((q << 4) | (s_t0[q] + r));
                 base += __shfl_sync(0xffffffffu, incl, 31);
             }
-            if (lane == 0) { s_ncand = base; s_nitems = 0; s_next = 0; }
+            if (lane == 0) { s_ncand = base; s_nlong = 0; s_nshort = 0; s_next = 0; }
         }
         __syncthreads();
         // ---- work items: every candidate (pair, strip) is examined by one thread: the second angle's group of bins, the columns
@@ -237,25 +240,30 @@ __global__ void __launch_bounds__(FM_THREADS, 1) k_forward_mma(const float *__re
                 const float sb = fmaxf(fmaf(fb, R.step0, hi0), fmaf(fb, R.step1, hi1)) - fminf(fmaf(fb, R.step0, lo0), fmaf(fb, R.step1, lo1));
                 pair_ok = sa < FM_SPAN && sb < FM_SPAN;
             }
+            // long items are handed out first (front of the list), short ones last (stored from the back): an even finish
+            auto push = [&](const FmItem &x) {
+                const bool lng = (int)x.khi - (int)x.klo >= FM_LONG;
+                s_item[lng ? atomicAdd(&s_nlong, 1) : FM_MAXITEMS - 1 - atomicAdd(&s_nshort, 1)] = x;
+            };
             FmItem it;
             it.pair_strip = (unsigned short)uu; it.b1s = (signed char)max(-100, min(100, b1s)); it.cnt1 = (unsigned char)min(cnt1, 8); it.pad = 0;
             if (pair_ok) {
                 it.mode = 0; it.klo = (unsigned char)min(ka0, ka1); it.khi = (unsigned char)max(kb0, kb1);
-                s_item[atomicAdd(&s_nitems, 1)] = it;
+                push(it);
             } else {
-                if (ka0 <= kb0) { it.mode = 1; it.klo = (unsigned char)ka0; it.khi = (unsigned char)kb0; s_item[atomicAdd(&s_nitems, 1)] = it; }
-                if (ka1 <= kb1) { it.mode = 2; it.klo = (unsigned char)ka1; it.khi = (unsigned char)kb1; s_item[atomicAdd(&s_nitems, 1)] = it; }
+                if (ka0 <= kb0) { it.mode = 1; it.klo = (unsigned char)ka0; it.khi = (unsigned char)kb0; push(it); }
+                if (ka1 <= kb1) { it.mode = 2; it.klo = (unsigned char)ka1; it.khi = (unsigned char)kb1; push(it); }
             }
         }
         __syncthreads();
-        const int n_items = s_nitems;
+        const int n_long = s_nlong, n_items = n_long + s_nshort;
 
         for (;;) {
             int u = 0;
             if (lane == 0) u = atomicAdd(&s_next, 1);
             u = __shfl_sync(0xffffffffu, u, 0);
             if (u >= n_items) break;
-            const FmItem it = s_item[u];
+            const FmItem it = s_item[u < n_long ? u : FM_MAXITEMS - 1 - (u - n_long)];
             const FmPair R = s_pair[it.pair_strip >> 4];
             const int ts = (int)(it.pair_strip & 15) - 1, klo = it.klo, khi = it.khi, b1s = it.b1s, cnt1 = it.cnt1;
             // slot n of the 8 rays -> (angle, window bin).  mode 0: 0-3 first angle, 4-7 second; else one angle, slots from 0
