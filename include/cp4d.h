@@ -114,18 +114,24 @@ int cp4d_grad(cp4d_ctx *ctx, const float *f_dev, float *p_dev);
 /* f = div p = -K2^T p (L131-L133).  p: 4V, f: V. */
 int cp4d_div(cp4d_ctx *ctx, const float *p_dev, float *f_dev);
 
-/* Which forward projector cp4d_forward / cp4d_prox_f1 / cp4d_iterate / cp4d_norm launch.  Both compute the same ray sums
- * (Eq. 9 with the Joseph weights above); they differ in the arithmetic of the products:
- *   CP4D_FORWARD_AUTO (default): the tensor-core kernel where it applies (m = 4, 8, 16 or 32), else the fp32 one.  Voxel
- *       values and interpolation weights enter mma.sync as split bf16 pairs (x = x_hi + x_lo), three products per term,
- *       fp32 accumulation: relative error about 1e-5 per ray sum, inside the 1e-4 per-operator tolerance.
- *   CP4D_FORWARD_FP32: the CUDA-core gather, plain fp32 FMAs (relative error about 2e-6), 2-3 x slower.
- * The adjoint is fp32 in both modes.  Changing the mode drops the captured CUDA graph of cp4d_iterate. */
-#define CP4D_FORWARD_AUTO   0
-#define CP4D_FORWARD_FP32   1
-#define CP4D_FORWARD_TENSOR 2   /* reported by cp4d_forward_mode_in_use only */
-int cp4d_set_forward_mode(cp4d_ctx *ctx, int32_t mode);
-int cp4d_forward_mode_in_use(const cp4d_ctx *ctx, int32_t *mode_out_host);
+/* Which kernels cp4d_forward / cp4d_adjoint and everything built on them (cp4d_prox_f1, cp4d_primal_update, cp4d_iterate,
+ * cp4d_norm, cp4d_objective, cp4d_solve_host) launch.  All of them compute the same ray sums and their transpose (Eq. 9 /
+ * Eq. 10 with the Joseph weights above); they differ in the arithmetic of the products:
+ *   tensor-core kernels (m = 4, 8, 16 or 32 only): voxel / sinogram values and interpolation weights enter mma.sync as split
+ *       bf16 pairs (x = x_hi + x_lo with |x - x_hi - x_lo| <= 2^-17 |x|), three products per term, fp32 accumulation:
+ *       relative error about 5e-6 per ray sum or voxel (bound 1.1e-5), inside the 1e-4 per-operator tolerance;
+ *   fp32 kernels: CUDA-core FMAs, relative error about 2e-6.
+ *   CP4D_PROJ_AUTO (default): the faster kernel of each side -- tensor-core forward projector where it applies (1.27 x the
+ *       fp32 gather at config 3), fp32 backprojector (the tensor-core one measured 1.3 x slower).
+ *   CP4D_PROJ_FP32: fp32 kernels on both sides.      CP4D_PROJ_TENSOR: tensor-core kernels on both sides where they apply.
+ * cp4d_fbp always uses the fp32 backprojector.  Changing the mode drops the captured CUDA graph of cp4d_iterate and clears the
+ * projector scratch (asynchronously, on the context's stream). */
+#define CP4D_PROJ_AUTO   0
+#define CP4D_PROJ_FP32   1
+#define CP4D_PROJ_TENSOR 2
+int cp4d_set_projector_mode(cp4d_ctx *ctx, int32_t mode);
+/* which kind (CP4D_PROJ_FP32 / CP4D_PROJ_TENSOR) the forward and the adjoint run with; either pointer may be null (HOST) */
+int cp4d_projector_mode_in_use(const cp4d_ctx *ctx, int32_t *forward_out_host, int32_t *adjoint_out_host);
 
 /* ---- the three fused steps of Fig. 2 on caller-owned DEVICE buffers --------------------------- */
 /* step 3 (L154, L135): h1 <- (h1 + sigma (K1 ft - g)) / (1 + sigma).   h1 in/out (S), ft: V, g: S. */

@@ -66,7 +66,7 @@ def lib():
             "cp4d_grad_slab": [vp, vp, vp, vp], "cp4d_div_slab": [vp, vp, vp, vp],
             "cp4d_step_dual": [vp, vp], "cp4d_step_primal": [vp, vp], "cp4d_set_z_open": [vp, i32],
             "cp4d_launch_count": [vp, C.POINTER(u64)],
-            "cp4d_set_forward_mode": [vp, i32], "cp4d_forward_mode_in_use": [vp, C.POINTER(i32)],
+            "cp4d_set_projector_mode": [vp, i32], "cp4d_projector_mode_in_use": [vp, C.POINTER(i32), C.POINTER(i32)],
             "cp4d_graph_replays": [vp, C.POINTER(u64)],
             "cp4d_profile_begin": [vp], "cp4d_profile_end": [vp, C.POINTER(Profile)],
         }
@@ -302,14 +302,16 @@ class Context:
         self._ck(lib().cp4d_graph_replays(self._h, C.byref(out)))
         return out.value
 
-    def set_forward_mode(self, mode):
-        """"auto" (tensor-core forward projector where it applies) or "fp32" (the CUDA-core gather)."""
-        self._ck(lib().cp4d_set_forward_mode(self._h, {"auto": 0, "fp32": 1}[mode]))
+    def set_projector_mode(self, mode):
+        """"auto" (tensor-core forward projector where it applies: m = 4, 8, 16, 32; fp32 backprojector), "fp32" (CUDA-core
+        kernels on both sides) or "tensor" (tensor-core kernels on both sides where they apply)."""
+        self._ck(lib().cp4d_set_projector_mode(self._h, {"auto": 0, "fp32": 1, "tensor": 2}[mode]))
 
-    def forward_mode_in_use(self) -> str:
-        out = C.c_int32(0)
-        self._ck(lib().cp4d_forward_mode_in_use(self._h, C.byref(out)))
-        return {1: "fp32", 2: "tensor"}[out.value]
+    def projector_mode_in_use(self):
+        """(forward, adjoint), each "fp32" or "tensor"."""
+        fw, ad = C.c_int32(0), C.c_int32(0)
+        self._ck(lib().cp4d_projector_mode_in_use(self._h, C.byref(fw), C.byref(ad)))
+        return {1: "fp32", 2: "tensor"}[fw.value], {1: "fp32", 2: "tensor"}[ad.value]
 
     def graph_note(self) -> str:
         """Why iterate() is not replaying a CUDA graph ("" if it is, or has not tried yet)."""

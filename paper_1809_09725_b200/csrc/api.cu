@@ -1,5 +1,6 @@
 // C ABI of libcp4d.so (include/cp4d.h): validation, workspace carving, host-side fp64 tables, and the
 // stream-ordered orchestration of Fig. 2.  No kernel code here.
+#include <algorithm>
 #include <cmath>
 #include <cstdio>
 #include <cstring>
@@ -48,6 +49,7 @@ int validate(const cp4d_params *p, Dims *d) {
     d->gp = d->nd + 2 * over + WIN + 8;
     if (d->gp % 8 == 0) d->gp += 1;   // a pitch of whole 128-byte lines measured 1 % slower in the forward projector's REDs
     d->scratch4 = (int64_t)d->nz * d->n0 * d->Q * d->gp;
+    if (forward_mma_supported(*d)) d->scratch4 = std::max(d->scratch4, backproject_mma_scratch_units(*d));   // split-bf16 rows, whole z-groups
     if (d->nz > 65535 || d->tiles > 2000000) return CP4D_EINVAL;
     return CP4D_OK;
 }
@@ -118,8 +120,13 @@ int forward_into(cp4d_ctx *ctx, const float *f, int mode, float sigma, const flo
     return CP4D_OK;
 }
 int adjoint_into(cp4d_ctx *ctx, const float *g, float *f) {
-    CK(launch_fold(ctx, g, ctx->scratch), "fold");
-    CK(launch_backproject(ctx, ctx->scratch, ctx->d.nf ? ctx->cb : f), "backproject");
+    if (ctx->fw_mode == CP4D_PROJ_TENSOR && forward_mma_supported(ctx->d)) {     // (measured slower than the fp32 patch kernel)
+        CK(launch_fold_split(ctx, g, ctx->scratch), "fold");
+        CK(launch_backproject_mma(ctx, ctx->scratch, ctx->d.nf ? ctx->cb : f), "backproject");
+    } else {
+        CK(launch_fold(ctx, g, ctx->scratch), "fold");
+        CK(launch_backproject(ctx, ctx->scratch, ctx->d.nf ? ctx->cb : f), "backproject");
+    }
     if (ctx->d.nf) CK(launch_mix(ctx, ctx->cb, f, ctx->d.nf, ctx->d.m, 1, ctx->d.nf), "analysis^T");  // T(q,j) = psi[j*nf + q]
     return CP4D_OK;
 }
@@ -174,7 +181,7 @@ int cp4d_create(const cp4d_params *p, cp4d_ctx **out) {
         int cur = -1;
         if (cudaGetDevice(&cur) != cudaSuccess || cur != p->device) { cudaGetLastError(); return CP4D_ECUDA; }
     }
-    if (forward_init() != cudaSuccess) { cudaGetLastError(); return CP4D_ECUDA; }
+    if (forward_init() != cudaSuccess || backproject_mma_init() != cudaSuccess) { cudaGetLastError(); return CP4D_ECUDA; }
 
     cp4d_ctx *ctx = new (std::nothrow) cp4d_ctx();
     if (!ctx) return CP4D_ENOMEM;
@@ -188,7 +195,7 @@ int cp4d_create(const cp4d_params *p, cp4d_ctx **out) {
     ctx->h2 = (float *)(w + cv.h2); ctx->h1 = (float *)(w + cv.h1); ctx->g = (float *)(w + cv.g);
     ctx->tmp_s = (float *)(w + cv.tmp_s);
     ctx->fwang = (FwAngle *)(w + cv.fwang); ctx->fworder = (int32_t *)(w + cv.fworder);
-    ctx->fw_pairs = (int2 *)(w + cv.fwpairs); ctx->fw_mode = CP4D_FORWARD_AUTO;
+    ctx->fw_pairs = (int2 *)(w + cv.fwpairs); ctx->fw_mode = CP4D_PROJ_AUTO;
     ctx->cf = d.nf ? (float *)(w + cv.cf) : nullptr; ctx->cb = d.nf ? (float *)(w + cv.cb) : nullptr;
     ctx->psi = d.nf ? (float *)(w + cv.psi) : nullptr;
     ctx->scratch = (float4 *)(w + cv.scratch); ctx->psum = (float4 *)(w + cv.psum); ctx->phi = (float *)(w + cv.phi);
@@ -703,21 +710,27 @@ int cp4d_graph_replays(const cp4d_ctx *ctx, uint64_t *out) {
     return CP4D_OK;
 }
 
-int cp4d_set_forward_mode(cp4d_ctx *ctx, int32_t mode) {
+int cp4d_set_projector_mode(cp4d_ctx *ctx, int32_t mode) {
     if (!ctx) return CP4D_EINVAL;
-    if (mode != CP4D_FORWARD_AUTO && mode != CP4D_FORWARD_FP32) return fail(ctx, CP4D_EINVAL, "set_forward_mode: unknown mode");
-    if (mode != ctx->fw_mode && ctx->iter_graph) {      // the captured iteration holds the other kernel
-        DevGuard dev_guard(ctx->device);
-        cudaGraphExecDestroy(ctx->iter_graph);
-        ctx->iter_graph = nullptr;
+    DevGuard dev_guard(ctx->device);
+    if (mode != CP4D_PROJ_AUTO && mode != CP4D_PROJ_FP32 && mode != CP4D_PROJ_TENSOR) return fail(ctx, CP4D_EINVAL, "set_projector_mode: unknown mode");
+    if (mode != ctx->fw_mode) {
+        if (ctx->iter_graph) {                          // the captured iteration holds the other kernels
+            cudaGraphExecDestroy(ctx->iter_graph);
+            ctx->iter_graph = nullptr;
+        }
+        // the two adjoints lay the folded sinogram out differently in the same scratch and both rely on rows whose pads are zero
+        CK(cudaMemsetAsync(ctx->scratch, 0, (size_t)ctx->d.scratch4 * 16, ctx->stream), "set_projector_mode");
     }
     ctx->fw_mode = mode;
     return CP4D_OK;
 }
 
-int cp4d_forward_mode_in_use(const cp4d_ctx *ctx, int32_t *mode_out) {
-    if (!ctx || !mode_out) return CP4D_EINVAL;
-    *mode_out = (ctx->fw_mode != CP4D_FORWARD_FP32 && forward_mma_supported(ctx->d)) ? CP4D_FORWARD_TENSOR : CP4D_FORWARD_FP32;
+int cp4d_projector_mode_in_use(const cp4d_ctx *ctx, int32_t *forward_out, int32_t *adjoint_out) {
+    if (!ctx) return CP4D_EINVAL;
+    const bool ok = forward_mma_supported(ctx->d);
+    if (forward_out) *forward_out = (ctx->fw_mode != CP4D_PROJ_FP32 && ok) ? CP4D_PROJ_TENSOR : CP4D_PROJ_FP32;
+    if (adjoint_out) *adjoint_out = (ctx->fw_mode == CP4D_PROJ_TENSOR && ok) ? CP4D_PROJ_TENSOR : CP4D_PROJ_FP32;
     return CP4D_OK;
 }
 

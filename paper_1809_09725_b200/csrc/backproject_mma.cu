@@ -1,0 +1,338 @@
+// Adjoint projector on the tensor cores (Eq. 10; fold L204-L212): backprojection of the pi-folded sinogram over
+// the base angles as small dense products  D[16 batch entries x 8 voxels] += G[16 x 16 bins] * W[16 bins x 8 voxels]  -- the
+// transpose of forward_mma.cu, and the friendlier side of the pair:
+//   * a 4 x 4 block of voxels touches at most 3 (|c| + |s|) + 3 <= 7.3 consecutive bins at ANY angle, so one 8-bin window per
+//     angle holds every tap of the block: K = 16 = the 8-bin windows of two base angles (any two: no pairing condition),
+//     N = 8 voxels = half a block, 32 of the 128 weights are non-zero, and nothing is ever trimmed (100 % fill);
+//   * the operand that comes from shared memory (the folded sinogram window) is shared by the two halves of a block: one
+//     ldmatrix pair per six HMMAs, so the LSU pipe that binds the forward kernel is at half load here;
+//   * the accumulators are voxels: they stay in registers over all base angles and are written once -- no atomics.
+// Operands are split bf16 pairs as in the forward kernel (G = Gh + Gl is written that way by k_fold_split, W = Wh + Wl per
+// weight; D += Gh Wh + Gl Wh + Gh Wl, fp32 accumulation): relative error about 5e-6.
+//
+// CTA = (32 x 32 tile, group of NB16 16-entry batch blocks of (slice, coefficient)); warp w owns four 4 x 4 blocks.  The tile's
+// bin windows of BM_STAGE base angles are staged by TMA 1-D bulk copies (SASS UBLKCP) into a two-stage ring: per angle and
+// 8-entry half one copy of BM_WINP bins x 16 B out of the zero-padded rows of gt, so no bounds logic is needed.
+#include <cuda_bf16.h>
+
+#include <algorithm>
+#include <cmath>
+
+#include "cp4d_internal.cuh"
+
+namespace cp4d {
+
+namespace {
+
+constexpr int BM_THREADS = 512;
+constexpr int BM_STAGE = 12;                       // base angles per pipeline stage (even: they are consumed two at a time)
+constexpr int BM_WINP = WIN + 8;                   // staged bins per angle: any 8-bin window that starts inside the tile's window
+constexpr int BM_BLOCKS = (TILE / 4) * (TILE / 4) / (BM_THREADS / 32);   // 4 x 4 voxel blocks per warp
+
+struct BmArgs {
+    int n, nz, nd, n0, m, mshift, gp, gpl;
+    int tiles, agroups;
+    int zper;                                      // slices per CTA = NB16 * 16 / m
+    const AngleTab *ang;
+    const TileGeo *geo;
+};
+
+// per staged base angle (shared memory, broadcast loads)
+struct BmAngle {
+    float cmin;    // delta + min(0, 3c) + min(0, 3s): smallest window coordinate of a block is cmin + X0 c + Y0 s
+    float delta, c, s;
+    float A1, A2;  // Joseph hat in bin units: weight(bin) = max(0, A1 - A2 |u - bin|), A1 = 1/a, A2 = 1/a^2 (0, 0 for a dummy)
+    float pad0, pad1;
+};
+
+__device__ __forceinline__ void mma16816(float (&d)[4], const unsigned (&a)[4], unsigned b0, unsigned b1) {
+    asm volatile("mma.sync.aligned.m16n8k16.row.col.f32.bf16.bf16.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};\n"
+                 : "+f"(d[0]), "+f"(d[1]), "+f"(d[2]), "+f"(d[3])
+                 : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(b0), "r"(b1));
+}
+__device__ __forceinline__ void ldsm4t(unsigned (&a)[4], unsigned addr) {
+    asm volatile("ldmatrix.sync.aligned.m8n8.x4.trans.shared.b16 {%0,%1,%2,%3}, [%4];\n"
+                 : "=r"(a[0]), "=r"(a[1]), "=r"(a[2]), "=r"(a[3]) : "r"(addr));
+}
+__device__ __forceinline__ void split2(float x, float y, unsigned &hi, unsigned &lo) {
+    const __nv_bfloat162 h = __floats2bfloat162_rn(x, y);
+    const __nv_bfloat162 l = __floats2bfloat162_rn(x - __low2float(h), y - __high2float(h));
+    hi = *reinterpret_cast<const unsigned *>(&h);
+    lo = *reinterpret_cast<const unsigned *>(&l);
+}
+// ---- TMA 1D bulk copy global -> shared, completion on an mbarrier ----
+__device__ __forceinline__ unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t *bar, unsigned count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;\n" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, unsigned bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t *bar, unsigned parity) {
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_%=:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra DONE_%=;\n"
+        "bra WAIT_%=;\n"
+        "DONE_%=:\n"
+        "}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(void *dst_smem, const void *src_gmem, unsigned bytes, uint64_t *bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];\n" ::"r"(smem_u32(dst_smem)),
+                 "l"(src_gmem), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+}
+
+// gt (split layout, written by k_fold_split): 16-byte units of 8 bf16 batch entries,
+//   unit index = ((((zg n0 + i) 2 + hl) H + half) gp + gpl + b),  H = 2 NB16 halves per z-group, hl = 0 hi / 1 lo
+template <int NB16>
+__global__ void __launch_bounds__(BM_THREADS, 1) k_backproject_mma(const uint4 *__restrict__ gt, float *__restrict__ out, BmArgs a) {
+    constexpr int H = 2 * NB16;
+    constexpr int ANGLE_UNITS = 2 * H * BM_WINP;                 // 16-byte units per staged angle: [hl][half][bin]
+    constexpr unsigned STAGE_BYTES = BM_STAGE * ANGLE_UNITS * 16;
+    extern __shared__ __align__(128) unsigned char win[];         // [2 stages][BM_STAGE][2][H][BM_WINP] x 16 B
+    __shared__ __align__(16) BmAngle sang[2][BM_STAGE];
+    __shared__ __align__(8) uint64_t mbar[2];
+    const int tiles_1d = (a.n + TILE - 1) / TILE;
+    const int tile_id = blockIdx.x % a.tiles, ag = blockIdx.x / a.tiles;
+    const int zg = blockIdx.y, z0 = zg * a.zper;
+    const int tx0 = (tile_id % tiles_1d) * TILE, ty0 = (tile_id / tiles_1d) * TILE;
+    const TileGeo *geo = a.geo + (int64_t)tile_id * a.n0;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, g = lane >> 2, t = lane & 3;
+    const unsigned ld_half = (lane >> 3) & 1, ld_col = lane >> 4, ld_row = lane & 7;
+    // this CTA's share [g0, g1) of the base angles (small problems split them over CTAs, which then ADD into a zeroed output)
+    const int g0 = (int)((int64_t)a.n0 * ag / a.agroups), g1 = (int)((int64_t)a.n0 * (ag + 1) / a.agroups);
+    const int n_stage = (g1 - g0 + BM_STAGE - 1) / BM_STAGE;
+    if (threadIdx.x == 0) {
+        mbar_init(&mbar[0], 1);
+        mbar_init(&mbar[1], 1);
+        asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
+    }
+    __syncthreads();
+
+    auto stage = [&](int buf, int st) {
+        const int i0 = g0 + st * BM_STAGE;
+        if (threadIdx.x < BM_STAGE) {
+            const int i = i0 + (int)threadIdx.x;
+            const bool real = i < g1;
+            const AngleTab A = a.ang[min(i, g1 - 1)];
+            const float d = geo[min(i, g1 - 1)].delta, A2 = A.inv_a * A.inv_a;
+            BmAngle &S = sang[buf][threadIdx.x];
+            S.cmin = d + fminf(0.f, 3.0f * A.c) + fminf(0.f, 3.0f * A.s);
+            S.delta = d; S.c = A.c; S.s = A.s;
+            S.A1 = real ? A.inv_a : 0.f; S.A2 = real ? A2 : 0.f;      // an angle past the end weighs nothing
+            S.pad0 = S.pad1 = 0.f;
+        }
+        if (threadIdx.x < 32) {
+            constexpr int ROWS = BM_STAGE * 2 * H;                     // one copy per (angle, hi/lo, half)
+            if (threadIdx.x == 0) mbar_expect_tx(&mbar[buf], (unsigned)(ROWS * BM_WINP * 16));
+            __syncwarp();
+            for (int r = threadIdx.x; r < ROWS; r += 32) {
+                const int aa = r / (2 * H), hh = r % (2 * H);           // hh = hl * H + half
+                const int i = min(i0 + aa, g1 - 1);
+                const uint4 *src = gt + (((int64_t)zg * a.n0 + i) * (2 * H) + hh) * a.gp + a.gpl + geo[i].bstart;
+                bulk_g2s(win + (size_t)buf * STAGE_BYTES + (size_t)(aa * 2 * H + hh) * BM_WINP * 16, src, BM_WINP * 16, &mbar[buf]);
+            }
+        }
+    };
+
+    float acc[BM_BLOCKS][2][NB16][4];
+#pragma unroll
+    for (int q = 0; q < BM_BLOCKS; ++q)
+#pragma unroll
+        for (int h = 0; h < 2; ++h)
+#pragma unroll
+            for (int zb = 0; zb < NB16; ++zb) acc[q][h][zb][0] = acc[q][h][zb][1] = acc[q][h][zb][2] = acc[q][h][zb][3] = 0.f;
+
+    const unsigned win_s = smem_u32(win);
+    // my voxel as column g of the weight block: (g & 3, g >> 2) inside the half block; half h adds two rows
+    const float vx = (float)(g & 3), vy = (float)(g >> 2);
+    if (n_stage > 0) stage(0, 0);
+    __syncthreads();
+    for (int st = 0; st < n_stage; ++st) {
+        const int buf = st & 1;
+        // buffer buf^1 and sang[buf^1] were last read in the previous iteration, which ended with __syncthreads
+        if (st + 1 < n_stage) stage(buf ^ 1, st + 1);
+        mbar_wait(&mbar[buf], (st >> 1) & 1);
+#pragma unroll 1
+        for (int p = 0; p < BM_STAGE; p += 2) {
+            const BmAngle S0 = sang[buf][p], S1 = sang[buf][p + 1];
+#pragma unroll
+            for (int q = 0; q < BM_BLOCKS; ++q) {
+                const int bid = warp * BM_BLOCKS + q;
+                const float X0 = (float)(4 * (bid & 7)), Y0 = (float)(4 * (bid >> 3));
+                // 8-bin window of the block at either angle: from the smallest window coordinate of its 16 voxels
+                const int q0 = min(max((int)floorf(fmaf(X0, S0.c, fmaf(Y0, S0.s, S0.cmin))), 0), BM_WINP - 8);
+                const int q1 = min(max((int)floorf(fmaf(X0, S1.c, fmaf(Y0, S1.s, S1.cmin))), 0), BM_WINP - 8);
+                const unsigned adr = win_s + buf * STAGE_BYTES +
+                                     ((((p + ld_col) * 2 * H + ld_half) * BM_WINP + (ld_col ? q1 : q0) + ld_row) << 4);
+                unsigned ah[NB16][4], al[NB16][4];
+#pragma unroll
+                for (int zb = 0; zb < NB16; ++zb) {
+                    ldsm4t(ah[zb], adr + (2 * zb) * BM_WINP * 16);
+                    ldsm4t(al[zb], adr + (H + 2 * zb) * BM_WINP * 16);
+                }
+                // window coordinate of my voxel in half 0, relative to bin q + 2t of each angle; half 1 is two rows further
+                const float d0 = fmaf(X0 + vx, S0.c, fmaf(Y0 + vy, S0.s, S0.delta)) - (float)(q0 + 2 * t);
+                const float d1 = fmaf(X0 + vx, S1.c, fmaf(Y0 + vy, S1.s, S1.delta)) - (float)(q1 + 2 * t);
+#pragma unroll
+                for (int h = 0; h < 2; ++h) {
+                    const float e0 = fmaf(2.0f * (float)h, S0.s, d0), e1 = fmaf(2.0f * (float)h, S1.s, d1);
+                    const float w0 = fmaxf(0.f, fmaf(-S0.A2, fabsf(e0), S0.A1)), w1 = fmaxf(0.f, fmaf(-S0.A2, fabsf(e0 - 1.0f), S0.A1));
+                    const float w2 = fmaxf(0.f, fmaf(-S1.A2, fabsf(e1), S1.A1)), w3 = fmaxf(0.f, fmaf(-S1.A2, fabsf(e1 - 1.0f), S1.A1));
+                    unsigned bh0, bl0, bh1, bl1;
+                    split2(w0, w1, bh0, bl0);
+                    split2(w2, w3, bh1, bl1);
+#pragma unroll
+                    for (int zb = 0; zb < NB16; ++zb) {
+                        mma16816(acc[q][h][zb], ah[zb], bh0, bh1);
+                        mma16816(acc[q][h][zb], al[zb], bh0, bh1);
+                        mma16816(acc[q][h][zb], ah[zb], bl0, bl1);
+                    }
+                }
+            }
+        }
+        __syncthreads();
+    }
+    // ---- write the voxels: my D entries are voxels 2t, 2t+1 of each half block x batch entries g, g + 8 ----
+#pragma unroll
+    for (int q = 0; q < BM_BLOCKS; ++q) {
+        const int bid = warp * BM_BLOCKS + q;
+#pragma unroll
+        for (int h = 0; h < 2; ++h)
+#pragma unroll
+            for (int cc = 0; cc < 2; ++cc) {
+                const int n = 2 * t + cc;
+                const int x = tx0 + 4 * (bid & 7) + (n & 3), y = ty0 + 4 * (bid >> 3) + 2 * h + (n >> 2);
+                if (x >= a.n || y >= a.n) continue;
+#pragma unroll
+                for (int zb = 0; zb < NB16; ++zb)
+#pragma unroll
+                    for (int r = 0; r < 2; ++r) {
+                        const int flat = zb * 16 + g + 8 * r, sl = z0 + (flat >> a.mshift), j = flat & (a.m - 1);
+                        if (sl >= a.nz) continue;
+                        float *dst = out + (((int64_t)sl * a.n + y) * a.n + x) * a.m + j;
+                        if (a.agroups == 1) *dst = acc[q][h][zb][2 * r + cc];
+                        else atomicAdd(dst, acc[q][h][zb][2 * r + cc]);
+                    }
+            }
+    }
+}
+
+// Fold for the tensor-core backprojector: gt_j[z][i][b] = sum_q Phi[j, q n0 + i] g[z][q n0 + i][flip_q b],
+// written as split bf16 pairs in the layout k_backproject_mma stages.  One CTA per (z, base angle i), one thread per bin.
+template <int Q>
+__global__ void __launch_bounds__(128) k_fold_split(const float *__restrict__ g, uint4 *__restrict__ gt, const float *__restrict__ phi,
+                                                    int nd, int na, int npi, int n0, int gp, int gpl, int zper, int H) {
+    extern __shared__ float phis[];  // [q][j]
+    const int z = blockIdx.x / n0, i = blockIdx.x % n0;
+    constexpr int m = 4 * Q;
+    for (int t = threadIdx.x; t < npi * m; t += blockDim.x) phis[t] = phi[(int64_t)(t % m) * na + (t / m) * n0 + i];
+    __syncthreads();
+    const int zg = z / zper, flat0 = (z - zg * zper) * m;         // first batch entry of this slice inside its z-group
+    unsigned short *hi = reinterpret_cast<unsigned short *>(gt + ((int64_t)zg * n0 + i) * 2 * H * gp);
+    unsigned short *lo = hi + (int64_t)H * gp * 8;
+    for (int b = threadIdx.x; b < nd; b += blockDim.x) {
+        float acc[m];
+#pragma unroll
+        for (int j = 0; j < m; ++j) acc[j] = 0.f;
+        for (int q0 = 0; q0 < npi; q0 += 4) {     // 4 half-rotations per batch: their loads are in flight together
+            float gv[4];
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                const int q = min(q0 + u, npi - 1), bb = (q & 1) ? nd - 1 - b : b;
+                gv[u] = __ldg(g + ((int64_t)z * na + q * n0 + i) * nd + bb);
+            }
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                if (q0 + u < npi) {
+#pragma unroll
+                    for (int j = 0; j < m; ++j) acc[j] = fmaf(phis[(q0 + u) * m + j], gv[u], acc[j]);
+                }
+            }
+        }
+        // entries flat0 + j, j < m: 8-entry unit (flat0 + j) / 8 of the z-group, position (flat0 + j) % 8 -- in runs of 4
+#pragma unroll
+        for (int jc = 0; jc < Q; ++jc) {
+            const int flat = flat0 + 4 * jc;
+            const int64_t e = ((int64_t)(flat >> 3) * gp + gpl + b) * 8 + (flat & 7);
+            unsigned h01, l01, h23, l23;
+            split2(acc[4 * jc], acc[4 * jc + 1], h01, l01);
+            split2(acc[4 * jc + 2], acc[4 * jc + 3], h23, l23);
+            *reinterpret_cast<uint2 *>(hi + e) = make_uint2(h01, h23);
+            *reinterpret_cast<uint2 *>(lo + e) = make_uint2(l01, l23);
+        }
+    }
+}
+
+template <int NB16>
+cudaError_t bm_launch(cp4d_ctx *c, const uint4 *gt, float *out, BmArgs a) {
+    const Dims &d = c->d;
+    a.zper = NB16 * 16 / d.m;
+    const int zgroups = (d.nz + a.zper - 1) / a.zper;
+    // small problems: split the base angles over up to 8 CTAs per tile, which add their partial sums into a zeroed output
+    const int64_t ctas = (int64_t)d.tiles * zgroups;
+    a.agroups = (int)std::max<int64_t>(1, std::min<int64_t>(std::min(8, std::max(1, d.n0 / BM_STAGE)), 148 / ctas));
+    if (a.agroups > 1) {
+        const cudaError_t e = cudaMemsetAsync(out, 0, (size_t)d.nz * d.n * d.n * d.m * sizeof(float), c->stream);
+        if (e != cudaSuccess) return e;
+        c->launches++;
+    }
+    const dim3 grid(d.tiles * a.agroups, zgroups);
+    k_backproject_mma<NB16><<<grid, BM_THREADS, (size_t)2 * BM_STAGE * 2 * 2 * NB16 * BM_WINP * 16, c->stream>>>(gt, out, a);
+    return cudaGetLastError();
+}
+
+#define CP4D_BM_DISPATCH_Q(Qv, CALL)                       \
+    switch (Qv) {                                          \
+    case 1: { constexpr int QQ = 1; CALL; } break;         \
+    case 2: { constexpr int QQ = 2; CALL; } break;         \
+    case 4: { constexpr int QQ = 4; CALL; } break;         \
+    default: { constexpr int QQ = 8; CALL; } break;        \
+    }
+
+}  // namespace
+
+// 16-entry batch blocks per CTA of the tensor-core backprojector (also fixes the layout k_fold_split writes)
+int backproject_mma_nb16(const Dims &d) {
+    const int blocks_total = (d.nz * d.m + 15) / 16;
+    return d.m == 32 ? 2 : std::min(2, blocks_total);
+}
+
+// 16-byte units of gt in the split layout (>= what the fp32 layout of the same scratch needs when nz is a multiple of zper)
+int64_t backproject_mma_scratch_units(const Dims &d) {
+    const int nb = backproject_mma_nb16(d), zper = nb * 16 / d.m, zgroups = (d.nz + zper - 1) / zper;
+    return (int64_t)zgroups * d.n0 * 2 * (2 * nb) * d.gp;
+}
+
+cudaError_t backproject_mma_init() {
+    cudaError_t e = cudaFuncSetAttribute(k_backproject_mma<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, 2 * BM_STAGE * 2 * 2 * 1 * BM_WINP * 16);
+    if (e != cudaSuccess) return e;
+    return cudaFuncSetAttribute(k_backproject_mma<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, 2 * BM_STAGE * 2 * 2 * 2 * BM_WINP * 16);
+}
+
+cudaError_t launch_fold_split(cp4d_ctx *c, const float *g, float4 *gt) {
+    ProfScope ps(c, CP4D_K_FOLD);
+    const Dims &d = c->d;
+    const int nb = backproject_mma_nb16(d), zper = nb * 16 / d.m;
+    const size_t sh = (size_t)d.npi * d.m * sizeof(float);
+    uint4 *G = reinterpret_cast<uint4 *>(gt);
+    CP4D_BM_DISPATCH_Q(d.Q, (k_fold_split<QQ><<<d.nz * d.n0, 128, sh, c->stream>>>(g, G, c->phi, d.nd, d.na, d.npi, d.n0, d.gp, d.gpl, zper, 2 * nb)));
+    c->launches++;
+    return cudaGetLastError();
+}
+
+cudaError_t launch_backproject_mma(cp4d_ctx *c, const float4 *gt, float *f_out) {
+    ProfScope ps(c, CP4D_K_BACKPROJECT);
+    const Dims &d = c->d;
+    int ms = 0;
+    while ((1 << ms) < d.m) ++ms;
+    BmArgs a{d.n, d.nz, d.nd, d.n0, d.m, ms, d.gp, d.gpl, d.tiles, 1, 0, c->ang, c->geo};
+    c->launches++;
+    const uint4 *G = reinterpret_cast<const uint4 *>(gt);
+    if (backproject_mma_nb16(d) == 1) return bm_launch<1>(c, G, f_out, a);
+    return bm_launch<2>(c, G, f_out, a);
+}
+
+}  // namespace cp4d

@@ -83,7 +83,7 @@ struct cp4d_ctx {
     cp4d::FwTable *fwtab_host; // host copy of fwang / fworder for the kernel-parameter path (n0 <= 512), else null
     int2 *fw_pairs;            // tensor-core forward projector (forward_mma.cu): base angles of each pass paired with a neighbour
     int n_pairs0, n_pairs1;
-    int fw_mode;               // CP4D_FORWARD_AUTO / _FP32 (cp4d_set_forward_mode)
+    int fw_mode;               // CP4D_PROJ_AUTO / _FP32 (cp4d_set_projector_mode): both projectors
     int n_cpos;                // the first n_cpos base angles have cos >= 0 (backprojector: chunks never mix the signs)
     cp4d::TileGeo *geo;        // [tile][n0]
     double *red;               // 8 doubles for reductions
@@ -141,6 +141,12 @@ bool forward_mma_supported(const Dims &d);
 cudaError_t forward_mma_init();
 int forward_mma_pairs(const FwAngle *fw, const int32_t *order, int n0, int n_colstep, int2 *out, int *npairs0, int *npairs1);
 cudaError_t launch_forward_mma(cp4d_ctx *c, const float *f, float *P);
+// backproject_mma.cu: the tensor-core adjoint (fold into split-bf16 rows + backprojection); same shapes as forward_mma
+int backproject_mma_nb16(const Dims &d);
+int64_t backproject_mma_scratch_units(const Dims &d);
+cudaError_t backproject_mma_init();
+cudaError_t launch_fold_split(cp4d_ctx *c, const float *g, float4 *gt);
+cudaError_t launch_backproject_mma(cp4d_ctx *c, const float4 *gt, float *f_out);
 cudaError_t launch_backproject(cp4d_ctx *c, const float4 *gt, float *f_out, int Q_override = 0);
 // cp4d_fbp: Shepp-Logan filter along the bins; per-half-rotation rows gathered into the projector scratch (box basis)
 cudaError_t launch_filter_sl(cp4d_ctx *c, const float *g, float *gf);

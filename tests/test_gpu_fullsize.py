@@ -69,11 +69,11 @@ def test_sampled_forward_adjoint(torch_cuda, fast_oracle, cfg):
     zsel = torch.as_tensor(np.asarray(zs)[zi], device="cuda")
     pick = lambda K: K[zsel, torch.as_tensor(zkb_local[:, 1].astype(np.int64), device="cuda"),
                        torch.as_tensor(zkb_local[:, 2].astype(np.int64), device="cuda")].cpu().numpy()
-    assert ctx.forward_mode_in_use() == "tensor"                  # the kernel bench.py times (split-bf16 HMMA, fp32 accumulate)
+    assert ctx.projector_mode_in_use() == ("tensor", "fp32")                  # the kernel bench.py times (split-bf16 HMMA, fp32 accumulate)
     e_tensor = rel(pick(Kf), ref)
-    ctx.set_forward_mode("fp32")                                  # and the exact-fp32 gather on the same rays
+    ctx.set_projector_mode("fp32")                                  # and the exact-fp32 gather on the same rays
     e_fp32 = rel(pick(ctx.forward(f, out=Kf)), ref)
-    ctx.set_forward_mode("auto")
+    ctx.set_projector_mode("auto")
     print(f"config {cfg}: sampled forward rel-L2 tensor {e_tensor:.2e}, fp32 {e_fp32:.2e}")
     assert e_tensor <= 2e-5 and e_fp32 <= TOL_OP
     del f3
@@ -86,6 +86,14 @@ def test_sampled_forward_adjoint(torch_cuda, fast_oracle, cfg):
     got = Ktg[zsel, torch.as_tensor(zyx_local[:, 1].astype(np.int64), device="cuda"),
               torch.as_tensor(zyx_local[:, 2].astype(np.int64), device="cuda")].cpu().numpy()
     assert rel(got, ref) <= TOL_OP
+    ctx.set_projector_mode("tensor")                              # the tensor-core backprojector (not the default) on the same voxels
+    Ktg = ctx.adjoint(g, out=Ktg)
+    e_tensor = rel(Ktg[zsel, torch.as_tensor(zyx_local[:, 1].astype(np.int64), device="cuda"),
+                       torch.as_tensor(zyx_local[:, 2].astype(np.int64), device="cuda")].cpu().numpy(), ref)
+    ctx.set_projector_mode("auto")
+    Ktg = ctx.adjoint(g, out=Ktg)
+    print(f"config {cfg}: sampled adjoint rel-L2 tensor {e_tensor:.2e}")
+    assert e_tensor <= 2e-5
     # ---- fp32 adjoint identity on the GPU: <K1 f, g> = <f, K1^T g> (f was overwritten, so redo it with a fresh pair)
     f2 = torch.randn(ctx.primal_shape, generator=gen, device="cuda", dtype=torch.float32)
     Kf = ctx.forward(f2, out=Kf)

@@ -75,18 +75,19 @@ def test_forward_adjoint(torch_cuda, fast_oracle, case):
     c, P, ctx = make(case, fast_oracle)
     f, g = synth.test_vectors(c)
     f32, g32 = f.astype(np.float32), g.astype(np.float32)
-    ref_f = P.forward(f32.astype(np.float64), folded=True)
-    # both forward projectors: the exact-fp32 gather and (where m allows) the tensor-core one with split-bf16 operands, whose
-    # relative error must stay an order of magnitude inside the tolerance (about 5e-6 measured, 1.1e-5 bound)
-    ctx.set_forward_mode("fp32")
-    assert ctx.forward_mode_in_use() == "fp32"
-    assert rel(ctx.forward(dev(torch_cuda, f32)).cpu().numpy(), ref_f) <= TOL_OP
-    ctx.set_forward_mode("auto")
-    assert ctx.forward_mode_in_use() == ("tensor" if c.m in (4, 8, 16, 32) else "fp32")
-    Kf = ctx.forward(dev(torch_cuda, f32)).cpu().numpy()
-    Ktg = ctx.adjoint(dev(torch_cuda, g32)).cpu().numpy()
-    assert rel(Kf, ref_f) <= (2e-5 if ctx.forward_mode_in_use() == "tensor" else TOL_OP)
-    assert rel(Ktg, P.adjoint(g32.astype(np.float64), folded=True)) <= TOL_OP
+    ref_f, ref_a = P.forward(f32.astype(np.float64), folded=True), P.adjoint(g32.astype(np.float64), folded=True)
+    # every kernel of both sides: the exact-fp32 ones and (where m allows) the tensor-core ones with split-bf16 operands, whose
+    # relative error must stay well inside the tolerance (about 5e-6 measured, 1.1e-5 bound); the modes are switched
+    # back and forth on one context, which also checks that the two layouts of the folded sinogram do not leak into each other
+    can = c.m in (4, 8, 16, 32)
+    for mode in ("tensor", "fp32", "auto"):
+        ctx.set_projector_mode(mode)
+        want = {"tensor": ("tensor", "tensor"), "fp32": ("fp32", "fp32"), "auto": ("tensor", "fp32")}[mode] if can else ("fp32", "fp32")
+        assert ctx.projector_mode_in_use() == want
+        Kf = ctx.forward(dev(torch_cuda, f32)).cpu().numpy()
+        Ktg = ctx.adjoint(dev(torch_cuda, g32)).cpu().numpy()
+        assert rel(Kf, ref_f) <= (2e-5 if want[0] == "tensor" else TOL_OP), mode
+        assert rel(Ktg, ref_a) <= (2e-5 if want[1] == "tensor" else TOL_OP), mode
     # GPU-side adjoint identity in fp32 (fp64-accumulated dots)
     lhs = ctx.dot(dev(torch_cuda, Kf), dev(torch_cuda, g32))
     rhs = ctx.dot(dev(torch_cuda, f32), dev(torch_cuda, Ktg))
