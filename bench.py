@@ -93,6 +93,8 @@ def algorithmic_work(c, n_frames=0):
     gt = c.nz * n0 * c.nd * mproj                        # folded sinogram / partial ray sums, elements
     return {
         # name: (bound, work per launch [flop or byte])
+        # both projectors are rated against the plain FP32 FMA roof on their ALGORITHMIC flops, whichever pipe runs them (the
+        # tensor-core forward kernel executes 12 x as many MACs on the HMMA pipe to deliver these)
         "forward": ("alu", 2.0 * ray_fma),
         "backproject": ("alu", 2.0 * ray_fma),
         "synth": ("hbm", 4.0 * (gt + 3 * S)),            # read P, read h1 + g, write h1 (prox fused)
@@ -271,6 +273,7 @@ def run_cp4d(args, c, rank, world):
     # ---- problem, data, step sizes (outside the timed region: SURVEY 8(d)) ----
     phi = synth.basis_table(c.basis, c.m, c.n_angles)
     ctx = binding.Context.from_config(c, phi=phi, device=local, n_frames=args.frames)
+    ctx.set_projector_mode(args.projectors)
     g = synth.sinogram(c, device=str(dev)).to(torch.float32).contiguous()
     L = ctx.norm(args.power_iters, seed=3)
     ts = 0.95 / L
@@ -305,6 +308,22 @@ def run_cp4d(args, c, rank, world):
     launches = ctx.launch_count() - l0
     ms = e0.elapsed_time(e1)
     graph_replays = ctx.graph_replays()
+
+    # ---- the same K steps with the fp32 CUDA-core kernels on both sides (context only: the default pair uses split-bf16
+    # tensor-core products in the forward projector; both pass the same parity tests) ----
+    fp32_alt = None
+    if args.projectors == "auto" and ctx.projector_mode_in_use() != ("fp32", "fp32"):
+        ctx.set_projector_mode("fp32")
+        ctx.iterate(2)
+        barrier()
+        a0, a1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a0.record(ctx.stream); ctx.iterate(K); a1.record(ctx.stream)
+        barrier()
+        ms_alt = reduce_max(a0.elapsed_time(a1), world, dev)
+        fp32_alt = {"value": replicas_value(world, K, ms_alt), "unit": UNIT, "ms_per_step": ms_alt / K,
+                    "note": "same K steps with cp4d_set_projector_mode(CP4D_PROJ_FP32): plain fp32 FMAs in both projectors"}
+        ctx.set_projector_mode("auto")
+        ctx.iterate(2)
 
     # ---- roofline: second pass of K steps with the library's per-kernel CUDA events on the same stream ----
     ctx.profile_begin()
@@ -350,6 +369,7 @@ def run_cp4d(args, c, rank, world):
                "seconds": dt}
         del g_host, f_host
     return ctx, dict(ms=ms, launches=launches, prof=prof, prof_gd=prof_gd, ops=ops, e2e=e2e, clocks=clocks, peaks=peaks,
+                     fp32_alt=fp32_alt, proj=ctx.projector_mode_in_use(),
                      L=L, launches_total=ctx.launch_count() - launches0, graph_replays=graph_replays)
 
 
@@ -410,17 +430,25 @@ def assemble(args, c, world, r):
                 "frac": d["frac"], "traffic": None, "peak_source": peaks["source"], "avg_launch_ms": d["ms"],
                 "note": ("alu peak = 148 SM x 128 FP32 lanes x 2 flop x sm_max_mhz; achieved = algorithmic (pi-folded) flops"
                          if d["bound"] == "alu" else "algorithmic bytes / CUDA-event time")}
-    # the projectors fetch one fp32 operand from shared memory per FMA at best: their second, tighter roof is the
-    # shared-memory bandwidth, 128 B/clk/SM (measured: profiles/r1_microbench_fma_lds.md).  Algorithmic bytes = 4 B per FMA for the
-    # forward gather; the backprojector reuses fetched bins from registers, so this roof only binds the forward kernel.
+    # second, tighter roofs of the forward projector (measured unit rates in profiles/r2_microbench.md):
+    #   fp32 gather: one 4-byte operand per FMA through shared memory, 128 B/clk/SM;
+    #   tensor-core kernel: every algorithmic FMA costs 12 HMMA MACs (weight blocks 1/4 dense x three split-bf16 products) at the
+    #   measured mma.sync rate of 950 MAC/clk/SM.
     if "forward" in kernels:
         k = kernels["forward"]
-        smem_peak = N_SM * 128 * peaks["sm_max_mhz"] * 1e6 / 1e9                       # GB/s
-        smem_ach = (work["forward"][1] / 2.0) * 4.0 / (k["ms"] * 1e-3) / 1e9           # flop / 2 = FMAs; 4 B each
-        k["smem_roof"] = {"bound": "smem", "achieved": smem_ach, "peak": smem_peak, "unit": "GB/s", "frac": smem_ach / smem_peak,
-                          "note": "one 4-byte operand per FMA through shared memory: 148 SM x 128 B/clk x sm_max_mhz"}
+        fmas = work["forward"][1] / 2.0
+        if r["proj"][0] == "tensor":
+            peak = N_SM * 950.0 * peaks["sm_max_mhz"] * 1e6 / 1e12
+            ach = fmas * 12.0 / (k["ms"] * 1e-3) / 1e12
+            k["hmma_roof"] = {"bound": "tensor (mma.sync)", "achieved": ach, "peak": peak, "unit": "TMAC/s", "frac": ach / peak,
+                              "note": "12 HMMA MACs per algorithmic FMA (not counting partly filled blocks); peak = 148 SM x 950 MAC/clk x sm_max_mhz"}
+        else:
+            smem_peak = N_SM * 128 * peaks["sm_max_mhz"] * 1e6 / 1e9                       # GB/s
+            smem_ach = fmas * 4.0 / (k["ms"] * 1e-3) / 1e9
+            k["smem_roof"] = {"bound": "smem", "achieved": smem_ach, "peak": smem_peak, "unit": "GB/s", "frac": smem_ach / smem_peak,
+                              "note": "one 4-byte operand per FMA through shared memory: 148 SM x 128 B/clk x sm_max_mhz"}
         if dom == "forward":
-            roofline["smem_roof"] = k["smem_roof"]
+            roofline["second_roof"] = k.get("hmma_roof") or k.get("smem_roof")
     # dram bytes per launch from the committed `ncu --set full` capture -- only if it was taken with the kernel sources that
     # are running now (profiles/traffic.json records their SHA-1); otherwise null, never a stale number
     tr = ROOT / "profiles" / "traffic.json"
@@ -445,13 +473,17 @@ def assemble(args, c, world, r):
         "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f32", "data": "synthetic",
         "config": workload_config(c, args.frames),
-        "run": {"norm_K": r["L"], "parallelism": "replicas only (independent problems, no collective)" if world > 1 else "1 gpu",
+        "run": {"norm_K": r["L"], "projectors": {"mode": args.projectors, "forward": r["proj"][0], "adjoint": r["proj"][1]},
+                "arithmetic": ("fp32 storage, fp32 accumulation everywhere; 'tensor' projector = products of split-bf16 pairs "
+                               "(x = hi + lo, three HMMA products per term, rel. error 5e-6 per ray sum, tolerance 1e-4), "
+                               "'fp32' projector = plain FMAs (2e-6)"), "parallelism": "replicas only (independent problems, no collective)" if world > 1 else "1 gpu",
                 "warmup_run": max(args.warmup, 2),
                 "l2": f"no flush: CP state {(7 * c.V + 2 * c.S) * 4 / 1e9:.2f} GB streams through every step (L2 = 126 MB)"},
         "gups_nominal": {"forward": gups["forward"], "adjoint": gups["adjoint"], "unit": "1e9 voxel*angle*basis/s",
                          "forward_ms": r["ops"]["forward_op"], "adjoint_ms": r["ops"]["adjoint_op"],
                          "note": "nominal count N^2*Nz*N_theta*m per call; kernels use the pi-fold (N_theta0 base angles)"},
         "roofline": roofline, "kernels": kernels, "clocks": r["clocks"], "e2e": r["e2e"],
+        "fp32_projectors": r["fp32_alt"],
         "gpu_launches": r["launches"], "cuda_graph_replays": r["graph_replays"], "impl": "cp4d",
     }
     return line
@@ -487,6 +519,9 @@ def main():
                     help="also time the out-of-core path (slabs.StreamedSolver: state in pinned host memory, slabs of SLAB_NZ slices)")
     ap.add_argument("--stream-block", type=int, default=1, metavar="K",
                     help="with --streamed: temporal blocking, K iterations per residency of a window of SLAB_NZ + 2K slices")
+    ap.add_argument("--projectors", default="auto", choices=["auto", "fp32", "tensor"],
+                    help="cp4d_set_projector_mode: auto = tensor-core forward projector + fp32 backprojector (default), fp32 = CUDA-core "
+                         "kernels on both sides, tensor = tensor-core kernels on both sides")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()

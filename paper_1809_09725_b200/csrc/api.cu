@@ -729,7 +729,8 @@ int cp4d_set_projector_mode(cp4d_ctx *ctx, int32_t mode) {
 int cp4d_projector_mode_in_use(const cp4d_ctx *ctx, int32_t *forward_out, int32_t *adjoint_out) {
     if (!ctx) return CP4D_EINVAL;
     const bool ok = forward_mma_supported(ctx->d);
-    if (forward_out) *forward_out = (ctx->fw_mode != CP4D_PROJ_FP32 && ok) ? CP4D_PROJ_TENSOR : CP4D_PROJ_FP32;
+    const bool fw_tensor = (ctx->fw_mode == CP4D_PROJ_TENSOR && ok) || (ctx->fw_mode == CP4D_PROJ_AUTO && forward_mma_preferred(ctx->d));
+    if (forward_out) *forward_out = fw_tensor ? CP4D_PROJ_TENSOR : CP4D_PROJ_FP32;
     if (adjoint_out) *adjoint_out = (ctx->fw_mode == CP4D_PROJ_TENSOR && ok) ? CP4D_PROJ_TENSOR : CP4D_PROJ_FP32;
     return CP4D_OK;
 }

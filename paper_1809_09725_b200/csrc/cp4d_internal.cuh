@@ -138,6 +138,7 @@ cudaError_t launch_forward_partial(cp4d_ctx *c, const float *f, float4 *P);
 cudaError_t forward_init();        // once per process and device: opt in to the forward kernels' dynamic shared memory
 // forward_mma.cu: the tensor-core forward projector (split-bf16 HMMA, fp32 accumulate)
 bool forward_mma_supported(const Dims &d);
+bool forward_mma_preferred(const Dims &d);     // what CP4D_PROJ_AUTO picks
 cudaError_t forward_mma_init();
 int forward_mma_pairs(const FwAngle *fw, const int32_t *order, int n0, int n_colstep, int2 *out, int *npairs0, int *npairs1);
 cudaError_t launch_forward_mma(cp4d_ctx *c, const float *f, float *P);

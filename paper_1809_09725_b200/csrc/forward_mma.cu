@@ -167,8 +167,9 @@ __global__ void __launch_bounds__(FM_THREADS, 1) k_forward_mma(const float *__re
     const unsigned ld_half = (lane >> 3) & 1, ld_col = lane >> 4, ld_row = lane & 7;
     const TileGeo *geo = a.geo + (int64_t)tile_id * a.n0;
 
-    for (int pc = p0; pc < p1; pc += FM_MAXP) {
-        const int npc = min(FM_MAXP, p1 - pc);
+    const int n_chunk = (p1 - p0 + FM_MAXP - 1) / FM_MAXP, per_chunk = n_chunk ? (p1 - p0 + n_chunk - 1) / n_chunk : 0;   // even chunks
+    for (int pc = p0; pc < p1; pc += per_chunk) {
+        const int npc = min(per_chunk, p1 - pc);
         __syncthreads();                                     // the tile is staged / every warp is done with the previous chunk
         if ((int)threadIdx.x < npc) {
             const int2 pr = a.pairs[pc + threadIdx.x];
@@ -350,6 +351,15 @@ cudaError_t fm_launch(cp4d_ctx *c, const float *f, float *P, FmArgs a) {
 
 bool forward_mma_supported(const Dims &d) {
     return (d.m == 4 || d.m == 8 || d.m == 16 || d.m == 32);
+}
+
+// CP4D_PROJ_AUTO: the tensor kernel runs one 512-thread CTA per SM and pays a tile staging and a work-item build per CTA, so it
+// only wins once (tile, pass, batch group) CTAs fill the GPU; below that the fp32 gather is faster (config 2: 85 vs 74 us)
+bool forward_mma_preferred(const Dims &d) {
+    if (!forward_mma_supported(d)) return false;
+    const int blocks_total = (d.nz * d.m + 15) / 16, nb = d.m == 32 ? 2 : std::min(3, blocks_total);
+    const int64_t ctas = (int64_t)d.tiles * 2 * ((blocks_total + nb - 1) / nb);
+    return ctas >= 148;
 }
 
 cudaError_t forward_mma_init() {

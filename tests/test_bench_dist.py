@@ -56,13 +56,13 @@ def test_json_line_contract_offline():
     from paper_1809_09725_b200 import synth
 
     class A:
-        steps, warmup, frames = 50, 5, 0
+        steps, warmup, frames, projectors = 50, 5, 0, "auto"
     c = synth.CONFIGS[3]
     prof = {k: (ms * 50, 50) for k, ms in dict(forward=6.7, backproject=3.8, prox_f2=0.76, update=0.61, synth=0.09, fold=0.07).items()}
     r = dict(ms=600.0, launches=350, prof=prof, prof_gd={"grad": (1.38, 3), "div": (1.2, 3)}, ops={"forward_op": 6.7, "adjoint_op": 3.85},
              e2e={"value": 81.0, "unit": bench.UNIT, "h2d_bytes_per_step": 1.0, "d2h_bytes_per_step": 2.0},
              clocks={"sm_mhz": 1965.0, "sm_max_mhz": 1965.0, "reasons": []}, peaks=bench.load_peaks(), L=1.0, launches_total=1,
-             graph_replays=55)
+             graph_replays=55, fp32_alt=None, proj=("tensor", "fp32"))
     line = bench.assemble(A, c, 1, r)
     for k in ("metric", "value", "unit", "n_gpus", "steps", "warmup", "ms_per_step", "higher_is_better", "scaling", "vs_baseline",
               "dtype", "data", "config", "roofline", "e2e", "clocks", "gpu_launches"):
@@ -75,7 +75,12 @@ def test_json_line_contract_offline():
     assert rf["frac"] == pytest.approx(rf["achieved"] / rf["peak"]) and 0 < rf["frac"] < 1
     # algorithmic flops of the forward kernel: 2 flop x 2 taps x m x N^2 Nz N_theta0
     assert rf["achieved"] * 1e12 * 6.7e-3 == pytest.approx(2 * 2 * c.m * c.n ** 2 * c.nz * c.n_theta0, rel=1e-9)
-    assert rf["smem_roof"]["frac"] == pytest.approx(4 * rf["frac"] * (148 * 128 * 2 * r["peaks"]["sm_max_mhz"] * 1e6 / 1e12) / rf["peak"], rel=1e-6)
+    # tensor-core forward kernel: 12 HMMA MACs per algorithmic FMA against 950 MAC/clk/SM (profiles/r2_microbench.md)
+    assert rf["second_roof"]["frac"] == pytest.approx(rf["achieved"] / 2 * 12 / (148 * 950 * r["peaks"]["sm_max_mhz"] * 1e6 / 1e12), rel=1e-6)
+    assert line["run"]["projectors"] == {"mode": "auto", "forward": "tensor", "adjoint": "fp32"}
+    r2 = dict(r, proj=("fp32", "fp32"))
+    rf2 = bench.assemble(A, c, 1, r2)["roofline"]
+    assert rf2["second_roof"]["frac"] == pytest.approx(4 * rf2["frac"] * (148 * 128 * 2 * r["peaks"]["sm_max_mhz"] * 1e6 / 1e12) / rf2["peak"], rel=1e-6)
     hbm = line["kernels"]["prox_f2"]
     assert hbm["bound"] == "hbm" and hbm["achieved"] == pytest.approx(9 * c.V * 4 / 0.76e-3 / 1e9)
 
