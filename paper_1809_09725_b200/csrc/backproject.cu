@@ -18,6 +18,7 @@
 #include <cmath>
 
 #include "cp4d_internal.cuh"
+#include "device_helpers.cuh"
 
 namespace cp4d {
 
@@ -47,30 +48,6 @@ __device__ __forceinline__ void fma4(float4 &a, const float2 ww, const float4 &v
     const float2 hi = __ffma2_rn(ww, make_float2(v.z, v.w), make_float2(a.z, a.w));
     a = make_float4(lo.x, lo.y, hi.x, hi.y);
 }
-// ---- TMA 1D bulk copy global -> shared, completion on an mbarrier (SASS UBLKCP) ----
-__device__ __forceinline__ unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ void mbar_init(uint64_t *bar, unsigned count) {
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;\n" ::"r"(smem_u32(bar)), "r"(count) : "memory");
-}
-__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, unsigned bytes) {
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void mbar_wait(uint64_t *bar, unsigned parity) {
-    asm volatile(
-        "{\n"
-        ".reg .pred p;\n"
-        "WAIT_%=:\n"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
-        "@p bra DONE_%=;\n"
-        "bra WAIT_%=;\n"
-        "DONE_%=:\n"
-        "}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
-}
-__device__ __forceinline__ void bulk_g2s(void *dst_smem, const void *src_gmem, unsigned bytes, uint64_t *bar) {
-    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];\n" ::"r"(smem_u32(dst_smem)),
-                 "l"(src_gmem), "r"(bytes), "r"(smem_u32(bar)) : "memory");
-}
-
 template <int PAT, int V, int JQ, int NB>
 __device__ __forceinline__ void bp_voxel(float4 (&acc)[8][JQ], const float4 (&B)[NB][JQ], float phi, const float (&tdv)[8],
                                          float A1, float A2, float A3) {

@@ -30,6 +30,7 @@
 #include <cmath>
 
 #include "cp4d_internal.cuh"
+#include "device_helpers.cuh"
 
 namespace cp4d {
 
@@ -54,23 +55,6 @@ struct FmArgs {
     const int2 *pairs;         // [pass 0 pairs | pass 1 pairs]: (ia, ib), |inv(ib)| >= |inv(ia)|, ib = -1 for a single angle
     int npairs0, npairs1;
 };
-
-__device__ __forceinline__ void mma16816(float (&d)[4], const unsigned (&a)[4], unsigned b0, unsigned b1) {
-    asm volatile("mma.sync.aligned.m16n8k16.row.col.f32.bf16.bf16.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};\n"
-                 : "+f"(d[0]), "+f"(d[1]), "+f"(d[2]), "+f"(d[3])
-                 : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(b0), "r"(b1));
-}
-__device__ __forceinline__ void ldsm4t(unsigned (&a)[4], unsigned addr) {
-    asm volatile("ldmatrix.sync.aligned.m8n8.x4.trans.shared.b16 {%0,%1,%2,%3}, [%4];\n"
-                 : "=r"(a[0]), "=r"(a[1]), "=r"(a[2]), "=r"(a[3]) : "r"(addr));
-}
-// (x, y) -> bf16 pairs hi, lo with x = hi.x + lo.x + O(2^-18 x); low half = first element
-__device__ __forceinline__ void split2(float x, float y, unsigned &hi, unsigned &lo) {
-    const __nv_bfloat162 h = __floats2bfloat162_rn(x, y);
-    const __nv_bfloat162 l = __floats2bfloat162_rn(x - __low2float(h), y - __high2float(h));
-    hi = *reinterpret_cast<const unsigned *>(&h);
-    lo = *reinterpret_cast<const unsigned *>(&l);
-}
 
 // per-CTA record of one angle pair (shared memory): the per-angle tables and this tile's window geometry, plus what the
 // strip bookkeeping needs, so that a unit's setup is a handful of FMAs
