@@ -181,7 +181,7 @@ int cp4d_create(const cp4d_params *p, cp4d_ctx **out) {
         int cur = -1;
         if (cudaGetDevice(&cur) != cudaSuccess || cur != p->device) { cudaGetLastError(); return CP4D_ECUDA; }
     }
-    if (forward_init() != cudaSuccess || backproject_mma_init() != cudaSuccess) { cudaGetLastError(); return CP4D_ECUDA; }
+    if (forward_init() != cudaSuccess || backproject_mma_init() != cudaSuccess || backproject22_init() != cudaSuccess) { cudaGetLastError(); return CP4D_ECUDA; }
 
     cp4d_ctx *ctx = new (std::nothrow) cp4d_ctx();
     if (!ctx) return CP4D_ENOMEM;

@@ -146,6 +146,7 @@ cudaError_t launch_forward_mma(cp4d_ctx *c, const float *f, float *P);
 int backproject_mma_nb16(const Dims &d);
 int64_t backproject_mma_scratch_units(const Dims &d);
 cudaError_t backproject_mma_init();
+cudaError_t backproject22_init();
 cudaError_t launch_fold_split(cp4d_ctx *c, const float *g, float4 *gt);
 cudaError_t launch_backproject_mma(cp4d_ctx *c, const float4 *gt, float *f_out);
 cudaError_t launch_backproject(cp4d_ctx *c, const float4 *gt, float *f_out, int Q_override = 0);
