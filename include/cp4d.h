@@ -123,7 +123,7 @@ int cp4d_div(cp4d_ctx *ctx, const float *p_dev, float *f_dev);
  *   fp32 kernels: CUDA-core FMAs, relative error about 2e-6.
  *   CP4D_PROJ_AUTO (default): the faster kernel of each side -- tensor-core forward projector where it applies and the
  *       problem fills the GPU (at least 148 CTAs of (tile, pass, batch group); 1.27 x the fp32 gather at config 3), fp32
- *       backprojector (the tensor-core one measured 1.3 x slower).
+ *       backprojector (the tensor-core one measured 1.5 x slower).
  *   CP4D_PROJ_FP32: fp32 kernels on both sides.      CP4D_PROJ_TENSOR: tensor-core kernels on both sides where they apply.
  * cp4d_fbp always uses the fp32 backprojector.  Changing the mode drops the captured CUDA graph of cp4d_iterate and clears the
  * projector scratch (asynchronously, on the context's stream). */
