@@ -149,6 +149,7 @@ __global__ void __launch_bounds__(FM_THREADS, 1) k_forward_mma(const float *__re
     const unsigned tile_s = (unsigned)__cvta_generic_to_shared(tile);
     // ldmatrix row address of this lane: matrix = lane / 8 -> (column k0 + matrix / 2, half matrix & 1), row lane & 7
     const unsigned ld_half = (lane >> 3) & 1, ld_col = lane >> 4, ld_row = lane & 7;
+    const unsigned ld_base = tile_s + (((ld_half * TILE + ld_col) * TILE + ld_row) << 4);
     const TileGeo *geo = a.geo + (int64_t)tile_id * a.n0;
 
     const int n_chunk = (p1 - p0 + FM_MAXP - 1) / FM_MAXP, per_chunk = n_chunk ? (p1 - p0 + n_chunk - 1) / n_chunk : 0;   // even chunks
@@ -266,23 +267,37 @@ __global__ void __launch_bounds__(FM_THREADS, 1) k_forward_mma(const float *__re
             // rows of column k0 at k = 2t, 2t+1 and of column k0+1 at k = 2t+8, 2t+9: first-tap row relative to row q + 2t
             const float byb = bok ? ((float)bub - (bang ? R.delta1 : R.delta0)) * (bang ? R.inv1 : R.inv0) - (float)(2 * t) : -1e6f;
 
+            // window start per column: floor of the lowest first-tap row, clamped into the tile.  They are the same for every
+            // lane, so lane s works out the pair of step s (columns kb + 2 s, kb + 2 s + 1) once per item and the loop fetches
+            // it with one shuffle
+            const int kb = klo & ~1;
+            int qpack;
+            {
+                const float fk = (float)(kb + 2 * lane), fk1 = fk + 1.0f;
+                const int qa = min(max((int)floorf(fminf(fmaf(fk, R.step0, wl0), fmaf(fk, R.step1, wl1))), 0), TILE - 8);
+                const int qb = min(max((int)floorf(fminf(fmaf(fk1, R.step0, wl0), fmaf(fk1, R.step1, wl1))), 0), TILE - 8);
+                qpack = qa | (qb << 8);
+            }
+            const float byb1 = byb + bstep;
+
             float acc[NB16][4];
 #pragma unroll
             for (int zb = 0; zb < NB16; ++zb) acc[zb][0] = acc[zb][1] = acc[zb][2] = acc[zb][3] = 0.f;
 
-            for (int k0 = klo & ~1; k0 <= khi; k0 += 2) {
-                const float fk = (float)k0, fk1 = fk + 1.0f;
-                // window start per column: floor of the lowest first-tap row, clamped into the tile
-                const int qa = min(max((int)floorf(fminf(fmaf(fk, R.step0, wl0), fmaf(fk, R.step1, wl1))), 0), TILE - 8);
-                const int qb = min(max((int)floorf(fminf(fmaf(fk1, R.step0, wl0), fmaf(fk1, R.step1, wl1))), 0), TILE - 8);
+            float fk = (float)kb;
+            unsigned adr_k = ld_base + (unsigned)kb * (TILE * 16);
+            const int nstep = ((khi - kb) >> 1) + 1;
+            for (int st = 0; st < nstep; ++st, fk += 2.0f, adr_k += 2 * TILE * 16) {
+                const int qp = __shfl_sync(0xffffffffu, qpack, st);
+                const int qa = qp & 0xff, qb = qp >> 8;
                 // weights of my ray at rows q + 2t, q + 2t + 1 of both columns: Joseph hat max(0, 1 - |row - y|)
-                const float da = fmaf(fk, bstep, byb) - (float)qa, db = fmaf(fk1, bstep, byb) - (float)qb;   // y - (q + 2t)
+                const float da = fmaf(fk, bstep, byb) - (float)qa, db = fmaf(fk, bstep, byb1) - (float)qb;   // y - (q + 2t)
                 const float w0 = __saturatef(1.0f - fabsf(da)), w1 = __saturatef(1.0f - fabsf(da - 1.0f));
                 const float w2 = __saturatef(1.0f - fabsf(db)), w3 = __saturatef(1.0f - fabsf(db - 1.0f));
                 unsigned bh0, bl0, bh1, bl1;
                 split2(w0, w1, bh0, bl0);
                 split2(w2, w3, bh1, bl1);
-                const unsigned adr = tile_s + (((ld_half * TILE + k0 + ld_col) * TILE + (ld_col ? qb : qa) + ld_row) << 4);
+                const unsigned adr = adr_k + ((unsigned)(ld_col ? qb : qa) << 4);
 #pragma unroll
                 for (int zb = 0; zb < NB16; ++zb) {
                     unsigned ah[4], al[4];
