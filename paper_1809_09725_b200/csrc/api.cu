@@ -67,7 +67,7 @@ Carve carve(const Dims &d) {
     c.phi = take((uint64_t)d.m * d.na * 4); c.ang = take((uint64_t)d.n0 * sizeof(AngleTab));
     c.geo = take((uint64_t)d.tiles * d.n0 * sizeof(TileGeo)); c.red = take(64);
     c.fwang = take((uint64_t)d.n0 * sizeof(FwAngle)); c.fworder = take((uint64_t)d.n0 * 4);
-    c.fwpairs = take((uint64_t)d.n0 * sizeof(int2));
+    c.fwpairs = take((uint64_t)d.n0 * sizeof(int4));
     c.cf = c.cb = c.psi = 0;
     if (d.nf) { c.cf = take(d.Vc * 4); c.cb = take(d.Vc * 4); c.psi = take((uint64_t)d.mb * d.nf * 4); }
     c.total = o;
@@ -195,7 +195,7 @@ int cp4d_create(const cp4d_params *p, cp4d_ctx **out) {
     ctx->h2 = (float *)(w + cv.h2); ctx->h1 = (float *)(w + cv.h1); ctx->g = (float *)(w + cv.g);
     ctx->tmp_s = (float *)(w + cv.tmp_s);
     ctx->fwang = (FwAngle *)(w + cv.fwang); ctx->fworder = (int32_t *)(w + cv.fworder);
-    ctx->fw_pairs = (int2 *)(w + cv.fwpairs); ctx->fw_mode = CP4D_PROJ_AUTO;
+    ctx->fw_groups = (int4 *)(w + cv.fwpairs); ctx->fw_mode = CP4D_PROJ_AUTO;
     ctx->cf = d.nf ? (float *)(w + cv.cf) : nullptr; ctx->cb = d.nf ? (float *)(w + cv.cb) : nullptr;
     ctx->psi = d.nf ? (float *)(w + cv.psi) : nullptr;
     ctx->scratch = (float4 *)(w + cv.scratch); ctx->psum = (float4 *)(w + cv.psum); ctx->phi = (float *)(w + cv.phi);
@@ -233,8 +233,8 @@ int cp4d_create(const cp4d_params *p, cp4d_ctx **out) {
     }
     for (int i = 0; i < d.n0; ++i) fwang[i] = FwAngle{ang[i].fw_inv, ang[i].fw_step, ang[i].fw_istep, ang[i].inv_a};
     ctx->fwtab_host = fwtable_new(fwang.data(), fworder.data(), d.n0);
-    std::vector<int2> fwpairs(d.n0);
-    forward_mma_pairs(fwang.data(), fworder.data(), d.n0, ctx->n_colstep, fwpairs.data(), &ctx->n_pairs0, &ctx->n_pairs1);
+    std::vector<int4> fwpairs(d.n0);
+    forward_mma_groups(fwang.data(), fworder.data(), d.n0, ctx->n_colstep, fwpairs.data(), &ctx->n_groups0, &ctx->n_groups1);
     std::vector<TileGeo> geo((size_t)d.tiles * d.n0);
     const double cen = 0.5 * (d.n - 1), cd = 0.5 * (d.nd - 1);
     for (int t = 0; t < d.tiles; ++t) {
@@ -272,7 +272,7 @@ int cp4d_create(const cp4d_params *p, cp4d_ctx **out) {
         (e = cudaMemcpyAsync(ctx->ang, ang.data(), ang.size() * sizeof(AngleTab), cudaMemcpyHostToDevice, ctx->stream)) != cudaSuccess ||
         (e = cudaMemcpyAsync(ctx->fwang, fwang.data(), fwang.size() * sizeof(FwAngle), cudaMemcpyHostToDevice, ctx->stream)) != cudaSuccess ||
         (e = cudaMemcpyAsync(ctx->fworder, fworder.data(), fworder.size() * 4, cudaMemcpyHostToDevice, ctx->stream)) != cudaSuccess ||
-        (e = cudaMemcpyAsync(ctx->fw_pairs, fwpairs.data(), fwpairs.size() * sizeof(int2), cudaMemcpyHostToDevice, ctx->stream)) != cudaSuccess ||
+        (e = cudaMemcpyAsync(ctx->fw_groups, fwpairs.data(), fwpairs.size() * sizeof(int4), cudaMemcpyHostToDevice, ctx->stream)) != cudaSuccess ||
         (e = cudaMemcpyAsync(ctx->geo, geo.data(), geo.size() * sizeof(TileGeo), cudaMemcpyHostToDevice, ctx->stream)) != cudaSuccess ||
         (e = cudaMemsetAsync(ctx->scratch, 0, (size_t)d.scratch4 * 16, ctx->stream)) != cudaSuccess ||
         (e = cudaStreamSynchronize(ctx->stream)) != cudaSuccess) {

@@ -81,8 +81,8 @@ struct cp4d_ctx {
     uint64_t iter_graph_launches, graph_replays;
     bool iter_graph_off;
     cp4d::FwTable *fwtab_host; // host copy of fwang / fworder for the kernel-parameter path (n0 <= 512), else null
-    int2 *fw_pairs;            // tensor-core forward projector (forward_mma.cu): base angles of each pass paired with a neighbour
-    int n_pairs0, n_pairs1;
+    int4 *fw_groups;           // tensor-core forward projector (forward_mma.cu): base angles of each pass in groups of up to four neighbours
+    int n_groups0, n_groups1;
     int fw_mode;               // CP4D_PROJ_AUTO / _FP32 (cp4d_set_projector_mode): both projectors
     int n_cpos;                // the first n_cpos base angles have cos >= 0 (backprojector: chunks never mix the signs)
     cp4d::TileGeo *geo;        // [tile][n0]
@@ -140,7 +140,7 @@ cudaError_t forward_init();        // once per process and device: opt in to the
 bool forward_mma_supported(const Dims &d);
 bool forward_mma_preferred(const Dims &d);     // what CP4D_PROJ_AUTO picks
 cudaError_t forward_mma_init();
-int forward_mma_pairs(const FwAngle *fw, const int32_t *order, int n0, int n_colstep, int2 *out, int *npairs0, int *npairs1);
+int forward_mma_groups(const FwAngle *fw, const int32_t *order, int n0, int n_colstep, int4 *out, int *ngroups0, int *ngroups1);
 cudaError_t launch_forward_mma(cp4d_ctx *c, const float *f, float *P);
 // backproject_mma.cu: the tensor-core adjoint (fold into split-bf16 rows + backprojection); same shapes as forward_mma
 int backproject_mma_nb16(const Dims &d);

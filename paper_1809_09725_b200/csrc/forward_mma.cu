@@ -49,25 +49,26 @@ struct FmArgs {
     int n, nz, nd, n0, m, mshift, gp, gpl;
     int tiles, agroups;
     int zper;                  // slices per CTA = NB16 * 16 / m
-    float margin;              // bins a ray of the second angle of a pair can sit from the first angle's bin of its touch point
+    float margin;              // bins a ray of another angle of a group can sit from the first angle's bin of its touch point
     const TileGeo *geo;
     const FwAngle *fwang;
-    const int2 *pairs;         // [pass 0 pairs | pass 1 pairs]: (ia, ib), |inv(ib)| >= |inv(ia)|, ib = -1 for a single angle
-    int npairs0, npairs1;
+    const int4 *groups;        // [pass 0 groups | pass 1 groups]: up to four adjacent base angles, the one with the smallest |1/ss|
+                               // first, -1 for an absent one
+    int ngroups0, ngroups1;
 };
 
-// per-CTA record of one angle pair (shared memory): the per-angle tables and this tile's window geometry, plus what the
-// strip bookkeeping needs, so that a unit's setup is a handful of FMAs
-struct FmPair {
-    float inv0, step0, delta0, inva0;     // angle 0 (the one with the smaller |1/ss|): 1/ss, -cc/ss, window offset, 1/a
-    float inv1, step1, delta1, inva1;     // angle 1 (= angle 0 for a single)
-    float r0, rinv1, istep0, istep1;      // angle-1 bin ub1 sits at angle-0 bin coordinate (ub1 - s0) / rinv1, s0 = -r0 rinv1, at the
-                                          // reference column; istep = 1/step (0 when the rays run along the columns)
-    int ia, ib, bstart0, bstart1;
+// per-CTA record of one angle group (shared memory): the per-angle tables and this tile's window geometry, plus what the
+// strip bookkeeping needs, so that an item's setup is a handful of FMAs.  Absent angles repeat angle 0 with ia = -1.
+struct FmGroup {
+    float inv[4], step[4], delta[4], inva[4];   // 1/ss, -cc/ss, window offset of the tile, 1/a
+    float istep[4];                             // 1/step (0 when the rays run along the columns)
+    float r0[4], rinv[4];                       // bin ub of angle x sits, at the reference column, at angle-0 bin coordinate
+                                                // ub / rinv[x] + r0[x]
+    int ia[4], bstart[4];
 };
-constexpr int FM_MAXP = 64;
-constexpr int FM_MAXITEMS = 2 * FM_MAXP * FM_STRIPS;   // every (pair, strip) may fall apart into two items
-constexpr int FM_LONG = 14;                           // columns from which an item counts as long               // pairs per chunk of a CTA's pair list
+constexpr int FM_MAXG = 24;                            // groups per chunk of a CTA's group list
+constexpr int FM_MAXITEMS = 4 * FM_MAXG * FM_STRIPS;   // every (group, strip) may fall apart into four single-angle items
+constexpr int FM_LONG = 14;                            // columns from which an item counts as long
 
 // columns k in [0, TILE) where a ray group whose first-tap rows lie in [ylo + k st, yhi + k st] touches rows 0 .. TILE-1:
 // ylo + k st < TILE and yhi + k st > -1
@@ -84,27 +85,22 @@ __device__ __forceinline__ void col_range(float ylo, float yhi, float st, float 
     }
 }
 
-// one work item of a CTA: (angle pair, strip, which of the two angles) with its trimmed column range, built once per CTA by
-// all threads in parallel so that a warp's per-item setup is a decode and a few FMAs
-struct FmItem {
-    unsigned short pair_strip;     // (pair << 4) | (strip + 1)
-    unsigned char klo, khi;        // columns of the tile the strip's rays touch
-    signed char b1s;               // first window bin of the second angle's group in this strip
-    unsigned char cnt1;            // bins of that group
-    unsigned char mode;            // 0: both angles in one window (slots 0-3 / 4-7), 1: first angle only, 2: second angle only
-    unsigned char pad;
-};
-static_assert(sizeof(FmItem) == 8, "FmItem is one 8-byte shared-memory word");
+// One work item of a CTA, three shared-memory words built once per CTA by all threads in parallel:
+//   w0 = (group << 4 | strip + 1) | klo << 16 | khi << 24            columns of the tile the item's rays touch
+//   w1 = bs1 | bs2 << 8 | bs3 << 16 (signed bytes) | used << 24       first window bin of angles 1-3 in this strip; angles in use
+//   w2 = 4 | cnt1 << 4 | cnt2 << 8 | cnt3 << 12 | hb << 16            bins per angle; hb = four nibbles, one per half block of
+//                                                                     four ray slots: angle | 4 (bins 4-7 of a long single) | 8 (valid)
+// Half blocks 0, 1 are the 8 rays of the first MMA column block, 2, 3 those of the second (only items of 3 or 4 angles).
 
 template <int NB16>
 __global__ void __launch_bounds__(FM_THREADS, 1) k_forward_mma(const float *__restrict__ f, float *__restrict__ P, FmArgs a) {
     extern __shared__ __align__(128) unsigned char tile[];     // [NB16][2][2][TILE][TILE] x 16 B
     __shared__ int s_next, s_nlong, s_nshort, s_ncand;
     __shared__ __align__(16) float s_stg[FM_WARPS][8 * FM_STG];
-    __shared__ __align__(16) FmPair s_pair[FM_MAXP];
-    __shared__ unsigned char s_t0[FM_MAXP], s_tn[FM_MAXP];      // first strip (+1) and number of strips of each pair
-    __shared__ unsigned short s_cand[FM_MAXP * FM_STRIPS];      // candidate -> (pair << 4) | (strip + 1)
-    __shared__ __align__(8) FmItem s_item[FM_MAXITEMS];
+    __shared__ __align__(16) FmGroup s_grp[FM_MAXG];
+    __shared__ unsigned char s_t0[FM_MAXG], s_tn[FM_MAXG];      // first strip (+1) and number of strips of each group
+    __shared__ unsigned short s_cand[FM_MAXG * FM_STRIPS];      // candidate -> (group << 4) | (strip + 1)
+    __shared__ unsigned s_item[3 * FM_MAXITEMS];
     float *stg = s_stg[threadIdx.x >> 5];
     const int tiles_1d = (a.n + TILE - 1) / TILE;
     const int tile_id = blockIdx.x % a.tiles, ag = blockIdx.x / a.tiles;
@@ -142,8 +138,8 @@ __global__ void __launch_bounds__(FM_THREADS, 1) k_forward_mma(const float *__re
         }
     }
 
-    // ---- this CTA's share of the pass's angle pairs, in chunks of FM_MAXP ----
-    const int pbeg = pass ? a.npairs0 : 0, pcnt = pass ? a.npairs1 : a.npairs0;
+    // ---- this CTA's share of the pass's angle groups, in chunks of FM_MAXG ----
+    const int pbeg = pass ? a.ngroups0 : 0, pcnt = pass ? a.ngroups1 : a.ngroups0;
     const int p0 = pbeg + (int)((int64_t)pcnt * ag / a.agroups), p1 = pbeg + (int)((int64_t)pcnt * (ag + 1) / a.agroups);
     const int lane = threadIdx.x & 31, g = lane >> 2, t = lane & 3;
     const unsigned tile_s = (unsigned)__cvta_generic_to_shared(tile);
@@ -152,27 +148,30 @@ __global__ void __launch_bounds__(FM_THREADS, 1) k_forward_mma(const float *__re
     const unsigned ld_base = tile_s + (((ld_half * TILE + ld_col) * TILE + ld_row) << 4);
     const TileGeo *geo = a.geo + (int64_t)tile_id * a.n0;
 
-    const int n_chunk = (p1 - p0 + FM_MAXP - 1) / FM_MAXP, per_chunk = n_chunk ? (p1 - p0 + n_chunk - 1) / n_chunk : 0;   // even chunks
+    const int n_chunk = (p1 - p0 + FM_MAXG - 1) / FM_MAXG, per_chunk = n_chunk ? (p1 - p0 + n_chunk - 1) / n_chunk : 0;   // even chunks
     for (int pc = p0; pc < p1; pc += per_chunk) {
         const int npc = min(per_chunk, p1 - pc);
         __syncthreads();                                     // the tile is staged / every warp is done with the previous chunk
         if ((int)threadIdx.x < npc) {
-            const int2 pr = a.pairs[pc + threadIdx.x];
-            const FwAngle A0 = a.fwang[pr.x], A1 = a.fwang[pr.y >= 0 ? pr.y : pr.x];
-            const TileGeo G0 = geo[pr.x], G1 = geo[pr.y >= 0 ? pr.y : pr.x];
-            FmPair R;
-            R.inv0 = A0.inv; R.step0 = A0.step; R.delta0 = G0.delta; R.inva0 = A0.inv_a;
-            R.inv1 = A1.inv; R.step1 = A1.step; R.delta1 = G1.delta; R.inva1 = A1.inv_a;
-            // angle-1 ray ub1 sits, at the reference column, at angle-0 bin coordinate phi = r1 ub1 + r0
-            const float r1 = A1.inv / A0.inv;
-            R.r0 = (FM_KC * (A1.step - A0.step) - G1.delta * A1.inv) / A0.inv + G0.delta;
-            R.rinv1 = 1.0f / r1;
-            R.istep0 = fabsf(A0.step) > 1e-6f ? 1.0f / A0.step : 0.0f;
-            R.istep1 = fabsf(A1.step) > 1e-6f ? 1.0f / A1.step : 0.0f;
-            R.ia = pr.x; R.ib = pr.y; R.bstart0 = G0.bstart; R.bstart1 = G1.bstart;
-            s_pair[threadIdx.x] = R;
+            const int4 gr = a.groups[pc + threadIdx.x];
+            const int idx[4] = {gr.x, gr.y, gr.z, gr.w};
+            const FwAngle A0 = a.fwang[gr.x];
+            const TileGeo G0 = geo[gr.x];
+            FmGroup &R = s_grp[threadIdx.x];
+#pragma unroll
+            for (int x = 0; x < 4; ++x) {
+                const int i = idx[x] >= 0 ? idx[x] : gr.x;
+                const FwAngle A = a.fwang[i];
+                const TileGeo G = geo[i];
+                R.inv[x] = A.inv; R.step[x] = A.step; R.delta[x] = G.delta; R.inva[x] = A.inv_a;
+                R.istep[x] = fabsf(A.step) > 1e-6f ? 1.0f / A.step : 0.0f;
+                // ray ub of angle x sits, at the reference column, at angle-0 bin coordinate phi = ub inv_x / inv_0 + r0
+                R.r0[x] = (FM_KC * (A.step - A0.step) - G.delta * A.inv) / A0.inv + G0.delta;
+                R.rinv[x] = A0.inv / A.inv;
+                R.ia[x] = idx[x]; R.bstart[x] = G.bstart;
+            }
             // strips that can hold a ray touching the tile: angle-0 window coordinates of the tile corners, widened by the
-            // distance an angle-1 ray can sit from the bin of its touch point at the reference column (a.margin)
+            // distance a ray of another angle can sit from the bin of its touch point at the reference column (a.margin)
             const float ss = 1.0f / A0.inv, cc = -A0.step * ss, e = (float)(TILE - 1);
             const float umin = G0.delta + fminf(0.f, e * cc) + fminf(0.f, e * ss), umax = G0.delta + fmaxf(0.f, e * cc) + fmaxf(0.f, e * ss);
             const int tf = max(-1, (int)floorf((umin - a.margin + 0.5f) * 0.25f)), tl = min(FM_STRIPS - 2, (int)floorf((umax + a.margin + 0.5f) * 0.25f));
@@ -180,7 +179,7 @@ __global__ void __launch_bounds__(FM_THREADS, 1) k_forward_mma(const float *__re
             s_tn[threadIdx.x] = (unsigned char)max(0, tl - tf + 1);
         }
         __syncthreads();
-        if (threadIdx.x < 32) {                              // candidate table: pairs in order, their strips in order
+        if (threadIdx.x < 32) {                              // candidate table: groups in order, their strips in order
             int base = 0;
             for (int q0 = 0; q0 < npc; q0 += 32) {
                 const int q = q0 + lane, n = q < npc ? s_tn[q] : 0;
@@ -196,49 +195,94 @@ __global__ void __launch_bounds__(FM_THREADS, 1) k_forward_mma(const float *__re
             if (lane == 0) { s_ncand = base; s_nlong = 0; s_nshort = 0; s_next = 0; }
         }
         __syncthreads();
-        // ---- work items: every candidate (pair, strip) is examined by one thread: the second angle's group of bins, the columns
-        // the rays touch, and whether one 8-row window per column holds both angles (else one item per angle) ----
+        // ---- work items: every candidate (group, strip) is examined by one thread: each angle's group of bins in the strip,
+        // the columns its rays touch, and whether one 8-row window per column holds all angles (one item: 8 rays per MMA for two
+        // angles, 16 for three or four), else the first two and the remaining angles are tried as pairs, else one item per angle ----
         for (int cnd = threadIdx.x; cnd < s_ncand; cnd += FM_THREADS) {
             const unsigned uu = s_cand[cnd];
-            const FmPair R = s_pair[uu >> 4];
+            const FmGroup &R = s_grp[uu >> 4];
             const int ts = (int)(uu & 15) - 1;
             const float ft4 = 4.0f * (float)ts;
-            int b1s = 0, cnt1 = 0;
-            if (R.ib >= 0) {
-                // angle-1 bin ub1 belongs to the strip whose extent [4 ts - 0.5, 4 ts + 3.5) holds phi(ub1): the extents tile the
-                // line and both ends use the same expression, so every bin is in exactly one strip
-                b1s = (int)ceilf((ft4 - 0.5f - R.r0) * R.rinv1);
-                cnt1 = (int)ceilf((ft4 + 3.5f - R.r0) * R.rinv1) - b1s;
+            int bs[4], cnt[4], ka[4], kb[4];
+            float lo[4], hi[4], stp[4];
+            unsigned ex = 0;                                   // angles with a ray that touches the tile in this strip
+#pragma unroll
+            for (int x = 0; x < 4; ++x) {
+                bs[x] = 4 * ts; cnt[x] = 4;
+                if (x > 0) {
+                    // bin ub of angle x belongs to the strip whose extent [4 ts - 0.5, 4 ts + 3.5) holds phi(ub): the extents tile the
+                    // line and both ends use the same expression, so every bin is in exactly one strip
+                    const float r0 = R.r0[x], ri = R.rinv[x];
+                    bs[x] = (int)ceilf((ft4 - 0.5f - r0) * ri);
+                    cnt[x] = R.ia[x] >= 0 ? (int)ceilf((ft4 + 3.5f - r0) * ri) - bs[x] : 0;
+                }
+                // first-tap row of window bin ub of angle x at column k:  (ub - delta) inv + k step
+                const float inv = R.inv[x], y0 = ((float)bs[x] - R.delta[x]) * inv, y1 = fmaf((float)(max(cnt[x], 1) - 1), inv, y0);
+                lo[x] = fminf(y0, y1); hi[x] = fmaxf(y0, y1); stp[x] = R.step[x];
+                ka[x] = TILE; kb[x] = -1;
+                if (cnt[x] > 0 && bs[x] + cnt[x] > 0 && bs[x] < WIN) col_range(lo[x], hi[x], stp[x], R.istep[x], ka[x], kb[x]);
+                if (ka[x] <= kb[x]) ex |= 1u << x;
+                bs[x] = max(-100, min(100, bs[x])); cnt[x] = min(cnt[x], 8);
             }
-            // first-tap row of window bin ub of angle x at column k:  (ub - delta) inv + k step
-            const float y00 = (ft4 - R.delta0) * R.inv0, y03 = fmaf(3.0f, R.inv0, y00);
-            const float y10 = ((float)b1s - R.delta1) * R.inv1, y11 = fmaf((float)(max(cnt1, 1) - 1), R.inv1, y10);
-            const float lo0 = fminf(y00, y03), hi0 = fmaxf(y00, y03), lo1 = fminf(y10, y11), hi1 = fmaxf(y10, y11);
-            int ka0, kb0, ka1 = TILE, kb1 = -1;
-            col_range(lo0, hi0, R.step0, R.istep0, ka0, kb0);
-            if (4 * ts + 3 < 0 || 4 * ts >= WIN) { ka0 = TILE; kb0 = -1; }          // no bin of the first angle's window in this strip
-            if (cnt1 > 0 && b1s + cnt1 > 0 && b1s < WIN) col_range(lo1, hi1, R.step1, R.istep1, ka1, kb1);
-            // one window for both angles?  The spread of first-tap rows is convex in k: check the two end columns
-            bool pair_ok = cnt1 > 0 && cnt1 <= 4 && ka0 <= kb0 && ka1 <= kb1;
-            if (pair_ok) {
-                const float fa = (float)min(ka0, ka1), fb = (float)max(kb0, kb1);
-                const float sa = fmaxf(fmaf(fa, R.step0, hi0), fmaf(fa, R.step1, hi1)) - fminf(fmaf(fa, R.step0, lo0), fmaf(fa, R.step1, lo1));
-                const float sb = fmaxf(fmaf(fb, R.step0, hi0), fmaf(fb, R.step1, hi1)) - fminf(fmaf(fb, R.step0, lo0), fmaf(fb, R.step1, lo1));
-                pair_ok = sa < FM_SPAN && sb < FM_SPAN;
-            }
-            // long items are handed out first (front of the list), short ones last (stored from the back): an even finish
-            auto push = [&](const FmItem &x) {
-                const bool lng = (int)x.khi - (int)x.klo >= FM_LONG;
-                s_item[lng ? atomicAdd(&s_nlong, 1) : FM_MAXITEMS - 1 - atomicAdd(&s_nshort, 1)] = x;
+            // columns of a set of angles and whether one window per column holds them: the spread of first-tap rows is convex
+            // in k, so the two end columns decide
+            auto cols = [&](unsigned S, int &fa, int &fb) {
+                fa = TILE; fb = -1;
+#pragma unroll
+                for (int x = 0; x < 4; ++x)
+                    if (S >> x & 1) { fa = min(fa, ka[x]); fb = max(fb, kb[x]); }
             };
-            FmItem it;
-            it.pair_strip = (unsigned short)uu; it.b1s = (signed char)max(-100, min(100, b1s)); it.cnt1 = (unsigned char)min(cnt1, 8); it.pad = 0;
-            if (pair_ok) {
-                it.mode = 0; it.klo = (unsigned char)min(ka0, ka1); it.khi = (unsigned char)max(kb0, kb1);
-                push(it);
+            auto fits = [&](unsigned S) {
+                int ia_, ib_;
+                cols(S, ia_, ib_);
+                const float fa = (float)ia_, fb = (float)ib_;
+                float ha = -1e30f, la = 1e30f, hb_ = -1e30f, lb = 1e30f;
+                bool ok = true;
+#pragma unroll
+                for (int x = 0; x < 4; ++x)
+                    if (S >> x & 1) {
+                        ok = ok && cnt[x] <= 4;
+                        ha = fmaxf(ha, fmaf(fa, stp[x], hi[x])); la = fminf(la, fmaf(fa, stp[x], lo[x]));
+                        hb_ = fmaxf(hb_, fmaf(fb, stp[x], hi[x])); lb = fminf(lb, fmaf(fb, stp[x], lo[x]));
+                    }
+                return ok && ha - la < FM_SPAN && hb_ - lb < FM_SPAN;
+            };
+            // long items are handed out first (front of the list), short ones last (stored from the back): an even finish
+            auto push = [&](unsigned S, unsigned hb) {
+                int fa, fb;
+                cols(S, fa, fb);
+                const bool lng = fb - fa >= FM_LONG;
+                const int at = lng ? atomicAdd(&s_nlong, 1) : FM_MAXITEMS - 1 - atomicAdd(&s_nshort, 1);
+                s_item[3 * at] = uu | ((unsigned)fa << 16) | ((unsigned)fb << 24);
+                s_item[3 * at + 1] = ((unsigned)bs[1] & 0xffu) | (((unsigned)bs[2] & 0xffu) << 8) | (((unsigned)bs[3] & 0xffu) << 16) | (S << 24);
+                s_item[3 * at + 2] = 4u | ((unsigned)cnt[1] << 4) | ((unsigned)cnt[2] << 8) | ((unsigned)cnt[3] << 12) | (hb << 16);
+            };
+            auto nibbles = [&](unsigned S) {                   // the angles of S on consecutive half blocks
+                unsigned hb = 0;
+                int h = 0;
+#pragma unroll
+                for (int x = 0; x < 4; ++x)
+                    if (S >> x & 1) { hb |= (8u | (unsigned)x) << (4 * h); ++h; }
+                return hb;
+            };
+            auto singles = [&](unsigned S) {
+#pragma unroll
+                for (int x = 0; x < 4; ++x)
+                    if (S >> x & 1) push(1u << x, (8u | (unsigned)x) | (cnt[x] > 4 ? (12u | (unsigned)x) << 4 : 0u));
+            };
+            auto pair_or_singles = [&](unsigned S) {
+                if (__popc(S) == 2 && fits(S)) push(S, nibbles(S));
+                else singles(S);
+            };
+            const int nex = __popc(ex);
+            if (nex >= 2 && fits(ex)) {
+                push(ex, nibbles(ex));
+            } else if (nex >= 3) {
+                const unsigned first = ex & (0u - ex), rest = ex ^ first, second = rest & (0u - rest);
+                pair_or_singles(first | second);
+                pair_or_singles(ex ^ (first | second));
             } else {
-                if (ka0 <= kb0) { it.mode = 1; it.klo = (unsigned char)ka0; it.khi = (unsigned char)kb0; push(it); }
-                if (ka1 <= kb1) { it.mode = 2; it.klo = (unsigned char)ka1; it.khi = (unsigned char)kb1; push(it); }
+                singles(ex);
             }
         }
         __syncthreads();
@@ -249,24 +293,21 @@ __global__ void __launch_bounds__(FM_THREADS, 1) k_forward_mma(const float *__re
             if (lane == 0) u = atomicAdd(&s_next, 1);
             u = __shfl_sync(0xffffffffu, u, 0);
             if (u >= n_items) break;
-            const FmItem it = s_item[u < n_long ? u : FM_MAXITEMS - 1 - (u - n_long)];
-            const FmPair R = s_pair[it.pair_strip >> 4];
-            const int ts = (int)(it.pair_strip & 15) - 1, klo = it.klo, khi = it.khi, b1s = it.b1s, cnt1 = it.cnt1;
-            // slot n of the 8 rays -> (angle, window bin).  mode 0: 0-3 first angle, 4-7 second; else one angle, slots from 0
-            const bool use0 = it.mode != 2, use1 = it.mode != 1;
-            const int off1 = it.mode == 0 ? 4 : 0;               // first slot of the second angle
+            const int at = u < n_long ? u : FM_MAXITEMS - 1 - (u - n_long);
+            const unsigned w0 = s_item[3 * at], w1 = s_item[3 * at + 1], w2 = s_item[3 * at + 2];
+            const FmGroup &R = s_grp[(w0 & 0xffffu) >> 4];
+            const int ts = (int)(w0 & 15u) - 1, klo = (int)((w0 >> 16) & 0xffu), khi = (int)(w0 >> 24);
+            const unsigned bspack = (w1 << 8) | ((unsigned)(4 * ts) & 0xffu);      // first bin of angle x: signed byte x
+            const unsigned used = w1 >> 24, hb = w2 >> 16;
             // lowest first-tap row of each angle in use at column 0: the window lines
-            const float y00 = (4.0f * (float)ts - R.delta0) * R.inv0, y10 = ((float)b1s - R.delta1) * R.inv1;
-            const float wl0 = use0 ? fminf(y00, fmaf(3.0f, R.inv0, y00)) : 1e6f;
-            const float wl1 = use1 ? fminf(y10, fmaf((float)(max(cnt1, 1) - 1), R.inv1, y10)) : 1e6f;
-            // my ray (slot g): B column g of the weight block, and the ray whose sums I add to P in the end
-            const int bang = (use1 && !(use0 && g < 4)) ? 1 : 0;
-            const int bub = bang ? b1s + g - off1 : 4 * ts + g;
-            const bool bok = (bang ? (g >= off1 && g - off1 < cnt1) : (use0 && g < 4)) && bub >= 0 && bub < WIN;
-            const float bstep = bang ? R.step1 : R.step0;
-            // rows of column k0 at k = 2t, 2t+1 and of column k0+1 at k = 2t+8, 2t+9: first-tap row relative to row q + 2t
-            const float byb = bok ? ((float)bub - (bang ? R.delta1 : R.delta0)) * (bang ? R.inv1 : R.inv0) - (float)(2 * t) : -1e6f;
-
+            float wl[4], wst[4];
+#pragma unroll
+            for (int x = 0; x < 4; ++x) {
+                const int bsx = (int)(bspack << (24 - 8 * x)) >> 24, cx = (int)((w2 >> (4 * x)) & 15u);
+                const float inv = R.inv[x], y0 = ((float)bsx - R.delta[x]) * inv;
+                wl[x] = (used >> x & 1u) ? fminf(y0, fmaf((float)(max(cx, 1) - 1), inv, y0)) : 1e6f;
+                wst[x] = R.step[x];
+            }
             // window start per column: floor of the lowest first-tap row, clamped into the tile.  They are the same for every
             // lane, so lane s works out the pair of step s (columns kb + 2 s, kb + 2 s + 1) once per item and the loop fetches
             // it with one shuffle
@@ -274,60 +315,117 @@ __global__ void __launch_bounds__(FM_THREADS, 1) k_forward_mma(const float *__re
             int qpack;
             {
                 const float fk = (float)(kb + 2 * lane), fk1 = fk + 1.0f;
-                const int qa = min(max((int)floorf(fminf(fmaf(fk, R.step0, wl0), fmaf(fk, R.step1, wl1))), 0), TILE - 8);
-                const int qb = min(max((int)floorf(fminf(fmaf(fk1, R.step0, wl0), fmaf(fk1, R.step1, wl1))), 0), TILE - 8);
-                qpack = qa | (qb << 8);
+                const float la = fminf(fminf(fmaf(fk, wst[0], wl[0]), fmaf(fk, wst[1], wl[1])), fminf(fmaf(fk, wst[2], wl[2]), fmaf(fk, wst[3], wl[3])));
+                const float lb = fminf(fminf(fmaf(fk1, wst[0], wl[0]), fmaf(fk1, wst[1], wl[1])), fminf(fmaf(fk1, wst[2], wl[2]), fmaf(fk1, wst[3], wl[3])));
+                qpack = min(max((int)floorf(la), 0), TILE - 8) | (min(max((int)floorf(lb), 0), TILE - 8) << 8);
             }
-            const float byb1 = byb + bstep;
-
-            float acc[NB16][4];
+            // my ray of column block nb (ray slot g): B column g of the weight block, and the ray whose sums I add to P in the
+            // end.  Half block 2 nb + g / 4 names the angle; its slots hold consecutive bins
+            int r_ang[2], r_bub[2];
+            bool r_ok[2];
+            float r_step[2], r_y[2];       // first-tap row at column 0, relative to row 2t (the rows of my B entries: 2t, 2t+1)
 #pragma unroll
-            for (int zb = 0; zb < NB16; ++zb) acc[zb][0] = acc[zb][1] = acc[zb][2] = acc[zb][3] = 0.f;
-
-            float fk = (float)kb;
-            unsigned adr_k = ld_base + (unsigned)kb * (TILE * 16);
+            for (int nb = 0; nb < 2; ++nb) {
+                const unsigned d = (hb >> (4 * (2 * nb + (g >> 2)))) & 15u;
+                const int x = (int)(d & 3u), off = (int)(d & 4u) + (g & 3);
+                const int bsx = (int)(bspack << (24 - 8 * x)) >> 24, cx = (int)((w2 >> (4 * x)) & 15u);
+                r_ang[nb] = x;
+                r_bub[nb] = bsx + off;
+                r_ok[nb] = (d & 8u) && off < cx && r_bub[nb] >= 0 && r_bub[nb] < WIN;
+                r_step[nb] = R.step[x];
+                r_y[nb] = r_ok[nb] ? ((float)r_bub[nb] - R.delta[x]) * R.inv[x] - (float)(2 * t) : -1e6f;
+            }
             const int nstep = ((khi - kb) >> 1) + 1;
-            for (int st = 0; st < nstep; ++st, fk += 2.0f, adr_k += 2 * TILE * 16) {
-                const int qp = __shfl_sync(0xffffffffu, qpack, st);
-                const int qa = qp & 0xff, qb = qp >> 8;
-                // weights of my ray at rows q + 2t, q + 2t + 1 of both columns: Joseph hat max(0, 1 - |row - y|)
-                const float da = fmaf(fk, bstep, byb) - (float)qa, db = fmaf(fk, bstep, byb1) - (float)qb;   // y - (q + 2t)
-                const float w0 = __saturatef(1.0f - fabsf(da)), w1 = __saturatef(1.0f - fabsf(da - 1.0f));
-                const float w2 = __saturatef(1.0f - fabsf(db)), w3 = __saturatef(1.0f - fabsf(db - 1.0f));
-                unsigned bh0, bl0, bh1, bl1;
-                split2(w0, w1, bh0, bl0);
-                split2(w2, w3, bh1, bl1);
-                const unsigned adr = adr_k + ((unsigned)(ld_col ? qb : qa) << 4);
-#pragma unroll
-                for (int zb = 0; zb < NB16; ++zb) {
-                    unsigned ah[4], al[4];
-                    ldsm4t(ah, adr + zb * 2 * FM_PLANE);
-                    ldsm4t(al, adr + zb * 2 * FM_PLANE + FM_PLANE);
-                    mma16816(acc[zb], ah, bh0, bh1);
-                    mma16816(acc[zb], al, bh0, bh1);
-                    mma16816(acc[zb], ah, bl0, bl1);
-                }
-            }
+
             // ---- partial ray sums of this tile -> P[z][i][b][j].  My D entries are rays 2t, 2t+1 x batch entries g, g+8; a RED
-            // costs about one clock per LANE whatever its width, so the block goes through a per-warp shared-memory patch and
+            // costs about one clock per LANE whatever its width, so a block goes through a per-warp shared-memory patch and
             // leaves as one 16-byte RED per lane: lane (ray g, quad t) adds entries 4t .. 4t+3 of ray g ----
-            const int i = bang ? R.ib : R.ia;
-            const int b = (bang ? R.bstart1 : R.bstart0) + bub;
-            const bool red_ok = bok && b >= 0 && b < a.nd;
-            const float sc = bang ? R.inva1 : R.inva0;
-#pragma unroll
-            for (int zb = 0; zb < NB16; ++zb) {
+            auto flush = [&](const float (&acc)[4], int zb, int nb) {
+                const int x = r_ang[nb];
+                const int i = R.ia[x], b = R.bstart[x] + r_bub[nb];
+                const float sc = R.inva[x];
                 __syncwarp();
-                stg[(2 * t) * FM_STG + g] = acc[zb][0];
-                stg[(2 * t + 1) * FM_STG + g] = acc[zb][1];
-                stg[(2 * t) * FM_STG + g + 8] = acc[zb][2];
-                stg[(2 * t + 1) * FM_STG + g + 8] = acc[zb][3];
+                stg[(2 * t) * FM_STG + g] = acc[0];
+                stg[(2 * t + 1) * FM_STG + g] = acc[1];
+                stg[(2 * t) * FM_STG + g + 8] = acc[2];
+                stg[(2 * t + 1) * FM_STG + g + 8] = acc[3];
                 __syncwarp();
                 const float4 v = *reinterpret_cast<const float4 *>(stg + g * FM_STG + 4 * t);
                 const int flat = zb * 16 + 4 * t, sl = z0 + (flat >> a.mshift), j = flat & (a.m - 1);
-                if (red_ok && sl < a.nz)
+                if (r_ok[nb] && b >= 0 && b < a.nd && sl < a.nz)
                     atomicAdd(reinterpret_cast<float4 *>(P + (((int64_t)sl * a.n0 + i) * a.gp + a.gpl + b) * a.m + j),
                               make_float4(v.x * sc, v.y * sc, v.z * sc, v.w * sc));
+            };
+
+            if (hb >> 8) {
+                // ---- three or four angles: 16 rays per voxel fragment ----
+                float acc[NB16][2][4];
+#pragma unroll
+                for (int zb = 0; zb < NB16; ++zb)
+#pragma unroll
+                    for (int nb = 0; nb < 2; ++nb) acc[zb][nb][0] = acc[zb][nb][1] = acc[zb][nb][2] = acc[zb][nb][3] = 0.f;
+                const float ya0 = r_y[0], yb0 = r_y[0] + r_step[0], ya1 = r_y[1], yb1 = r_y[1] + r_step[1];
+                float fk = (float)kb;
+                unsigned adr_k = ld_base + (unsigned)kb * (TILE * 16);
+                for (int st = 0; st < nstep; ++st, fk += 2.0f, adr_k += 2 * TILE * 16) {
+                    const int qp = __shfl_sync(0xffffffffu, qpack, st);
+                    const int qa = qp & 0xff, qb = qp >> 8;
+                    const float fqa = (float)qa, fqb = (float)qb;
+                    // weights of my rays at rows q + 2t, q + 2t + 1 of both columns: Joseph hat max(0, 1 - |row - y|)
+                    unsigned bh[2][2], bl[2][2];
+#pragma unroll
+                    for (int nb = 0; nb < 2; ++nb) {
+                        const float da = fmaf(fk, r_step[nb], nb ? ya1 : ya0) - fqa, db = fmaf(fk, r_step[nb], nb ? yb1 : yb0) - fqb;
+                        split2(__saturatef(1.0f - fabsf(da)), __saturatef(1.0f - fabsf(da - 1.0f)), bh[nb][0], bl[nb][0]);
+                        split2(__saturatef(1.0f - fabsf(db)), __saturatef(1.0f - fabsf(db - 1.0f)), bh[nb][1], bl[nb][1]);
+                    }
+                    const unsigned adr = adr_k + ((unsigned)(ld_col ? qb : qa) << 4);
+#pragma unroll
+                    for (int zb = 0; zb < NB16; ++zb) {
+                        unsigned ah[4], al[4];
+                        ldsm4t(ah, adr + zb * 2 * FM_PLANE);
+                        ldsm4t(al, adr + zb * 2 * FM_PLANE + FM_PLANE);
+#pragma unroll
+                        for (int nb = 0; nb < 2; ++nb) {
+                            mma16816(acc[zb][nb], ah, bh[nb][0], bh[nb][1]);
+                            mma16816(acc[zb][nb], al, bh[nb][0], bh[nb][1]);
+                            mma16816(acc[zb][nb], ah, bl[nb][0], bl[nb][1]);
+                        }
+                    }
+                }
+#pragma unroll
+                for (int zb = 0; zb < NB16; ++zb) {
+                    flush(acc[zb][0], zb, 0);
+                    flush(acc[zb][1], zb, 1);
+                }
+            } else {
+                // ---- one or two angles: 8 rays per voxel fragment ----
+                float acc[NB16][4];
+#pragma unroll
+                for (int zb = 0; zb < NB16; ++zb) acc[zb][0] = acc[zb][1] = acc[zb][2] = acc[zb][3] = 0.f;
+                const float bstep = r_step[0], ya = r_y[0], yb = r_y[0] + bstep;
+                float fk = (float)kb;
+                unsigned adr_k = ld_base + (unsigned)kb * (TILE * 16);
+                for (int st = 0; st < nstep; ++st, fk += 2.0f, adr_k += 2 * TILE * 16) {
+                    const int qp = __shfl_sync(0xffffffffu, qpack, st);
+                    const int qa = qp & 0xff, qb = qp >> 8;
+                    const float da = fmaf(fk, bstep, ya) - (float)qa, db = fmaf(fk, bstep, yb) - (float)qb;   // y - (q + 2t)
+                    unsigned bh0, bl0, bh1, bl1;
+                    split2(__saturatef(1.0f - fabsf(da)), __saturatef(1.0f - fabsf(da - 1.0f)), bh0, bl0);
+                    split2(__saturatef(1.0f - fabsf(db)), __saturatef(1.0f - fabsf(db - 1.0f)), bh1, bl1);
+                    const unsigned adr = adr_k + ((unsigned)(ld_col ? qb : qa) << 4);
+#pragma unroll
+                    for (int zb = 0; zb < NB16; ++zb) {
+                        unsigned ah[4], al[4];
+                        ldsm4t(ah, adr + zb * 2 * FM_PLANE);
+                        ldsm4t(al, adr + zb * 2 * FM_PLANE + FM_PLANE);
+                        mma16816(acc[zb], ah, bh0, bh1);
+                        mma16816(acc[zb], al, bh0, bh1);
+                        mma16816(acc[zb], ah, bl0, bl1);
+                    }
+                }
+#pragma unroll
+                for (int zb = 0; zb < NB16; ++zb) flush(acc[zb], zb, 0);
             }
         }
     }
@@ -340,7 +438,7 @@ cudaError_t fm_launch(cp4d_ctx *c, const float *f, float *P, FmArgs a) {
     const int zgroups = (d.nz + a.zper - 1) / a.zper;
     // small problems: split the angle pairs of a pass over up to 8 CTAs per tile so that every SM has work
     const int64_t ctas = (int64_t)d.tiles * 2 * zgroups;
-    a.agroups = (int)std::max<int64_t>(1, std::min<int64_t>(std::min(8, std::max(1, std::min(c->n_pairs0, c->n_pairs1))), 148 / ctas));
+    a.agroups = (int)std::max<int64_t>(1, std::min<int64_t>(std::min(8, std::max(1, std::min(c->n_groups0, c->n_groups1))), 148 / ctas));
     const dim3 grid(d.tiles * a.agroups, 2 * zgroups);
     k_forward_mma<NB16><<<grid, FM_THREADS, (size_t)NB16 * 2 * FM_PLANE, c->stream>>>(f, P, a);
     return cudaGetLastError();
@@ -368,29 +466,30 @@ cudaError_t forward_mma_init() {
     return cudaFuncSetAttribute(k_forward_mma<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, 3 * 2 * FM_PLANE);
 }
 
-// host: pair adjacent base angles of one pass (same stepping axis, same sign of 1/ss, neighbouring indices); the angle with
-// the smaller |1/ss| comes first, so that a strip of four of its bins holds at most four bins of the other
-int forward_mma_pairs(const FwAngle *fw, const int32_t *order, int n0, int n_colstep, int2 *out, int *npairs0, int *npairs1) {
+// largest group of adjacent base angles whose rays one strip bookkeeping serves: a ray of another angle that touches the tile
+// sits, at the tile's middle column, at most (gs - 1) 16 sqrt2 sin(pi/n0) bins outside the first angle's window, which the two
+// spare strips (bins -4 .. -1 and 48 .. 51) absorb for n0 >= 24 (pairs) and n0 >= 72 (four).  Coarser sets: every angle on its own.
+static int fm_group_size(int n0) { return n0 >= 72 ? 4 : n0 >= 24 ? 2 : 1; }
+
+// host: group adjacent base angles of one pass (same stepping axis, same sign of 1/ss, consecutive indices); the angle with
+// the smallest |1/ss| comes first, so that a strip of four of its bins holds at most four bins of each of the others
+int forward_mma_groups(const FwAngle *fw, const int32_t *order, int n0, int n_colstep, int4 *out, int *ngroups0, int *ngroups1) {
     int n = 0;
-    // the second angle's rays are sorted into the first angle's strips by their position at the tile's middle column; a ray that
-    // touches the tile is then at most 16 sqrt2 sin(pi/n0) bins outside the first angle's window, which the two spare strips
-    // (bins -4 .. -1 and 48 .. 51) absorb for n0 >= 24.  Coarser angle sets run every angle on its own.
-    const bool may_pair = n0 >= 24;
+    const int gs = fm_group_size(n0);
     for (int pass = 0; pass < 2; ++pass) {
         const int l0 = pass ? n_colstep : 0, l1 = pass ? n0 : n_colstep;
         const int start = n;
         for (int q = l0; q < l1;) {
-            const int i = order[q];
-            if (may_pair && q + 1 < l1 && order[q + 1] == i + 1 && (fw[i].inv > 0.f) == (fw[i + 1].inv > 0.f)) {
-                const bool first = std::fabs(fw[i].inv) <= std::fabs(fw[i + 1].inv);
-                out[n++] = first ? make_int2(i, i + 1) : make_int2(i + 1, i);
-                q += 2;
-            } else {
-                out[n++] = make_int2(i, -1);
-                q += 1;
+            int idx[4] = {order[q], -1, -1, -1}, cnt = 1;
+            while (cnt < gs && q + cnt < l1 && order[q + cnt] == order[q] + cnt && (fw[order[q]].inv > 0.f) == (fw[order[q + cnt]].inv > 0.f)) {
+                idx[cnt] = order[q + cnt];
+                ++cnt;
             }
+            std::stable_sort(idx, idx + cnt, [&](int x, int y) { return std::fabs(fw[x].inv) < std::fabs(fw[y].inv); });
+            out[n++] = make_int4(idx[0], idx[1], idx[2], idx[3]);
+            q += cnt;
         }
-        *(pass ? npairs1 : npairs0) = n - start;
+        *(pass ? ngroups1 : ngroups0) = n - start;
     }
     return n;
 }
@@ -399,9 +498,9 @@ cudaError_t launch_forward_mma(cp4d_ctx *c, const float *f, float *P) {
     const Dims &d = c->d;
     int ms = 0;
     while ((1 << ms) < d.m) ++ms;
-    // 1.5 bins for the taps and the half-bin extents + (TILE/2) sqrt2 sin(pi/n0) for the drift over half a tile (pairs only)
-    const float margin = 1.5f + (d.n0 >= 24 ? 0.5f * TILE * 1.41421356f * std::sin(3.14159265f / (float)d.n0) : 0.0f);
-    FmArgs a{d.n, d.nz, d.nd, d.n0, d.m, ms, d.nd, 0, d.tiles, 1, 0, margin, c->geo, c->fwang, c->fw_pairs, c->n_pairs0, c->n_pairs1};
+    // 1.5 bins for the taps and the half-bin extents + (TILE/2) sqrt2 sin(pi/n0) per angle step for the drift over half a tile
+    const float margin = 1.5f + (float)(fm_group_size(d.n0) - 1) * 0.5f * TILE * 1.41421356f * std::sin(3.14159265f / (float)d.n0);
+    FmArgs a{d.n, d.nz, d.nd, d.n0, d.m, ms, d.nd, 0, d.tiles, 1, 0, margin, c->geo, c->fwang, c->fw_groups, c->n_groups0, c->n_groups1};
     // 16-entry batch blocks per CTA: three (192 KB of shared memory) unless the volume has fewer; m = 32 needs whole slices
     const int blocks_total = (d.nz * d.m + 15) / 16;
     int nb = std::min(3, blocks_total);
