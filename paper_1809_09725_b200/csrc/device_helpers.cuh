@@ -19,10 +19,9 @@ __device__ __forceinline__ void ldsm4t(unsigned (&a)[4], unsigned addr) {
 }
 // (x, y) -> bf16 pairs hi, lo with x = hi.x + lo.x + O(2^-18 x); low half = first element
 __device__ __forceinline__ void split2(float x, float y, unsigned &hi, unsigned &lo) {
-    const __nv_bfloat162 h = __floats2bfloat162_rn(x, y);
-    const __nv_bfloat162 l = __floats2bfloat162_rn(x - __low2float(h), y - __high2float(h));
-    hi = *reinterpret_cast<const unsigned *>(&h);
-    lo = *reinterpret_cast<const unsigned *>(&l);
+    asm("cvt.rn.bf16x2.f32 %0, %1, %2;\n" : "=r"(hi) : "f"(y), "f"(x));
+    const float hx = __uint_as_float(hi << 16), hy = __uint_as_float(hi & 0xffff0000u);       // bf16 -> fp32 is a shift
+    asm("cvt.rn.bf16x2.f32 %0, %1, %2;\n" : "=r"(lo) : "f"(y - hy), "f"(x - hx));
 }
 
 // ---- TMA 1-D bulk copy global -> shared, completion on an mbarrier (SASS UBLKCP / SYNCS) ----

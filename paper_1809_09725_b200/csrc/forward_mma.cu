@@ -147,6 +147,15 @@ __global__ void __launch_bounds__(FM_THREADS, 1) k_forward_mma(const float *__re
     const unsigned ld_half = (lane >> 3) & 1, ld_col = lane >> 4, ld_row = lane & 7;
     const unsigned ld_base = tile_s + (((ld_half * TILE + ld_col) * TILE + ld_row) << 4);
     const TileGeo *geo = a.geo + (int64_t)tile_id * a.n0;
+    // epilogue: I add batch entries 4t .. 4t+3 of block zb = coefficients j .. j+3 of slice sl; element offset of (sl, j) in P
+    unsigned zoff[NB16];
+    bool zok[NB16];
+#pragma unroll
+    for (int zb = 0; zb < NB16; ++zb) {
+        const int flat = zb * 16 + 4 * t, sl = z0 + (flat >> a.mshift), j = flat & (a.m - 1);
+        zok[zb] = sl < a.nz;
+        zoff[zb] = (unsigned)sl * (unsigned)(a.n0 * a.gp) * (unsigned)a.m + (unsigned)j;
+    }
 
     const int n_chunk = (p1 - p0 + FM_MAXG - 1) / FM_MAXG, per_chunk = n_chunk ? (p1 - p0 + n_chunk - 1) / n_chunk : 0;   // even chunks
     for (int pc = p0; pc < p1; pc += per_chunk) {
@@ -340,10 +349,16 @@ __global__ void __launch_bounds__(FM_THREADS, 1) k_forward_mma(const float *__re
             // ---- partial ray sums of this tile -> P[z][i][b][j].  My D entries are rays 2t, 2t+1 x batch entries g, g+8; a RED
             // costs about one clock per LANE whatever its width, so a block goes through a per-warp shared-memory patch and
             // leaves as one 16-byte RED per lane: lane (ray g, quad t) adds entries 4t .. 4t+3 of ray g ----
+            unsigned r_off[2];       // element offset of (angle, bin) of my ray in a slice of P
+            float r_sc[2];
+#pragma unroll
+            for (int nb = 0; nb < 2; ++nb) {
+                const int x = r_ang[nb], b = R.bstart[x] + r_bub[nb];
+                r_ok[nb] = r_ok[nb] && b >= 0 && b < a.nd;
+                r_off[nb] = (unsigned)((R.ia[x] * a.gp + a.gpl + b) * a.m);
+                r_sc[nb] = R.inva[x];
+            }
             auto flush = [&](const float (&acc)[4], int zb, int nb) {
-                const int x = r_ang[nb];
-                const int i = R.ia[x], b = R.bstart[x] + r_bub[nb];
-                const float sc = R.inva[x];
                 __syncwarp();
                 stg[(2 * t) * FM_STG + g] = acc[0];
                 stg[(2 * t + 1) * FM_STG + g] = acc[1];
@@ -351,10 +366,9 @@ __global__ void __launch_bounds__(FM_THREADS, 1) k_forward_mma(const float *__re
                 stg[(2 * t + 1) * FM_STG + g + 8] = acc[3];
                 __syncwarp();
                 const float4 v = *reinterpret_cast<const float4 *>(stg + g * FM_STG + 4 * t);
-                const int flat = zb * 16 + 4 * t, sl = z0 + (flat >> a.mshift), j = flat & (a.m - 1);
-                if (r_ok[nb] && b >= 0 && b < a.nd && sl < a.nz)
-                    atomicAdd(reinterpret_cast<float4 *>(P + (((int64_t)sl * a.n0 + i) * a.gp + a.gpl + b) * a.m + j),
-                              make_float4(v.x * sc, v.y * sc, v.z * sc, v.w * sc));
+                const float sc = r_sc[nb];
+                if (r_ok[nb] && zok[zb])
+                    atomicAdd(reinterpret_cast<float4 *>(P + (size_t)zoff[zb] + r_off[nb]), make_float4(v.x * sc, v.y * sc, v.z * sc, v.w * sc));
             };
 
             if (hb >> 8) {
@@ -447,6 +461,7 @@ cudaError_t fm_launch(cp4d_ctx *c, const float *f, float *P, FmArgs a) {
 }  // namespace
 
 bool forward_mma_supported(const Dims &d) {
+    if ((int64_t)d.nz * d.n0 * d.nd * d.m >= (int64_t)1 << 31) return false;      // the epilogue keeps 32-bit element offsets into P
     return (d.m == 4 || d.m == 8 || d.m == 16 || d.m == 32);
 }
 
