@@ -51,13 +51,18 @@ CASES = {
     "many_angles": synth.CONFIGS[1].scaled(cfg=18, n=36, nd=41, nz=2, n_angles=530, n_half_rot=1, m=4),
     # a volume smaller than one tile and a detector wider than the scratch window
     "tiny": synth.CONFIGS[1].scaled(cfg=19, n=5, nd=9, nz=1, n_angles=14, n_half_rot=2, m=4),
-    # tensor-core forward projector (forward_mma.cu): adjacent angles paired at 1 degree and at the coarsest spacing that still
-    # pairs (24 base angles: most strips fall back to one window per angle), 7 slices of m = 8 (3.5 batch blocks: a ragged last
+    # tensor-core forward projector (forward_mma.cu): adjacent angles grouped at 1 degree (four at a time) and at the coarsest
+    # spacing that still pairs (24 base angles: most strips fall back to one window per angle), 7 slices of m = 8 (3.5 batch blocks: a ragged last
     # CTA), m = 32 (two blocks per slice), m = 4 with 13 slices (4 slices per block), ragged tiles, nd != n
     "pairs_1deg_m16": synth.CONFIGS[3].scaled(cfg=22, n=100, nd=110, nz=5, n_angles=360, n_half_rot=2, m=16, n_objects=5),
     "pairs_coarse_m8": synth.CONFIGS[3].scaled(cfg=23, n=97, nd=140, nz=7, n_angles=72, n_half_rot=3, m=8, n_objects=5),
     "pairs_m32": synth.CONFIGS[2].scaled(cfg=24, n=66, nd=70, nz=3, n_angles=200, n_half_rot=2, m=32),
     "pairs_m4_z13": synth.CONFIGS[1].scaled(cfg=25, n=50, nd=47, nz=13, n_angles=90, n_half_rot=2, m=4),
+    # groups of four adjacent angles (n_theta0 >= 72: 16 rays per voxel fragment where the four angles share the 8-row windows):
+    # the coarsest spacing that still groups by four (many items fall back to pairs and single angles), and a base-angle count
+    # that leaves groups of three and two at the ends of the passes
+    "groups4_coarsest_m16": synth.CONFIGS[3].scaled(cfg=26, n=90, nd=100, nz=4, n_angles=144, n_half_rot=2, m=16, n_objects=5),
+    "groups4_tail_m8": synth.CONFIGS[3].scaled(cfg=27, n=81, nd=120, nz=5, n_angles=150, n_half_rot=1, m=8, n_objects=5),
 }
 
 
