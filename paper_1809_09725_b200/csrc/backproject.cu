@@ -243,7 +243,7 @@ __global__ void __launch_bounds__(BP_THREADS, 4) k_backproject(const float4 *__r
 // = 16 LDS.128 per angle and thread against 12 for twice the voxels.
 // ---------------------------------------------------------------------------------------------------
 constexpr int B22_THREADS = 256;         // one thread per 2 x 2 patch of a 32 x 32 tile
-constexpr int B22_CHUNK = 12;            // angles staged per pipeline stage
+constexpr int B22_CHUNK = 15;            // angles staged per pipeline stage (2 stages x 15 x 4 rows of 896 B = 105 KB: two CTAs per SM)
 
 struct B22Angle {
     float4 g;    // delta (tile origin - window start), c, s, |c|
