@@ -53,8 +53,8 @@ extern "C" {
 #define CP4D_ECUDA        -4  /* a CUDA runtime call or kernel failed; text in cp4d_last_error() */
 #define CP4D_ESTATE       -5  /* call order: cp4d_iterate before cp4d_set_data / cp4d_set_steps */
 #define CP4D_ENOMEM       -6  /* a host allocation failed (cp4d_create) */
-#define CP4D_EINTERNAL    -7  /* an invariant of the host prologue failed (cp4d_create: no backprojection pattern covers an
-                                 angle, or a tile window leaves the padded scratch row); a bug, never an input error */
+#define CP4D_EINTERNAL    -7  /* an invariant of the host prologue failed (cp4d_create: the base angles are not sorted by
+                                 the sign of cos, or a tile window leaves the padded scratch row); a bug, never an input error */
 
 typedef struct cp4d_ctx cp4d_ctx; /* opaque; owns host-side metadata only */
 

@@ -146,7 +146,7 @@ const char *cp4d_strerror(int code) {
     case CP4D_ECUDA: return "CUDA error";
     case CP4D_ESTATE: return "call order: set_data/set_steps before iterate";
     case CP4D_ENOMEM: return "host allocation failed";
-    case CP4D_EINTERNAL: return "internal invariant violated (backprojection pattern or scratch window)";
+    case CP4D_EINTERNAL: return "internal invariant violated (scratch window)";
     default: return "unknown error";
     }
 }
@@ -216,9 +216,6 @@ int cp4d_create(const cp4d_params *p, cp4d_ctx **out) {
             ang[i].fw_inv = (float)(1.0 / ss); ang[i].fw_step = (float)st;
             ang[i].fw_istep = std::fabs(st) < 1e-6 ? 0.0f : (float)(1.0 / st);
         }
-        ang[i].pat = bp_pattern(ang[i].c, ang[i].s);
-        if (ang[i].pat < 0) { delete ctx; return CP4D_EINTERNAL; }   // the 7 patterns cover [0, pi): cannot happen
-        ang[i].pat_fl = bp_pattern_fl(ang[i].pat);
     }
     ctx->n_cpos = 0;
     while (ctx->n_cpos < d.n0 && ang[ctx->n_cpos].c >= 0.f) ++ctx->n_cpos;

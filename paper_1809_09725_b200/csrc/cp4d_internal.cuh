@@ -13,7 +13,6 @@ namespace cp4d {
 constexpr int TILE = 32;          // voxel tile side of both projector kernels
 constexpr int WIN = 48;           // bins a TILE x TILE tile can touch at one angle: floor(31*sqrt2)+4
 constexpr int MAX_M = 32;
-constexpr int BP_NPAT = 7;       // bin-offset patterns of a 4x2 voxel patch (backproject.cu)
 
 // per (tile, base angle) geometry, computed in fp64 on the host at create:
 // bin coordinate of tile-local voxel (lx, ly) relative to the window start is  delta + lx*c + ly*s.
@@ -26,8 +25,6 @@ struct TileGeo {
 struct AngleTab {
     float c, s, inv_a;  // cos, sin, 1/max(|c|,|s|)
     int32_t col_step;   // 1: |s| >= |c| (ray steps over columns ix), 0: steps over rows iy
-    int32_t pat;        // backprojection patch pattern, bp_pattern(c, s)
-    uint32_t pat_fl;    // its 8 bin offsets FL_v, 4 bits each
     // forward projector, dominant-axis stepping: the ray with window coordinate du crosses step k at (du - k cc)/ss,
     // (cc, ss) = (c, s) when col_step else (s, c)
     float fw_inv, fw_step, fw_istep;  // 1/ss, -cc/ss, 1/fw_step (0 when |fw_step| < 1e-6), rounded from fp64
@@ -153,8 +150,6 @@ cudaError_t launch_backproject(cp4d_ctx *c, const float4 *gt, float *f_out, int 
 // cp4d_fbp: Shepp-Logan filter along the bins; per-half-rotation rows gathered into the projector scratch (box basis)
 cudaError_t launch_filter_sl(cp4d_ctx *c, const float *g, float *gf);
 cudaError_t launch_fold_halfrot(cp4d_ctx *c, const float *gf, float4 *gt, int Qf, float scale);
-int bp_pattern(float c, float s);  // host: pattern index in [0, BP_NPAT) or -1
-uint32_t bp_pattern_fl(int pat);   // host: the pattern's FL_v packed 4 bits each
 // out[v][a] = sum_b T(a,b) in[v][b] per voxel v, T(a,b) = psi[a*sa + b*sb]  (frame <-> coefficient contraction, L231-L237)
 cudaError_t launch_mix(cp4d_ctx *c, const float *in, float *out, int na_out, int nb_in, int sa, int sb);
 cudaError_t launch_tv_sum(cp4d_ctx *c, const float *f, double *slot);                       // sum |K2 f|_2
