@@ -48,7 +48,7 @@ constexpr int FM_STG = 20;                             // floats per ray of a wa
 struct FmArgs {
     int n, nz, nd, n0, m, mshift, gp, gpl;
     int tiles, agroups;
-    int zper;                  // slices per CTA = NB16 * 16 / m
+    int zper, z_base;          // slices per CTA = NB16 * 16 / m; first slice of this launch
     float margin;              // bins a ray of another angle of a group can sit from the first angle's bin of its touch point
     const TileGeo *geo;
     const FwAngle *fwang;
@@ -104,7 +104,7 @@ __global__ void __launch_bounds__(FM_THREADS, 1) k_forward_mma(const float *__re
     float *stg = s_stg[threadIdx.x >> 5];
     const int tiles_1d = (a.n + TILE - 1) / TILE;
     const int tile_id = blockIdx.x % a.tiles, ag = blockIdx.x / a.tiles;
-    const int pass = blockIdx.y & 1, z0 = (blockIdx.y >> 1) * a.zper;
+    const int pass = blockIdx.y & 1, z0 = a.z_base + (blockIdx.y >> 1) * a.zper;
     const int x0 = (tile_id % tiles_1d) * TILE, y0 = (tile_id / tiles_1d) * TILE;
 
     // ---- stage the tile: fp32 -> (hi, lo) bf16, pass coordinates (column = stepping axis); 4 entries (8 loads) in flight ----
@@ -445,12 +445,14 @@ __global__ void __launch_bounds__(FM_THREADS, 1) k_forward_mma(const float *__re
     }
 }
 
+// slices [z_base, z_base + nz_part) in groups of NB16 batch blocks per CTA
 template <int NB16>
-cudaError_t fm_launch(cp4d_ctx *c, const float *f, float *P, FmArgs a) {
+cudaError_t fm_launch(cp4d_ctx *c, const float *f, float *P, FmArgs a, int z_base, int nz_part) {
     const Dims &d = c->d;
     a.zper = NB16 * 16 / d.m;
-    const int zgroups = (d.nz + a.zper - 1) / a.zper;
-    // small problems: split the angle pairs of a pass over up to 8 CTAs per tile so that every SM has work
+    a.z_base = z_base;
+    const int zgroups = (nz_part + a.zper - 1) / a.zper;
+    // small problems: split the angle groups of a pass over up to 8 CTAs per tile so that every SM has work
     const int64_t ctas = (int64_t)d.tiles * 2 * zgroups;
     a.agroups = (int)std::max<int64_t>(1, std::min<int64_t>(std::min(8, std::max(1, std::min(c->n_groups0, c->n_groups1))), 148 / ctas));
     const dim3 grid(d.tiles * a.agroups, 2 * zgroups);
@@ -515,16 +517,20 @@ cudaError_t launch_forward_mma(cp4d_ctx *c, const float *f, float *P) {
     while ((1 << ms) < d.m) ++ms;
     // 1.5 bins for the taps and the half-bin extents + (TILE/2) sqrt2 sin(pi/n0) per angle step for the drift over half a tile
     const float margin = 1.5f + (float)(fm_group_size(d.n0) - 1) * 0.5f * TILE * 1.41421356f * std::sin(3.14159265f / (float)d.n0);
-    FmArgs a{d.n, d.nz, d.nd, d.n0, d.m, ms, d.nd, 0, d.tiles, 1, 0, margin, c->geo, c->fwang, c->fw_groups, c->n_groups0, c->n_groups1};
-    // 16-entry batch blocks per CTA: three (192 KB of shared memory) unless the volume has fewer; m = 32 needs whole slices
+    FmArgs a{d.n, d.nz, d.nd, d.n0, d.m, ms, d.nd, 0, d.tiles, 1, 0, 0, margin, c->geo, c->fwang, c->fw_groups, c->n_groups0, c->n_groups1};
+    // 16-entry batch blocks per CTA: three (192 KB of shared memory) unless the volume has fewer; m = 32 needs whole slices.
+    // Slices that do not fill a last group of three blocks go to a second launch with one or two blocks per CTA (config 3:
+    // 32 slices = 10 x 3 + 2), instead of a group that multiplies a block of zeros
     const int blocks_total = (d.nz * d.m + 15) / 16;
-    int nb = std::min(3, blocks_total);
-    if (d.m == 32) nb = 2;
-    switch (nb) {
-    case 1: return fm_launch<1>(c, f, P, a);
-    case 2: return fm_launch<2>(c, f, P, a);
-    default: return fm_launch<3>(c, f, P, a);
-    }
+    if (d.m == 32) return fm_launch<2>(c, f, P, a, 0, d.nz);
+    const int spb = 16 / d.m;                                   // slices per block
+    const int full = blocks_total / 3, rem = blocks_total % 3;
+    cudaError_t e = cudaSuccess;
+    if (full > 0) e = fm_launch<3>(c, f, P, a, 0, std::min(d.nz, full * 3 * spb));
+    if (e != cudaSuccess || rem == 0) return e;
+    if (full > 0) c->launches++;
+    const int zb = full * 3 * spb;
+    return rem == 1 ? fm_launch<1>(c, f, P, a, zb, d.nz - zb) : fm_launch<2>(c, f, P, a, zb, d.nz - zb);
 }
 
 }  // namespace cp4d
