@@ -40,7 +40,9 @@ static_assert(TILE == 32, "the tile staging decodes indices with shifts for TILE
 constexpr int FM_THREADS = 512;
 constexpr int FM_WARPS = FM_THREADS / 32;
 constexpr int FM_STRIPS = WIN / 4 + 2;                 // strips -1 .. WIN/4 of four window bins
-constexpr int FM_PLANE = 2 * TILE * TILE * 16;         // bytes of one (block, hi/lo) plane: [half][column][row] x 16 B
+constexpr int FM_COL = (TILE + 1) * 16;                // bytes of one tile column: 32 rows x 16 B + 16 B of padding, so that the
+                                                       // staging stores of one row across 8 columns hit 8 different bank groups
+constexpr int FM_PLANE = 2 * TILE * FM_COL;            // bytes of one (block, hi/lo) plane: [half][column][row] x 16 B
 constexpr float FM_KC = 0.5f * (TILE - 1);             // reference column where the two angles of a pair are aligned
 constexpr float FM_SPAN = 5.99f;                       // largest spread of first-tap rows an 8-row window holds
 constexpr int FM_STG = 20;                             // floats per ray of a warp's 8 x 16 epilogue patch (20: conflict-free stores)
@@ -66,7 +68,7 @@ struct FmGroup {
                                                 // ub / rinv[x] + r0[x]
     int ia[4], bstart[4];
 };
-constexpr int FM_MAXG = 24;                            // groups per chunk of a CTA's group list
+constexpr int FM_MAXG = 23;                            // groups per chunk of a CTA's group list
 constexpr int FM_MAXITEMS = 4 * FM_MAXG * FM_STRIPS;   // every (group, strip) may fall apart into four single-angle items
 constexpr int FM_LONG = 14;                            // columns from which an item counts as long
 
@@ -99,9 +101,11 @@ __global__ void __launch_bounds__(FM_THREADS, 1) k_forward_mma(const float *__re
     __shared__ __align__(16) float s_stg[FM_WARPS][8 * FM_STG];
     __shared__ __align__(16) FmGroup s_grp[FM_MAXG];
     __shared__ unsigned char s_t0[FM_MAXG], s_tn[FM_MAXG];      // first strip (+1) and number of strips of each group
-    __shared__ unsigned short s_cand[FM_MAXG * FM_STRIPS];      // candidate -> (group << 4) | (strip + 1)
     __shared__ unsigned s_item[3 * FM_MAXITEMS];
     float *stg = s_stg[threadIdx.x >> 5];
+    // candidate -> (group << 4) | (strip + 1): only alive while a chunk's items are built, when no warp uses its patch
+    unsigned short *s_cand = reinterpret_cast<unsigned short *>(&s_stg[0][0]);
+    static_assert(sizeof(unsigned short) * FM_MAXG * FM_STRIPS <= sizeof(float) * FM_WARPS * 8 * FM_STG, "candidate table fits the epilogue patches");
     const int tiles_1d = (a.n + TILE - 1) / TILE;
     const int tile_id = blockIdx.x % a.tiles, ag = blockIdx.x / a.tiles;
     const int pass = blockIdx.y & 1, z0 = a.z_base + (blockIdx.y >> 1) * a.zper;
@@ -115,7 +119,12 @@ __global__ void __launch_bounds__(FM_THREADS, 1) k_forward_mma(const float *__re
 #pragma unroll
         for (int r = 0; r < 4; ++r) {
             const int e = e0 + r * FM_THREADS;
-            const int row = e & (TILE - 1), kcol = (e >> 5) & (TILE - 1), jh = (e >> 10) & 1, zb = e >> 11;
+            // pass 1: 32 consecutive threads take the 32 rows (= x) of one column; pass 0: 16 consecutive columns (= x) of one
+            // row for each half -- either way a warp reads 1 KB of contiguous global memory per load pair
+            const int zb = e >> 11;
+            const int row = pass ? e & (TILE - 1) : (e >> 6) & (TILE - 1);
+            const int kcol = pass ? (e >> 5) & (TILE - 1) : (e & 15) | ((e >> 1) & 16);
+            const int jh = pass ? (e >> 10) & 1 : (e >> 4) & 1;
             const int gx = x0 + (pass ? row : kcol), gy = y0 + (pass ? kcol : row);
 #pragma unroll
             for (int h = 0; h < 2; ++h) {
@@ -128,11 +137,16 @@ __global__ void __launch_bounds__(FM_THREADS, 1) k_forward_mma(const float *__re
 #pragma unroll
         for (int r = 0; r < 4; ++r) {
             const int e = e0 + r * FM_THREADS;
-            const int row = e & (TILE - 1), kcol = (e >> 5) & (TILE - 1), jh = (e >> 10) & 1, zb = e >> 11;
+            // pass 1: 32 consecutive threads take the 32 rows (= x) of one column; pass 0: 16 consecutive columns (= x) of one
+            // row for each half -- either way a warp reads 1 KB of contiguous global memory per load pair
+            const int zb = e >> 11;
+            const int row = pass ? e & (TILE - 1) : (e >> 6) & (TILE - 1);
+            const int kcol = pass ? (e >> 5) & (TILE - 1) : (e & 15) | ((e >> 1) & 16);
+            const int jh = pass ? (e >> 10) & 1 : (e >> 4) & 1;
             uint4 hi, lo;
             split2(q[r][0].x, q[r][0].y, hi.x, lo.x); split2(q[r][0].z, q[r][0].w, hi.y, lo.y);
             split2(q[r][1].x, q[r][1].y, hi.z, lo.z); split2(q[r][1].z, q[r][1].w, hi.w, lo.w);
-            unsigned char *dst = tile + (size_t)(zb * 2) * FM_PLANE + ((jh * TILE + kcol) * TILE + row) * 16;
+            unsigned char *dst = tile + (size_t)(zb * 2) * FM_PLANE + (jh * TILE + kcol) * FM_COL + row * 16;
             *reinterpret_cast<uint4 *>(dst) = hi;
             *reinterpret_cast<uint4 *>(dst + FM_PLANE) = lo;
         }
@@ -145,7 +159,7 @@ __global__ void __launch_bounds__(FM_THREADS, 1) k_forward_mma(const float *__re
     const unsigned tile_s = (unsigned)__cvta_generic_to_shared(tile);
     // ldmatrix row address of this lane: matrix = lane / 8 -> (column k0 + matrix / 2, half matrix & 1), row lane & 7
     const unsigned ld_half = (lane >> 3) & 1, ld_col = lane >> 4, ld_row = lane & 7;
-    const unsigned ld_base = tile_s + (((ld_half * TILE + ld_col) * TILE + ld_row) << 4);
+    const unsigned ld_base = tile_s + (ld_half * TILE + ld_col) * FM_COL + (ld_row << 4);
     const TileGeo *geo = a.geo + (int64_t)tile_id * a.n0;
     // epilogue: I add batch entries 4t .. 4t+3 of block zb = coefficients j .. j+3 of slice sl; element offset of (sl, j) in P
     unsigned zoff[NB16];
@@ -380,8 +394,8 @@ __global__ void __launch_bounds__(FM_THREADS, 1) k_forward_mma(const float *__re
                     for (int nb = 0; nb < 2; ++nb) acc[zb][nb][0] = acc[zb][nb][1] = acc[zb][nb][2] = acc[zb][nb][3] = 0.f;
                 const float ya0 = r_y[0], yb0 = r_y[0] + r_step[0], ya1 = r_y[1], yb1 = r_y[1] + r_step[1];
                 float fk = (float)kb;
-                unsigned adr_k = ld_base + (unsigned)kb * (TILE * 16);
-                for (int st = 0; st < nstep; ++st, fk += 2.0f, adr_k += 2 * TILE * 16) {
+                unsigned adr_k = ld_base + (unsigned)kb * FM_COL;
+                for (int st = 0; st < nstep; ++st, fk += 2.0f, adr_k += 2 * FM_COL) {
                     const int qp = __shfl_sync(0xffffffffu, qpack, st);
                     const int qa = qp & 0xff, qb = qp >> 8;
                     const float fqa = (float)qa, fqb = (float)qb;
@@ -419,8 +433,8 @@ __global__ void __launch_bounds__(FM_THREADS, 1) k_forward_mma(const float *__re
                 for (int zb = 0; zb < NB16; ++zb) acc[zb][0] = acc[zb][1] = acc[zb][2] = acc[zb][3] = 0.f;
                 const float bstep = r_step[0], ya = r_y[0], yb = r_y[0] + bstep;
                 float fk = (float)kb;
-                unsigned adr_k = ld_base + (unsigned)kb * (TILE * 16);
-                for (int st = 0; st < nstep; ++st, fk += 2.0f, adr_k += 2 * TILE * 16) {
+                unsigned adr_k = ld_base + (unsigned)kb * FM_COL;
+                for (int st = 0; st < nstep; ++st, fk += 2.0f, adr_k += 2 * FM_COL) {
                     const int qp = __shfl_sync(0xffffffffu, qpack, st);
                     const int qa = qp & 0xff, qb = qp >> 8;
                     const float da = fmaf(fk, bstep, ya) - (float)qa, db = fmaf(fk, bstep, yb) - (float)qb;   // y - (q + 2t)
