@@ -55,7 +55,7 @@ int validate(const cp4d_params *p, Dims *d) {
 }
 
 struct Carve {
-    uint64_t f, ft, bp, h2, h1, g, tmp_s, scratch, psum, phi, ang, geo, red, cf, cb, psi, fwang, fworder, fwpairs, total;
+    uint64_t f, ft, bp, h2, h1, g, tmp_s, scratch, psum, phi, ang, geo, red, cf, cb, psi, fwang, fworder, fwpairs, fwitems, fwcounts, total;
 };
 Carve carve(const Dims &d) {
     Carve c;
@@ -68,6 +68,7 @@ Carve carve(const Dims &d) {
     c.geo = take((uint64_t)d.tiles * d.n0 * sizeof(TileGeo)); c.red = take(64);
     c.fwang = take((uint64_t)d.n0 * sizeof(FwAngle)); c.fworder = take((uint64_t)d.n0 * 4);
     c.fwpairs = take((uint64_t)d.n0 * sizeof(int4));
+    c.fwitems = take(forward_mma_item_bytes(d)); c.fwcounts = take((uint64_t)d.tiles * 2 * sizeof(int2));
     c.cf = c.cb = c.psi = 0;
     if (d.nf) { c.cf = take(d.Vc * 4); c.cb = take(d.Vc * 4); c.psi = take((uint64_t)d.mb * d.nf * 4); }
     c.total = o;
@@ -120,7 +121,7 @@ int forward_into(cp4d_ctx *ctx, const float *f, int mode, float sigma, const flo
     return CP4D_OK;
 }
 int adjoint_into(cp4d_ctx *ctx, const float *g, float *f) {
-    if (ctx->fw_mode == CP4D_PROJ_TENSOR && forward_mma_supported(ctx->d)) {     // (measured slower than the fp32 patch kernel)
+    if (ctx->fw_mode == CP4D_PROJ_TENSOR && forward_mma_usable(ctx)) {     // (measured slower than the fp32 patch kernel)
         CK(launch_fold_split(ctx, g, ctx->scratch), "fold");
         CK(launch_backproject_mma(ctx, ctx->scratch, ctx->d.nf ? ctx->cb : f), "backproject");
     } else {
@@ -196,6 +197,7 @@ int cp4d_create(const cp4d_params *p, cp4d_ctx **out) {
     ctx->tmp_s = (float *)(w + cv.tmp_s);
     ctx->fwang = (FwAngle *)(w + cv.fwang); ctx->fworder = (int32_t *)(w + cv.fworder);
     ctx->fw_groups = (int4 *)(w + cv.fwpairs); ctx->fw_mode = CP4D_PROJ_AUTO;
+    ctx->fw_items = forward_mma_item_bytes(d) ? (unsigned *)(w + cv.fwitems) : nullptr; ctx->fw_counts = (int2 *)(w + cv.fwcounts);
     ctx->cf = d.nf ? (float *)(w + cv.cf) : nullptr; ctx->cb = d.nf ? (float *)(w + cv.cb) : nullptr;
     ctx->psi = d.nf ? (float *)(w + cv.psi) : nullptr;
     ctx->scratch = (float4 *)(w + cv.scratch); ctx->psum = (float4 *)(w + cv.psum); ctx->phi = (float *)(w + cv.phi);
@@ -272,6 +274,7 @@ int cp4d_create(const cp4d_params *p, cp4d_ctx **out) {
         (e = cudaMemcpyAsync(ctx->fw_groups, fwpairs.data(), fwpairs.size() * sizeof(int4), cudaMemcpyHostToDevice, ctx->stream)) != cudaSuccess ||
         (e = cudaMemcpyAsync(ctx->geo, geo.data(), geo.size() * sizeof(TileGeo), cudaMemcpyHostToDevice, ctx->stream)) != cudaSuccess ||
         (e = cudaMemsetAsync(ctx->scratch, 0, (size_t)d.scratch4 * 16, ctx->stream)) != cudaSuccess ||
+        (e = forward_mma_build(ctx)) != cudaSuccess ||
         (e = cudaStreamSynchronize(ctx->stream)) != cudaSuccess) {
         ctx->err = cudaGetErrorString(e);   // (the context dies with the error: the caller only sees CP4D_ECUDA)
         cudaGetLastError();
@@ -725,8 +728,8 @@ int cp4d_set_projector_mode(cp4d_ctx *ctx, int32_t mode) {
 
 int cp4d_projector_mode_in_use(const cp4d_ctx *ctx, int32_t *forward_out, int32_t *adjoint_out) {
     if (!ctx) return CP4D_EINVAL;
-    const bool ok = forward_mma_supported(ctx->d);
-    const bool fw_tensor = (ctx->fw_mode == CP4D_PROJ_TENSOR && ok) || (ctx->fw_mode == CP4D_PROJ_AUTO && forward_mma_preferred(ctx->d));
+    const bool ok = forward_mma_usable(ctx);
+    const bool fw_tensor = (ctx->fw_mode == CP4D_PROJ_TENSOR && ok) || (ctx->fw_mode == CP4D_PROJ_AUTO && ok && forward_mma_preferred(ctx->d));
     if (forward_out) *forward_out = fw_tensor ? CP4D_PROJ_TENSOR : CP4D_PROJ_FP32;
     if (adjoint_out) *adjoint_out = (ctx->fw_mode == CP4D_PROJ_TENSOR && ok) ? CP4D_PROJ_TENSOR : CP4D_PROJ_FP32;
     return CP4D_OK;

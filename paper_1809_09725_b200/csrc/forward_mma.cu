@@ -57,6 +57,11 @@ struct FmArgs {
     const int4 *groups;        // [pass 0 groups | pass 1 groups]: up to four adjacent base angles, the one with the smallest |1/ss|
                                // first, -1 for an absent one
     int ngroups0, ngroups1;
+    unsigned *items;           // work items of every (tile, pass), built once per context by k_fm_build: slot of (tile, pass) =
+                               // 3 words x item_cap(pass) at word offset 3 (tile (cap0 + cap1) + (pass ? cap0 : 0)); long items
+                               // from the front, short ones from the back
+    int2 *counts;              // [tile][pass]: (long, short) items in the slot
+    int cap0, cap1;            // item capacity of a slot = 4 FM_STRIPS groups of the pass
 };
 
 // per-CTA record of one angle group (shared memory): the per-angle tables and this tile's window geometry, plus what the
@@ -68,8 +73,8 @@ struct FmGroup {
                                                 // ub / rinv[x] + r0[x]
     int ia[4], bstart[4];
 };
-constexpr int FM_MAXG = 23;                            // groups per chunk of a CTA's group list
-constexpr int FM_MAXITEMS = 4 * FM_MAXG * FM_STRIPS;   // every (group, strip) may fall apart into four single-angle items
+constexpr int FM_MAXG = 128;                           // angle groups of a pass whose records a CTA keeps in shared memory (18 KB)
+constexpr int FM_BUILDG = 32;                          // groups per round of the item builder
 constexpr int FM_LONG = 14;                            // columns from which an item counts as long
 
 // columns k in [0, TILE) where a ray group whose first-tap rows lie in [ylo + k st, yhi + k st] touches rows 0 .. TILE-1:
@@ -87,112 +92,51 @@ __device__ __forceinline__ void col_range(float ylo, float yhi, float st, float 
     }
 }
 
-// One work item of a CTA, three shared-memory words built once per CTA by all threads in parallel:
-//   w0 = (group << 4 | strip + 1) | klo << 16 | khi << 24            columns of the tile the item's rays touch
+// One work item of a (tile, pass), three words built once per context by k_fm_build (the geometry does not change):
+//   w0 = (group in pass << 4 | strip + 1) | klo << 16 | khi << 24    columns of the tile the item's rays touch
 //   w1 = bs1 | bs2 << 8 | bs3 << 16 (signed bytes) | used << 24       first window bin of angles 1-3 in this strip; angles in use
 //   w2 = 4 | cnt1 << 4 | cnt2 << 8 | cnt3 << 12 | hb << 16            bins per angle; hb = four nibbles, one per half block of
 //                                                                     four ray slots: angle | 4 (bins 4-7 of a long single) | 8 (valid)
 // Half blocks 0, 1 are the 8 rays of the first MMA column block, 2, 3 those of the second (only items of 3 or 4 angles).
 
-template <int NB16>
-__global__ void __launch_bounds__(FM_THREADS, 1) k_forward_mma(const float *__restrict__ f, float *__restrict__ P, FmArgs a) {
-    extern __shared__ __align__(128) unsigned char tile[];     // [NB16][2][2][TILE][TILE] x 16 B
-    __shared__ int s_next, s_nlong, s_nshort, s_ncand;
-    __shared__ __align__(16) float s_stg[FM_WARPS][8 * FM_STG];
-    __shared__ __align__(16) FmGroup s_grp[FM_MAXG];
-    __shared__ unsigned char s_t0[FM_MAXG], s_tn[FM_MAXG];      // first strip (+1) and number of strips of each group
-    __shared__ unsigned s_item[3 * FM_MAXITEMS];
-    float *stg = s_stg[threadIdx.x >> 5];
-    // candidate -> (group << 4) | (strip + 1): only alive while a chunk's items are built, when no warp uses its patch
-    unsigned short *s_cand = reinterpret_cast<unsigned short *>(&s_stg[0][0]);
-    static_assert(sizeof(unsigned short) * FM_MAXG * FM_STRIPS <= sizeof(float) * FM_WARPS * 8 * FM_STG, "candidate table fits the epilogue patches");
-    const int tiles_1d = (a.n + TILE - 1) / TILE;
-    const int tile_id = blockIdx.x % a.tiles, ag = blockIdx.x / a.tiles;
-    const int pass = blockIdx.y & 1, z0 = a.z_base + (blockIdx.y >> 1) * a.zper;
-    const int x0 = (tile_id % tiles_1d) * TILE, y0 = (tile_id / tiles_1d) * TILE;
-
-    // ---- stage the tile: fp32 -> (hi, lo) bf16, pass coordinates (column = stepping axis); 4 entries (8 loads) in flight ----
-    constexpr int N_ENT = NB16 * 2 * TILE * TILE;
-    static_assert(N_ENT % (4 * FM_THREADS) == 0, "staging loop is unrolled by 4");
-    for (int e0 = threadIdx.x; e0 < N_ENT; e0 += 4 * FM_THREADS) {
-        float4 q[4][2];
+// the shared-memory record of one angle group for one tile
+__device__ __forceinline__ void fm_group_record(const FmArgs &a, const TileGeo *geo, const int4 gr, FmGroup &R, FwAngle &A0, TileGeo &G0) {
+    const int idx[4] = {gr.x, gr.y, gr.z, gr.w};
+    A0 = a.fwang[gr.x];
+    G0 = geo[gr.x];
 #pragma unroll
-        for (int r = 0; r < 4; ++r) {
-            const int e = e0 + r * FM_THREADS;
-            // pass 1: 32 consecutive threads take the 32 rows (= x) of one column; pass 0: 16 consecutive columns (= x) of one
-            // row for each half -- either way a warp reads 1 KB of contiguous global memory per load pair
-            const int zb = e >> 11;
-            const int row = pass ? e & (TILE - 1) : (e >> 6) & (TILE - 1);
-            const int kcol = pass ? (e >> 5) & (TILE - 1) : (e & 15) | ((e >> 1) & 16);
-            const int jh = pass ? (e >> 10) & 1 : (e >> 4) & 1;
-            const int gx = x0 + (pass ? row : kcol), gy = y0 + (pass ? kcol : row);
-#pragma unroll
-            for (int h = 0; h < 2; ++h) {
-                const int flat = zb * 16 + jh * 8 + h * 4, sl = z0 + (flat >> a.mshift), j = flat & (a.m - 1);
-                q[r][h] = make_float4(0.f, 0.f, 0.f, 0.f);
-                if (gx < a.n && gy < a.n && sl < a.nz)
-                    q[r][h] = __ldg(reinterpret_cast<const float4 *>(f + (((int64_t)sl * a.n + gy) * a.n + gx) * a.m + j));
-            }
-        }
-#pragma unroll
-        for (int r = 0; r < 4; ++r) {
-            const int e = e0 + r * FM_THREADS;
-            // pass 1: 32 consecutive threads take the 32 rows (= x) of one column; pass 0: 16 consecutive columns (= x) of one
-            // row for each half -- either way a warp reads 1 KB of contiguous global memory per load pair
-            const int zb = e >> 11;
-            const int row = pass ? e & (TILE - 1) : (e >> 6) & (TILE - 1);
-            const int kcol = pass ? (e >> 5) & (TILE - 1) : (e & 15) | ((e >> 1) & 16);
-            const int jh = pass ? (e >> 10) & 1 : (e >> 4) & 1;
-            uint4 hi, lo;
-            split2(q[r][0].x, q[r][0].y, hi.x, lo.x); split2(q[r][0].z, q[r][0].w, hi.y, lo.y);
-            split2(q[r][1].x, q[r][1].y, hi.z, lo.z); split2(q[r][1].z, q[r][1].w, hi.w, lo.w);
-            unsigned char *dst = tile + (size_t)(zb * 2) * FM_PLANE + (jh * TILE + kcol) * FM_COL + row * 16;
-            *reinterpret_cast<uint4 *>(dst) = hi;
-            *reinterpret_cast<uint4 *>(dst + FM_PLANE) = lo;
-        }
+    for (int x = 0; x < 4; ++x) {
+        const int i = idx[x] >= 0 ? idx[x] : gr.x;
+        const FwAngle A = a.fwang[i];
+        const TileGeo G = geo[i];
+        R.inv[x] = A.inv; R.step[x] = A.step; R.delta[x] = G.delta; R.inva[x] = A.inv_a;
+        R.istep[x] = fabsf(A.step) > 1e-6f ? 1.0f / A.step : 0.0f;
+        // ray ub of angle x sits, at the reference column, at angle-0 bin coordinate phi = ub inv_x / inv_0 + r0
+        R.r0[x] = (FM_KC * (A.step - A0.step) - G.delta * A.inv) / A0.inv + G0.delta;
+        R.rinv[x] = A0.inv / A.inv;
+        R.ia[x] = idx[x]; R.bstart[x] = G.bstart;
     }
+}
 
-    // ---- this CTA's share of the pass's angle groups, in chunks of FM_MAXG ----
-    const int pbeg = pass ? a.ngroups0 : 0, pcnt = pass ? a.ngroups1 : a.ngroups0;
-    const int p0 = pbeg + (int)((int64_t)pcnt * ag / a.agroups), p1 = pbeg + (int)((int64_t)pcnt * (ag + 1) / a.agroups);
-    const int lane = threadIdx.x & 31, g = lane >> 2, t = lane & 3;
-    const unsigned tile_s = (unsigned)__cvta_generic_to_shared(tile);
-    // ldmatrix row address of this lane: matrix = lane / 8 -> (column k0 + matrix / 2, half matrix & 1), row lane & 7
-    const unsigned ld_half = (lane >> 3) & 1, ld_col = lane >> 4, ld_row = lane & 7;
-    const unsigned ld_base = tile_s + (ld_half * TILE + ld_col) * FM_COL + (ld_row << 4);
+// Builds the work items of one (tile, pass) into its global slot (once per context: they depend on the geometry only).
+__global__ void __launch_bounds__(FM_THREADS, 1) k_fm_build(FmArgs a) {
+    __shared__ int s_nlong, s_nshort, s_ncand;
+    __shared__ __align__(16) FmGroup s_grp[FM_BUILDG];
+    __shared__ unsigned char s_t0[FM_BUILDG], s_tn[FM_BUILDG];      // first strip (+1) and number of strips of each group
+    __shared__ unsigned short s_cand[FM_BUILDG * FM_STRIPS];        // candidate -> (group in round << 4) | (strip + 1)
+    const int tile_id = blockIdx.x, pass = blockIdx.y, lane = threadIdx.x & 31;
     const TileGeo *geo = a.geo + (int64_t)tile_id * a.n0;
-    // epilogue: I add batch entries 4t .. 4t+3 of block zb = coefficients j .. j+3 of slice sl; element offset of (sl, j) in P
-    unsigned zoff[NB16];
-    bool zok[NB16];
-#pragma unroll
-    for (int zb = 0; zb < NB16; ++zb) {
-        const int flat = zb * 16 + 4 * t, sl = z0 + (flat >> a.mshift), j = flat & (a.m - 1);
-        zok[zb] = sl < a.nz;
-        zoff[zb] = (unsigned)sl * (unsigned)(a.n0 * a.gp) * (unsigned)a.m + (unsigned)j;
-    }
-
-    const int n_chunk = (p1 - p0 + FM_MAXG - 1) / FM_MAXG, per_chunk = n_chunk ? (p1 - p0 + n_chunk - 1) / n_chunk : 0;   // even chunks
-    for (int pc = p0; pc < p1; pc += per_chunk) {
-        const int npc = min(per_chunk, p1 - pc);
-        __syncthreads();                                     // the tile is staged / every warp is done with the previous chunk
+    const int pbeg = pass ? a.ngroups0 : 0, p1 = pbeg + (pass ? a.ngroups1 : a.ngroups0);
+    const int cap = pass ? a.cap1 : a.cap0;
+    unsigned *slot = a.items + 3 * ((size_t)tile_id * (a.cap0 + a.cap1) + (pass ? a.cap0 : 0));
+    if (threadIdx.x == 0) { s_nlong = 0; s_nshort = 0; }
+    for (int pc = pbeg; pc < p1; pc += FM_BUILDG) {
+        const int npc = min(FM_BUILDG, p1 - pc);
+        __syncthreads();
         if ((int)threadIdx.x < npc) {
-            const int4 gr = a.groups[pc + threadIdx.x];
-            const int idx[4] = {gr.x, gr.y, gr.z, gr.w};
-            const FwAngle A0 = a.fwang[gr.x];
-            const TileGeo G0 = geo[gr.x];
-            FmGroup &R = s_grp[threadIdx.x];
-#pragma unroll
-            for (int x = 0; x < 4; ++x) {
-                const int i = idx[x] >= 0 ? idx[x] : gr.x;
-                const FwAngle A = a.fwang[i];
-                const TileGeo G = geo[i];
-                R.inv[x] = A.inv; R.step[x] = A.step; R.delta[x] = G.delta; R.inva[x] = A.inv_a;
-                R.istep[x] = fabsf(A.step) > 1e-6f ? 1.0f / A.step : 0.0f;
-                // ray ub of angle x sits, at the reference column, at angle-0 bin coordinate phi = ub inv_x / inv_0 + r0
-                R.r0[x] = (FM_KC * (A.step - A0.step) - G.delta * A.inv) / A0.inv + G0.delta;
-                R.rinv[x] = A0.inv / A.inv;
-                R.ia[x] = idx[x]; R.bstart[x] = G.bstart;
-            }
+            FwAngle A0;
+            TileGeo G0;
+            fm_group_record(a, geo, a.groups[pc + threadIdx.x], s_grp[threadIdx.x], A0, G0);
             // strips that can hold a ray touching the tile: angle-0 window coordinates of the tile corners, widened by the
             // distance a ray of another angle can sit from the bin of its touch point at the reference column (a.margin)
             const float ss = 1.0f / A0.inv, cc = -A0.step * ss, e = (float)(TILE - 1);
@@ -215,7 +159,7 @@ __global__ void __launch_bounds__(FM_THREADS, 1) k_forward_mma(const float *__re
                 for (int r = 0; r < n; ++r) s_cand[base + incl - n + r] = (unsigned short)((q << 4) | (s_t0[q] + r));
                 base += __shfl_sync(0xffffffffu, incl, 31);
             }
-            if (lane == 0) { s_ncand = base; s_nlong = 0; s_nshort = 0; s_next = 0; }
+            if (lane == 0) s_ncand = base;
         }
         __syncthreads();
         // ---- work items: every candidate (group, strip) is examined by one thread: each angle's group of bins in the strip,
@@ -224,6 +168,7 @@ __global__ void __launch_bounds__(FM_THREADS, 1) k_forward_mma(const float *__re
         for (int cnd = threadIdx.x; cnd < s_ncand; cnd += FM_THREADS) {
             const unsigned uu = s_cand[cnd];
             const FmGroup &R = s_grp[uu >> 4];
+            const unsigned gg = (unsigned)(pc - pbeg) + (uu >> 4);          // group index within the pass
             const int ts = (int)(uu & 15) - 1;
             const float ft4 = 4.0f * (float)ts;
             int bs[4], cnt[4], ka[4], kb[4];
@@ -275,10 +220,10 @@ __global__ void __launch_bounds__(FM_THREADS, 1) k_forward_mma(const float *__re
                 int fa, fb;
                 cols(S, fa, fb);
                 const bool lng = fb - fa >= FM_LONG;
-                const int at = lng ? atomicAdd(&s_nlong, 1) : FM_MAXITEMS - 1 - atomicAdd(&s_nshort, 1);
-                s_item[3 * at] = uu | ((unsigned)fa << 16) | ((unsigned)fb << 24);
-                s_item[3 * at + 1] = ((unsigned)bs[1] & 0xffu) | (((unsigned)bs[2] & 0xffu) << 8) | (((unsigned)bs[3] & 0xffu) << 16) | (S << 24);
-                s_item[3 * at + 2] = 4u | ((unsigned)cnt[1] << 4) | ((unsigned)cnt[2] << 8) | ((unsigned)cnt[3] << 12) | (hb << 16);
+                const int at = lng ? atomicAdd(&s_nlong, 1) : cap - 1 - atomicAdd(&s_nshort, 1);
+                slot[3 * at] = (gg << 4) | (uu & 15u) | ((unsigned)fa << 16) | ((unsigned)fb << 24);
+                slot[3 * at + 1] = ((unsigned)bs[1] & 0xffu) | (((unsigned)bs[2] & 0xffu) << 8) | (((unsigned)bs[3] & 0xffu) << 16) | (S << 24);
+                slot[3 * at + 2] = 4u | ((unsigned)cnt[1] << 4) | ((unsigned)cnt[2] << 8) | ((unsigned)cnt[3] << 12) | (hb << 16);
             };
             auto nibbles = [&](unsigned S) {                   // the angles of S on consecutive half blocks
                 unsigned hb = 0;
@@ -309,15 +254,111 @@ __global__ void __launch_bounds__(FM_THREADS, 1) k_forward_mma(const float *__re
             }
         }
         __syncthreads();
-        const int n_long = s_nlong, n_items = n_long + s_nshort;
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) a.counts[tile_id * 2 + pass] = make_int2(s_nlong, s_nshort);
+}
 
-        for (;;) {
-            int u = 0;
-            if (lane == 0) u = atomicAdd(&s_next, 1);
-            u = __shfl_sync(0xffffffffu, u, 0);
-            if (u >= n_items) break;
-            const int at = u < n_long ? u : FM_MAXITEMS - 1 - (u - n_long);
-            const unsigned w0 = s_item[3 * at], w1 = s_item[3 * at + 1], w2 = s_item[3 * at + 2];
+template <int NB16>
+__global__ void __launch_bounds__(FM_THREADS, 1) k_forward_mma(const float *__restrict__ f, float *__restrict__ P, FmArgs a) {
+    extern __shared__ __align__(128) unsigned char tile[];     // [NB16][2][2][TILE][TILE + 1] x 16 B
+    __shared__ int s_next;
+    __shared__ __align__(16) float s_stg[FM_WARPS][8 * FM_STG];
+    __shared__ __align__(16) FmGroup s_grp[FM_MAXG];
+    float *stg = s_stg[threadIdx.x >> 5];
+    const int tiles_1d = (a.n + TILE - 1) / TILE;
+    const int tile_id = blockIdx.x % a.tiles, ag = blockIdx.x / a.tiles;
+    const int pass = blockIdx.y & 1, z0 = a.z_base + (blockIdx.y >> 1) * a.zper;
+    const int x0 = (tile_id % tiles_1d) * TILE, y0 = (tile_id / tiles_1d) * TILE;
+
+    // ---- stage the tile: fp32 -> (hi, lo) bf16, pass coordinates (column = stepping axis); 4 entries (8 loads) in flight ----
+    constexpr int N_ENT = NB16 * 2 * TILE * TILE;
+    static_assert(N_ENT % (4 * FM_THREADS) == 0, "staging loop is unrolled by 4");
+    for (int e0 = threadIdx.x; e0 < N_ENT; e0 += 4 * FM_THREADS) {
+        float4 q[4][2];
+#pragma unroll
+        for (int r = 0; r < 4; ++r) {
+            const int e = e0 + r * FM_THREADS;
+            // pass 1: 32 consecutive threads take the 32 rows (= x) of one column; pass 0: 16 consecutive columns (= x) of one
+            // row for each half -- either way a warp reads 1 KB of contiguous global memory per load pair
+            const int zb = e >> 11;
+            const int row = pass ? e & (TILE - 1) : (e >> 6) & (TILE - 1);
+            const int kcol = pass ? (e >> 5) & (TILE - 1) : (e & 15) | ((e >> 1) & 16);
+            const int jh = pass ? (e >> 10) & 1 : (e >> 4) & 1;
+            const int gx = x0 + (pass ? row : kcol), gy = y0 + (pass ? kcol : row);
+#pragma unroll
+            for (int h = 0; h < 2; ++h) {
+                const int flat = zb * 16 + jh * 8 + h * 4, sl = z0 + (flat >> a.mshift), j = flat & (a.m - 1);
+                q[r][h] = make_float4(0.f, 0.f, 0.f, 0.f);
+                if (gx < a.n && gy < a.n && sl < a.nz)
+                    q[r][h] = __ldg(reinterpret_cast<const float4 *>(f + (((int64_t)sl * a.n + gy) * a.n + gx) * a.m + j));
+            }
+        }
+#pragma unroll
+        for (int r = 0; r < 4; ++r) {
+            const int e = e0 + r * FM_THREADS;
+            // pass 1: 32 consecutive threads take the 32 rows (= x) of one column; pass 0: 16 consecutive columns (= x) of one
+            // row for each half -- either way a warp reads 1 KB of contiguous global memory per load pair
+            const int zb = e >> 11;
+            const int row = pass ? e & (TILE - 1) : (e >> 6) & (TILE - 1);
+            const int kcol = pass ? (e >> 5) & (TILE - 1) : (e & 15) | ((e >> 1) & 16);
+            const int jh = pass ? (e >> 10) & 1 : (e >> 4) & 1;
+            uint4 hi, lo;
+            split2(q[r][0].x, q[r][0].y, hi.x, lo.x); split2(q[r][0].z, q[r][0].w, hi.y, lo.y);
+            split2(q[r][1].x, q[r][1].y, hi.z, lo.z); split2(q[r][1].z, q[r][1].w, hi.w, lo.w);
+            unsigned char *dst = tile + (size_t)(zb * 2) * FM_PLANE + (jh * TILE + kcol) * FM_COL + row * 16;
+            *reinterpret_cast<uint4 *>(dst) = hi;
+            *reinterpret_cast<uint4 *>(dst + FM_PLANE) = lo;
+        }
+    }
+
+    const int pbeg = pass ? a.ngroups0 : 0, pcnt = pass ? a.ngroups1 : a.ngroups0;
+    const int lane = threadIdx.x & 31, g = lane >> 2, t = lane & 3;
+    const unsigned tile_s = (unsigned)__cvta_generic_to_shared(tile);
+    // ldmatrix row address of this lane: matrix = lane / 8 -> (column k0 + matrix / 2, half matrix & 1), row lane & 7
+    const unsigned ld_half = (lane >> 3) & 1, ld_col = lane >> 4, ld_row = lane & 7;
+    const unsigned ld_base = tile_s + (ld_half * TILE + ld_col) * FM_COL + (ld_row << 4);
+    const TileGeo *geo = a.geo + (int64_t)tile_id * a.n0;
+    // epilogue: I add batch entries 4t .. 4t+3 of block zb = coefficients j .. j+3 of slice sl; element offset of (sl, j) in P
+    unsigned zoff[NB16];
+    bool zok[NB16];
+#pragma unroll
+    for (int zb = 0; zb < NB16; ++zb) {
+        const int flat = zb * 16 + 4 * t, sl = z0 + (flat >> a.mshift), j = flat & (a.m - 1);
+        zok[zb] = sl < a.nz;
+        zoff[zb] = (unsigned)sl * (unsigned)(a.n0 * a.gp) * (unsigned)a.m + (unsigned)j;
+    }
+
+    // ---- the records of all angle groups of this pass for this tile; the item list of (tile, pass) ----
+    if (threadIdx.x == 0) s_next = 0;
+    for (int q = threadIdx.x; q < pcnt; q += FM_THREADS) {
+        FwAngle A0;
+        TileGeo G0;
+        fm_group_record(a, geo, a.groups[pbeg + q], s_grp[q], A0, G0);
+    }
+    __syncthreads();                                         // the tile is staged, the records are written
+    {
+        const int2 cnt = a.counts[tile_id * 2 + pass];
+        const int n_long = cnt.x, n_items = cnt.x + cnt.y, cap = pass ? a.cap1 : a.cap0;
+        const unsigned *slot = a.items + 3 * ((size_t)tile_id * (a.cap0 + a.cap1) + (pass ? a.cap0 : 0));
+        // warps draw items from one counter; small problems split the list over the agroups CTAs of a tile (item u of CTA ag
+        // is list entry u agroups + ag, which keeps long and short items on every CTA).  The next item is fetched while the
+        // current one runs
+        auto fetch = [&](int &u, unsigned &w0, unsigned &w1, unsigned &w2) {
+            int v = 0;
+            if (lane == 0) v = atomicAdd(&s_next, 1);
+            u = __shfl_sync(0xffffffffu, v, 0) * a.agroups + ag;
+            w0 = w1 = w2 = 0u;
+            if (u < n_items) {
+                const unsigned *it = slot + 3 * (size_t)(u < n_long ? u : cap - 1 - (u - n_long));
+                w0 = __ldg(it); w1 = __ldg(it + 1); w2 = __ldg(it + 2);
+            }
+        };
+        int u, un;
+        unsigned w0, w1, w2, x0w, x1w, x2w;
+        fetch(u, w0, w1, w2);
+        for (; u < n_items; u = un, w0 = x0w, w1 = x1w, w2 = x2w) {
+            fetch(un, x0w, x1w, x2w);
             const FmGroup &R = s_grp[(w0 & 0xffffu) >> 4];
             const int ts = (int)(w0 & 15u) - 1, klo = (int)((w0 >> 16) & 0xffu), khi = (int)(w0 >> 24);
             const unsigned bspack = (w1 << 8) | ((unsigned)(4 * ts) & 0xffu);      // first bin of angle x: signed byte x
@@ -466,9 +507,9 @@ cudaError_t fm_launch(cp4d_ctx *c, const float *f, float *P, FmArgs a, int z_bas
     a.zper = NB16 * 16 / d.m;
     a.z_base = z_base;
     const int zgroups = (nz_part + a.zper - 1) / a.zper;
-    // small problems: split the angle groups of a pass over up to 8 CTAs per tile so that every SM has work
+    // small problems: split the item list of a (tile, pass) over up to 8 CTAs so that every SM has work
     const int64_t ctas = (int64_t)d.tiles * 2 * zgroups;
-    a.agroups = (int)std::max<int64_t>(1, std::min<int64_t>(std::min(8, std::max(1, std::min(c->n_groups0, c->n_groups1))), 148 / ctas));
+    a.agroups = (int)std::max<int64_t>(1, std::min<int64_t>(8, 148 / ctas));
     const dim3 grid(d.tiles * a.agroups, 2 * zgroups);
     k_forward_mma<NB16><<<grid, FM_THREADS, (size_t)NB16 * 2 * FM_PLANE, c->stream>>>(f, P, a);
     return cudaGetLastError();
@@ -525,13 +566,40 @@ int forward_mma_groups(const FwAngle *fw, const int32_t *order, int n0, int n_co
     return n;
 }
 
-cudaError_t launch_forward_mma(cp4d_ctx *c, const float *f, float *P) {
+static FmArgs fm_args(const cp4d_ctx *c) {
     const Dims &d = c->d;
     int ms = 0;
     while ((1 << ms) < d.m) ++ms;
     // 1.5 bins for the taps and the half-bin extents + (TILE/2) sqrt2 sin(pi/n0) per angle step for the drift over half a tile
     const float margin = 1.5f + (float)(fm_group_size(d.n0) - 1) * 0.5f * TILE * 1.41421356f * std::sin(3.14159265f / (float)d.n0);
-    FmArgs a{d.n, d.nz, d.nd, d.n0, d.m, ms, d.nd, 0, d.tiles, 1, 0, 0, margin, c->geo, c->fwang, c->fw_groups, c->n_groups0, c->n_groups1};
+    return FmArgs{d.n, d.nz, d.nd, d.n0, d.m, ms, d.nd, 0, d.tiles, 1, 0, 0, margin, c->geo, c->fwang, c->fw_groups, c->n_groups0, c->n_groups1,
+                  c->fw_items, c->fw_counts, 4 * FM_STRIPS * c->n_groups0, 4 * FM_STRIPS * c->n_groups1};
+}
+
+// item slots of a context: every (group, strip) of a tile may fall apart into four single-angle items; the groups of both
+// passes together are at most n0 / group size + 8 (a pass ends, the sign of 1/ss changes or the order jumps at most 8 times)
+uint64_t forward_mma_item_bytes(const Dims &d) {
+    if (!forward_mma_supported(d)) return 0;
+    return (uint64_t)d.tiles * 4 * FM_STRIPS * (uint64_t)(d.n0 / fm_group_size(d.n0) + 8) * 12;
+}
+
+// the tensor kernel can run in this context: supported shape, the group records of a pass fit its shared memory, and the
+// groups fit the item slots (cp4d_create: after forward_mma_groups)
+bool forward_mma_usable(const cp4d_ctx *c) {
+    return forward_mma_supported(c->d) && c->fw_items != nullptr && c->n_groups0 <= FM_MAXG && c->n_groups1 <= FM_MAXG &&
+           c->n_groups0 + c->n_groups1 <= c->d.n0 / fm_group_size(c->d.n0) + 8;
+}
+
+// cp4d_create: the work items of every (tile, pass), once (they depend on the geometry only)
+cudaError_t forward_mma_build(cp4d_ctx *c) {
+    if (!forward_mma_usable(c)) return cudaSuccess;
+    k_fm_build<<<dim3(c->d.tiles, 2), FM_THREADS, 0, c->stream>>>(fm_args(c));
+    return cudaGetLastError();
+}
+
+cudaError_t launch_forward_mma(cp4d_ctx *c, const float *f, float *P) {
+    const Dims &d = c->d;
+    const FmArgs a = fm_args(c);
     // 16-entry batch blocks per CTA: three (192 KB of shared memory) unless the volume has fewer; m = 32 needs whole slices.
     // Slices that do not fill a last group of three blocks go to a second launch with one or two blocks per CTA (config 3:
     // 32 slices = 10 x 3 + 2), instead of a group that multiplies a block of zeros

@@ -210,7 +210,7 @@ cudaError_t launch_forward_partial(cp4d_ctx *c, const float *f, float4 *P) {
     if (e != cudaSuccess) return e;
     c->launches += 2;
     float *Pf = reinterpret_cast<float *>(P);
-    if ((c->fw_mode == CP4D_PROJ_TENSOR && forward_mma_supported(d)) || (c->fw_mode == CP4D_PROJ_AUTO && forward_mma_preferred(d)))
+    if (forward_mma_usable(c) && (c->fw_mode == CP4D_PROJ_TENSOR || (c->fw_mode == CP4D_PROJ_AUTO && forward_mma_preferred(d))))
         return launch_forward_mma(c, f, Pf);
     switch (pick_jq(d.Q)) {
     case 4: return fwd_launch_rays<4>(c, f, Pf, a);
