@@ -90,7 +90,7 @@ typedef struct {
 /* Bytes of device workspace a context for these sizes needs (state f, f~, K1^T h1, h2[4], h1, g, one sinogram-sized
  * temporary, the zero-padded folded sinogram of the adjoint (m * n_theta0 * (nd + pads) * nz floats), the forward projector's
  * partial ray sums (m * n_theta0 * nd * nz floats), tables -- among them the work items of the tensor-core forward
- * projector, 672 bytes per 32 x 32 tile and group of four base angles; in frame mode with N_t > m two coefficient stacks
+ * projector, 2.7 KB per 32 x 32 tile and group of four base angles; in frame mode with N_t > m two coefficient stacks
  * as well).
  * Host only; ignores workspace_dev/stream/phi_host.  Errors: CP4D_EINVAL (see cp4d_params). */
 int cp4d_workspace_bytes(const cp4d_params *p, uint64_t *bytes_out);

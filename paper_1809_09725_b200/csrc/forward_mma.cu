@@ -58,7 +58,7 @@ struct FmArgs {
                                // first, -1 for an absent one
     int ngroups0, ngroups1;
     unsigned *items;           // work items of every (tile, pass), built once per context by k_fm_build: slot of (tile, pass) =
-                               // 3 words x item_cap(pass) at word offset 3 (tile (cap0 + cap1) + (pass ? cap0 : 0)); long items
+                               // 12 words x item_cap(pass) at word offset 12 (tile (cap0 + cap1) + (pass ? cap0 : 0)); long items
                                // from the front, short ones from the back
     int2 *counts;              // [tile][pass]: (long, short) items in the slot
     int cap0, cap1;            // item capacity of a slot = 4 FM_STRIPS groups of the pass
@@ -75,6 +75,7 @@ struct FmGroup {
 };
 constexpr int FM_MAXG = 128;                           // angle groups of a pass whose records a CTA keeps in shared memory (18 KB)
 constexpr int FM_BUILDG = 32;                          // groups per round of the item builder
+constexpr int FM_ITEMW = 12;                           // 32-bit words per work item
 constexpr int FM_LONG = 14;                            // columns from which an item counts as long
 
 // columns k in [0, TILE) where a ray group whose first-tap rows lie in [ylo + k st, yhi + k st] touches rows 0 .. TILE-1:
@@ -97,6 +98,7 @@ __device__ __forceinline__ void col_range(float ylo, float yhi, float st, float 
 //   w1 = bs1 | bs2 << 8 | bs3 << 16 (signed bytes) | used << 24       first window bin of angles 1-3 in this strip; angles in use
 //   w2 = 4 | cnt1 << 4 | cnt2 << 8 | cnt3 << 12 | hb << 16            bins per angle; hb = four nibbles, one per half block of
 //                                                                     four ray slots: angle | 4 (bins 4-7 of a long single) | 8 (valid)
+//   w3 = 0;  w4 .. w11 = 16 x (qa | qb << 8)                          first row of the 8-row window at the two columns of step s
 // Half blocks 0, 1 are the 8 rays of the first MMA column block, 2, 3 those of the second (only items of 3 or 4 angles).
 
 // the shared-memory record of one angle group for one tile
@@ -128,7 +130,7 @@ __global__ void __launch_bounds__(FM_THREADS, 1) k_fm_build(FmArgs a) {
     const TileGeo *geo = a.geo + (int64_t)tile_id * a.n0;
     const int pbeg = pass ? a.ngroups0 : 0, p1 = pbeg + (pass ? a.ngroups1 : a.ngroups0);
     const int cap = pass ? a.cap1 : a.cap0;
-    unsigned *slot = a.items + 3 * ((size_t)tile_id * (a.cap0 + a.cap1) + (pass ? a.cap0 : 0));
+    unsigned *slot = a.items + FM_ITEMW * ((size_t)tile_id * (a.cap0 + a.cap1) + (pass ? a.cap0 : 0));
     if (threadIdx.x == 0) { s_nlong = 0; s_nshort = 0; }
     for (int pc = pbeg; pc < p1; pc += FM_BUILDG) {
         const int npc = min(FM_BUILDG, p1 - pc);
@@ -221,9 +223,24 @@ __global__ void __launch_bounds__(FM_THREADS, 1) k_fm_build(FmArgs a) {
                 cols(S, fa, fb);
                 const bool lng = fb - fa >= FM_LONG;
                 const int at = lng ? atomicAdd(&s_nlong, 1) : cap - 1 - atomicAdd(&s_nshort, 1);
-                slot[3 * at] = (gg << 4) | (uu & 15u) | ((unsigned)fa << 16) | ((unsigned)fb << 24);
-                slot[3 * at + 1] = ((unsigned)bs[1] & 0xffu) | (((unsigned)bs[2] & 0xffu) << 8) | (((unsigned)bs[3] & 0xffu) << 16) | (S << 24);
-                slot[3 * at + 2] = 4u | ((unsigned)cnt[1] << 4) | ((unsigned)cnt[2] << 8) | ((unsigned)cnt[3] << 12) | (hb << 16);
+                unsigned *it = slot + FM_ITEMW * (size_t)at;
+                it[0] = (gg << 4) | (uu & 15u) | ((unsigned)fa << 16) | ((unsigned)fb << 24);
+                it[1] = ((unsigned)bs[1] & 0xffu) | (((unsigned)bs[2] & 0xffu) << 8) | (((unsigned)bs[3] & 0xffu) << 16) | (S << 24);
+                it[2] = 4u | ((unsigned)cnt[1] << 4) | ((unsigned)cnt[2] << 8) | ((unsigned)cnt[3] << 12) | (hb << 16);
+                it[3] = 0u;
+                // window start of every step (column pair from fa & ~1 on): floor of the lowest first-tap row of the item's angles
+                // at each of the two columns, clamped into the tile
+                auto wstart = [&](float fk) {
+                    float l = 1e6f;
+#pragma unroll
+                    for (int x = 0; x < 4; ++x)
+                        if (S >> x & 1) l = fminf(l, fmaf(fk, stp[x], lo[x]));
+                    return (unsigned)min(max((int)floorf(l), 0), TILE - 8);
+                };
+                for (int w = 0; w < 8; ++w) {
+                    const float fk = (float)((fa & ~1) + 4 * w);
+                    it[4 + w] = wstart(fk) | (wstart(fk + 1.0f) << 8) | (wstart(fk + 2.0f) << 16) | (wstart(fk + 3.0f) << 24);
+                }
             };
             auto nibbles = [&](unsigned S) {                   // the angles of S on consecutive half blocks
                 unsigned hb = 0;
@@ -340,49 +357,37 @@ __global__ void __launch_bounds__(FM_THREADS, 1) k_forward_mma(const float *__re
     {
         const int2 cnt = a.counts[tile_id * 2 + pass];
         const int n_long = cnt.x, n_items = cnt.x + cnt.y, cap = pass ? a.cap1 : a.cap0;
-        const unsigned *slot = a.items + 3 * ((size_t)tile_id * (a.cap0 + a.cap1) + (pass ? a.cap0 : 0));
+        const unsigned *slot = a.items + FM_ITEMW * ((size_t)tile_id * (a.cap0 + a.cap1) + (pass ? a.cap0 : 0));
         // warps draw items from one counter; small problems split the list over the agroups CTAs of a tile (item u of CTA ag
         // is list entry u agroups + ag, which keeps long and short items on every CTA).  The next item is fetched while the
         // current one runs
-        auto fetch = [&](int &u, unsigned &w0, unsigned &w1, unsigned &w2) {
+        auto fetch = [&](int &u, uint4 &w, unsigned &q) {      // q: lane s (< 16) gets the window starts of step s
             int v = 0;
             if (lane == 0) v = atomicAdd(&s_next, 1);
             u = __shfl_sync(0xffffffffu, v, 0) * a.agroups + ag;
-            w0 = w1 = w2 = 0u;
+            w = make_uint4(0u, 0u, 0u, 0u);
+            q = 0u;
             if (u < n_items) {
-                const unsigned *it = slot + 3 * (size_t)(u < n_long ? u : cap - 1 - (u - n_long));
-                w0 = __ldg(it); w1 = __ldg(it + 1); w2 = __ldg(it + 2);
+                const unsigned *it = slot + FM_ITEMW * (size_t)(u < n_long ? u : cap - 1 - (u - n_long));
+                w = __ldg(reinterpret_cast<const uint4 *>(it));
+                q = __ldg(it + 4 + ((lane & 15) >> 1));
             }
         };
         int u, un;
-        unsigned w0, w1, w2, x0w, x1w, x2w;
-        fetch(u, w0, w1, w2);
-        for (; u < n_items; u = un, w0 = x0w, w1 = x1w, w2 = x2w) {
-            fetch(un, x0w, x1w, x2w);
+        uint4 wi, wn;
+        unsigned qi, qn;
+        fetch(u, wi, qi);
+        for (; u < n_items; u = un, wi = wn, qi = qn) {
+            fetch(un, wn, qn);
+            const unsigned w0 = wi.x, w1 = wi.y, w2 = wi.z;
             const FmGroup &R = s_grp[(w0 & 0xffffu) >> 4];
             const int ts = (int)(w0 & 15u) - 1, klo = (int)((w0 >> 16) & 0xffu), khi = (int)(w0 >> 24);
             const unsigned bspack = (w1 << 8) | ((unsigned)(4 * ts) & 0xffu);      // first bin of angle x: signed byte x
-            const unsigned used = w1 >> 24, hb = w2 >> 16;
-            // lowest first-tap row of each angle in use at column 0: the window lines
-            float wl[4], wst[4];
-#pragma unroll
-            for (int x = 0; x < 4; ++x) {
-                const int bsx = (int)(bspack << (24 - 8 * x)) >> 24, cx = (int)((w2 >> (4 * x)) & 15u);
-                const float inv = R.inv[x], y0 = ((float)bsx - R.delta[x]) * inv;
-                wl[x] = (used >> x & 1u) ? fminf(y0, fmaf((float)(max(cx, 1) - 1), inv, y0)) : 1e6f;
-                wst[x] = R.step[x];
-            }
-            // window start per column: floor of the lowest first-tap row, clamped into the tile.  They are the same for every
-            // lane, so lane s works out the pair of step s (columns kb + 2 s, kb + 2 s + 1) once per item and the loop fetches
-            // it with one shuffle
+            const unsigned hb = w2 >> 16;
+            // window start per column (the same for every lane): lane s holds the pair of step s (columns kb + 2 s, kb + 2 s + 1)
+            // from the item; the loop fetches it with one shuffle
             const int kb = klo & ~1;
-            int qpack;
-            {
-                const float fk = (float)(kb + 2 * lane), fk1 = fk + 1.0f;
-                const float la = fminf(fminf(fmaf(fk, wst[0], wl[0]), fmaf(fk, wst[1], wl[1])), fminf(fmaf(fk, wst[2], wl[2]), fmaf(fk, wst[3], wl[3])));
-                const float lb = fminf(fminf(fmaf(fk1, wst[0], wl[0]), fmaf(fk1, wst[1], wl[1])), fminf(fmaf(fk1, wst[2], wl[2]), fmaf(fk1, wst[3], wl[3])));
-                qpack = min(max((int)floorf(la), 0), TILE - 8) | (min(max((int)floorf(lb), 0), TILE - 8) << 8);
-            }
+            const int qpack = (int)((lane & 1) ? qi >> 16 : qi & 0xffffu);
             // my ray of column block nb (ray slot g): B column g of the weight block, and the ray whose sums I add to P in the
             // end.  Half block 2 nb + g / 4 names the angle; its slots hold consecutive bins
             int r_ang[2], r_bub[2];
@@ -580,7 +585,7 @@ static FmArgs fm_args(const cp4d_ctx *c) {
 // passes together are at most n0 / group size + 8 (a pass ends, the sign of 1/ss changes or the order jumps at most 8 times)
 uint64_t forward_mma_item_bytes(const Dims &d) {
     if (!forward_mma_supported(d)) return 0;
-    return (uint64_t)d.tiles * 4 * FM_STRIPS * (uint64_t)(d.n0 / fm_group_size(d.n0) + 8) * 12;
+    return (uint64_t)d.tiles * 4 * FM_STRIPS * (uint64_t)(d.n0 / fm_group_size(d.n0) + 8) * (FM_ITEMW * 4);
 }
 
 // the tensor kernel can run in this context: supported shape, the group records of a pass fit its shared memory, and the

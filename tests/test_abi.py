@@ -42,11 +42,11 @@ def test_workspace_bytes_counts_state(L):
         pitch = c.nd + pad + (1 if (c.nd + pad) % 8 == 0 else 0)
         scratch = c.nz * c.n_theta0 * pitch * c.m * 4          # folded sinogram of the adjoint (zero-padded rows)
         scratch += c.nz * c.n_theta0 * c.nd * c.m * 4          # partial ray sums of the forward projector (no padding)
-        # work items of the tensor forward projector, built once per context: per 32 x 32 tile, 4 x 14 items of 12 bytes
+        # work items of the tensor forward projector, built once per context: per 32 x 32 tile, 4 x 14 items of 48 bytes
         # for each of at most n_theta0 / 4 + 8 angle groups (groups of four from 72 base angles on, pairs from 24)
         gs = 4 if c.n_theta0 >= 72 else 2 if c.n_theta0 >= 24 else 1
         tiles = ((c.n + 31) // 32) ** 2
-        scratch += tiles * 4 * 14 * (c.n_theta0 // gs + 8) * 12
+        scratch += tiles * 4 * 14 * (c.n_theta0 // gs + 8) * 48
         assert state + scratch <= nb <= state + scratch + (64 << 20)
     c = synth.CONFIGS[5]
     assert binding.workspace_bytes(c.n, c.nz, c.nd, c.n_angles, c.n_half_rot, c.m) < 170e9   # fits 180 GB HBM
