@@ -66,7 +66,8 @@ struct cp4d_ctx {
     float *cf, *cb, *psi;      // frame mode: coefficient stacks (analysis output, backprojection output), Psi[j][q] = phi_j(t_q)
     float4 *scratch;           // folded sinogram gt of the adjoint: [z][i][jc][gpl + b] float4, pitch gp; the pads stay ZERO (nothing
                                // else may write here), so every tile window of the backprojector is readable and reads 0 off the detector
-    float4 *psum;              // forward partial ray sums P[z][i][b][j], j fastest, no padding: zeroed before, RED'ed by the projector
+    float4 *psum;              // forward partial ray sums P[z][i][b][j] (without the 1/a of the base angle, which k_synth applies),
+                               // j fastest, no padding: zeroed before, RED'ed by the projector
     float *phi;                // [j][k]
     cp4d::AngleTab *ang;       // [n0]
     cp4d::FwAngle *fwang;      // [n0]

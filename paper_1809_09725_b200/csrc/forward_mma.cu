@@ -67,13 +67,13 @@ struct FmArgs {
 // per-CTA record of one angle group (shared memory): the per-angle tables and this tile's window geometry, plus what the
 // strip bookkeeping needs, so that an item's setup is a handful of FMAs.  Absent angles repeat angle 0 with ia = -1.
 struct FmGroup {
-    float inv[4], step[4], delta[4], inva[4];   // 1/ss, -cc/ss, window offset of the tile, 1/a
+    float inv[4], step[4], delta[4];            // 1/ss, -cc/ss, window offset of the tile
     float istep[4];                             // 1/step (0 when the rays run along the columns)
     float r0[4], rinv[4];                       // bin ub of angle x sits, at the reference column, at angle-0 bin coordinate
                                                 // ub / rinv[x] + r0[x]
     int ia[4], bstart[4];
 };
-constexpr int FM_MAXG = 128;                           // angle groups of a pass whose records a CTA keeps in shared memory (18 KB)
+constexpr int FM_MAXG = 128;                           // angle groups of a pass whose records a CTA keeps in shared memory (16 KB)
 constexpr int FM_BUILDG = 32;                          // groups per round of the item builder
 constexpr int FM_ITEMW = 12;                           // 32-bit words per work item
 constexpr int FM_LONG = 14;                            // columns from which an item counts as long
@@ -111,7 +111,7 @@ __device__ __forceinline__ void fm_group_record(const FmArgs &a, const TileGeo *
         const int i = idx[x] >= 0 ? idx[x] : gr.x;
         const FwAngle A = a.fwang[i];
         const TileGeo G = geo[i];
-        R.inv[x] = A.inv; R.step[x] = A.step; R.delta[x] = G.delta; R.inva[x] = A.inv_a;
+        R.inv[x] = A.inv; R.step[x] = A.step; R.delta[x] = G.delta;
         R.istep[x] = fabsf(A.step) > 1e-6f ? 1.0f / A.step : 0.0f;
         // ray ub of angle x sits, at the reference column, at angle-0 bin coordinate phi = ub inv_x / inv_0 + r0
         R.r0[x] = (FM_KC * (A.step - A0.step) - G.delta * A.inv) / A0.inv + G0.delta;
@@ -410,13 +410,11 @@ __global__ void __launch_bounds__(FM_THREADS, 1) k_forward_mma(const float *__re
             // costs about one clock per LANE whatever its width, so a block goes through a per-warp shared-memory patch and
             // leaves as one 16-byte RED per lane: lane (ray g, quad t) adds entries 4t .. 4t+3 of ray g ----
             unsigned r_off[2];       // element offset of (angle, bin) of my ray in a slice of P
-            float r_sc[2];
 #pragma unroll
             for (int nb = 0; nb < 2; ++nb) {
                 const int x = r_ang[nb], b = R.bstart[x] + r_bub[nb];
                 r_ok[nb] = r_ok[nb] && b >= 0 && b < a.nd;
                 r_off[nb] = (unsigned)((R.ia[x] * a.gp + a.gpl + b) * a.m);
-                r_sc[nb] = R.inva[x];
             }
             auto flush = [&](const float (&acc)[4], int zb, int nb) {
                 __syncwarp();
@@ -426,9 +424,7 @@ __global__ void __launch_bounds__(FM_THREADS, 1) k_forward_mma(const float *__re
                 stg[(2 * t + 1) * FM_STG + g + 8] = acc[3];
                 __syncwarp();
                 const float4 v = *reinterpret_cast<const float4 *>(stg + g * FM_STG + 4 * t);
-                const float sc = r_sc[nb];
-                if (r_ok[nb] && zok[zb])
-                    atomicAdd(reinterpret_cast<float4 *>(P + (size_t)zoff[zb] + r_off[nb]), make_float4(v.x * sc, v.y * sc, v.z * sc, v.w * sc));
+                if (r_ok[nb] && zok[zb]) atomicAdd(reinterpret_cast<float4 *>(P + (size_t)zoff[zb] + r_off[nb]), v);      // 1/a: k_synth
             };
 
             if (hb >> 8) {

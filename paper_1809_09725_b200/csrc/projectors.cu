@@ -148,7 +148,7 @@ __global__ void __launch_bounds__(FR_THREADS, 3) k_forward_rays(const float *__r
             const int b = G.bstart + u;
             if (touched && b >= 0 && b < a.nd && z < a.nz) {
                 float2 *dst = reinterpret_cast<float2 *>(P + ((((int64_t)z * a.n0 + i) * a.gp + a.gpl + b) * a.Q + jg * JQ + jc) * 4) + sp;
-                atomicAdd(dst, make_float2(tot.x * A.inv_a, tot.y * A.inv_a));
+                atomicAdd(dst, make_float2(tot.x, tot.y));          // 1/a is applied by k_synth
             }
         }
     }

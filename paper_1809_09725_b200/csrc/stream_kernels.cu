@@ -370,11 +370,14 @@ __global__ void __launch_bounds__(128) k_fold(const float *__restrict__ g, float
 template <int Q>
 __global__ void __launch_bounds__(128) k_synth(const float4 *__restrict__ P, int mode, float sigma,
                                                const float *__restrict__ g, float *__restrict__ out,
-                                               const float *__restrict__ phi, int nd, int na, int npi, int n0, int gp, int gpl) {
+                                               const float *__restrict__ phi, const FwAngle *__restrict__ fwang, int nd, int na, int npi,
+                                               int n0, int gp, int gpl) {
     extern __shared__ float phis[];
     const int z = blockIdx.x / n0, i = blockIdx.x % n0;
     constexpr int m = 4 * Q;
-    for (int t = threadIdx.x; t < npi * m; t += blockDim.x) phis[t] = phi[(int64_t)(t % m) * na + (t / m) * n0 + i];
+    // the projectors leave P without the Joseph normalisation 1/max(|c|,|s|) of its base angle: it is folded into Phi here
+    const float inv_a = fwang[i].inv_a;
+    for (int t = threadIdx.x; t < npi * m; t += blockDim.x) phis[t] = phi[(int64_t)(t % m) * na + (t / m) * n0 + i] * inv_a;
     __syncthreads();
     const float rs = 1.0f / (1.0f + sigma);
     for (int b = threadIdx.x; b < nd; b += blockDim.x) {
@@ -430,7 +433,7 @@ cudaError_t launch_synth(cp4d_ctx *c, const float4 *P, int mode, float sigma, co
     ProfScope ps(c, CP4D_K_SYNTH);
     const Dims &d = c->d;
     const size_t sh = (size_t)d.npi * d.m * sizeof(float);
-    CP4D_DISPATCH_Q(d.Q, (k_synth<QQ><<<d.nz * d.n0, 128, sh, c->stream>>>(P, mode, sigma, g, out, c->phi, d.nd, d.na, d.npi, d.n0, d.nd, 0)));
+    CP4D_DISPATCH_Q(d.Q, (k_synth<QQ><<<d.nz * d.n0, 128, sh, c->stream>>>(P, mode, sigma, g, out, c->phi, c->fwang, d.nd, d.na, d.npi, d.n0, d.nd, 0)));
     c->launches++;
     return cudaGetLastError();
 }
