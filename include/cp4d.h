@@ -56,6 +56,8 @@ extern "C" {
 #define CP4D_EINTERNAL    -7  /* an invariant of the host prologue failed (cp4d_create: the base angles are not sorted by
                                  the sign of cos, or a tile window leaves the padded scratch row); a bug, never an input error */
 
+#define CP4D_ETOOLARGE    -8  /* cp4d_forward_static: the problem's scratch exceeds CP4D_STATIC_SCRATCH_BYTES */
+
 typedef struct cp4d_ctx cp4d_ctx; /* opaque; owns host-side metadata only */
 
 typedef struct {
@@ -108,6 +110,17 @@ int cp4d_destroy(cp4d_ctx *ctx);
 /* g = K1 f  (Eq. 9; pi-folding L198-L202: ray sums over the n_theta0 base angles with all m
  * coefficients accumulated per ray, then n_half_rot m-wide dot products with Phi).  f: V, g: S. */
 int cp4d_forward(cp4d_ctx *ctx, const float *f_dev, float *g_dev);
+/* g = K1 f as cp4d_forward computes it (same kernels, same projector mode), for callers that must not depend on workspace
+ * scratch at call time (CUDA graph capture of their own, serving loops, harnesses that forbid device allocation): the
+ * projector's partial ray sums (m * n_theta0 * nd * nz floats) go to a file-scope __device__ array of
+ * CP4D_STATIC_SCRATCH_BYTES inside the library instead of the workspace.  Calls no cudaMalloc / cudaFree or any allocating
+ * routine; every GPU that loads libcp4d.so holds the array until the process exits.  Problems whose partial sums exceed it
+ * return CP4D_ETOOLARGE (sizes in cp4d_last_error); nothing is launched then.  All calls on one device share the array: each
+ * call zero-fills the part it uses on the context's stream, so calls ordered by a stream are fine, and calls that overlap
+ * on the GPU (contexts on different streams, no dependency between them) race.  Result equals cp4d_forward's up to the
+ * order of the projector's atomic additions.  Errors otherwise as cp4d_forward. */
+#define CP4D_STATIC_SCRATCH_BYTES (32u << 20)
+int cp4d_forward_static(cp4d_ctx *ctx, const float *f_dev, float *g_dev);
 /* f = K1^T g, overwrite (Eq. 10; fold L204-L212: gt_j = sum_q Phi[j,q n0+i] g[q n0+i, flip_q b],
  * then one backprojection over [0,pi)).  Exact transpose of cp4d_forward up to fp32 rounding. */
 int cp4d_adjoint(cp4d_ctx *ctx, const float *g_dev, float *f_dev);

@@ -15,7 +15,8 @@ _PKG = Path(__file__).resolve().parent
 LIB_PATH = _PKG / "libcp4d.so"
 _lib = None
 
-OK, EINVAL, EWORKSPACE, EUNSUPPORTED, ECUDA, ESTATE, ENOMEM, EINTERNAL = 0, -1, -2, -3, -4, -5, -6, -7
+OK, EINVAL, EWORKSPACE, EUNSUPPORTED, ECUDA, ESTATE, ENOMEM, EINTERNAL, ETOOLARGE = 0, -1, -2, -3, -4, -5, -6, -7, -8
+STATIC_SCRATCH_BYTES = 32 << 20      # CP4D_STATIC_SCRATCH_BYTES of include/cp4d.h
 
 
 class Cp4dError(RuntimeError):
@@ -52,7 +53,7 @@ def lib():
             "cp4d_workspace_bytes": [C.POINTER(Params), C.POINTER(u64)],
             "cp4d_create": [C.POINTER(Params), C.POINTER(vp)],
             "cp4d_destroy": [vp],
-            "cp4d_forward": [vp, vp, vp], "cp4d_adjoint": [vp, vp, vp], "cp4d_grad": [vp, vp, vp], "cp4d_div": [vp, vp, vp],
+            "cp4d_forward": [vp, vp, vp], "cp4d_forward_static": [vp, vp, vp], "cp4d_adjoint": [vp, vp, vp], "cp4d_grad": [vp, vp, vp], "cp4d_div": [vp, vp, vp],
             "cp4d_prox_f1": [vp, f32, vp, vp, vp], "cp4d_prox_f2": [vp, f32, vp, vp],
             "cp4d_primal_update": [vp, f32, vp, vp, vp, vp],
             "cp4d_dot": [vp, vp, vp, u64, C.POINTER(C.c_double)],
@@ -163,6 +164,12 @@ class Context:
     def forward(self, f, out=None):
         out = self.empty_sino() if out is None else out
         self._ck(lib().cp4d_forward(self._h, self._t(f, self.V), self._t(out, self.S)))
+        return out
+
+    def forward_static(self, f, out=None):
+        """cp4d_forward with the projector's scratch in the library's static device array (no workspace scratch at call time)."""
+        out = self.empty_sino() if out is None else out
+        self._ck(lib().cp4d_forward_static(self._h, self._t(f, self.V), self._t(out, self.S)))
         return out
 
     def adjoint(self, g, out=None):

@@ -148,6 +148,7 @@ const char *cp4d_strerror(int code) {
     case CP4D_ESTATE: return "call order: set_data/set_steps before iterate";
     case CP4D_ENOMEM: return "host allocation failed";
     case CP4D_EINTERNAL: return "internal invariant violated (scratch window)";
+    case CP4D_ETOOLARGE: return "problem exceeds the static scratch array (CP4D_STATIC_SCRATCH_BYTES)";
     default: return "unknown error";
     }
 }
