@@ -64,6 +64,25 @@ def test_forward_static_matches_forward_twice(torch_cuda, oracle, mode):
         ctx.close()
 
 
+@pytest.mark.parametrize("nt", [8, 4])
+def test_forward_static_in_frame_mode(torch_cuda, nt):
+    """Frame mode: N_t = 8 > M = 4 keeps the analysis step in front of the projector (cp4d_forward_static runs it too);
+    N_t = 4 <= M collapses to a coefficient-mode problem.  Against cp4d_forward, two calls in a row."""
+    torch = torch_cuda
+    from paper_1809_09725_b200 import binding
+    c = synth.CONFIGS[2].scaled(cfg=33, n=50, nd=61, nz=3, n_angles=96, n_half_rot=2, m=4)
+    phi = synth.basis_table(c.basis, c.m, c.n_angles)
+    ctx = binding.Context.from_config(c, phi=phi, n_frames=nt)
+    try:
+        f1, f2 = ctx.empty_primal().normal_(), ctx.empty_primal().normal_()
+        want1, want2 = ctx.forward(f1).cpu().numpy(), ctx.forward(f2).cpu().numpy()
+        got1, got2 = ctx.forward_static(f1).cpu().numpy(), ctx.forward_static(f2).cpu().numpy()
+        assert rel(got1, want1) <= TOL_SAME and rel(got2, want2) <= TOL_SAME
+        assert rel(want1, want2) > 0.5
+    finally:
+        ctx.close()
+
+
 def test_forward_static_refuses_what_does_not_fit(torch_cuda):
     torch = torch_cuda
     from paper_1809_09725_b200 import binding
