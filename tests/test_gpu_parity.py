@@ -100,6 +100,23 @@ def test_forward_adjoint(torch_cuda, fast_oracle, case):
     ctx.close()
 
 
+def test_tensor_request_falls_back_beyond_its_tables(torch_cuda, fast_oracle):
+    """More than 128 angle groups in a pass (here 1100 base angles in groups of four: about 138 per pass) do not fit the tensor
+    forward kernel's shared-memory records: a CP4D_PROJ_TENSOR request then runs the fp32 kernels, says so, and is still right."""
+    from paper_1809_09725_b200 import binding
+    c = synth.CONFIGS[1].scaled(cfg=28, n=24, nd=29, nz=1, n_angles=1100, n_half_rot=1, m=4)
+    phi = synth.basis_table(c.basis, c.m, c.n_angles)
+    P = fast_oracle.Problem.from_config(c, phi=phi)
+    ctx = binding.Context.from_config(c, phi=phi)
+    f, g = synth.test_vectors(c)
+    f32, g32 = f.astype(np.float32), g.astype(np.float32)
+    ctx.set_projector_mode("tensor")
+    assert ctx.projector_mode_in_use() == ("fp32", "fp32")
+    assert rel(ctx.forward(dev(torch_cuda, f32)).cpu().numpy(), P.forward(f32.astype(np.float64), folded=True)) <= 1e-5
+    assert rel(ctx.adjoint(dev(torch_cuda, g32)).cpu().numpy(), P.adjoint(g32.astype(np.float64), folded=True)) <= 1e-5
+    ctx.close()
+
+
 @pytest.mark.parametrize("case", list(CASES))
 def test_grad_div(torch_cuda, fast_oracle, case):
     c, P, ctx = make(case, fast_oracle)
