@@ -12,6 +12,18 @@ __device__ __forceinline__ void mma16816(float (&d)[4], const unsigned (&a)[4], 
                  : "+f"(d[0]), "+f"(d[1]), "+f"(d[2]), "+f"(d[3])
                  : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(b0), "r"(b1));
 }
+// D[16 x 8] += A[16 x 32] * B[32 x 8] with A 2:4 sparse along K (two kept elements per group of four, as a 16 x 16 compressed
+// matrix in the layout of the dense m16n8k16 A fragment; SASS HMMA.SP.16832.F32.BF16).  Metadata e (selector 0): lane 4g holds
+// the 2-bit positions of row g's compressed elements 0..7 in its low half and of row g + 8's in its high half, lane 4g + 1 the
+// same for the compressed elements 8..15 (element c at bits 2c; positions of a group in ascending order); lanes 4g + 2, 4g + 3
+// are not read.  Measured on B200 (profiles/r2_microbench.md): 9.7 clk per instruction and sub-partition against 8.7 for the dense
+// m16n8k16, i.e. 1.8 x the products per clock.
+__device__ __forceinline__ void mma_sp16832(float (&d)[4], const unsigned (&a)[4], const unsigned (&b)[4], unsigned e) {
+    asm volatile("mma.sp::ordered_metadata.sync.aligned.m16n8k32.row.col.f32.bf16.bf16.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9,%10,%11}, "
+                 "{%0,%1,%2,%3}, %12, 0x0;\n"
+                 : "+f"(d[0]), "+f"(d[1]), "+f"(d[2]), "+f"(d[3])
+                 : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(b[0]), "r"(b[1]), "r"(b[2]), "r"(b[3]), "r"(e));
+}
 // four 8 x 8 b16 matrices, transposed on the way: lane l gives the row address of matrix l / 8, row l % 8 (SASS LDSM.16.MT88.4)
 __device__ __forceinline__ void ldsm4t(unsigned (&a)[4], unsigned addr) {
     asm volatile("ldmatrix.sync.aligned.m8n8.x4.trans.shared.b16 {%0,%1,%2,%3}, [%4];\n"

@@ -1,29 +1,31 @@
 // Forward projector on the tensor cores (Eq. 9, with the pi-fold of L198-L202): the Joseph ray sums of all
-// coefficients over the base angles, as small dense products  D[16 batch entries x 8 rays] += F[16 x 16 voxels] * W[16 voxels x 8 rays].
+// coefficients over the base angles, as small products  D[16 rays x 8 batch entries] += W[16 rays x 32 voxels] * F[32 voxels x 8]
+// with the weight block W as the 2:4 SPARSE operand of mma.sp (SASS HMMA.SP.16832).
 //
 // Why.  The CUDA-core gather (projectors.cu) needs one shared-memory word per FMA and sits on the LSU data pipe at 0.19 of
 // the FP32 peak.  The interpolation weights do not depend on the slice or on the coefficient, so the batch axis (slice, j) is
-// a dense axis: a block of 16 voxels along a short column segment times the 2-nonzeros-per-ray weight block is a real matrix
-// product.  mma.sync (HMMA.16816) measured 950 MAC/clk/SM on B200, 7.4x the FP32 FMA rate, and it does not touch the LSU pipe
-// beyond one ldmatrix per 16 x 16 operand -- so a weight block that is 1/4 dense still wins.
+// a dense axis: a block of voxels along short column segments times the 2-nonzeros-per-ray-and-column weight block is a real
+// matrix product.  A ray's two taps in a column are in adjacent rows, so every group of four consecutive rows of a column
+// holds at most two of them: exactly the 2:4 structure the sparse MMA skips, which runs 32 voxels per instruction at 9.7 clk
+// against 16 voxels at 8.7 clk for the dense mma.sync (measured, profiles/r2_microbench.md).
 //
-// Block shape.  K = 16 voxels = 2 adjacent columns (of the stepping axis) x 8 consecutive rows; N = 8 rays = 4 adjacent bins of
-// each of TWO adjacent base angles (a "strip pair"); M = 16 batch entries = (slices x coefficients) of one voxel.  Four bins of
-// one angle span at most 3*sqrt2 + 2 rows at a column, and the rays of the neighbouring angle that lie in the same strip of the
-// detector stay within one more row of them, so an 8-row window per column holds every tap: 32 of the 128 weights are
-// non-zero.  Windows are clamped to the tile, so taps outside the tile (which belong to other tiles) simply have no row.
-// When the two angles are too far apart for one window (coarse angular sampling), or the pairing leaves five bins of the
-// second angle in a strip, the unit is processed as two single-angle units -- a warp-uniform decision, never a wrong result.
+// Block shape.  K = 32 voxels = 4 adjacent columns (of the stepping axis) x an 8-row window each; M = 16 rays = 4 adjacent
+// bins of each of up to FOUR adjacent base angles (a "strip" of an angle group); N = 8 batch entries = half a 16-entry block of
+// (slice, coefficient).  Four bins of one angle span at most 3*sqrt2 + 2 rows at a column, and the rays of the neighbouring
+// angles that lie in the same strip of the detector stay within the 8-row window: 64 of the 512 weights are non-zero, 256 are
+// stored.  Windows are clamped to the tile, so taps outside the tile (which belong to other tiles) simply have no row.
+// When the angles of a group are too far apart for one window (coarse angular sampling), or the grouping leaves five bins of
+// an angle in a strip, the item falls apart into pairs or single angles -- decided by the item builder, never a wrong result.
 //
 // Precision.  Operands are split bf16 pairs: F = Fh + Fl (tile, once per CTA), W = Wh + Wl (per weight), and
-// D += Fh Wh + Fl Wh + Fh Wl with fp32 accumulation: relative error about 3 * 2^-18 = 1.1e-5 per product, inside the 1e-4
-// per-operator tolerance.  cp4d_set_forward_mode selects the exact-fp32 gather instead.
+// D += Wh Fh + Wh Fl + Wl Fh with fp32 accumulation: relative error about 3 * 2^-18 = 1.1e-5 per product, inside the 1e-4
+// per-operator tolerance.  cp4d_set_projector_mode selects the exact-fp32 gather instead.
 //
 // Work split.  CTA = (32 x 32 tile, pass, group of NB16 16-entry batch blocks); pass 0 = base angles whose rays step over
 // columns, pass 1 = the others on the transposed tile, so one code path serves both.  The tile sits in shared memory as
-// [block][hi/lo][8-entry half][column][row] x 16 B, which makes every 8 x 8 ldmatrix operand 128 contiguous bytes.  Warps
-// draw units (angle pair, strip) from a shared counter; partial ray sums go to P[z][i][b][j] with scalar REDs (32-byte
-// runs of 8 coefficients per bin).
+// [block][hi/lo][8-entry half][column][33 rows] x 16 B, which makes every 8 x 8 ldmatrix operand 128 contiguous bytes.  The work
+// items (angle group, strip, column range, window starts) are built once per context by k_fm_build; warps draw them from a
+// shared counter; partial ray sums go to P[z][i][b][j] as one 16-byte RED per lane.
 #include <cuda_bf16.h>
 
 #include <algorithm>
@@ -38,14 +40,12 @@ namespace {
 
 static_assert(TILE == 32, "the tile staging decodes indices with shifts for TILE = 32");
 constexpr int FM_THREADS = 512;
-constexpr int FM_WARPS = FM_THREADS / 32;
 constexpr int FM_STRIPS = WIN / 4 + 2;                 // strips -1 .. WIN/4 of four window bins
 constexpr int FM_COL = (TILE + 1) * 16;                // bytes of one tile column: 32 rows x 16 B + 16 B of padding, so that the
                                                        // staging stores of one row across 8 columns hit 8 different bank groups
 constexpr int FM_PLANE = 2 * TILE * FM_COL;            // bytes of one (block, hi/lo) plane: [half][column][row] x 16 B
 constexpr float FM_KC = 0.5f * (TILE - 1);             // reference column where the two angles of a pair are aligned
 constexpr float FM_SPAN = 5.99f;                       // largest spread of first-tap rows an 8-row window holds
-constexpr int FM_STG = 20;                             // floats per ray of a warp's 8 x 16 epilogue patch (20: conflict-free stores)
 
 struct FmArgs {
     int n, nz, nd, n0, m, mshift, gp, gpl;
@@ -228,8 +228,8 @@ __global__ void __launch_bounds__(FM_THREADS, 1) k_fm_build(FmArgs a) {
                 it[1] = ((unsigned)bs[1] & 0xffu) | (((unsigned)bs[2] & 0xffu) << 8) | (((unsigned)bs[3] & 0xffu) << 16) | (S << 24);
                 it[2] = 4u | ((unsigned)cnt[1] << 4) | ((unsigned)cnt[2] << 8) | ((unsigned)cnt[3] << 12) | (hb << 16);
                 it[3] = 0u;
-                // window start of every step (column pair from fa & ~1 on): floor of the lowest first-tap row of the item's angles
-                // at each of the two columns, clamped into the tile
+                // window start of every step (four columns from fa & ~3 on): floor of the lowest first-tap row of the item's angles
+                // at each column, clamped into the tile
                 auto wstart = [&](float fk) {
                     float l = 1e6f;
 #pragma unroll
@@ -238,7 +238,7 @@ __global__ void __launch_bounds__(FM_THREADS, 1) k_fm_build(FmArgs a) {
                     return (unsigned)min(max((int)floorf(l), 0), TILE - 8);
                 };
                 for (int w = 0; w < 8; ++w) {
-                    const float fk = (float)((fa & ~1) + 4 * w);
+                    const float fk = (float)((fa & ~3) + 4 * w);
                     it[4 + w] = wstart(fk) | (wstart(fk + 1.0f) << 8) | (wstart(fk + 2.0f) << 16) | (wstart(fk + 3.0f) << 24);
                 }
             };
@@ -280,9 +280,7 @@ template <int NB16>
 __global__ void __launch_bounds__(FM_THREADS, 1) k_forward_mma(const float *__restrict__ f, float *__restrict__ P, FmArgs a) {
     extern __shared__ __align__(128) unsigned char tile[];     // [NB16][2][2][TILE][TILE + 1] x 16 B
     __shared__ int s_next;
-    __shared__ __align__(16) float s_stg[FM_WARPS][8 * FM_STG];
     __shared__ __align__(16) FmGroup s_grp[FM_MAXG];
-    float *stg = s_stg[threadIdx.x >> 5];
     const int tiles_1d = (a.n + TILE - 1) / TILE;
     const int tile_id = blockIdx.x % a.tiles, ag = blockIdx.x / a.tiles;
     const int pass = blockIdx.y & 1, z0 = a.z_base + (blockIdx.y >> 1) * a.zper;
@@ -332,19 +330,21 @@ __global__ void __launch_bounds__(FM_THREADS, 1) k_forward_mma(const float *__re
     const int pbeg = pass ? a.ngroups0 : 0, pcnt = pass ? a.ngroups1 : a.ngroups0;
     const int lane = threadIdx.x & 31, g = lane >> 2, t = lane & 3;
     const unsigned tile_s = (unsigned)__cvta_generic_to_shared(tile);
-    // ldmatrix row address of this lane: matrix = lane / 8 -> (column k0 + matrix / 2, half matrix & 1), row lane & 7
-    const unsigned ld_half = (lane >> 3) & 1, ld_col = lane >> 4, ld_row = lane & 7;
-    const unsigned ld_base = tile_s + (ld_half * TILE + ld_col) * FM_COL + (ld_row << 4);
+    // ldmatrix row address of this lane: matrix = lane / 8 = column of the step, row lane & 7 of its window
+    const unsigned ld_base = tile_s + (lane >> 3) * FM_COL + ((lane & 7) << 4);
     const TileGeo *geo = a.geo + (int64_t)tile_id * a.n0;
-    // epilogue: I add batch entries 4t .. 4t+3 of block zb = coefficients j .. j+3 of slice sl; element offset of (sl, j) in P
-    unsigned zoff[NB16];
-    bool zok[NB16];
+    // epilogue: I add batch entries 8 half + 4 (t / 2) .. + 3 of block zb = coefficients j .. j+3 of slice sl; element offset of
+    // (sl, j) in P
+    unsigned zoff[NB16][2];
+    bool zok[NB16][2];
 #pragma unroll
-    for (int zb = 0; zb < NB16; ++zb) {
-        const int flat = zb * 16 + 4 * t, sl = z0 + (flat >> a.mshift), j = flat & (a.m - 1);
-        zok[zb] = sl < a.nz;
-        zoff[zb] = (unsigned)sl * (unsigned)(a.n0 * a.gp) * (unsigned)a.m + (unsigned)j;
-    }
+    for (int zb = 0; zb < NB16; ++zb)
+#pragma unroll
+        for (int hf = 0; hf < 2; ++hf) {
+            const int flat = zb * 16 + hf * 8 + 4 * (t >> 1), sl = z0 + (flat >> a.mshift), j = flat & (a.m - 1);
+            zok[zb][hf] = sl < a.nz;
+            zoff[zb][hf] = (unsigned)sl * (unsigned)(a.n0 * a.gp) * (unsigned)a.m + (unsigned)j;
+        }
 
     // ---- the records of all angle groups of this pass for this tile; the item list of (tile, pass) ----
     if (threadIdx.x == 0) s_next = 0;
@@ -361,7 +361,7 @@ __global__ void __launch_bounds__(FM_THREADS, 1) k_forward_mma(const float *__re
         // warps draw items from one counter; small problems split the list over the agroups CTAs of a tile (item u of CTA ag
         // is list entry u agroups + ag, which keeps long and short items on every CTA).  The next item is fetched while the
         // current one runs
-        auto fetch = [&](int &u, uint4 &w, unsigned &q) {      // q: lane s (< 16) gets the window starts of step s
+        auto fetch = [&](int &u, uint4 &w, unsigned &q) {      // q: lane s (< 8) gets the window starts of step s (4 columns)
             int v = 0;
             if (lane == 0) v = atomicAdd(&s_next, 1);
             u = __shfl_sync(0xffffffffu, v, 0) * a.agroups + ag;
@@ -370,7 +370,7 @@ __global__ void __launch_bounds__(FM_THREADS, 1) k_forward_mma(const float *__re
             if (u < n_items) {
                 const unsigned *it = slot + FM_ITEMW * (size_t)(u < n_long ? u : cap - 1 - (u - n_long));
                 w = __ldg(reinterpret_cast<const uint4 *>(it));
-                q = __ldg(it + 4 + ((lane & 15) >> 1));
+                q = __ldg(it + 4 + (lane & 7));
             }
         };
         int u, un;
@@ -384,119 +384,95 @@ __global__ void __launch_bounds__(FM_THREADS, 1) k_forward_mma(const float *__re
             const int ts = (int)(w0 & 15u) - 1, klo = (int)((w0 >> 16) & 0xffu), khi = (int)(w0 >> 24);
             const unsigned bspack = (w1 << 8) | ((unsigned)(4 * ts) & 0xffu);      // first bin of angle x: signed byte x
             const unsigned hb = w2 >> 16;
-            // window start per column (the same for every lane): lane s holds the pair of step s (columns kb + 2 s, kb + 2 s + 1)
-            // from the item; the loop fetches it with one shuffle
-            const int kb = klo & ~1;
-            const int qpack = (int)((lane & 1) ? qi >> 16 : qi & 0xffffu);
-            // my ray of column block nb (ray slot g): B column g of the weight block, and the ray whose sums I add to P in the
-            // end.  Half block 2 nb + g / 4 names the angle; its slots hold consecutive bins
-            int r_ang[2], r_bub[2];
+            // window start per column (the same for every lane): lane s holds the four bytes of step s (columns kb + 4 s .. + 3)
+            // from the item; the loop fetches them with one shuffle
+            const int kb = klo & ~3;
+            const int nstep = ((khi - kb) >> 2) + 1;
+            // The weight block is the sparse operand: A[16 rays x 32 voxels], voxel k = 8 c + r = row r of the 8-row window of
+            // column c of the step; a ray has its two taps in adjacent rows, so every group of four rows holds at most two of
+            // them (2:4).  Lane (g, t) computes, for rays g (slot g, "nb 0") and g + 8 ("nb 1"), the two kept elements of group t
+            // (column t / 2, rows 4 (t & 1) .. + 3) and of group t + 4 (column 2 + t / 2, same rows).  Half block 2 nb + g / 4 of
+            // the item names a ray's angle; its slots hold consecutive bins.
+            int r_bub[2], r_x[2];
             bool r_ok[2];
-            float r_step[2], r_y[2];       // first-tap row at column 0, relative to row 2t (the rows of my B entries: 2t, 2t+1)
+            float r_step[2], r_y[2];       // first-tap row at column kb + t / 2, relative to the first row of my row half
 #pragma unroll
             for (int nb = 0; nb < 2; ++nb) {
                 const unsigned d = (hb >> (4 * (2 * nb + (g >> 2)))) & 15u;
                 const int x = (int)(d & 3u), off = (int)(d & 4u) + (g & 3);
                 const int bsx = (int)(bspack << (24 - 8 * x)) >> 24, cx = (int)((w2 >> (4 * x)) & 15u);
-                r_ang[nb] = x;
+                r_x[nb] = x;
                 r_bub[nb] = bsx + off;
                 r_ok[nb] = (d & 8u) && off < cx && r_bub[nb] >= 0 && r_bub[nb] < WIN;
                 r_step[nb] = R.step[x];
-                r_y[nb] = r_ok[nb] ? ((float)r_bub[nb] - R.delta[x]) * R.inv[x] - (float)(2 * t) : -1e6f;
+                r_y[nb] = r_ok[nb] ? fmaf((float)(kb + (t >> 1)), r_step[nb], ((float)r_bub[nb] - R.delta[x]) * R.inv[x]) - (float)(4 * (t & 1)) : -1e6f;
             }
-            const int nstep = ((khi - kb) >> 1) + 1;
+            // ---- partial ray sums of this tile -> P[z][i][b][j]: an even lane adds four batch entries of ray g, an odd lane of
+            // ray g + 8 (see the epilogue) ----
+            const int mynb = t & 1;
+            const int myx = mynb ? r_x[1] : r_x[0], mybub = mynb ? r_bub[1] : r_bub[0];
+            const int myb = R.bstart[myx] + mybub;
+            const bool my_ok = (mynb ? r_ok[1] : r_ok[0]) && myb >= 0 && myb < a.nd;
+            const unsigned my_off = (unsigned)((R.ia[myx] * a.gp + a.gpl + myb) * a.m);
 
-            // ---- partial ray sums of this tile -> P[z][i][b][j].  My D entries are rays 2t, 2t+1 x batch entries g, g+8; a RED
-            // costs about one clock per LANE whatever its width, so a block goes through a per-warp shared-memory patch and
-            // leaves as one 16-byte RED per lane: lane (ray g, quad t) adds entries 4t .. 4t+3 of ray g ----
-            unsigned r_off[2];       // element offset of (angle, bin) of my ray in a slice of P
+            float acc[NB16][2][4];         // [batch block][8-entry half]: rays g (0, 1) and g + 8 (2, 3) x batch entries 2t, 2t + 1
 #pragma unroll
-            for (int nb = 0; nb < 2; ++nb) {
-                const int x = r_ang[nb], b = R.bstart[x] + r_bub[nb];
-                r_ok[nb] = r_ok[nb] && b >= 0 && b < a.nd;
-                r_off[nb] = (unsigned)((R.ia[x] * a.gp + a.gpl + b) * a.m);
-            }
-            auto flush = [&](const float (&acc)[4], int zb, int nb) {
-                __syncwarp();
-                stg[(2 * t) * FM_STG + g] = acc[0];
-                stg[(2 * t + 1) * FM_STG + g] = acc[1];
-                stg[(2 * t) * FM_STG + g + 8] = acc[2];
-                stg[(2 * t + 1) * FM_STG + g + 8] = acc[3];
-                __syncwarp();
-                const float4 v = *reinterpret_cast<const float4 *>(stg + g * FM_STG + 4 * t);
-                if (r_ok[nb] && zok[zb]) atomicAdd(reinterpret_cast<float4 *>(P + (size_t)zoff[zb] + r_off[nb]), v);      // 1/a: k_synth
-            };
+            for (int zb = 0; zb < NB16; ++zb)
+#pragma unroll
+                for (int hf = 0; hf < 2; ++hf) acc[zb][hf][0] = acc[zb][hf][1] = acc[zb][hf][2] = acc[zb][hf][3] = 0.f;
 
-            if (hb >> 8) {
-                // ---- three or four angles: 16 rays per voxel fragment ----
-                float acc[NB16][2][4];
+            const unsigned qsel = 0x4440u + (unsigned)(t >> 1), qsel2 = qsel + 2u;       // byte t / 2 (resp. 2 + t / 2) of the step's word
+            const unsigned msel = 0x4440u + (lane >> 3);                                  // byte of my ldmatrix column
+            unsigned adr_k = ld_base + (unsigned)kb * FM_COL;
+            float ys[2][2] = {{r_y[0], fmaf(2.0f, r_step[0], r_y[0])}, {r_y[1], fmaf(2.0f, r_step[1], r_y[1])}};   // [nb][column]
+            const float st4[2] = {4.0f * r_step[0], 4.0f * r_step[1]};
+            for (int st = 0; st < nstep; ++st, adr_k += 4 * FM_COL) {
+                const unsigned qw = __shfl_sync(0xffffffffu, qi, st);
+                const float fq[2] = {(float)__byte_perm(qw, 0u, qsel), (float)__byte_perm(qw, 0u, qsel2)};
+                unsigned ah[4], al[4], nib[4];
+#pragma unroll
+                for (int cc = 0; cc < 2; ++cc)
+#pragma unroll
+                    for (int nb = 0; nb < 2; ++nb) {
+                        // row of the first tap relative to my row half; the kept pair starts at row i0 = clamp(floor(z), 0, 2)
+                        const float z = ys[nb][cc] - fq[cc];
+                        const bool p1 = z >= 1.0f, p2 = z >= 2.0f;
+                        const float dd = z - (p2 ? 2.0f : p1 ? 1.0f : 0.0f);
+                        nib[2 * cc + nb] = p2 ? 14u : p1 ? 9u : 4u;                       // positions (i0, i0 + 1), two bits each
+                        split2(__saturatef(1.0f - fabsf(dd)), __saturatef(1.0f - fabsf(dd - 1.0f)), ah[2 * cc + nb], al[2 * cc + nb]);
+                        ys[nb][cc] += st4[nb];
+                    }
+                // metadata: lane 4g wants the groups 0-3 (low half: ray g, high half: ray g + 8), lane 4g + 1 the groups 4-7
+                // (a butterfly over the quad: first the lanes two apart, then lanes 0 and 1 hand each other what the other needs)
+                unsigned e0 = (nib[0] | (nib[1] << 16)) << (4 * t), e1 = (nib[2] | (nib[3] << 16)) << (4 * t);
+                e0 |= __shfl_xor_sync(0xffffffffu, e0, 2);
+                e1 |= __shfl_xor_sync(0xffffffffu, e1, 2);
+                const unsigned e = ((t & 1) ? e1 : e0) | __shfl_xor_sync(0xffffffffu, (t & 1) ? e0 : e1, 1);
+                const unsigned adr = adr_k + (__byte_perm(qw, 0u, msel) << 4);
 #pragma unroll
                 for (int zb = 0; zb < NB16; ++zb)
 #pragma unroll
-                    for (int nb = 0; nb < 2; ++nb) acc[zb][nb][0] = acc[zb][nb][1] = acc[zb][nb][2] = acc[zb][nb][3] = 0.f;
-                const float ya0 = r_y[0], yb0 = r_y[0] + r_step[0], ya1 = r_y[1], yb1 = r_y[1] + r_step[1];
-                float fk = (float)kb;
-                unsigned adr_k = ld_base + (unsigned)kb * FM_COL;
-                for (int st = 0; st < nstep; ++st, fk += 2.0f, adr_k += 2 * FM_COL) {
-                    const int qp = __shfl_sync(0xffffffffu, qpack, st);
-                    const int qa = qp & 0xff, qb = qp >> 8;
-                    const float fqa = (float)qa, fqb = (float)qb;
-                    // weights of my rays at rows q + 2t, q + 2t + 1 of both columns: Joseph hat max(0, 1 - |row - y|)
-                    unsigned bh[2][2], bl[2][2];
-#pragma unroll
-                    for (int nb = 0; nb < 2; ++nb) {
-                        const float da = fmaf(fk, r_step[nb], nb ? ya1 : ya0) - fqa, db = fmaf(fk, r_step[nb], nb ? yb1 : yb0) - fqb;
-                        split2(__saturatef(1.0f - fabsf(da)), __saturatef(1.0f - fabsf(da - 1.0f)), bh[nb][0], bl[nb][0]);
-                        split2(__saturatef(1.0f - fabsf(db)), __saturatef(1.0f - fabsf(db - 1.0f)), bh[nb][1], bl[nb][1]);
+                    for (int hf = 0; hf < 2; ++hf) {
+                        unsigned bh[4], bl[4];
+                        ldsm4t(bh, adr + zb * 2 * FM_PLANE + hf * (TILE * FM_COL));
+                        ldsm4t(bl, adr + zb * 2 * FM_PLANE + FM_PLANE + hf * (TILE * FM_COL));
+                        mma_sp16832(acc[zb][hf], ah, bh, e);
+                        mma_sp16832(acc[zb][hf], ah, bl, e);
+                        mma_sp16832(acc[zb][hf], al, bh, e);
                     }
-                    const unsigned adr = adr_k + ((unsigned)(ld_col ? qb : qa) << 4);
-#pragma unroll
-                    for (int zb = 0; zb < NB16; ++zb) {
-                        unsigned ah[4], al[4];
-                        ldsm4t(ah, adr + zb * 2 * FM_PLANE);
-                        ldsm4t(al, adr + zb * 2 * FM_PLANE + FM_PLANE);
-#pragma unroll
-                        for (int nb = 0; nb < 2; ++nb) {
-                            mma16816(acc[zb][nb], ah, bh[nb][0], bh[nb][1]);
-                            mma16816(acc[zb][nb], al, bh[nb][0], bh[nb][1]);
-                            mma16816(acc[zb][nb], ah, bl[nb][0], bl[nb][1]);
-                        }
-                    }
-                }
-#pragma unroll
-                for (int zb = 0; zb < NB16; ++zb) {
-                    flush(acc[zb][0], zb, 0);
-                    flush(acc[zb][1], zb, 1);
-                }
-            } else {
-                // ---- one or two angles: 8 rays per voxel fragment ----
-                float acc[NB16][4];
-#pragma unroll
-                for (int zb = 0; zb < NB16; ++zb) acc[zb][0] = acc[zb][1] = acc[zb][2] = acc[zb][3] = 0.f;
-                const float bstep = r_step[0], ya = r_y[0], yb = r_y[0] + bstep;
-                float fk = (float)kb;
-                unsigned adr_k = ld_base + (unsigned)kb * FM_COL;
-                for (int st = 0; st < nstep; ++st, fk += 2.0f, adr_k += 2 * FM_COL) {
-                    const int qp = __shfl_sync(0xffffffffu, qpack, st);
-                    const int qa = qp & 0xff, qb = qp >> 8;
-                    const float da = fmaf(fk, bstep, ya) - (float)qa, db = fmaf(fk, bstep, yb) - (float)qb;   // y - (q + 2t)
-                    unsigned bh0, bl0, bh1, bl1;
-                    split2(__saturatef(1.0f - fabsf(da)), __saturatef(1.0f - fabsf(da - 1.0f)), bh0, bl0);
-                    split2(__saturatef(1.0f - fabsf(db)), __saturatef(1.0f - fabsf(db - 1.0f)), bh1, bl1);
-                    const unsigned adr = adr_k + ((unsigned)(ld_col ? qb : qa) << 4);
-#pragma unroll
-                    for (int zb = 0; zb < NB16; ++zb) {
-                        unsigned ah[4], al[4];
-                        ldsm4t(ah, adr + zb * 2 * FM_PLANE);
-                        ldsm4t(al, adr + zb * 2 * FM_PLANE + FM_PLANE);
-                        mma16816(acc[zb], ah, bh0, bh1);
-                        mma16816(acc[zb], al, bh0, bh1);
-                        mma16816(acc[zb], ah, bl0, bl1);
-                    }
-                }
-#pragma unroll
-                for (int zb = 0; zb < NB16; ++zb) flush(acc[zb], zb, 0);
             }
+            // epilogue: lanes t and t ^ 1 exchange halves so that each holds four consecutive batch entries of one ray (even t:
+            // ray g, odd t: ray g + 8), and add them with one 16-byte RED (a RED costs about one clock per LANE whatever its width)
+#pragma unroll
+            for (int zb = 0; zb < NB16; ++zb)
+#pragma unroll
+                for (int hf = 0; hf < 2; ++hf) {
+                    const float (&d)[4] = acc[zb][hf];
+                    const float sx = mynb ? d[0] : d[2], sy = mynb ? d[1] : d[3];
+                    const float rx = __shfl_xor_sync(0xffffffffu, sx, 1), ry = __shfl_xor_sync(0xffffffffu, sy, 1);
+                    const float4 v = mynb ? make_float4(rx, ry, d[2], d[3]) : make_float4(d[0], d[1], rx, ry);
+                    if (my_ok && zok[zb][hf]) atomicAdd(reinterpret_cast<float4 *>(P + (size_t)zoff[zb][hf] + my_off), v);      // 1/a: k_synth
+                }
         }
     }
 }
