@@ -1,14 +1,14 @@
 // Adjoint projector on the tensor cores (Eq. 10; fold L204-L212): backprojection of the pi-folded sinogram over
-// the base angles as small dense products  D[16 batch entries x 8 voxels] += G[16 x 16 bins] * W[16 bins x 8 voxels]  -- the
-// transpose of forward_mma.cu, and the friendlier side of the pair:
+// the base angles as small products  D[16 voxels x 8 batch entries] += W[16 voxels x 32 bins] * G[32 bins x 8]  with the
+// weight block W as the 2:4 SPARSE operand of mma.sp (SASS HMMA.SP.16832) -- the transpose of forward_mma.cu, and the
+// friendlier side of the pair:
 //   * a 4 x 4 block of voxels touches at most 3 (|c| + |s|) + 3 <= 7.3 consecutive bins at ANY angle, so one 8-bin window per
-//     angle holds every tap of the block: K = 16 = the 8-bin windows of two base angles (any two: no pairing condition),
-//     N = 8 voxels = half a block, 32 of the 128 weights are non-zero, and nothing is ever trimmed (100 % fill);
-//   * the operand that comes from shared memory (the folded sinogram window) is shared by the two halves of a block: one
-//     ldmatrix pair per six HMMAs, so the LSU pipe that binds the forward kernel is at half load here;
+//     angle holds every tap of the block: K = 32 = the 8-bin windows of four base angles (any four: no grouping condition),
+//     M = 16 voxels = the block, and nothing is ever trimmed (100 % fill); a voxel's two taps at an angle are adjacent bins, so
+//     every group of four bins of a window holds at most two of them -- the 2:4 structure;
 //   * the accumulators are voxels: they stay in registers over all base angles and are written once -- no atomics.
 // Operands are split bf16 pairs as in the forward kernel (G = Gh + Gl is written that way by k_fold_split, W = Wh + Wl per
-// weight; D += Gh Wh + Gl Wh + Gh Wl, fp32 accumulation): relative error about 5e-6.
+// weight; D += Wh Gh + Wh Gl + Wl Gh, fp32 accumulation): relative error about 5e-6.
 //
 // CTA = (32 x 32 tile, group of NB16 16-entry batch blocks of (slice, coefficient)); warp w owns four 4 x 4 blocks.  The tile's
 // bin windows of BM_STAGE base angles are staged by TMA 1-D bulk copies (SASS UBLKCP) into a two-stage ring: per angle and
@@ -26,7 +26,7 @@ namespace cp4d {
 namespace {
 
 constexpr int BM_THREADS = 512;
-constexpr int BM_STAGE = 12;                       // base angles per pipeline stage (even: they are consumed two at a time)
+constexpr int BM_STAGE = 12;                       // base angles per pipeline stage (a multiple of four: they are consumed four at a time)
 constexpr int BM_WINP = WIN + 8;                   // staged bins per angle: any 8-bin window that starts inside the tile's window
 constexpr int BM_BLOCKS = (TILE / 4) * (TILE / 4) / (BM_THREADS / 32);   // 4 x 4 voxel blocks per warp
 
@@ -55,6 +55,7 @@ __global__ void __launch_bounds__(BM_THREADS, 1) k_backproject_mma(const uint4 *
     constexpr unsigned STAGE_BYTES = BM_STAGE * ANGLE_UNITS * 16;
     extern __shared__ __align__(128) unsigned char win[];         // [2 stages][BM_STAGE][2][H][BM_WINP] x 16 B
     __shared__ __align__(16) BmAngle sang[2][BM_STAGE];
+    __shared__ __align__(4) unsigned char s_q[2][(TILE / 4) * (TILE / 4)][BM_STAGE];     // first bin of the 8-bin window of (block, angle)
     __shared__ __align__(8) uint64_t mbar[2];
     const int tiles_1d = (a.n + TILE - 1) / TILE;
     const int tile_id = blockIdx.x % a.tiles, ag = blockIdx.x / a.tiles;
@@ -62,7 +63,6 @@ __global__ void __launch_bounds__(BM_THREADS, 1) k_backproject_mma(const uint4 *
     const int tx0 = (tile_id % tiles_1d) * TILE, ty0 = (tile_id / tiles_1d) * TILE;
     const TileGeo *geo = a.geo + (int64_t)tile_id * a.n0;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, g = lane >> 2, t = lane & 3;
-    const unsigned ld_half = (lane >> 3) & 1, ld_col = lane >> 4, ld_row = lane & 7;
     // this CTA's share [g0, g1) of the base angles (small problems split them over CTAs, which then ADD into a zeroed output)
     const int g0 = (int)((int64_t)a.n0 * ag / a.agroups), g1 = (int)((int64_t)a.n0 * (ag + 1) / a.agroups);
     const int n_stage = (g1 - g0 + BM_STAGE - 1) / BM_STAGE;
@@ -86,6 +86,14 @@ __global__ void __launch_bounds__(BM_THREADS, 1) k_backproject_mma(const uint4 *
             S.A1 = real ? A.inv_a : 0.f; S.A2 = real ? A2 : 0.f;      // an angle past the end weighs nothing
             S.pad0 = S.pad1 = 0.f;
         }
+        // 8-bin window of every (4 x 4 block, angle): from the smallest window coordinate of the block's 16 voxels
+        for (int e = threadIdx.x; e < (TILE / 4) * (TILE / 4) * BM_STAGE; e += BM_THREADS) {
+            const int bid = e / BM_STAGE, p = e % BM_STAGE, i = min(i0 + p, g1 - 1);
+            const AngleTab A = a.ang[i];
+            const float cmin = geo[i].delta + fminf(0.f, 3.0f * A.c) + fminf(0.f, 3.0f * A.s);
+            const float u = fmaf((float)(4 * (bid & 7)), A.c, fmaf((float)(4 * (bid >> 3)), A.s, cmin));
+            s_q[buf][bid][p] = (unsigned char)min(max((int)floorf(u), 0), BM_WINP - 8);
+        }
         if (threadIdx.x < 32) {
             constexpr int ROWS = BM_STAGE * 2 * H;                     // one copy per (angle, hi/lo, half)
             if (threadIdx.x == 0) mbar_expect_tx(&mbar[buf], (unsigned)(ROWS * BM_WINP * 16));
@@ -99,86 +107,96 @@ __global__ void __launch_bounds__(BM_THREADS, 1) k_backproject_mma(const uint4 *
         }
     };
 
-    float acc[BM_BLOCKS][2][NB16][4];
+    float acc[BM_BLOCKS][NB16][2][4];     // [block][batch block][8-entry half]: voxels g (0, 1) and g + 8 (2, 3) x batch entries 2t, 2t + 1
 #pragma unroll
     for (int q = 0; q < BM_BLOCKS; ++q)
 #pragma unroll
-        for (int h = 0; h < 2; ++h)
+        for (int zb = 0; zb < NB16; ++zb)
 #pragma unroll
-            for (int zb = 0; zb < NB16; ++zb) acc[q][h][zb][0] = acc[q][h][zb][1] = acc[q][h][zb][2] = acc[q][h][zb][3] = 0.f;
+            for (int hf = 0; hf < 2; ++hf) acc[q][zb][hf][0] = acc[q][zb][hf][1] = acc[q][zb][hf][2] = acc[q][zb][hf][3] = 0.f;
 
     const unsigned win_s = smem_u32(win);
-    // my voxel as column g of the weight block: (g & 3, g >> 2) inside the half block; half h adds two rows
+    // The weight block is the sparse operand: A[16 voxels x 32 bins], bin k = 8 aa + r = bin r of the 8-bin window of angle aa of
+    // the group of four.  Lane (g, t) computes, for voxels g and g + 8 of the block ((g & 3, g >> 2) and two rows further), the
+    // two kept elements of group t (angle t / 2, bins 4 (t & 1) .. + 3) and of group t + 4 (angle 2 + t / 2, same bins).
     const float vx = (float)(g & 3), vy = (float)(g >> 2);
+    const int ka = t >> 1;                                           // my angles within the group: ka and ka + 2
+    const float fh = (float)(4 * (t & 1));
+    const unsigned qsel = 0x4440u + (unsigned)ka, qsel2 = qsel + 2u, msel = 0x4440u + (lane >> 3);
     if (n_stage > 0) stage(0, 0);
     __syncthreads();
     for (int st = 0; st < n_stage; ++st) {
         const int buf = st & 1;
-        // buffer buf^1 and sang[buf^1] were last read in the previous iteration, which ended with __syncthreads
+        // buffer buf^1, sang[buf^1] and s_q[buf^1] were last read in the previous iteration, which ended with __syncthreads
         if (st + 1 < n_stage) stage(buf ^ 1, st + 1);
         mbar_wait(&mbar[buf], (st >> 1) & 1);
 #pragma unroll 1
-        for (int p = 0; p < BM_STAGE; p += 2) {
-            const BmAngle S0 = sang[buf][p], S1 = sang[buf][p + 1];
+        for (int p = 0; p < BM_STAGE; p += 4) {
+            const BmAngle S0 = sang[buf][p + ka], S1 = sang[buf][p + 2 + ka];
 #pragma unroll
             for (int q = 0; q < BM_BLOCKS; ++q) {
                 const int bid = warp * BM_BLOCKS + q;
-                const float X0 = (float)(4 * (bid & 7)), Y0 = (float)(4 * (bid >> 3));
-                // 8-bin window of the block at either angle: from the smallest window coordinate of its 16 voxels
-                const int q0 = min(max((int)floorf(fmaf(X0, S0.c, fmaf(Y0, S0.s, S0.cmin))), 0), BM_WINP - 8);
-                const int q1 = min(max((int)floorf(fmaf(X0, S1.c, fmaf(Y0, S1.s, S1.cmin))), 0), BM_WINP - 8);
-                const unsigned adr = win_s + buf * STAGE_BYTES +
-                                     ((((p + ld_col) * 2 * H + ld_half) * BM_WINP + (ld_col ? q1 : q0) + ld_row) << 4);
-                unsigned ah[NB16][4], al[NB16][4];
+                const float fx = (float)(4 * (bid & 7)) + vx, fy = (float)(4 * (bid >> 3)) + vy;
+                const unsigned qw = *reinterpret_cast<const unsigned *>(&s_q[buf][bid][p]);      // window starts of the four angles
+                const float fq0 = (float)__byte_perm(qw, 0u, qsel) + fh, fq1 = (float)__byte_perm(qw, 0u, qsel2) + fh;
+                // window coordinate of my voxels relative to the first bin of my half window: voxel g, and g + 8 two rows further
+                const float z00 = fmaf(fx, S0.c, fmaf(fy, S0.s, S0.delta)) - fq0, z01 = fmaf(2.0f, S0.s, z00);
+                const float z10 = fmaf(fx, S1.c, fmaf(fy, S1.s, S1.delta)) - fq1, z11 = fmaf(2.0f, S1.s, z10);
+                unsigned ah[4], al[4], nib[4];
+                auto kept = [&](float z, float A1, float A2, int slot) {
+                    // the kept pair starts at bin i0 = clamp(floor(z), 0, 2) of the half window; Joseph hat in bin units
+                    const bool p1 = z >= 1.0f, p2 = z >= 2.0f;
+                    const float dd = z - (p2 ? 2.0f : p1 ? 1.0f : 0.0f);
+                    nib[slot] = p2 ? 14u : p1 ? 9u : 4u;
+                    split2(fmaxf(0.f, fmaf(-A2, fabsf(dd), A1)), fmaxf(0.f, fmaf(-A2, fabsf(dd - 1.0f), A1)), ah[slot], al[slot]);
+                };
+                kept(z00, S0.A1, S0.A2, 0);      // a0: voxel g,     group t
+                kept(z01, S0.A1, S0.A2, 1);      // a1: voxel g + 8, group t
+                kept(z10, S1.A1, S1.A2, 2);      // a2: voxel g,     group t + 4
+                kept(z11, S1.A1, S1.A2, 3);      // a3: voxel g + 8, group t + 4
+                // metadata (device_helpers.cuh): lane 4g wants the groups 0-3 (low half: voxel g, high half: voxel g + 8), lane
+                // 4g + 1 the groups 4-7; a butterfly over the quad
+                unsigned e0 = (nib[0] | (nib[1] << 16)) << (4 * t), e1 = (nib[2] | (nib[3] << 16)) << (4 * t);
+                e0 |= __shfl_xor_sync(0xffffffffu, e0, 2);
+                e1 |= __shfl_xor_sync(0xffffffffu, e1, 2);
+                const unsigned e = ((t & 1) ? e1 : e0) | __shfl_xor_sync(0xffffffffu, (t & 1) ? e0 : e1, 1);
+                // ldmatrix: matrix = lane / 8 = angle of the group, row lane & 7 = bin of its window
+                const unsigned adr = win_s + buf * STAGE_BYTES + ((((p + (lane >> 3)) * 2 * H) * BM_WINP + __byte_perm(qw, 0u, msel) + (lane & 7)) << 4);
 #pragma unroll
-                for (int zb = 0; zb < NB16; ++zb) {
-                    ldsm4t(ah[zb], adr + (2 * zb) * BM_WINP * 16);
-                    ldsm4t(al[zb], adr + (H + 2 * zb) * BM_WINP * 16);
-                }
-                // window coordinate of my voxel in half 0, relative to bin q + 2t of each angle; half 1 is two rows further
-                const float d0 = fmaf(X0 + vx, S0.c, fmaf(Y0 + vy, S0.s, S0.delta)) - (float)(q0 + 2 * t);
-                const float d1 = fmaf(X0 + vx, S1.c, fmaf(Y0 + vy, S1.s, S1.delta)) - (float)(q1 + 2 * t);
+                for (int zb = 0; zb < NB16; ++zb)
 #pragma unroll
-                for (int h = 0; h < 2; ++h) {
-                    const float e0 = fmaf(2.0f * (float)h, S0.s, d0), e1 = fmaf(2.0f * (float)h, S1.s, d1);
-                    const float w0 = fmaxf(0.f, fmaf(-S0.A2, fabsf(e0), S0.A1)), w1 = fmaxf(0.f, fmaf(-S0.A2, fabsf(e0 - 1.0f), S0.A1));
-                    const float w2 = fmaxf(0.f, fmaf(-S1.A2, fabsf(e1), S1.A1)), w3 = fmaxf(0.f, fmaf(-S1.A2, fabsf(e1 - 1.0f), S1.A1));
-                    unsigned bh0, bl0, bh1, bl1;
-                    split2(w0, w1, bh0, bl0);
-                    split2(w2, w3, bh1, bl1);
-#pragma unroll
-                    for (int zb = 0; zb < NB16; ++zb) {
-                        mma16816(acc[q][h][zb], ah[zb], bh0, bh1);
-                        mma16816(acc[q][h][zb], al[zb], bh0, bh1);
-                        mma16816(acc[q][h][zb], ah[zb], bl0, bl1);
+                    for (int hf = 0; hf < 2; ++hf) {
+                        unsigned bh[4], bl[4];
+                        ldsm4t(bh, adr + (2 * zb + hf) * BM_WINP * 16);
+                        ldsm4t(bl, adr + (H + 2 * zb + hf) * BM_WINP * 16);
+                        mma_sp16832(acc[q][zb][hf], ah, bh, e);
+                        mma_sp16832(acc[q][zb][hf], ah, bl, e);
+                        mma_sp16832(acc[q][zb][hf], al, bh, e);
                     }
-                }
             }
         }
         __syncthreads();
     }
-    // ---- write the voxels: my D entries are voxels 2t, 2t+1 of each half block x batch entries g, g + 8 ----
+    // ---- write the voxels: my D entries are voxels g, g + 8 of each block x batch entries 2t, 2t + 1 of each 8-entry half ----
 #pragma unroll
     for (int q = 0; q < BM_BLOCKS; ++q) {
         const int bid = warp * BM_BLOCKS + q;
 #pragma unroll
-        for (int h = 0; h < 2; ++h)
+        for (int r = 0; r < 2; ++r) {
+            const int x = tx0 + 4 * (bid & 7) + (g & 3), y = ty0 + 4 * (bid >> 3) + (g >> 2) + 2 * r;
+            if (x >= a.n || y >= a.n) continue;
 #pragma unroll
-            for (int cc = 0; cc < 2; ++cc) {
-                const int n = 2 * t + cc;
-                const int x = tx0 + 4 * (bid & 7) + (n & 3), y = ty0 + 4 * (bid >> 3) + 2 * h + (n >> 2);
-                if (x >= a.n || y >= a.n) continue;
+            for (int zb = 0; zb < NB16; ++zb)
 #pragma unroll
-                for (int zb = 0; zb < NB16; ++zb)
-#pragma unroll
-                    for (int r = 0; r < 2; ++r) {
-                        const int flat = zb * 16 + g + 8 * r, sl = z0 + (flat >> a.mshift), j = flat & (a.m - 1);
-                        if (sl >= a.nz) continue;
-                        float *dst = out + (((int64_t)sl * a.n + y) * a.n + x) * a.m + j;
-                        if (a.agroups == 1) *dst = acc[q][h][zb][2 * r + cc];
-                        else atomicAdd(dst, acc[q][h][zb][2 * r + cc]);
-                    }
-            }
+                for (int hf = 0; hf < 2; ++hf) {
+                    const int flat = zb * 16 + hf * 8 + 2 * t, sl = z0 + (flat >> a.mshift), j = flat & (a.m - 1);
+                    if (sl >= a.nz) continue;
+                    float *dst = out + (((int64_t)sl * a.n + y) * a.n + x) * a.m + j;
+                    const float v0 = acc[q][zb][hf][2 * r], v1 = acc[q][zb][hf][2 * r + 1];
+                    if (a.agroups == 1) *reinterpret_cast<float2 *>(dst) = make_float2(v0, v1);
+                    else { atomicAdd(dst, v0); atomicAdd(dst + 1, v1); }
+                }
+        }
     }
 }
 
