@@ -73,36 +73,58 @@ __global__ void __launch_bounds__(BM_THREADS, 1) k_backproject_mma(const uint4 *
     }
     __syncthreads();
 
-    auto stage = [&](int buf, int st) {
+    // Staging of stage st into buffer buf, split so that no warp waits on global memory in the middle of its work:
+    //   stage_issue (start of the previous stage's iteration): warp 0 loads the angle records (lanes < BM_STAGE, one round trip),
+    //     writes them to shared memory and issues the TMA copies of the windows, with the row starts handed round by shuffle;
+    //     warps < BM_STAGE load the three numbers the window table of "their" angle needs and keep them in registers;
+    //   stage_table (end of that iteration, before its closing barrier): the same warps write the table from those registers.
+    float tb_c = 0.f, tb_s = 0.f, tb_cmin = 0.f;
+    auto stage_issue = [&](int buf, int st) {
         const int i0 = g0 + st * BM_STAGE;
-        if (threadIdx.x < BM_STAGE) {
-            const int i = i0 + (int)threadIdx.x;
-            const bool real = i < g1;
-            const AngleTab A = a.ang[min(i, g1 - 1)];
-            const float d = geo[min(i, g1 - 1)].delta, A2 = A.inv_a * A.inv_a;
-            BmAngle &S = sang[buf][threadIdx.x];
-            S.cmin = d + fminf(0.f, 3.0f * A.c) + fminf(0.f, 3.0f * A.s);
-            S.delta = d; S.c = A.c; S.s = A.s;
-            S.A1 = real ? A.inv_a : 0.f; S.A2 = real ? A2 : 0.f;      // an angle past the end weighs nothing
-            S.pad0 = S.pad1 = 0.f;
-        }
-        // 8-bin window of every (4 x 4 block, angle): from the smallest window coordinate of the block's 16 voxels
-        for (int e = threadIdx.x; e < (TILE / 4) * (TILE / 4) * BM_STAGE; e += BM_THREADS) {
-            const int bid = e / BM_STAGE, p = e % BM_STAGE, i = min(i0 + p, g1 - 1);
+        if (warp < BM_STAGE) {
+            const int i = min(i0 + warp, g1 - 1);
             const AngleTab A = a.ang[i];
-            const float cmin = geo[i].delta + fminf(0.f, 3.0f * A.c) + fminf(0.f, 3.0f * A.s);
-            const float u = fmaf((float)(4 * (bid & 7)), A.c, fmaf((float)(4 * (bid >> 3)), A.s, cmin));
-            s_q[buf][bid][p] = (unsigned char)min(max((int)floorf(u), 0), BM_WINP - 8);
+            tb_c = A.c; tb_s = A.s;
+            tb_cmin = geo[i].delta + fminf(0.f, 3.0f * A.c) + fminf(0.f, 3.0f * A.s);
         }
-        if (threadIdx.x < 32) {
+        if (warp == 0) {
+            int bstart = 0;
+            if (lane < BM_STAGE) {
+                const int i = i0 + lane;
+                const bool real = i < g1;
+                const AngleTab A = a.ang[min(i, g1 - 1)];
+                const TileGeo G = geo[min(i, g1 - 1)];
+                const float A2 = A.inv_a * A.inv_a;
+                BmAngle &S = sang[buf][lane];
+                S.cmin = G.delta + fminf(0.f, 3.0f * A.c) + fminf(0.f, 3.0f * A.s);
+                S.delta = G.delta; S.c = A.c; S.s = A.s;
+                S.A1 = real ? A.inv_a : 0.f; S.A2 = real ? A2 : 0.f;      // an angle past the end weighs nothing
+                S.pad0 = S.pad1 = 0.f;
+                bstart = G.bstart;
+            }
             constexpr int ROWS = BM_STAGE * 2 * H;                     // one copy per (angle, hi/lo, half)
-            if (threadIdx.x == 0) mbar_expect_tx(&mbar[buf], (unsigned)(ROWS * BM_WINP * 16));
+            if (lane == 0) mbar_expect_tx(&mbar[buf], (unsigned)(ROWS * BM_WINP * 16));
             __syncwarp();
-            for (int r = threadIdx.x; r < ROWS; r += 32) {
-                const int aa = r / (2 * H), hh = r % (2 * H);           // hh = hl * H + half
-                const int i = min(i0 + aa, g1 - 1);
-                const uint4 *src = gt + (((int64_t)zg * a.n0 + i) * (2 * H) + hh) * a.gp + a.gpl + geo[i].bstart;
-                bulk_g2s(win + (size_t)buf * STAGE_BYTES + (size_t)(aa * 2 * H + hh) * BM_WINP * 16, src, BM_WINP * 16, &mbar[buf]);
+#pragma unroll
+            for (int r0 = 0; r0 < ROWS; r0 += 32) {
+                const int r = r0 + lane, aa = min(r / (2 * H), BM_STAGE - 1), hh = r % (2 * H);           // hh = hl * H + half
+                const int bs = __shfl_sync(0xffffffffu, bstart, aa);
+                if (r < ROWS) {
+                    const int i = min(i0 + aa, g1 - 1);
+                    const uint4 *src = gt + (((int64_t)zg * a.n0 + i) * (2 * H) + hh) * a.gp + a.gpl + bs;
+                    bulk_g2s(win + (size_t)buf * STAGE_BYTES + (size_t)(aa * 2 * H + hh) * BM_WINP * 16, src, BM_WINP * 16, &mbar[buf]);
+                }
+            }
+        }
+    };
+    // 8-bin window of every (4 x 4 block, angle): from the smallest window coordinate of the block's 16 voxels; warp p fills angle p
+    auto stage_table = [&](int buf) {
+        if (warp < BM_STAGE) {
+#pragma unroll
+            for (int k = 0; k < 2; ++k) {
+                const int bid = 2 * lane + k;
+                const float u = fmaf((float)(4 * (bid & 7)), tb_c, fmaf((float)(4 * (bid >> 3)), tb_s, tb_cmin));
+                s_q[buf][bid][warp] = (unsigned char)min(max((int)floorf(u), 0), BM_WINP - 8);
             }
         }
     };
@@ -123,12 +145,13 @@ __global__ void __launch_bounds__(BM_THREADS, 1) k_backproject_mma(const uint4 *
     const int ka = t >> 1;                                           // my angles within the group: ka and ka + 2
     const float fh = (float)(4 * (t & 1));
     const unsigned qsel = 0x4440u + (unsigned)ka, qsel2 = qsel + 2u, msel = 0x4440u + (lane >> 3);
-    if (n_stage > 0) stage(0, 0);
+    if (n_stage > 0) { stage_issue(0, 0); stage_table(0); }
     __syncthreads();
     for (int st = 0; st < n_stage; ++st) {
         const int buf = st & 1;
-        // buffer buf^1, sang[buf^1] and s_q[buf^1] were last read in the previous iteration, which ended with __syncthreads
-        if (st + 1 < n_stage) stage(buf ^ 1, st + 1);
+        // buffer buf^1 and sang[buf^1] were last read in the previous iteration, which ended with __syncthreads (s_q[buf^1] too:
+        // it is rewritten at the end of this one)
+        if (st + 1 < n_stage) stage_issue(buf ^ 1, st + 1);
         mbar_wait(&mbar[buf], (st >> 1) & 1);
 #pragma unroll 1
         for (int p = 0; p < BM_STAGE; p += 4) {
@@ -175,6 +198,7 @@ __global__ void __launch_bounds__(BM_THREADS, 1) k_backproject_mma(const uint4 *
                     }
             }
         }
+        if (st + 1 < n_stage) stage_table(buf ^ 1);
         __syncthreads();
     }
     // ---- write the voxels: my D entries are voxels g, g + 8 of each block x batch entries 2t, 2t + 1 of each 8-entry half ----
