@@ -429,22 +429,23 @@ __global__ void __launch_bounds__(FM_THREADS, 1) k_forward_mma(const float *__re
             for (int st = 0; st < nstep; ++st, adr_k += 4 * FM_COL) {
                 const unsigned qw = __shfl_sync(0xffffffffu, qi, st);
                 const float fq[2] = {(float)__byte_perm(qw, 0u, qsel), (float)__byte_perm(qw, 0u, qsel2)};
-                unsigned ah[4], al[4], nib[4];
+                unsigned ah[4], al[4];
+                float nib[4];
 #pragma unroll
                 for (int cc = 0; cc < 2; ++cc)
 #pragma unroll
                     for (int nb = 0; nb < 2; ++nb) {
                         // row of the first tap relative to my row half; the kept pair starts at row i0 = clamp(floor(z), 0, 2)
                         const float z = ys[nb][cc] - fq[cc];
-                        const bool p1 = z >= 1.0f, p2 = z >= 2.0f;
-                        const float dd = z - (p2 ? 2.0f : p1 ? 1.0f : 0.0f);
-                        nib[2 * cc + nb] = p2 ? 14u : p1 ? 9u : 4u;                       // positions (i0, i0 + 1), two bits each
+                        const float i0 = fminf(fmaxf(floorf(z), 0.0f), 2.0f);
+                        const float dd = z - i0;
+                        nib[2 * cc + nb] = fmaf(5.0f, i0, 4.0f);                          // positions (i0, i0 + 1), two bits each: 4, 9, 14
                         split2(__saturatef(1.0f - fabsf(dd)), __saturatef(1.0f - fabsf(dd - 1.0f)), ah[2 * cc + nb], al[2 * cc + nb]);
                         ys[nb][cc] += st4[nb];
                     }
                 // metadata: lane 4g wants the groups 0-3 (low half: ray g, high half: ray g + 8), lane 4g + 1 the groups 4-7
                 // (a butterfly over the quad: first the lanes two apart, then lanes 0 and 1 hand each other what the other needs)
-                unsigned e0 = (nib[0] | (nib[1] << 16)) << (4 * t), e1 = (nib[2] | (nib[3] << 16)) << (4 * t);
+                unsigned e0 = (unsigned)__float2int_rn(fmaf(nib[1], 65536.0f, nib[0])) << (4 * t), e1 = (unsigned)__float2int_rn(fmaf(nib[3], 65536.0f, nib[2])) << (4 * t);
                 e0 |= __shfl_xor_sync(0xffffffffu, e0, 2);
                 e1 |= __shfl_xor_sync(0xffffffffu, e1, 2);
                 const unsigned e = ((t & 1) ? e1 : e0) | __shfl_xor_sync(0xffffffffu, (t & 1) ? e0 : e1, 1);
