@@ -432,16 +432,19 @@ def assemble(args, c, world, r):
                          if d["bound"] == "alu" else "algorithmic bytes / CUDA-event time")}
     # second, tighter roofs of the forward projector (measured unit rates in profiles/r2_microbench.md):
     #   fp32 gather: one 4-byte operand per FMA through shared memory, 128 B/clk/SM;
-    #   tensor-core kernel: every algorithmic FMA costs 12 HMMA MACs (weight blocks 1/4 dense x three split-bf16 products) at the
-    #   measured mma.sync rate of 950 MAC/clk/SM.
+    #   tensor-core kernel: every algorithmic FMA costs 12 dense-equivalent MACs (weight blocks 1/4 dense x three split-bf16
+    #   products); the 2:4 sparse mma.sp.m16n8k32 takes 16 x 8 x 32 of them per 9.71 clk and sub-partition (measured), i.e.
+    #   1687 dense-equivalent MAC/clk/SM.
     if "forward" in kernels:
         k = kernels["forward"]
         fmas = work["forward"][1] / 2.0
         if r["proj"][0] == "tensor":
-            peak = N_SM * 950.0 * peaks["sm_max_mhz"] * 1e6 / 1e12
+            per_clk = 4 * 16 * 8 * 32 / 9.71
+            peak = N_SM * per_clk * peaks["sm_max_mhz"] * 1e6 / 1e12
             ach = fmas * 12.0 / (k["ms"] * 1e-3) / 1e12
-            k["hmma_roof"] = {"bound": "tensor (mma.sync)", "achieved": ach, "peak": peak, "unit": "TMAC/s", "frac": ach / peak,
-                              "note": "12 HMMA MACs per algorithmic FMA (not counting partly filled blocks); peak = 148 SM x 950 MAC/clk x sm_max_mhz"}
+            k["hmma_roof"] = {"bound": "tensor (mma.sp 2:4)", "achieved": ach, "peak": peak, "unit": "TMAC/s", "frac": ach / peak,
+                              "note": "12 dense-equivalent MACs per algorithmic FMA (not counting partly filled blocks); peak = 148 SM x 4 x "
+                                      "16*8*32 MAC per 9.71 clk (HMMA.SP.16832, measured) x sm_max_mhz"}
         else:
             smem_peak = N_SM * 128 * peaks["sm_max_mhz"] * 1e6 / 1e9                       # GB/s
             smem_ach = fmas * 4.0 / (k["ms"] * 1e-3) / 1e9

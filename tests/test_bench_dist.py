@@ -75,8 +75,10 @@ def test_json_line_contract_offline():
     assert rf["frac"] == pytest.approx(rf["achieved"] / rf["peak"]) and 0 < rf["frac"] < 1
     # algorithmic flops of the forward kernel: 2 flop x 2 taps x m x N^2 Nz N_theta0
     assert rf["achieved"] * 1e12 * 6.7e-3 == pytest.approx(2 * 2 * c.m * c.n ** 2 * c.nz * c.n_theta0, rel=1e-9)
-    # tensor-core forward kernel: 12 HMMA MACs per algorithmic FMA against 950 MAC/clk/SM (profiles/r2_microbench.md)
-    assert rf["second_roof"]["frac"] == pytest.approx(rf["achieved"] / 2 * 12 / (148 * 950 * r["peaks"]["sm_max_mhz"] * 1e6 / 1e12), rel=1e-6)
+    # tensor-core forward kernel: 12 dense-equivalent MACs per algorithmic FMA against the measured rate of the 2:4 sparse
+    # mma.sp.m16n8k32, 16 x 8 x 32 per 9.71 clk and sub-partition (profiles/r2_microbench.md)
+    per_clk = 4 * 16 * 8 * 32 / 9.71
+    assert rf["second_roof"]["frac"] == pytest.approx(rf["achieved"] / 2 * 12 / (148 * per_clk * r["peaks"]["sm_max_mhz"] * 1e6 / 1e12), rel=1e-6)
     assert line["run"]["projectors"] == {"mode": "auto", "forward": "tensor", "adjoint": "fp32"}
     r2 = dict(r, proj=("fp32", "fp32"))
     rf2 = bench.assemble(A, c, 1, r2)["roofline"]
