@@ -55,7 +55,7 @@ int validate(const cp4d_params *p, Dims *d) {
 }
 
 struct Carve {
-    uint64_t f, ft, bp, h2, h1, g, tmp_s, scratch, psum, phi, ang, geo, red, cf, cb, psi, fwang, fworder, fwpairs, fwitems, fwcounts, total;
+    uint64_t f, ft, bp, h2, h1, g, tmp_s, scratch, psum, phi, ang, geo, red, cf, cb, psi, fwang, fworder, fwpairs, fwitems, fwcounts, bmrec, total;
 };
 Carve carve(const Dims &d) {
     Carve c;
@@ -69,6 +69,7 @@ Carve carve(const Dims &d) {
     c.fwang = take((uint64_t)d.n0 * sizeof(FwAngle)); c.fworder = take((uint64_t)d.n0 * 4);
     c.fwpairs = take((uint64_t)d.n0 * sizeof(int4));
     c.fwitems = take(forward_mma_item_bytes(d)); c.fwcounts = take((uint64_t)d.tiles * 2 * sizeof(int2));
+    c.bmrec = take(backproject_mma_rec_bytes(d));
     c.cf = c.cb = c.psi = 0;
     if (d.nf) { c.cf = take(d.Vc * 4); c.cb = take(d.Vc * 4); c.psi = take((uint64_t)d.mb * d.nf * 4); }
     c.total = o;
@@ -199,6 +200,7 @@ int cp4d_create(const cp4d_params *p, cp4d_ctx **out) {
     ctx->fwang = (FwAngle *)(w + cv.fwang); ctx->fworder = (int32_t *)(w + cv.fworder);
     ctx->fw_groups = (int4 *)(w + cv.fwpairs); ctx->fw_mode = CP4D_PROJ_AUTO;
     ctx->fw_items = forward_mma_item_bytes(d) ? (unsigned *)(w + cv.fwitems) : nullptr; ctx->fw_counts = (int2 *)(w + cv.fwcounts);
+    ctx->bm_rec = backproject_mma_rec_bytes(d) ? (void *)(w + cv.bmrec) : nullptr;
     ctx->cf = d.nf ? (float *)(w + cv.cf) : nullptr; ctx->cb = d.nf ? (float *)(w + cv.cb) : nullptr;
     ctx->psi = d.nf ? (float *)(w + cv.psi) : nullptr;
     ctx->scratch = (float4 *)(w + cv.scratch); ctx->psum = (float4 *)(w + cv.psum); ctx->phi = (float *)(w + cv.phi);
@@ -276,6 +278,7 @@ int cp4d_create(const cp4d_params *p, cp4d_ctx **out) {
         (e = cudaMemcpyAsync(ctx->geo, geo.data(), geo.size() * sizeof(TileGeo), cudaMemcpyHostToDevice, ctx->stream)) != cudaSuccess ||
         (e = cudaMemsetAsync(ctx->scratch, 0, (size_t)d.scratch4 * 16, ctx->stream)) != cudaSuccess ||
         (e = forward_mma_build(ctx)) != cudaSuccess ||
+        (e = backproject_mma_build(ctx)) != cudaSuccess ||
         (e = cudaStreamSynchronize(ctx->stream)) != cudaSuccess) {
         ctx->err = cudaGetErrorString(e);   // (the context dies with the error: the caller only sees CP4D_ECUDA)
         cudaGetLastError();

@@ -34,17 +34,35 @@ struct BmArgs {
     int n, nz, nd, n0, m, mshift, gp, gpl;
     int tiles, agroups;
     int zper;                                      // slices per CTA = NB16 * 16 / m
-    const AngleTab *ang;
-    const TileGeo *geo;
+    const struct BmAngle *rec;                      // [tile][n0 + BM_STAGE] angle records, built once per context by k_bm_build
 };
 
-// per staged base angle (shared memory, broadcast loads)
+// per (tile, base angle): built once per context, staged by TMA (shared memory, broadcast loads)
 struct BmAngle {
     float cmin;    // delta + min(0, 3c) + min(0, 3s): smallest window coordinate of a block is cmin + X0 c + Y0 s
     float delta, c, s;
     float A1, A2;  // Joseph hat in bin units: weight(bin) = max(0, A1 - A2 |u - bin|), A1 = 1/a, A2 = 1/a^2 (0, 0 for a dummy)
-    float pad0, pad1;
+    int bstart;    // first bin of the tile's window at this angle
+    float pad;
 };
+static_assert(sizeof(BmAngle) == 32, "BmAngle is two 16-byte units");
+
+// The angle records of every tile (they depend on the geometry only): n0 real ones and BM_STAGE that weigh nothing, so that the
+// last stage of a CTA can always be staged whole.
+__global__ void __launch_bounds__(128) k_bm_build(BmAngle *rec, const AngleTab *ang, const TileGeo *geo, int n0) {
+    const int tile = blockIdx.x;
+    for (int i = threadIdx.x; i < n0 + BM_STAGE; i += blockDim.x) {
+        const int ii = min(i, n0 - 1);
+        const AngleTab A = ang[ii];
+        const TileGeo G = geo[(int64_t)tile * n0 + ii];
+        BmAngle R;
+        R.cmin = G.delta + fminf(0.f, 3.0f * A.c) + fminf(0.f, 3.0f * A.s);
+        R.delta = G.delta; R.c = A.c; R.s = A.s;
+        R.A1 = i < n0 ? A.inv_a : 0.f; R.A2 = i < n0 ? A.inv_a * A.inv_a : 0.f;
+        R.bstart = G.bstart; R.pad = 0.f;
+        rec[(int64_t)tile * (n0 + BM_STAGE) + i] = R;
+    }
+}
 
 // gt (split layout, written by k_fold_split): 16-byte units of 8 bf16 batch entries,
 //   unit index = ((((zg n0 + i) 2 + hl) H + half) gp + gpl + b),  H = 2 NB16 halves per z-group, hl = 0 hi / 1 lo
@@ -61,7 +79,7 @@ __global__ void __launch_bounds__(BM_THREADS, 1) k_backproject_mma(const uint4 *
     const int tile_id = blockIdx.x % a.tiles, ag = blockIdx.x / a.tiles;
     const int zg = blockIdx.y, z0 = zg * a.zper;
     const int tx0 = (tile_id % tiles_1d) * TILE, ty0 = (tile_id / tiles_1d) * TILE;
-    const TileGeo *geo = a.geo + (int64_t)tile_id * a.n0;
+    const BmAngle *rec = a.rec + (int64_t)tile_id * (a.n0 + BM_STAGE);
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, g = lane >> 2, t = lane & 3;
     // this CTA's share [g0, g1) of the base angles (small problems split them over CTAs, which then ADD into a zeroed output)
     const int g0 = (int)((int64_t)a.n0 * ag / a.agroups), g1 = (int)((int64_t)a.n0 * (ag + 1) / a.agroups);
@@ -73,57 +91,45 @@ __global__ void __launch_bounds__(BM_THREADS, 1) k_backproject_mma(const uint4 *
     }
     __syncthreads();
 
-    // Staging of stage st into buffer buf, split so that no warp waits on global memory in the middle of its work:
-    //   stage_issue (start of the previous stage's iteration): warp 0 loads the angle records (lanes < BM_STAGE, one round trip),
-    //     writes them to shared memory and issues the TMA copies of the windows, with the row starts handed round by shuffle;
-    //     warps < BM_STAGE load the three numbers the window table of "their" angle needs and keep them in registers;
-    //   stage_table (end of that iteration, before its closing barrier): the same warps write the table from those registers.
-    float tb_c = 0.f, tb_s = 0.f, tb_cmin = 0.f;
+    // Staging of stage st into buffer buf, so that no warp waits on global memory in the middle of its work:
+    //   stage_issue (start of the previous stage's iteration, warp 0): one TMA copy of the stage's angle records and the TMA copies
+    //     of the windows, whose row starts lanes < BM_STAGE loaded one call earlier (nb_bstart) and hand round by shuffle;
+    //   stage_table (end of that iteration, warps < BM_STAGE): the window table of the stage from its records, which have landed
+    //     long before (the mbarrier is still waited for: it orders the reads after the copies).
+    int nb_bstart = 0;
+    if (warp == 0 && lane < BM_STAGE) nb_bstart = rec[g0 + lane].bstart;
     auto stage_issue = [&](int buf, int st) {
         const int i0 = g0 + st * BM_STAGE;
-        if (warp < BM_STAGE) {
-            const int i = min(i0 + warp, g1 - 1);
-            const AngleTab A = a.ang[i];
-            tb_c = A.c; tb_s = A.s;
-            tb_cmin = geo[i].delta + fminf(0.f, 3.0f * A.c) + fminf(0.f, 3.0f * A.s);
-        }
         if (warp == 0) {
-            int bstart = 0;
-            if (lane < BM_STAGE) {
-                const int i = i0 + lane;
-                const bool real = i < g1;
-                const AngleTab A = a.ang[min(i, g1 - 1)];
-                const TileGeo G = geo[min(i, g1 - 1)];
-                const float A2 = A.inv_a * A.inv_a;
-                BmAngle &S = sang[buf][lane];
-                S.cmin = G.delta + fminf(0.f, 3.0f * A.c) + fminf(0.f, 3.0f * A.s);
-                S.delta = G.delta; S.c = A.c; S.s = A.s;
-                S.A1 = real ? A.inv_a : 0.f; S.A2 = real ? A2 : 0.f;      // an angle past the end weighs nothing
-                S.pad0 = S.pad1 = 0.f;
-                bstart = G.bstart;
-            }
             constexpr int ROWS = BM_STAGE * 2 * H;                     // one copy per (angle, hi/lo, half)
-            if (lane == 0) mbar_expect_tx(&mbar[buf], (unsigned)(ROWS * BM_WINP * 16));
+            if (lane == 0) {
+                mbar_expect_tx(&mbar[buf], (unsigned)(ROWS * BM_WINP * 16 + BM_STAGE * sizeof(BmAngle)));
+                bulk_g2s(&sang[buf][0], rec + i0, (unsigned)(BM_STAGE * sizeof(BmAngle)), &mbar[buf]);
+            }
             __syncwarp();
 #pragma unroll
             for (int r0 = 0; r0 < ROWS; r0 += 32) {
                 const int r = r0 + lane, aa = min(r / (2 * H), BM_STAGE - 1), hh = r % (2 * H);           // hh = hl * H + half
-                const int bs = __shfl_sync(0xffffffffu, bstart, aa);
+                const int bs = __shfl_sync(0xffffffffu, nb_bstart, aa);
                 if (r < ROWS) {
-                    const int i = min(i0 + aa, g1 - 1);
+                    const int i = min(i0 + aa, a.n0 - 1);
                     const uint4 *src = gt + (((int64_t)zg * a.n0 + i) * (2 * H) + hh) * a.gp + a.gpl + bs;
                     bulk_g2s(win + (size_t)buf * STAGE_BYTES + (size_t)(aa * 2 * H + hh) * BM_WINP * 16, src, BM_WINP * 16, &mbar[buf]);
                 }
             }
+            if (lane < BM_STAGE && st + 1 < n_stage) nb_bstart = rec[i0 + BM_STAGE + lane].bstart;      // used by the next call
         }
     };
     // 8-bin window of every (4 x 4 block, angle): from the smallest window coordinate of the block's 16 voxels; warp p fills angle p
-    auto stage_table = [&](int buf) {
+    auto stage_table = [&](int buf, int st) {
         if (warp < BM_STAGE) {
+            mbar_wait(&mbar[buf], (st >> 1) & 1);
+            const BmAngle &S = sang[buf][warp];
+            const float tc = S.c, ts = S.s, tcmin = S.cmin;
 #pragma unroll
             for (int k = 0; k < 2; ++k) {
                 const int bid = 2 * lane + k;
-                const float u = fmaf((float)(4 * (bid & 7)), tb_c, fmaf((float)(4 * (bid >> 3)), tb_s, tb_cmin));
+                const float u = fmaf((float)(4 * (bid & 7)), tc, fmaf((float)(4 * (bid >> 3)), ts, tcmin));
                 s_q[buf][bid][warp] = (unsigned char)min(max((int)floorf(u), 0), BM_WINP - 8);
             }
         }
@@ -145,7 +151,7 @@ __global__ void __launch_bounds__(BM_THREADS, 1) k_backproject_mma(const uint4 *
     const int ka = t >> 1;                                           // my angles within the group: ka and ka + 2
     const float fh = (float)(4 * (t & 1));
     const unsigned qsel = 0x4440u + (unsigned)ka, qsel2 = qsel + 2u, msel = 0x4440u + (lane >> 3);
-    if (n_stage > 0) { stage_issue(0, 0); stage_table(0); }
+    if (n_stage > 0) { stage_issue(0, 0); stage_table(0, 0); }
     __syncthreads();
     for (int st = 0; st < n_stage; ++st) {
         const int buf = st & 1;
@@ -155,7 +161,10 @@ __global__ void __launch_bounds__(BM_THREADS, 1) k_backproject_mma(const uint4 *
         mbar_wait(&mbar[buf], (st >> 1) & 1);
 #pragma unroll 1
         for (int p = 0; p < BM_STAGE; p += 4) {
-            const BmAngle S0 = sang[buf][p + ka], S1 = sang[buf][p + 2 + ka];
+            BmAngle S0 = sang[buf][p + ka], S1 = sang[buf][p + 2 + ka];
+            // angles past this CTA's share (the tail of its last stage) weigh nothing
+            if (g0 + st * BM_STAGE + p + ka >= g1) S0.A1 = S0.A2 = 0.f;
+            if (g0 + st * BM_STAGE + p + 2 + ka >= g1) S1.A1 = S1.A2 = 0.f;
 #pragma unroll
             for (int q = 0; q < BM_BLOCKS; ++q) {
                 const int bid = warp * BM_BLOCKS + q;
@@ -198,7 +207,7 @@ __global__ void __launch_bounds__(BM_THREADS, 1) k_backproject_mma(const uint4 *
                     }
             }
         }
-        if (st + 1 < n_stage) stage_table(buf ^ 1);
+        if (st + 1 < n_stage) stage_table(buf ^ 1, st + 1);
         __syncthreads();
     }
     // ---- write the voxels: my D entries are voxels g, g + 8 of each block x batch entries 2t, 2t + 1 of each 8-entry half ----
@@ -310,6 +319,18 @@ int64_t backproject_mma_scratch_units(const Dims &d) {
     return (int64_t)zgroups * d.n0 * 2 * (2 * nb) * d.gp;
 }
 
+// bytes of the per-(tile, angle) records of a context (0 if the shape is not supported)
+uint64_t backproject_mma_rec_bytes(const Dims &d) {
+    return forward_mma_supported(d) ? (uint64_t)d.tiles * (d.n0 + BM_STAGE) * sizeof(BmAngle) : 0;
+}
+
+// cp4d_create: the angle records of every tile, once (they depend on the geometry only)
+cudaError_t backproject_mma_build(cp4d_ctx *c) {
+    if (!c->bm_rec) return cudaSuccess;
+    k_bm_build<<<c->d.tiles, 128, 0, c->stream>>>(reinterpret_cast<BmAngle *>(c->bm_rec), c->ang, c->geo, c->d.n0);
+    return cudaGetLastError();
+}
+
 cudaError_t backproject_mma_init() {
     cudaError_t e = cudaFuncSetAttribute(k_backproject_mma<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, 2 * BM_STAGE * 2 * 2 * 1 * BM_WINP * 16);
     if (e != cudaSuccess) return e;
@@ -332,7 +353,7 @@ cudaError_t launch_backproject_mma(cp4d_ctx *c, const float4 *gt, float *f_out) 
     const Dims &d = c->d;
     int ms = 0;
     while ((1 << ms) < d.m) ++ms;
-    BmArgs a{d.n, d.nz, d.nd, d.n0, d.m, ms, d.gp, d.gpl, d.tiles, 1, 0, c->ang, c->geo};
+    BmArgs a{d.n, d.nz, d.nd, d.n0, d.m, ms, d.gp, d.gpl, d.tiles, 1, 0, reinterpret_cast<const BmAngle *>(c->bm_rec)};
     c->launches++;
     const uint4 *G = reinterpret_cast<const uint4 *>(gt);
     if (backproject_mma_nb16(d) == 1) return bm_launch<1>(c, G, f_out, a);

@@ -47,6 +47,7 @@ def test_workspace_bytes_counts_state(L):
         gs = 4 if c.n_theta0 >= 72 else 2 if c.n_theta0 >= 24 else 1
         tiles = ((c.n + 31) // 32) ** 2
         scratch += tiles * 4 * 14 * (c.n_theta0 // gs + 8) * 48
+        scratch += tiles * (c.n_theta0 + 12) * 32              # angle records of the tensor backprojector per (tile, angle)
         assert state + scratch <= nb <= state + scratch + (64 << 20)
     c = synth.CONFIGS[5]
     assert binding.workspace_bytes(c.n, c.nz, c.nd, c.n_angles, c.n_half_rot, c.m) < 170e9   # fits 180 GB HBM
