@@ -65,13 +65,18 @@ __global__ void __launch_bounds__(128) k_bm_build(BmAngle *rec, const AngleTab *
 }
 
 // gt (split layout, written by k_fold_split): 16-byte units of 8 bf16 batch entries,
-//   unit index = ((((zg n0 + i) 2 + hl) H + half) gp + gpl + b),  H = 2 NB16 halves per z-group, hl = 0 hi / 1 lo
+//   unit index = ((zg n0 + i) gp + gpl + b) U + hl H + half,  H = 2 NB16 halves per z-group, hl = 0 hi / 1 lo, U = 2 H + 1:
+//   bin-major, so that the window of a tile at an angle is ONE contiguous run (one TMA copy per angle: the issue of a bulk copy
+//   costs about 80 clk and holds up the other warps' shared-memory instructions, and 8 copies per angle were a fifth of the
+//   kernel's time), and one unit of padding per bin, so that the 8 bins of an ldmatrix operand (stride U x 16 B) fall into 8
+//   different bank groups
 template <int NB16>
 __global__ void __launch_bounds__(BM_THREADS, 1) k_backproject_mma(const uint4 *__restrict__ gt, float *__restrict__ out, BmArgs a) {
     constexpr int H = 2 * NB16;
-    constexpr int ANGLE_UNITS = 2 * H * BM_WINP;                 // 16-byte units per staged angle: [hl][half][bin]
+    constexpr int U = 2 * H + 1;
+    constexpr int ANGLE_UNITS = U * BM_WINP;                     // 16-byte units per staged angle: [bin][hl][half] + 1 of padding
     constexpr unsigned STAGE_BYTES = BM_STAGE * ANGLE_UNITS * 16;
-    extern __shared__ __align__(128) unsigned char win[];         // [2 stages][BM_STAGE][2][H][BM_WINP] x 16 B
+    extern __shared__ __align__(128) unsigned char win[];         // [2 stages][BM_STAGE][BM_WINP][U] x 16 B
     __shared__ __align__(16) BmAngle sang[2][BM_STAGE];
     __shared__ __align__(4) unsigned char s_q[2][(TILE / 4) * (TILE / 4)][BM_STAGE];     // first bin of the 8-bin window of (block, angle)
     __shared__ __align__(8) uint64_t mbar[2];
@@ -101,21 +106,15 @@ __global__ void __launch_bounds__(BM_THREADS, 1) k_backproject_mma(const uint4 *
     auto stage_issue = [&](int buf, int st) {
         const int i0 = g0 + st * BM_STAGE;
         if (warp == 0) {
-            constexpr int ROWS = BM_STAGE * 2 * H;                     // one copy per (angle, hi/lo, half)
             if (lane == 0) {
-                mbar_expect_tx(&mbar[buf], (unsigned)(ROWS * BM_WINP * 16 + BM_STAGE * sizeof(BmAngle)));
+                mbar_expect_tx(&mbar[buf], (unsigned)(BM_STAGE * ANGLE_UNITS * 16 + BM_STAGE * sizeof(BmAngle)));
                 bulk_g2s(&sang[buf][0], rec + i0, (unsigned)(BM_STAGE * sizeof(BmAngle)), &mbar[buf]);
             }
             __syncwarp();
-#pragma unroll
-            for (int r0 = 0; r0 < ROWS; r0 += 32) {
-                const int r = r0 + lane, aa = min(r / (2 * H), BM_STAGE - 1), hh = r % (2 * H);           // hh = hl * H + half
-                const int bs = __shfl_sync(0xffffffffu, nb_bstart, aa);
-                if (r < ROWS) {
-                    const int i = min(i0 + aa, a.n0 - 1);
-                    const uint4 *src = gt + (((int64_t)zg * a.n0 + i) * (2 * H) + hh) * a.gp + a.gpl + bs;
-                    bulk_g2s(win + (size_t)buf * STAGE_BYTES + (size_t)(aa * 2 * H + hh) * BM_WINP * 16, src, BM_WINP * 16, &mbar[buf]);
-                }
+            if (lane < BM_STAGE) {                                     // one copy per angle
+                const int i = min(i0 + lane, a.n0 - 1);
+                const uint4 *src = gt + (((int64_t)zg * a.n0 + i) * a.gp + a.gpl + nb_bstart) * U;
+                bulk_g2s(win + (size_t)buf * STAGE_BYTES + (size_t)lane * ANGLE_UNITS * 16, src, ANGLE_UNITS * 16, &mbar[buf]);
             }
             if (lane < BM_STAGE && st + 1 < n_stage) nb_bstart = rec[i0 + BM_STAGE + lane].bstart;      // used by the next call
         }
@@ -193,14 +192,14 @@ __global__ void __launch_bounds__(BM_THREADS, 1) k_backproject_mma(const uint4 *
                 e1 |= __shfl_xor_sync(0xffffffffu, e1, 2);
                 const unsigned e = ((t & 1) ? e1 : e0) | __shfl_xor_sync(0xffffffffu, (t & 1) ? e0 : e1, 1);
                 // ldmatrix: matrix = lane / 8 = angle of the group, row lane & 7 = bin of its window
-                const unsigned adr = win_s + buf * STAGE_BYTES + ((((p + (lane >> 3)) * 2 * H) * BM_WINP + __byte_perm(qw, 0u, msel) + (lane & 7)) << 4);
+                const unsigned adr = win_s + buf * STAGE_BYTES + (((p + (lane >> 3)) * BM_WINP + __byte_perm(qw, 0u, msel) + (lane & 7)) * (U * 16));
 #pragma unroll
                 for (int zb = 0; zb < NB16; ++zb)
 #pragma unroll
                     for (int hf = 0; hf < 2; ++hf) {
                         unsigned bh[4], bl[4];
-                        ldsm4t(bh, adr + (2 * zb + hf) * BM_WINP * 16);
-                        ldsm4t(bl, adr + (H + 2 * zb + hf) * BM_WINP * 16);
+                        ldsm4t(bh, adr + (2 * zb + hf) * 16);
+                        ldsm4t(bl, adr + (H + 2 * zb + hf) * 16);
                         mma_sp16832(acc[q][zb][hf], ah, bh, e);
                         mma_sp16832(acc[q][zb][hf], ah, bl, e);
                         mma_sp16832(acc[q][zb][hf], al, bh, e);
@@ -244,8 +243,9 @@ __global__ void __launch_bounds__(128) k_fold_split(const float *__restrict__ g,
     for (int t = threadIdx.x; t < npi * m; t += blockDim.x) phis[t] = phi[(int64_t)(t % m) * na + (t / m) * n0 + i];
     __syncthreads();
     const int zg = z / zper, flat0 = (z - zg * zper) * m;         // first batch entry of this slice inside its z-group
-    unsigned short *hi = reinterpret_cast<unsigned short *>(gt + ((int64_t)zg * n0 + i) * 2 * H * gp);
-    unsigned short *lo = hi + (int64_t)H * gp * 8;
+    const int U = 2 * H + 1;
+    unsigned short *hi = reinterpret_cast<unsigned short *>(gt + ((int64_t)zg * n0 + i) * gp * U);
+    unsigned short *lo = hi + H * 8;
     for (int b = threadIdx.x; b < nd; b += blockDim.x) {
         float acc[m];
 #pragma unroll
@@ -269,7 +269,7 @@ __global__ void __launch_bounds__(128) k_fold_split(const float *__restrict__ g,
 #pragma unroll
         for (int jc = 0; jc < Q; ++jc) {
             const int flat = flat0 + 4 * jc;
-            const int64_t e = ((int64_t)(flat >> 3) * gp + gpl + b) * 8 + (flat & 7);
+            const int64_t e = ((int64_t)(gpl + b) * U + (flat >> 3)) * 8 + (flat & 7);
             unsigned h01, l01, h23, l23;
             split2(acc[4 * jc], acc[4 * jc + 1], h01, l01);
             split2(acc[4 * jc + 2], acc[4 * jc + 3], h23, l23);
@@ -293,7 +293,7 @@ cudaError_t bm_launch(cp4d_ctx *c, const uint4 *gt, float *out, BmArgs a) {
         c->launches++;
     }
     const dim3 grid(d.tiles * a.agroups, zgroups);
-    k_backproject_mma<NB16><<<grid, BM_THREADS, (size_t)2 * BM_STAGE * 2 * 2 * NB16 * BM_WINP * 16, c->stream>>>(gt, out, a);
+    k_backproject_mma<NB16><<<grid, BM_THREADS, (size_t)2 * BM_STAGE * (4 * NB16 + 1) * BM_WINP * 16, c->stream>>>(gt, out, a);
     return cudaGetLastError();
 }
 
@@ -316,7 +316,7 @@ int backproject_mma_nb16(const Dims &d) {
 // 16-byte units of gt in the split layout (>= what the fp32 layout of the same scratch needs when nz is a multiple of zper)
 int64_t backproject_mma_scratch_units(const Dims &d) {
     const int nb = backproject_mma_nb16(d), zper = nb * 16 / d.m, zgroups = (d.nz + zper - 1) / zper;
-    return (int64_t)zgroups * d.n0 * 2 * (2 * nb) * d.gp;
+    return (int64_t)zgroups * d.n0 * (4 * nb + 1) * d.gp;
 }
 
 // bytes of the per-(tile, angle) records of a context (0 if the shape is not supported)
@@ -332,9 +332,9 @@ cudaError_t backproject_mma_build(cp4d_ctx *c) {
 }
 
 cudaError_t backproject_mma_init() {
-    cudaError_t e = cudaFuncSetAttribute(k_backproject_mma<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, 2 * BM_STAGE * 2 * 2 * 1 * BM_WINP * 16);
+    cudaError_t e = cudaFuncSetAttribute(k_backproject_mma<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, 2 * BM_STAGE * (4 * 1 + 1) * BM_WINP * 16);
     if (e != cudaSuccess) return e;
-    return cudaFuncSetAttribute(k_backproject_mma<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, 2 * BM_STAGE * 2 * 2 * 2 * BM_WINP * 16);
+    return cudaFuncSetAttribute(k_backproject_mma<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, 2 * BM_STAGE * (4 * 2 + 1) * BM_WINP * 16);
 }
 
 cudaError_t launch_fold_split(cp4d_ctx *c, const float *g, float4 *gt) {
