@@ -233,20 +233,23 @@ __global__ void __launch_bounds__(BM_THREADS, 1) k_backproject_mma(const uint4 *
 }
 
 // Fold for the tensor-core backprojector: gt_j[z][i][b] = sum_q Phi[j, q n0 + i] g[z][q n0 + i][flip_q b],
-// written as split bf16 pairs in the layout k_backproject_mma stages.  One CTA per (z, base angle i), one thread per bin.
+// written as split bf16 pairs in the layout k_backproject_mma stages.
 template <int Q>
 __global__ void __launch_bounds__(128) k_fold_split(const float *__restrict__ g, uint4 *__restrict__ gt, const float *__restrict__ phi,
-                                                    int nd, int na, int npi, int n0, int gp, int gpl, int zper, int H) {
+                                                    int nd, int nz, int na, int npi, int n0, int gp, int gpl, int zper, int H) {
     extern __shared__ float phis[];  // [q][j]
-    const int z = blockIdx.x / n0, i = blockIdx.x % n0;
+    // one CTA per (z-group, base angle i); thread = (bin, slice of the z-group), the slices of a bin in adjacent threads, so that
+    // a bin's units (the 2 H hi / lo units of its U-unit record) are written by neighbouring lanes
+    const int zg = blockIdx.x / n0, i = blockIdx.x % n0;
     constexpr int m = 4 * Q;
     for (int t = threadIdx.x; t < npi * m; t += blockDim.x) phis[t] = phi[(int64_t)(t % m) * na + (t / m) * n0 + i];
     __syncthreads();
-    const int zg = z / zper, flat0 = (z - zg * zper) * m;         // first batch entry of this slice inside its z-group
+    const int sl = threadIdx.x % zper, z = zg * zper + sl, flat0 = sl * m;         // first batch entry of my slice inside its z-group
     const int U = 2 * H + 1;
     unsigned short *hi = reinterpret_cast<unsigned short *>(gt + ((int64_t)zg * n0 + i) * gp * U);
     unsigned short *lo = hi + H * 8;
-    for (int b = threadIdx.x; b < nd; b += blockDim.x) {
+    if (z >= nz) return;                                                            // (the scratch is zero there)
+    for (int b = threadIdx.x / zper; b < nd; b += blockDim.x / zper) {
         float acc[m];
 #pragma unroll
         for (int j = 0; j < m; ++j) acc[j] = 0.f;
@@ -343,7 +346,8 @@ cudaError_t launch_fold_split(cp4d_ctx *c, const float *g, float4 *gt) {
     const int nb = backproject_mma_nb16(d), zper = nb * 16 / d.m;
     const size_t sh = (size_t)d.npi * d.m * sizeof(float);
     uint4 *G = reinterpret_cast<uint4 *>(gt);
-    CP4D_BM_DISPATCH_Q(d.Q, (k_fold_split<QQ><<<d.nz * d.n0, 128, sh, c->stream>>>(g, G, c->phi, d.nd, d.na, d.npi, d.n0, d.gp, d.gpl, zper, 2 * nb)));
+    const int zgroups = (d.nz + zper - 1) / zper;
+    CP4D_BM_DISPATCH_Q(d.Q, (k_fold_split<QQ><<<zgroups * d.n0, 128, sh, c->stream>>>(g, G, c->phi, d.nd, d.nz, d.na, d.npi, d.n0, d.gp, d.gpl, zper, 2 * nb)));
     c->launches++;
     return cudaGetLastError();
 }
