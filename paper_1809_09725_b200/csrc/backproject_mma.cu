@@ -41,7 +41,8 @@ struct BmArgs {
 struct BmAngle {
     float cmin;    // delta + min(0, 3c) + min(0, 3s): smallest window coordinate of a block is cmin + X0 c + Y0 s
     float delta, c, s;
-    float A1, A2;  // Joseph hat in bin units: weight(bin) = max(0, A1 - A2 |u - bin|), A1 = 1/a, A2 = 1/a^2 (0, 0 for a dummy)
+    float A1, A2;  // Joseph hat in bin units, without its factor 1/a (k_fold_split applies it to the sinogram rows):
+                   // weight(bin) = sat(A1 - A2 |u - bin|), A1 = 1, A2 = 1/a (0, 0 for an angle that weighs nothing)
     int bstart;    // first bin of the tile's window at this angle
     float pad;
 };
@@ -58,7 +59,7 @@ __global__ void __launch_bounds__(128) k_bm_build(BmAngle *rec, const AngleTab *
         BmAngle R;
         R.cmin = G.delta + fminf(0.f, 3.0f * A.c) + fminf(0.f, 3.0f * A.s);
         R.delta = G.delta; R.c = A.c; R.s = A.s;
-        R.A1 = i < n0 ? A.inv_a : 0.f; R.A2 = i < n0 ? A.inv_a * A.inv_a : 0.f;
+        R.A1 = i < n0 ? 1.0f : 0.f; R.A2 = i < n0 ? A.inv_a : 0.f;
         R.bstart = G.bstart; R.pad = 0.f;
         rec[(int64_t)tile * (n0 + BM_STAGE) + i] = R;
     }
@@ -173,13 +174,14 @@ __global__ void __launch_bounds__(BM_THREADS, 1) k_backproject_mma(const uint4 *
                 // window coordinate of my voxels relative to the first bin of my half window: voxel g, and g + 8 two rows further
                 const float z00 = fmaf(fx, S0.c, fmaf(fy, S0.s, S0.delta)) - fq0, z01 = fmaf(2.0f, S0.s, z00);
                 const float z10 = fmaf(fx, S1.c, fmaf(fy, S1.s, S1.delta)) - fq1, z11 = fmaf(2.0f, S1.s, z10);
-                unsigned ah[4], al[4], nib[4];
+                unsigned ah[4], al[4];
+                float nib[4];
                 auto kept = [&](float z, float A1, float A2, int slot) {
-                    // the kept pair starts at bin i0 = clamp(floor(z), 0, 2) of the half window; Joseph hat in bin units
-                    const bool p1 = z >= 1.0f, p2 = z >= 2.0f;
-                    const float dd = z - (p2 ? 2.0f : p1 ? 1.0f : 0.0f);
-                    nib[slot] = p2 ? 14u : p1 ? 9u : 4u;
-                    split2(fmaxf(0.f, fmaf(-A2, fabsf(dd), A1)), fmaxf(0.f, fmaf(-A2, fabsf(dd - 1.0f), A1)), ah[slot], al[slot]);
+                    // the kept pair starts at bin i0 = clamp(floor(z), 0, 2) of the half window; positions (i0, i0 + 1), two bits each
+                    const float i0 = fminf(fmaxf(floorf(z), 0.0f), 2.0f);
+                    const float dd = z - i0;
+                    nib[slot] = fmaf(5.0f, i0, 4.0f);
+                    split2(__saturatef(fmaf(-A2, fabsf(dd), A1)), __saturatef(fmaf(-A2, fabsf(dd - 1.0f), A1)), ah[slot], al[slot]);
                 };
                 kept(z00, S0.A1, S0.A2, 0);      // a0: voxel g,     group t
                 kept(z01, S0.A1, S0.A2, 1);      // a1: voxel g + 8, group t
@@ -187,7 +189,7 @@ __global__ void __launch_bounds__(BM_THREADS, 1) k_backproject_mma(const uint4 *
                 kept(z11, S1.A1, S1.A2, 3);      // a3: voxel g + 8, group t + 4
                 // metadata (device_helpers.cuh): lane 4g wants the groups 0-3 (low half: voxel g, high half: voxel g + 8), lane
                 // 4g + 1 the groups 4-7; a butterfly over the quad
-                unsigned e0 = (nib[0] | (nib[1] << 16)) << (4 * t), e1 = (nib[2] | (nib[3] << 16)) << (4 * t);
+                unsigned e0 = (unsigned)__float2int_rn(fmaf(nib[1], 65536.0f, nib[0])) << (4 * t), e1 = (unsigned)__float2int_rn(fmaf(nib[3], 65536.0f, nib[2])) << (4 * t);
                 e0 |= __shfl_xor_sync(0xffffffffu, e0, 2);
                 e1 |= __shfl_xor_sync(0xffffffffu, e1, 2);
                 const unsigned e = ((t & 1) ? e1 : e0) | __shfl_xor_sync(0xffffffffu, (t & 1) ? e0 : e1, 1);
@@ -236,13 +238,14 @@ __global__ void __launch_bounds__(BM_THREADS, 1) k_backproject_mma(const uint4 *
 // written as split bf16 pairs in the layout k_backproject_mma stages.
 template <int Q>
 __global__ void __launch_bounds__(128) k_fold_split(const float *__restrict__ g, uint4 *__restrict__ gt, const float *__restrict__ phi,
-                                                    int nd, int nz, int na, int npi, int n0, int gp, int gpl, int zper, int H) {
-    extern __shared__ float phis[];  // [q][j]
+                                                    int nd, int nz, int na, int npi, int n0, int gp, int gpl, int zper, int H, const AngleTab *__restrict__ ang) {
+    extern __shared__ float phis[];  // [q][j], times the Joseph factor 1/a of the base angle (the backprojector's hat is normalised)
     // one CTA per (z-group, base angle i); thread = (bin, slice of the z-group), the slices of a bin in adjacent threads, so that
     // a bin's units (the 2 H hi / lo units of its U-unit record) are written by neighbouring lanes
     const int zg = blockIdx.x / n0, i = blockIdx.x % n0;
     constexpr int m = 4 * Q;
-    for (int t = threadIdx.x; t < npi * m; t += blockDim.x) phis[t] = phi[(int64_t)(t % m) * na + (t / m) * n0 + i];
+    const float inv_a = ang[i].inv_a;
+    for (int t = threadIdx.x; t < npi * m; t += blockDim.x) phis[t] = phi[(int64_t)(t % m) * na + (t / m) * n0 + i] * inv_a;
     __syncthreads();
     const int sl = threadIdx.x % zper, z = zg * zper + sl, flat0 = sl * m;         // first batch entry of my slice inside its z-group
     const int U = 2 * H + 1;
@@ -347,7 +350,7 @@ cudaError_t launch_fold_split(cp4d_ctx *c, const float *g, float4 *gt) {
     const size_t sh = (size_t)d.npi * d.m * sizeof(float);
     uint4 *G = reinterpret_cast<uint4 *>(gt);
     const int zgroups = (d.nz + zper - 1) / zper;
-    CP4D_BM_DISPATCH_Q(d.Q, (k_fold_split<QQ><<<zgroups * d.n0, 128, sh, c->stream>>>(g, G, c->phi, d.nd, d.nz, d.na, d.npi, d.n0, d.gp, d.gpl, zper, 2 * nb)));
+    CP4D_BM_DISPATCH_Q(d.Q, (k_fold_split<QQ><<<zgroups * d.n0, 128, sh, c->stream>>>(g, G, c->phi, d.nd, d.nz, d.na, d.npi, d.n0, d.gp, d.gpl, zper, 2 * nb, c->ang)));
     c->launches++;
     return cudaGetLastError();
 }
