@@ -478,7 +478,7 @@ def assemble(args, c, world, r):
         "config": workload_config(c, args.frames),
         "run": {"norm_K": r["L"], "projectors": {"mode": args.projectors, "forward": r["proj"][0], "adjoint": r["proj"][1]},
                 "arithmetic": ("fp32 storage, fp32 accumulation everywhere; 'tensor' projector = products of split-bf16 pairs "
-                               "(x = hi + lo, three HMMA products per term, rel. error 5e-6 per ray sum, tolerance 1e-4), "
+                               "(x = hi + lo, three products per term on the 2:4 sparse mma.sp, rel. error 5e-6 per ray sum or voxel, tolerance 1e-4), "
                                "'fp32' projector = plain FMAs (2e-6)"), "parallelism": "replicas only (independent problems, no collective)" if world > 1 else "1 gpu",
                 "warmup_run": max(args.warmup, 2),
                 "l2": f"no flush: CP state {(7 * c.V + 2 * c.S) * 4 / 1e9:.2f} GB streams through every step (L2 = 126 MB)"},

@@ -137,9 +137,9 @@ int cp4d_div(cp4d_ctx *ctx, const float *p_dev, float *f_dev);
  *       (the weight block is the sparse operand: two adjacent taps per ray and column, per voxel and angle) as split bf16 pairs (x = x_hi + x_lo with |x - x_hi - x_lo| <= 2^-17 |x|), three products per term, fp32 accumulation:
  *       relative error about 5e-6 per ray sum or voxel (bound 1.1e-5), inside the 1e-4 per-operator tolerance;
  *   fp32 kernels: CUDA-core FMAs, relative error about 2e-6.
- *   CP4D_PROJ_AUTO (default): the faster kernel of each side -- tensor-core forward projector where it applies and the
- *       problem fills the GPU (at least 148 CTAs of (tile, pass, batch group); 2.1 x the fp32 gather at config 3), fp32
- *       backprojector (the tensor-core one measured 6 % slower).
+ *   CP4D_PROJ_AUTO (default): the faster pair -- the tensor-core kernels on both sides where they apply and the problem
+ *       fills the GPU (at least 148 CTAs of (tile, pass, batch group): forward 2.1 x the fp32 gather, adjoint 1.12 x the fp32
+ *       backprojector at config 3), the fp32 kernels otherwise.
  *   CP4D_PROJ_FP32: fp32 kernels on both sides.      CP4D_PROJ_TENSOR: tensor-core kernels on both sides where they apply.
  * cp4d_fbp always uses the fp32 backprojector.  Changing the mode drops the captured CUDA graph of cp4d_iterate and clears the
  * projector scratch (asynchronously, on the context's stream). */

@@ -122,7 +122,8 @@ int forward_into(cp4d_ctx *ctx, const float *f, int mode, float sigma, const flo
     return CP4D_OK;
 }
 int adjoint_into(cp4d_ctx *ctx, const float *g, float *f) {
-    if (ctx->fw_mode == CP4D_PROJ_TENSOR && forward_mma_usable(ctx)) {     // (measured slower than the fp32 patch kernel)
+    // the tensor-core pair where it is asked for, and in auto mode where the problem fills the GPU (there it is the faster one)
+    if (forward_mma_usable(ctx) && (ctx->fw_mode == CP4D_PROJ_TENSOR || (ctx->fw_mode == CP4D_PROJ_AUTO && forward_mma_preferred(ctx->d)))) {
         CK(launch_fold_split(ctx, g, ctx->scratch), "fold");
         CK(launch_backproject_mma(ctx, ctx->scratch, ctx->d.nf ? ctx->cb : f), "backproject");
     } else {
@@ -735,7 +736,7 @@ int cp4d_projector_mode_in_use(const cp4d_ctx *ctx, int32_t *forward_out, int32_
     const bool ok = forward_mma_usable(ctx);
     const bool fw_tensor = (ctx->fw_mode == CP4D_PROJ_TENSOR && ok) || (ctx->fw_mode == CP4D_PROJ_AUTO && ok && forward_mma_preferred(ctx->d));
     if (forward_out) *forward_out = fw_tensor ? CP4D_PROJ_TENSOR : CP4D_PROJ_FP32;
-    if (adjoint_out) *adjoint_out = (ctx->fw_mode == CP4D_PROJ_TENSOR && ok) ? CP4D_PROJ_TENSOR : CP4D_PROJ_FP32;
+    if (adjoint_out) *adjoint_out = fw_tensor ? CP4D_PROJ_TENSOR : CP4D_PROJ_FP32;
     return CP4D_OK;
 }
 

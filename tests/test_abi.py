@@ -44,9 +44,9 @@ def test_workspace_bytes_counts_state(L):
         if c.m in (4, 8, 16, 32):
             # the tensor backprojector keeps it as split bf16 pairs, bin-major with one 16-byte unit of padding per bin:
             # 4 nb + 1 units per bin for groups of nb 16-entry batch blocks (whole z-groups)
-            nb = 2 if c.m == 32 else min(2, (c.nz * c.m + 15) // 16)
-            zper = nb * 16 // c.m
-            scratch = max(scratch, -(-c.nz // zper) * c.n_theta0 * (4 * nb + 1) * pitch * 16)
+            nblk = 2 if c.m == 32 else min(2, (c.nz * c.m + 15) // 16)
+            zper = nblk * 16 // c.m
+            scratch = max(scratch, -(-c.nz // zper) * c.n_theta0 * (4 * nblk + 1) * pitch * 16)
         scratch += c.nz * c.n_theta0 * c.nd * c.m * 4          # partial ray sums of the forward projector (no padding)
         # work items of the tensor forward projector, built once per context: per 32 x 32 tile, 4 x 14 items of 48 bytes
         # for each of at most n_theta0 / 4 + 8 angle groups (groups of four from 72 base angles on, pairs from 24)

@@ -62,7 +62,7 @@ def test_json_line_contract_offline():
     r = dict(ms=600.0, launches=350, prof=prof, prof_gd={"grad": (1.38, 3), "div": (1.2, 3)}, ops={"forward_op": 6.7, "adjoint_op": 3.85},
              e2e={"value": 81.0, "unit": bench.UNIT, "h2d_bytes_per_step": 1.0, "d2h_bytes_per_step": 2.0},
              clocks={"sm_mhz": 1965.0, "sm_max_mhz": 1965.0, "reasons": []}, peaks=bench.load_peaks(), L=1.0, launches_total=1,
-             graph_replays=55, fp32_alt=None, proj=("tensor", "fp32"))
+             graph_replays=55, fp32_alt=None, proj=("tensor", "tensor"))
     line = bench.assemble(A, c, 1, r)
     for k in ("metric", "value", "unit", "n_gpus", "steps", "warmup", "ms_per_step", "higher_is_better", "scaling", "vs_baseline",
               "dtype", "data", "config", "roofline", "e2e", "clocks", "gpu_launches"):
@@ -79,7 +79,7 @@ def test_json_line_contract_offline():
     # mma.sp.m16n8k32, 16 x 8 x 32 per 9.71 clk and sub-partition (profiles/r2_microbench.md)
     per_clk = 4 * 16 * 8 * 32 / 9.71
     assert rf["second_roof"]["frac"] == pytest.approx(rf["achieved"] / 2 * 12 / (148 * per_clk * r["peaks"]["sm_max_mhz"] * 1e6 / 1e12), rel=1e-6)
-    assert line["run"]["projectors"] == {"mode": "auto", "forward": "tensor", "adjoint": "fp32"}
+    assert line["run"]["projectors"] == {"mode": "auto", "forward": "tensor", "adjoint": "tensor"}
     r2 = dict(r, proj=("fp32", "fp32"))
     rf2 = bench.assemble(A, c, 1, r2)["roofline"]
     assert rf2["second_roof"]["frac"] == pytest.approx(4 * rf2["frac"] * (148 * 128 * 2 * r["peaks"]["sm_max_mhz"] * 1e6 / 1e12) / rf2["peak"], rel=1e-6)
