@@ -271,14 +271,26 @@ __global__ void __launch_bounds__(128) k_fold_split(const float *__restrict__ g,
                 }
             }
         }
-        // entries flat0 + j, j < m: 8-entry unit (flat0 + j) / 8 of the z-group, position (flat0 + j) % 8 -- in runs of 4
+        // entries flat0 + j, j < m: 8-entry unit (flat0 + j) / 8 of the z-group, position (flat0 + j) % 8 -- whole 16-byte units
+        // where the slice has 8 coefficients or more, runs of 4 otherwise
+        if constexpr (Q >= 2) {
 #pragma unroll
-        for (int jc = 0; jc < Q; ++jc) {
-            const int flat = flat0 + 4 * jc;
-            const int64_t e = ((int64_t)(gpl + b) * U + (flat >> 3)) * 8 + (flat & 7);
+            for (int jc = 0; jc < Q; jc += 2) {
+                const int flat = flat0 + 4 * jc;
+                const int64_t e = ((int64_t)(gpl + b) * U + (flat >> 3)) * 8;
+                uint4 h, l;
+                split2(acc[4 * jc], acc[4 * jc + 1], h.x, l.x);
+                split2(acc[4 * jc + 2], acc[4 * jc + 3], h.y, l.y);
+                split2(acc[4 * jc + 4], acc[4 * jc + 5], h.z, l.z);
+                split2(acc[4 * jc + 6], acc[4 * jc + 7], h.w, l.w);
+                *reinterpret_cast<uint4 *>(hi + e) = h;
+                *reinterpret_cast<uint4 *>(lo + e) = l;
+            }
+        } else {
+            const int64_t e = ((int64_t)(gpl + b) * U + (flat0 >> 3)) * 8 + (flat0 & 7);
             unsigned h01, l01, h23, l23;
-            split2(acc[4 * jc], acc[4 * jc + 1], h01, l01);
-            split2(acc[4 * jc + 2], acc[4 * jc + 3], h23, l23);
+            split2(acc[0], acc[1], h01, l01);
+            split2(acc[2], acc[3], h23, l23);
             *reinterpret_cast<uint2 *>(hi + e) = make_uint2(h01, h23);
             *reinterpret_cast<uint2 *>(lo + e) = make_uint2(l01, l23);
         }
