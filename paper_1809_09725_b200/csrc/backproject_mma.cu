@@ -26,9 +26,11 @@ namespace cp4d {
 namespace {
 
 constexpr int BM_THREADS = 512;
-constexpr int BM_STAGE = 12;                       // base angles per pipeline stage (a multiple of four: they are consumed four at a time)
-constexpr int BM_WINP = WIN + 8;                   // staged bins per angle: any 8-bin window that starts inside the tile's window
-constexpr int BM_BLOCKS = (TILE / 4) * (TILE / 4) / (BM_THREADS / 32);   // 4 x 4 voxel blocks per warp
+constexpr int BM_STAGE = 8;                        // base angles per pipeline stage (a multiple of four: they are consumed four at a time)
+constexpr int BM_WINP = 48;                        // staged bins per angle: a HALF tile (32 x 16 voxels) touches at most 31 |c| + 15 s + 3 < 38 bins,
+                                                   // and any 8-bin window that starts among them is inside
+constexpr int BM_HBLOCKS = (TILE / 4) * (TILE / 8);  // 4 x 4 voxel blocks of a half tile
+constexpr int BM_BLOCKS = BM_HBLOCKS / (BM_THREADS / 32);               // 4 x 4 voxel blocks per warp
 
 struct BmArgs {
     int n, nz, nd, n0, m, mshift, gp, gpl;
@@ -51,17 +53,21 @@ static_assert(sizeof(BmAngle) == 32, "BmAngle is two 16-byte units");
 // The angle records of every tile (they depend on the geometry only): n0 real ones and BM_STAGE that weigh nothing, so that the
 // last stage of a CTA can always be staged whole.
 __global__ void __launch_bounds__(128) k_bm_build(BmAngle *rec, const AngleTab *ang, const TileGeo *geo, int n0) {
-    const int tile = blockIdx.x;
+    const int tile = blockIdx.x, half = blockIdx.y;
     for (int i = threadIdx.x; i < n0 + BM_STAGE; i += blockDim.x) {
         const int ii = min(i, n0 - 1);
         const AngleTab A = ang[ii];
         const TileGeo G = geo[(int64_t)tile * n0 + ii];
+        // the lower half (rows 16 .. 31) starts 16 s further along the detector (s >= 0 on [0, pi)): its window starts floor(16 s)
+        // bins later, and its coordinates are taken relative to its own first row
+        const float off = 16.0f * (float)half * A.s, sh = floorf(off);
         BmAngle R;
-        R.cmin = G.delta + fminf(0.f, 3.0f * A.c) + fminf(0.f, 3.0f * A.s);
-        R.delta = G.delta; R.c = A.c; R.s = A.s;
+        R.delta = G.delta + (off - sh);
+        R.cmin = R.delta + fminf(0.f, 3.0f * A.c) + fminf(0.f, 3.0f * A.s);
+        R.c = A.c; R.s = A.s;
         R.A1 = i < n0 ? 1.0f : 0.f; R.A2 = i < n0 ? A.inv_a : 0.f;
-        R.bstart = G.bstart; R.pad = 0.f;
-        rec[(int64_t)tile * (n0 + BM_STAGE) + i] = R;
+        R.bstart = G.bstart + (int)sh; R.pad = 0.f;
+        rec[((int64_t)tile * 2 + half) * (n0 + BM_STAGE) + i] = R;
     }
 }
 
@@ -79,13 +85,13 @@ __global__ void __launch_bounds__(BM_THREADS, 1) k_backproject_mma(const uint4 *
     constexpr unsigned STAGE_BYTES = BM_STAGE * ANGLE_UNITS * 16;
     extern __shared__ __align__(128) unsigned char win[];         // [2 stages][BM_STAGE][BM_WINP][U] x 16 B
     __shared__ __align__(16) BmAngle sang[2][BM_STAGE];
-    __shared__ __align__(4) unsigned char s_q[2][(TILE / 4) * (TILE / 4)][BM_STAGE];     // first bin of the 8-bin window of (block, angle)
+    __shared__ __align__(4) unsigned char s_q[2][BM_HBLOCKS][BM_STAGE];                  // first bin of the 8-bin window of (block, angle)
     __shared__ __align__(8) uint64_t mbar[2];
     const int tiles_1d = (a.n + TILE - 1) / TILE;
     const int tile_id = blockIdx.x % a.tiles, ag = blockIdx.x / a.tiles;
-    const int zg = blockIdx.y, z0 = zg * a.zper;
-    const int tx0 = (tile_id % tiles_1d) * TILE, ty0 = (tile_id / tiles_1d) * TILE;
-    const BmAngle *rec = a.rec + (int64_t)tile_id * (a.n0 + BM_STAGE);
+    const int zg = blockIdx.y, z0 = zg * a.zper, half = blockIdx.z;
+    const int tx0 = (tile_id % tiles_1d) * TILE, ty0 = (tile_id / tiles_1d) * TILE + half * (TILE / 2);      // origin of my half tile
+    const BmAngle *rec = a.rec + ((int64_t)tile_id * 2 + half) * (a.n0 + BM_STAGE);
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, g = lane >> 2, t = lane & 3;
     // this CTA's share [g0, g1) of the base angles (small problems split them over CTAs, which then ADD into a zeroed output)
     const int g0 = (int)((int64_t)a.n0 * ag / a.agroups), g1 = (int)((int64_t)a.n0 * (ag + 1) / a.agroups);
@@ -126,12 +132,9 @@ __global__ void __launch_bounds__(BM_THREADS, 1) k_backproject_mma(const uint4 *
             mbar_wait(&mbar[buf], (st >> 1) & 1);
             const BmAngle &S = sang[buf][warp];
             const float tc = S.c, ts = S.s, tcmin = S.cmin;
-#pragma unroll
-            for (int k = 0; k < 2; ++k) {
-                const int bid = 2 * lane + k;
-                const float u = fmaf((float)(4 * (bid & 7)), tc, fmaf((float)(4 * (bid >> 3)), ts, tcmin));
-                s_q[buf][bid][warp] = (unsigned char)min(max((int)floorf(u), 0), BM_WINP - 8);
-            }
+            const int bid = lane;                                      // BM_HBLOCKS = 32 blocks: one per lane
+            const float u = fmaf((float)(4 * (bid & 7)), tc, fmaf((float)(4 * (bid >> 3)), ts, tcmin));
+            s_q[buf][bid][warp] = (unsigned char)min(max((int)floorf(u), 0), BM_WINP - 8);
         }
     };
 
@@ -303,14 +306,14 @@ cudaError_t bm_launch(cp4d_ctx *c, const uint4 *gt, float *out, BmArgs a) {
     a.zper = NB16 * 16 / d.m;
     const int zgroups = (d.nz + a.zper - 1) / a.zper;
     // small problems: split the base angles over up to 8 CTAs per tile, which add their partial sums into a zeroed output
-    const int64_t ctas = (int64_t)d.tiles * zgroups;
+    const int64_t ctas = (int64_t)d.tiles * 2 * zgroups;
     a.agroups = (int)std::max<int64_t>(1, std::min<int64_t>(std::min(8, std::max(1, d.n0 / BM_STAGE)), 148 / ctas));
     if (a.agroups > 1) {
         const cudaError_t e = cudaMemsetAsync(out, 0, (size_t)d.nz * d.n * d.n * d.m * sizeof(float), c->stream);
         if (e != cudaSuccess) return e;
         c->launches++;
     }
-    const dim3 grid(d.tiles * a.agroups, zgroups);
+    const dim3 grid(d.tiles * a.agroups, zgroups, 2);
     k_backproject_mma<NB16><<<grid, BM_THREADS, (size_t)2 * BM_STAGE * (4 * NB16 + 1) * BM_WINP * 16, c->stream>>>(gt, out, a);
     return cudaGetLastError();
 }
@@ -328,7 +331,7 @@ cudaError_t bm_launch(cp4d_ctx *c, const uint4 *gt, float *out, BmArgs a) {
 // 16-entry batch blocks per CTA of the tensor-core backprojector (also fixes the layout k_fold_split writes)
 int backproject_mma_nb16(const Dims &d) {
     const int blocks_total = (d.nz * d.m + 15) / 16;
-    return d.m == 32 ? 2 : std::min(2, blocks_total);
+    return blocks_total >= 4 ? 4 : blocks_total >= 2 ? 2 : 1;      // (m = 32: the blocks of a slice come in pairs, so 2 or 4)
 }
 
 // 16-byte units of gt in the split layout (>= what the fp32 layout of the same scratch needs when nz is a multiple of zper)
@@ -339,20 +342,22 @@ int64_t backproject_mma_scratch_units(const Dims &d) {
 
 // bytes of the per-(tile, angle) records of a context (0 if the shape is not supported)
 uint64_t backproject_mma_rec_bytes(const Dims &d) {
-    return forward_mma_supported(d) ? (uint64_t)d.tiles * (d.n0 + BM_STAGE) * sizeof(BmAngle) : 0;
+    return forward_mma_supported(d) ? (uint64_t)d.tiles * 2 * (d.n0 + BM_STAGE) * sizeof(BmAngle) : 0;
 }
 
 // cp4d_create: the angle records of every tile, once (they depend on the geometry only)
 cudaError_t backproject_mma_build(cp4d_ctx *c) {
     if (!c->bm_rec) return cudaSuccess;
-    k_bm_build<<<c->d.tiles, 128, 0, c->stream>>>(reinterpret_cast<BmAngle *>(c->bm_rec), c->ang, c->geo, c->d.n0);
+    k_bm_build<<<dim3(c->d.tiles, 2), 128, 0, c->stream>>>(reinterpret_cast<BmAngle *>(c->bm_rec), c->ang, c->geo, c->d.n0);
     return cudaGetLastError();
 }
 
 cudaError_t backproject_mma_init() {
     cudaError_t e = cudaFuncSetAttribute(k_backproject_mma<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, 2 * BM_STAGE * (4 * 1 + 1) * BM_WINP * 16);
     if (e != cudaSuccess) return e;
-    return cudaFuncSetAttribute(k_backproject_mma<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, 2 * BM_STAGE * (4 * 2 + 1) * BM_WINP * 16);
+    e = cudaFuncSetAttribute(k_backproject_mma<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, 2 * BM_STAGE * (4 * 2 + 1) * BM_WINP * 16);
+    if (e != cudaSuccess) return e;
+    return cudaFuncSetAttribute(k_backproject_mma<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, 2 * BM_STAGE * (4 * 4 + 1) * BM_WINP * 16);
 }
 
 cudaError_t launch_fold_split(cp4d_ctx *c, const float *g, float4 *gt) {
@@ -375,8 +380,11 @@ cudaError_t launch_backproject_mma(cp4d_ctx *c, const float4 *gt, float *f_out) 
     BmArgs a{d.n, d.nz, d.nd, d.n0, d.m, ms, d.gp, d.gpl, d.tiles, 1, 0, reinterpret_cast<const BmAngle *>(c->bm_rec)};
     c->launches++;
     const uint4 *G = reinterpret_cast<const uint4 *>(gt);
-    if (backproject_mma_nb16(d) == 1) return bm_launch<1>(c, G, f_out, a);
-    return bm_launch<2>(c, G, f_out, a);
+    switch (backproject_mma_nb16(d)) {
+    case 1: return bm_launch<1>(c, G, f_out, a);
+    case 2: return bm_launch<2>(c, G, f_out, a);
+    default: return bm_launch<4>(c, G, f_out, a);
+    }
 }
 
 }  // namespace cp4d

@@ -44,7 +44,8 @@ def test_workspace_bytes_counts_state(L):
         if c.m in (4, 8, 16, 32):
             # the tensor backprojector keeps it as split bf16 pairs, bin-major with one 16-byte unit of padding per bin:
             # 4 nb + 1 units per bin for groups of nb 16-entry batch blocks (whole z-groups)
-            nblk = 2 if c.m == 32 else min(2, (c.nz * c.m + 15) // 16)
+            blocks = (c.nz * c.m + 15) // 16
+            nblk = 4 if blocks >= 4 else 2 if blocks >= 2 else 1
             zper = nblk * 16 // c.m
             scratch = max(scratch, -(-c.nz // zper) * c.n_theta0 * (4 * nblk + 1) * pitch * 16)
         scratch += c.nz * c.n_theta0 * c.nd * c.m * 4          # partial ray sums of the forward projector (no padding)
@@ -53,7 +54,7 @@ def test_workspace_bytes_counts_state(L):
         gs = 4 if c.n_theta0 >= 72 else 2 if c.n_theta0 >= 24 else 1
         tiles = ((c.n + 31) // 32) ** 2
         scratch += tiles * 4 * 14 * (c.n_theta0 // gs + 8) * 48
-        scratch += tiles * (c.n_theta0 + 12) * 32              # angle records of the tensor backprojector per (tile, angle)
+        scratch += tiles * 2 * (c.n_theta0 + 8) * 32           # angle records of the tensor backprojector per (half tile, angle)
         assert state + scratch <= nb <= state + scratch + (64 << 20)
     c = synth.CONFIGS[5]
     assert binding.workspace_bytes(c.n, c.nz, c.nd, c.n_angles, c.n_half_rot, c.m) < 170e9   # fits 180 GB HBM
