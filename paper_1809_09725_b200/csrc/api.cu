@@ -55,7 +55,7 @@ int validate(const cp4d_params *p, Dims *d) {
 }
 
 struct Carve {
-    uint64_t f, ft, bp, h2, h1, g, tmp_s, scratch, psum, phi, ang, geo, red, cf, cb, psi, fwang, fworder, fwpairs, fwitems, fwcounts, bmrec, total;
+    uint64_t f, ft, bp, h2, h1, g, tmp_s, scratch, psum, phi, ang, geo, red, cf, cb, psi, fwang, fworder, fwpairs, fwitems, fwcounts, bmrec, bmorder, total;
 };
 Carve carve(const Dims &d) {
     Carve c;
@@ -69,7 +69,7 @@ Carve carve(const Dims &d) {
     c.fwang = take((uint64_t)d.n0 * sizeof(FwAngle)); c.fworder = take((uint64_t)d.n0 * 4);
     c.fwpairs = take((uint64_t)d.n0 * sizeof(int4));
     c.fwitems = take(forward_mma_item_bytes(d)); c.fwcounts = take((uint64_t)d.tiles * 2 * sizeof(int2));
-    c.bmrec = take(backproject_mma_rec_bytes(d));
+    c.bmrec = take(backproject_mma_rec_bytes(d)); c.bmorder = take((uint64_t)d.tiles * sizeof(int));
     c.cf = c.cb = c.psi = 0;
     if (d.nf) { c.cf = take(d.Vc * 4); c.cb = take(d.Vc * 4); c.psi = take((uint64_t)d.mb * d.nf * 4); }
     c.total = o;
@@ -201,7 +201,7 @@ int cp4d_create(const cp4d_params *p, cp4d_ctx **out) {
     ctx->fwang = (FwAngle *)(w + cv.fwang); ctx->fworder = (int32_t *)(w + cv.fworder);
     ctx->fw_groups = (int4 *)(w + cv.fwpairs); ctx->fw_mode = CP4D_PROJ_AUTO;
     ctx->fw_items = forward_mma_item_bytes(d) ? (unsigned *)(w + cv.fwitems) : nullptr; ctx->fw_counts = (int2 *)(w + cv.fwcounts);
-    ctx->bm_rec = backproject_mma_rec_bytes(d) ? (void *)(w + cv.bmrec) : nullptr;
+    ctx->bm_rec = backproject_mma_rec_bytes(d) ? (void *)(w + cv.bmrec) : nullptr; ctx->bm_order = (int *)(w + cv.bmorder);
     ctx->cf = d.nf ? (float *)(w + cv.cf) : nullptr; ctx->cb = d.nf ? (float *)(w + cv.cb) : nullptr;
     ctx->psi = d.nf ? (float *)(w + cv.psi) : nullptr;
     ctx->scratch = (float4 *)(w + cv.scratch); ctx->psum = (float4 *)(w + cv.psum); ctx->phi = (float *)(w + cv.phi);
@@ -269,6 +269,8 @@ int cp4d_create(const cp4d_params *p, cp4d_ctx **out) {
             for (int j = 0; j < d.mb; ++j) acc += (double)p->phi_host[(size_t)j * d.na + (size_t)r * fstride] * (double)p->phi_host[(size_t)j * d.na + k];
             phi_eff[(size_t)r * d.na + k] = (float)acc;
         }
+    std::vector<int> bmorder(d.tiles);
+    backproject_mma_order((d.n + TILE - 1) / TILE, bmorder.data());
     cudaError_t e;
     if ((d.nf && (e = cudaMemcpyAsync(ctx->psi, psi.data(), psi.size() * 4, cudaMemcpyHostToDevice, ctx->stream)) != cudaSuccess) ||
         (e = cudaMemcpyAsync(ctx->phi, phi_eff.data(), (size_t)d.m * d.na * 4, cudaMemcpyHostToDevice, ctx->stream)) != cudaSuccess ||
@@ -276,6 +278,7 @@ int cp4d_create(const cp4d_params *p, cp4d_ctx **out) {
         (e = cudaMemcpyAsync(ctx->fwang, fwang.data(), fwang.size() * sizeof(FwAngle), cudaMemcpyHostToDevice, ctx->stream)) != cudaSuccess ||
         (e = cudaMemcpyAsync(ctx->fworder, fworder.data(), fworder.size() * 4, cudaMemcpyHostToDevice, ctx->stream)) != cudaSuccess ||
         (e = cudaMemcpyAsync(ctx->fw_groups, fwpairs.data(), fwpairs.size() * sizeof(int4), cudaMemcpyHostToDevice, ctx->stream)) != cudaSuccess ||
+        (e = cudaMemcpyAsync(ctx->bm_order, bmorder.data(), bmorder.size() * sizeof(int), cudaMemcpyHostToDevice, ctx->stream)) != cudaSuccess ||
         (e = cudaMemcpyAsync(ctx->geo, geo.data(), geo.size() * sizeof(TileGeo), cudaMemcpyHostToDevice, ctx->stream)) != cudaSuccess ||
         (e = cudaMemsetAsync(ctx->scratch, 0, (size_t)d.scratch4 * 16, ctx->stream)) != cudaSuccess ||
         (e = forward_mma_build(ctx)) != cudaSuccess ||

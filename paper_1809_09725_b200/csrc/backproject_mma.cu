@@ -36,7 +36,8 @@ struct BmArgs {
     int n, nz, nd, n0, m, mshift, gp, gpl;
     int tiles, agroups;
     int zper;                                      // slices per CTA = NB16 * 16 / m
-    const struct BmAngle *rec;                      // [tile][n0 + BM_STAGE] angle records, built once per context by k_bm_build
+    const struct BmAngle *rec;                      // [tile][half][n0 + BM_STAGE] angle records, built once per context by k_bm_build
+    const int *order;                               // tile of the i-th CTA of a launch row: bands of 8 tile rows, column by column
 };
 
 // per (tile, base angle): built once per context, staged by TMA (shared memory, broadcast loads)
@@ -88,7 +89,9 @@ __global__ void __launch_bounds__(BM_THREADS, 1) k_backproject_mma(const uint4 *
     __shared__ __align__(4) unsigned char s_q[2][BM_HBLOCKS][BM_STAGE];                  // first bin of the 8-bin window of (block, angle)
     __shared__ __align__(8) uint64_t mbar[2];
     const int tiles_1d = (a.n + TILE - 1) / TILE;
-    const int tile_id = blockIdx.x % a.tiles, ag = blockIdx.x / a.tiles;
+    // CTAs that run at the same time should stage neighbouring windows (the folded sinogram of a z-group does not fit L2 at the
+    // large configs): consecutive block indices walk the tiles in bands of 8 tile rows, column by column (a.order, host-made)
+    const int ag = blockIdx.x / a.tiles, tile_id = a.order[blockIdx.x % a.tiles];
     const int zg = blockIdx.y, z0 = zg * a.zper, half = blockIdx.z;
     const int tx0 = (tile_id % tiles_1d) * TILE, ty0 = (tile_id / tiles_1d) * TILE + half * (TILE / 2);      // origin of my half tile
     const BmAngle *rec = a.rec + ((int64_t)tile_id * 2 + half) * (a.n0 + BM_STAGE);
@@ -345,6 +348,16 @@ uint64_t backproject_mma_rec_bytes(const Dims &d) {
     return forward_mma_supported(d) ? (uint64_t)d.tiles * 2 * (d.n0 + BM_STAGE) * sizeof(BmAngle) : 0;
 }
 
+// host: the order in which a launch walks the tiles
+void backproject_mma_order(int tiles_1d, int *order) {
+    int k = 0;
+    for (int band = 0; band * 8 < tiles_1d; ++band) {
+        const int rows = std::min(8, tiles_1d - 8 * band);
+        for (int tx = 0; tx < tiles_1d; ++tx)
+            for (int r = 0; r < rows; ++r) order[k++] = (8 * band + r) * tiles_1d + tx;
+    }
+}
+
 // cp4d_create: the angle records of every tile, once (they depend on the geometry only)
 cudaError_t backproject_mma_build(cp4d_ctx *c) {
     if (!c->bm_rec) return cudaSuccess;
@@ -377,7 +390,7 @@ cudaError_t launch_backproject_mma(cp4d_ctx *c, const float4 *gt, float *f_out) 
     const Dims &d = c->d;
     int ms = 0;
     while ((1 << ms) < d.m) ++ms;
-    BmArgs a{d.n, d.nz, d.nd, d.n0, d.m, ms, d.gp, d.gpl, d.tiles, 1, 0, reinterpret_cast<const BmAngle *>(c->bm_rec)};
+    BmArgs a{d.n, d.nz, d.nd, d.n0, d.m, ms, d.gp, d.gpl, d.tiles, 1, 0, reinterpret_cast<const BmAngle *>(c->bm_rec), c->bm_order};
     c->launches++;
     const uint4 *G = reinterpret_cast<const uint4 *>(gt);
     switch (backproject_mma_nb16(d)) {

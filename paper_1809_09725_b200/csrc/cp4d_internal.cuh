@@ -83,6 +83,7 @@ struct cp4d_ctx {
     int n_groups0, n_groups1;
     unsigned *fw_items;        // its work items per (tile, pass), built once by cp4d_create (forward_mma_build); null if the shape is not supported
     int2 *fw_counts;           // [tile][pass]: (long, short) items
+    int *bm_order;             // its tile order (backproject_mma_order), tiles ints
     void *bm_rec;              // tensor-core backprojector (backproject_mma.cu): angle records per (tile, angle), built once by cp4d_create; null if unsupported
     int fw_mode;               // CP4D_PROJ_AUTO / _FP32 (cp4d_set_projector_mode): both projectors
     int n_cpos;                // the first n_cpos base angles have cos >= 0 (backprojector: chunks never mix the signs)
@@ -148,6 +149,7 @@ bool forward_mma_usable(const cp4d_ctx *c);       // supported shape and the gro
 cudaError_t forward_mma_build(cp4d_ctx *c);       // cp4d_create: builds the work items
 uint64_t backproject_mma_rec_bytes(const Dims &d);  // workspace bytes of the tensor backprojector's angle records (0 if unsupported)
 cudaError_t backproject_mma_build(cp4d_ctx *c);     // cp4d_create: builds them
+void backproject_mma_order(int tiles_1d, int *order);  // host: tile order of a launch, tiles_1d^2 entries
 // backproject_mma.cu: the tensor-core adjoint (fold into split-bf16 rows + backprojection); same shapes as forward_mma
 int backproject_mma_nb16(const Dims &d);
 int64_t backproject_mma_scratch_units(const Dims &d);
