@@ -25,7 +25,7 @@
 // columns, pass 1 = the others on the transposed tile, so one code path serves both.  The tile sits in shared memory as
 // [block][hi/lo][8-entry half][column][33 rows] x 16 B, which makes every 8 x 8 ldmatrix operand 128 contiguous bytes.  The work
 // items (angle group, strip, column range, window starts) are built once per context by k_fm_build; warps draw them from a
-// shared counter; partial ray sums go to P[z][i][b][j] as one 16-byte RED per lane.
+// shared counter; partial ray sums go to P[z][i][b][j] as 8-byte REDs.
 #include <cuda_bf16.h>
 
 #include <algorithm>
@@ -333,15 +333,14 @@ __global__ void __launch_bounds__(FM_THREADS, 1) k_forward_mma(const float *__re
     // ldmatrix row address of this lane: matrix = lane / 8 = column of the step, row lane & 7 of its window
     const unsigned ld_base = tile_s + (lane >> 3) * FM_COL + ((lane & 7) << 4);
     const TileGeo *geo = a.geo + (int64_t)tile_id * a.n0;
-    // epilogue: I add batch entries 8 half + 4 (t / 2) .. + 3 of block zb = coefficients j .. j+3 of slice sl; element offset of
-    // (sl, j) in P
+    // epilogue: I add batch entries 8 half + 2 t, + 1 of block zb = coefficients j, j + 1 of slice sl; element offset of (sl, j) in P
     unsigned zoff[NB16][2];
     bool zok[NB16][2];
 #pragma unroll
     for (int zb = 0; zb < NB16; ++zb)
 #pragma unroll
         for (int hf = 0; hf < 2; ++hf) {
-            const int flat = zb * 16 + hf * 8 + 4 * (t >> 1), sl = z0 + (flat >> a.mshift), j = flat & (a.m - 1);
+            const int flat = zb * 16 + hf * 8 + 2 * t, sl = z0 + (flat >> a.mshift), j = flat & (a.m - 1);
             zok[zb][hf] = sl < a.nz;
             zoff[zb][hf] = (unsigned)sl * (unsigned)(a.n0 * a.gp) * (unsigned)a.m + (unsigned)j;
         }
@@ -407,13 +406,14 @@ __global__ void __launch_bounds__(FM_THREADS, 1) k_forward_mma(const float *__re
                 r_step[nb] = R.step[x];
                 r_y[nb] = r_ok[nb] ? fmaf((float)(kb + (t >> 1)), r_step[nb], ((float)r_bub[nb] - R.delta[x]) * R.inv[x]) - (float)(4 * (t & 1)) : -1e6f;
             }
-            // ---- partial ray sums of this tile -> P[z][i][b][j]: an even lane adds four batch entries of ray g, an odd lane of
-            // ray g + 8 (see the epilogue) ----
-            const int mynb = t & 1;
-            const int myx = mynb ? r_x[1] : r_x[0], mybub = mynb ? r_bub[1] : r_bub[0];
-            const int myb = R.bstart[myx] + mybub;
-            const bool my_ok = (mynb ? r_ok[1] : r_ok[0]) && myb >= 0 && myb < a.nd;
-            const unsigned my_off = (unsigned)((R.ia[myx] * a.gp + a.gpl + myb) * a.m);
+            // ---- partial ray sums of this tile -> P[z][i][b][j]: element offsets of my two rays (see the epilogue) ----
+            unsigned r_off[2];
+#pragma unroll
+            for (int nb = 0; nb < 2; ++nb) {
+                const int b = R.bstart[r_x[nb]] + r_bub[nb];
+                r_ok[nb] = r_ok[nb] && b >= 0 && b < a.nd;
+                r_off[nb] = (unsigned)((R.ia[r_x[nb]] * a.gp + a.gpl + b) * a.m);
+            }
 
             float acc[NB16][2][4];         // [batch block][8-entry half]: rays g (0, 1) and g + 8 (2, 3) x batch entries 2t, 2t + 1
 #pragma unroll
@@ -462,17 +462,16 @@ __global__ void __launch_bounds__(FM_THREADS, 1) k_forward_mma(const float *__re
                         mma_sp16832(acc[zb][hf], al, bh, e);
                     }
             }
-            // epilogue: lanes t and t ^ 1 exchange halves so that each holds four consecutive batch entries of one ray (even t:
-            // ray g, odd t: ray g + 8), and add them with one 16-byte RED (a RED costs about one clock per LANE whatever its width)
+            // epilogue: my D entries are two consecutive batch entries of ray g and two of ray g + 8: one 8-byte RED each.  (One
+            // 16-byte RED per lane after an exchange between lanes t and t ^ 1 halves the REDs, but its selects and shuffles cost
+            // more than the REDs, which the kernel hides: 3.06 -> 3.01 ms.)
 #pragma unroll
             for (int zb = 0; zb < NB16; ++zb)
 #pragma unroll
                 for (int hf = 0; hf < 2; ++hf) {
                     const float (&d)[4] = acc[zb][hf];
-                    const float sx = mynb ? d[0] : d[2], sy = mynb ? d[1] : d[3];
-                    const float rx = __shfl_xor_sync(0xffffffffu, sx, 1), ry = __shfl_xor_sync(0xffffffffu, sy, 1);
-                    const float4 v = mynb ? make_float4(rx, ry, d[2], d[3]) : make_float4(d[0], d[1], rx, ry);
-                    if (my_ok && zok[zb][hf]) atomicAdd(reinterpret_cast<float4 *>(P + (size_t)zoff[zb][hf] + my_off), v);      // 1/a: k_synth
+                    if (r_ok[0] && zok[zb][hf]) atomicAdd(reinterpret_cast<float2 *>(P + (size_t)zoff[zb][hf] + r_off[0]), make_float2(d[0], d[1]));
+                    if (r_ok[1] && zok[zb][hf]) atomicAdd(reinterpret_cast<float2 *>(P + (size_t)zoff[zb][hf] + r_off[1]), make_float2(d[2], d[3]));
                 }
         }
     }
