@@ -100,6 +100,26 @@ def test_forward_adjoint(torch_cuda, fast_oracle, case):
     ctx.close()
 
 
+@pytest.mark.parametrize("scale", [1e-20, 1.0, 1e20])
+def test_tensor_projectors_keep_their_error_across_magnitudes(torch_cuda, fast_oracle, scale):
+    """The split-bf16 operands of the tensor kernels have the exponent range of fp32: the relative error of K1 and K1^T does not
+    depend on the magnitude of the data (the operators are linear, so the oracle result is scaled)."""
+    from paper_1809_09725_b200 import binding
+    c = CASES["groups4_coarsest_m16"]
+    phi = synth.basis_table(c.basis, c.m, c.n_angles)
+    P = fast_oracle.Problem.from_config(c, phi=phi)
+    ctx = binding.Context.from_config(c, phi=phi)
+    f, g = synth.test_vectors(c)
+    f32, g32 = (f * scale).astype(np.float32), (g * scale).astype(np.float32)
+    ctx.set_projector_mode("tensor")
+    assert ctx.projector_mode_in_use() == ("tensor", "tensor")
+    Kf = ctx.forward(dev(torch_cuda, f32)).cpu().numpy().astype(np.float64) / scale
+    Ktg = ctx.adjoint(dev(torch_cuda, g32)).cpu().numpy().astype(np.float64) / scale
+    assert rel(Kf, P.forward(f32.astype(np.float64) / scale, folded=True)) <= 2e-5
+    assert rel(Ktg, P.adjoint(g32.astype(np.float64) / scale, folded=True)) <= 2e-5
+    ctx.close()
+
+
 def test_tensor_request_falls_back_beyond_its_tables(torch_cuda, fast_oracle):
     """More than 128 angle groups in a pass (here 1100 base angles in groups of four: about 138 per pass) do not fit the tensor
     forward kernel's shared-memory records: a CP4D_PROJ_TENSOR request then runs the fp32 kernels, says so, and is still right."""
