@@ -96,6 +96,16 @@ typedef struct {
  * as well).
  * Host only; ignores workspace_dev/stream/phi_host.  Errors: CP4D_EINVAL (see cp4d_params). */
 int cp4d_workspace_bytes(const cp4d_params *p, uint64_t *bytes_out);
+/* The same plus second copies of h2[4] and f~ (5 * V floats more).  A context created on a workspace of at least this size
+ * (whole volume, z_open == 0) runs steps 4-6 of Fig. 2 as ONE pass over the volume -- the dual variable
+ * goes from its projection to the divergence of the primal update through shared memory, 13 V instead of 17 V floats of HBM
+ * traffic per iteration -- which needs the two arrays double-buffered: a CTA recomputes the projection
+ * on a one-voxel halo from the OLD values while its neighbour writes the new ones.  cp4d_iterate then swaps the roles of the
+ * copies after every iteration (see cp4d_state_ptrs).  The iterates are those of the two-kernel path. */
+int cp4d_workspace_bytes_fused(const cp4d_params *p, uint64_t *bytes_out);
+/* *out_host = 1 if cp4d_iterate of this context runs the one-pass step (workspace >= cp4d_workspace_bytes_fused at create and
+ * z_open == 0), else 0 */
+int cp4d_fused_step_in_use(const cp4d_ctx *ctx, int32_t *out_host);
 
 /* Validate, compute the fp64 angle/tile tables on the host, copy them and phi into the workspace,
  * carve the workspace.  Launches one kernel on the stream (the work items of the tensor-core forward projector, which depend
@@ -180,7 +190,8 @@ int cp4d_reset(cp4d_ctx *ctx, const float *f0_dev /* nullable => zeros */); /* f
 int cp4d_iterate(cp4d_ctx *ctx, int32_t n_iters);                     /* n_iters x steps 3-6, async */
 int cp4d_get_f(cp4d_ctx *ctx, float *f_dev_out);                      /* copy f (V) */
 /* device pointers of the state arrays inside the workspace (for inspection / teacher forcing);
- * any of the out pointers may be null. */
+ * any of the out pointers may be null.  With the one-pass step (cp4d_fused_step_in_use) ft and h2 alternate between their two
+ * copies: the pointers are those of the CURRENT state and stay valid until the next cp4d_iterate. */
 int cp4d_state_ptrs(cp4d_ctx *ctx, float **f, float **ft, float **h1, float **h2, float **g);
 
 /* ---- convergence monitor (off the timed path).  Syncs. ---------------------------------------- */
@@ -226,7 +237,8 @@ int cp4d_sync(cp4d_ctx *ctx);
 /* number of kernels (and memset nodes) this context has enqueued since create */
 int cp4d_launch_count(const cp4d_ctx *ctx, uint64_t *count_out);
 /* cp4d_iterate(n >= 2) on a capturable stream (any stream but the legacy default stream 0) captures one iteration of
- * Fig. 2 into a CUDA graph on first use and replays it n times; the graph is rebuilt when cp4d_set_steps changes tau or
+ * Fig. 2 into a CUDA graph on first use and replays it n times (with the one-pass step: TWO iterations, after which the
+ * double-buffered arrays are back in their roles, replayed n / 2 times; an odd iteration is launched directly); the graph is rebuilt when cp4d_set_steps changes tau or
  * sigma, and it is bypassed while cp4d_profile_begin is active (the per-kernel events sit between the launches) and on
  * stream 0, where the launches are issued one by one.  count_out: graph replays since create (each one is counted in
  * cp4d_launch_count with the number of kernels and memset nodes of one iteration). */
@@ -249,7 +261,8 @@ const char *cp4d_graph_note(const cp4d_ctx *ctx);
 #define CP4D_K_REDUCE      8
 #define CP4D_K_MISC        9
 #define CP4D_K_MIX        10  /* frame mode: per-voxel frame <-> coefficient contraction (L231-L237)           */
-#define CP4D_K_COUNT      11
+#define CP4D_K_PROX_UPDATE 11 /* steps 4-6 in one pass (cp4d_workspace_bytes_fused)                              */
+#define CP4D_K_COUNT      12
 typedef struct {
     double   ms[CP4D_K_COUNT];        /* summed device time of the class since cp4d_profile_begin       */
     uint64_t launches[CP4D_K_COUNT];  /* timed launches of the class                                      */

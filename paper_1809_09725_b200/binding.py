@@ -33,7 +33,7 @@ class Params(C.Structure):
                 ("stream", C.c_void_p), ("n_frames", C.c_int32), ("z_open", C.c_int32)]
 
 
-K_COUNT = 11
+K_COUNT = 12
 
 
 class Profile(C.Structure):
@@ -51,6 +51,8 @@ def lib():
         vp, f32, i32, u64 = C.c_void_p, C.c_float, C.c_int32, C.c_uint64
         sig = {
             "cp4d_workspace_bytes": [C.POINTER(Params), C.POINTER(u64)],
+            "cp4d_workspace_bytes_fused": [C.POINTER(Params), C.POINTER(u64)],
+            "cp4d_fused_step_in_use": [vp, C.POINTER(i32)],
             "cp4d_create": [C.POINTER(Params), C.POINTER(vp)],
             "cp4d_destroy": [vp],
             "cp4d_forward": [vp, vp, vp], "cp4d_forward_static": [vp, vp, vp], "cp4d_adjoint": [vp, vp, vp], "cp4d_grad": [vp, vp, vp], "cp4d_div": [vp, vp, vp],
@@ -96,10 +98,11 @@ def make_params(n, nz, nd, n_angles, n_half_rot, m, phi=None, lambda1=1e-3, lamb
     return p
 
 
-def workspace_bytes(n, nz, nd, n_angles, n_half_rot, m, n_frames=0) -> int:
+def workspace_bytes(n, nz, nd, n_angles, n_half_rot, m, n_frames=0, fused=False) -> int:
+    """cp4d_workspace_bytes, or with fused=True cp4d_workspace_bytes_fused (second copies of h2 and ft for the one-pass step)."""
     out = C.c_uint64(0)
     p = make_params(n, nz, nd, n_angles, n_half_rot, m, n_frames=n_frames)
-    r = lib().cp4d_workspace_bytes(C.byref(p), C.byref(out))
+    r = (lib().cp4d_workspace_bytes_fused if fused else lib().cp4d_workspace_bytes)(C.byref(p), C.byref(out))
     if r:
         raise Cp4dError(r, lib().cp4d_strerror(r).decode())
     return out.value
@@ -109,7 +112,7 @@ class Context:
     """One reconstruction problem on one GPU.  Tensors are torch CUDA float32, contiguous, layouts of cp4d.h."""
 
     def __init__(self, n, nz, nd, n_angles, n_half_rot, m, phi, lambda1=1e-3, lambda2=1.0, theta=1.0, device=0, n_frames=0,
-                 z_open=0):
+                 z_open=0, fused=False):
         import torch
         self.torch = torch
         self.n, self.nz, self.nd, self.n_angles, self.n_half_rot, self.m = n, nz, nd, n_angles, n_half_rot, m
@@ -119,7 +122,8 @@ class Context:
         self.V, self.S = nz * n * n * mp, nz * n_angles * nd
         self.device = torch.device("cuda", device)
         self._phi = np.ascontiguousarray(phi, dtype=np.float32).reshape(m, n_angles)
-        nbytes = workspace_bytes(n, nz, nd, n_angles, n_half_rot, m, n_frames)
+        # fused=True: a workspace with room for the one-pass step of cp4d_iterate (5 V floats more; whole-volume contexts only)
+        nbytes = workspace_bytes(n, nz, nd, n_angles, n_half_rot, m, n_frames, fused=bool(fused) and not z_open)
         with torch.cuda.device(self.device):
             self.workspace = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
             base = (self.workspace.data_ptr() + 255) // 256 * 256
@@ -302,6 +306,11 @@ class Context:
         out = C.c_uint64(0)
         self._ck(lib().cp4d_launch_count(self._h, C.byref(out)))
         return out.value
+
+    def fused_step_in_use(self) -> bool:
+        out = C.c_int32(0)
+        self._ck(lib().cp4d_fused_step_in_use(self._h, C.byref(out)))
+        return bool(out.value)
 
     def graph_replays(self) -> int:
         """CUDA-graph replays of one CP iteration issued by iterate() so far (0 on the legacy default stream)."""

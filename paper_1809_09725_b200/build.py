@@ -10,7 +10,7 @@ PKG = Path(__file__).resolve().parent
 ROOT = PKG.parent
 CSRC = PKG / "csrc"
 LIB = PKG / "libcp4d.so"
-SOURCES = ["api.cu", "stream_kernels.cu", "projectors.cu", "forward_mma.cu", "backproject.cu", "backproject_mma.cu", "forward_static.cu"]
+SOURCES = ["api.cu", "stream_kernels.cu", "projectors.cu", "forward_mma.cu", "backproject.cu", "backproject_mma.cu", "forward_static.cu", "fused_step.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC,-O2", "-Xptxas", "-v", "--expt-relaxed-constexpr"]
 

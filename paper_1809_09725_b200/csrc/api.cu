@@ -55,9 +55,10 @@ int validate(const cp4d_params *p, Dims *d) {
 }
 
 struct Carve {
+    uint64_t ft_alt, h2_alt;
     uint64_t f, ft, bp, h2, h1, g, tmp_s, scratch, psum, phi, ang, geo, red, cf, cb, psi, fwang, fworder, fwpairs, fwitems, fwcounts, bmrec, bmorder, total;
 };
-Carve carve(const Dims &d) {
+Carve carve(const Dims &d, bool fused = false) {
     Carve c;
     uint64_t o = 0;
     auto take = [&](uint64_t bytes) { uint64_t r = o; o += up(bytes); return r; };
@@ -72,6 +73,8 @@ Carve carve(const Dims &d) {
     c.bmrec = take(backproject_mma_rec_bytes(d)); c.bmorder = take((uint64_t)d.tiles * sizeof(int));
     c.cf = c.cb = c.psi = 0;
     if (d.nf) { c.cf = take(d.Vc * 4); c.cb = take(d.Vc * 4); c.psi = take((uint64_t)d.mb * d.nf * 4); }
+    c.ft_alt = c.h2_alt = 0;
+    if (fused) { c.ft_alt = take(d.V * 4); c.h2_alt = take(d.V * 16); }
     c.total = o;
     return c;
 }
@@ -166,6 +169,21 @@ int cp4d_workspace_bytes(const cp4d_params *p, uint64_t *out) {
     return CP4D_OK;
 }
 
+int cp4d_workspace_bytes_fused(const cp4d_params *p, uint64_t *out) {
+    Dims d;
+    if (!out) return CP4D_EINVAL;
+    int r = validate(p, &d);
+    if (r) return r;
+    *out = carve(d, true).total;
+    return CP4D_OK;
+}
+
+int cp4d_fused_step_in_use(const cp4d_ctx *ctx, int32_t *out) {
+    if (!ctx || !out) return CP4D_EINVAL;
+    *out = ctx->fused ? 1 : 0;
+    return CP4D_OK;
+}
+
 int cp4d_create(const cp4d_params *p, cp4d_ctx **out) {
     if (!out) return CP4D_EINVAL;
     *out = nullptr;
@@ -173,7 +191,9 @@ int cp4d_create(const cp4d_params *p, cp4d_ctx **out) {
     int r = validate(p, &d);
     if (r) return r;
     if (!p->phi_host) return CP4D_EINVAL;
-    const Carve cv = carve(d);
+    // a whole-volume context on a workspace with room for the second copies of ft and h2 runs steps 4-6 as one pass
+    const bool fused = p->z_open == 0 && d.slice4 < (int64_t)1 << 31 && p->workspace_dev && p->workspace_bytes >= carve(d, true).total;
+    const Carve cv = carve(d, fused);
     if (!p->workspace_dev || p->workspace_bytes < cv.total) return CP4D_EWORKSPACE;
     if ((uintptr_t)p->workspace_dev & (ALIGN - 1)) return CP4D_EINVAL;
     int ndev = 0;
@@ -185,7 +205,7 @@ int cp4d_create(const cp4d_params *p, cp4d_ctx **out) {
         int cur = -1;
         if (cudaGetDevice(&cur) != cudaSuccess || cur != p->device) { cudaGetLastError(); return CP4D_ECUDA; }
     }
-    if (forward_init() != cudaSuccess || backproject_mma_init() != cudaSuccess || backproject22_init() != cudaSuccess) { cudaGetLastError(); return CP4D_ECUDA; }
+    if (forward_init() != cudaSuccess || backproject_mma_init() != cudaSuccess || backproject22_init() != cudaSuccess || fused_step_init() != cudaSuccess) { cudaGetLastError(); return CP4D_ECUDA; }
 
     cp4d_ctx *ctx = new (std::nothrow) cp4d_ctx();
     if (!ctx) return CP4D_ENOMEM;
@@ -198,6 +218,8 @@ int cp4d_create(const cp4d_params *p, cp4d_ctx **out) {
     ctx->f = (float *)(w + cv.f); ctx->ft = (float *)(w + cv.ft); ctx->bp = (float *)(w + cv.bp);
     ctx->h2 = (float *)(w + cv.h2); ctx->h1 = (float *)(w + cv.h1); ctx->g = (float *)(w + cv.g);
     ctx->tmp_s = (float *)(w + cv.tmp_s);
+    ctx->fused = fused; ctx->flip = 0;
+    ctx->ft_alt = fused ? (float *)(w + cv.ft_alt) : nullptr; ctx->h2_alt = fused ? (float *)(w + cv.h2_alt) : nullptr;
     ctx->fwang = (FwAngle *)(w + cv.fwang); ctx->fworder = (int32_t *)(w + cv.fworder);
     ctx->fw_groups = (int4 *)(w + cv.fwpairs); ctx->fw_mode = CP4D_PROJ_AUTO;
     ctx->fw_items = forward_mma_item_bytes(d) ? (unsigned *)(w + cv.fwitems) : nullptr; ctx->fw_counts = (int2 *)(w + cv.fwcounts);
@@ -464,6 +486,13 @@ int cp4d_reset(cp4d_ctx *ctx, const float *f0) {
 static int iterate_once(cp4d_ctx *ctx) {
     // step 3: h1 <- prox_{sigma F1*}(h1 + sigma K1 ft)
     if (int r = forward_into(ctx, ctx->ft, 1, ctx->sigma, ctx->g, ctx->h1)) return r;
+    if (ctx->fused) {
+        // steps 4-6 in one pass over the volume, into the second copies of h2 and ft, which then take over
+        if (int r = adjoint_into(ctx, ctx->h1, ctx->bp)) return r;
+        CK(launch_prox_update(ctx, ctx->sigma, ctx->tau, ctx->ft, ctx->h2, ctx->h2_alt, ctx->bp, ctx->f, ctx->ft_alt), "prox_update");
+        std::swap(ctx->ft, ctx->ft_alt); std::swap(ctx->h2, ctx->h2_alt); ctx->flip ^= 1;
+        return CP4D_OK;
+    }
     // step 4: h2 <- prox_{sigma F2*}(h2 + sigma K2 ft)
     CK(launch_prox_f2(ctx, ctx->sigma, ctx->ft, ctx->h2), "prox_f2");
     // steps 5-6: f <- f - tau K1^T h1 + tau div h2 ; ft <- f+ + theta (f+ - f)
@@ -488,7 +517,8 @@ static bool capture_iteration(cp4d_ctx *ctx) {
         ctx->iter_graph_off = true;
         return false;
     }
-    const int r = iterate_once(ctx);
+    int r = iterate_once(ctx);
+    if (ctx->fused && r == CP4D_OK) r = iterate_once(ctx);      // two iterations: the double-buffered arrays are back in their roles
     cudaGraph_t g = nullptr;
     const cudaError_t e = cudaStreamEndCapture(ctx->stream, &g);
     ctx->iter_graph_launches = ctx->launches - l0;
@@ -517,14 +547,23 @@ int cp4d_iterate(cp4d_ctx *ctx, int32_t n_iters) {
     if (n_iters < 0) return fail(ctx, CP4D_EINVAL, "iterate: n_iters < 0");
     if (!ctx->have_steps || !ctx->have_data) return fail(ctx, CP4D_ESTATE, "iterate: set_data and set_steps first");
     // the per-kernel timing of cp4d_profile_begin records events between the launches, so it takes the eager path
-    const bool graph = !ctx->prof_on && n_iters >= 2 && (ctx->iter_graph || capture_iteration(ctx));
-    for (int it = 0; it < n_iters; ++it) {
-        if (graph) {
+    int it = 0;
+    const int per = ctx->fused ? 2 : 1;                      // iterations per replay
+    bool graph = !ctx->prof_on && n_iters >= 2;
+    if (graph && ctx->fused && ctx->flip) {                  // the graph holds the launches of flip == 0
+        if (int r = iterate_once(ctx)) return r;
+        ++it;
+    }
+    graph = graph && n_iters - it >= per && (ctx->iter_graph || capture_iteration(ctx));
+    while (it < n_iters) {
+        if (graph && n_iters - it >= per) {
             CK(cudaGraphLaunch(ctx->iter_graph, ctx->stream), "iterate (graph)");
             ctx->launches += ctx->iter_graph_launches;
             ctx->graph_replays++;
-        } else if (int r = iterate_once(ctx)) {
-            return r;
+            it += per;
+        } else {
+            if (int r = iterate_once(ctx)) return r;
+            ++it;
         }
     }
     return CP4D_OK;
@@ -708,7 +747,7 @@ int cp4d_profile_end(cp4d_ctx *ctx, cp4d_profile *out) {
 }
 
 const char *cp4d_kernel_name(int k) {
-    static const char *names[CP4D_K_COUNT] = {"forward", "synth", "fold", "backproject", "grad", "div", "prox_f2", "update", "reduce", "misc", "mix"};
+    static const char *names[CP4D_K_COUNT] = {"forward", "synth", "fold", "backproject", "grad", "div", "prox_f2", "update", "reduce", "misc", "mix", "prox_update"};
     return (k >= 0 && k < CP4D_K_COUNT) ? names[k] : "?";
 }
 

@@ -63,6 +63,11 @@ struct cp4d_ctx {
     cudaStream_t stream;
     // workspace carve-up (device pointers)
     float *f, *ft, *bp, *h2, *h1, *g, *tmp_s;
+    // one-pass step (fused_step.cu): the second copies of ft and h2; cp4d_iterate swaps (ft, ft_alt) and (h2, h2_alt) after every
+    // iteration, flip = iterations since the copies were in the roles they had at create, mod 2
+    bool fused;
+    float *ft_alt, *h2_alt;
+    int flip;
     float *cf, *cb, *psi;      // frame mode: coefficient stacks (analysis output, backprojection output), Psi[j][q] = phi_j(t_q)
     float4 *scratch;           // folded sinogram gt of the adjoint: [z][i][jc][gpl + b] float4, pitch gp; the pads stay ZERO (nothing
                                // else may write here), so every tile window of the backprojector is readable and reads 0 off the detector
@@ -155,6 +160,10 @@ int backproject_mma_nb16(const Dims &d);
 int64_t backproject_mma_scratch_units(const Dims &d);
 cudaError_t backproject_mma_init();
 cudaError_t backproject22_init();
+cudaError_t fused_step_init();
+// steps 4-6 of Fig. 2 in one pass: reads ft, h2, bp, f; writes h2_new, ft_new (second copies) and f in place
+cudaError_t launch_prox_update(cp4d_ctx *c, float sigma, float tau, const float *ft, const float *h2, float *h2_new,
+                               const float *bp, float *f, float *ft_new);
 cudaError_t launch_fold_split(cp4d_ctx *c, const float *g, float4 *gt);
 cudaError_t launch_backproject_mma(cp4d_ctx *c, const float4 *gt, float *f_out);
 cudaError_t launch_backproject(cp4d_ctx *c, const float4 *gt, float *f_out, int Q_override = 0);
