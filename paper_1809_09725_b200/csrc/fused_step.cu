@@ -38,7 +38,7 @@ enum : unsigned { FL_LIVE = 1, FL_OWN = 2, FL_XP = 4, FL_YP = 8, FL_TP = 16, FL_
 __device__ __forceinline__ float4 ldg4(const float4 *p) { return __ldg(p); }
 __device__ __forceinline__ float4 diff4(float4 a, float4 b) { return make_float4(a.x - b.x, a.y - b.y, a.z - b.z, a.w - b.w); }
 
-__global__ void __launch_bounds__(FU_THREADS) k_prox_update(const float4 *__restrict__ ft, const float4 *__restrict__ h2,
+__global__ void __launch_bounds__(FU_THREADS, 4) k_prox_update(const float4 *__restrict__ ft, const float4 *__restrict__ h2,
                                                             float4 *__restrict__ h2n, const float4 *__restrict__ bp,
                                                             float4 *f, float4 *__restrict__ ftn, FusedArgs a) {
     extern __shared__ float4 fu_sm[];
