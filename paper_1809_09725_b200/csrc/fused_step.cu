@@ -23,7 +23,7 @@ namespace {
 
 constexpr int FU_TX = 16;            // tile width in voxels; the height ty follows from Q (launcher)
 constexpr int FU_THREADS = 256;
-constexpr int FU_KMAX = 3;           // elements per thread: (FU_TX + 1) * (ty + 1) * Q <= FU_KMAX * FU_THREADS
+constexpr int FU_KMAX = 2;           // elements per thread: (FU_TX + 1) * (ty + 1) * Q <= FU_KMAX * FU_THREADS
 constexpr int FU_SMEM_MAX = 5 * FU_KMAX * FU_THREADS * 16;
 
 struct FusedArgs {
@@ -68,7 +68,7 @@ __global__ void __launch_bounds__(FU_THREADS, 4) k_prox_update(const float4 *__r
             if (c > 0) fl |= FL_TM;
         }
         flag[k] = fl;
-        goff[k] = (y * a.n + x) * a.Q + c;
+        goff[k] = fl ? (y * a.n + x) * a.Q + c : 0;      // (a dead element loads from offset 0 and stores nothing)
     }
     const float4 zero = make_float4(0.f, 0.f, 0.f, 0.f);
 
@@ -80,14 +80,16 @@ __global__ void __launch_bounds__(FU_THREADS, 4) k_prox_update(const float4 *__r
 #pragma unroll
         for (int k = 0; k < FU_KMAX; ++k) {
             const unsigned fl = flag[k];
-            if (!(fl & FL_LIVE) || (pre && !(fl & FL_OWN))) continue;
+            // no branches around the loads, so that those of all my elements are in flight together: a missing neighbour
+            // is the element itself (difference 0), a dead element computes on offset 0 and stores nothing
+            const bool act = (fl & FL_LIVE) && !(pre && !(fl & FL_OWN));
             const int e = threadIdx.x + k * FU_THREADS;
             const int64_t idx = (int64_t)z * a.slice4 + goff[k];
             const float4 cur = ldg4(ft + idx);
-            const float4 fz = (z + 1 < a.nz) ? ldg4(ft + idx + a.slice4) : cur;
-            const float4 fx = (fl & FL_XP) ? ldg4(ft + idx + a.Q) : cur;
-            const float4 fy = (fl & FL_YP) ? ldg4(ft + idx + sy) : cur;
-            const float ftp = (fl & FL_TP) ? __ldg(reinterpret_cast<const float *>(ft) + (idx + 1) * 4) : cur.w;
+            const float4 fz = ldg4(ft + idx + ((z + 1 < a.nz) ? a.slice4 : 0));
+            const float4 fx = ldg4(ft + idx + ((fl & FL_XP) ? a.Q : 0));
+            const float4 fy = ldg4(ft + idx + ((fl & FL_YP) ? sy : 0));
+            const float ftp = __ldg(reinterpret_cast<const float *>(ft) + idx * 4 + ((fl & FL_TP) ? 4 : 3));
             const float4 qx = ldg4(h2 + idx), qy = ldg4(h2 + idx + a.V4), qz = ldg4(h2 + idx + 2 * a.V4), qt = ldg4(h2 + idx + 3 * a.V4);
             float4 gx = diff4(fx, cur), gy = diff4(fy, cur), gz = diff4(fz, cur);
             float4 gt = make_float4(a.lambda2 * (cur.y - cur.x), a.lambda2 * (cur.z - cur.y), a.lambda2 * (cur.w - cur.z),
@@ -102,8 +104,8 @@ __global__ void __launch_bounds__(FU_THREADS, 4) k_prox_update(const float4 *__r
     }
             CP4D_FU_PROX(x) CP4D_FU_PROX(y) CP4D_FU_PROX(z) CP4D_FU_PROX(w)
 #undef CP4D_FU_PROX
-            hz_cur[e] = gz;
-            if (!pre) {
+            if (act) hz_cur[e] = gz;
+            if (act && !pre) {
                 s_hx[e] = gx; s_hy[e] = gy; s_ht[e] = gt;
                 if (fl & FL_OWN) {
                     h2n[idx] = gx; h2n[idx + a.V4] = gy; h2n[idx + 2 * a.V4] = gz; h2n[idx + 3 * a.V4] = gt;
