@@ -103,6 +103,7 @@ def algorithmic_work(c, n_frames=0):
         "div": ("hbm", 4.0 * 5 * V),
         "prox_f2": ("hbm", 4.0 * 9 * V),                 # read ft + h2[4], write h2[4]
         "update": ("hbm", 4.0 * 8 * V),                  # read h2[4] + f + K1^T h1, write f + ft
+        "prox_update": ("hbm", 4.0 * 13 * V),            # the two in one pass: read ft + h2[4] + f + K1^T h1, write h2[4] + f + ft
         "mix": ("hbm", 4.0 * (V + Vc)),                  # frame mode: read frames / write coefficients or the reverse
     }
 
@@ -272,7 +273,8 @@ def run_cp4d(args, c, rank, world):
 
     # ---- problem, data, step sizes (outside the timed region: SURVEY 8(d)) ----
     phi = synth.basis_table(c.basis, c.m, c.n_angles)
-    ctx = binding.Context.from_config(c, phi=phi, device=local, n_frames=args.frames)
+    # --step one-pass: the workspace holds second copies of h2 and ft, and cp4d_iterate runs steps 4-6 as one kernel
+    ctx = binding.Context.from_config(c, phi=phi, device=local, n_frames=args.frames, fused=args.step == "one-pass")
     ctx.set_projector_mode(args.projectors)
     g = synth.sinogram(c, device=str(dev)).to(torch.float32).contiguous()
     L = ctx.norm(args.power_iters, seed=3)
@@ -369,7 +371,7 @@ def run_cp4d(args, c, rank, world):
                "seconds": dt}
         del g_host, f_host
     return ctx, dict(ms=ms, launches=launches, prof=prof, prof_gd=prof_gd, ops=ops, e2e=e2e, clocks=clocks, peaks=peaks,
-                     fp32_alt=fp32_alt, proj=ctx.projector_mode_in_use(),
+                     fp32_alt=fp32_alt, proj=ctx.projector_mode_in_use(), step="one-pass" if ctx.fused_step_in_use() else "two-kernel",
                      L=L, launches_total=ctx.launch_count() - launches0, graph_replays=graph_replays)
 
 
@@ -477,6 +479,7 @@ def assemble(args, c, world, r):
         "dtype": "f32", "data": "synthetic",
         "config": workload_config(c, args.frames),
         "run": {"norm_K": r["L"], "projectors": {"mode": args.projectors, "forward": r["proj"][0], "adjoint": r["proj"][1]},
+                "step": r["step"],
                 "arithmetic": ("fp32 storage, fp32 accumulation everywhere; 'tensor' projector = products of split-bf16 pairs "
                                "(x = hi + lo, three products per term on the 2:4 sparse mma.sp, rel. error 5e-6 per ray sum or voxel, tolerance 1e-4), "
                                "'fp32' projector = plain FMAs (2e-6)"), "parallelism": "replicas only (independent problems, no collective)" if world > 1 else "1 gpu",
@@ -523,8 +526,11 @@ def main():
     ap.add_argument("--stream-block", type=int, default=1, metavar="K",
                     help="with --streamed: temporal blocking, K iterations per residency of a window of SLAB_NZ + 2K slices")
     ap.add_argument("--projectors", default="auto", choices=["auto", "fp32", "tensor"],
-                    help="cp4d_set_projector_mode: auto = tensor-core forward projector + fp32 backprojector (default), fp32 = CUDA-core "
-                         "kernels on both sides, tensor = tensor-core kernels on both sides")
+                    help="cp4d_set_projector_mode: auto = the tensor-core pair where the problem fills the GPU, else the fp32 kernels "
+                         "(default); fp32 = CUDA-core kernels on both sides; tensor = tensor-core kernels on both sides")
+    ap.add_argument("--step", default="one-pass", choices=["one-pass", "two-kernel"],
+                    help="one-pass (default): workspace of cp4d_workspace_bytes_fused, steps 4-6 of Fig. 2 in one kernel (13 V floats of "
+                         "HBM traffic); two-kernel: the smaller workspace, prox and update as two kernels (17 V)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()

@@ -56,8 +56,11 @@ def test_workspace_bytes_counts_state(L):
         scratch += tiles * 4 * 14 * (c.n_theta0 // gs + 8) * 48
         scratch += tiles * 2 * (c.n_theta0 + 8) * 32           # angle records of the tensor backprojector per (half tile, angle)
         assert state + scratch <= nb <= state + scratch + (64 << 20)
+        # the one-pass step of cp4d_iterate double-buffers h2[4] and ft: 5 V floats more
+        nbf = binding.workspace_bytes(c.n, c.nz, c.nd, c.n_angles, c.n_half_rot, c.m, fused=True)
+        assert 5 * c.V * 4 <= nbf - nb <= 5 * c.V * 4 + 512
     c = synth.CONFIGS[5]
-    assert binding.workspace_bytes(c.n, c.nz, c.nd, c.n_angles, c.n_half_rot, c.m) < 170e9   # fits 180 GB HBM
+    assert binding.workspace_bytes(c.n, c.nz, c.nd, c.n_angles, c.n_half_rot, c.m, fused=True) < 170e9   # fits 180 GB HBM
 
 
 @pytest.mark.parametrize("bad", [dict(ny=31), dict(m=6), dict(m=36), dict(n_half_rot=3), dict(nd=1), dict(nz=0), dict(lambda1=-1.0),

@@ -62,7 +62,7 @@ def test_json_line_contract_offline():
     r = dict(ms=600.0, launches=350, prof=prof, prof_gd={"grad": (1.38, 3), "div": (1.2, 3)}, ops={"forward_op": 6.7, "adjoint_op": 3.85},
              e2e={"value": 81.0, "unit": bench.UNIT, "h2d_bytes_per_step": 1.0, "d2h_bytes_per_step": 2.0},
              clocks={"sm_mhz": 1965.0, "sm_max_mhz": 1965.0, "reasons": []}, peaks=bench.load_peaks(), L=1.0, launches_total=1,
-             graph_replays=55, fp32_alt=None, proj=("tensor", "tensor"))
+             graph_replays=55, fp32_alt=None, proj=("tensor", "tensor"), step="two-kernel")
     line = bench.assemble(A, c, 1, r)
     for k in ("metric", "value", "unit", "n_gpus", "steps", "warmup", "ms_per_step", "higher_is_better", "scaling", "vs_baseline",
               "dtype", "data", "config", "roofline", "e2e", "clocks", "gpu_launches"):
