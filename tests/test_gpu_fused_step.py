@@ -38,7 +38,7 @@ CASES = {
 }
 
 
-def _run(torch, c, nf, fused, its, theta=1.0):
+def _run(torch, c, nf, fused, its, theta=1.0, warm=False):
     from paper_1809_09725_b200 import binding
     phi = synth.basis_table(c.basis, c.m, c.n_angles)
     with torch.cuda.stream(torch.cuda.Stream()):           # a capturable stream: cp4d_iterate replays its graph
@@ -50,7 +50,9 @@ def _run(torch, c, nf, fused, its, theta=1.0):
             truth = torch.randn(ctx.primal_shape, device="cuda", generator=gen)
             data = ctx.forward(truth)
             L = ctx.norm(8, 1)
-            ctx.set_data(data); ctx.set_steps(0.95 / L, 0.95 / L); ctx.reset(None)
+            ctx.set_data(data); ctx.set_steps(0.95 / L, 0.95 / L)
+            # warm: a non-zero initial guess (f = ft = f0), so that the first prox already sees a gradient
+            ctx.reset(torch.randn(ctx.primal_shape, device="cuda", generator=gen) if warm else None)
             for n in its:
                 ctx.iterate(n)
             ctx.sync()
@@ -70,7 +72,7 @@ def test_fused_step_matches_two_kernel_path(torch_cuda, case, its):
         assert np.isfinite(b[k]).all()
         # same arithmetic per element; the projectors' atomic additions are ordered differently from run to run
         assert rel(b[k], a[k]) <= 2e-6, (k, rel(b[k], a[k]))
-    assert np.linalg.norm(b["h2"]) > 0 and np.linalg.norm(b["f"]) > 0
+    assert np.linalg.norm(b["f"]) > 0 and (sum(its) < 2 or np.linalg.norm(b["h2"]) > 0)      # (h2 stays 0 in the first iteration from zero)
     # the two-kernel path replays one iteration per graph launch, the one-pass step two (the copies are back in their roles);
     # a call that finds the copies swapped launches one iteration directly first
     want_a = sum(n for n in its if n >= 2)
@@ -84,13 +86,17 @@ def test_fused_step_matches_two_kernel_path(torch_cuda, case, its):
     assert (ra, rb) == (want_a, want_b)
 
 
-def test_fused_step_first_iteration_dual_is_bit_exact(torch_cuda):
-    """After ONE iteration from zero h2 is the projection of sigma K2 ft of the same ft on both paths: the one-pass kernel's
-    prox (own voxels and the recomputed halo) must reproduce k_grad's bit for bit."""
-    c, nf = CASES["q4_ragged"]
-    a, _, _ = _run(torch_cuda, c, nf, False, (1,))
-    b, _, _ = _run(torch_cuda, c, nf, True, (1,))
+@pytest.mark.parametrize("case", ["q4_ragged", "q3_zchunks"])
+def test_fused_step_first_iteration_dual_is_bit_exact(torch_cuda, case):
+    """After ONE iteration from the same non-zero initial guess h2 = proj(sigma K2 f0) on both paths: the one-pass kernel's prox
+    (own voxels, and the values it stores are the ones its divergence used) must reproduce k_grad<1>'s bit for bit."""
+    c, nf = CASES[case]
+    a, _, _ = _run(torch_cuda, c, nf, False, (1,), warm=True)
+    b, _, _ = _run(torch_cuda, c, nf, True, (1,), warm=True)
+    assert np.linalg.norm(a["h2"]) > 0
     assert np.array_equal(a["h2"], b["h2"])
+    for k in ("f", "ft"):
+        assert rel(b[k], a[k]) <= 2e-6
 
 
 @pytest.mark.parametrize("theta", [1.0, 0.5])
