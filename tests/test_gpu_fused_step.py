@@ -26,6 +26,13 @@ def torch_cuda():
     return torch
 
 
+@pytest.fixture(scope="module")
+def fast_oracle(oracle):
+    oracle.set_threads(oracle.max_threads())
+    yield oracle
+    oracle.set_threads(1)
+
+
 CASES = {
     # Q = 4, tiles of 16 x 4 voxels: 75 = 4 * 16 + 11 and 18 * 4 + 3 (ragged in x and y)
     "q4_ragged": (synth.CONFIGS[3].scaled(cfg=41, n=75, nd=90, nz=5, n_angles=60, n_half_rot=2, m=16, n_objects=3), 0),
