@@ -19,7 +19,8 @@ numbered 1..5 as in SURVEY.md 8).  Inputs are seeded and synthetic (paper_1809_0
              sample (a few full in-plane slices), extrapolated to the whole problem.
 
 The default workload is config 5 (2048^2 x 32, 3600 angles, m = 16: the largest single-GPU configuration of BASELINE.json,
-65 GB of workspace); `--config 3` is the quick one.
+110 GB of workspace with the one-pass step of `--step one-pass`, the default; 67 GB with `--step two-kernel`); `--config 3` is
+the quick one.
 
 N > 1: the path does not shard (north_star: one GPU); `--gpus N` runs N independent replicas, one per rank,
 no data-path collective ("replicas only"): the value is REPLICA throughput.  Started without a
