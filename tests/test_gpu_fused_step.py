@@ -34,7 +34,7 @@ def fast_oracle(oracle):
 
 
 CASES = {
-    # Q = 4, tiles of 16 x 4 voxels: 75 = 4 * 16 + 11 and 18 * 4 + 3 (ragged in x and y)
+    # Q = 4, tiles of 16 x 6 voxels: 75 = 4 * 16 + 11 = 12 * 6 + 3 (ragged in x and y)
     "q4_ragged": (synth.CONFIGS[3].scaled(cfg=41, n=75, nd=90, nz=5, n_angles=60, n_half_rot=2, m=16, n_objects=3), 0),
     "q1": (synth.CONFIGS[2].scaled(cfg=42, n=50, nd=61, nz=3, n_angles=48, n_half_rot=2, m=4), 0),
     # few tiles: the launcher splits z into chunks, each of which recomputes the prox of the slice below it
