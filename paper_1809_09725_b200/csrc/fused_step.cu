@@ -23,11 +23,12 @@ namespace {
 
 constexpr int FU_TX = 16;            // tile width in voxels; the height ty follows from Q (launcher)
 constexpr int FU_THREADS = 256;
+constexpr int FU_BAND = 8;            // tile rows per band of the launch order
 constexpr int FU_KMAX = 2;           // elements per thread: (FU_TX + 1) * (ty + 1) * Q <= FU_KMAX * FU_THREADS
 constexpr int FU_SMEM_MAX = 5 * FU_KMAX * FU_THREADS * 16;
 
 struct FusedArgs {
-    int n, nz, Q, zper, ty, tiles_x, l1_zero;
+    int n, nz, Q, zper, ty, tiles_x, tiles_y, l1_zero;
     int slice4;                      // float4 per slice (< 2^31: validate() bounds n * n * Q)
     int64_t V4;
     float lambda2, sigma, inv_l1, tau, theta;
@@ -44,7 +45,11 @@ __global__ void __launch_bounds__(FU_THREADS, 4) k_prox_update(const float4 *__r
     extern __shared__ float4 fu_sm[];
     const int W = (FU_TX + 1) * a.Q, items = W * (a.ty + 1);
     float4 *s_hx = fu_sm, *s_hy = fu_sm + items, *s_ht = fu_sm + 2 * items, *s_hz = fu_sm + 3 * items;      // s_hz: two slices
-    const int x0 = (blockIdx.x % a.tiles_x) * FU_TX, y0 = (blockIdx.x / a.tiles_x) * a.ty;
+    // tiles in bands of FU_BAND tile rows, inside a band column by column: CTAs next to each other in launch order share a halo
+    // row and walk z in step, so the halo reads of one are the other's own reads of a moment ago (L2 hits at any N)
+    const int per_band = a.tiles_x * FU_BAND, band = blockIdx.x / per_band, rb = blockIdx.x - band * per_band;
+    const int rows = min(FU_BAND, a.tiles_y - band * FU_BAND);
+    const int x0 = (rb / rows) * FU_TX, y0 = (band * FU_BAND + rb % rows) * a.ty;
     const int z0 = blockIdx.y * a.zper, z1 = min(a.nz, z0 + a.zper);
     const int sy = a.n * a.Q;
 
@@ -170,7 +175,8 @@ cudaError_t launch_prox_update(cp4d_ctx *c, float sigma, float tau, const float 
     const int items = (FU_TX + 1) * (a.ty + 1) * a.Q;
     if (items > FU_KMAX * FU_THREADS) return cudaErrorInvalidConfiguration;
     a.tiles_x = (d.n + FU_TX - 1) / FU_TX;
-    const int64_t tiles = (int64_t)a.tiles_x * ((d.n + a.ty - 1) / a.ty);
+    a.tiles_y = (d.n + a.ty - 1) / a.ty;
+    const int64_t tiles = (int64_t)a.tiles_x * a.tiles_y;
     // enough CTAs to fill the GPU a few times over; otherwise split z (each chunk recomputes the prox of one slice below it)
     int zchunks = 1;
     while (tiles * zchunks < 148 * 8 && zchunks * 4 <= d.nz) zchunks *= 2;
