@@ -109,7 +109,10 @@ def workspace_bytes(n, nz, nd, n_angles, n_half_rot, m, n_frames=0, fused=False)
 
 
 class Context:
-    """One reconstruction problem on one GPU.  Tensors are torch CUDA float32, contiguous, layouts of cp4d.h."""
+    """One reconstruction problem on one GPU.  Tensors are torch CUDA float32, contiguous, layouts of cp4d.h.
+    fused=True allocates the workspace of cp4d_workspace_bytes_fused (5 V floats more), on which cp4d_iterate runs steps 4-6 of
+    Fig. 2 as one kernel (13 V instead of 17 V floats of HBM traffic per iteration; same iterates); state() then returns the
+    CURRENT copies of ft and h2, valid until the next iterate()."""
 
     def __init__(self, n, nz, nd, n_angles, n_half_rot, m, phi, lambda1=1e-3, lambda2=1.0, theta=1.0, device=0, n_frames=0,
                  z_open=0, fused=False):
