@@ -117,14 +117,17 @@ def _valid(c, o0, size):
     return (0 if o0 == 0 else 1), (size if o0 + size == c.n else size - 1)
 
 
-@pytest.mark.parametrize("cfg", [3, 4, 5])
-def test_teacher_forced_cp_step(torch_cuda, fast_oracle, cfg):
+@pytest.mark.parametrize("cfg,fused", [(3, False), (4, False), (5, False), (3, True), (5, True)])
+def test_teacher_forced_cp_step(torch_cuda, fast_oracle, cfg, fused):
+    """One iteration of Fig. 2 from a random state at full size, checked step by step on sampled rays and windows.  fused: the
+    context bench.py times (workspace of cp4d_workspace_bytes_fused: steps 4-6 as the one-pass kernel)."""
     torch = torch_cuda
     from paper_1809_09725_b200 import binding
     c = synth.CONFIGS[cfg]
     lam1, lam2, sigma, tau = 1.8, 0.8, 0.05, 0.03          # lam1 ~ median |h2 + sigma grad ft|: both prox branches occur
     phi = synth.basis_table(c.basis, c.m, c.n_angles)
-    ctx = binding.Context.from_config(c, phi=phi, lambda1=lam1, lambda2=lam2)
+    ctx = binding.Context.from_config(c, phi=phi, lambda1=lam1, lambda2=lam2, fused=fused)
+    assert ctx.fused_step_in_use() == fused
     gen = torch.Generator(device="cuda").manual_seed(2000 + cfg)
     st = ctx.state()
     for name in ("f", "ft", "h1", "h2", "g"):
@@ -151,6 +154,7 @@ def test_teacher_forced_cp_step(torch_cuda, fast_oracle, cfg):
     ctx.set_steps(tau, sigma)
     ctx.iterate(1)
     ctx.sync()
+    st = ctx.state()                                       # (the one-pass step wrote ft and h2 to their second copies)
     # ---- step 3 at the sampled rays
     P3 = _sub_problem(fast_oracle, c, phi, len(zs))
     kf = P3.forward_rays(ft3, np.stack([zi, kk, bb], 1).astype(np.int32))
