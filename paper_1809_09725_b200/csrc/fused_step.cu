@@ -117,6 +117,15 @@ __global__ void __launch_bounds__(FU_THREADS, 4) k_prox_update(const float4 *__r
                 }
             }
         }
+        // f and K1^T h1 of my own voxels: on their way while the CTA meets at the barrier
+        float4 fo_k[FU_KMAX], b_k[FU_KMAX];
+#pragma unroll
+        for (int k = 0; k < FU_KMAX; ++k) {
+            // (elements I do not own read offset 0 of the slice and use nothing of it)
+            const int64_t idx = (int64_t)z * a.slice4 + ((flag[k] & FL_OWN) ? goff[k] : 0);
+            fo_k[k] = f[idx];
+            b_k[k] = ldg4(bp + idx);
+        }
         __syncthreads();
         // ---- steps 5-6 on my own voxels ----
         if (!pre) {
@@ -140,8 +149,7 @@ __global__ void __launch_bounds__(FU_THREADS, 4) k_prox_update(const float4 *__r
                 d.y = (xc.y - xm.y) + (yc.y - ym.y) + (zc.y - prevz.y) + a.lambda2 * (tc.y - tc.x);
                 d.z = (xc.z - xm.z) + (yc.z - ym.z) + (zc.z - prevz.z) + a.lambda2 * (tc.z - tc.y);
                 d.w = (xc.w - xm.w) + (yc.w - ym.w) + (zc.w - prevz.w) + a.lambda2 * (tw - tc.z);
-                const float4 fo = f[idx];
-                const float4 b = ldg4(bp + idx);
+                const float4 fo = fo_k[k], b = b_k[k];
                 float4 fn, fr;
                 fn.x = fmaf(a.tau, d.x - b.x, fo.x); fn.y = fmaf(a.tau, d.y - b.y, fo.y);
                 fn.z = fmaf(a.tau, d.z - b.z, fo.z); fn.w = fmaf(a.tau, d.w - b.w, fo.w);
